@@ -1,0 +1,169 @@
+"""CPU oracle for the RKETD-FDTD hot path — TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+
+ctypes front-end of ``oracle/rketd_oracle.cpp`` (plain serial C++17, fp64; see
+the header of that file for what it states and which pins hold it).  Only
+``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package.  It imports nothing from
+``paper_1709_00821_b200`` (the CUDA path) and that package never imports this.
+
+Two builds of the one source: ``liboracle_rketd.so`` (serial) and
+``liboracle_rketd_omp.so`` (``-fopenmp``); ``run(..., omp=True)`` selects the
+latter.  Both are compiled with ``-O2 -ffp-contract=off`` so that the
+arithmetic is the plain expression of the source (no fused multiply-add).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "rketd_oracle.cpp")
+_LIBS = {False: os.path.join(_HERE, "liboracle_rketd.so"), True: os.path.join(_HERE, "liboracle_rketd_omp.so")}
+_loaded = {}
+
+BOUNDARY_MUR = 0
+BOUNDARY_PEC = 1
+SRC_NONE = -1
+SRC_GAUSS_DERIV = 0
+SRC_TABLE = 1
+
+
+def build(force: bool = False) -> None:
+    """Compile both builds of the oracle with g++ (a few seconds)."""
+    for omp, out in _LIBS.items():
+        if not force and os.path.exists(out) and os.path.getmtime(out) >= os.path.getmtime(_SRC):
+            continue
+        cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fPIC", "-shared", _SRC, "-o", out + ".tmp"]
+        if omp:
+            cmd.insert(1, "-fopenmp")
+        subprocess.run(cmd, check=True)
+        os.replace(out + ".tmp", out)
+
+
+_D = ctypes.POINTER(ctypes.c_double)
+_I64 = ctypes.POINTER(ctypes.c_int64)
+
+
+def _lib(omp: bool = False) -> ctypes.CDLL:
+    if omp not in _loaded:
+        build()
+        lib = ctypes.CDLL(_LIBS[omp])
+        lib.oracle_constants.argtypes = [_D, _D, _D]
+        lib.oracle_constants.restype = None
+        lib.oracle_phi.argtypes = [ctypes.c_double, _D, _D]
+        lib.oracle_phi.restype = None
+        lib.oracle_coefficients.argtypes = [ctypes.c_int64, _D, _D, ctypes.c_double, ctypes.c_double] + [_D] * 8
+        lib.oracle_coefficients.restype = ctypes.c_int
+        lib.oracle_source.argtypes = [ctypes.c_int, _D, ctypes.c_int64, ctypes.c_int64, ctypes.c_double]
+        lib.oracle_source.restype = ctypes.c_double
+        lib.oracle_run.argtypes = [ctypes.c_int64, ctypes.c_int64, ctypes.c_double, ctypes.c_double,
+                                   _D, _D, _D, _D, _D,
+                                   ctypes.c_int, _D, ctypes.c_int64, ctypes.c_int64,
+                                   _I64, ctypes.c_int, ctypes.c_int64, ctypes.c_int64,
+                                   _D, _D, _D, ctypes.c_int, _D, _D, ctypes.c_int]
+        lib.oracle_run.restype = ctypes.c_int
+        _loaded[omp] = lib
+    return _loaded[omp]
+
+
+def _p(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data_as(_D)
+
+
+def constants():
+    """(c0, mu0, eps0) as hard-coded in the oracle."""
+    c0, mu0, eps0 = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+    _lib().oracle_constants(ctypes.byref(c0), ctypes.byref(mu0), ctypes.byref(eps0))
+    return c0.value, mu0.value, eps0.value
+
+
+def phi(x: float):
+    p1, p2 = ctypes.c_double(), ctypes.c_double()
+    _lib().oracle_phi(float(x), ctypes.byref(p1), ctypes.byref(p2))
+    return p1.value, p2.value
+
+
+def coefficients(wp: np.ndarray, nu: np.ndarray, dz: float, dt: float):
+    """S0: returns dict(ca, cj, ch, ka, kb, kc [same shape as wp], chh, m)."""
+    wp = np.ascontiguousarray(wp, np.float64)
+    nu = np.ascontiguousarray(nu, np.float64)
+    out = {k: np.empty_like(wp) for k in ("ca", "cj", "ch", "ka", "kb", "kc")}
+    chh, m = ctypes.c_double(), ctypes.c_double()
+    rc = _lib().oracle_coefficients(wp.size, _p(wp), _p(nu), dz, dt, *[_p(out[k]) for k in
+                                    ("ca", "cj", "ch", "ka", "kb", "kc")], ctypes.byref(chh), ctypes.byref(m))
+    if rc:
+        raise ValueError("oracle_coefficients: invalid argument")
+    out["chh"], out["m"] = chh.value, m.value
+    return out
+
+
+def source(kind: int, params: Sequence[float], step_index: int, dt: float) -> float:
+    prm = np.ascontiguousarray(params, np.float64)
+    return _lib().oracle_source(kind, _p(prm), prm.size, step_index, dt)
+
+
+class State:
+    """E, H, J [nbatch][ncells] fp64 plus the global step counter; advanced in place by run()."""
+
+    def __init__(self, ncells: int, nbatch: int = 1, E0=None, H0=None, J0=None):
+        shp = (nbatch, ncells)
+        self.E = np.zeros(shp) if E0 is None else np.array(E0, np.float64).reshape(shp).copy()
+        self.H = np.zeros(shp) if H0 is None else np.array(H0, np.float64).reshape(shp).copy()
+        self.J = np.zeros(shp) if J0 is None else np.array(J0, np.float64).reshape(shp).copy()
+        self.step = 0
+
+
+def run(state: State, wp, nu, dz: float, dt: float, nsteps: int, *, src_kind: int = SRC_NONE,
+        src_params: Sequence[float] = (), src_cell: int = 0, probes: Sequence[int] = (),
+        freqs=None, dft=None, record_J: bool = False, boundary: int = BOUNDARY_MUR, omp: bool = False):
+    """Advance ``state`` by nsteps.  Returns (rec, recJ) with rec[nbatch][nprobes][nsteps]
+    (recJ None unless record_J).  ``dft`` = (re, im) accumulator arrays [nbatch][nprobes][nfreq],
+    updated in place when ``freqs`` is given."""
+    nbatch, ncells = state.E.shape
+    wp = np.ascontiguousarray(wp, np.float64).reshape(nbatch, ncells)
+    nu = np.ascontiguousarray(nu, np.float64).reshape(nbatch, ncells)
+    prm = np.ascontiguousarray(src_params, np.float64)
+    prb = np.ascontiguousarray(probes, np.int64)
+    rec = np.zeros((nbatch, prb.size, nsteps))
+    recJ = np.zeros((nbatch, prb.size, nsteps)) if record_J else None
+    fr = None if freqs is None else np.ascontiguousarray(freqs, np.float64)
+    re = im = None
+    if fr is not None:
+        re, im = dft
+        assert re.shape == (nbatch, prb.size, fr.size) and re.flags.c_contiguous and im.flags.c_contiguous
+    rc = _lib(omp).oracle_run(ncells, nbatch, dz, dt, _p(wp), _p(nu), _p(state.E), _p(state.H), _p(state.J),
+                              src_kind, _p(prm) if prm.size else None, prm.size, src_cell,
+                              prb.ctypes.data_as(_I64) if prb.size else None, prb.size, state.step, nsteps,
+                              _p(rec), _p(recJ), _p(fr), 0 if fr is None else fr.size, _p(re), _p(im), boundary)
+    if rc:
+        raise ValueError("oracle_run: invalid argument")
+    state.step += nsteps
+    return rec, recJ
+
+
+def run_workload(w, nsteps: Optional[int] = None, b0: int = 0, b1: Optional[int] = None, omp: bool = False,
+                 cells: Optional[tuple] = None):
+    """Run a ``workloads.Workload`` (duck-typed: only its data attributes are used) on grids
+    b0..b1-1.  ``cells=(lo, hi)`` runs the window lo..hi-1 only, with Mur at the window ends
+    (pin P7: exact for probes at distance > nsteps from both window ends).
+    Returns dict(rec, dft_mag, state)."""
+    b1 = w.nbatch if b1 is None else b1
+    lo, hi = (0, w.ncells) if cells is None else cells
+    nsteps = w.nsteps if nsteps is None else nsteps
+    wp, nu = w.media(lo, hi, b0, b1)
+    E0 = w.initial_E(lo, hi, b0, b1)
+    st = State(hi - lo, b1 - b0, E0)
+    probes = [int(p) - lo for p in w.probes if lo <= p < hi]
+    in_src = lo <= w.src_cell < hi
+    dft = None
+    if w.dft_freqs is not None:
+        dft = (np.zeros((b1 - b0, len(probes), len(w.dft_freqs))), np.zeros((b1 - b0, len(probes), len(w.dft_freqs))))
+    rec, _ = run(st, wp, nu, w.dz, w.dt, nsteps, src_kind=w.src_kind if in_src else SRC_NONE,
+                 src_params=w.src_params, src_cell=w.src_cell - lo if in_src else 0, probes=probes,
+                 freqs=w.dft_freqs, dft=dft, omp=omp)
+    mag = None if dft is None else np.hypot(dft[0], dft[1])
+    return {"rec": rec, "dft_mag": mag, "state": st, "probe_cells": [p + lo for p in probes]}

@@ -1,0 +1,227 @@
+// ============================================================================
+// oracle/rketd_oracle.cpp  —  TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+//
+// Plain, serial, fp64 restatement of the 1-D RKETD-FDTD leapfrog of
+// arxiv 1709.00821 (§II, eqs. (11), (12), (14)), plus
+// the parts BASELINE.json's north_star adds around it (Mur-1 ABC, soft source,
+// probe records, probe DFT).  It follows SURVEY.md §8(c) S0-S6 step by step, in
+// that order, with no blocking, fusion or reordering, so that it can be checked
+// against the paper by eye.
+//
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl
+// reference legs may build, load or call this file.  It shares no code, header,
+// table or helper with paper_1709_00821_b200/ (the CUDA path) and neither
+// imports the other.  Build: g++ -O2 -ffp-contract=off [-fopenmp] -shared -fPIC.
+// The OpenMP build is the same source; it parallelises the k loops of a single
+// grid or the grid loop of a batch, has no reductions, and is therefore
+// bit-identical to the serial build (pin P9).
+//
+// Parity pins (tests/test_oracle_pins.py): P1 Courant-1 translation, P2 eq.(12)
+// residual with eq.(11) literal, P3 discrete energy, P4 RK4 brute force of
+// eq.(6), P5 analytic slab R/T, P6 stability, P7 domain of dependence, P8 DFT,
+// P9 OpenMP == serial, and the phi-functions against 50-digit arithmetic.
+// Nothing in this file is "parity unpinned".
+//
+// Notation: N E-nodes k = 0..N-1; E[k] = Ex(k dz) at integer steps;
+// H[k] = Hy((k+1/2) dz) at half steps, k = 0..N-2 (H[N-1] is padding, kept 0);
+// J[k] = Jx(k dz) collocated with E in space and time (eq. (11)/(12) use J^n,
+// J^{n+1}: PAPER.md:68, :74).  x = nu dt, a = exp(-x).
+// ============================================================================
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+
+namespace {
+
+// the paper gives no values; both sides hard-code SI values.
+const double kC0 = 299792458.0;                 // m/s
+const double kPi = 3.14159265358979323846;
+const double kMu0 = 4.0 * kPi * 1e-7;           // H/m
+const double kEps0 = 1.0 / (kMu0 * kC0 * kC0);  // F/m
+
+// phi1(x) = (1 - e^-x)/x,  phi2(x) = (e^-x - 1 + x)/x^2   (the two brackets of
+// eq. (11), divided by dt and by dt resp.).  The literal forms are
+// 0/0 at x = 0 and lose digits for small x, hence expm1 / a series.
+void phi(double x, double* phi1, double* phi2) {
+  *phi1 = (x == 0.0) ? 1.0 : -std::expm1(-x) / x;
+  if (std::fabs(x) < 0.5) {
+    // sum_{j>=0} (-x)^j / (j+2)!
+    double term = 0.5, sum = 0.5;
+    for (int j = 1; j <= 40; ++j) {
+      term = term * (-x) / double(j + 2);
+      double next = sum + term;
+      if (next == sum) break;
+      sum = next;
+    }
+    *phi2 = sum;
+  } else {
+    *phi2 = (std::expm1(-x) + x) / (x * x);
+  }
+}
+
+struct Coef {
+  std::vector<double> ca, cj, ch, ka, kb, kc;
+  double chh, m;
+};
+
+// S0 — the six per-cell coefficients of SURVEY §8(a) row a0.  Derivation:
+// write (11) as J' = a J + (b-c) E + c E', put it into (12), collect E'
+// (this is eq. (13) with the 1/D the print drops restored — SURVEY G1).
+void coefficients(int64_t n, const double* wp, const double* nu, double dz, double dt,
+                  double* ca, double* cj, double* ch, double* ka, double* kb, double* kc,
+                  double* chh, double* m) {
+  for (int64_t k = 0; k < n; ++k) {
+    const double x = nu[k] * dt;
+    const double a = std::exp(-x);
+    double p1, p2;
+    phi(x, &p1, &p2);
+    const double beta = dt * p1;                 // (1 - a)/nu
+    const double gamma = dt * p2;                // (a - 1 + x)/(nu^2 dt)
+    const double wp2 = wp[k] * wp[k];
+    const double b = kEps0 * wp2 * beta;
+    const double c = kEps0 * wp2 * gamma;
+    const double D = 1.0 + wp2 * gamma * dt / 2.0;
+    ca[k] = 1.0 - (wp2 * beta * dt / 2.0) / D;
+    cj[k] = (dt / (2.0 * kEps0)) * (1.0 + a) / D;
+    ch[k] = (dt / (kEps0 * dz)) / D;
+    ka[k] = a;
+    kb[k] = b - c;
+    kc[k] = c;
+  }
+  *chh = dt / (kMu0 * dz);                        // eq. (14), PAPER.md:84 ("dx" is dz, G3)
+  const double S = kC0 * dt / dz;
+  *m = (S - 1.0) / (S + 1.0);                     // Mur first order
+}
+
+// Source sample added to E^{n+1}: s[n+1], s[i] = s(i dt).
+// kind 0: eq. (15) PAPER.md:125 normalised to unit peak:
+//   s(t) = A ((t-t0)/tau) exp(1/2 - (t-t0)^2/(2 tau^2)),  params = {tau, t0, A}.
+// kind 1: table; params[i] is the value added at step index i (0-based), 0 beyond.
+double source_sample(int kind, const double* params, int64_t nparams, int64_t step_index, double dt) {
+  if (kind == 0) {
+    const double tau = params[0], t0 = params[1], A = params[2];
+    const double t = double(step_index + 1) * dt;
+    const double u = (t - t0) / tau;
+    return A * u * std::exp(0.5 - 0.5 * u * u);
+  }
+  if (kind == 1) return (step_index >= 0 && step_index < nparams) ? params[step_index] : 0.0;
+  return 0.0;
+}
+
+}  // namespace
+
+extern "C" {
+
+void oracle_constants(double* c0, double* mu0, double* eps0) {
+  *c0 = kC0; *mu0 = kMu0; *eps0 = kEps0;
+}
+
+void oracle_phi(double x, double* phi1, double* phi2) { phi(x, phi1, phi2); }
+
+int oracle_coefficients(int64_t n, const double* wp, const double* nu, double dz, double dt,
+                        double* ca, double* cj, double* ch, double* ka, double* kb, double* kc,
+                        double* chh, double* m) {
+  if (n < 0 || dz <= 0 || dt <= 0) return 1;
+  coefficients(n, wp, nu, dz, dt, ca, cj, ch, ka, kb, kc, chh, m);
+  return 0;
+}
+
+double oracle_source(int kind, const double* params, int64_t nparams, int64_t step_index, double dt) {
+  return source_sample(kind, params, nparams, step_index, dt);
+}
+
+// Advance nbatch independent grids by nsteps steps, continuing from global step
+// index step0 (so that repeated calls continue the same run).
+//   wp, nu          [nbatch][ncells]  rad/s, 1/s
+//   E, H, J         [nbatch][ncells]  in/out (state at step step0 in, step0+nsteps out)
+//   probes          [nprobes]         cells, the same in every grid (may be NULL if nprobes==0)
+//   rec, recJ       [nbatch][nprobes][nsteps]  E' resp. J' at the probe cells, sample n <-> time
+//                   (step0+n+1) dt; either may be NULL
+//   freqs           [nfreq] Hz; dft_re/dft_im [nbatch][nprobes][nfreq] accumulators (in/out), NULL = off
+//   boundary        0 = Mur first order (a3), 1 = PEC (E[0] = E[N-1] = 0; oracle-only, for pin P3)
+int oracle_run(int64_t ncells, int64_t nbatch, double dz, double dt,
+               const double* wp, const double* nu, double* E, double* H, double* J,
+               int src_kind, const double* src_params, int64_t nparams, int64_t src_cell,
+               const int64_t* probes, int nprobes, int64_t step0, int64_t nsteps,
+               double* rec, double* recJ,
+               const double* freqs, int nfreq, double* dft_re, double* dft_im,
+               int boundary) {
+  const int64_t N = ncells;
+  if (N < 3 || nbatch < 1 || nsteps < 0 || dz <= 0 || dt <= 0) return 1;
+  if (src_kind >= 0 && (src_cell < 0 || src_cell >= N)) return 1;
+  for (int p = 0; p < nprobes; ++p)
+    if (probes[p] < 0 || probes[p] >= N) return 1;
+
+  // Single grid: parallelise over k inside a step.  Batch: parallelise over grids.
+  const bool par_cells = (nbatch == 1);
+  (void)par_cells;
+
+#pragma omp parallel for schedule(static) if (!par_cells)
+  for (int64_t g = 0; g < nbatch; ++g) {
+    const double* wpg = wp + g * N;
+    const double* nug = nu + g * N;
+    double* Eg = E + g * N;
+    double* Hg = H + g * N;
+    double* Jg = J + g * N;
+
+    // S0
+    Coef cf;
+    cf.ca.resize(N); cf.cj.resize(N); cf.ch.resize(N); cf.ka.resize(N); cf.kb.resize(N); cf.kc.resize(N);
+    coefficients(N, wpg, nug, dz, dt, cf.ca.data(), cf.cj.data(), cf.ch.data(), cf.ka.data(),
+                 cf.kb.data(), cf.kc.data(), &cf.chh, &cf.m);
+    const double* ca = cf.ca.data(); const double* cj = cf.cj.data(); const double* ch = cf.ch.data();
+    const double* ka = cf.ka.data(); const double* kb = cf.kb.data(); const double* kc = cf.kc.data();
+    const double chh = cf.chh, m = cf.m;
+    std::vector<double> Eold_v(N);
+    double* Eold = Eold_v.data();
+
+    for (int64_t n = 0; n < nsteps; ++n) {
+      const int64_t ng = step0 + n;             // global step index: advances E^{ng} -> E^{ng+1}
+
+      // S1: H update, eq. (14)
+#pragma omp parallel for schedule(static) if (par_cells)
+      for (int64_t k = 0; k <= N - 2; ++k) Hg[k] = Hg[k] - chh * (Eg[k + 1] - Eg[k]);
+
+      // S2: E update, eq. (12) with (11) substituted
+#pragma omp parallel for schedule(static) if (par_cells)
+      for (int64_t k = 0; k < N; ++k) Eold[k] = Eg[k];
+#pragma omp parallel for schedule(static) if (par_cells)
+      for (int64_t k = 1; k <= N - 2; ++k)
+        Eg[k] = ca[k] * Eold[k] - cj[k] * Jg[k] - ch[k] * (Hg[k] - Hg[k - 1]);
+
+      // S3: boundary cells (not in the paper, which uses PML: PAPER.md:123)
+      if (boundary == 0) {
+        Eg[0] = Eold[1] + m * (Eg[1] - Eold[0]);
+        Eg[N - 1] = Eold[N - 2] + m * (Eg[N - 2] - Eold[N - 1]);
+      } else {
+        Eg[0] = 0.0;
+        Eg[N - 1] = 0.0;
+      }
+
+      // S4: soft source, eq. (15)
+      if (src_kind >= 0) Eg[src_cell] += source_sample(src_kind, src_params, nparams, ng, dt);
+
+      // S5: J update, eq. (11)  PAPER.md:68 — every node, with the final E'
+#pragma omp parallel for schedule(static) if (par_cells)
+      for (int64_t k = 0; k < N; ++k) Jg[k] = ka[k] * Jg[k] + kb[k] * Eold[k] + kc[k] * Eg[k];
+
+      // S6: probes (and the running DFT, evaluated directly — no phasor recurrence)
+      for (int p = 0; p < nprobes; ++p) {
+        const double v = Eg[probes[p]];
+        if (rec) rec[(g * nprobes + p) * nsteps + n] = v;
+        if (recJ) recJ[(g * nprobes + p) * nsteps + n] = Jg[probes[p]];
+        if (dft_re && dft_im) {
+          for (int q = 0; q < nfreq; ++q) {
+            const double theta = 2.0 * kPi * freqs[q] * (double(ng + 1) * dt);
+            dft_re[(g * nprobes + p) * nfreq + q] += v * std::cos(theta);
+            dft_im[(g * nprobes + p) * nfreq + q] -= v * std::sin(theta);
+          }
+        }
+      }
+    }
+  }
+  return 0;
+}
+
+}  // extern "C"
