@@ -1,0 +1,132 @@
+/* ============================================================================
+ * rketd.h — C ABI of librketd: the per-time-step leapfrog hot path of the 1-D
+ * RKETD-FDTD method for an unmagnetized collisional (Drude) plasma
+ * (arxiv 1709.00821; citations are PAPER.md:<line> of /root/reference/PAPER.md
+ * and SURVEY.md §8 rows).  sm_100a (B200) only; there is no CPU fallback: every
+ * compute entry point returns RKETD_ECUDA when no CUDA device is usable.
+ *
+ * Conventions
+ *   - Every call returns an int status (RKETD_OK = 0) and never throws.
+ *   - The caller owns every buffer it passes; set_* copy, so the buffer may be
+ *     freed or reused as soon as the call returns.  The library owns the handle
+ *     and all device state.  One handle is used from one host thread.
+ *   - "host or device" pointers: any pointer cudaMemcpy(..., cudaMemcpyDefault)
+ *     accepts (pageable / pinned host memory, device memory, managed memory).
+ *   - Grids: nbatch independent 1-D grids of ncells E-nodes each.  Node k holds
+ *     E[k] = Ex(k dz) and J[k] = Jx(k dz) at integer time steps and
+ *     H[k] = Hy((k+1/2) dz) at half steps (k = 0..ncells-2; H[ncells-1] is
+ *     padding, reported as 0).  User arrays are row-major [nbatch][ncells].
+ *   - Physical constants are fixed: c = 299792458 m/s, mu0 = 4 pi 1e-7 H/m,
+ *     eps0 = 1/(mu0 c^2)  (the paper gives no values).
+ *   - All work is enqueued on the CUDA stream given to rketd_create.
+ * ========================================================================== */
+#ifndef RKETD_H_
+#define RKETD_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rketd_sim rketd_sim; /* opaque */
+
+enum { RKETD_F64 = 0, RKETD_F32 = 1 };
+enum { RKETD_OK = 0, RKETD_EINVAL = 1, RKETD_ENOMEM = 2, RKETD_ECUDA = 3, RKETD_ESTATE = 4 };
+enum { RKETD_SRC_NONE = -1, RKETD_SRC_GAUSS_DERIV = 0, RKETD_SRC_TABLE = 1 };
+/* kernel selection for rketd_set_plan */
+enum {
+  RKETD_KERNEL_AUTO = 0,     /* resident (K3) when a grid fits one CTA, else temporal blocking (K2) */
+  RKETD_KERNEL_STEP = 1,     /* K1: one fused H/E/J launch per time step (baseline / cross-check)   */
+  RKETD_KERNEL_TBLOCK = 2,   /* K2: T leapfrog steps per pass on a register-resident tile, TMA-staged */
+  RKETD_KERNEL_RESIDENT = 3  /* K3: whole grid resident on chip for the whole run, one CTA per grid  */
+};
+/* counters for rketd_get_counter */
+enum {
+  RKETD_CTR_LAUNCHES = 0,      /* kernels launched by this handle so far (all kinds)               */
+  RKETD_CTR_STEP_LAUNCHES = 1, /* launches of the stencil kernel (K1/K2/K3) so far                  */
+  RKETD_CTR_KERNEL_USED = 2,   /* RKETD_KERNEL_* the last rketd_run used                            */
+  RKETD_CTR_DEPTH_USED = 3,    /* temporal depth T of the last K2 run (steps per pass)              */
+  RKETD_CTR_STEPS_DONE = 4,    /* global step counter                                               */
+  RKETD_CTR_TILE_CELLS = 5,    /* cells per CTA tile, halo included, of the last K2/K3 run          */
+  RKETD_CTR_HALO_CELLS = 6,    /* halo cells on each side of a K2 tile                              */
+  RKETD_CTR_STATE_BYTES = 7    /* device bytes held by this handle (fields + coefficients)          */
+};
+
+/* Create a simulation of nbatch grids of ncells nodes ("grid" of the north_star =
+ * (ncells, nbatch)).  dz [m], dt [s]; dtype RKETD_F64 or RKETD_F32 (arithmetic and
+ * storage type of fields, coefficients, probe records).  cuda_stream: a cudaStream_t
+ * (e.g. torch.cuda.current_stream().cuda_stream) or NULL for the default stream.
+ * Fields start at zero, step counter at 0, no source, no probes.
+ * EINVAL: ncells < 3, nbatch < 1, dz <= 0, dt <= 0, c dt/dz > 1 (unstable), bad dtype.
+ * Host code role: PAPER.md:93 (init, device alloc, copies). */
+int rketd_create(rketd_sim **out, int64_t ncells, int64_t nbatch, double dz, double dt, int dtype,
+                 void *cuda_stream);
+
+/* Per-node plasma frequency wp [rad/s] and collision frequency nu [1/s], always fp64,
+ * [nbatch][ncells], host or device.  Precomputes (in fp64, on the device) the six per-node
+ * coefficients of SURVEY §8(a) row a0, i.e. eq. (11) PAPER.md:68 written as
+ * J' = ka J + kb E + kc E' and eq. (12) PAPER.md:74 with (11) substituted, solved for E'
+ * (eq. (13) PAPER.md:79 with the missing 1/D restored): E' = ca E - cj J - ch (H[k]-H[k-1]).
+ * EINVAL: any wp or nu negative or non-finite.  Synchronises the stream. */
+int rketd_set_media(rketd_sim *s, const double *wp, const double *nu);
+
+/* Soft source added to E^{n+1}[cell] in every grid (eq. (15)).
+ * kind RKETD_SRC_GAUSS_DERIV: params = {tau, t0, amplitude},
+ *   s(t) = amplitude ((t-t0)/tau) exp(1/2 - (t-t0)^2/(2 tau^2)), sample added at step n: s((n+1) dt).
+ * kind RKETD_SRC_TABLE: params[i] is added at step index i (0-based); 0 beyond nparams.
+ * kind RKETD_SRC_NONE: no source.  params is a HOST pointer.  EINVAL: cell outside [0, ncells). */
+int rketd_set_source(rketd_sim *s, int kind, const double *params, int64_t nparams, int64_t cell);
+
+/* Probe nodes (host pointer), the same in every grid; at most 64.  Each step records
+ * E^{n+1}[cell].  Discards earlier records.  EINVAL: cell outside [0, ncells). */
+int rketd_set_probes(rketd_sim *s, const int64_t *cells, int nprobes);
+
+/* Reduce the probe records on the device to DFT magnitudes (BASELINE config 5):
+ * X[g][p][m] = sum_n rec[g][p][n] exp(-j 2 pi f_m (n+1) dt), accumulated in fp64.
+ * freqs_hz host pointer; nfreq = 0 switches back to time-series mode.  Discards earlier records. */
+int rketd_set_probe_dft(rketd_sim *s, const double *freqs_hz, int nfreq);
+
+/* Overwrite the fields; arrays are [nbatch][ncells] in the handle's dtype, host or device;
+ * NULL = zeros.  Does not touch the step counter or the probe records.  Synchronises. */
+int rketd_set_fields(rketd_sim *s, const void *E, const void *H, const void *J);
+
+/* Fields zero, step counter 0, probe records and DFT accumulators discarded; media, source and
+ * probes kept. */
+int rketd_reset(rketd_sim *s);
+
+/* Choose the kernel (RKETD_KERNEL_*) and, for K2, the temporal depth T (0 = default).
+ * EINVAL if the choice cannot run this grid (e.g. RESIDENT with a grid larger than one CTA). */
+int rketd_set_plan(rketd_sim *s, int kernel, int depth);
+
+/* Advance every grid by nsteps leapfrog steps (H eq. (14); E eq. (12)
+ * with (11); Mur-1 at both ends; soft source; J eq. (11); probe record), asynchronously on the
+ * stream.  Repeatable: time continues.  ESTATE before rketd_set_media. */
+int rketd_run(rketd_sim *s, int64_t nsteps);
+
+/* Synchronise and copy out the probe records (host or device `out`, handle's dtype).
+ * Time-series mode: [nbatch][nprobes][nsamples], nsamples = steps run since the records were last
+ * discarded; sample n is E at time (n+1) dt.  DFT mode: [nbatch][nprobes][nfreq] magnitudes,
+ * *nsamples = nfreq.  out may be NULL to query *nsamples.  EINVAL if out_bytes is too small. */
+int rketd_read_probes(rketd_sim *s, void *out, int64_t out_bytes, int64_t *nsamples);
+
+/* Copy the fields out ([nbatch][ncells], handle's dtype, host or device; any may be NULL).
+ * Synchronises. */
+int rketd_get_fields(rketd_sim *s, void *E, void *H, void *J);
+
+/* Copy the six coefficient arrays out as fp64, order ca, cj, ch, ka, kb, kc:
+ * out[6][nbatch][ncells] (host or device); chh_m[2] = {dt/(mu0 dz), Mur m} (host; may be NULL). */
+int rketd_get_coefficients(rketd_sim *s, double *out, double *chh_m);
+
+/* RKETD_CTR_* counters (for bench.py's gpu_launches and roofline bookkeeping). */
+int64_t rketd_get_counter(const rketd_sim *s, int which);
+
+void rketd_destroy(rketd_sim *s);
+
+/* Text of the last error on this handle (or of the last failed rketd_create when s is NULL). */
+const char *rketd_last_error(const rketd_sim *s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RKETD_H_ */

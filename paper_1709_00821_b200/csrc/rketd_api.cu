@@ -1,0 +1,574 @@
+// rketd_api.cu — the C ABI of librketd (include/rketd.h): handle, device state, plans, launches.
+// Host-side logic only; every step of the hot path runs in the kernels of rketd_kernels.cu.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/rketd.h"
+#include "rketd_device.cuh"
+#include "rketd_internal.h"
+
+using namespace rketd;
+
+namespace {
+std::string g_create_error;
+
+struct Chunk {
+  void *buf;
+  int64_t nsteps;
+};
+}  // namespace
+
+struct rketd_sim {
+  Layout L;
+  double dz = 0, dt = 0;
+  int dtype = 0;
+  cudaStream_t stream = nullptr;
+  void *fld[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};
+  int cur = 0;
+  void *coef[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  uint8_t *rowflag = nullptr;
+  bool flags_dirty = true;
+  bool have_media = false;
+  int *d_bad = nullptr;
+  int src_kind = RKETD_SRC_NONE;
+  std::vector<double> src_params;
+  int64_t src_cell = -1;
+  void *d_srctab = nullptr;
+  int64_t srctab_cap = 0;
+  std::vector<int64_t> probes;
+  std::vector<double> freqs;
+  double *d_freqs = nullptr, *dft_re = nullptr, *dft_im = nullptr;
+  std::vector<Chunk> chunks;
+  int64_t nsamples = 0;
+  int64_t step = 0;
+  int plan_kernel = RKETD_KERNEL_AUTO, plan_depth = 0;
+  K2Plan k2;
+  bool k2_valid = false;
+  int64_t ctr_launches = 0, ctr_step_launches = 0, ctr_kernel_used = 0, ctr_depth_used = 0, ctr_tile_cells = 0,
+          ctr_halo_cells = 0, state_bytes = 0;
+  std::string err;
+};
+
+namespace {
+
+int fail(rketd_sim *s, int code, const std::string &msg) {
+  if (s) s->err = msg; else g_create_error = msg;
+  return code;
+}
+#define CU_TRY(s, expr)                                                                          \
+  do {                                                                                           \
+    cudaError_t e__ = (expr);                                                                    \
+    if (e__ != cudaSuccess)                                                                      \
+      return fail(s, e__ == cudaErrorMemoryAllocation ? RKETD_ENOMEM : RKETD_ECUDA,              \
+                  std::string(#expr) + ": " + cudaGetErrorString(e__));                          \
+  } while (0)
+
+size_t arr_bytes(const Layout &L) { return (size_t)L.gstride * L.nbatch * L.esize; }
+
+// pack / unpack between the user's [nbatch][ncells] and the padded physical layout
+cudaError_t copy_in(const rketd_sim *s, void *dst_phys, const void *src_user) {
+  const Layout &L = s->L;
+  return cudaMemcpy2DAsync((char *)dst_phys + (size_t)L.off * L.esize, (size_t)L.gstride * L.esize, src_user,
+                           (size_t)L.ncells * L.esize, (size_t)L.ncells * L.esize, (size_t)L.nbatch, cudaMemcpyDefault,
+                           s->stream);
+}
+cudaError_t copy_out(const rketd_sim *s, void *dst_user, const void *src_phys) {
+  const Layout &L = s->L;
+  return cudaMemcpy2DAsync(dst_user, (size_t)L.ncells * L.esize, (const char *)src_phys + (size_t)L.off * L.esize,
+                           (size_t)L.gstride * L.esize, (size_t)L.ncells * L.esize, (size_t)L.nbatch, cudaMemcpyDefault,
+                           s->stream);
+}
+
+void discard_records(rketd_sim *s) {
+  for (auto &c : s->chunks) cudaFree(c.buf);
+  s->chunks.clear();
+  s->nsamples = 0;
+  if (s->dft_re) {
+    const size_t n = (size_t)s->L.nbatch * s->probes.size() * s->freqs.size() * sizeof(double);
+    cudaMemsetAsync(s->dft_re, 0, n, s->stream);
+    cudaMemsetAsync(s->dft_im, 0, n, s->stream);
+  }
+}
+
+int realloc_dft(rketd_sim *s) {
+  if (s->dft_re) { cudaFree(s->dft_re); cudaFree(s->dft_im); s->dft_re = s->dft_im = nullptr; }
+  if (s->d_freqs) { cudaFree(s->d_freqs); s->d_freqs = nullptr; }
+  if (s->freqs.empty() || s->probes.empty()) return RKETD_OK;
+  const size_t n = (size_t)s->L.nbatch * s->probes.size() * s->freqs.size() * sizeof(double);
+  CU_TRY(s, cudaMalloc(&s->dft_re, n));
+  CU_TRY(s, cudaMalloc(&s->dft_im, n));
+  CU_TRY(s, cudaMalloc(&s->d_freqs, s->freqs.size() * sizeof(double)));
+  CU_TRY(s, cudaMemcpyAsync(s->d_freqs, s->freqs.data(), s->freqs.size() * sizeof(double), cudaMemcpyHostToDevice,
+                            s->stream));
+  CU_TRY(s, cudaMemsetAsync(s->dft_re, 0, n, s->stream));
+  CU_TRY(s, cudaMemsetAsync(s->dft_im, 0, n, s->stream));
+  CU_TRY(s, cudaStreamSynchronize(s->stream));
+  return RKETD_OK;
+}
+
+int rebuild_rowflags(rketd_sim *s) {
+  const Layout &L = s->L;
+  std::vector<uint8_t> f((size_t)L.nrows, 0);
+  f[(size_t)(L.off / L.C)] |= F_MURL;
+  f[(size_t)((L.off + L.ncells - 1) / L.C)] |= F_MURR;
+  if (s->src_kind != RKETD_SRC_NONE) f[(size_t)((L.off + s->src_cell) / L.C)] |= F_SRC;
+  for (int64_t c : s->probes) f[(size_t)((L.off + c) / L.C)] |= F_PROBE;
+  CU_TRY(s, cudaMemcpyAsync(s->rowflag, f.data(), f.size(), cudaMemcpyHostToDevice, s->stream));
+  CU_TRY(s, cudaStreamSynchronize(s->stream));   // f is a local
+  s->flags_dirty = false;
+  return RKETD_OK;
+}
+
+double source_sample(const rketd_sim *s, int64_t step_index) {
+  if (s->src_kind == RKETD_SRC_GAUSS_DERIV) {
+    const double tau = s->src_params[0], t0 = s->src_params[1], A = s->src_params[2];
+    const double u = ((double)(step_index + 1) * s->dt - t0) / tau;
+    return A * u * std::exp(0.5 - 0.5 * u * u);
+  }
+  if (s->src_kind == RKETD_SRC_TABLE)
+    return (step_index >= 0 && step_index < (int64_t)s->src_params.size()) ? s->src_params[(size_t)step_index] : 0.0;
+  return 0.0;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode() {
+  static EncodeTiledFn fn = nullptr;
+  if (!fn) {
+    void *p = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+        qres == cudaDriverEntryPointSuccess)
+      fn = (EncodeTiledFn)p;
+  }
+  return fn;
+}
+
+// 3-D view {C, nrows, nbatch} of one per-node array, rows of 64 B, box {C, box_rows, 1}, 64-B swizzle.
+int make_map(rketd_sim *s, CUtensorMap *m, void *base, int box_rows) {
+  EncodeTiledFn enc = get_encode();
+  if (!enc) return fail(s, RKETD_ECUDA, "cuTensorMapEncodeTiled not available from the driver");
+  const Layout &L = s->L;
+  cuuint64_t dims[3] = {(cuuint64_t)L.C, (cuuint64_t)L.nrows, (cuuint64_t)L.nbatch};
+  cuuint64_t strides[2] = {(cuuint64_t)kRowBytes, (cuuint64_t)L.nrows * kRowBytes};
+  cuuint32_t box[3] = {(cuuint32_t)L.C, (cuuint32_t)box_rows, 1u};
+  cuuint32_t estr[3] = {1u, 1u, 1u};
+  CUresult r = enc(m, L.esize == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, base, dims,
+                   strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B,
+                   CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return fail(s, RKETD_ECUDA, "cuTensorMapEncodeTiled failed: " + std::to_string((int)r));
+  return RKETD_OK;
+}
+
+int default_depth(const rketd_sim *s) { return s->dtype == RKETD_F64 ? 24 : 32; }
+int default_k2_threads(const rketd_sim *) { return 128; }
+
+int build_k2_plan(rketd_sim *s, int depth, int NT) {
+  const Layout &L = s->L;
+  K2Plan &P = s->k2;
+  if (s->k2_valid && P.depth == depth && P.NT == NT) return RKETD_OK;
+  const int HR = (depth + L.C - 1) / L.C;
+  if (NT - 2 * HR < 1) return fail(s, RKETD_EINVAL, "temporal depth too large for the tile");
+  P.NT = NT; P.HR = HR; P.rows_out = NT - 2 * HR; P.depth = depth;
+  P.tiles_per_grid = (L.nrows + P.rows_out - 1) / P.rows_out;
+  P.total_tiles = P.tiles_per_grid * L.nbatch;
+  P.smem_bytes = k2_smem_bytes(NT);
+  int ctas = 0, dev = 0, sms = 0;
+  CU_TRY(s, k2_configure(s->dtype, NT, &ctas));
+  if (ctas < 1) return fail(s, RKETD_ECUDA, "K2 kernel does not fit on an SM");
+  CU_TRY(s, cudaGetDevice(&dev));
+  CU_TRY(s, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  P.ctas_per_sm = ctas;
+  P.grid = (int)std::min<int64_t>(P.total_tiles, (int64_t)sms * ctas);
+  for (int b = 0; b < 2; ++b) {
+    for (int a = 0; a < 3; ++a) {
+      int rc = make_map(s, &P.maps[b].ld[a], s->fld[b][a], NT);
+      if (rc) return rc;
+      rc = make_map(s, &P.maps[b].st[a], s->fld[1 - b][a], P.rows_out);
+      if (rc) return rc;
+    }
+    for (int a = 0; a < 6; ++a) {
+      int rc = make_map(s, &P.maps[b].ld[3 + a], s->coef[a], NT);
+      if (rc) return rc;
+    }
+  }
+  s->k2_valid = true;
+  return RKETD_OK;
+}
+
+int resolve_kernel(rketd_sim *s) {
+  if (s->plan_kernel != RKETD_KERNEL_AUTO) return s->plan_kernel;
+  return k3_threads_for_rows(s->dtype, s->L.nrows) ? RKETD_KERNEL_RESIDENT : RKETD_KERNEL_TBLOCK;
+}
+
+// run nsteps steps whose probe samples go to rec ([nbatch][nprobes][nsteps] or nullptr)
+int run_segment(rketd_sim *s, int64_t nsteps, void *rec) {
+  const Layout &L = s->L;
+  // source samples of this segment
+  const void *d_src = nullptr;
+  if (s->src_kind != RKETD_SRC_NONE) {
+    if (s->srctab_cap < nsteps) {
+      if (s->d_srctab) cudaFree(s->d_srctab);
+      s->d_srctab = nullptr; s->srctab_cap = 0;
+      CU_TRY(s, cudaMalloc(&s->d_srctab, (size_t)nsteps * L.esize));
+      s->srctab_cap = nsteps;
+    }
+    if (s->dtype == RKETD_F64) {
+      std::vector<double> tab((size_t)nsteps);
+      for (int64_t n = 0; n < nsteps; ++n) tab[(size_t)n] = source_sample(s, s->step + n);
+      CU_TRY(s, cudaMemcpyAsync(s->d_srctab, tab.data(), tab.size() * 8, cudaMemcpyHostToDevice, s->stream));
+    } else {
+      std::vector<float> tab((size_t)nsteps);
+      for (int64_t n = 0; n < nsteps; ++n) tab[(size_t)n] = (float)source_sample(s, s->step + n);
+      CU_TRY(s, cudaMemcpyAsync(s->d_srctab, tab.data(), tab.size() * 4, cudaMemcpyHostToDevice, s->stream));
+    }
+    d_src = s->d_srctab;
+  }
+  StepCommon sc;
+  std::memset(&sc, 0, sizeof(sc));
+  sc.nchh = -(s->dt / (kMu0 * s->dz));
+  const double S = kC0 * s->dt / s->dz;
+  sc.mur_m = (S - 1.0) / (S + 1.0);
+  sc.cellL = L.off; sc.cellR = L.off + L.ncells - 1;
+  sc.cellS = s->src_kind == RKETD_SRC_NONE ? -1 : L.off + s->src_cell;
+  sc.nprobes = (int)s->probes.size();
+  for (size_t i = 0; i < s->probes.size(); ++i) sc.probe_cell[i] = L.off + s->probes[i];
+  sc.rec_stride = nsteps; sc.n0 = 0; sc.src_tab = d_src; sc.rec = rec; sc.rowflag = s->rowflag;
+
+  const int kern = resolve_kernel(s);
+  s->ctr_kernel_used = kern;
+  if (kern == RKETD_KERNEL_STEP) {
+    for (int64_t n = 0; n < nsteps; ++n) {
+      sc.n0 = n;
+      FieldPtrs src{s->fld[s->cur][0], s->fld[s->cur][1], s->fld[s->cur][2]};
+      FieldPtrs dst{s->fld[1 - s->cur][0], s->fld[1 - s->cur][1], s->fld[1 - s->cur][2]};
+      CU_TRY(s, launch_k1(s->dtype, L, src, dst, s->coef, sc, s->stream));
+      s->cur ^= 1;
+      ++s->ctr_launches; ++s->ctr_step_launches;
+    }
+    s->ctr_tile_cells = L.C; s->ctr_halo_cells = 1; s->ctr_depth_used = 1;
+  } else if (kern == RKETD_KERNEL_RESIDENT) {
+    const int NT = k3_threads_for_rows(s->dtype, L.nrows);
+    if (!NT) return fail(s, RKETD_EINVAL, "grid too large for the resident kernel");
+    FieldPtrs f{s->fld[s->cur][0], s->fld[s->cur][1], s->fld[s->cur][2]};
+    CU_TRY(s, launch_k3(s->dtype, L, f, s->coef, sc, nsteps, NT, s->stream));
+    ++s->ctr_launches; ++s->ctr_step_launches;
+    s->ctr_tile_cells = (int64_t)NT * L.C; s->ctr_halo_cells = 0; s->ctr_depth_used = nsteps;
+  } else {
+    const int NT = default_k2_threads(s);
+    int depth = s->plan_depth > 0 ? s->plan_depth : default_depth(s);
+    depth = std::min<int>(depth, (NT / 2 - 1) * L.C);
+    int rc = build_k2_plan(s, depth, NT);
+    if (rc) return rc;
+    for (int64_t n = 0; n < nsteps; n += depth) {
+      const int steps = (int)std::min<int64_t>(depth, nsteps - n);
+      sc.n0 = n;
+      CU_TRY(s, launch_k2(s->dtype, L, s->k2, s->cur, sc, steps, s->stream));
+      s->cur ^= 1;
+      ++s->ctr_launches; ++s->ctr_step_launches;
+    }
+    s->ctr_tile_cells = (int64_t)NT * L.C; s->ctr_halo_cells = (int64_t)s->k2.HR * L.C; s->ctr_depth_used = depth;
+  }
+  s->step += nsteps;
+  return RKETD_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int rketd_create(rketd_sim **out, int64_t ncells, int64_t nbatch, double dz, double dt, int dtype, void *cuda_stream) {
+  if (!out) return fail(nullptr, RKETD_EINVAL, "out is NULL");
+  *out = nullptr;
+  if (ncells < 3 || nbatch < 1 || !(dz > 0) || !(dt > 0) || (dtype != RKETD_F64 && dtype != RKETD_F32))
+    return fail(nullptr, RKETD_EINVAL, "rketd_create: invalid argument");
+  if (kC0 * dt / dz > 1.0 + 1e-12) return fail(nullptr, RKETD_EINVAL, "rketd_create: c dt/dz > 1 is unstable");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+    cudaGetLastError();
+    return fail(nullptr, RKETD_ECUDA, "rketd_create: no CUDA device (librketd has no CPU fallback)");
+  }
+  rketd_sim *s = new rketd_sim();
+  Layout &L = s->L;
+  L.ncells = ncells; L.nbatch = nbatch;
+  L.esize = dtype == RKETD_F64 ? 8 : 4;
+  L.C = kRowBytes / L.esize;
+  L.off = ((ncells - 1) % L.C == 0) ? 1 : 0;
+  L.nrows = (L.off + ncells + L.C - 1) / L.C;
+  L.gstride = L.nrows * L.C;
+  if (L.nrows > 0x7fffff00LL || nbatch > 0x7fffff00LL) { delete s; return fail(nullptr, RKETD_EINVAL, "grid too large"); }
+  s->dz = dz; s->dt = dt; s->dtype = dtype; s->stream = (cudaStream_t)cuda_stream;
+  const size_t nb = arr_bytes(L);
+  auto bail = [&](cudaError_t e) {
+    std::string m = std::string("rketd_create: ") + cudaGetErrorString(e);
+    rketd_destroy(s);
+    return fail(nullptr, e == cudaErrorMemoryAllocation ? RKETD_ENOMEM : RKETD_ECUDA, m);
+  };
+  cudaError_t e;
+  for (int b = 0; b < 2; ++b)
+    for (int a = 0; a < 3; ++a) {
+      if ((e = cudaMalloc(&s->fld[b][a], nb)) != cudaSuccess) return bail(e);
+      if ((e = cudaMemsetAsync(s->fld[b][a], 0, nb, s->stream)) != cudaSuccess) return bail(e);
+    }
+  for (int a = 0; a < 6; ++a) {
+    if ((e = cudaMalloc(&s->coef[a], nb)) != cudaSuccess) return bail(e);
+    if ((e = cudaMemsetAsync(s->coef[a], 0, nb, s->stream)) != cudaSuccess) return bail(e);
+  }
+  if ((e = cudaMalloc(&s->rowflag, (size_t)L.nrows)) != cudaSuccess) return bail(e);
+  if ((e = cudaMalloc(&s->d_bad, sizeof(int))) != cudaSuccess) return bail(e);
+  s->state_bytes = (int64_t)nb * 12 + L.nrows;
+  *out = s;
+  return RKETD_OK;
+}
+
+int rketd_set_media(rketd_sim *s, const double *wp, const double *nu) {
+  if (!s || !wp || !nu) return fail(s, RKETD_EINVAL, "rketd_set_media: NULL argument");
+  const Layout &L = s->L;
+  const size_t n = (size_t)L.ncells * L.nbatch * sizeof(double);
+  const double *dwp = wp, *dnu = nu;
+  void *twp = nullptr, *tnu = nullptr;
+  auto is_device = [](const void *p) {
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+  };
+  if (!is_device(wp)) {
+    CU_TRY(s, cudaMalloc(&twp, n));
+    CU_TRY(s, cudaMemcpyAsync(twp, wp, n, cudaMemcpyDefault, s->stream));
+    dwp = (const double *)twp;
+  }
+  if (!is_device(nu)) {
+    cudaError_t e = cudaMalloc(&tnu, n);
+    if (e != cudaSuccess) { if (twp) cudaFree(twp); CU_TRY(s, e); }
+    CU_TRY(s, cudaMemcpyAsync(tnu, nu, n, cudaMemcpyDefault, s->stream));
+    dnu = (const double *)tnu;
+  }
+  cudaMemsetAsync(s->d_bad, 0, sizeof(int), s->stream);
+  cudaError_t e = launch_coefficients(s->dtype, L, dwp, dnu, s->dz, s->dt, s->coef, s->d_bad, s->stream);
+  ++s->ctr_launches;
+  int bad = 0;
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&bad, s->d_bad, sizeof(int), cudaMemcpyDeviceToHost, s->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+  if (twp) cudaFree(twp);
+  if (tnu) cudaFree(tnu);
+  CU_TRY(s, e);
+  if (bad) {
+    s->have_media = false;
+    return fail(s, RKETD_EINVAL, "rketd_set_media: wp and nu must be finite and non-negative");
+  }
+  s->have_media = true;
+  return RKETD_OK;
+}
+
+int rketd_set_source(rketd_sim *s, int kind, const double *params, int64_t nparams, int64_t cell) {
+  if (!s) return RKETD_EINVAL;
+  if (kind == RKETD_SRC_NONE) { s->src_kind = kind; s->src_params.clear(); s->src_cell = -1; s->flags_dirty = true; return RKETD_OK; }
+  if (kind != RKETD_SRC_GAUSS_DERIV && kind != RKETD_SRC_TABLE) return fail(s, RKETD_EINVAL, "rketd_set_source: unknown kind");
+  if (cell < 0 || cell >= s->L.ncells) return fail(s, RKETD_EINVAL, "rketd_set_source: cell outside the grid");
+  if (nparams < 0 || (nparams > 0 && !params)) return fail(s, RKETD_EINVAL, "rketd_set_source: bad params");
+  if (kind == RKETD_SRC_GAUSS_DERIV && (nparams != 3 || !(params[0] > 0)))
+    return fail(s, RKETD_EINVAL, "rketd_set_source: GAUSS_DERIV needs {tau > 0, t0, amplitude}");
+  s->src_kind = kind;
+  s->src_params.assign(params, params + nparams);
+  s->src_cell = cell;
+  s->flags_dirty = true;
+  return RKETD_OK;
+}
+
+int rketd_set_probes(rketd_sim *s, const int64_t *cells, int nprobes) {
+  if (!s) return RKETD_EINVAL;
+  if (nprobes < 0 || nprobes > kMaxProbes || (nprobes > 0 && !cells)) return fail(s, RKETD_EINVAL, "rketd_set_probes: 0..64 probes");
+  for (int i = 0; i < nprobes; ++i)
+    if (cells[i] < 0 || cells[i] >= s->L.ncells) return fail(s, RKETD_EINVAL, "rketd_set_probes: cell outside the grid");
+  discard_records(s);
+  s->probes.assign(cells, cells + nprobes);
+  s->flags_dirty = true;
+  return realloc_dft(s);
+}
+
+int rketd_set_probe_dft(rketd_sim *s, const double *freqs_hz, int nfreq) {
+  if (!s) return RKETD_EINVAL;
+  if (nfreq < 0 || (nfreq > 0 && !freqs_hz)) return fail(s, RKETD_EINVAL, "rketd_set_probe_dft: bad argument");
+  discard_records(s);
+  s->freqs.assign(freqs_hz, freqs_hz + nfreq);
+  return realloc_dft(s);
+}
+
+int rketd_set_fields(rketd_sim *s, const void *E, const void *H, const void *J) {
+  if (!s) return RKETD_EINVAL;
+  const void *src[3] = {E, H, J};
+  for (int a = 0; a < 3; ++a) {
+    CU_TRY(s, cudaMemsetAsync(s->fld[s->cur][a], 0, arr_bytes(s->L), s->stream));
+    if (src[a]) CU_TRY(s, copy_in(s, s->fld[s->cur][a], src[a]));
+  }
+  CU_TRY(s, cudaStreamSynchronize(s->stream));
+  return RKETD_OK;
+}
+
+int rketd_reset(rketd_sim *s) {
+  if (!s) return RKETD_EINVAL;
+  for (int a = 0; a < 3; ++a) CU_TRY(s, cudaMemsetAsync(s->fld[s->cur][a], 0, arr_bytes(s->L), s->stream));
+  discard_records(s);
+  s->step = 0;
+  return RKETD_OK;
+}
+
+int rketd_set_plan(rketd_sim *s, int kernel, int depth) {
+  if (!s) return RKETD_EINVAL;
+  if (kernel < RKETD_KERNEL_AUTO || kernel > RKETD_KERNEL_RESIDENT || depth < 0) return fail(s, RKETD_EINVAL, "rketd_set_plan: bad argument");
+  if (kernel == RKETD_KERNEL_RESIDENT && !k3_threads_for_rows(s->dtype, s->L.nrows))
+    return fail(s, RKETD_EINVAL, "rketd_set_plan: grid does not fit the resident kernel");
+  if (depth > (default_k2_threads(s) / 2 - 1) * s->L.C) return fail(s, RKETD_EINVAL, "rketd_set_plan: depth too large");
+  s->plan_kernel = kernel;
+  s->plan_depth = depth;
+  return RKETD_OK;
+}
+
+int rketd_run(rketd_sim *s, int64_t nsteps) {
+  if (!s) return RKETD_EINVAL;
+  if (nsteps < 0) return fail(s, RKETD_EINVAL, "rketd_run: nsteps < 0");
+  if (!s->have_media) return fail(s, RKETD_ESTATE, "rketd_run before rketd_set_media");
+  if (nsteps == 0) return RKETD_OK;
+  if (s->flags_dirty) { int rc = rebuild_rowflags(s); if (rc) return rc; }
+  const Layout &L = s->L;
+  const int64_t nseries = L.nbatch * (int64_t)s->probes.size();
+  if (nseries == 0) return run_segment(s, nsteps, nullptr);
+  if (s->freqs.empty()) {   // time-series mode: one record chunk per call
+    void *buf = nullptr;
+    CU_TRY(s, cudaMalloc(&buf, (size_t)nseries * nsteps * L.esize));
+    s->chunks.push_back(Chunk{buf, nsteps});
+    int rc = run_segment(s, nsteps, buf);
+    if (rc) return rc;
+    s->nsamples += nsteps;
+    return RKETD_OK;
+  }
+  // DFT mode (a7): records of a segment are reduced by a second kernel, then dropped
+  const int nfreq = (int)s->freqs.size();
+  const int64_t seg_max = std::max<int64_t>(64, std::min<int64_t>(nsteps, ((int64_t)1 << 29) / (nseries * L.esize)));
+  void *buf = nullptr;
+  double2 *tw = nullptr;
+  CU_TRY(s, cudaMalloc(&buf, (size_t)nseries * std::min(seg_max, nsteps) * L.esize));
+  cudaError_t e = cudaMalloc(&tw, (size_t)std::min(seg_max, nsteps) * nfreq * sizeof(double2));
+  if (e != cudaSuccess) { cudaFree(buf); CU_TRY(s, e); }
+  int rc = RKETD_OK;
+  for (int64_t n = 0; n < nsteps && rc == RKETD_OK; n += seg_max) {
+    const int64_t seg = std::min(seg_max, nsteps - n);
+    const int64_t step0 = s->step;
+    rc = run_segment(s, seg, buf);
+    if (rc) break;
+    e = launch_twiddles(s->d_freqs, nfreq, step0, seg, s->dt, tw, s->stream);
+    if (e == cudaSuccess) e = launch_dft_accumulate(s->dtype, buf, nseries, seg, tw, nfreq, s->dft_re, s->dft_im, s->stream);
+    s->ctr_launches += 2;
+    if (e != cudaSuccess) rc = fail(s, RKETD_ECUDA, std::string("dft: ") + cudaGetErrorString(e));
+    s->nsamples += seg;
+  }
+  cudaStreamSynchronize(s->stream);   // buf and tw are freed below
+  cudaFree(buf);
+  cudaFree(tw);
+  return rc;
+}
+
+int rketd_read_probes(rketd_sim *s, void *out, int64_t out_bytes, int64_t *nsamples) {
+  if (!s) return RKETD_EINVAL;
+  const Layout &L = s->L;
+  const int64_t nseries = L.nbatch * (int64_t)s->probes.size();
+  const bool dft = !s->freqs.empty();
+  const int64_t per = dft ? (int64_t)s->freqs.size() : s->nsamples;
+  if (nsamples) *nsamples = per;
+  if (!out) { CU_TRY(s, cudaStreamSynchronize(s->stream)); return RKETD_OK; }
+  const int64_t need = nseries * per * L.esize;
+  if (out_bytes < need) return fail(s, RKETD_EINVAL, "rketd_read_probes: out buffer too small");
+  if (need == 0) { CU_TRY(s, cudaStreamSynchronize(s->stream)); return RKETD_OK; }
+  if (dft) {
+    void *tmp = nullptr;
+    CU_TRY(s, cudaMalloc(&tmp, (size_t)need));
+    cudaError_t e = launch_dft_magnitude(s->dtype, s->dft_re, s->dft_im, nseries * per, tmp, s->stream);
+    ++s->ctr_launches;
+    if (e == cudaSuccess) e = cudaMemcpyAsync(out, tmp, (size_t)need, cudaMemcpyDefault, s->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+    cudaFree(tmp);
+    CU_TRY(s, e);
+    return RKETD_OK;
+  }
+  int64_t o = 0;
+  for (const Chunk &c : s->chunks) {
+    CU_TRY(s, cudaMemcpy2DAsync((char *)out + o * L.esize, (size_t)per * L.esize, c.buf, (size_t)c.nsteps * L.esize,
+                                (size_t)c.nsteps * L.esize, (size_t)nseries, cudaMemcpyDefault, s->stream));
+    o += c.nsteps;
+  }
+  CU_TRY(s, cudaStreamSynchronize(s->stream));
+  return RKETD_OK;
+}
+
+int rketd_get_fields(rketd_sim *s, void *E, void *H, void *J) {
+  if (!s) return RKETD_EINVAL;
+  void *dst[3] = {E, H, J};
+  for (int a = 0; a < 3; ++a)
+    if (dst[a]) CU_TRY(s, copy_out(s, dst[a], s->fld[s->cur][a]));
+  CU_TRY(s, cudaStreamSynchronize(s->stream));
+  return RKETD_OK;
+}
+
+int rketd_get_coefficients(rketd_sim *s, double *out, double *chh_m) {
+  if (!s || !out) return fail(s, RKETD_EINVAL, "rketd_get_coefficients: NULL argument");
+  if (!s->have_media) return fail(s, RKETD_ESTATE, "rketd_get_coefficients before rketd_set_media");
+  const size_t n = (size_t)6 * s->L.ncells * s->L.nbatch * sizeof(double);
+  void *tmp = nullptr;
+  CU_TRY(s, cudaMalloc(&tmp, n));
+  cudaError_t e = launch_unpack_coefficients(s->dtype, s->L, s->coef, (double *)tmp, s->stream);
+  ++s->ctr_launches;
+  if (e == cudaSuccess) e = cudaMemcpyAsync(out, tmp, n, cudaMemcpyDefault, s->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+  cudaFree(tmp);
+  CU_TRY(s, e);
+  if (chh_m) {
+    chh_m[0] = s->dt / (kMu0 * s->dz);
+    const double S = kC0 * s->dt / s->dz;
+    chh_m[1] = (S - 1.0) / (S + 1.0);
+  }
+  return RKETD_OK;
+}
+
+int64_t rketd_get_counter(const rketd_sim *s, int which) {
+  if (!s) return -1;
+  switch (which) {
+    case RKETD_CTR_LAUNCHES: return s->ctr_launches;
+    case RKETD_CTR_STEP_LAUNCHES: return s->ctr_step_launches;
+    case RKETD_CTR_KERNEL_USED: return s->ctr_kernel_used;
+    case RKETD_CTR_DEPTH_USED: return s->ctr_depth_used;
+    case RKETD_CTR_STEPS_DONE: return s->step;
+    case RKETD_CTR_TILE_CELLS: return s->ctr_tile_cells;
+    case RKETD_CTR_HALO_CELLS: return s->ctr_halo_cells;
+    case RKETD_CTR_STATE_BYTES: return s->state_bytes;
+  }
+  return -1;
+}
+
+void rketd_destroy(rketd_sim *s) {
+  if (!s) return;
+  cudaStreamSynchronize(s->stream);
+  for (int b = 0; b < 2; ++b)
+    for (int a = 0; a < 3; ++a)
+      if (s->fld[b][a]) cudaFree(s->fld[b][a]);
+  for (int a = 0; a < 6; ++a)
+    if (s->coef[a]) cudaFree(s->coef[a]);
+  if (s->rowflag) cudaFree(s->rowflag);
+  if (s->d_bad) cudaFree(s->d_bad);
+  if (s->d_srctab) cudaFree(s->d_srctab);
+  for (auto &c : s->chunks) cudaFree(c.buf);
+  if (s->dft_re) cudaFree(s->dft_re);
+  if (s->dft_im) cudaFree(s->dft_im);
+  if (s->d_freqs) cudaFree(s->d_freqs);
+  cudaGetLastError();
+  delete s;
+}
+
+const char *rketd_last_error(const rketd_sim *s) { return s ? s->err.c_str() : g_create_error.c_str(); }
+
+}  // extern "C"

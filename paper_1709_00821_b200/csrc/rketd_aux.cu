@@ -1,0 +1,196 @@
+// rketd_aux.cu — setup and post-processing kernels of librketd:
+//   coefficient precompute (eqs. (11), (13) PAPER.md:68, :79),
+//   coefficient read-back, DFT twiddles / accumulation / magnitude (row a7, BASELINE config 5).
+#include <math_constants.h>
+
+#include "rketd_internal.h"
+
+namespace rketd {
+
+const double kC0 = 299792458.0;
+static const double kPiH = 3.14159265358979323846;
+const double kMu0 = 4.0 * kPiH * 1e-7;
+const double kEps0 = 1.0 / (kMu0 * kC0 * kC0);
+
+// ---------------------------------------------------------------------------- a0
+// phi1(x) = (1 - e^-x)/x and phi2(x) = (e^-x - 1 + x)/x^2 are the two brackets of eq. (11)
+// divided by dt; the printed forms are 0/0 at nu = 0 and lose all digits for
+// small nu dt, so: expm1 for phi1, Taylor series for phi2 when |x| < 1/2.
+// Explicit round-to-nearest intrinsics keep the compiler from fusing or reassociating.
+__device__ __forceinline__ void phi_functions(double x, double &p1, double &p2) {
+  p1 = (x == 0.0) ? 1.0 : __ddiv_rn(-expm1(-x), x);
+  if (fabs(x) < 0.5) {
+    double term = 0.5, sum = 0.5;
+    for (int j = 1; j <= 40; ++j) {
+      term = __ddiv_rn(__dmul_rn(term, -x), (double)(j + 2));
+      const double next = __dadd_rn(sum, term);
+      if (next == sum) break;
+      sum = next;
+    }
+    p2 = sum;
+  } else {
+    p2 = __ddiv_rn(__dadd_rn(expm1(-x), x), __dmul_rn(x, x));
+  }
+}
+
+template <typename R>
+__global__ void coefficients_kernel(Layout L, const double *__restrict__ wp, const double *__restrict__ nu,
+                                    double dz, double dt, double eps0, R *ca, R *cj, R *ch, R *ka, R *kb, R *kc,
+                                    int *bad) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= L.gstride * L.nbatch) return;
+  const int64_t g = idx / L.gstride, kp = idx - g * L.gstride, k = kp - L.off;
+  double vca = 0, vcj = 0, vch = 0, vka = 0, vkb = 0, vkc = 0;     // padding nodes: all zero
+  if (k >= 0 && k < L.ncells) {
+    const double w = wp[g * L.ncells + k], v = nu[g * L.ncells + k];
+    if (!(w >= 0.0) || !(v >= 0.0) || isinf(w) || isinf(v)) atomicOr(bad, 1);
+    const double x = __dmul_rn(v, dt);
+    const double a = exp(-x);
+    double p1, p2;
+    phi_functions(x, p1, p2);
+    const double beta = __dmul_rn(dt, p1);              // (1 - a)/nu
+    const double gamma = __dmul_rn(dt, p2);             // (a - 1 + nu dt)/(nu^2 dt)
+    const double w2 = __dmul_rn(w, w);
+    const double b = __dmul_rn(__dmul_rn(eps0, w2), beta);
+    const double c = __dmul_rn(__dmul_rn(eps0, w2), gamma);
+    const double D = __dadd_rn(1.0, __ddiv_rn(__dmul_rn(__dmul_rn(w2, gamma), dt), 2.0));
+    vca = __dsub_rn(1.0, __ddiv_rn(__ddiv_rn(__dmul_rn(__dmul_rn(w2, beta), dt), 2.0), D));
+    vcj = __ddiv_rn(__dmul_rn(__ddiv_rn(dt, __dmul_rn(2.0, eps0)), __dadd_rn(1.0, a)), D);
+    vch = __ddiv_rn(__ddiv_rn(dt, __dmul_rn(eps0, dz)), D);
+    vka = a;
+    vkb = __dsub_rn(b, c);
+    vkc = c;
+  }
+  ca[idx] = (R)vca; cj[idx] = (R)vcj; ch[idx] = (R)vch;
+  ka[idx] = (R)vka; kb[idx] = (R)vkb; kc[idx] = (R)vkc;
+}
+
+cudaError_t launch_coefficients(int dtype, const Layout &L, const double *wp, const double *nu, double dz,
+                                double dt, void *const coef[6], int *d_bad, cudaStream_t st) {
+  const int64_t total = L.gstride * L.nbatch;
+  const unsigned blocks = (unsigned)((total + 255) / 256);
+  if (dtype == 0)
+    coefficients_kernel<double><<<blocks, 256, 0, st>>>(L, wp, nu, dz, dt, kEps0, (double *)coef[0], (double *)coef[1],
+                                                        (double *)coef[2], (double *)coef[3], (double *)coef[4],
+                                                        (double *)coef[5], d_bad);
+  else
+    coefficients_kernel<float><<<blocks, 256, 0, st>>>(L, wp, nu, dz, dt, kEps0, (float *)coef[0], (float *)coef[1],
+                                                       (float *)coef[2], (float *)coef[3], (float *)coef[4],
+                                                       (float *)coef[5], d_bad);
+  return cudaGetLastError();
+}
+
+template <typename R>
+__global__ void unpack_coefficients_kernel(Layout L, const R *c0, const R *c1, const R *c2, const R *c3, const R *c4,
+                                           const R *c5, double *out) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t n = L.ncells * L.nbatch;
+  if (idx >= n) return;
+  const int64_t g = idx / L.ncells, k = idx - g * L.ncells, src = g * L.gstride + L.off + k;
+  out[0 * n + idx] = (double)c0[src]; out[1 * n + idx] = (double)c1[src]; out[2 * n + idx] = (double)c2[src];
+  out[3 * n + idx] = (double)c3[src]; out[4 * n + idx] = (double)c4[src]; out[5 * n + idx] = (double)c5[src];
+}
+cudaError_t launch_unpack_coefficients(int dtype, const Layout &L, void *const c[6], double *out, cudaStream_t st) {
+  const int64_t n = L.ncells * L.nbatch;
+  const unsigned blocks = (unsigned)((n + 255) / 256);
+  if (dtype == 0)
+    unpack_coefficients_kernel<double><<<blocks, 256, 0, st>>>(L, (double *)c[0], (double *)c[1], (double *)c[2],
+                                                               (double *)c[3], (double *)c[4], (double *)c[5], out);
+  else
+    unpack_coefficients_kernel<float><<<blocks, 256, 0, st>>>(L, (float *)c[0], (float *)c[1], (float *)c[2],
+                                                              (float *)c[3], (float *)c[4], (float *)c[5], out);
+  return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------- a7
+// tw[n][m] = (cos theta, sin theta), theta = 2 pi f_m ((step0 + n + 1) dt), evaluated directly
+// (no phasor recurrence).
+__global__ void twiddle_kernel(const double *__restrict__ freqs, int nfreq, int64_t step0, int64_t nsteps, double dt,
+                               double2 *tw) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= nsteps * nfreq) return;
+  const int64_t n = idx / nfreq;
+  const int m = (int)(idx - n * nfreq);
+  const double t = __dmul_rn((double)(step0 + n + 1), dt);
+  const double theta = __dmul_rn(__dmul_rn(__dmul_rn(2.0, CUDART_PI), freqs[m]), t);
+  double s, c;
+  sincos(theta, &s, &c);
+  tw[idx] = make_double2(c, s);
+}
+cudaError_t launch_twiddles(const double *d_freqs, int nfreq, int64_t step0, int64_t nsteps, double dt, double2 *tw,
+                            cudaStream_t st) {
+  const int64_t n = nsteps * nfreq;
+  twiddle_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(d_freqs, nfreq, step0, nsteps, dt, tw);
+  return cudaGetLastError();
+}
+
+// X[s][m] += sum_n rec[s][n] (cos - j sin)(theta[n][m]).  Block: 32 series x 64 frequencies;
+// thread (m, q) owns 8 series; record tiles of 32 steps are staged through shared memory.
+template <typename R>
+__global__ void __launch_bounds__(256) dft_accumulate_kernel(const R *__restrict__ rec, int64_t nseries, int64_t nsteps,
+                                                             const double2 *__restrict__ tw, int nfreq, double *re,
+                                                             double *im) {
+  constexpr int SB = 32, TN = 32, SPT = 8;
+  __shared__ double srec[SB][TN + 1];
+  const int tid = threadIdx.x;
+  const int m = blockIdx.y * 64 + (tid & 63);
+  const int q = tid >> 6;
+  const int64_t s0 = (int64_t)blockIdx.x * SB;
+  double are[SPT], aim[SPT];
+#pragma unroll
+  for (int i = 0; i < SPT; ++i) { are[i] = 0.0; aim[i] = 0.0; }
+  for (int64_t n0 = 0; n0 < nsteps; n0 += TN) {
+    __syncthreads();
+    for (int e = tid; e < SB * TN; e += 256) {
+      const int s = e / TN, nn = e % TN;
+      const int64_t ser = s0 + s, n = n0 + nn;
+      srec[s][nn] = (ser < nseries && n < nsteps) ? (double)rec[ser * nsteps + n] : 0.0;
+    }
+    __syncthreads();
+    if (m < nfreq) {
+      const int lim = (int)((nsteps - n0) < TN ? (nsteps - n0) : TN);
+      for (int nn = 0; nn < lim; ++nn) {
+        const double2 w = tw[(n0 + nn) * nfreq + m];
+#pragma unroll
+        for (int i = 0; i < SPT; ++i) {
+          const double v = srec[q * SPT + i][nn];
+          are[i] = fma(v, w.x, are[i]);
+          aim[i] = fma(-v, w.y, aim[i]);
+        }
+      }
+    }
+  }
+  if (m < nfreq) {
+#pragma unroll
+    for (int i = 0; i < SPT; ++i) {
+      const int64_t ser = s0 + q * SPT + i;
+      if (ser < nseries) {
+        re[ser * nfreq + m] += are[i];
+        im[ser * nfreq + m] += aim[i];
+      }
+    }
+  }
+}
+cudaError_t launch_dft_accumulate(int dtype, const void *rec, int64_t nseries, int64_t nsteps, const double2 *tw,
+                                  int nfreq, double *re, double *im, cudaStream_t st) {
+  dim3 grid((unsigned)((nseries + 31) / 32), (unsigned)((nfreq + 63) / 64));
+  if (dtype == 0)
+    dft_accumulate_kernel<double><<<grid, 256, 0, st>>>((const double *)rec, nseries, nsteps, tw, nfreq, re, im);
+  else
+    dft_accumulate_kernel<float><<<grid, 256, 0, st>>>((const float *)rec, nseries, nsteps, tw, nfreq, re, im);
+  return cudaGetLastError();
+}
+
+template <typename R>
+__global__ void dft_magnitude_kernel(const double *re, const double *im, int64_t n, R *out) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx < n) out[idx] = (R)hypot(re[idx], im[idx]);
+}
+cudaError_t launch_dft_magnitude(int dtype, const double *re, const double *im, int64_t n, void *out, cudaStream_t st) {
+  const unsigned blocks = (unsigned)((n + 255) / 256);
+  if (dtype == 0) dft_magnitude_kernel<double><<<blocks, 256, 0, st>>>(re, im, n, (double *)out);
+  else dft_magnitude_kernel<float><<<blocks, 256, 0, st>>>(re, im, n, (float *)out);
+  return cudaGetLastError();
+}
+
+}  // namespace rketd

@@ -1,0 +1,83 @@
+// rketd_internal.h — host-side types shared by the API (rketd_api.cu) and the kernel
+// launchers (rketd_kernels.cu, rketd_aux.cu).  Not part of the public boundary.
+#pragma once
+#include <cuda.h>            // CUtensorMap type only; libcuda is reached through cudaGetDriverEntryPoint
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace rketd {
+
+// HBM layout of every per-node array (fields E, H, J x2 for ping-pong; six coefficient arrays):
+//   [nbatch][nrows][C] with rows of 64 B (C = 8 fp64 / 16 fp32 nodes) — one row is what one thread
+//   owns in registers.  Node k of grid g sits at physical in-grid index off + k.  off is 0, or 1
+//   when (ncells-1) % C == 0, so that nodes {0,1} share a row and nodes {ncells-2, ncells-1}
+//   share a row (Mur needs both in one thread).  Padding nodes carry zero fields and zero
+//   coefficients and never influence real nodes (they sit behind the Mur nodes).
+struct Layout {
+  int64_t ncells = 0, nbatch = 0;
+  int esize = 8;       // bytes per value
+  int C = 8;           // nodes per row
+  int off = 0;         // physical index of node 0
+  int64_t nrows = 0;   // rows per grid
+  int64_t gstride = 0; // physical nodes per grid = nrows * C
+};
+
+struct FieldPtrs { void *E, *H, *J; };
+
+// dtype-agnostic description of what a step needs (converted to StepParams<R> by the launchers)
+struct StepCommon {
+  double nchh, mur_m;
+  int64_t cellL, cellR, cellS;
+  int nprobes;
+  int64_t rec_stride, n0;
+  const void *src_tab;
+  void *rec;
+  const uint8_t *rowflag;
+  int64_t probe_cell[64];
+};
+
+// K2 (temporal blocking) plan: tiling + the TMA descriptors for one ping-pong direction.
+struct K2Maps {
+  CUtensorMap ld[9];   // E, H, J (source buffers), ca, cj, ch, ka, kb, kc : box {C, NT, 1}, SWIZZLE_64B
+  CUtensorMap st[3];   // E, H, J (destination buffers)                  : box {C, rows_out, 1}
+};
+struct K2Plan {
+  int NT = 0;              // threads per CTA = rows per tile (halo included)
+  int HR = 0;              // halo rows on each side (HR * C >= T)
+  int rows_out = 0;        // NT - 2 HR
+  int depth = 0;           // T, steps per pass
+  int64_t tiles_per_grid = 0, total_tiles = 0;
+  int grid = 0;            // CTAs launched (persistent)
+  int ctas_per_sm = 0;
+  size_t smem_bytes = 0;
+  K2Maps maps[2];          // maps[s]: read buffer s, write buffer 1-s
+};
+
+int k2_threads_options(int idx);   // NT variants compiled in: 128, 256
+int k3_threads_for_rows(int dtype, int64_t nrows);   // smallest compiled NT >= nrows, or 0
+size_t k2_smem_bytes(int NT);
+size_t k3_smem_bytes(int dtype, int NT);
+
+cudaError_t launch_k1(int dtype, const Layout &L, FieldPtrs src, FieldPtrs dst, void *const coef[6],
+                      const StepCommon &sc, cudaStream_t st);
+cudaError_t launch_k2(int dtype, const Layout &L, const K2Plan &plan, int src_buf, const StepCommon &sc,
+                      int steps, cudaStream_t st);
+cudaError_t launch_k3(int dtype, const Layout &L, FieldPtrs fld, void *const coef[6], const StepCommon &sc,
+                      int64_t nsteps, int NT, cudaStream_t st);
+cudaError_t k2_configure(int dtype, int NT, int *ctas_per_sm);   // sets smem attribute, returns occupancy
+
+// auxiliary kernels (rketd_aux.cu)
+cudaError_t launch_coefficients(int dtype, const Layout &L, const double *wp, const double *nu, double dz,
+                                double dt, void *const coef[6], int *d_bad, cudaStream_t st);
+cudaError_t launch_unpack_coefficients(int dtype, const Layout &L, void *const coef[6], double *out,
+                                       cudaStream_t st);
+cudaError_t launch_twiddles(const double *d_freqs, int nfreq, int64_t step0, int64_t nsteps, double dt,
+                            double2 *tw, cudaStream_t st);
+cudaError_t launch_dft_accumulate(int dtype, const void *rec, int64_t nseries, int64_t nsteps, const double2 *tw,
+                                  int nfreq, double *re, double *im, cudaStream_t st);
+cudaError_t launch_dft_magnitude(int dtype, const double *re, const double *im, int64_t n, void *out,
+                                 cudaStream_t st);
+
+extern const double kC0, kMu0, kEps0;
+
+}  // namespace rketd
