@@ -45,7 +45,7 @@ struct rketd_sim {
   std::vector<Chunk> chunks;
   int64_t nsamples = 0;
   int64_t step = 0;
-  int plan_kernel = RKETD_KERNEL_AUTO, plan_depth = 0;
+  int plan_kernel = RKETD_KERNEL_AUTO, plan_depth = 0, plan_variant = -1;
   K2Plan k2;
   bool k2_valid = false;
   int64_t ctr_launches = 0, ctr_step_launches = 0, ctr_kernel_used = 0, ctr_depth_used = 0, ctr_tile_cells = 0,
@@ -167,20 +167,23 @@ int make_map(rketd_sim *s, CUtensorMap *m, void *base, int box_rows) {
 }
 
 int default_depth(const rketd_sim *s) { return s->dtype == RKETD_F64 ? 24 : 32; }
-int default_k2_threads(const rketd_sim *) { return 128; }
+int default_k2_variant(const rketd_sim *) { return 0; }
+int default_k3_variant(const rketd_sim *) { return 0; }
+int max_depth(const rketd_sim *s, int variant) { return (k2_tile_rows(variant) / 2 - 1) * s->L.C; }
 
-int build_k2_plan(rketd_sim *s, int depth, int NT) {
+int build_k2_plan(rketd_sim *s, int depth, int variant) {
   const Layout &L = s->L;
   K2Plan &P = s->k2;
-  if (s->k2_valid && P.depth == depth && P.NT == NT) return RKETD_OK;
+  if (s->k2_valid && P.depth == depth && P.variant == variant) return RKETD_OK;
+  const int rows = k2_tile_rows(variant);
   const int HR = (depth + L.C - 1) / L.C;
-  if (NT - 2 * HR < 1) return fail(s, RKETD_EINVAL, "temporal depth too large for the tile");
-  P.NT = NT; P.HR = HR; P.rows_out = NT - 2 * HR; P.depth = depth;
+  if (rows - 2 * HR < 1) return fail(s, RKETD_EINVAL, "temporal depth too large for the tile");
+  P.variant = variant; P.rows = rows; P.HR = HR; P.rows_out = rows - 2 * HR; P.depth = depth;
   P.tiles_per_grid = (L.nrows + P.rows_out - 1) / P.rows_out;
   P.total_tiles = P.tiles_per_grid * L.nbatch;
-  P.smem_bytes = k2_smem_bytes(NT);
+  P.smem_bytes = k2_smem_bytes(variant);
   int ctas = 0, dev = 0, sms = 0;
-  CU_TRY(s, k2_configure(s->dtype, NT, &ctas));
+  CU_TRY(s, k2_configure(s->dtype, variant, &ctas));
   if (ctas < 1) return fail(s, RKETD_ECUDA, "K2 kernel does not fit on an SM");
   CU_TRY(s, cudaGetDevice(&dev));
   CU_TRY(s, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
@@ -188,13 +191,13 @@ int build_k2_plan(rketd_sim *s, int depth, int NT) {
   P.grid = (int)std::min<int64_t>(P.total_tiles, (int64_t)sms * ctas);
   for (int b = 0; b < 2; ++b) {
     for (int a = 0; a < 3; ++a) {
-      int rc = make_map(s, &P.maps[b].ld[a], s->fld[b][a], NT);
+      int rc = make_map(s, &P.maps[b].ld[a], s->fld[b][a], rows);
       if (rc) return rc;
       rc = make_map(s, &P.maps[b].st[a], s->fld[1 - b][a], P.rows_out);
       if (rc) return rc;
     }
     for (int a = 0; a < 6; ++a) {
-      int rc = make_map(s, &P.maps[b].ld[3 + a], s->coef[a], NT);
+      int rc = make_map(s, &P.maps[b].ld[3 + a], s->coef[a], rows);
       if (rc) return rc;
     }
   }
@@ -204,7 +207,7 @@ int build_k2_plan(rketd_sim *s, int depth, int NT) {
 
 int resolve_kernel(rketd_sim *s) {
   if (s->plan_kernel != RKETD_KERNEL_AUTO) return s->plan_kernel;
-  return k3_threads_for_rows(s->dtype, s->L.nrows) ? RKETD_KERNEL_RESIDENT : RKETD_KERNEL_TBLOCK;
+  return k3_threads_for_rows(s->dtype, s->L.nrows, 0) ? RKETD_KERNEL_RESIDENT : RKETD_KERNEL_TBLOCK;
 }
 
 // run nsteps steps whose probe samples go to rec ([nbatch][nprobes][nsteps] or nullptr)
@@ -254,17 +257,19 @@ int run_segment(rketd_sim *s, int64_t nsteps, void *rec) {
     }
     s->ctr_tile_cells = L.C; s->ctr_halo_cells = 1; s->ctr_depth_used = 1;
   } else if (kern == RKETD_KERNEL_RESIDENT) {
-    const int NT = k3_threads_for_rows(s->dtype, L.nrows);
+    int variant = s->plan_variant >= 0 ? s->plan_variant : default_k3_variant(s);
+    if (!k3_threads_for_rows(s->dtype, L.nrows, variant)) variant = 0;
+    const int NT = k3_threads_for_rows(s->dtype, L.nrows, variant);
     if (!NT) return fail(s, RKETD_EINVAL, "grid too large for the resident kernel");
     FieldPtrs f{s->fld[s->cur][0], s->fld[s->cur][1], s->fld[s->cur][2]};
-    CU_TRY(s, launch_k3(s->dtype, L, f, s->coef, sc, nsteps, NT, s->stream));
+    CU_TRY(s, launch_k3(s->dtype, L, f, s->coef, sc, nsteps, NT, variant, s->stream));
     ++s->ctr_launches; ++s->ctr_step_launches;
-    s->ctr_tile_cells = (int64_t)NT * L.C; s->ctr_halo_cells = 0; s->ctr_depth_used = nsteps;
+    s->ctr_tile_cells = L.gstride; s->ctr_halo_cells = 0; s->ctr_depth_used = nsteps;
   } else {
-    const int NT = default_k2_threads(s);
+    const int variant = s->plan_variant >= 0 ? s->plan_variant : default_k2_variant(s);
     int depth = s->plan_depth > 0 ? s->plan_depth : default_depth(s);
-    depth = std::min<int>(depth, (NT / 2 - 1) * L.C);
-    int rc = build_k2_plan(s, depth, NT);
+    depth = std::min<int>(depth, max_depth(s, variant));
+    int rc = build_k2_plan(s, depth, variant);
     if (rc) return rc;
     for (int64_t n = 0; n < nsteps; n += depth) {
       const int steps = (int)std::min<int64_t>(depth, nsteps - n);
@@ -273,7 +278,7 @@ int run_segment(rketd_sim *s, int64_t nsteps, void *rec) {
       s->cur ^= 1;
       ++s->ctr_launches; ++s->ctr_step_launches;
     }
-    s->ctr_tile_cells = (int64_t)NT * L.C; s->ctr_halo_cells = (int64_t)s->k2.HR * L.C; s->ctr_depth_used = depth;
+    s->ctr_tile_cells = (int64_t)s->k2.rows * L.C; s->ctr_halo_cells = (int64_t)s->k2.HR * L.C; s->ctr_depth_used = depth;
   }
   s->step += nsteps;
   return RKETD_OK;
@@ -299,7 +304,7 @@ int rketd_create(rketd_sim **out, int64_t ncells, int64_t nbatch, double dz, dou
   L.ncells = ncells; L.nbatch = nbatch;
   L.esize = dtype == RKETD_F64 ? 8 : 4;
   L.C = kRowBytes / L.esize;
-  L.off = ((ncells - 1) % L.C == 0) ? 1 : 0;
+  L.off = ((ncells - 1) % (L.C / 2) == 0) ? 1 : 0;
   L.nrows = (L.off + ncells + L.C - 1) / L.C;
   L.gstride = L.nrows * L.C;
   if (L.nrows > 0x7fffff00LL || nbatch > 0x7fffff00LL) { delete s; return fail(nullptr, RKETD_EINVAL, "grid too large"); }
@@ -419,14 +424,19 @@ int rketd_reset(rketd_sim *s) {
   return RKETD_OK;
 }
 
-int rketd_set_plan(rketd_sim *s, int kernel, int depth) {
+int rketd_set_plan(rketd_sim *s, int kernel, int depth, int variant) {
   if (!s) return RKETD_EINVAL;
   if (kernel < RKETD_KERNEL_AUTO || kernel > RKETD_KERNEL_RESIDENT || depth < 0) return fail(s, RKETD_EINVAL, "rketd_set_plan: bad argument");
-  if (kernel == RKETD_KERNEL_RESIDENT && !k3_threads_for_rows(s->dtype, s->L.nrows))
+  if (kernel == RKETD_KERNEL_RESIDENT && !k3_threads_for_rows(s->dtype, s->L.nrows, variant < 0 ? 0 : variant))
     return fail(s, RKETD_EINVAL, "rketd_set_plan: grid does not fit the resident kernel");
-  if (depth > (default_k2_threads(s) / 2 - 1) * s->L.C) return fail(s, RKETD_EINVAL, "rketd_set_plan: depth too large");
+  if (kernel == RKETD_KERNEL_TBLOCK || kernel == RKETD_KERNEL_AUTO) {
+    if (variant >= 0 && kernel == RKETD_KERNEL_TBLOCK && !k2_tile_rows(variant)) return fail(s, RKETD_EINVAL, "rketd_set_plan: unknown variant");
+    const int v = (variant >= 0 && k2_tile_rows(variant)) ? variant : default_k2_variant(s);
+    if (depth > max_depth(s, v)) return fail(s, RKETD_EINVAL, "rketd_set_plan: depth too large");
+  }
   s->plan_kernel = kernel;
   s->plan_depth = depth;
+  s->plan_variant = variant;
   return RKETD_OK;
 }
 

@@ -53,27 +53,53 @@ struct StepParams {
   int64_t probe_cell[kMaxProbes];
 };
 
-// Unpack / pack a 64-B row between C scalars and 16-B vectors.
-template <typename R, int C>
-__device__ __forceinline__ void vec_to_regs(const typename Arith<R>::Vec &v, R (&r)[C], int j);
-template <>
-__device__ __forceinline__ void vec_to_regs<double, 8>(const double2 &v, double (&r)[8], int j) {
-  r[2 * j] = v.x; r[2 * j + 1] = v.y;
-}
-template <>
-__device__ __forceinline__ void vec_to_regs<float, 16>(const float4 &v, float (&r)[16], int j) {
-  r[4 * j] = v.x; r[4 * j + 1] = v.y; r[4 * j + 2] = v.z; r[4 * j + 3] = v.w;
-}
-__device__ __forceinline__ double2 regs_to_vec(const double (&r)[8], int j) { return make_double2(r[2 * j], r[2 * j + 1]); }
-__device__ __forceinline__ float4 regs_to_vec(const float (&r)[16], int j) {
-  return make_float4(r[4 * j], r[4 * j + 1], r[4 * j + 2], r[4 * j + 3]);
-}
-
+// 16-B vector <-> scalars
 __device__ __forceinline__ void vec_unpack(const double2 &v, double (&o)[2]) { o[0] = v.x; o[1] = v.y; }
 __device__ __forceinline__ void vec_unpack(const float4 &v, float (&o)[4]) { o[0] = v.x; o[1] = v.y; o[2] = v.z; o[3] = v.w; }
+__device__ __forceinline__ double2 vec_pack(const double (&o)[2]) { return make_double2(o[0], o[1]); }
+__device__ __forceinline__ float4 vec_pack(const float (&o)[4]) { return make_float4(o[0], o[1], o[2], o[3]); }
 
-// Coefficients of one row held in registers.  chunk<a>(j, out) hands out the V = 16/sizeof(R)
-// values of array a (0..5 = ca, cj, ch, ka, kb, kc) for nodes j*V .. j*V+V-1 of the row.
+// chunk j (16 B) of a thread's C values
+template <typename R, int C>
+__device__ __forceinline__ void vec_to_regs(const typename Arith<R>::Vec &v, R (&r)[C], int j) {
+  constexpr int V = 16 / sizeof(R);
+  R o[V];
+  vec_unpack(v, o);
+#pragma unroll
+  for (int u = 0; u < V; ++u) r[j * V + u] = o[u];
+}
+template <typename R, int C>
+__device__ __forceinline__ typename Arith<R>::Vec regs_to_vec(const R (&r)[C], int j) {
+  constexpr int V = 16 / sizeof(R);
+  R o[V];
+#pragma unroll
+  for (int u = 0; u < V; ++u) o[u] = r[j * V + u];
+  return vec_pack(o);
+}
+
+// keep a loop-invariant value in a register (stops the compiler from re-reading the constant
+// bank inside the time loop, where the load latency would sit on the critical path)
+__device__ __forceinline__ void pin_register(double &x) { asm volatile("" : "+d"(x)); }
+__device__ __forceinline__ void pin_register(float &x) { asm volatile("" : "+f"(x)); }
+
+// Geometry of the register tiling: a thread owns C consecutive nodes (32 or 64 B) of every
+// array; a 64-B row of the HBM layout is shared by TPR = 1 or 2 threads.
+template <typename R, int C>
+struct Geom {
+  static constexpr int V = 16 / sizeof(R);          // nodes per 16-B chunk
+  static constexpr int NCH = C / V;                 // chunks per thread
+  static constexpr int CR = kRowBytes / sizeof(R);  // nodes per row
+  static constexpr int TPR = CR / C;                // threads per row
+  static_assert(C % V == 0 && CR % C == 0 && (TPR == 1 || TPR == 2), "bad cells per thread");
+};
+
+// Swizzled shared-memory address of chunk j (0..3) of row `row` in an array of 64-B rows whose base
+// is 512-B aligned: CU_TENSOR_MAP_SWIZZLE_64B = XOR of address bits [4:5] with bits [7:8].  With it
+// a warp's 128-bit accesses (thread stride 32 or 64 B) cover all 32 banks.
+__device__ __forceinline__ uint32_t swz_off(int row, int j) { return row * kRowBytes + ((j ^ ((row >> 1) & 3)) << 4); }
+
+// Coefficients of a thread's nodes held in registers.  chunk<a>(j, out) hands out the V values of
+// array a (0..5 = ca, cj, ch, ka, kb, kc) for the thread's nodes j*V .. j*V+V-1.
 template <typename R, int C>
 struct CoefRegs {
   static constexpr int V = 16 / sizeof(R);
@@ -85,70 +111,86 @@ struct CoefRegs {
   }
 };
 
-// Coefficients of one row held in shared memory: six arrays of NT 64-B rows; the 16-B chunks
-// of a row are XOR-swizzled with (row>>1)&3 so that a warp's 128-bit accesses cover all banks.
-template <typename R, int C, int NT>
+// Coefficients held in shared memory: six arrays of ROWS swizzled 64-B rows.
+template <typename R, int C, int ROWS>
 struct CoefSmem {
   static constexpr int V = 16 / sizeof(R);
-  const uint8_t *chunk_ptr[C / V];     // address of chunk j of this thread's row in array 0
-  __device__ __forceinline__ void init(const uint8_t *array0, int row) {
-    const uint32_t sw = (row >> 1) & 3;
+  const uint8_t *chunk_ptr[C / V];     // address of the thread's chunk j in array 0
+  __device__ __forceinline__ void init(const uint8_t *array0, int tid) {
+    const int row = tid / Geom<R, C>::TPR, sub = tid % Geom<R, C>::TPR;
 #pragma unroll
-    for (int j = 0; j < C / V; ++j) chunk_ptr[j] = array0 + row * kRowBytes + ((j ^ sw) << 4);
+    for (int j = 0; j < C / V; ++j) chunk_ptr[j] = array0 + swz_off(row, sub * (C / V) + j);
   }
   template <int a>
   __device__ __forceinline__ void chunk(int j, R (&out)[V]) const {
     typedef typename Arith<R>::Vec Vec;
-    vec_unpack(*reinterpret_cast<const Vec *>(chunk_ptr[j] + a * (NT * kRowBytes)), out);
+    vec_unpack(*reinterpret_cast<const Vec *>(chunk_ptr[j] + a * (ROWS * kRowBytes)), out);
   }
   template <int a>
   __device__ __forceinline__ void store_chunk(int j, const typename Arith<R>::Vec &v) const {
     typedef typename Arith<R>::Vec Vec;
-    *reinterpret_cast<Vec *>(const_cast<uint8_t *>(chunk_ptr[j]) + a * (NT * kRowBytes)) = v;
+    *reinterpret_cast<Vec *>(const_cast<uint8_t *>(chunk_ptr[j]) + a * (ROWS * kRowBytes)) = v;
   }
 };
 
-// One leapfrog step of one row.  El, Hl: E and H (both OLD) of the node left of the row;
-// Er: old E of the node right of the row.  k0: physical in-grid index of the row's first
-// node; g: grid; nloc: local step index; owner: this thread records probes in its row.
+// ---- one leapfrog step of a thread's C nodes, in two phases so that the halo values the
+// neighbours need for the NEXT step can be sent between them.
+//
+// Phase 1: H' (a1), E' in place (a2), Mur (a3), source (a4), probe record (a6), and the part
+// t = kb E + ka J of eq. (11) that needs the old E.  El, Hl: old E and H of the node left of the
+// thread's nodes; Er: old E of the node to the right.  k0: physical in-grid index of the first
+// node; g: grid; nloc: local step index; owner: this thread records probes among its nodes.
 template <typename R, int C, typename CF>
-__device__ __forceinline__ void leapfrog_row(R (&E)[C], R (&H)[C], R (&J)[C], const CF &cf, R El, R Hl, R Er,
-                                             const StepParams<R> &p, uint32_t flag, int64_t k0, int64_t g,
-                                             int64_t nloc, bool owner) {
+__device__ __forceinline__ void step_fields(R (&E)[C], R (&H)[C], const R (&J)[C], R (&t)[C], const CF &cf, R El, R Hl,
+                                            R Er, R nchh, const StepParams<R> &p, uint32_t flag, int64_t k0,
+                                            int64_t g, int64_t nloc, bool owner) {
   typedef Arith<R> A;
-  // a1: H update, eq. (14).  The left neighbour's new H is recomputed here from old values
-  // so that one exchange of old values per step is enough.
-  const R Hl_new = A::fma(p.nchh, A::sub(E[0], El), Hl);
-#pragma unroll
-  for (int i = 0; i < C; ++i) H[i] = A::fma(p.nchh, A::sub(i + 1 < C ? E[i + 1] : Er, E[i]), H[i]);
-  // a2: E update, eq. (12) with (11) substituted
-  R En[C];
   constexpr int V = 16 / sizeof(R);
+  // a1: H update, eq. (14).  The left neighbour's new H is recomputed here from old values so
+  // that one exchange of old values per step is enough.
+  const R Hl_new = A::fma(nchh, A::sub(E[0], El), Hl);
+#pragma unroll
+  for (int i = 0; i < C; ++i) H[i] = A::fma(nchh, A::sub(i + 1 < C ? E[i + 1] : Er, E[i]), H[i]);
+  // old E at the Mur nodes and their inner neighbours (flagged rows only)
+  R mL0 = R(0), mL1 = R(0), mR0 = R(0), mR1 = R(0);
+  if (flag & (F_MURL | F_MURR)) {
+#pragma unroll
+    for (int i = 0; i < C - 1; ++i)
+      if (k0 + i == p.cellL) { mL0 = E[i]; mL1 = E[i + 1]; }
+#pragma unroll
+    for (int i = 1; i < C; ++i)
+      if (k0 + i == p.cellR) { mR0 = E[i]; mR1 = E[i - 1]; }
+  }
+  // a2: E update, eq. (12) with (11) substituted; t = kb E + ka J (first two terms of eq. (11))
 #pragma unroll
   for (int j = 0; j < C / V; ++j) {
-    R ca[V], cj[V], ch[V];
+    R ca[V], cj[V], ch[V], ka[V], kb[V];
     cf.template chunk<0>(j, ca);
     cf.template chunk<1>(j, cj);
     cf.template chunk<2>(j, ch);
+    cf.template chunk<3>(j, ka);
+    cf.template chunk<4>(j, kb);
 #pragma unroll
     for (int u = 0; u < V; ++u) {
       const int i = j * V + u;
-      En[i] = A::fma(-ch[u], A::sub(H[i], i ? H[i - 1] : Hl_new), A::fma(-cj[u], J[i], A::mul(ca[u], E[i])));
+      const R w = A::fma(-cj[u], J[i], A::mul(ca[u], E[i]));
+      t[i] = A::fma(kb[u], E[i], A::mul(ka[u], J[i]));
+      E[i] = A::fma(-ch[u], A::sub(H[i], i ? H[i - 1] : Hl_new), w);
     }
   }
-  if (flag) {   // rows that hold a boundary node, the source node or a probe (rare)
-    if (flag & F_MURL) {   // a3, left end.  The layout guarantees node 1 is in the same row.
+  if (flag) {   // threads that hold a boundary node, the source node or a probe (rare)
+    if (flag & F_MURL) {   // a3, left end.  The layout guarantees node 1 is held by the same thread.
 #pragma unroll
       for (int i = 0; i < C - 1; ++i)
-        if (k0 + i == p.cellL) En[i] = A::fma(p.mur_m, A::sub(En[i + 1], E[i]), E[i + 1]);
+        if (k0 + i == p.cellL) E[i] = A::fma(p.mur_m, A::sub(E[i + 1], mL0), mL1);
 #pragma unroll
       for (int i = 0; i < C; ++i)
         if (k0 + i < p.cellL) H[i] = R(0);      // padding left of node 0
     }
-    if (flag & F_MURR) {   // a3, right end.  Node ncells-2 is in the same row.
+    if (flag & F_MURR) {   // a3, right end.  Node ncells-2 is held by the same thread.
 #pragma unroll
       for (int i = 1; i < C; ++i)
-        if (k0 + i == p.cellR) En[i] = A::fma(p.mur_m, A::sub(En[i - 1], E[i]), E[i - 1]);
+        if (k0 + i == p.cellR) E[i] = A::fma(p.mur_m, A::sub(E[i - 1], mR0), mR1);
 #pragma unroll
       for (int i = 0; i < C; ++i)
         if (k0 + i >= p.cellR) H[i] = R(0);     // H[ncells-1] and padding
@@ -157,64 +199,71 @@ __device__ __forceinline__ void leapfrog_row(R (&E)[C], R (&H)[C], R (&J)[C], co
       const R s = p.src_tab[nloc];
 #pragma unroll
       for (int i = 0; i < C; ++i)
-        if (k0 + i == p.cellS) En[i] = A::add(En[i], s);
+        if (k0 + i == p.cellS) E[i] = A::add(E[i], s);
     }
     if ((flag & F_PROBE) && owner && p.rec) {   // a6: probe record
       for (int q = 0; q < p.nprobes; ++q) {
         const int64_t d = p.probe_cell[q] - k0;
         if (d >= 0 && d < C) {
-          R v = En[0];
+          R v = E[0];
 #pragma unroll
           for (int i = 1; i < C; ++i)
-            if (d == i) v = En[i];
+            if (d == i) v = E[i];
           p.rec[(g * p.nprobes + q) * p.rec_stride + nloc] = v;
         }
       }
     }
   }
-  // a5: J update, eq. (11), with the final E'
+}
+
+// Phase 2 — a5: J' = kc E' + (kb E + ka J), eq. (11), with the final E'.
+template <typename R, int C, typename CF>
+__device__ __forceinline__ void step_current(R (&J)[C], const R (&E)[C], const R (&t)[C], const CF &cf) {
+  typedef Arith<R> A;
+  constexpr int V = 16 / sizeof(R);
 #pragma unroll
   for (int j = 0; j < C / V; ++j) {
-    R ka[V], kb[V], kc[V];
-    cf.template chunk<3>(j, ka);
-    cf.template chunk<4>(j, kb);
+    R kc[V];
     cf.template chunk<5>(j, kc);
 #pragma unroll
-    for (int u = 0; u < V; ++u) {
-      const int i = j * V + u;
-      J[i] = A::fma(kc[u], En[i], A::fma(kb[u], E[i], A::mul(ka[u], J[i])));
-      E[i] = En[i];
-    }
+    for (int u = 0; u < V; ++u) J[j * V + u] = A::fma(kc[u], E[j * V + u], t[j * V + u]);
   }
 }
 
-// ---- halo exchange inside a CTA: shuffles inside a warp, shared-memory slots between warps.
-// One __syncthreads per step: slots are double-buffered by step parity.
+// ---- halo exchange inside a CTA: shuffles inside a warp, shared-memory slots between warps
+// (index warp+1; slots 0 and NW+1 stay zero = the outside of the tile), double-buffered by step
+// parity so that one __syncthreads per step is enough.  send_halo is called as soon as a step's
+// E', H' exist (between the two phases); the barrier and recv_halo come after phase 2, off the
+// critical path.
 template <typename R, int NW>
 struct HaloSlots {
-  R e_first[2][NW], e_last[2][NW], h_last[2][NW];
+  R e_first[2][NW + 2], e_last[2][NW + 2], h_last[2][NW + 2];
+  __device__ __forceinline__ void clear(int tid) {
+    if (tid < 2) {
+      e_first[tid][0] = e_first[tid][NW + 1] = R(0);
+      e_last[tid][0] = e_last[tid][NW + 1] = R(0);
+      h_last[tid][0] = h_last[tid][NW + 1] = R(0);
+    }
+  }
 };
 
 template <typename R, int C, int NW>
-__device__ __forceinline__ void exchange_halo(const R (&E)[C], const R (&H)[C], HaloSlots<R, NW> &hs, int par,
-                                              int warp, int lane, R &El, R &Hl, R &Er) {
-  if (NW > 1) {
-    if (lane == 0) hs.e_first[par][warp] = E[0];
-    if (lane == 31) { hs.e_last[par][warp] = E[C - 1]; hs.h_last[par][warp] = H[C - 1]; }
-    __syncthreads();
-  }
+__device__ __forceinline__ void send_halo(const R (&E)[C], const R (&H)[C], HaloSlots<R, NW> &hs, int par, int warp,
+                                          int lane, R &El, R &Hl, R &Er) {
   El = __shfl_up_sync(0xffffffffu, E[C - 1], 1);
   Hl = __shfl_up_sync(0xffffffffu, H[C - 1], 1);
   Er = __shfl_down_sync(0xffffffffu, E[0], 1);
-  if (lane == 0) {
-    const bool has = NW > 1 && warp > 0;
-    El = has ? hs.e_last[par][has ? warp - 1 : 0] : R(0);
-    Hl = has ? hs.h_last[par][has ? warp - 1 : 0] : R(0);
-  }
-  if (lane == 31) {
-    const bool has = NW > 1 && warp < NW - 1;
-    Er = has ? hs.e_first[par][has ? warp + 1 : 0] : R(0);
-  }
+  if (lane == 0) hs.e_first[par][warp + 1] = E[0];
+  if (lane == 31) hs.e_last[par][warp + 1] = E[C - 1];
+  if (lane == 31) hs.h_last[par][warp + 1] = H[C - 1];
+}
+template <typename R, int NW>
+__device__ __forceinline__ void recv_halo(const HaloSlots<R, NW> &hs, int par, int warp, int lane, R &El, R &Hl,
+                                          R &Er) {
+  const R a = hs.e_last[par][warp], b = hs.h_last[par][warp], c = hs.e_first[par][warp + 2];
+  El = lane == 0 ? a : El;
+  Hl = lane == 0 ? b : Hl;
+  Er = lane == 31 ? c : Er;
 }
 
 // ---- PTX wrappers: shared-memory 128-bit access, mbarrier, TMA (cp.async.bulk.tensor)

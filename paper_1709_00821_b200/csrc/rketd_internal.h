@@ -9,9 +9,9 @@ namespace rketd {
 
 // HBM layout of every per-node array (fields E, H, J x2 for ping-pong; six coefficient arrays):
 //   [nbatch][nrows][C] with rows of 64 B (C = 8 fp64 / 16 fp32 nodes) — one row is what one thread
-//   owns in registers.  Node k of grid g sits at physical in-grid index off + k.  off is 0, or 1
-//   when (ncells-1) % C == 0, so that nodes {0,1} share a row and nodes {ncells-2, ncells-1}
-//   share a row (Mur needs both in one thread).  Padding nodes carry zero fields and zero
+//   (or half of what) one thread owns in registers.  Node k of grid g sits at physical in-grid
+//   index off + k.  off is 0, or 1 when (ncells-1) % (C/2) == 0, so that nodes {0,1} sit in the same
+//   half row and so do nodes {ncells-2, ncells-1} (Mur needs both in one thread).  Padding nodes carry zero fields and zero
 //   coefficients and never influence real nodes (they sit behind the Mur nodes).
 struct Layout {
   int64_t ncells = 0, nbatch = 0;
@@ -42,9 +42,10 @@ struct K2Maps {
   CUtensorMap st[3];   // E, H, J (destination buffers)                  : box {C, rows_out, 1}
 };
 struct K2Plan {
-  int NT = 0;              // threads per CTA = rows per tile (halo included)
-  int HR = 0;              // halo rows on each side (HR * C >= T)
-  int rows_out = 0;        // NT - 2 HR
+  int variant = -1;        // K2 kernel variant (see rketd_kernels.cu)
+  int rows = 0;            // rows per tile (halo included)
+  int HR = 0;              // halo rows on each side (HR * nodes-per-row >= T)
+  int rows_out = 0;        // rows - 2 HR
   int depth = 0;           // T, steps per pass
   int64_t tiles_per_grid = 0, total_tiles = 0;
   int grid = 0;            // CTAs launched (persistent)
@@ -53,18 +54,17 @@ struct K2Plan {
   K2Maps maps[2];          // maps[s]: read buffer s, write buffer 1-s
 };
 
-int k2_threads_options(int idx);   // NT variants compiled in: 128, 256
-int k3_threads_for_rows(int dtype, int64_t nrows);   // smallest compiled NT >= nrows, or 0
-size_t k2_smem_bytes(int NT);
-size_t k3_smem_bytes(int dtype, int NT);
+int k2_tile_rows(int variant);                                    // rows per tile of a K2 variant, 0 if none
+size_t k2_smem_bytes(int variant);
+int k3_threads_for_rows(int dtype, int64_t nrows, int variant);   // threads per CTA of the K3 kernel, or 0
 
 cudaError_t launch_k1(int dtype, const Layout &L, FieldPtrs src, FieldPtrs dst, void *const coef[6],
                       const StepCommon &sc, cudaStream_t st);
 cudaError_t launch_k2(int dtype, const Layout &L, const K2Plan &plan, int src_buf, const StepCommon &sc,
                       int steps, cudaStream_t st);
 cudaError_t launch_k3(int dtype, const Layout &L, FieldPtrs fld, void *const coef[6], const StepCommon &sc,
-                      int64_t nsteps, int NT, cudaStream_t st);
-cudaError_t k2_configure(int dtype, int NT, int *ctas_per_sm);   // sets smem attribute, returns occupancy
+                      int64_t nsteps, int NT, int variant, cudaStream_t st);
+cudaError_t k2_configure(int dtype, int variant, int *ctas_per_sm);   // sets smem attribute, returns occupancy
 
 // auxiliary kernels (rketd_aux.cu)
 cudaError_t launch_coefficients(int dtype, const Layout &L, const double *wp, const double *nu, double dz,

@@ -15,7 +15,7 @@
 //                    streams probe samples out; the batched variant of the north_star.
 //
 // Mur boundaries, the soft source and probe recording are folded into the rows that hold
-// those nodes (rowflag) inside the same kernels — see leapfrog_row in rketd_device.cuh.
+// those nodes (rowflag) inside the same kernels — see step_fields in rketd_device.cuh.
 #include "rketd_device.cuh"
 #include "rketd_internal.h"
 
@@ -24,21 +24,20 @@ namespace rketd {
 template <typename R> struct RowPtrs { R *E, *H, *J; };
 template <typename R> struct CoefPtrs { const R *c[6]; };
 
+// a thread's C nodes <-> global memory (first node at physical index `first`, 16-B aligned)
 template <typename R, int C>
-__device__ __forceinline__ void load_row_global(const R *base, int64_t row, R (&out)[C]) {
+__device__ __forceinline__ void load_nodes_global(const R *base, int64_t first, R (&out)[C]) {
   typedef typename Arith<R>::Vec Vec;
-  constexpr int V = 16 / sizeof(R);
-  const Vec *p = reinterpret_cast<const Vec *>(base + row * C);
+  const Vec *p = reinterpret_cast<const Vec *>(base + first);
 #pragma unroll
-  for (int j = 0; j < C / V; ++j) vec_to_regs<R, C>(p[j], out, j);
+  for (int j = 0; j < Geom<R, C>::NCH; ++j) vec_to_regs<R, C>(p[j], out, j);
 }
 template <typename R, int C>
-__device__ __forceinline__ void store_row_global(R *base, int64_t row, const R (&in)[C]) {
+__device__ __forceinline__ void store_nodes_global(R *base, int64_t first, const R (&in)[C]) {
   typedef typename Arith<R>::Vec Vec;
-  constexpr int V = 16 / sizeof(R);
-  Vec *p = reinterpret_cast<Vec *>(base + row * C);
+  Vec *p = reinterpret_cast<Vec *>(base + first);
 #pragma unroll
-  for (int j = 0; j < C / V; ++j) p[j] = regs_to_vec(in, j);
+  for (int j = 0; j < Geom<R, C>::NCH; ++j) p[j] = regs_to_vec<R, C>(in, j);
 }
 
 // ------------------------------------------------------------------------------------ K1
@@ -50,93 +49,113 @@ __global__ void __launch_bounds__(128) k1_step(RowPtrs<R> src, RowPtrs<R> dst, C
   const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (r >= total_rows) return;
   const int64_t g = r / nrows, row = r - g * nrows;
-  R E[C], H[C], J[C];
+  R E[C], H[C], J[C], t[C];
   CoefRegs<R, C> cf;
-  load_row_global<R, C>(src.E, r, E);
-  load_row_global<R, C>(src.H, r, H);
-  load_row_global<R, C>(src.J, r, J);
+  load_nodes_global<R, C>(src.E, r * C, E);
+  load_nodes_global<R, C>(src.H, r * C, H);
+  load_nodes_global<R, C>(src.J, r * C, J);
 #pragma unroll
-  for (int a = 0; a < 6; ++a) load_row_global<R, C>(cp.c[a], r, cf.c[a]);
+  for (int a = 0; a < 6; ++a) load_nodes_global<R, C>(cp.c[a], r * C, cf.c[a]);
   const R El = row > 0 ? src.E[r * C - 1] : R(0);
   const R Hl = row > 0 ? src.H[r * C - 1] : R(0);
   const R Er = row < nrows - 1 ? src.E[(r + 1) * C] : R(0);
   const uint32_t flag = p.rowflag[row];
-  leapfrog_row<R, C>(E, H, J, cf, El, Hl, Er, p, flag, row * C, g, p.n0, true);
-  store_row_global<R, C>(dst.E, r, E);
-  store_row_global<R, C>(dst.H, r, H);
-  store_row_global<R, C>(dst.J, r, J);
+  step_fields<R, C>(E, H, J, t, cf, El, Hl, Er, p.nchh, p, flag, row * C, g, p.n0, true);
+  step_current<R, C>(J, E, t, cf);
+  store_nodes_global<R, C>(dst.E, r * C, E);
+  store_nodes_global<R, C>(dst.H, r * C, H);
+  store_nodes_global<R, C>(dst.J, r * C, J);
+}
+
+// The time loop shared by K2 and K3: nsteps leapfrog steps of this thread's nodes, halos
+// exchanged inside the CTA.  One __syncthreads per step, placed after phase 2.
+template <typename R, int C, int NW, typename CF>
+__device__ __forceinline__ void time_loop(R (&E)[C], R (&H)[C], R (&J)[C], const CF &cf, HaloSlots<R, NW> &hs,
+                                          const StepParams<R> &p, uint32_t flag, int64_t k0, int64_t g, bool owner,
+                                          int64_t nsteps, int warp, int lane) {
+  R nchh = p.nchh;
+  pin_register(nchh);
+  R El, Hl, Er;
+  send_halo<R, C, NW>(E, H, hs, 0, warp, lane, El, Hl, Er);
+  __syncthreads();
+  recv_halo<R, NW>(hs, 0, warp, lane, El, Hl, Er);
+  for (int64_t s = 0; s < nsteps; ++s) {
+    R t[C];
+    step_fields<R, C>(E, H, J, t, cf, El, Hl, Er, nchh, p, flag, k0, g, p.n0 + s, owner);
+    const int par = (int)((s + 1) & 1);
+    send_halo<R, C, NW>(E, H, hs, par, warp, lane, El, Hl, Er);     // for step s+1
+    step_current<R, C>(J, E, t, cf);
+    __syncthreads();
+    recv_halo<R, NW>(hs, par, warp, lane, El, Hl, Er);
+  }
 }
 
 // ------------------------------------------------------------------------------------ K3
-template <typename R, int NT, bool CSM, int MINB>
+// One CTA per grid; NT threads x C nodes cover the grid (NT * C >= physical nodes per grid).
+template <typename R, int C, int NT, bool CSM, int MINB>
 __global__ void __launch_bounds__(NT, MINB) k3_resident(RowPtrs<R> f, CoefPtrs<R> cp,
                                                         const __grid_constant__ StepParams<R> p, int64_t nrows,
                                                         int64_t nsteps) {
-  constexpr int C = kRowBytes / sizeof(R);
-  constexpr int V = 16 / sizeof(R);
+  typedef Geom<R, C> G;
   constexpr int NW = NT / 32;
+  constexpr int ROWS = NT / G::TPR;
   typedef typename Arith<R>::Vec Vec;
   __shared__ HaloSlots<R, NW> hs;
   extern __shared__ uint8_t smem_raw[];
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int64_t g = blockIdx.x;
-  const bool valid = tid < nrows;
-  const int64_t r = g * nrows + tid;
+  const int row = tid / G::TPR;
+  const bool valid = row < nrows;
+  const int64_t k0 = (int64_t)tid * C;                       // physical in-grid index of the first node
+  const int64_t first = g * nrows * G::CR + k0;
+  hs.clear(tid);
 
   R E[C], H[C], J[C];
 #pragma unroll
   for (int i = 0; i < C; ++i) { E[i] = R(0); H[i] = R(0); J[i] = R(0); }
   if (valid) {
-    load_row_global<R, C>(f.E, r, E);
-    load_row_global<R, C>(f.H, r, H);
-    load_row_global<R, C>(f.J, r, J);
+    load_nodes_global<R, C>(f.E, first, E);
+    load_nodes_global<R, C>(f.H, first, H);
+    load_nodes_global<R, C>(f.J, first, J);
   }
-  const uint32_t flag = valid ? p.rowflag[tid] : 0u;
-  const int64_t k0 = (int64_t)tid * C;
-
-  auto time_loop = [&](const auto &cf) {
-    for (int64_t n = 0; n < nsteps; ++n) {
-      R El, Hl, Er;
-      exchange_halo<R, C, NW>(E, H, hs, (int)(n & 1), warp, lane, El, Hl, Er);
-      leapfrog_row<R, C>(E, H, J, cf, El, Hl, Er, p, flag, k0, g, p.n0 + n, true);
-    }
-  };
+  const uint32_t flag = valid ? p.rowflag[row] : 0u;
+  __syncthreads();
 
   if constexpr (CSM) {
     uint8_t *sm = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-    CoefSmem<R, C, NT> cf;
+    CoefSmem<R, C, ROWS> cf;
     cf.init(sm, tid);
-    // each thread stages its own coefficient rows (only it reads them back: no barrier needed)
+    // each thread stages its own coefficient chunks (only it reads them back: no barrier needed)
     auto stage = [&](auto ac) {
       constexpr int a = decltype(ac)::value;
 #pragma unroll
-      for (int j = 0; j < C / V; ++j) {
-        Vec v;
-        if (valid) v = reinterpret_cast<const Vec *>(cp.c[a] + r * C)[j];
-        else { R z[C] = {}; v = regs_to_vec(z, 0); }
+      for (int j = 0; j < G::NCH; ++j) {
+        R z[G::V] = {};
+        Vec v = vec_pack(z);
+        if (valid) v = reinterpret_cast<const Vec *>(cp.c[a] + first)[j];
         cf.template store_chunk<a>(j, v);
       }
     };
     stage(std::integral_constant<int, 0>{}); stage(std::integral_constant<int, 1>{});
     stage(std::integral_constant<int, 2>{}); stage(std::integral_constant<int, 3>{});
     stage(std::integral_constant<int, 4>{}); stage(std::integral_constant<int, 5>{});
-    time_loop(cf);
+    time_loop<R, C, NW>(E, H, J, cf, hs, p, flag, k0, g, true, nsteps, warp, lane);
   } else {
     CoefRegs<R, C> cf;
 #pragma unroll
     for (int a = 0; a < 6; ++a) {
 #pragma unroll
       for (int i = 0; i < C; ++i) cf.c[a][i] = R(0);
-      if (valid) load_row_global<R, C>(cp.c[a], r, cf.c[a]);
+      if (valid) load_nodes_global<R, C>(cp.c[a], first, cf.c[a]);
     }
-    time_loop(cf);
+    time_loop<R, C, NW>(E, H, J, cf, hs, p, flag, k0, g, true, nsteps, warp, lane);
   }
 
   if (valid) {
-    store_row_global<R, C>(f.E, r, E);
-    store_row_global<R, C>(f.H, r, H);
-    store_row_global<R, C>(f.J, r, J);
+    store_nodes_global<R, C>(f.E, first, E);
+    store_nodes_global<R, C>(f.H, first, H);
+    store_nodes_global<R, C>(f.J, first, J);
   }
 }
 
@@ -144,18 +163,18 @@ __global__ void __launch_bounds__(NT, MINB) k3_resident(RowPtrs<R> f, CoefPtrs<R
 struct K2Args {
   int T;                  // steps this pass
   int HR;                 // halo rows
-  int rows_out;           // NT - 2 HR
+  int rows_out;           // ROWS - 2 HR
   int64_t tiles_per_grid, total_tiles, nrows;
 };
 
-template <typename R, int NT, int MINB>
+// Persistent CTAs; tile = ROWS = NT / TPR rows of 64 B (halo of HR rows on each side included).
+template <typename R, int C, int NT, int MINB>
 __global__ void __launch_bounds__(NT, MINB) k2_tblock(const __grid_constant__ K2Maps maps,
                                                       const __grid_constant__ StepParams<R> p, K2Args q) {
-  constexpr int C = kRowBytes / sizeof(R);
-  constexpr int V = 16 / sizeof(R);
-  constexpr int NCH = C / V;
+  typedef Geom<R, C> G;
   constexpr int NW = NT / 32;
-  constexpr uint32_t kArrayBytes = NT * kRowBytes;
+  constexpr int ROWS = NT / G::TPR;
+  constexpr uint32_t kArrayBytes = ROWS * kRowBytes;
   typedef typename Arith<R>::Vec Vec;
 
   __shared__ HaloSlots<R, NW> hs;
@@ -165,6 +184,7 @@ __global__ void __launch_bounds__(NT, MINB) k2_tblock(const __grid_constant__ K2
   uint8_t *sout = sin + 9 * kArrayBytes;
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int row = tid / G::TPR, sub = tid % G::TPR;
 
   auto issue_loads = [&](int64_t tile) {   // one elected thread
     const int64_t g = tile / q.tiles_per_grid, ti = tile - g * q.tiles_per_grid;
@@ -174,6 +194,7 @@ __global__ void __launch_bounds__(NT, MINB) k2_tblock(const __grid_constant__ K2
     for (int a = 0; a < 9; ++a) tma_load_3d(sin + a * kArrayBytes, &maps.ld[a], &mbar, 0, row0, (int)g);
   };
 
+  hs.clear(tid);
   if (tid == 0) {
     mbar_init(&mbar, 1);
     fence_barrier_init();
@@ -183,32 +204,33 @@ __global__ void __launch_bounds__(NT, MINB) k2_tblock(const __grid_constant__ K2
   if (tid == 0 && tile < q.total_tiles) issue_loads(tile);
   uint32_t phase = 0;
 
-  const uint32_t sw_in = (tid >> 1) & 3;
-  const int r_out = tid - q.HR;
+  const int r_out = row - q.HR;
   const bool owner = r_out >= 0 && r_out < q.rows_out;
-  const uint32_t sw_out = (r_out >> 1) & 3;
+  uint32_t off_in[G::NCH], off_out[G::NCH];
+#pragma unroll
+  for (int j = 0; j < G::NCH; ++j) {
+    off_in[j] = swz_off(row, sub * G::NCH + j);
+    off_out[j] = swz_off(owner ? r_out : 0, sub * G::NCH + j);
+  }
 
   for (; tile < q.total_tiles; tile += gridDim.x) {
     const int64_t g = tile / q.tiles_per_grid, ti = tile - g * q.tiles_per_grid;
-    const int64_t rowg = ti * q.rows_out - q.HR + tid;     // this thread's row in the grid
+    const int64_t rowg = ti * q.rows_out - q.HR + row;     // this thread's row in the grid
 
     mbar_wait(&mbar, phase);
     phase ^= 1u;
 
     R E[C], H[C], J[C];
     CoefRegs<R, C> cf;
-    {
-      const uint8_t *my = sin + tid * kRowBytes;
 #pragma unroll
-      for (int j = 0; j < NCH; ++j) {
-        const uint32_t o = (j ^ sw_in) << 4;
-        vec_to_regs<R, C>(*reinterpret_cast<const Vec *>(my + 0 * kArrayBytes + o), E, j);
-        vec_to_regs<R, C>(*reinterpret_cast<const Vec *>(my + 1 * kArrayBytes + o), H, j);
-        vec_to_regs<R, C>(*reinterpret_cast<const Vec *>(my + 2 * kArrayBytes + o), J, j);
+    for (int j = 0; j < G::NCH; ++j) {
+      const uint8_t *my = sin + off_in[j];
+      vec_to_regs<R, C>(*reinterpret_cast<const Vec *>(my + 0 * kArrayBytes), E, j);
+      vec_to_regs<R, C>(*reinterpret_cast<const Vec *>(my + 1 * kArrayBytes), H, j);
+      vec_to_regs<R, C>(*reinterpret_cast<const Vec *>(my + 2 * kArrayBytes), J, j);
 #pragma unroll
-        for (int a = 0; a < 6; ++a)
-          vec_to_regs<R, C>(*reinterpret_cast<const Vec *>(my + (3 + a) * kArrayBytes + o), cf.c[a], j);
-      }
+      for (int a = 0; a < 6; ++a)
+        vec_to_regs<R, C>(*reinterpret_cast<const Vec *>(my + (3 + a) * kArrayBytes), cf.c[a], j);
     }
     const uint32_t flag = (rowg >= 0 && rowg < q.nrows) ? p.rowflag[rowg] : 0u;
     __syncthreads();                       // everyone has left the input stage
@@ -218,21 +240,16 @@ __global__ void __launch_bounds__(NT, MINB) k2_tblock(const __grid_constant__ K2
       tma_wait_read0();                    // previous tile's stores have drained the output stage
     }
 
-    const int64_t k0 = rowg * C;
-    for (int s = 0; s < q.T; ++s) {
-      R El, Hl, Er;
-      exchange_halo<R, C, NW>(E, H, hs, s & 1, warp, lane, El, Hl, Er);
-      leapfrog_row<R, C>(E, H, J, cf, El, Hl, Er, p, flag, k0, g, p.n0 + s, owner);
-    }
-    // (the barrier inside the first exchange orders tma_wait_read0 before the writes below)
+    time_loop<R, C, NW>(E, H, J, cf, hs, p, flag, rowg * G::CR + sub * C, g, owner, q.T, warp, lane);
+
+    // (the barriers of the time loop order tma_wait_read0 before the writes below)
     if (owner) {
-      uint8_t *my = sout + r_out * kRowBytes;
 #pragma unroll
-      for (int j = 0; j < NCH; ++j) {
-        const uint32_t o = (j ^ sw_out) << 4;
-        *reinterpret_cast<Vec *>(my + 0 * kArrayBytes + o) = regs_to_vec(E, j);
-        *reinterpret_cast<Vec *>(my + 1 * kArrayBytes + o) = regs_to_vec(H, j);
-        *reinterpret_cast<Vec *>(my + 2 * kArrayBytes + o) = regs_to_vec(J, j);
+      for (int j = 0; j < G::NCH; ++j) {
+        uint8_t *my = sout + off_out[j];
+        *reinterpret_cast<Vec *>(my + 0 * kArrayBytes) = regs_to_vec<R, C>(E, j);
+        *reinterpret_cast<Vec *>(my + 1 * kArrayBytes) = regs_to_vec<R, C>(H, j);
+        *reinterpret_cast<Vec *>(my + 2 * kArrayBytes) = regs_to_vec<R, C>(J, j);
       }
     }
     fence_proxy_async_smem();
@@ -282,20 +299,24 @@ cudaError_t launch_k1(int dtype, const Layout &L, FieldPtrs src, FieldPtrs dst, 
   return dtype == 0 ? launch_k1_t<double>(L, src, dst, coef, sc, st) : launch_k1_t<float>(L, src, dst, coef, sc, st);
 }
 
-// K3 variants: NT rows per grid; coefficients in registers up to NT = 256, in shared memory at 512.
-int k3_threads_for_rows(int, int64_t nrows) {
+// K3 variants.  variant 0: a thread owns a whole 64-B row (ROWS = NT); coefficients in registers
+// up to 256 rows, in shared memory at 512 rows.  variant 1: a thread owns half a row (twice the
+// warps per grid, half the registers per thread); up to 256 rows.
+int k3_threads_for_rows(int, int64_t nrows, int variant) {
   const int opts[] = {32, 64, 128, 256, 512};
   for (int o : opts)
-    if (nrows <= o) return o;
+    if (nrows <= o) {
+      if (variant == 1) return o <= 256 ? 2 * o : 0;
+      return o;
+    }
   return 0;
 }
-size_t k3_smem_bytes(int, int NT) { return NT == 512 ? (size_t)6 * NT * kRowBytes + 1024 : 0; }
 
-template <typename R, int NT, bool CSM, int MINB>
+template <typename R, int C, int NT, bool CSM, int MINB>
 static cudaError_t launch_k3_v(const Layout &L, FieldPtrs f, void *const coef[6], const StepCommon &sc,
                                int64_t nsteps, cudaStream_t st) {
-  auto kern = k3_resident<R, NT, CSM, MINB>;
-  const size_t smem = CSM ? (size_t)6 * NT * kRowBytes + 1024 : 0;
+  auto kern = k3_resident<R, C, NT, CSM, MINB>;
+  const size_t smem = CSM ? (size_t)6 * (NT / Geom<R, C>::TPR) * kRowBytes + 1024 : 0;
   if (smem > 48 * 1024) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
@@ -305,54 +326,89 @@ static cudaError_t launch_k3_v(const Layout &L, FieldPtrs f, void *const coef[6]
 }
 template <typename R>
 static cudaError_t launch_k3_t(const Layout &L, FieldPtrs f, void *const coef[6], const StepCommon &sc,
-                               int64_t nsteps, int NT, cudaStream_t st) {
-  switch (NT) {
-    case 32: return launch_k3_v<R, 32, false, 8>(L, f, coef, sc, nsteps, st);
-    case 64: return launch_k3_v<R, 64, false, 5>(L, f, coef, sc, nsteps, st);
-    case 128: return launch_k3_v<R, 128, false, 2>(L, f, coef, sc, nsteps, st);
-    case 256: return launch_k3_v<R, 256, false, 1>(L, f, coef, sc, nsteps, st);
-    case 512: return launch_k3_v<R, 512, true, 1>(L, f, coef, sc, nsteps, st);
+                               int64_t nsteps, int NT, int variant, cudaStream_t st) {
+  constexpr int CF = kRowBytes / sizeof(R), CH = CF / 2;
+  if (variant == 0) switch (NT) {
+    case 32: return launch_k3_v<R, CF, 32, false, 8>(L, f, coef, sc, nsteps, st);
+    case 64: return launch_k3_v<R, CF, 64, false, 4>(L, f, coef, sc, nsteps, st);
+    case 128: return launch_k3_v<R, CF, 128, false, 2>(L, f, coef, sc, nsteps, st);
+    case 256: return launch_k3_v<R, CF, 256, false, 1>(L, f, coef, sc, nsteps, st);
+    case 512: return launch_k3_v<R, CF, 512, true, 1>(L, f, coef, sc, nsteps, st);
+  }
+  else switch (NT) {
+    case 64: return launch_k3_v<R, CH, 64, false, 8>(L, f, coef, sc, nsteps, st);
+    case 128: return launch_k3_v<R, CH, 128, false, 4>(L, f, coef, sc, nsteps, st);
+    case 256: return launch_k3_v<R, CH, 256, false, 2>(L, f, coef, sc, nsteps, st);
+    case 512: return launch_k3_v<R, CH, 512, false, 1>(L, f, coef, sc, nsteps, st);
   }
   return cudaErrorInvalidValue;
 }
 cudaError_t launch_k3(int dtype, const Layout &L, FieldPtrs f, void *const coef[6], const StepCommon &sc,
-                      int64_t nsteps, int NT, cudaStream_t st) {
-  return dtype == 0 ? launch_k3_t<double>(L, f, coef, sc, nsteps, NT, st)
-                    : launch_k3_t<float>(L, f, coef, sc, nsteps, NT, st);
+                      int64_t nsteps, int NT, int variant, cudaStream_t st) {
+  return dtype == 0 ? launch_k3_t<double>(L, f, coef, sc, nsteps, NT, variant, st)
+                    : launch_k3_t<float>(L, f, coef, sc, nsteps, NT, variant, st);
 }
 
-// K2 variants
-int k2_threads_options(int idx) { const int o[] = {128, 256}; return idx < 2 ? o[idx] : 0; }
-size_t k2_smem_bytes(int NT) { return (size_t)12 * NT * kRowBytes + 1024; }
+// K2 variants: {nodes per thread, threads per CTA, CTAs per SM aimed at}
+//   0: full row, 128 threads, 2 CTAs/SM     1: half row, 256 threads, 2 CTAs/SM
+//   2: full row, 256 threads, 1 CTA/SM      3: half row, 512 threads, 1 CTA/SM
+int k2_tile_rows(int variant) { const int r[] = {128, 128, 256, 256}; return (variant >= 0 && variant < 4) ? r[variant] : 0; }
+size_t k2_smem_bytes(int variant) { return (size_t)12 * k2_tile_rows(variant) * kRowBytes + 1024; }
 
-template <typename R, int NT, int MINB>
+template <typename R, int V> struct K2Variant;
+template <typename R> struct K2Variant<R, 0> { static constexpr int C = kRowBytes / sizeof(R), NT = 128, MINB = 2; };
+template <typename R> struct K2Variant<R, 1> { static constexpr int C = kRowBytes / sizeof(R) / 2, NT = 256, MINB = 2; };
+template <typename R> struct K2Variant<R, 2> { static constexpr int C = kRowBytes / sizeof(R), NT = 256, MINB = 1; };
+template <typename R> struct K2Variant<R, 3> { static constexpr int C = kRowBytes / sizeof(R) / 2, NT = 512, MINB = 1; };
+
+template <typename R, int V>
 static cudaError_t k2_configure_v(int *ctas) {
-  auto kern = k2_tblock<R, NT, MINB>;
-  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k2_smem_bytes(NT));
+  typedef K2Variant<R, V> KV;
+  auto kern = k2_tblock<R, KV::C, KV::NT, KV::MINB>;
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k2_smem_bytes(V));
   if (e != cudaSuccess) return e;
-  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas, kern, NT, k2_smem_bytes(NT));
+  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas, kern, KV::NT, k2_smem_bytes(V));
 }
-cudaError_t k2_configure(int dtype, int NT, int *ctas) {
-  if (dtype == 0) return NT == 128 ? k2_configure_v<double, 128, 2>(ctas) : k2_configure_v<double, 256, 1>(ctas);
-  return NT == 128 ? k2_configure_v<float, 128, 2>(ctas) : k2_configure_v<float, 256, 1>(ctas);
+template <typename R>
+static cudaError_t k2_configure_t(int variant, int *ctas) {
+  switch (variant) {
+    case 0: return k2_configure_v<R, 0>(ctas);
+    case 1: return k2_configure_v<R, 1>(ctas);
+    case 2: return k2_configure_v<R, 2>(ctas);
+    case 3: return k2_configure_v<R, 3>(ctas);
+  }
+  return cudaErrorInvalidValue;
+}
+cudaError_t k2_configure(int dtype, int variant, int *ctas) {
+  return dtype == 0 ? k2_configure_t<double>(variant, ctas) : k2_configure_t<float>(variant, ctas);
 }
 
-template <typename R, int NT, int MINB>
+template <typename R, int V>
 static cudaError_t launch_k2_v(const Layout &L, const K2Plan &plan, int src_buf, const StepCommon &sc, int steps,
                                cudaStream_t st) {
+  typedef K2Variant<R, V> KV;
   K2Args q;
   q.T = steps; q.HR = plan.HR; q.rows_out = plan.rows_out;
   q.tiles_per_grid = plan.tiles_per_grid; q.total_tiles = plan.total_tiles; q.nrows = L.nrows;
-  k2_tblock<R, NT, MINB><<<plan.grid, NT, plan.smem_bytes, st>>>(plan.maps[src_buf], make_params<R>(sc), q);
+  k2_tblock<R, KV::C, KV::NT, KV::MINB><<<plan.grid, KV::NT, plan.smem_bytes, st>>>(plan.maps[src_buf],
+                                                                                   make_params<R>(sc), q);
   return cudaGetLastError();
+}
+template <typename R>
+static cudaError_t launch_k2_t(const Layout &L, const K2Plan &plan, int src_buf, const StepCommon &sc, int steps,
+                               cudaStream_t st) {
+  switch (plan.variant) {
+    case 0: return launch_k2_v<R, 0>(L, plan, src_buf, sc, steps, st);
+    case 1: return launch_k2_v<R, 1>(L, plan, src_buf, sc, steps, st);
+    case 2: return launch_k2_v<R, 2>(L, plan, src_buf, sc, steps, st);
+    case 3: return launch_k2_v<R, 3>(L, plan, src_buf, sc, steps, st);
+  }
+  return cudaErrorInvalidValue;
 }
 cudaError_t launch_k2(int dtype, const Layout &L, const K2Plan &plan, int src_buf, const StepCommon &sc, int steps,
                       cudaStream_t st) {
-  if (dtype == 0)
-    return plan.NT == 128 ? launch_k2_v<double, 128, 2>(L, plan, src_buf, sc, steps, st)
-                          : launch_k2_v<double, 256, 1>(L, plan, src_buf, sc, steps, st);
-  return plan.NT == 128 ? launch_k2_v<float, 128, 2>(L, plan, src_buf, sc, steps, st)
-                        : launch_k2_v<float, 256, 1>(L, plan, src_buf, sc, steps, st);
+  return dtype == 0 ? launch_k2_t<double>(L, plan, src_buf, sc, steps, st)
+                    : launch_k2_t<float>(L, plan, src_buf, sc, steps, st);
 }
 
 }  // namespace rketd

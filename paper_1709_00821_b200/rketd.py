@@ -40,7 +40,7 @@ _lib.rketd_set_probes.argtypes = [_vp, _vp, _i32]
 _lib.rketd_set_probe_dft.argtypes = [_vp, _vp, _i32]
 _lib.rketd_set_fields.argtypes = [_vp, _vp, _vp, _vp]
 _lib.rketd_reset.argtypes = [_vp]
-_lib.rketd_set_plan.argtypes = [_vp, _i32, _i32]
+_lib.rketd_set_plan.argtypes = [_vp, _i32, _i32, _i32]
 _lib.rketd_run.argtypes = [_vp, _i64]
 _lib.rketd_read_probes.argtypes = [_vp, _vp, _i64, ctypes.POINTER(_i64)]
 _lib.rketd_get_fields.argtypes = [_vp, _vp, _vp, _vp]
@@ -115,8 +115,8 @@ def rketd_reset(h):
     _check(h, _lib.rketd_reset(h))
 
 
-def rketd_set_plan(h, kernel: int = KERNEL_AUTO, depth: int = 0):
-    _check(h, _lib.rketd_set_plan(h, kernel, depth))
+def rketd_set_plan(h, kernel: int = KERNEL_AUTO, depth: int = 0, variant: int = -1):
+    _check(h, _lib.rketd_set_plan(h, kernel, depth, variant))
 
 
 def rketd_run(h, nsteps: int):
@@ -189,7 +189,7 @@ class Sim:
 
     def set_fields(self, E=None, H=None, J=None): rketd_set_fields(self.h, E, H, J)
     def reset(self): rketd_reset(self.h)
-    def set_plan(self, kernel=KERNEL_AUTO, depth=0): rketd_set_plan(self.h, kernel, depth)
+    def set_plan(self, kernel=KERNEL_AUTO, depth=0, variant=-1): rketd_set_plan(self.h, kernel, depth, variant)
     def run(self, nsteps): rketd_run(self.h, nsteps)
     def counter(self, which): return rketd_get_counter(self.h, which)
 
