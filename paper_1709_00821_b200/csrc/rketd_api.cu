@@ -188,7 +188,8 @@ int build_k2_plan(rketd_sim *s, int depth, int variant) {
   CU_TRY(s, cudaGetDevice(&dev));
   CU_TRY(s, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
   P.ctas_per_sm = ctas;
-  P.grid = (int)std::min<int64_t>(P.total_tiles, (int64_t)sms * ctas);
+  const int tpc = k2_tiles_per_cta(variant);
+  P.grid = (int)std::min<int64_t>((P.total_tiles + tpc - 1) / tpc, (int64_t)sms * ctas);
   for (int b = 0; b < 2; ++b) {
     for (int a = 0; a < 3; ++a) {
       int rc = make_map(s, &P.maps[b].ld[a], s->fld[b][a], rows);

@@ -77,10 +77,10 @@ __device__ __forceinline__ typename Arith<R>::Vec regs_to_vec(const R (&r)[C], i
   return vec_pack(o);
 }
 
-// keep a loop-invariant value in a register (stops the compiler from re-reading the constant
-// bank inside the time loop, where the load latency would sit on the critical path)
-__device__ __forceinline__ void pin_register(double &x) { asm volatile("" : "+d"(x)); }
-__device__ __forceinline__ void pin_register(float &x) { asm volatile("" : "+f"(x)); }
+// keep a loop-invariant kernel parameter in a vector register: a value that went through a
+// shuffle cannot be re-read from the constant bank by ptxas inside the time loop, where the
+// load latency would sit on the critical path
+template <typename R> __device__ __forceinline__ R pin_register(R x) { return __shfl_sync(0xffffffffu, x, 0); }
 
 // Geometry of the register tiling: a thread owns C consecutive nodes (32 or 64 B) of every
 // array; a 64-B row of the HBM layout is shared by TPR = 1 or 2 threads.
@@ -136,14 +136,15 @@ struct CoefSmem {
 // ---- one leapfrog step of a thread's C nodes, in two phases so that the halo values the
 // neighbours need for the NEXT step can be sent between them.
 //
-// Phase 1: H' (a1), E' in place (a2), Mur (a3), source (a4), probe record (a6), and the part
-// t = kb E + ka J of eq. (11) that needs the old E.  El, Hl: old E and H of the node left of the
-// thread's nodes; Er: old E of the node to the right.  k0: physical in-grid index of the first
+// Phase 1: H' in place (a1), E' into En (a2), Mur (a3), source (a4), probe record (a6), and the
+// part t = kb E + ka J of eq. (11) that needs the old E.  El, Hl: old E and H of the node left of
+// the thread's nodes; Er: old E of the node to the right.  k0: physical in-grid index of the first
 // node; g: grid; nloc: local step index; owner: this thread records probes among its nodes.
-template <typename R, int C, typename CF>
-__device__ __forceinline__ void step_fields(R (&E)[C], R (&H)[C], const R (&J)[C], R (&t)[C], const CF &cf, R El, R Hl,
-                                            R Er, R nchh, const StepParams<R> &p, uint32_t flag, int64_t k0,
-                                            int64_t g, int64_t nloc, bool owner) {
+// SPECIAL = false compiles the boundary/source/probe handling out (tiles without such rows).
+template <bool SPECIAL, typename R, int C, typename CF>
+__device__ __forceinline__ void step_fields(const R (&E)[C], R (&En)[C], R (&H)[C], const R (&J)[C], R (&t)[C],
+                                            const CF &cf, R El, R Hl, R Er, R nchh, const StepParams<R> &p,
+                                            uint32_t flag, int64_t k0, int64_t g, int64_t nloc, bool owner) {
   typedef Arith<R> A;
   constexpr int V = 16 / sizeof(R);
   // a1: H update, eq. (14).  The left neighbour's new H is recomputed here from old values so
@@ -151,16 +152,6 @@ __device__ __forceinline__ void step_fields(R (&E)[C], R (&H)[C], const R (&J)[C
   const R Hl_new = A::fma(nchh, A::sub(E[0], El), Hl);
 #pragma unroll
   for (int i = 0; i < C; ++i) H[i] = A::fma(nchh, A::sub(i + 1 < C ? E[i + 1] : Er, E[i]), H[i]);
-  // old E at the Mur nodes and their inner neighbours (flagged rows only)
-  R mL0 = R(0), mL1 = R(0), mR0 = R(0), mR1 = R(0);
-  if (flag & (F_MURL | F_MURR)) {
-#pragma unroll
-    for (int i = 0; i < C - 1; ++i)
-      if (k0 + i == p.cellL) { mL0 = E[i]; mL1 = E[i + 1]; }
-#pragma unroll
-    for (int i = 1; i < C; ++i)
-      if (k0 + i == p.cellR) { mR0 = E[i]; mR1 = E[i - 1]; }
-  }
   // a2: E update, eq. (12) with (11) substituted; t = kb E + ka J (first two terms of eq. (11))
 #pragma unroll
   for (int j = 0; j < C / V; ++j) {
@@ -173,43 +164,44 @@ __device__ __forceinline__ void step_fields(R (&E)[C], R (&H)[C], const R (&J)[C
 #pragma unroll
     for (int u = 0; u < V; ++u) {
       const int i = j * V + u;
-      const R w = A::fma(-cj[u], J[i], A::mul(ca[u], E[i]));
+      En[i] = A::fma(-ch[u], A::sub(H[i], i ? H[i - 1] : Hl_new), A::fma(-cj[u], J[i], A::mul(ca[u], E[i])));
       t[i] = A::fma(kb[u], E[i], A::mul(ka[u], J[i]));
-      E[i] = A::fma(-ch[u], A::sub(H[i], i ? H[i - 1] : Hl_new), w);
     }
   }
-  if (flag) {   // threads that hold a boundary node, the source node or a probe (rare)
-    if (flag & F_MURL) {   // a3, left end.  The layout guarantees node 1 is held by the same thread.
+  if constexpr (SPECIAL) {
+    if (flag) {   // threads that hold a boundary node, the source node or a probe (rare)
+      if (flag & F_MURL) {   // a3, left end.  The layout guarantees node 1 is held by the same thread.
 #pragma unroll
-      for (int i = 0; i < C - 1; ++i)
-        if (k0 + i == p.cellL) E[i] = A::fma(p.mur_m, A::sub(E[i + 1], mL0), mL1);
+        for (int i = 0; i < C - 1; ++i)
+          if (k0 + i == p.cellL) En[i] = A::fma(p.mur_m, A::sub(En[i + 1], E[i]), E[i + 1]);
 #pragma unroll
-      for (int i = 0; i < C; ++i)
-        if (k0 + i < p.cellL) H[i] = R(0);      // padding left of node 0
-    }
-    if (flag & F_MURR) {   // a3, right end.  Node ncells-2 is held by the same thread.
+        for (int i = 0; i < C; ++i)
+          if (k0 + i < p.cellL) H[i] = R(0);      // padding left of node 0
+      }
+      if (flag & F_MURR) {   // a3, right end.  Node ncells-2 is held by the same thread.
 #pragma unroll
-      for (int i = 1; i < C; ++i)
-        if (k0 + i == p.cellR) E[i] = A::fma(p.mur_m, A::sub(E[i - 1], mR0), mR1);
+        for (int i = 1; i < C; ++i)
+          if (k0 + i == p.cellR) En[i] = A::fma(p.mur_m, A::sub(En[i - 1], E[i]), E[i - 1]);
 #pragma unroll
-      for (int i = 0; i < C; ++i)
-        if (k0 + i >= p.cellR) H[i] = R(0);     // H[ncells-1] and padding
-    }
-    if (flag & F_SRC) {    // a4: soft source
-      const R s = p.src_tab[nloc];
+        for (int i = 0; i < C; ++i)
+          if (k0 + i >= p.cellR) H[i] = R(0);     // H[ncells-1] and padding
+      }
+      if (flag & F_SRC) {    // a4: soft source
+        const R s = p.src_tab[nloc];
 #pragma unroll
-      for (int i = 0; i < C; ++i)
-        if (k0 + i == p.cellS) E[i] = A::add(E[i], s);
-    }
-    if ((flag & F_PROBE) && owner && p.rec) {   // a6: probe record
-      for (int q = 0; q < p.nprobes; ++q) {
-        const int64_t d = p.probe_cell[q] - k0;
-        if (d >= 0 && d < C) {
-          R v = E[0];
+        for (int i = 0; i < C; ++i)
+          if (k0 + i == p.cellS) En[i] = A::add(En[i], s);
+      }
+      if ((flag & F_PROBE) && owner && p.rec) {   // a6: probe record
+        for (int q = 0; q < p.nprobes; ++q) {
+          const int64_t d = p.probe_cell[q] - k0;
+          if (d >= 0 && d < C) {
+            R v = En[0];
 #pragma unroll
-          for (int i = 1; i < C; ++i)
-            if (d == i) v = E[i];
-          p.rec[(g * p.nprobes + q) * p.rec_stride + nloc] = v;
+            for (int i = 1; i < C; ++i)
+              if (d == i) v = En[i];
+            p.rec[(g * p.nprobes + q) * p.rec_stride + nloc] = v;
+          }
         }
       }
     }
@@ -218,7 +210,7 @@ __device__ __forceinline__ void step_fields(R (&E)[C], R (&H)[C], const R (&J)[C
 
 // Phase 2 — a5: J' = kc E' + (kb E + ka J), eq. (11), with the final E'.
 template <typename R, int C, typename CF>
-__device__ __forceinline__ void step_current(R (&J)[C], const R (&E)[C], const R (&t)[C], const CF &cf) {
+__device__ __forceinline__ void step_current(R (&J)[C], const R (&En)[C], const R (&t)[C], const CF &cf) {
   typedef Arith<R> A;
   constexpr int V = 16 / sizeof(R);
 #pragma unroll
@@ -226,7 +218,7 @@ __device__ __forceinline__ void step_current(R (&J)[C], const R (&E)[C], const R
     R kc[V];
     cf.template chunk<5>(j, kc);
 #pragma unroll
-    for (int u = 0; u < V; ++u) J[j * V + u] = A::fma(kc[u], E[j * V + u], t[j * V + u]);
+    for (int u = 0; u < V; ++u) J[j * V + u] = A::fma(kc[u], En[j * V + u], t[j * V + u]);
   }
 }
 

@@ -55,6 +55,7 @@ struct K2Plan {
 };
 
 int k2_tile_rows(int variant);                                    // rows per tile of a K2 variant, 0 if none
+int k2_tiles_per_cta(int variant);                               // tiles a CTA works on at a time (warp tiles)
 size_t k2_smem_bytes(int variant);
 int k3_threads_for_rows(int dtype, int64_t nrows, int variant);   // threads per CTA of the K3 kernel, or 0
 

@@ -49,7 +49,7 @@ __global__ void __launch_bounds__(128) k1_step(RowPtrs<R> src, RowPtrs<R> dst, C
   const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (r >= total_rows) return;
   const int64_t g = r / nrows, row = r - g * nrows;
-  R E[C], H[C], J[C], t[C];
+  R E[C], En[C], H[C], J[C], t[C];
   CoefRegs<R, C> cf;
   load_nodes_global<R, C>(src.E, r * C, E);
   load_nodes_global<R, C>(src.H, r * C, H);
@@ -60,33 +60,45 @@ __global__ void __launch_bounds__(128) k1_step(RowPtrs<R> src, RowPtrs<R> dst, C
   const R Hl = row > 0 ? src.H[r * C - 1] : R(0);
   const R Er = row < nrows - 1 ? src.E[(r + 1) * C] : R(0);
   const uint32_t flag = p.rowflag[row];
-  step_fields<R, C>(E, H, J, t, cf, El, Hl, Er, p.nchh, p, flag, row * C, g, p.n0, true);
-  step_current<R, C>(J, E, t, cf);
-  store_nodes_global<R, C>(dst.E, r * C, E);
+  step_fields<true, R, C>(E, En, H, J, t, cf, El, Hl, Er, p.nchh, p, flag, row * C, g, p.n0, true);
+  step_current<R, C>(J, En, t, cf);
+  store_nodes_global<R, C>(dst.E, r * C, En);
   store_nodes_global<R, C>(dst.H, r * C, H);
   store_nodes_global<R, C>(dst.J, r * C, J);
 }
 
 // The time loop shared by K2 and K3: nsteps leapfrog steps of this thread's nodes, halos
-// exchanged inside the CTA.  One __syncthreads per step, placed after phase 2.
-template <typename R, int C, int NW, typename CF>
+// exchanged inside the CTA.  One __syncthreads per step, placed after phase 2.  The loop is
+// unrolled by two so that E ping-pongs between two register arrays without copies.
+template <bool SPECIAL, typename R, int C, int NW, typename CF>
 __device__ __forceinline__ void time_loop(R (&E)[C], R (&H)[C], R (&J)[C], const CF &cf, HaloSlots<R, NW> &hs,
                                           const StepParams<R> &p, uint32_t flag, int64_t k0, int64_t g, bool owner,
                                           int64_t nsteps, int warp, int lane) {
-  R nchh = p.nchh;
-  pin_register(nchh);
+  const R nchh = pin_register(p.nchh);
+  int64_t nloc = p.n0;
   R El, Hl, Er;
   send_halo<R, C, NW>(E, H, hs, 0, warp, lane, El, Hl, Er);
   __syncthreads();
   recv_halo<R, NW>(hs, 0, warp, lane, El, Hl, Er);
-  for (int64_t s = 0; s < nsteps; ++s) {
+  R Eb[C];
+  auto one_step = [&](const R (&Ein)[C], R (&Eout)[C], int par) {
     R t[C];
-    step_fields<R, C>(E, H, J, t, cf, El, Hl, Er, nchh, p, flag, k0, g, p.n0 + s, owner);
-    const int par = (int)((s + 1) & 1);
-    send_halo<R, C, NW>(E, H, hs, par, warp, lane, El, Hl, Er);     // for step s+1
-    step_current<R, C>(J, E, t, cf);
+    step_fields<SPECIAL, R, C>(Ein, Eout, H, J, t, cf, El, Hl, Er, nchh, p, flag, k0, g, nloc, owner);
+    send_halo<R, C, NW>(Eout, H, hs, par, warp, lane, El, Hl, Er);     // for the next step
+    step_current<R, C>(J, Eout, t, cf);
     __syncthreads();
     recv_halo<R, NW>(hs, par, warp, lane, El, Hl, Er);
+    if (SPECIAL) ++nloc;
+  };
+  int64_t left = nsteps;
+  for (; left >= 2; left -= 2) {
+    one_step(E, Eb, 1);
+    one_step(Eb, E, 0);
+  }
+  if (left) {
+    one_step(E, Eb, 1);
+#pragma unroll
+    for (int i = 0; i < C; ++i) E[i] = Eb[i];
   }
 }
 
@@ -140,7 +152,7 @@ __global__ void __launch_bounds__(NT, MINB) k3_resident(RowPtrs<R> f, CoefPtrs<R
     stage(std::integral_constant<int, 0>{}); stage(std::integral_constant<int, 1>{});
     stage(std::integral_constant<int, 2>{}); stage(std::integral_constant<int, 3>{});
     stage(std::integral_constant<int, 4>{}); stage(std::integral_constant<int, 5>{});
-    time_loop<R, C, NW>(E, H, J, cf, hs, p, flag, k0, g, true, nsteps, warp, lane);
+    time_loop<true, R, C, NW>(E, H, J, cf, hs, p, flag, k0, g, true, nsteps, warp, lane);
   } else {
     CoefRegs<R, C> cf;
 #pragma unroll
@@ -149,7 +161,7 @@ __global__ void __launch_bounds__(NT, MINB) k3_resident(RowPtrs<R> f, CoefPtrs<R
       for (int i = 0; i < C; ++i) cf.c[a][i] = R(0);
       if (valid) load_nodes_global<R, C>(cp.c[a], first, cf.c[a]);
     }
-    time_loop<R, C, NW>(E, H, J, cf, hs, p, flag, k0, g, true, nsteps, warp, lane);
+    time_loop<true, R, C, NW>(E, H, J, cf, hs, p, flag, k0, g, true, nsteps, warp, lane);
   }
 
   if (valid) {
@@ -233,14 +245,17 @@ __global__ void __launch_bounds__(NT, MINB) k2_tblock(const __grid_constant__ K2
         vec_to_regs<R, C>(*reinterpret_cast<const Vec *>(my + (3 + a) * kArrayBytes), cf.c[a], j);
     }
     const uint32_t flag = (rowg >= 0 && rowg < q.nrows) ? p.rowflag[rowg] : 0u;
-    __syncthreads();                       // everyone has left the input stage
+    const bool special = __syncthreads_or(flag != 0u);   // barrier: everyone has left the input stage
     if (tid == 0) {
       const int64_t next = tile + gridDim.x;
       if (next < q.total_tiles) issue_loads(next);   // overlaps with the T steps below
       tma_wait_read0();                    // previous tile's stores have drained the output stage
     }
 
-    time_loop<R, C, NW>(E, H, J, cf, hs, p, flag, rowg * G::CR + sub * C, g, owner, q.T, warp, lane);
+    if (special)   // tile holds a boundary, source or probe row (a handful of tiles per grid)
+      time_loop<true, R, C, NW>(E, H, J, cf, hs, p, flag, rowg * G::CR + sub * C, g, owner, q.T, warp, lane);
+    else
+      time_loop<false, R, C, NW>(E, H, J, cf, hs, p, 0u, 0, g, false, q.T, warp, lane);
 
     // (the barriers of the time loop order tma_wait_read0 before the writes below)
     if (owner) {
@@ -262,6 +277,140 @@ __global__ void __launch_bounds__(NT, MINB) k2_tblock(const __grid_constant__ K2
     }
   }
   if (tid == 0) tma_wait0();
+}
+
+// ------------------------------------------------------------------------------------ K2, warp tiles
+// Same temporal blocking, but every WARP owns an independent tile of 32 rows (halo included),
+// its own shared-memory stage and its own mbarrier: halos travel by warp shuffles only, there is
+// no block barrier and no shared-memory exchange in the time loop.  Lanes 0 and 31 receive their
+// own values from the shuffles at the tile edge, which is fine: those nodes are in the halo that
+// is thrown away.  The price is a smaller tile (more redundant halo work per tile).
+template <bool SPECIAL, typename R, int C, typename CF>
+__device__ __forceinline__ void warp_time_loop(R (&E)[C], R (&H)[C], R (&J)[C], const CF &cf, const StepParams<R> &p,
+                                               uint32_t flag, int64_t k0, int64_t g, bool owner, int nsteps) {
+  const R nchh = pin_register(p.nchh);
+  int64_t nloc = p.n0;
+  R El = __shfl_up_sync(0xffffffffu, E[C - 1], 1);
+  R Hl = __shfl_up_sync(0xffffffffu, H[C - 1], 1);
+  R Er = __shfl_down_sync(0xffffffffu, E[0], 1);
+  R Eb[C];
+  auto one_step = [&](const R (&Ein)[C], R (&Eout)[C]) {
+    R t[C];
+    step_fields<SPECIAL, R, C>(Ein, Eout, H, J, t, cf, El, Hl, Er, nchh, p, flag, k0, g, nloc, owner);
+    El = __shfl_up_sync(0xffffffffu, Eout[C - 1], 1);
+    Hl = __shfl_up_sync(0xffffffffu, H[C - 1], 1);
+    Er = __shfl_down_sync(0xffffffffu, Eout[0], 1);
+    step_current<R, C>(J, Eout, t, cf);
+    if (SPECIAL) ++nloc;
+  };
+  int left = nsteps;
+  for (; left >= 2; left -= 2) {
+    one_step(E, Eb);
+    one_step(Eb, E);
+  }
+  if (left) {
+    one_step(E, Eb);
+#pragma unroll
+    for (int i = 0; i < C; ++i) E[i] = Eb[i];
+  }
+}
+
+template <typename R, int NW, int MINB>
+__global__ void __launch_bounds__(NW * 32, MINB) k2_wtile(const __grid_constant__ K2Maps maps,
+                                                          const __grid_constant__ StepParams<R> p, K2Args q) {
+  constexpr int C = kRowBytes / sizeof(R);
+  typedef Geom<R, C> G;
+  constexpr uint32_t kArrayBytes = 32 * kRowBytes;      // one array of one warp tile: 2 KB
+  constexpr uint32_t kWarpBytes = 12 * kArrayBytes;     // 9 input + 3 output arrays
+  typedef typename Arith<R>::Vec Vec;
+
+  __shared__ __align__(8) uint64_t mbars[NW];
+  extern __shared__ uint8_t smem_raw[];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  uint8_t *sin = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023)) +
+                 warp * kWarpBytes;
+  uint8_t *sout = sin + 9 * kArrayBytes;
+  uint64_t *mbar = &mbars[warp];
+
+  auto issue_loads = [&](int64_t tile) {   // lane 0
+    const int64_t g = tile / q.tiles_per_grid, ti = tile - g * q.tiles_per_grid;
+    const int row0 = (int)(ti * q.rows_out - q.HR);
+    mbar_expect_tx(mbar, 9u * kArrayBytes);
+#pragma unroll 1
+    for (int a = 0; a < 9; ++a) tma_load_3d(sin + a * kArrayBytes, &maps.ld[a], mbar, 0, row0, (int)g);
+  };
+
+  if (lane == 0) {
+    mbar_init(mbar, 1);
+    fence_barrier_init();
+  }
+  __syncwarp();
+  const int64_t stride = (int64_t)gridDim.x * NW;
+  int64_t tile = (int64_t)blockIdx.x * NW + warp;
+  if (lane == 0 && tile < q.total_tiles) issue_loads(tile);
+  uint32_t phase = 0;
+
+  const int r_out = lane - q.HR;
+  const bool owner = r_out >= 0 && r_out < q.rows_out;
+  uint32_t off_in[G::NCH], off_out[G::NCH];
+#pragma unroll
+  for (int j = 0; j < G::NCH; ++j) {
+    off_in[j] = swz_off(lane, j);
+    off_out[j] = swz_off(owner ? r_out : 0, j);
+  }
+
+  for (; tile < q.total_tiles; tile += stride) {
+    const int64_t g = tile / q.tiles_per_grid, ti = tile - g * q.tiles_per_grid;
+    const int64_t rowg = ti * q.rows_out - q.HR + lane;
+
+    mbar_wait(mbar, phase);
+    phase ^= 1u;
+
+    R E[C], H[C], J[C];
+    CoefRegs<R, C> cf;
+#pragma unroll
+    for (int j = 0; j < G::NCH; ++j) {
+      const uint8_t *my = sin + off_in[j];
+      vec_to_regs<R, C>(*reinterpret_cast<const Vec *>(my + 0 * kArrayBytes), E, j);
+      vec_to_regs<R, C>(*reinterpret_cast<const Vec *>(my + 1 * kArrayBytes), H, j);
+      vec_to_regs<R, C>(*reinterpret_cast<const Vec *>(my + 2 * kArrayBytes), J, j);
+#pragma unroll
+      for (int a = 0; a < 6; ++a)
+        vec_to_regs<R, C>(*reinterpret_cast<const Vec *>(my + (3 + a) * kArrayBytes), cf.c[a], j);
+    }
+    const uint32_t flag = (rowg >= 0 && rowg < q.nrows) ? p.rowflag[rowg] : 0u;
+    const bool special = __any_sync(0xffffffffu, flag != 0u);   // also: every lane has left the input stage
+    if (lane == 0) {
+      const int64_t next = tile + stride;
+      if (next < q.total_tiles) issue_loads(next);   // overlaps with the T steps below
+      tma_wait_read0();                              // previous tile's stores have drained the output stage
+    }
+
+    if (special)
+      warp_time_loop<true, R, C>(E, H, J, cf, p, flag, rowg * C, g, owner, q.T);
+    else
+      warp_time_loop<false, R, C>(E, H, J, cf, p, 0u, 0, g, false, q.T);
+
+    __syncwarp();                                    // orders lane 0's tma_wait_read0 before the writes below
+    if (owner) {
+#pragma unroll
+      for (int j = 0; j < G::NCH; ++j) {
+        uint8_t *my = sout + off_out[j];
+        *reinterpret_cast<Vec *>(my + 0 * kArrayBytes) = regs_to_vec<R, C>(E, j);
+        *reinterpret_cast<Vec *>(my + 1 * kArrayBytes) = regs_to_vec<R, C>(H, j);
+        *reinterpret_cast<Vec *>(my + 2 * kArrayBytes) = regs_to_vec<R, C>(J, j);
+      }
+    }
+    fence_proxy_async_smem();
+    __syncwarp();
+    if (lane == 0) {
+      const int row_out0 = (int)(ti * q.rows_out);
+#pragma unroll 1
+      for (int a = 0; a < 3; ++a) tma_store_3d(&maps.st[a], sout + a * kArrayBytes, 0, row_out0, (int)g);
+      tma_commit();
+    }
+  }
+  if (lane == 0) tma_wait0();
 }
 
 // ------------------------------------------------------------------------------------ launchers
@@ -352,8 +501,12 @@ cudaError_t launch_k3(int dtype, const Layout &L, FieldPtrs f, void *const coef[
 // K2 variants: {nodes per thread, threads per CTA, CTAs per SM aimed at}
 //   0: full row, 128 threads, 2 CTAs/SM     1: half row, 256 threads, 2 CTAs/SM
 //   2: full row, 256 threads, 1 CTA/SM      3: half row, 512 threads, 1 CTA/SM
-int k2_tile_rows(int variant) { const int r[] = {128, 128, 256, 256}; return (variant >= 0 && variant < 4) ? r[variant] : 0; }
-size_t k2_smem_bytes(int variant) { return (size_t)12 * k2_tile_rows(variant) * kRowBytes + 1024; }
+//   4: warp tiles (32 rows per warp), 8 warps, 1 CTA/SM      5: warp tiles, 4 warps, 2 CTAs/SM
+int k2_tile_rows(int variant) { const int r[] = {128, 128, 256, 256, 32, 32}; return (variant >= 0 && variant < 6) ? r[variant] : 0; }
+int k2_tiles_per_cta(int variant) { return variant == 4 ? 8 : variant == 5 ? 4 : 1; }
+size_t k2_smem_bytes(int variant) {
+  return (size_t)12 * k2_tile_rows(variant) * k2_tiles_per_cta(variant) * kRowBytes + 1024;
+}
 
 template <typename R, int V> struct K2Variant;
 template <typename R> struct K2Variant<R, 0> { static constexpr int C = kRowBytes / sizeof(R), NT = 128, MINB = 2; };
@@ -361,13 +514,16 @@ template <typename R> struct K2Variant<R, 1> { static constexpr int C = kRowByte
 template <typename R> struct K2Variant<R, 2> { static constexpr int C = kRowBytes / sizeof(R), NT = 256, MINB = 1; };
 template <typename R> struct K2Variant<R, 3> { static constexpr int C = kRowBytes / sizeof(R) / 2, NT = 512, MINB = 1; };
 
+template <typename K>
+static cudaError_t k2_configure_k(K kern, int variant, int threads, int *ctas) {
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k2_smem_bytes(variant));
+  if (e != cudaSuccess) return e;
+  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas, kern, threads, k2_smem_bytes(variant));
+}
 template <typename R, int V>
 static cudaError_t k2_configure_v(int *ctas) {
   typedef K2Variant<R, V> KV;
-  auto kern = k2_tblock<R, KV::C, KV::NT, KV::MINB>;
-  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k2_smem_bytes(V));
-  if (e != cudaSuccess) return e;
-  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas, kern, KV::NT, k2_smem_bytes(V));
+  return k2_configure_k(k2_tblock<R, KV::C, KV::NT, KV::MINB>, V, KV::NT, ctas);
 }
 template <typename R>
 static cudaError_t k2_configure_t(int variant, int *ctas) {
@@ -376,6 +532,8 @@ static cudaError_t k2_configure_t(int variant, int *ctas) {
     case 1: return k2_configure_v<R, 1>(ctas);
     case 2: return k2_configure_v<R, 2>(ctas);
     case 3: return k2_configure_v<R, 3>(ctas);
+    case 4: return k2_configure_k(k2_wtile<R, 8, 1>, 4, 256, ctas);
+    case 5: return k2_configure_k(k2_wtile<R, 4, 2>, 5, 128, ctas);
   }
   return cudaErrorInvalidValue;
 }
@@ -402,6 +560,17 @@ static cudaError_t launch_k2_t(const Layout &L, const K2Plan &plan, int src_buf,
     case 1: return launch_k2_v<R, 1>(L, plan, src_buf, sc, steps, st);
     case 2: return launch_k2_v<R, 2>(L, plan, src_buf, sc, steps, st);
     case 3: return launch_k2_v<R, 3>(L, plan, src_buf, sc, steps, st);
+    case 4:
+    case 5: {
+      K2Args q;
+      q.T = steps; q.HR = plan.HR; q.rows_out = plan.rows_out;
+      q.tiles_per_grid = plan.tiles_per_grid; q.total_tiles = plan.total_tiles; q.nrows = L.nrows;
+      if (plan.variant == 4)
+        k2_wtile<R, 8, 1><<<plan.grid, 256, plan.smem_bytes, st>>>(plan.maps[src_buf], make_params<R>(sc), q);
+      else
+        k2_wtile<R, 4, 2><<<plan.grid, 128, plan.smem_bytes, st>>>(plan.maps[src_buf], make_params<R>(sc), q);
+      return cudaGetLastError();
+    }
   }
   return cudaErrorInvalidValue;
 }
