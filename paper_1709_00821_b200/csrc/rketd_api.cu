@@ -167,7 +167,7 @@ int make_map(rketd_sim *s, CUtensorMap *m, void *base, int box_rows) {
 }
 
 int default_depth(const rketd_sim *s) { return s->dtype == RKETD_F64 ? 24 : 32; }
-int default_k2_variant(const rketd_sim *) { return 0; }
+int default_k2_variant(const rketd_sim *) { return 4; }
 int default_k3_variant(const rketd_sim *) { return 0; }
 int max_depth(const rketd_sim *s, int variant) { return (k2_tile_rows(variant) / 2 - 1) * s->L.C; }
 

@@ -1,0 +1,316 @@
+"""Parity of the CUDA path (librketd, through its C ABI) against the CPU oracle — `-m gpu`.
+
+Tolerances (BASELINE.json north_star; SURVEY.md §8(c) "Tolerance rule"):
+  fp64: per grid, max over all probes and samples of |gpu - oracle| / max |oracle|  <= 1e-12
+  fp32: the same ratio against the fp64 oracle                                       <= 1e-5
+Final fields are held to the same bars (normalised by the field's own max).  K1, K2 (all launch
+variants and depths) and K3 must agree BIT FOR BIT with each other: they run the same correctly
+rounded operation sequence per node, only the schedule differs.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1709_00821_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"f64": 1e-12, "f32": 1e-5}
+C0 = 299792458.0
+
+
+@pytest.fixture(scope="module")
+def rk():
+    from paper_1709_00821_b200 import rketd
+    return rketd
+
+
+def grid_err(gpu, ref):
+    """max over grids of (max |gpu-ref| over probes, samples) / (max |ref| over probes, samples)"""
+    gpu = np.asarray(gpu, np.float64)
+    d = np.abs(gpu - ref).reshape(ref.shape[0], -1).max(1)
+    s = np.abs(ref).reshape(ref.shape[0], -1).max(1)
+    assert np.all(s > 0), "vacuous comparison: oracle record is identically zero"
+    return float(np.max(d / s))
+
+
+def run_gpu(rk, w, dtype="f64", kernel=0, depth=0, variant=-1, nsteps=None, chunks=None, fields=True):
+    s = rk.Sim.from_workload(w, dtype)
+    s.set_plan(kernel, depth, variant)
+    n = w.nsteps if nsteps is None else nsteps
+    for c in (chunks or [n]):
+        s.run(c)
+    out = {"rec": s.read_probes(), "kernel": s.counter(rk.CTR_KERNEL_USED), "launches": s.counter(rk.CTR_STEP_LAUNCHES)}
+    if fields:
+        out["E"], out["H"], out["J"] = s.get_fields()
+    s.close()
+    return out
+
+
+def floors_of(w, ref):
+    return np.max(np.abs(ref["rec"])), float(np.max(w.media(0, w.ncells, 0, min(w.nbatch, 64))[0]))
+
+
+def check_fields(gpu, st, tol, peak=0.0, wp_max=0.0):
+    """Final fields.  Errors scale with the largest amplitude the run has seen, not with what is left in
+    the grid at the end, hence the floors from the probe peak: E ~ peak, H ~ peak/eta0,
+    J ~ eps0 wp^2 tau peak (tau = 20 ps, the source width)."""
+    floors = {"E": peak, "H": peak / 376.73, "J": 8.854e-12 * wp_max ** 2 * 20e-12 * peak}
+    for k, ref in (("E", st.E), ("H", st.H), ("J", st.J)):
+        ref = ref.copy()
+        if k == "H":
+            ref[:, -1] = 0.0            # H[ncells-1] is padding: the library reports 0
+        scale = max(np.max(np.abs(ref)), floors[k])
+        if scale > 0:
+            assert np.max(np.abs(np.asarray(gpu[k], np.float64) - ref)) <= tol * scale, k
+
+
+ALL_PLANS = [(1, 0, -1), (3, 0, 0), (3, 0, 1)] + [(2, 0, v) for v in range(6)] + [(2, d, 4) for d in (1, 7, 16, 33)] + \
+            [(2, 5, 0), (2, 40, 2)]
+
+
+# ------------------------------------------------------------------------------------------ config 1
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_config1_full_all_kernels(rk, dtype):
+    """BASELINE config 1 at full size (2000 nodes, 6000 steps), every kernel, variant and a few depths."""
+    w = wl.config1()
+    ref = oracle.run_workload(w)
+    first = None
+    for kernel, depth, variant in ALL_PLANS:
+        g = run_gpu(rk, w, dtype, kernel, depth, variant)
+        assert g["kernel"] == kernel
+        assert grid_err(g["rec"], ref["rec"]) <= TOL[dtype], (kernel, depth, variant)
+        check_fields(g, ref["state"], TOL[dtype], *floors_of(w, ref))
+        if first is None:
+            first = g
+        else:
+            for k in ("rec", "E", "H", "J"):
+                assert np.array_equal(first[k], g[k]), f"{k}: plan {(kernel, depth, variant)} differs from K1"
+
+
+def test_coefficients_match_oracle_in_ulps(rk):
+    """T1: the six per-node coefficients vs the oracle's S0, random media incl. nu = 0, tiny nu."""
+    rng = np.random.default_rng(5)
+    n = 5000
+    wp = rng.uniform(0, 2 * np.pi * 60e9, (3, n))
+    nu = rng.uniform(0, 1e11, (3, n))
+    wp[0, :100] = 0.0
+    nu[1, :100] = 0.0
+    nu[2, :200] = 10.0 ** rng.uniform(-3, 13, 200)        # includes x = nu dt > 0.5 (formula branch)
+    s = rk.Sim(n, 3, wl.DZ, wl.DT, "f64")
+    s.set_media(wp, nu)
+    c = s.get_coefficients()
+    o = oracle.coefficients(wp, nu, wl.DZ, wl.DT)
+    small = nu * wl.DT < 0.02           # every BASELINE config has nu dt <= 1.25e-2
+    for k in ("ca", "cj", "ch", "ka", "kb", "kc"):
+        ulp = np.abs(c[k] - o[k]) / np.maximum(np.spacing(np.abs(o[k])), 1e-300)
+        # kb = b - c ~ b/2: one ulp of b (expm1 of glibc vs CUDA) is two ulps of kb
+        assert ulp[small].max() <= (4.0 if k == "kb" else 2.0), (k, ulp[small].max())
+        assert (ulp[small] > 0).mean() < 0.05, (k, "more than 5 % of nodes differ by an ulp")
+        # larger nu dt: kb = b - c cancels (b - c ~ c / (nu dt) for large nu dt), so the 1-ulp freedom of
+        # exp / expm1 between glibc and CUDA is amplified
+        assert np.all(np.abs(c[k] - o[k])[~small] <= 1e-12 * np.abs(o[k])[~small]), k
+    assert c["chh"] == o["chh"] and c["m"] == o["m"]
+    s.close()
+    # fp32 mode: fp64 values rounded once
+    s = rk.Sim(n, 3, wl.DZ, wl.DT, "f32")
+    s.set_media(wp, nu)
+    c32 = s.get_coefficients()
+    for k in ("ca", "cj", "ch", "ka", "kb", "kc"):
+        assert np.array_equal(c32[k], c[k].astype(np.float32).astype(np.float64)), k
+    s.close()
+
+
+# ------------------------------------------------------------------------------------------ reduced configs 2-5
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_config2_reduced(rk, dtype):
+    """Periodic random slabs, noise start; several tiles and a ragged tail (200 003 nodes)."""
+    w = wl.config2(ncells=200_003, nsteps=700)
+    ref = oracle.run_workload(w, omp=True)
+    for plan in [(0, 0, -1), (2, 24, 0), (1, 0, -1)]:
+        g = run_gpu(rk, w, dtype, *plan)
+        assert grid_err(g["rec"], ref["rec"]) <= TOL[dtype], plan
+        check_fields(g, ref["state"], TOL[dtype], *floors_of(w, ref))
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_config3_reduced(rk, dtype):
+    """Batched 4096-node grids (K3 with coefficients in shared memory in fp64), 24 grids, 6000 steps."""
+    w = wl.config3(nbatch=24, nsteps=6000)
+    ref = oracle.run_workload(w, omp=True)
+    g = run_gpu(rk, w, dtype)
+    assert g["kernel"] == 3 and g["launches"] == 1
+    assert grid_err(g["rec"], ref["rec"]) <= TOL[dtype]
+    check_fields(g, ref["state"], TOL[dtype], *floors_of(w, ref))
+    g2 = run_gpu(rk, w, dtype, 2, 16, 4)      # the same batch through temporal blocking
+    assert np.array_equal(g["rec"], g2["rec"]) and np.array_equal(g["J"], g2["J"])
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_config4_reduced(rk, dtype):
+    """tanh density profile, per-node coefficients, source inside the plasma, noise start (2^20 nodes)."""
+    w = wl.config4(ncells=1 << 20, nsteps=300)
+    ref = oracle.run_workload(w, omp=True)
+    g = run_gpu(rk, w, dtype)
+    assert g["kernel"] == 2
+    assert grid_err(g["rec"], ref["rec"]) <= TOL[dtype]
+    check_fields(g, ref["state"], TOL[dtype], *floors_of(w, ref))
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_config5_reduced_dft(rk, dtype):
+    """Random multilayers, probes reduced on the device to |DFT| at 64 frequencies (48 grids, 5000 steps)."""
+    w = wl.config5(nbatch=48)
+    ref = oracle.run_workload(w, omp=True)
+    s = rk.Sim.from_workload(w, dtype)
+    s.run(2000)
+    s.run(3000)
+    mag = s.read_probes()
+    s.close()
+    assert mag.shape == (48, 2, 64)
+    assert grid_err(mag, ref["dft_mag"]) <= TOL[dtype]
+    # time-series mode of the same workload
+    w2 = wl.config5(nbatch=48, dft=False)
+    ref2 = oracle.run_workload(w2, omp=True)
+    for variant in (0, 1):
+        g = run_gpu(rk, w2, dtype, 3, 0, variant)
+        assert grid_err(g["rec"], ref2["rec"]) <= TOL[dtype]
+
+
+# ------------------------------------------------------------------------------------------ edge cases
+@pytest.mark.parametrize("ncells", [3, 4, 5, 8, 9, 16, 17, 33, 127, 1025, 4093, 4097])
+def test_small_and_ragged_grids(rk, ncells):
+    """Smallest legal grid, grids around row boundaries, both layout offsets; source and probes ON the Mur nodes."""
+    rng = np.random.default_rng(ncells)
+    nb = 3
+    wp = rng.uniform(0, 2 * np.pi * 40e9, (nb, ncells))
+    nu = rng.uniform(0, 5e10, (nb, ncells))
+    E0, H0, J0 = (rng.uniform(-1, 1, (nb, ncells)) for _ in range(3))
+    H0 /= 376.73
+    J0 *= 10.0
+    H0[:, -1] = 0.0
+    probes = sorted({0, 1, ncells // 2, ncells - 2, ncells - 1})
+    tab = rng.uniform(-1, 1, 50)
+    for src_cell in (0, ncells - 1, ncells // 2):
+        st = oracle.State(ncells, nb, E0, H0, J0)
+        rec, _ = oracle.run(st, wp, nu, wl.DZ, wl.DT, 60, src_kind=1, src_params=tab, src_cell=src_cell, probes=probes)
+        outs = []
+        for kernel, depth, variant in [(1, 0, -1), (0, 0, -1), (2, 7, 0), (2, 7, 4), (2, 3, 1)]:
+            s = rk.Sim(ncells, nb, wl.DZ, wl.DT, "f64")
+            s.set_media(wp, nu)
+            s.set_fields(E0, H0, J0)
+            s.set_source(rk.SRC_TABLE, tab, src_cell)
+            s.set_probes(probes)
+            s.set_plan(kernel, depth, variant)
+            s.run(60)
+            outs.append((s.read_probes(),) + s.get_fields())
+            s.close()
+            assert grid_err(outs[-1][0], rec) <= 1e-12
+            assert np.max(np.abs(outs[-1][1] - st.E)) <= 1e-12 * np.max(np.abs(st.E))
+            assert np.max(np.abs(outs[-1][3] - st.J)) <= 1e-12 * np.max(np.abs(st.J))
+            assert np.all(outs[-1][2][:, -1] == 0.0)
+        for o in outs[1:]:
+            assert all(np.array_equal(a, b) for a, b in zip(outs[0], o))
+
+
+def test_repeated_runs_continue_time(rk):
+    w = wl.config1(nsteps=900)
+    one = run_gpu(rk, w, "f64")
+    for plan in [(0, 0, -1), (2, 16, 4), (1, 0, -1)]:
+        parts = run_gpu(rk, w, "f64", *plan, chunks=[1, 0, 299, 17, 583])
+        assert parts["rec"].shape == one["rec"].shape
+        for k in ("rec", "E", "H", "J"):
+            assert np.array_equal(one[k], parts[k]), (plan, k)
+
+
+def test_P1_courant_one_translation_on_gpu(rk):
+    """North_star pin (a) on the CUDA path: wp = 0, S = 1, a pulse moves one node per step; Mur (m = 0) absorbs."""
+    N, n1 = 3000, 1200
+    dt = wl.DZ / C0
+    eta0 = 4e-7 * np.pi * C0
+    k = np.arange(N, dtype=np.float64)
+    f = lambda x: np.exp(-((x - 300.0) / 25.0) ** 2) * np.sin(0.2 * x)
+    for kernel, variant in [(0, -1), (2, 4), (2, 0)]:
+        s = rk.Sim(N, 1, wl.DZ, dt, "f64")
+        z = np.zeros((1, N))
+        s.set_media(z, z)
+        s.set_fields(f(k)[None, :].copy(), (f(k + 1.0) / eta0)[None, :].copy(), None)
+        s.set_plan(kernel, 0, variant)
+        s.run(n1)
+        E, _, _ = s.get_fields()
+        assert np.max(np.abs(E[0] - f(k - n1))) < 2e-13
+        s.run(2500)
+        E, _, _ = s.get_fields()
+        assert np.max(np.abs(E)) < 1e-12
+        s.close()
+
+
+def test_gauss_deriv_source_and_reset(rk):
+    w = wl.config1(nsteps=400)
+    s = rk.Sim.from_workload(w, "f64")
+    s.run(400)
+    a = s.read_probes()
+    s.reset()
+    s.set_fields(E=np.ascontiguousarray(w.initial_E_full()))
+    s.run(400)
+    b = s.read_probes()
+    assert b.shape == a.shape and np.array_equal(a, b)
+    assert s.counter(rk.CTR_STEPS_DONE) == 400
+    s.close()
+
+
+def test_device_pointers_and_stream(rk):
+    """set_media / set_fields / read_probes / get_fields with torch CUDA tensors on a non-default stream."""
+    import torch
+    w = wl.config1(nsteps=300)
+    ref = oracle.run_workload(w)
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        wp, nu = (torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in w.media_full())
+        E0 = torch.from_numpy(w.initial_E_full()).cuda()
+        stream.synchronize()
+        s = rk.Sim(w.ncells, 1, w.dz, w.dt, "f64", stream=stream.cuda_stream)
+        s.set_media(wp, nu)
+        s.set_fields(E=E0)
+        s.set_source(w.src_kind, w.src_params, w.src_cell)
+        s.set_probes(w.probes)
+        s.run(300)
+        out = torch.empty((1, 2, 300), dtype=torch.float64, device="cuda")
+        s.read_probes(out)
+        assert grid_err(out.cpu().numpy(), ref["rec"]) <= 1e-12
+        s.close()
+
+
+def test_error_codes(rk):
+    with pytest.raises(rk.RketdError) as e:
+        rk.Sim(2, 1, wl.DZ, wl.DT)
+    assert e.value.code == rk.EINVAL
+    with pytest.raises(rk.RketdError):
+        rk.Sim(100, 1, wl.DZ, 2.1 * wl.DT)              # c dt/dz > 1
+    s = rk.Sim(100, 2, wl.DZ, wl.DT)
+    with pytest.raises(rk.RketdError) as e:
+        s.run(1)
+    assert e.value.code == rk.ESTATE
+    bad = np.zeros((2, 100))
+    bad[1, 7] = -1.0
+    with pytest.raises(rk.RketdError) as e:
+        s.set_media(bad, np.zeros((2, 100)))
+    assert e.value.code == rk.EINVAL
+    bad[1, 7] = np.nan
+    with pytest.raises(rk.RketdError):
+        s.set_media(np.zeros((2, 100)), bad)
+    s.set_media(np.zeros((2, 100)), np.zeros((2, 100)))
+    for call in (lambda: s.set_probes([100]), lambda: s.set_probes([-1]), lambda: s.set_source(0, (1e-11, 0, 1), 100),
+                 lambda: s.set_source(0, (0.0, 0, 1), 5), lambda: s.set_source(7, (), 5), lambda: s.set_plan(9, 0, -1),
+                 lambda: s.set_plan(2, 100000, 4), lambda: s.run(-1)):
+        with pytest.raises(rk.RketdError) as e:
+            call()
+        assert e.value.code == rk.EINVAL
+    s.run(0)
+    s.set_probes([3, 4])
+    assert s.read_probes().shape == (2, 2, 0)
+    big = rk.Sim(5000, 1, wl.DZ, wl.DT)
+    with pytest.raises(rk.RketdError):
+        big.set_plan(rk.KERNEL_RESIDENT, 0, -1)          # 5000 fp64 nodes do not fit one CTA
+    big.close()
+    s.close()
