@@ -1,0 +1,393 @@
+#!/usr/bin/env python
+"""bench.py — throughput of the RKETD-FDTD hot path (librketd) on B200, in cell-updates/s.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--workload config4|config2|config3|config5] [--dtype f64|f32]
+                    [--kernel K] [--depth T] [--variant V] [--no-e2e] [--no-cpu]
+
+A "step" is one pass of the whole hot path over one batch of synthetic input: one rketd_run of the
+workload's full step count (config 4: 2^28 nodes x 1000 leapfrog steps = 2.68e11 cell updates) —
+H update eq. (14), E update eq. (12)+(11), Mur, soft source, J update eq. (11), probe records.
+Default workload: BASELINE config 4 in fp64, "the largest single-grid config" the north_star's
+70 % gate names; it fits one GPU (25.8 GB).  The state (6.4 GB) is far larger than the 126 MB L2,
+so every launch streams from HBM ("inputs larger than L2").
+
+  value     whole-job Gcell/s with inputs resident in HBM; CUDA events on the library's stream,
+            barrier + synchronize on both sides, max over ranks.
+  e2e       the same job through the C ABI with HOST buffers: set_media (wp, nu), set_fields (E0)
+            from pinned host memory, rketd_run, read_probes to pinned host memory — all timed.
+  roofline  dominant kernel (K2 temporal blocking): algorithmic bytes per launch (12 arrays x N nodes:
+            read E,H,J + six coefficients, write E,H,J — SURVEY §8(d), 96 B per node and pass in fp64)
+            / average launch duration, against the measured copy bandwidth of MEASURED_PEAKS.json.
+  cpu_baseline  the CPU oracle (oracle/, as it stands) on this host's cores over a bounded sample.
+
+N > 1 (torchrun): the path does not shard (BASELINE: "no multi-GPU sharding") -> N independent
+replicas, no collective on the data path; value = N x replica work / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "cell-updates/sec"
+UNIT = "Gcell/s"
+FALLBACK_HBM_GBS = 6650.0     # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+FP64_LANES_PER_SM = 64        # DFMA per SM per clock (B200: 40 TFLOP/s fp64 / 148 SMs / 1.965 GHz / 2)
+FP32_LANES_PER_SM = 128
+FP_INSTR_PER_CELL_STEP = 9    # H 2, E 4, J 3
+
+
+def make_workload(name: str):
+    from paper_1709_00821_b200 import workloads as wl
+    if name == "config4":
+        return wl.config4()
+    if name == "config2":
+        return wl.config2()
+    if name == "config3":
+        return wl.config3()
+    if name == "config5":
+        return wl.config5()
+    if name == "config1":
+        return wl.config1()
+    if name.startswith("config4:"):          # config4:<log2 cells> (development aid)
+        return wl.config4(ncells=1 << int(name.split(":")[1]))
+    raise SystemExit(f"unknown workload {name}")
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons of one GPU every 100 ms while the timed region runs."""
+
+    def __init__(self, index: int):
+        self.index = index
+        self.samples = []
+        self.reasons = set()
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._thr = None
+        self._nvml = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nvml = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self._nvml = None
+
+    def _poll_nvml(self):
+        p = self._nvml
+        names = {"hw_slowdown": p.nvmlClocksThrottleReasonHwSlowdown,
+                 "hw_thermal_slowdown": p.nvmlClocksThrottleReasonHwThermalSlowdown,
+                 "sw_thermal_slowdown": p.nvmlClocksThrottleReasonSwThermalSlowdown,
+                 "sw_power_cap": p.nvmlClocksThrottleReasonSwPowerCap,
+                 "hw_power_brake": p.nvmlClocksThrottleReasonHwPowerBrakeSlowdown}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(p.nvmlDeviceGetClockInfo(self._h, p.NVML_CLOCK_SM))
+                r = p.nvmlDeviceGetCurrentClocksThrottleReasons(self._h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def _poll_smi(self):
+        q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+            "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+        keys = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={q}",
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                f = [x.strip() for x in out.strip().split(",")]
+                self.samples.append(int(f[0]))
+                self.max_mhz = int(f[1])
+                for k, v in zip(keys, f[2:]):
+                    if v.lower().startswith("active"):
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            self._stop.wait(0.2)
+
+    def __enter__(self):
+        self._thr = threading.Thread(target=self._poll_nvml if self._nvml else self._poll_smi, daemon=True)
+        self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self._thr.join(timeout=10)
+
+    def summary(self):
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2] if s else None, "sm_min_mhz": s[0] if s else None,
+                "sm_max_mhz": self.max_mhz, "samples": len(s), "reasons": sorted(self.reasons)}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as fh:
+            d = json.load(fh)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, torch copy)", float(d.get("sm_max_mhz", 1965.0))
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)", 1965.0
+
+
+def cpu_baseline(w, target_updates_serial=6e8, target_updates_omp=2.5e9):
+    """The oracle as it stands (S0 coefficient setup included — it is part of oracle_run), serial and
+    OpenMP builds, on a prefix / subset of the same workload."""
+    import oracle
+    oracle.build()
+    cores = os.cpu_count() or 1
+    out = {}
+    for omp, target in ((False, target_updates_serial), (True, target_updates_omp)):
+        if w.nbatch == 1:
+            steps = min(w.nsteps, 200)
+            cells = int(min(w.ncells, max(4096, target // steps)))
+            lo = max(0, w.src_cell - cells // 2)
+            lo = min(lo, w.ncells - cells)
+            kw = dict(cells=(lo, lo + cells))
+            sample = f"nodes {lo}..{lo + cells - 1} of the {w.ncells}-node line x {steps} steps"
+            units = cells * steps
+        else:
+            steps = min(w.nsteps, 2000)
+            nb = int(max(cores if omp else 1, min(w.nbatch, target // (steps * w.ncells))))
+            kw = dict(b0=0, b1=nb)
+            sample = f"grids 0..{nb - 1} of {w.nbatch} x {w.ncells} nodes x {steps} steps"
+            units = nb * w.ncells * steps
+        t0 = time.perf_counter()
+        oracle.run_workload(w, nsteps=steps, omp=omp, **kw)
+        dt = time.perf_counter() - t0
+        out["omp" if omp else "serial"] = (units / dt / 1e9, sample, dt)
+    return {"value": out["omp"][0], "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": out["omp"][1] + f" (OpenMP build, {cores} threads, {out['omp'][2]:.1f} s)",
+            "serial_value": out["serial"][0],
+            "serial_sample": out["serial"][1] + f" (serial build, 1 thread, {out['serial'][2]:.1f} s)"}
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on this host's cores, same metric/config, bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    oracle.build()
+    w = make_workload(args.workload)
+    cores = os.cpu_count() or 1
+    if w.nbatch == 1:
+        steps = 100
+        cells = min(w.ncells, 1 << 22)
+        lo = min(max(0, w.src_cell - cells // 2), w.ncells - cells)
+        kw = dict(cells=(lo, lo + cells))
+        sample = f"nodes {lo}..{lo + cells - 1} of the {w.ncells}-node line x {steps} leapfrog steps per bench step"
+        units = cells * steps
+    else:
+        steps = 500
+        nb = min(w.nbatch, max(cores, 64))
+        kw = dict(b0=0, b1=nb)
+        sample = f"grids 0..{nb - 1} of {w.nbatch} x {w.ncells} nodes x {steps} leapfrog steps per bench step"
+        units = nb * w.ncells * steps
+    for _ in range(args.warmup):
+        oracle.run_workload(w, nsteps=steps, omp=True, **kw)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.run_workload(w, nsteps=steps, omp=True, **kw)
+    dt = time.perf_counter() - t0
+    val = units * args.steps / dt / 1e9
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "ncells": w.ncells, "nbatch": w.nbatch, "nsteps_per_run": w.nsteps,
+                       "note": "CPU oracle (OpenMP build) on a bounded sample of the workload"},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="config4")
+    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--kernel", type=int, default=0)
+    ap.add_argument("--depth", type=int, default=0)
+    ap.add_argument("--variant", type=int, default=-1)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: librketd has no CPU fallback")
+    from paper_1709_00821_b200 import rketd      # raises if librketd.so is missing
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    w = make_workload(args.workload)
+    esize = 8 if args.dtype == "f64" else 4
+    npdt = np.float64 if args.dtype == "f64" else np.float32
+    stream = torch.cuda.current_stream()
+
+    # ---- inputs: seeded synthetic (workloads.py), generated on the host, uploaded once -------------------
+    wp, nu = w.media_full()
+    E0 = w.initial_E_full()
+    wp_d = torch.from_numpy(np.ascontiguousarray(wp)).cuda()
+    nu_d = torch.from_numpy(np.ascontiguousarray(nu)).cuda()
+    E0_d = None if E0 is None else torch.from_numpy(np.ascontiguousarray(E0, npdt)).cuda()
+
+    sim = rketd.Sim(w.ncells, w.nbatch, w.dz, w.dt, args.dtype, stream=stream.cuda_stream)
+    sim.set_media(wp_d, nu_d)
+    del wp_d, nu_d
+    torch.cuda.empty_cache()
+    if E0_d is not None:
+        sim.set_fields(E=E0_d)
+    sim.set_source(w.src_kind, w.src_params, w.src_cell)
+    sim.set_probes(w.probes)
+    if w.dft_freqs is not None:
+        sim.set_probe_dft(w.dft_freqs)
+    sim.set_plan(args.kernel, args.depth, args.variant)
+
+    units_per_step = w.ncells * w.nbatch * w.nsteps        # cell updates per bench step (per replica)
+
+    def one_step():
+        sim.run(w.nsteps)
+        if w.dft_freqs is None:
+            sim.discard_records()
+
+    for _ in range(args.warmup):
+        one_step()
+    barrier()
+    l0, sl0 = sim.counter(rketd.CTR_LAUNCHES), sim.counter(rketd.CTR_STEP_LAUNCHES)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as clk:
+        ev0.record(stream)
+        for _ in range(args.steps):
+            one_step()
+        ev1.record(stream)
+        barrier()
+    ms = ev0.elapsed_time(ev1)
+    launches = sim.counter(rketd.CTR_LAUNCHES) - l0
+    step_launches = sim.counter(rketd.CTR_STEP_LAUNCHES) - sl0
+    kernel_used = sim.counter(rketd.CTR_KERNEL_USED)
+    depth = sim.counter(rketd.CTR_DEPTH_USED)
+    tile_cells, halo_cells = sim.counter(rketd.CTR_TILE_CELLS), sim.counter(rketd.CTR_HALO_CELLS)
+    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t.item())
+    value = world * units_per_step * args.steps / (ms * 1e-3) / 1e9
+
+    # ---- roofline of the dominant kernel (the stencil kernel: K2 / K3 / K1) -----------------------------------
+    hbm_gbs, peak_src, sm_max = measured_peaks()
+    ncell_total = w.ncells * w.nbatch
+    ms_per_launch = ms / max(1, step_launches)             # launches are back to back on one stream
+    lanes = FP64_LANES_PER_SM if args.dtype == "f64" else FP32_LANES_PER_SM
+    clocks = clk.summary()
+    r_alu = 148 * lanes * (sm_max * 1e6) / FP_INSTR_PER_CELL_STEP / 1e9            # Gcell/s at max clock
+    r_hbm1 = hbm_gbs / (12 * esize)                                                 # Gcell/s, one step per pass
+    if kernel_used == rketd.KERNEL_RESIDENT:
+        roof = {"bound": "alu", "achieved": value / world, "peak": r_alu, "unit": UNIT, "frac": value / world / r_alu,
+                "traffic": None,
+                "note": "grid resident on chip for the whole run: HBM traffic is setup + probe records only; "
+                        f"peak = 148 SMs x {lanes} FMA lanes x {sm_max:.0f} MHz / 9 instr per cell-step"}
+    else:
+        alg_bytes = 12 * esize * ncell_total                                        # per launch (one pass)
+        achieved = alg_bytes / (ms_per_launch * 1e-3) / 1e9
+        roof = {"bound": "hbm", "achieved": achieved, "peak": hbm_gbs, "unit": "GB/s", "frac": achieved / hbm_gbs,
+                "traffic": None, "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": alg_bytes, "ms_per_launch": ms_per_launch,
+                "depth_T": depth, "tile_cells": tile_cells, "halo_cells": halo_cells,
+                "frac_vs_8TBps_nominal": achieved / 8000.0,
+                "gcells_vs_one_step_hbm_roofline": value / world / r_hbm1,
+                "alu_frac": (value / world) * (tile_cells / max(1, tile_cells - 2 * halo_cells)) / r_alu,
+                "note": "achieved = 12 arrays x nodes x esize per pass / mean launch time; every byte serves depth_T "
+                        "steps; alu_frac counts the redundant halo work against 148 x lanes x max clock / 9"}
+
+    # ---- end to end through the C ABI with host buffers ----------------------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        wp_h = torch.from_numpy(np.ascontiguousarray(wp)).pin_memory()
+        nu_h = torch.from_numpy(np.ascontiguousarray(nu)).pin_memory()
+        E0_h = None if E0 is None else torch.from_numpy(np.ascontiguousarray(E0, npdt)).pin_memory()
+        nser = w.nbatch * len(w.probes)
+        nout = len(w.dft_freqs) if w.dft_freqs is not None else w.nsteps
+        out_h = torch.empty((nser, nout), dtype=torch.float64 if args.dtype == "f64" else torch.float32).pin_memory()
+        h2d = wp_h.numel() * 8 + nu_h.numel() * 8 + (0 if E0_h is None else E0_h.numel() * esize)
+        d2h = out_h.numel() * esize
+
+        def e2e_step():
+            sim.reset()
+            sim.set_media(wp_h, nu_h)
+            sim.set_fields(E=E0_h)
+            sim.run(w.nsteps)
+            sim.read_probes(out_h)
+
+        e2e_step()
+        barrier()
+        t0 = time.perf_counter()
+        nrep = max(1, min(args.steps, 3))
+        for _ in range(nrep):
+            e2e_step()
+        barrier()
+        dt = time.perf_counter() - t0
+        tt = torch.tensor([dt], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        dt = float(tt.item())
+        e2e = {"value": world * units_per_step * nrep / dt / 1e9, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(d2h), "steps": nrep,
+               "note": "set_media(wp, nu) + set_fields(E0) from pinned host, rketd_run, read_probes to pinned host"}
+        del wp_h, nu_h, E0_h, out_h
+    sim.close()
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        cpu = cpu_baseline(w)
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": args.dtype, "data": "synthetic",
+                "config": {"workload": w.name, "ncells": w.ncells, "nbatch": w.nbatch, "nsteps_per_run": w.nsteps,
+                           "cell_updates_per_step": units_per_step, "kernel": int(kernel_used), "depth_T": int(depth),
+                           "l2": "inputs larger than L2 (state+coefficients %.1f GB)" % (12 * esize * ncell_total / 1e9)
+                           if kernel_used != rketd.KERNEL_RESIDENT else "state resident on chip; no HBM re-reads to flush",
+                           "parallelism": "replicas only (the path does not shard)" if world > 1 else "single GPU"},
+                "clocks": clocks, "roofline": roof, "e2e": e2e, "cpu_baseline": cpu,
+                "gpu_launches": int(launches), "stencil_launches": int(step_launches)}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

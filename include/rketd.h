@@ -95,6 +95,11 @@ int rketd_set_fields(rketd_sim *s, const void *E, const void *H, const void *J);
  * probes kept. */
 int rketd_reset(rketd_sim *s);
 
+/* Drop the probe records (time-series chunks) and zero the DFT accumulators gathered so far; fields,
+ * step counter, media, source and probes are kept.  The next rketd_run starts a fresh record.
+ * Synchronises (device buffers are freed). */
+int rketd_discard_records(rketd_sim *s);
+
 /* Choose the kernel (RKETD_KERNEL_*), for K2 the temporal depth T (0 = default), and the launch
  * variant of K2/K3 (-1 = default; K2: 0..3 = CTA tiles with {nodes per thread, threads per CTA} combinations, 4..5 = warp tiles,
  * K3: 0 = a thread owns a 64-B row, 1 = half a row).  All choices compute identical bits.

@@ -425,6 +425,13 @@ int rketd_reset(rketd_sim *s) {
   return RKETD_OK;
 }
 
+int rketd_discard_records(rketd_sim *s) {
+  if (!s) return RKETD_EINVAL;
+  CU_TRY(s, cudaStreamSynchronize(s->stream));
+  discard_records(s);
+  return RKETD_OK;
+}
+
 int rketd_set_plan(rketd_sim *s, int kernel, int depth, int variant) {
   if (!s) return RKETD_EINVAL;
   if (kernel < RKETD_KERNEL_AUTO || kernel > RKETD_KERNEL_RESIDENT || depth < 0) return fail(s, RKETD_EINVAL, "rketd_set_plan: bad argument");

@@ -24,7 +24,7 @@ CTR_LAUNCHES, CTR_STEP_LAUNCHES, CTR_KERNEL_USED, CTR_DEPTH_USED, CTR_STEPS_DONE
     CTR_HALO_CELLS, CTR_STATE_BYTES = range(8)
 
 EXPORTS = ["rketd_create", "rketd_set_media", "rketd_set_source", "rketd_set_probes", "rketd_set_probe_dft",
-           "rketd_set_fields", "rketd_reset", "rketd_set_plan", "rketd_run", "rketd_read_probes",
+           "rketd_set_fields", "rketd_reset", "rketd_discard_records", "rketd_set_plan", "rketd_run", "rketd_read_probes",
            "rketd_get_fields", "rketd_get_coefficients", "rketd_get_counter", "rketd_destroy", "rketd_last_error"]
 
 if not os.path.exists(LIB_PATH):
@@ -40,6 +40,7 @@ _lib.rketd_set_probes.argtypes = [_vp, _vp, _i32]
 _lib.rketd_set_probe_dft.argtypes = [_vp, _vp, _i32]
 _lib.rketd_set_fields.argtypes = [_vp, _vp, _vp, _vp]
 _lib.rketd_reset.argtypes = [_vp]
+_lib.rketd_discard_records.argtypes = [_vp]
 _lib.rketd_set_plan.argtypes = [_vp, _i32, _i32, _i32]
 _lib.rketd_run.argtypes = [_vp, _i64]
 _lib.rketd_read_probes.argtypes = [_vp, _vp, _i64, ctypes.POINTER(_i64)]
@@ -51,7 +52,7 @@ _lib.rketd_destroy.argtypes = [_vp]
 _lib.rketd_destroy.restype = None
 _lib.rketd_last_error.argtypes = [_vp]
 _lib.rketd_last_error.restype = ctypes.c_char_p
-for _n in EXPORTS[:12]:
+for _n in EXPORTS[:13]:
     getattr(_lib, _n).restype = _i32
 
 
@@ -113,6 +114,10 @@ def rketd_set_fields(h, E=None, H=None, J=None):
 
 def rketd_reset(h):
     _check(h, _lib.rketd_reset(h))
+
+
+def rketd_discard_records(h):
+    _check(h, _lib.rketd_discard_records(h))
 
 
 def rketd_set_plan(h, kernel: int = KERNEL_AUTO, depth: int = 0, variant: int = -1):
@@ -189,6 +194,7 @@ class Sim:
 
     def set_fields(self, E=None, H=None, J=None): rketd_set_fields(self.h, E, H, J)
     def reset(self): rketd_reset(self.h)
+    def discard_records(self): rketd_discard_records(self.h)
     def set_plan(self, kernel=KERNEL_AUTO, depth=0, variant=-1): rketd_set_plan(self.h, kernel, depth, variant)
     def run(self, nsteps): rketd_run(self.h, nsteps)
     def counter(self, which): return rketd_get_counter(self.h, which)
