@@ -16,9 +16,10 @@ so every launch streams from HBM ("inputs larger than L2").
             barrier + synchronize on both sides, max over ranks.
   e2e       the same job through the C ABI with HOST buffers: set_media (wp, nu), set_fields (E0)
             from pinned host memory, rketd_run, read_probes to pinned host memory — all timed.
-  roofline  dominant kernel (K2 temporal blocking): algorithmic bytes per launch (12 arrays x N nodes:
-            read E,H,J + six coefficients, write E,H,J — SURVEY §8(d), 96 B per node and pass in fp64)
-            / average launch duration, against the measured copy bandwidth of MEASURED_PEAKS.json.
+  roofline  dominant kernel (K2 temporal blocking): algorithmic bytes per launch (10 arrays x N nodes:
+            read E,H,G + four coefficients P,ch,ka,Q, write E,H,G — 80 B per node and pass in fp64; the
+            plain six-coefficient form of SURVEY §8(d) would be 96 B) / average launch duration, against
+            the measured copy bandwidth of MEASURED_PEAKS.json.
   cpu_baseline  the CPU oracle (oracle/, as it stands) on this host's cores over a bounded sample.
 
 N > 1 (torchrun): the path does not shard (BASELINE: "no multi-GPU sharding") -> N independent
@@ -45,7 +46,8 @@ UNIT = "Gcell/s"
 FALLBACK_HBM_GBS = 6650.0     # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 FP64_LANES_PER_SM = 64        # DFMA per SM per clock (B200: 40 TFLOP/s fp64 / 148 SMs / 1.965 GHz / 2)
 FP32_LANES_PER_SM = 128
-FP_INSTR_PER_CELL_STEP = 9    # H 2, E 4, J 3
+FP_INSTR_PER_CELL_STEP = 7    # kernel form (rketd_device.cuh): H 2, E 3, G 2  (SURVEY §8(d) counts 9 for the plain form)
+ARRAYS_PER_PASS = 10          # read E, H, G, P, ch, ka, Q; write E, H, G
 
 
 def make_workload(name: str):
@@ -313,14 +315,14 @@ def main():
     lanes = FP64_LANES_PER_SM if args.dtype == "f64" else FP32_LANES_PER_SM
     clocks = clk.summary()
     r_alu = 148 * lanes * (sm_max * 1e6) / FP_INSTR_PER_CELL_STEP / 1e9            # Gcell/s at max clock
-    r_hbm1 = hbm_gbs / (12 * esize)                                                 # Gcell/s, one step per pass
+    r_hbm1 = hbm_gbs / (ARRAYS_PER_PASS * esize)                                                 # Gcell/s, one step per pass
     if kernel_used == rketd.KERNEL_RESIDENT:
         roof = {"bound": "alu", "achieved": value / world, "peak": r_alu, "unit": UNIT, "frac": value / world / r_alu,
                 "traffic": None,
                 "note": "grid resident on chip for the whole run: HBM traffic is setup + probe records only; "
-                        f"peak = 148 SMs x {lanes} FMA lanes x {sm_max:.0f} MHz / 9 instr per cell-step"}
+                        f"peak = 148 SMs x {lanes} FMA lanes x {sm_max:.0f} MHz / 7 instr per cell-step"}
     else:
-        alg_bytes = 12 * esize * ncell_total                                        # per launch (one pass)
+        alg_bytes = ARRAYS_PER_PASS * esize * ncell_total                                        # per launch (one pass)
         achieved = alg_bytes / (ms_per_launch * 1e-3) / 1e9
         roof = {"bound": "hbm", "achieved": achieved, "peak": hbm_gbs, "unit": "GB/s", "frac": achieved / hbm_gbs,
                 "traffic": None, "peak_source": peak_src,
@@ -329,8 +331,9 @@ def main():
                 "frac_vs_8TBps_nominal": achieved / 8000.0,
                 "gcells_vs_one_step_hbm_roofline": value / world / r_hbm1,
                 "alu_frac": (value / world) * (tile_cells / max(1, tile_cells - 2 * halo_cells)) / r_alu,
-                "note": "achieved = 12 arrays x nodes x esize per pass / mean launch time; every byte serves depth_T "
-                        "steps; alu_frac counts the redundant halo work against 148 x lanes x max clock / 9"}
+                "note": "achieved = 10 arrays (read E,H,G,P,ch,ka,Q; write E,H,G) x nodes x esize per pass / mean launch "
+                        "time; every byte serves depth_T steps; alu_frac counts the redundant halo work against "
+                        "148 SMs x lanes x max clock / 7 instr per cell-step"}
 
     # ---- end to end through the C ABI with host buffers ----------------------------------------------------
     e2e = None
@@ -379,7 +382,7 @@ def main():
                 "dtype": args.dtype, "data": "synthetic",
                 "config": {"workload": w.name, "ncells": w.ncells, "nbatch": w.nbatch, "nsteps_per_run": w.nsteps,
                            "cell_updates_per_step": units_per_step, "kernel": int(kernel_used), "depth_T": int(depth),
-                           "l2": "inputs larger than L2 (state+coefficients %.1f GB)" % (12 * esize * ncell_total / 1e9)
+                           "l2": "inputs larger than L2 (state+coefficients %.1f GB)" % (ARRAYS_PER_PASS * esize * ncell_total / 1e9)
                            if kernel_used != rketd.KERNEL_RESIDENT else "state resident on chip; no HBM re-reads to flush",
                            "parallelism": "replicas only (the path does not shard)" if world > 1 else "single GPU"},
                 "clocks": clocks, "roofline": roof, "e2e": e2e, "cpu_baseline": cpu,

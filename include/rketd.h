@@ -64,11 +64,12 @@ int rketd_create(rketd_sim **out, int64_t ncells, int64_t nbatch, double dz, dou
                  void *cuda_stream);
 
 /* Per-node plasma frequency wp [rad/s] and collision frequency nu [1/s], always fp64,
- * [nbatch][ncells], host or device.  Precomputes (in fp64, on the device) the six per-node
+ * [nbatch][ncells], host or device.  Precomputes (in fp64, on the device) the per-node
  * coefficients of SURVEY §8(a) row a0, i.e. eq. (11) PAPER.md:68 written as
  * J' = ka J + kb E + kc E' and eq. (12) PAPER.md:74 with (11) substituted, solved for E'
- * (eq. (13) PAPER.md:79 with the missing 1/D restored): E' = ca E - cj J - ch (H[k]-H[k-1]).
- * EINVAL: any wp or nu negative or non-finite.  Synchronises the stream. */
+ * (eq. (13) PAPER.md:79 with the missing 1/D restored): E' = ca E - cj J - ch (H[k]-H[k-1]),
+ * and from them the four arrays the kernels read (rketd_get_kernel_coefficients).
+ * The current fields E, H, J are kept.  EINVAL: any wp or nu negative or non-finite.  Synchronises. */
 int rketd_set_media(rketd_sim *s, const double *wp, const double *nu);
 
 /* Soft source added to E^{n+1}[cell] in every grid (eq. (15)).
@@ -101,7 +102,7 @@ int rketd_reset(rketd_sim *s);
 int rketd_discard_records(rketd_sim *s);
 
 /* Choose the kernel (RKETD_KERNEL_*), for K2 the temporal depth T (0 = default), and the launch
- * variant of K2/K3 (-1 = default; K2: 0..3 = CTA tiles with {nodes per thread, threads per CTA} combinations, 4..5 = warp tiles,
+ * variant of K2/K3 (-1 = default; K2: 0..3 = CTA tiles with {nodes per thread, threads per CTA} combinations, 4..7 = warp tiles,
  * K3: 0 = a thread owns a 64-B row, 1 = half a row).  All choices compute identical bits.
  * EINVAL if the choice cannot run this grid (e.g. RESIDENT with a grid larger than one CTA). */
 int rketd_set_plan(rketd_sim *s, int kernel, int depth, int variant);
@@ -121,9 +122,16 @@ int rketd_read_probes(rketd_sim *s, void *out, int64_t out_bytes, int64_t *nsamp
  * Synchronises. */
 int rketd_get_fields(rketd_sim *s, void *E, void *H, void *J);
 
-/* Copy the six coefficient arrays out as fp64, order ca, cj, ch, ka, kb, kc:
- * out[6][nbatch][ncells] (host or device); chh_m[2] = {dt/(mu0 dz), Mur m} (host; may be NULL). */
+/* The six coefficients of SURVEY a0 as fp64, order ca, cj, ch, ka, kb, kc (E' = ca E - cj J - ch dH,
+ * J' = ka J + kb E + kc E'), computed on the device from the media: out[6][nbatch][ncells] (host or
+ * device); chh_m[2] = {dt/(mu0 dz), Mur m} (host; may be NULL). */
 int rketd_get_coefficients(rketd_sim *s, double *out, double *chh_m);
+
+/* The four per-node coefficient arrays the stencil kernels actually read, converted to fp64, order
+ * P = ca - cj kc, ch, ka, Q = ka cj kc + cj kb (the kernels carry G = cj J - cj kc E in place of J, for
+ * which E' = P E - G - ch dH and G' = ka G + Q E hold exactly):
+ * out[4][nbatch][ncells] (host or device).  In fp32 mode these are the fp64 values rounded once. */
+int rketd_get_kernel_coefficients(rketd_sim *s, double *out);
 
 /* RKETD_CTR_* counters (for bench.py's gpu_launches and roofline bookkeeping). */
 int64_t rketd_get_counter(const rketd_sim *s, int which);

@@ -29,10 +29,13 @@ struct rketd_sim {
   cudaStream_t stream = nullptr;
   void *fld[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};
   int cur = 0;
-  void *coef[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+  void *coef[kNumCoefArrays] = {nullptr, nullptr, nullptr, nullptr};   // P, ch, ka, Q (rketd_device.cuh)
+  double *wp_p = nullptr, *nu_p = nullptr;                              // media in the padded layout, fp64
   uint8_t *rowflag = nullptr;
   bool flags_dirty = true;
   bool have_media = false;
+  bool fields_zero = true;      // E = H = J = 0 (after create / reset): no J <-> G conversion needed
+  bool third_is_J = false;      // the third field array holds J, not G (fields set before the media)
   int *d_bad = nullptr;
   int src_kind = RKETD_SRC_NONE;
   std::vector<double> src_params;
@@ -68,6 +71,12 @@ int fail(rketd_sim *s, int code, const std::string &msg) {
   } while (0)
 
 size_t arr_bytes(const Layout &L) { return (size_t)L.gstride * L.nbatch * L.esize; }
+
+bool is_device_ptr(const void *p) {
+  cudaPointerAttributes at;
+  if (cudaPointerGetAttributes(&at, p) != cudaSuccess) { cudaGetLastError(); return false; }
+  return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
 
 // pack / unpack between the user's [nbatch][ncells] and the padded physical layout
 cudaError_t copy_in(const rketd_sim *s, void *dst_phys, const void *src_user) {
@@ -167,7 +176,7 @@ int make_map(rketd_sim *s, CUtensorMap *m, void *base, int box_rows) {
 }
 
 int default_depth(const rketd_sim *s) { return s->dtype == RKETD_F64 ? 24 : 32; }
-int default_k2_variant(const rketd_sim *) { return 4; }
+int default_k2_variant(const rketd_sim *) { return 6; }
 int default_k3_variant(const rketd_sim *) { return 0; }
 int max_depth(const rketd_sim *s, int variant) { return (k2_tile_rows(variant) / 2 - 1) * s->L.C; }
 
@@ -197,7 +206,7 @@ int build_k2_plan(rketd_sim *s, int depth, int variant) {
       rc = make_map(s, &P.maps[b].st[a], s->fld[1 - b][a], P.rows_out);
       if (rc) return rc;
     }
-    for (int a = 0; a < 6; ++a) {
+    for (int a = 0; a < kNumCoefArrays; ++a) {
       int rc = make_map(s, &P.maps[b].ld[3 + a], s->coef[a], rows);
       if (rc) return rc;
     }
@@ -275,7 +284,8 @@ int run_segment(rketd_sim *s, int64_t nsteps, void *rec) {
     for (int64_t n = 0; n < nsteps; n += depth) {
       const int steps = (int)std::min<int64_t>(depth, nsteps - n);
       sc.n0 = n;
-      CU_TRY(s, launch_k2(s->dtype, L, s->k2, s->cur, sc, steps, s->stream));
+      FieldPtrs dst{s->fld[1 - s->cur][0], s->fld[1 - s->cur][1], s->fld[1 - s->cur][2]};
+      CU_TRY(s, launch_k2(s->dtype, L, s->k2, s->cur, dst, sc, steps, s->stream));
       s->cur ^= 1;
       ++s->ctr_launches; ++s->ctr_step_launches;
     }
@@ -322,13 +332,16 @@ int rketd_create(rketd_sim **out, int64_t ncells, int64_t nbatch, double dz, dou
       if ((e = cudaMalloc(&s->fld[b][a], nb)) != cudaSuccess) return bail(e);
       if ((e = cudaMemsetAsync(s->fld[b][a], 0, nb, s->stream)) != cudaSuccess) return bail(e);
     }
-  for (int a = 0; a < 6; ++a) {
+  for (int a = 0; a < kNumCoefArrays; ++a) {
     if ((e = cudaMalloc(&s->coef[a], nb)) != cudaSuccess) return bail(e);
     if ((e = cudaMemsetAsync(s->coef[a], 0, nb, s->stream)) != cudaSuccess) return bail(e);
   }
+  const size_t nb64 = (size_t)L.gstride * L.nbatch * sizeof(double);
+  if ((e = cudaMalloc(&s->wp_p, nb64)) != cudaSuccess) return bail(e);
+  if ((e = cudaMalloc(&s->nu_p, nb64)) != cudaSuccess) return bail(e);
   if ((e = cudaMalloc(&s->rowflag, (size_t)L.nrows)) != cudaSuccess) return bail(e);
   if ((e = cudaMalloc(&s->d_bad, sizeof(int))) != cudaSuccess) return bail(e);
-  s->state_bytes = (int64_t)nb * 12 + L.nrows;
+  s->state_bytes = (int64_t)nb * (6 + kNumCoefArrays) + 2 * (int64_t)nb64 + L.nrows;
   *out = s;
   return RKETD_OK;
 }
@@ -338,36 +351,51 @@ int rketd_set_media(rketd_sim *s, const double *wp, const double *nu) {
   const Layout &L = s->L;
   const size_t n = (size_t)L.ncells * L.nbatch * sizeof(double);
   const double *dwp = wp, *dnu = nu;
-  void *twp = nullptr, *tnu = nullptr;
-  auto is_device = [](const void *p) {
-    cudaPointerAttributes at;
-    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) { cudaGetLastError(); return false; }
-    return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
-  };
-  if (!is_device(wp)) {
-    CU_TRY(s, cudaMalloc(&twp, n));
-    CU_TRY(s, cudaMemcpyAsync(twp, wp, n, cudaMemcpyDefault, s->stream));
+  void *twp = nullptr, *tnu = nullptr, *tJ = nullptr;
+  auto cleanup = [&]() { if (twp) cudaFree(twp); if (tnu) cudaFree(tnu); if (tJ) cudaFree(tJ); };
+#define SM_TRY(expr) do { cudaError_t sm_e = (expr); if (sm_e != cudaSuccess) { cleanup(); CU_TRY(s, sm_e); } } while (0)
+  // live fields carry G = cj J - cj kc E of the OLD media: take J out before the coefficients change
+  const bool reconvert = s->have_media && !s->fields_zero && !s->third_is_J;
+  if (reconvert) {
+    SM_TRY(cudaMalloc(&tJ, (size_t)L.ncells * L.nbatch * L.esize));
+    SM_TRY(launch_G_to_current(s->dtype, L, s->wp_p, s->nu_p, s->dz, s->dt, s->fld[s->cur][0], s->fld[s->cur][2], tJ,
+                               s->stream));
+    ++s->ctr_launches;
+  }
+  if (!is_device_ptr(wp)) {
+    SM_TRY(cudaMalloc(&twp, n));
+    SM_TRY(cudaMemcpyAsync(twp, wp, n, cudaMemcpyDefault, s->stream));
     dwp = (const double *)twp;
   }
-  if (!is_device(nu)) {
-    cudaError_t e = cudaMalloc(&tnu, n);
-    if (e != cudaSuccess) { if (twp) cudaFree(twp); CU_TRY(s, e); }
-    CU_TRY(s, cudaMemcpyAsync(tnu, nu, n, cudaMemcpyDefault, s->stream));
+  if (!is_device_ptr(nu)) {
+    SM_TRY(cudaMalloc(&tnu, n));
+    SM_TRY(cudaMemcpyAsync(tnu, nu, n, cudaMemcpyDefault, s->stream));
     dnu = (const double *)tnu;
   }
-  cudaMemsetAsync(s->d_bad, 0, sizeof(int), s->stream);
-  cudaError_t e = launch_coefficients(s->dtype, L, dwp, dnu, s->dz, s->dt, s->coef, s->d_bad, s->stream);
+  SM_TRY(cudaMemsetAsync(s->d_bad, 0, sizeof(int), s->stream));
+  SM_TRY(launch_coefficients(s->dtype, L, dwp, dnu, s->dz, s->dt, s->wp_p, s->nu_p, s->coef, s->d_bad, s->stream));
   ++s->ctr_launches;
   int bad = 0;
-  if (e == cudaSuccess) e = cudaMemcpyAsync(&bad, s->d_bad, sizeof(int), cudaMemcpyDeviceToHost, s->stream);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
-  if (twp) cudaFree(twp);
-  if (tnu) cudaFree(tnu);
-  CU_TRY(s, e);
+  SM_TRY(cudaMemcpyAsync(&bad, s->d_bad, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
+  SM_TRY(cudaStreamSynchronize(s->stream));
   if (bad) {
+    cleanup();
     s->have_media = false;
     return fail(s, RKETD_EINVAL, "rketd_set_media: wp and nu must be finite and non-negative");
   }
+  if (reconvert) {
+    SM_TRY(cudaMemsetAsync(s->fld[s->cur][2], 0, arr_bytes(L), s->stream));
+    SM_TRY(copy_in(s, s->fld[s->cur][2], tJ));
+  }
+  if (reconvert || s->third_is_J) {
+    SM_TRY(launch_current_to_G(s->dtype, L, s->wp_p, s->nu_p, s->dz, s->dt, s->fld[s->cur][0], s->fld[s->cur][2],
+                               s->stream));
+    ++s->ctr_launches;
+    SM_TRY(cudaStreamSynchronize(s->stream));
+  }
+#undef SM_TRY
+  cleanup();
+  s->third_is_J = false;
   s->have_media = true;
   return RKETD_OK;
 }
@@ -413,6 +441,17 @@ int rketd_set_fields(rketd_sim *s, const void *E, const void *H, const void *J) 
     CU_TRY(s, cudaMemsetAsync(s->fld[s->cur][a], 0, arr_bytes(s->L), s->stream));
     if (src[a]) CU_TRY(s, copy_in(s, s->fld[s->cur][a], src[a]));
   }
+  s->fields_zero = !E && !H && !J;
+  s->third_is_J = false;
+  if (E || J) {   // the kernels carry G = cj J - cj kc E in the third array (rketd_device.cuh)
+    if (s->have_media) {
+      CU_TRY(s, launch_current_to_G(s->dtype, s->L, s->wp_p, s->nu_p, s->dz, s->dt, s->fld[s->cur][0], s->fld[s->cur][2],
+                                    s->stream));
+      ++s->ctr_launches;
+    } else {
+      s->third_is_J = true;   // converted by rketd_set_media
+    }
+  }
   CU_TRY(s, cudaStreamSynchronize(s->stream));
   return RKETD_OK;
 }
@@ -422,6 +461,8 @@ int rketd_reset(rketd_sim *s) {
   for (int a = 0; a < 3; ++a) CU_TRY(s, cudaMemsetAsync(s->fld[s->cur][a], 0, arr_bytes(s->L), s->stream));
   discard_records(s);
   s->step = 0;
+  s->fields_zero = true;
+  s->third_is_J = false;
   return RKETD_OK;
 }
 
@@ -454,6 +495,7 @@ int rketd_run(rketd_sim *s, int64_t nsteps) {
   if (!s->have_media) return fail(s, RKETD_ESTATE, "rketd_run before rketd_set_media");
   if (nsteps == 0) return RKETD_OK;
   if (s->flags_dirty) { int rc = rebuild_rowflags(s); if (rc) return rc; }
+  s->fields_zero = false;
   const Layout &L = s->L;
   const int64_t nseries = L.nbatch * (int64_t)s->probes.size();
   if (nseries == 0) return run_segment(s, nsteps, nullptr);
@@ -526,10 +568,26 @@ int rketd_read_probes(rketd_sim *s, void *out, int64_t out_bytes, int64_t *nsamp
 
 int rketd_get_fields(rketd_sim *s, void *E, void *H, void *J) {
   if (!s) return RKETD_EINVAL;
-  void *dst[3] = {E, H, J};
-  for (int a = 0; a < 3; ++a)
-    if (dst[a]) CU_TRY(s, copy_out(s, dst[a], s->fld[s->cur][a]));
-  CU_TRY(s, cudaStreamSynchronize(s->stream));
+  if (E) CU_TRY(s, copy_out(s, E, s->fld[s->cur][0]));
+  if (H) CU_TRY(s, copy_out(s, H, s->fld[s->cur][1]));
+  void *tmp = nullptr;
+  if (J) {
+    if (!s->have_media || s->third_is_J) {   // nothing has run yet: the array still holds J itself
+      CU_TRY(s, copy_out(s, J, s->fld[s->cur][2]));
+    } else {                                 // J = (G + cj kc E)/cj
+      const size_t n = (size_t)s->L.ncells * s->L.nbatch * s->L.esize;
+      void *dst = J;
+      if (!is_device_ptr(J)) { CU_TRY(s, cudaMalloc(&tmp, n)); dst = tmp; }
+      cudaError_t e = launch_G_to_current(s->dtype, s->L, s->wp_p, s->nu_p, s->dz, s->dt, s->fld[s->cur][0],
+                                          s->fld[s->cur][2], dst, s->stream);
+      ++s->ctr_launches;
+      if (e == cudaSuccess && tmp) e = cudaMemcpyAsync(J, tmp, n, cudaMemcpyDefault, s->stream);
+      if (e != cudaSuccess) { if (tmp) cudaFree(tmp); CU_TRY(s, e); }
+    }
+  }
+  const cudaError_t e = cudaStreamSynchronize(s->stream);
+  if (tmp) cudaFree(tmp);
+  CU_TRY(s, e);
   return RKETD_OK;
 }
 
@@ -539,7 +597,7 @@ int rketd_get_coefficients(rketd_sim *s, double *out, double *chh_m) {
   const size_t n = (size_t)6 * s->L.ncells * s->L.nbatch * sizeof(double);
   void *tmp = nullptr;
   CU_TRY(s, cudaMalloc(&tmp, n));
-  cudaError_t e = launch_unpack_coefficients(s->dtype, s->L, s->coef, (double *)tmp, s->stream);
+  cudaError_t e = launch_six_coefficients(s->L, s->wp_p, s->nu_p, s->dz, s->dt, (double *)tmp, s->stream);
   ++s->ctr_launches;
   if (e == cudaSuccess) e = cudaMemcpyAsync(out, tmp, n, cudaMemcpyDefault, s->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
@@ -550,6 +608,21 @@ int rketd_get_coefficients(rketd_sim *s, double *out, double *chh_m) {
     const double S = kC0 * s->dt / s->dz;
     chh_m[1] = (S - 1.0) / (S + 1.0);
   }
+  return RKETD_OK;
+}
+
+int rketd_get_kernel_coefficients(rketd_sim *s, double *out) {
+  if (!s || !out) return fail(s, RKETD_EINVAL, "rketd_get_kernel_coefficients: NULL argument");
+  if (!s->have_media) return fail(s, RKETD_ESTATE, "rketd_get_kernel_coefficients before rketd_set_media");
+  const size_t n = (size_t)kNumCoefArrays * s->L.ncells * s->L.nbatch * sizeof(double);
+  void *tmp = nullptr;
+  CU_TRY(s, cudaMalloc(&tmp, n));
+  cudaError_t e = launch_unpack_coefficients(s->dtype, s->L, s->coef, (double *)tmp, s->stream);
+  ++s->ctr_launches;
+  if (e == cudaSuccess) e = cudaMemcpyAsync(out, tmp, n, cudaMemcpyDefault, s->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+  cudaFree(tmp);
+  CU_TRY(s, e);
   return RKETD_OK;
 }
 
@@ -574,8 +647,10 @@ void rketd_destroy(rketd_sim *s) {
   for (int b = 0; b < 2; ++b)
     for (int a = 0; a < 3; ++a)
       if (s->fld[b][a]) cudaFree(s->fld[b][a]);
-  for (int a = 0; a < 6; ++a)
+  for (int a = 0; a < kNumCoefArrays; ++a)
     if (s->coef[a]) cudaFree(s->coef[a]);
+  if (s->wp_p) cudaFree(s->wp_p);
+  if (s->nu_p) cudaFree(s->nu_p);
   if (s->rowflag) cudaFree(s->rowflag);
   if (s->d_bad) cudaFree(s->d_bad);
   if (s->d_srctab) cudaFree(s->d_srctab);

@@ -1,6 +1,6 @@
 // rketd_aux.cu — setup and post-processing kernels of librketd:
 //   coefficient precompute (eqs. (11), (13) PAPER.md:68, :79),
-//   coefficient read-back, DFT twiddles / accumulation / magnitude (row a7, BASELINE config 5).
+//   coefficient read-back, the J <-> G change of variable at the boundary, DFT twiddles / accumulation / magnitude (row a7, BASELINE config 5).
 #include <math_constants.h>
 
 #include "rketd_internal.h"
@@ -33,72 +33,152 @@ __device__ __forceinline__ void phi_functions(double x, double &p1, double &p2) 
   }
 }
 
+// The six coefficients of SURVEY a0 for one node, in fp64 with explicit round-to-nearest operations.
+struct Six { double ca, cj, ch, ka, kb, kc; };
+__device__ __forceinline__ Six six_coefficients(double w, double v, double dz, double dt, double eps0) {
+  const double x = __dmul_rn(v, dt);
+  const double a = exp(-x);
+  double p1, p2;
+  phi_functions(x, p1, p2);
+  const double beta = __dmul_rn(dt, p1);              // (1 - a)/nu
+  const double gamma = __dmul_rn(dt, p2);             // (a - 1 + nu dt)/(nu^2 dt)
+  const double w2 = __dmul_rn(w, w);
+  const double b = __dmul_rn(__dmul_rn(eps0, w2), beta);
+  const double c = __dmul_rn(__dmul_rn(eps0, w2), gamma);
+  const double D = __dadd_rn(1.0, __ddiv_rn(__dmul_rn(__dmul_rn(w2, gamma), dt), 2.0));
+  Six s;
+  s.ca = __dsub_rn(1.0, __ddiv_rn(__ddiv_rn(__dmul_rn(__dmul_rn(w2, beta), dt), 2.0), D));
+  s.cj = __ddiv_rn(__dmul_rn(__ddiv_rn(dt, __dmul_rn(2.0, eps0)), __dadd_rn(1.0, a)), D);
+  s.ch = __ddiv_rn(__ddiv_rn(dt, __dmul_rn(eps0, dz)), D);
+  s.ka = a;
+  s.kb = __dsub_rn(b, c);
+  s.kc = c;
+  return s;
+}
+
+// a0: pads the media into the physical layout and derives the four per-node coefficients the stencil
+// kernels use (rketd_device.cuh): P = ca - cj kc, ch, ka, Q = ka (cj kc) + cj kb; padding nodes get zeros.
 template <typename R>
 __global__ void coefficients_kernel(Layout L, const double *__restrict__ wp, const double *__restrict__ nu,
-                                    double dz, double dt, double eps0, R *ca, R *cj, R *ch, R *ka, R *kb, R *kc,
-                                    int *bad) {
+                                    double dz, double dt, double eps0, double *wp_p, double *nu_p, R *cP, R *cch, R *cka,
+                                    R *cQ, int *bad) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= L.gstride * L.nbatch) return;
   const int64_t g = idx / L.gstride, kp = idx - g * L.gstride, k = kp - L.off;
-  double vca = 0, vcj = 0, vch = 0, vka = 0, vkb = 0, vkc = 0;     // padding nodes: all zero
+  double vP = 0, vch = 0, vka = 0, vQ = 0, w = 0, v = 0;     // padding nodes: all zero
   if (k >= 0 && k < L.ncells) {
-    const double w = wp[g * L.ncells + k], v = nu[g * L.ncells + k];
+    w = wp[g * L.ncells + k];
+    v = nu[g * L.ncells + k];
     if (!(w >= 0.0) || !(v >= 0.0) || isinf(w) || isinf(v)) atomicOr(bad, 1);
-    const double x = __dmul_rn(v, dt);
-    const double a = exp(-x);
-    double p1, p2;
-    phi_functions(x, p1, p2);
-    const double beta = __dmul_rn(dt, p1);              // (1 - a)/nu
-    const double gamma = __dmul_rn(dt, p2);             // (a - 1 + nu dt)/(nu^2 dt)
-    const double w2 = __dmul_rn(w, w);
-    const double b = __dmul_rn(__dmul_rn(eps0, w2), beta);
-    const double c = __dmul_rn(__dmul_rn(eps0, w2), gamma);
-    const double D = __dadd_rn(1.0, __ddiv_rn(__dmul_rn(__dmul_rn(w2, gamma), dt), 2.0));
-    vca = __dsub_rn(1.0, __ddiv_rn(__ddiv_rn(__dmul_rn(__dmul_rn(w2, beta), dt), 2.0), D));
-    vcj = __ddiv_rn(__dmul_rn(__ddiv_rn(dt, __dmul_rn(2.0, eps0)), __dadd_rn(1.0, a)), D);
-    vch = __ddiv_rn(__ddiv_rn(dt, __dmul_rn(eps0, dz)), D);
-    vka = a;
-    vkb = __dsub_rn(b, c);
-    vkc = c;
+    const Six s = six_coefficients(w, v, dz, dt, eps0);
+    const double kcp = __dmul_rn(s.cj, s.kc), kbp = __dmul_rn(s.cj, s.kb);
+    vP = __dsub_rn(s.ca, kcp);
+    vch = s.ch;
+    vka = s.ka;
+    vQ = __dadd_rn(__dmul_rn(s.ka, kcp), kbp);
   }
-  ca[idx] = (R)vca; cj[idx] = (R)vcj; ch[idx] = (R)vch;
-  ka[idx] = (R)vka; kb[idx] = (R)vkb; kc[idx] = (R)vkc;
+  wp_p[idx] = w; nu_p[idx] = v;
+  cP[idx] = (R)vP; cch[idx] = (R)vch; cka[idx] = (R)vka; cQ[idx] = (R)vQ;
 }
 
 cudaError_t launch_coefficients(int dtype, const Layout &L, const double *wp, const double *nu, double dz,
-                                double dt, void *const coef[6], int *d_bad, cudaStream_t st) {
+                                double dt, double *wp_p, double *nu_p, void *const coef[kNumCoefArrays], int *d_bad,
+                                cudaStream_t st) {
   const int64_t total = L.gstride * L.nbatch;
   const unsigned blocks = (unsigned)((total + 255) / 256);
   if (dtype == 0)
-    coefficients_kernel<double><<<blocks, 256, 0, st>>>(L, wp, nu, dz, dt, kEps0, (double *)coef[0], (double *)coef[1],
-                                                        (double *)coef[2], (double *)coef[3], (double *)coef[4],
-                                                        (double *)coef[5], d_bad);
+    coefficients_kernel<double><<<blocks, 256, 0, st>>>(L, wp, nu, dz, dt, kEps0, wp_p, nu_p, (double *)coef[0],
+                                                        (double *)coef[1], (double *)coef[2], (double *)coef[3], d_bad);
   else
-    coefficients_kernel<float><<<blocks, 256, 0, st>>>(L, wp, nu, dz, dt, kEps0, (float *)coef[0], (float *)coef[1],
-                                                       (float *)coef[2], (float *)coef[3], (float *)coef[4],
-                                                       (float *)coef[5], d_bad);
+    coefficients_kernel<float><<<blocks, 256, 0, st>>>(L, wp, nu, dz, dt, kEps0, wp_p, nu_p, (float *)coef[0],
+                                                       (float *)coef[1], (float *)coef[2], (float *)coef[3], d_bad);
   return cudaGetLastError();
 }
 
-template <typename R>
-__global__ void unpack_coefficients_kernel(Layout L, const R *c0, const R *c1, const R *c2, const R *c3, const R *c4,
-                                           const R *c5, double *out) {
+__global__ void six_coefficients_kernel(Layout L, const double *__restrict__ wp_p, const double *__restrict__ nu_p,
+                                        double dz, double dt, double eps0, double *out) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const int64_t n = L.ncells * L.nbatch;
   if (idx >= n) return;
   const int64_t g = idx / L.ncells, k = idx - g * L.ncells, src = g * L.gstride + L.off + k;
-  out[0 * n + idx] = (double)c0[src]; out[1 * n + idx] = (double)c1[src]; out[2 * n + idx] = (double)c2[src];
-  out[3 * n + idx] = (double)c3[src]; out[4 * n + idx] = (double)c4[src]; out[5 * n + idx] = (double)c5[src];
+  const Six s = six_coefficients(wp_p[src], nu_p[src], dz, dt, eps0);
+  out[0 * n + idx] = s.ca; out[1 * n + idx] = s.cj; out[2 * n + idx] = s.ch;
+  out[3 * n + idx] = s.ka; out[4 * n + idx] = s.kb; out[5 * n + idx] = s.kc;
 }
-cudaError_t launch_unpack_coefficients(int dtype, const Layout &L, void *const c[6], double *out, cudaStream_t st) {
+cudaError_t launch_six_coefficients(const Layout &L, const double *wp_p, const double *nu_p, double dz, double dt,
+                                    double *out, cudaStream_t st) {
+  const int64_t n = L.ncells * L.nbatch;
+  six_coefficients_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(L, wp_p, nu_p, dz, dt, kEps0, out);
+  return cudaGetLastError();
+}
+
+template <typename R>
+__global__ void unpack_coefficients_kernel(Layout L, const R *c0, const R *c1, const R *c2, const R *c3, double *out) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t n = L.ncells * L.nbatch;
+  if (idx >= n) return;
+  const int64_t g = idx / L.ncells, k = idx - g * L.ncells, src = g * L.gstride + L.off + k;
+  out[0 * n + idx] = (double)c0[src]; out[1 * n + idx] = (double)c1[src];
+  out[2 * n + idx] = (double)c2[src]; out[3 * n + idx] = (double)c3[src];
+}
+cudaError_t launch_unpack_coefficients(int dtype, const Layout &L, void *const c[kNumCoefArrays], double *out,
+                                       cudaStream_t st) {
   const int64_t n = L.ncells * L.nbatch;
   const unsigned blocks = (unsigned)((n + 255) / 256);
   if (dtype == 0)
     unpack_coefficients_kernel<double><<<blocks, 256, 0, st>>>(L, (double *)c[0], (double *)c[1], (double *)c[2],
-                                                               (double *)c[3], (double *)c[4], (double *)c[5], out);
+                                                               (double *)c[3], out);
   else
     unpack_coefficients_kernel<float><<<blocks, 256, 0, st>>>(L, (float *)c[0], (float *)c[1], (float *)c[2],
-                                                              (float *)c[3], (float *)c[4], (float *)c[5], out);
+                                                              (float *)c[3], out);
+  return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------- J <-> G
+// The kernels carry G = cj J - (cj kc) E instead of J (rketd_device.cuh).  Both conversions run in
+// fp64 and round once to the storage type.  Padding nodes: G = 0.
+template <typename R>
+__global__ void current_to_G_kernel(Layout L, const double *__restrict__ wp_p, const double *__restrict__ nu_p, double dz,
+                                    double dt, double eps0, const R *__restrict__ E, R *JG) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= L.gstride * L.nbatch) return;
+  const int64_t kp = idx % L.gstride, k = kp - L.off;
+  double G = 0.0;
+  if (k >= 0 && k < L.ncells) {
+    const Six s = six_coefficients(wp_p[idx], nu_p[idx], dz, dt, eps0);
+    G = __fma_rn(-__dmul_rn(s.cj, s.kc), (double)E[idx], __dmul_rn(s.cj, (double)JG[idx]));
+  }
+  JG[idx] = (R)G;
+}
+cudaError_t launch_current_to_G(int dtype, const Layout &L, const double *wp_p, const double *nu_p, double dz,
+                                double dt, const void *E, void *JG, cudaStream_t st) {
+  const int64_t total = L.gstride * L.nbatch;
+  const unsigned blocks = (unsigned)((total + 255) / 256);
+  if (dtype == 0) current_to_G_kernel<double><<<blocks, 256, 0, st>>>(L, wp_p, nu_p, dz, dt, kEps0, (const double *)E, (double *)JG);
+  else current_to_G_kernel<float><<<blocks, 256, 0, st>>>(L, wp_p, nu_p, dz, dt, kEps0, (const float *)E, (float *)JG);
+  return cudaGetLastError();
+}
+
+// J = (G + cj kc E)/cj, written in the user's [nbatch][ncells] layout
+template <typename R>
+__global__ void G_to_current_kernel(Layout L, const double *__restrict__ wp_p, const double *__restrict__ nu_p, double dz,
+                                    double dt, double eps0, const R *__restrict__ E, const R *__restrict__ G, R *J_user) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t n = L.ncells * L.nbatch;
+  if (idx >= n) return;
+  const int64_t g = idx / L.ncells, k = idx - g * L.ncells, src = g * L.gstride + L.off + k;
+  const Six s = six_coefficients(wp_p[src], nu_p[src], dz, dt, eps0);
+  const double J = __ddiv_rn(__fma_rn(__dmul_rn(s.cj, s.kc), (double)E[src], (double)G[src]), s.cj);
+  J_user[idx] = (R)J;
+}
+cudaError_t launch_G_to_current(int dtype, const Layout &L, const double *wp_p, const double *nu_p, double dz,
+                                double dt, const void *E, const void *G, void *J_user, cudaStream_t st) {
+  const int64_t n = L.ncells * L.nbatch;
+  const unsigned blocks = (unsigned)((n + 255) / 256);
+  if (dtype == 0)
+    G_to_current_kernel<double><<<blocks, 256, 0, st>>>(L, wp_p, nu_p, dz, dt, kEps0, (const double *)E, (const double *)G, (double *)J_user);
+  else
+    G_to_current_kernel<float><<<blocks, 256, 0, st>>>(L, wp_p, nu_p, dz, dt, kEps0, (const float *)E, (const float *)G, (float *)J_user);
   return cudaGetLastError();
 }
 

@@ -1,22 +1,28 @@
-// rketd_device.cuh — device-side building blocks shared by the three stencil kernels
-// (K1 one step per launch, K2 temporal blocking, K3 grid resident).  All three advance
-// a "row" (64 bytes = C consecutive nodes held in one thread's registers) with the SAME
-// sequence of correctly rounded operations (explicit fma/mul/sub intrinsics, so the
-// compiler cannot contract or reassociate differently per kernel): K1, K2 and K3 agree
-// bit for bit on the same input, which tests/test_gpu_parity.py checks.
+// rketd_device.cuh — device-side building blocks shared by the stencil kernels (K1 one step per
+// launch, K2 temporal blocking, K3 grid resident).  All of them advance a thread's C consecutive
+// nodes with the SAME sequence of correctly rounded operations (explicit fma/mul/sub intrinsics, so
+// the compiler cannot contract or reassociate differently per kernel): K1, K2 and K3 agree bit for
+// bit on the same input, which tests/test_gpu_parity.py checks.
 //
-// Per node and step (eqs. (14), (12)+(11), (11)):
-//   H'[k] = fma(-chh, E[k+1] - E[k], H[k])                                  2 flop-instr
-//   E'[k] = fma(-ch, H'[k] - H'[k-1], fma(-cj, J[k], ca * E[k]))            4
-//   J'[k] = fma(kc, E'[k], fma(kb, E[k], ka * J[k]))                        3
+// The recurrence (eqs. (14), (12)+(11), (11)) in the form the
+// kernels run it.  With the six coefficients of row a0 (E' = ca E - cj J - ch dH; J' = ka J + kb E + kc E')
+// define the scaled, shifted current  G := cj J - (cj kc) E.  Then, exactly:
+//   H'[k] = fma(-chh, E[k+1] - E[k], H[k])                                  2 flop-instr   eq. (14)
+//   E'[k] = fma(-ch, H'[k] - H'[k-1], fma(P, E[k], -G[k])),  P = ca - cj kc  3              eq. (12)+(11)
+//   G'[k] = fma(Q, E[k], ka * G[k]),                         Q = ka cj kc + cj kb   2       eq. (11)
+// G' needs only OLD values, so Mur, the source and the probes (which change E') do not touch it, and
+// J is recovered on read-out as J = (G + cj kc E)/cj.  7 instructions and 4 per-node coefficients
+// (P, ch, ka, Q) per node and step instead of 9 and 6.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
 
 namespace rketd {
 
-constexpr int kRowBytes = 64;       // one thread owns 64 B of every array
+constexpr int kRowBytes = 64;       // one thread owns 64 B (or 32 B) of every array
 constexpr int kMaxProbes = 64;
+constexpr int kNumCoef = 4;         // P, ch, ka, Q
+enum { COEF_P = 0, COEF_CH = 1, COEF_KA = 2, COEF_Q = 3 };
 
 enum : uint32_t { F_MURL = 1u, F_MURR = 2u, F_SRC = 4u, F_PROBE = 8u };
 
@@ -93,17 +99,72 @@ struct Geom {
   static_assert(C % V == 0 && CR % C == 0 && (TPR == 1 || TPR == 2), "bad cells per thread");
 };
 
-// Swizzled shared-memory address of chunk j (0..3) of row `row` in an array of 64-B rows whose base
+// Swizzled shared-memory offset of chunk j (0..3) of row `row` in an array of 64-B rows whose base
 // is 512-B aligned: CU_TENSOR_MAP_SWIZZLE_64B = XOR of address bits [4:5] with bits [7:8].  With it
 // a warp's 128-bit accesses (thread stride 32 or 64 B) cover all 32 banks.
 __device__ __forceinline__ uint32_t swz_off(int row, int j) { return row * kRowBytes + ((j ^ ((row >> 1) & 3)) << 4); }
 
-// Coefficients of a thread's nodes held in registers.  chunk<a>(j, out) hands out the V values of
-// array a (0..5 = ca, cj, ch, ka, kb, kc) for the thread's nodes j*V .. j*V+V-1.
+// ---- shared-memory access by 32-bit shared address (LDS.128 / STS.128, never generic LD/ST)
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void lds128(uint32_t a, double2 &v) {
+  asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a));
+}
+__device__ __forceinline__ void lds128(uint32_t a, float4 &v) {
+  asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+}
+__device__ __forceinline__ void sts128(uint32_t a, const double2 &v) {
+  asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(a), "d"(v.x), "d"(v.y) : "memory");
+}
+__device__ __forceinline__ void sts128(uint32_t a, const float4 &v) {
+  asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(a), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+
+// ---- 256-bit global access (sm_100: LDG.E.ENL2.256 / STG.E.ENL2.256): a thread's 64-B row in two
+// instructions, every store a full 32-B sector.  p must be 32-B aligned.
+__device__ __forceinline__ void ldg256(const double *p, double (&o)[4]) {
+  asm volatile("ld.global.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(o[0]), "=d"(o[1]), "=d"(o[2]), "=d"(o[3]) : "l"(p));
+}
+__device__ __forceinline__ void ldg256(const float *p, float (&o)[8]) {
+  asm volatile("ld.global.v8.f32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+               : "=f"(o[0]), "=f"(o[1]), "=f"(o[2]), "=f"(o[3]), "=f"(o[4]), "=f"(o[5]), "=f"(o[6]), "=f"(o[7]) : "l"(p));
+}
+__device__ __forceinline__ void stg256(double *p, const double (&o)[4]) {
+  asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(p), "d"(o[0]), "d"(o[1]), "d"(o[2]), "d"(o[3]) : "memory");
+}
+__device__ __forceinline__ void stg256(float *p, const float (&o)[8]) {
+  asm volatile("st.global.v8.f32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};"
+               ::"l"(p), "f"(o[0]), "f"(o[1]), "f"(o[2]), "f"(o[3]), "f"(o[4]), "f"(o[5]), "f"(o[6]), "f"(o[7]) : "memory");
+}
+// a thread's C nodes (32 or 64 B, 32-B aligned) <-> global memory
+template <typename R, int C>
+__device__ __forceinline__ void load_nodes_global(const R *base, int64_t first, R (&out)[C]) {
+  constexpr int W = 32 / sizeof(R);
+  static_assert(C % W == 0, "a thread owns a multiple of 32 B");
+#pragma unroll
+  for (int j = 0; j < C / W; ++j) {
+    R o[W];
+    ldg256(base + first + j * W, o);
+#pragma unroll
+    for (int u = 0; u < W; ++u) out[j * W + u] = o[u];
+  }
+}
+template <typename R, int C>
+__device__ __forceinline__ void store_nodes_global(R *base, int64_t first, const R (&in)[C]) {
+  constexpr int W = 32 / sizeof(R);
+#pragma unroll
+  for (int j = 0; j < C / W; ++j) {
+    R o[W];
+#pragma unroll
+    for (int u = 0; u < W; ++u) o[u] = in[j * W + u];
+    stg256(base + first + j * W, o);
+  }
+}
+
+// Coefficients of a thread's nodes held in registers: c[a][i], a = COEF_*.
 template <typename R, int C>
 struct CoefRegs {
   static constexpr int V = 16 / sizeof(R);
-  R c[6][C];
+  R c[kNumCoef][C];
   template <int a>
   __device__ __forceinline__ void chunk(int j, R (&out)[V]) const {
 #pragma unroll
@@ -111,122 +172,123 @@ struct CoefRegs {
   }
 };
 
-// Coefficients held in shared memory: six arrays of ROWS swizzled 64-B rows.
+// Coefficients held in shared memory: kNumCoef arrays of ROWS swizzled 64-B rows.
 template <typename R, int C, int ROWS>
 struct CoefSmem {
   static constexpr int V = 16 / sizeof(R);
-  const uint8_t *chunk_ptr[C / V];     // address of the thread's chunk j in array 0
-  __device__ __forceinline__ void init(const uint8_t *array0, int tid) {
+  uint32_t chunk_addr[C / V];     // shared address of the thread's chunk j in array 0
+  __device__ __forceinline__ void init(uint32_t array0, int tid) {
     const int row = tid / Geom<R, C>::TPR, sub = tid % Geom<R, C>::TPR;
 #pragma unroll
-    for (int j = 0; j < C / V; ++j) chunk_ptr[j] = array0 + swz_off(row, sub * (C / V) + j);
+    for (int j = 0; j < C / V; ++j) chunk_addr[j] = array0 + swz_off(row, sub * (C / V) + j);
   }
   template <int a>
   __device__ __forceinline__ void chunk(int j, R (&out)[V]) const {
-    typedef typename Arith<R>::Vec Vec;
-    vec_unpack(*reinterpret_cast<const Vec *>(chunk_ptr[j] + a * (ROWS * kRowBytes)), out);
+    typename Arith<R>::Vec v;
+    lds128(chunk_addr[j] + a * (ROWS * kRowBytes), v);
+    vec_unpack(v, out);
   }
   template <int a>
   __device__ __forceinline__ void store_chunk(int j, const typename Arith<R>::Vec &v) const {
-    typedef typename Arith<R>::Vec Vec;
-    *reinterpret_cast<Vec *>(const_cast<uint8_t *>(chunk_ptr[j]) + a * (ROWS * kRowBytes)) = v;
+    sts128(chunk_addr[j] + a * (ROWS * kRowBytes), v);
   }
 };
 
-// ---- one leapfrog step of a thread's C nodes, in two phases so that the halo values the
-// neighbours need for the NEXT step can be sent between them.
-//
-// Phase 1: H' in place (a1), E' into En (a2), Mur (a3), source (a4), probe record (a6), and the
-// part t = kb E + ka J of eq. (11) that needs the old E.  El, Hl: old E and H of the node left of
-// the thread's nodes; Er: old E of the node to the right.  k0: physical in-grid index of the first
-// node; g: grid; nloc: local step index; owner: this thread records probes among its nodes.
-// SPECIAL = false compiles the boundary/source/probe handling out (tiles without such rows).
-template <bool SPECIAL, typename R, int C, typename CF>
-__device__ __forceinline__ void step_fields(const R (&E)[C], R (&En)[C], R (&H)[C], const R (&J)[C], R (&t)[C],
-                                            const CF &cf, R El, R Hl, R Er, R nchh, const StepParams<R> &p,
-                                            uint32_t flag, int64_t k0, int64_t g, int64_t nloc, bool owner) {
+// ---- Mur (a3), soft source (a4), probe record (a6) and padding hygiene for the threads whose
+// nodes include a boundary, the source or a probe.  E: old values, En: new values (modified), H: new
+// values (padding zeroed).  k0: physical in-grid index of the thread's first node; g: grid; nloc:
+// local step index; owner: this thread records probes among its nodes.
+template <typename R, int C>
+__device__ __forceinline__ void step_special(const R (&E)[C], R (&En)[C], R (&H)[C], const StepParams<R> &p,
+                                             uint32_t flag, int64_t k0, int64_t g, int64_t nloc, bool owner) {
   typedef Arith<R> A;
-  constexpr int V = 16 / sizeof(R);
-  // a1: H update, eq. (14).  The left neighbour's new H is recomputed here from old values so
-  // that one exchange of old values per step is enough.
-  const R Hl_new = A::fma(nchh, A::sub(E[0], El), Hl);
+  if (flag & F_MURL) {   // a3, left end.  The layout guarantees node 1 is held by the same thread.
 #pragma unroll
-  for (int i = 0; i < C; ++i) H[i] = A::fma(nchh, A::sub(i + 1 < C ? E[i + 1] : Er, E[i]), H[i]);
-  // a2: E update, eq. (12) with (11) substituted; t = kb E + ka J (first two terms of eq. (11))
+    for (int i = 0; i < C - 1; ++i)
+      if (k0 + i == p.cellL) En[i] = A::fma(p.mur_m, A::sub(En[i + 1], E[i]), E[i + 1]);
 #pragma unroll
-  for (int j = 0; j < C / V; ++j) {
-    R ca[V], cj[V], ch[V], ka[V], kb[V];
-    cf.template chunk<0>(j, ca);
-    cf.template chunk<1>(j, cj);
-    cf.template chunk<2>(j, ch);
-    cf.template chunk<3>(j, ka);
-    cf.template chunk<4>(j, kb);
-#pragma unroll
-    for (int u = 0; u < V; ++u) {
-      const int i = j * V + u;
-      En[i] = A::fma(-ch[u], A::sub(H[i], i ? H[i - 1] : Hl_new), A::fma(-cj[u], J[i], A::mul(ca[u], E[i])));
-      t[i] = A::fma(kb[u], E[i], A::mul(ka[u], J[i]));
-    }
+    for (int i = 0; i < C; ++i)
+      if (k0 + i < p.cellL) H[i] = R(0);      // padding left of node 0
   }
-  if constexpr (SPECIAL) {
-    if (flag) {   // threads that hold a boundary node, the source node or a probe (rare)
-      if (flag & F_MURL) {   // a3, left end.  The layout guarantees node 1 is held by the same thread.
+  if (flag & F_MURR) {   // a3, right end.  Node ncells-2 is held by the same thread.
 #pragma unroll
-        for (int i = 0; i < C - 1; ++i)
-          if (k0 + i == p.cellL) En[i] = A::fma(p.mur_m, A::sub(En[i + 1], E[i]), E[i + 1]);
+    for (int i = 1; i < C; ++i)
+      if (k0 + i == p.cellR) En[i] = A::fma(p.mur_m, A::sub(En[i - 1], E[i]), E[i - 1]);
 #pragma unroll
-        for (int i = 0; i < C; ++i)
-          if (k0 + i < p.cellL) H[i] = R(0);      // padding left of node 0
-      }
-      if (flag & F_MURR) {   // a3, right end.  Node ncells-2 is held by the same thread.
+    for (int i = 0; i < C; ++i)
+      if (k0 + i >= p.cellR) H[i] = R(0);     // H[ncells-1] and padding
+  }
+  if (flag & F_SRC) {    // a4: soft source
+    const R s = p.src_tab[nloc];
+#pragma unroll
+    for (int i = 0; i < C; ++i)
+      if (k0 + i == p.cellS) En[i] = A::add(En[i], s);
+  }
+  if ((flag & F_PROBE) && owner && p.rec) {   // a6: probe record
+    for (int q = 0; q < p.nprobes; ++q) {
+      const int64_t d = p.probe_cell[q] - k0;
+      if (d >= 0 && d < C) {
+        R v = En[0];
 #pragma unroll
         for (int i = 1; i < C; ++i)
-          if (k0 + i == p.cellR) En[i] = A::fma(p.mur_m, A::sub(En[i - 1], E[i]), E[i - 1]);
-#pragma unroll
-        for (int i = 0; i < C; ++i)
-          if (k0 + i >= p.cellR) H[i] = R(0);     // H[ncells-1] and padding
-      }
-      if (flag & F_SRC) {    // a4: soft source
-        const R s = p.src_tab[nloc];
-#pragma unroll
-        for (int i = 0; i < C; ++i)
-          if (k0 + i == p.cellS) En[i] = A::add(En[i], s);
-      }
-      if ((flag & F_PROBE) && owner && p.rec) {   // a6: probe record
-        for (int q = 0; q < p.nprobes; ++q) {
-          const int64_t d = p.probe_cell[q] - k0;
-          if (d >= 0 && d < C) {
-            R v = En[0];
-#pragma unroll
-            for (int i = 1; i < C; ++i)
-              if (d == i) v = En[i];
-            p.rec[(g * p.nprobes + q) * p.rec_stride + nloc] = v;
-          }
-        }
+          if (d == i) v = En[i];
+        p.rec[(g * p.nprobes + q) * p.rec_stride + nloc] = v;
       }
     }
   }
 }
 
-// Phase 2 — a5: J' = kc E' + (kb E + ka J), eq. (11), with the final E'.
+// ---- one leapfrog step of a thread's C nodes, halos given as OLD values (K1, K3, CTA-tile K2):
+// El, Hl: old E and H of the node left of the thread's nodes; Er: old E of the node to the right.
+// The left neighbour's new H is recomputed here from old values (same expression, same bits as the
+// neighbour's own), so that one exchange of old values per step is enough.
+// SPECIAL = false compiles the boundary/source/probe handling out (tiles without such rows).
+template <bool SPECIAL, typename R, int C, typename CF>
+__device__ __forceinline__ void step_fields(const R (&E)[C], R (&En)[C], R (&H)[C], const R (&G)[C], const CF &cf, R El,
+                                            R Hl, R Er, R nchh, const StepParams<R> &p, uint32_t flag, int64_t k0,
+                                            int64_t g, int64_t nloc, bool owner) {
+  typedef Arith<R> A;
+  constexpr int V = 16 / sizeof(R);
+  // a1: H update, eq. (14)
+  const R Hl_new = A::fma(nchh, A::sub(E[0], El), Hl);
+#pragma unroll
+  for (int i = 0; i < C; ++i) H[i] = A::fma(nchh, A::sub(i + 1 < C ? E[i + 1] : Er, E[i]), H[i]);
+  // a2: E update, eq. (12) with (11) substituted, in the (P, G) form
+#pragma unroll
+  for (int j = 0; j < C / V; ++j) {
+    R cp[V], ch[V];
+    cf.template chunk<COEF_P>(j, cp);
+    cf.template chunk<COEF_CH>(j, ch);
+#pragma unroll
+    for (int u = 0; u < V; ++u) {
+      const int i = j * V + u;
+      En[i] = A::fma(-ch[u], A::sub(H[i], i ? H[i - 1] : Hl_new), A::fma(cp[u], E[i], -G[i]));
+    }
+  }
+  if constexpr (SPECIAL) {
+    if (flag) step_special<R, C>(E, En, H, p, flag, k0, g, nloc, owner);
+  }
+}
+
+// a5 — eq. (11) in the G form: G' = Q E + ka G with the OLD E (independent of E').
 template <typename R, int C, typename CF>
-__device__ __forceinline__ void step_current(R (&J)[C], const R (&En)[C], const R (&t)[C], const CF &cf) {
+__device__ __forceinline__ void step_current(R (&G)[C], const R (&E)[C], const CF &cf) {
   typedef Arith<R> A;
   constexpr int V = 16 / sizeof(R);
 #pragma unroll
   for (int j = 0; j < C / V; ++j) {
-    R kc[V];
-    cf.template chunk<5>(j, kc);
+    R ka[V], cq[V];
+    cf.template chunk<COEF_KA>(j, ka);
+    cf.template chunk<COEF_Q>(j, cq);
 #pragma unroll
-    for (int u = 0; u < V; ++u) J[j * V + u] = A::fma(kc[u], En[j * V + u], t[j * V + u]);
+    for (int u = 0; u < V; ++u) G[j * V + u] = A::fma(cq[u], E[j * V + u], A::mul(ka[u], G[j * V + u]));
   }
 }
 
 // ---- halo exchange inside a CTA: shuffles inside a warp, shared-memory slots between warps
 // (index warp+1; slots 0 and NW+1 stay zero = the outside of the tile), double-buffered by step
 // parity so that one __syncthreads per step is enough.  send_halo is called as soon as a step's
-// E', H' exist (between the two phases); the barrier and recv_halo come after phase 2, off the
-// critical path.
+// E', H' exist; the G update, the barrier and recv_halo come after, off the critical path.
 template <typename R, int NW>
 struct HaloSlots {
   R e_first[2][NW + 2], e_last[2][NW + 2], h_last[2][NW + 2];
@@ -258,9 +320,7 @@ __device__ __forceinline__ void recv_halo(const HaloSlots<R, NW> &hs, int par, i
   Er = lane == 31 ? c : Er;
 }
 
-// ---- PTX wrappers: shared-memory 128-bit access, mbarrier, TMA (cp.async.bulk.tensor)
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
+// ---- PTX wrappers: mbarrier, TMA (cp.async.bulk.tensor)
 __device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
 }
@@ -281,18 +341,21 @@ __device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarr
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 // 3-D tiled TMA load global -> shared, completion on an mbarrier (SASS: UTMALDG)
-__device__ __forceinline__ void tma_load_3d(void *dst, const void *tmap, uint64_t *bar, int c0, int c1, int c2) {
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const void *tmap, uint64_t *bar, int c0, int c1, int c2) {
   asm volatile(
       "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
-      ::"r"(smem_u32(dst)), "l"(tmap), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2) : "memory");
+      ::"r"(dst), "l"(tmap), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2) : "memory");
 }
 // 3-D tiled TMA store shared -> global (SASS: UTMASTG)
-__device__ __forceinline__ void tma_store_3d(const void *tmap, const void *src, int c0, int c1, int c2) {
+__device__ __forceinline__ void tma_store_3d(const void *tmap, uint32_t src, int c0, int c1, int c2) {
   asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.tile.bulk_group [%0, {%2, %3, %4}], [%1];"
-               ::"l"(tmap), "r"(smem_u32(src)), "r"(c0), "r"(c1), "r"(c2) : "memory");
+               ::"l"(tmap), "r"(src), "r"(c0), "r"(c1), "r"(c2) : "memory");
 }
 __device__ __forceinline__ void tma_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void tma_wait_read0() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 __device__ __forceinline__ void tma_wait0() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void prefetch_tmap(const void *tmap) {
+  asm volatile("prefetch.tensormap [%0];" ::"l"(tmap) : "memory");
+}
 
 }  // namespace rketd

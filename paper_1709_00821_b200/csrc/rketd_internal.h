@@ -7,7 +7,8 @@
 
 namespace rketd {
 
-// HBM layout of every per-node array (fields E, H, J x2 for ping-pong; six coefficient arrays):
+// HBM layout of every per-node array (fields E, H, G x2 for ping-pong; four coefficient arrays P, ch, ka, Q;
+// the media wp, nu in fp64):
 //   [nbatch][nrows][C] with rows of 64 B (C = 8 fp64 / 16 fp32 nodes) — one row is what one thread
 //   (or half of what) one thread owns in registers.  Node k of grid g sits at physical in-grid
 //   index off + k.  off is 0, or 1 when (ncells-1) % (C/2) == 0, so that nodes {0,1} sit in the same
@@ -38,8 +39,8 @@ struct StepCommon {
 
 // K2 (temporal blocking) plan: tiling + the TMA descriptors for one ping-pong direction.
 struct K2Maps {
-  CUtensorMap ld[9];   // E, H, J (source buffers), ca, cj, ch, ka, kb, kc : box {C, NT, 1}, SWIZZLE_64B
-  CUtensorMap st[3];   // E, H, J (destination buffers)                  : box {C, rows_out, 1}
+  CUtensorMap ld[7];   // E, H, G (source buffers), P, ch, ka, Q : box {C, rows, 1}, SWIZZLE_64B
+  CUtensorMap st[3];   // E, H, G (destination buffers)         : box {C, rows_out, 1}
 };
 struct K2Plan {
   int variant = -1;        // K2 kernel variant (see rketd_kernels.cu)
@@ -54,24 +55,37 @@ struct K2Plan {
   K2Maps maps[2];          // maps[s]: read buffer s, write buffer 1-s
 };
 
+constexpr int kK2Variants = 8;
+constexpr int kNumCoefArrays = 4;                                 // P, ch, ka, Q (rketd_device.cuh COEF_*)
 int k2_tile_rows(int variant);                                    // rows per tile of a K2 variant, 0 if none
 int k2_tiles_per_cta(int variant);                               // tiles a CTA works on at a time (warp tiles)
 size_t k2_smem_bytes(int variant);
 int k3_threads_for_rows(int dtype, int64_t nrows, int variant);   // threads per CTA of the K3 kernel, or 0
 
-cudaError_t launch_k1(int dtype, const Layout &L, FieldPtrs src, FieldPtrs dst, void *const coef[6],
+cudaError_t launch_k1(int dtype, const Layout &L, FieldPtrs src, FieldPtrs dst, void *const coef[kNumCoefArrays],
                       const StepCommon &sc, cudaStream_t st);
-cudaError_t launch_k2(int dtype, const Layout &L, const K2Plan &plan, int src_buf, const StepCommon &sc,
+cudaError_t launch_k2(int dtype, const Layout &L, const K2Plan &plan, int src_buf, FieldPtrs dst, const StepCommon &sc,
                       int steps, cudaStream_t st);
-cudaError_t launch_k3(int dtype, const Layout &L, FieldPtrs fld, void *const coef[6], const StepCommon &sc,
+cudaError_t launch_k3(int dtype, const Layout &L, FieldPtrs fld, void *const coef[kNumCoefArrays], const StepCommon &sc,
                       int64_t nsteps, int NT, int variant, cudaStream_t st);
 cudaError_t k2_configure(int dtype, int variant, int *ctas_per_sm);   // sets smem attribute, returns occupancy
 
 // auxiliary kernels (rketd_aux.cu)
+// media: user wp, nu [nbatch][ncells] -> padded fp64 copies wp_p, nu_p + the four kernel coefficients
 cudaError_t launch_coefficients(int dtype, const Layout &L, const double *wp, const double *nu, double dz,
-                                double dt, void *const coef[6], int *d_bad, cudaStream_t st);
-cudaError_t launch_unpack_coefficients(int dtype, const Layout &L, void *const coef[6], double *out,
+                                double dt, double *wp_p, double *nu_p, void *const coef[kNumCoefArrays], int *d_bad,
+                                cudaStream_t st);
+// the six coefficients of SURVEY a0 (ca, cj, ch, ka, kb, kc), recomputed in fp64 from the padded media
+cudaError_t launch_six_coefficients(const Layout &L, const double *wp_p, const double *nu_p, double dz, double dt,
+                                    double *out, cudaStream_t st);
+// the four kernel coefficients as stored (P, ch, ka, Q), converted to fp64, user layout
+cudaError_t launch_unpack_coefficients(int dtype, const Layout &L, void *const coef[kNumCoefArrays], double *out,
                                        cudaStream_t st);
+// J <-> G = cj J - cj kc E on the padded arrays (in place on the third field array)
+cudaError_t launch_current_to_G(int dtype, const Layout &L, const double *wp_p, const double *nu_p, double dz,
+                                double dt, const void *E, void *JG, cudaStream_t st);
+cudaError_t launch_G_to_current(int dtype, const Layout &L, const double *wp_p, const double *nu_p, double dz,
+                                double dt, const void *E, const void *G, void *J_user, cudaStream_t st);
 cudaError_t launch_twiddles(const double *d_freqs, int nfreq, int64_t step0, int64_t nsteps, double dt,
                             double2 *tw, cudaStream_t st);
 cudaError_t launch_dft_accumulate(int dtype, const void *rec, int64_t nseries, int64_t nsteps, const double2 *tw,

@@ -3,13 +3,16 @@
 //   K1  k1_step      one fused H/E/J step per launch; a thread owns one 64-B row; halos from
 //                    global memory; ping-pong buffers.  HBM-bound baseline and cross-check
 //                    (this is the paper's H-kernel + E-kernel pair, fused).
-//   K2  k2_tblock    temporal blocking: a persistent CTA stages a tile (NT rows, halo included)
-//                    of all nine arrays into shared memory with 3-D tiled TMA loads (hardware
-//                    64-B swizzle -> conflict-free 128-bit reads), moves it into registers,
-//                    advances T steps exchanging halos by warp shuffles (+ one shared-memory
-//                    slot per warp edge and one barrier per step), and writes the valid
-//                    interior back with TMA stores.  Every HBM byte serves T steps.  The next
-//                    tile's TMA loads are in flight while the current tile computes.
+//   K2  k2_wtile     temporal blocking, warp tiles (default): every WARP of a persistent CTA owns
+//                    a tile of 32 rows x 64 B (halo included) of the seven input arrays (E, H, G,
+//                    P, ch, ka, Q), staged into shared memory by 3-D tiled TMA loads (hardware
+//                    64-B swizzle -> conflict-free 128-bit reads) on the warp's own mbarrier,
+//                    moved into registers, advanced T steps with halos travelling by warp
+//                    shuffles only (no block barrier, no shared memory in the time loop), and the
+//                    valid interior written back by TMA stores or 256-bit global stores.  Every
+//                    HBM byte serves T steps; the next tile's loads fly while this one computes.
+//       k2_tblock    the same with one tile per CTA (128/256 rows: less redundant halo work, but
+//                    one block barrier per step).
 //   K3  k3_resident  one CTA per grid keeps the whole grid on chip (fields in registers,
 //                    coefficients in registers or shared memory) for ALL steps of the run and
 //                    streams probe samples out; the batched variant of the north_star.
@@ -22,23 +25,7 @@
 namespace rketd {
 
 template <typename R> struct RowPtrs { R *E, *H, *J; };
-template <typename R> struct CoefPtrs { const R *c[6]; };
-
-// a thread's C nodes <-> global memory (first node at physical index `first`, 16-B aligned)
-template <typename R, int C>
-__device__ __forceinline__ void load_nodes_global(const R *base, int64_t first, R (&out)[C]) {
-  typedef typename Arith<R>::Vec Vec;
-  const Vec *p = reinterpret_cast<const Vec *>(base + first);
-#pragma unroll
-  for (int j = 0; j < Geom<R, C>::NCH; ++j) vec_to_regs<R, C>(p[j], out, j);
-}
-template <typename R, int C>
-__device__ __forceinline__ void store_nodes_global(R *base, int64_t first, const R (&in)[C]) {
-  typedef typename Arith<R>::Vec Vec;
-  Vec *p = reinterpret_cast<Vec *>(base + first);
-#pragma unroll
-  for (int j = 0; j < Geom<R, C>::NCH; ++j) p[j] = regs_to_vec<R, C>(in, j);
-}
+template <typename R> struct CoefPtrs { const R *c[kNumCoef]; };
 
 // ------------------------------------------------------------------------------------ K1
 template <typename R>
@@ -49,22 +36,22 @@ __global__ void __launch_bounds__(128) k1_step(RowPtrs<R> src, RowPtrs<R> dst, C
   const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (r >= total_rows) return;
   const int64_t g = r / nrows, row = r - g * nrows;
-  R E[C], En[C], H[C], J[C], t[C];
+  R E[C], En[C], H[C], G[C];
   CoefRegs<R, C> cf;
   load_nodes_global<R, C>(src.E, r * C, E);
   load_nodes_global<R, C>(src.H, r * C, H);
-  load_nodes_global<R, C>(src.J, r * C, J);
+  load_nodes_global<R, C>(src.J, r * C, G);
 #pragma unroll
-  for (int a = 0; a < 6; ++a) load_nodes_global<R, C>(cp.c[a], r * C, cf.c[a]);
+  for (int a = 0; a < kNumCoef; ++a) load_nodes_global<R, C>(cp.c[a], r * C, cf.c[a]);
   const R El = row > 0 ? src.E[r * C - 1] : R(0);
   const R Hl = row > 0 ? src.H[r * C - 1] : R(0);
   const R Er = row < nrows - 1 ? src.E[(r + 1) * C] : R(0);
   const uint32_t flag = p.rowflag[row];
-  step_fields<true, R, C>(E, En, H, J, t, cf, El, Hl, Er, p.nchh, p, flag, row * C, g, p.n0, true);
-  step_current<R, C>(J, En, t, cf);
+  step_fields<true, R, C>(E, En, H, G, cf, El, Hl, Er, p.nchh, p, flag, row * C, g, p.n0, true);
+  step_current<R, C>(G, E, cf);
   store_nodes_global<R, C>(dst.E, r * C, En);
   store_nodes_global<R, C>(dst.H, r * C, H);
-  store_nodes_global<R, C>(dst.J, r * C, J);
+  store_nodes_global<R, C>(dst.J, r * C, G);
 }
 
 // The time loop shared by K2 and K3: nsteps leapfrog steps of this thread's nodes, halos
@@ -82,10 +69,9 @@ __device__ __forceinline__ void time_loop(R (&E)[C], R (&H)[C], R (&J)[C], const
   recv_halo<R, NW>(hs, 0, warp, lane, El, Hl, Er);
   R Eb[C];
   auto one_step = [&](const R (&Ein)[C], R (&Eout)[C], int par) {
-    R t[C];
-    step_fields<SPECIAL, R, C>(Ein, Eout, H, J, t, cf, El, Hl, Er, nchh, p, flag, k0, g, nloc, owner);
+    step_fields<SPECIAL, R, C>(Ein, Eout, H, J, cf, El, Hl, Er, nchh, p, flag, k0, g, nloc, owner);
     send_halo<R, C, NW>(Eout, H, hs, par, warp, lane, El, Hl, Er);     // for the next step
-    step_current<R, C>(J, Eout, t, cf);
+    step_current<R, C>(J, Ein, cf);
     __syncthreads();
     recv_halo<R, NW>(hs, par, warp, lane, El, Hl, Er);
     if (SPECIAL) ++nloc;
@@ -135,9 +121,9 @@ __global__ void __launch_bounds__(NT, MINB) k3_resident(RowPtrs<R> f, CoefPtrs<R
   __syncthreads();
 
   if constexpr (CSM) {
-    uint8_t *sm = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    const uint32_t base = smem_u32(smem_raw);
     CoefSmem<R, C, ROWS> cf;
-    cf.init(sm, tid);
+    cf.init(base + ((1024u - (base & 1023u)) & 1023u), tid);
     // each thread stages its own coefficient chunks (only it reads them back: no barrier needed)
     auto stage = [&](auto ac) {
       constexpr int a = decltype(ac)::value;
@@ -151,12 +137,11 @@ __global__ void __launch_bounds__(NT, MINB) k3_resident(RowPtrs<R> f, CoefPtrs<R
     };
     stage(std::integral_constant<int, 0>{}); stage(std::integral_constant<int, 1>{});
     stage(std::integral_constant<int, 2>{}); stage(std::integral_constant<int, 3>{});
-    stage(std::integral_constant<int, 4>{}); stage(std::integral_constant<int, 5>{});
     time_loop<true, R, C, NW>(E, H, J, cf, hs, p, flag, k0, g, true, nsteps, warp, lane);
   } else {
     CoefRegs<R, C> cf;
 #pragma unroll
-    for (int a = 0; a < 6; ++a) {
+    for (int a = 0; a < kNumCoef; ++a) {
 #pragma unroll
       for (int i = 0; i < C; ++i) cf.c[a][i] = R(0);
       if (valid) load_nodes_global<R, C>(cp.c[a], first, cf.c[a]);
@@ -178,6 +163,38 @@ struct K2Args {
   int rows_out;           // ROWS - 2 HR
   int64_t tiles_per_grid, total_tiles, nrows;
 };
+constexpr int kNumIn = 3 + kNumCoef;      // arrays a tile loads: E, H, G, P, ch, ka, Q
+
+// a thread's chunks of one staged tile: shared memory -> registers
+template <typename R, int C>
+__device__ __forceinline__ void tile_to_regs(uint32_t sin, const uint32_t (&off)[Geom<R, C>::NCH], uint32_t array_bytes,
+                                             R (&E)[C], R (&H)[C], R (&J)[C], CoefRegs<R, C> &cf) {
+  typedef typename Arith<R>::Vec Vec;
+#pragma unroll
+  for (int j = 0; j < Geom<R, C>::NCH; ++j) {
+    const uint32_t my = sin + off[j];
+    Vec v;
+    lds128(my + 0 * array_bytes, v); vec_to_regs<R, C>(v, E, j);
+    lds128(my + 1 * array_bytes, v); vec_to_regs<R, C>(v, H, j);
+    lds128(my + 2 * array_bytes, v); vec_to_regs<R, C>(v, J, j);
+#pragma unroll
+    for (int a = 0; a < kNumCoef; ++a) {
+      lds128(my + (3 + a) * array_bytes, v);
+      vec_to_regs<R, C>(v, cf.c[a], j);
+    }
+  }
+}
+template <typename R, int C>
+__device__ __forceinline__ void regs_to_tile(uint32_t sout, const uint32_t (&off)[Geom<R, C>::NCH], uint32_t array_bytes,
+                                             const R (&E)[C], const R (&H)[C], const R (&J)[C]) {
+#pragma unroll
+  for (int j = 0; j < Geom<R, C>::NCH; ++j) {
+    const uint32_t my = sout + off[j];
+    sts128(my + 0 * array_bytes, regs_to_vec<R, C>(E, j));
+    sts128(my + 1 * array_bytes, regs_to_vec<R, C>(H, j));
+    sts128(my + 2 * array_bytes, regs_to_vec<R, C>(J, j));
+  }
+}
 
 // Persistent CTAs; tile = ROWS = NT / TPR rows of 64 B (halo of HR rows on each side included).
 template <typename R, int C, int NT, int MINB>
@@ -187,13 +204,13 @@ __global__ void __launch_bounds__(NT, MINB) k2_tblock(const __grid_constant__ K2
   constexpr int NW = NT / 32;
   constexpr int ROWS = NT / G::TPR;
   constexpr uint32_t kArrayBytes = ROWS * kRowBytes;
-  typedef typename Arith<R>::Vec Vec;
 
   __shared__ HaloSlots<R, NW> hs;
   __shared__ __align__(8) uint64_t mbar;
   extern __shared__ uint8_t smem_raw[];
-  uint8_t *sin = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-  uint8_t *sout = sin + 9 * kArrayBytes;
+  const uint32_t base = smem_u32(smem_raw);
+  const uint32_t sin = base + ((1024u - (base & 1023u)) & 1023u);
+  const uint32_t sout = sin + kNumIn * kArrayBytes;
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int row = tid / G::TPR, sub = tid % G::TPR;
@@ -201,9 +218,9 @@ __global__ void __launch_bounds__(NT, MINB) k2_tblock(const __grid_constant__ K2
   auto issue_loads = [&](int64_t tile) {   // one elected thread
     const int64_t g = tile / q.tiles_per_grid, ti = tile - g * q.tiles_per_grid;
     const int row0 = (int)(ti * q.rows_out - q.HR);
-    mbar_expect_tx(&mbar, 9u * kArrayBytes);
+    mbar_expect_tx(&mbar, (uint32_t)kNumIn * kArrayBytes);
 #pragma unroll 1
-    for (int a = 0; a < 9; ++a) tma_load_3d(sin + a * kArrayBytes, &maps.ld[a], &mbar, 0, row0, (int)g);
+    for (int a = 0; a < kNumIn; ++a) tma_load_3d(sin + a * kArrayBytes, &maps.ld[a], &mbar, 0, row0, (int)g);
   };
 
   hs.clear(tid);
@@ -228,23 +245,14 @@ __global__ void __launch_bounds__(NT, MINB) k2_tblock(const __grid_constant__ K2
   for (; tile < q.total_tiles; tile += gridDim.x) {
     const int64_t g = tile / q.tiles_per_grid, ti = tile - g * q.tiles_per_grid;
     const int64_t rowg = ti * q.rows_out - q.HR + row;     // this thread's row in the grid
+    const uint32_t flag = (rowg >= 0 && rowg < q.nrows) ? p.rowflag[rowg] : 0u;
 
     mbar_wait(&mbar, phase);
     phase ^= 1u;
 
     R E[C], H[C], J[C];
     CoefRegs<R, C> cf;
-#pragma unroll
-    for (int j = 0; j < G::NCH; ++j) {
-      const uint8_t *my = sin + off_in[j];
-      vec_to_regs<R, C>(*reinterpret_cast<const Vec *>(my + 0 * kArrayBytes), E, j);
-      vec_to_regs<R, C>(*reinterpret_cast<const Vec *>(my + 1 * kArrayBytes), H, j);
-      vec_to_regs<R, C>(*reinterpret_cast<const Vec *>(my + 2 * kArrayBytes), J, j);
-#pragma unroll
-      for (int a = 0; a < 6; ++a)
-        vec_to_regs<R, C>(*reinterpret_cast<const Vec *>(my + (3 + a) * kArrayBytes), cf.c[a], j);
-    }
-    const uint32_t flag = (rowg >= 0 && rowg < q.nrows) ? p.rowflag[rowg] : 0u;
+    tile_to_regs<R, C>(sin, off_in, kArrayBytes, E, H, J, cf);
     const bool special = __syncthreads_or(flag != 0u);   // barrier: everyone has left the input stage
     if (tid == 0) {
       const int64_t next = tile + gridDim.x;
@@ -258,15 +266,7 @@ __global__ void __launch_bounds__(NT, MINB) k2_tblock(const __grid_constant__ K2
       time_loop<false, R, C, NW>(E, H, J, cf, hs, p, 0u, 0, g, false, q.T, warp, lane);
 
     // (the barriers of the time loop order tma_wait_read0 before the writes below)
-    if (owner) {
-#pragma unroll
-      for (int j = 0; j < G::NCH; ++j) {
-        uint8_t *my = sout + off_out[j];
-        *reinterpret_cast<Vec *>(my + 0 * kArrayBytes) = regs_to_vec<R, C>(E, j);
-        *reinterpret_cast<Vec *>(my + 1 * kArrayBytes) = regs_to_vec<R, C>(H, j);
-        *reinterpret_cast<Vec *>(my + 2 * kArrayBytes) = regs_to_vec<R, C>(J, j);
-      }
-    }
+    if (owner) regs_to_tile<R, C>(sout, off_out, kArrayBytes, E, H, J);
     fence_proxy_async_smem();
     __syncthreads();
     if (tid == 0) {
@@ -280,64 +280,85 @@ __global__ void __launch_bounds__(NT, MINB) k2_tblock(const __grid_constant__ K2
 }
 
 // ------------------------------------------------------------------------------------ K2, warp tiles
-// Same temporal blocking, but every WARP owns an independent tile of 32 rows (halo included),
-// its own shared-memory stage and its own mbarrier: halos travel by warp shuffles only, there is
-// no block barrier and no shared-memory exchange in the time loop.  Lanes 0 and 31 receive their
-// own values from the shuffles at the tile edge, which is fine: those nodes are in the halo that
-// is thrown away.  The price is a smaller tile (more redundant halo work per tile).
-template <bool SPECIAL, typename R, int C, typename CF>
-__device__ __forceinline__ void warp_time_loop(R (&E)[C], R (&H)[C], R (&J)[C], const CF &cf, const StepParams<R> &p,
-                                               uint32_t flag, int64_t k0, int64_t g, bool owner, int nsteps) {
+// One leapfrog step of a warp tile.  Only NEW values travel: H'[C-1] goes up one lane as soon as it
+// exists (the left neighbour's H' that E'[0] needs), E'[0] goes down one lane at the end (the E[C] the
+// next step's H'[C-1] needs).  Two 64-bit shuffles per step and no redundant arithmetic.  Lanes 0 and 31
+// receive their own values at the tile edge, which is fine: those nodes are in the halo that is thrown
+// away (garbage moves inwards one node per step; the halo is >= T nodes wide).
+template <bool SPECIAL, typename R, int C>
+__device__ __forceinline__ void warp_step(const R (&E)[C], R (&En)[C], R (&H)[C], R (&G)[C], const CoefRegs<R, C> &cf,
+                                          R &Er, R nchh, const StepParams<R> &p, uint32_t flag, int64_t k0, int64_t g,
+                                          int64_t nloc, bool owner) {
+  typedef Arith<R> A;
+  H[C - 1] = A::fma(nchh, A::sub(Er, E[C - 1]), H[C - 1]);                    // a1, last node first
+  const R Hl = __shfl_up_sync(0xffffffffu, H[C - 1], 1);
+#pragma unroll
+  for (int i = 0; i < C - 1; ++i) H[i] = A::fma(nchh, A::sub(E[i + 1], E[i]), H[i]);
+#pragma unroll
+  for (int i = C - 1; i >= 1; --i)                                            // a2
+    En[i] = A::fma(-cf.c[COEF_CH][i], A::sub(H[i], H[i - 1]), A::fma(cf.c[COEF_P][i], E[i], -G[i]));
+  En[0] = A::fma(-cf.c[COEF_CH][0], A::sub(H[0], Hl), A::fma(cf.c[COEF_P][0], E[0], -G[0]));
+  if constexpr (SPECIAL) {
+    if (flag) step_special<R, C>(E, En, H, p, flag, k0, g, nloc, owner);       // a3, a4, a6
+  }
+  Er = __shfl_down_sync(0xffffffffu, En[0], 1);
+#pragma unroll
+  for (int i = 0; i < C; ++i) G[i] = A::fma(cf.c[COEF_Q][i], E[i], A::mul(cf.c[COEF_KA][i], G[i]));   // a5
+}
+
+template <bool SPECIAL, typename R, int C>
+__device__ __forceinline__ void warp_time_loop(R (&E)[C], R (&H)[C], R (&G)[C], const CoefRegs<R, C> &cf,
+                                               const StepParams<R> &p, uint32_t flag, int64_t k0, int64_t g, bool owner,
+                                               int nsteps) {
   const R nchh = pin_register(p.nchh);
   int64_t nloc = p.n0;
-  R El = __shfl_up_sync(0xffffffffu, E[C - 1], 1);
-  R Hl = __shfl_up_sync(0xffffffffu, H[C - 1], 1);
   R Er = __shfl_down_sync(0xffffffffu, E[0], 1);
   R Eb[C];
-  auto one_step = [&](const R (&Ein)[C], R (&Eout)[C]) {
-    R t[C];
-    step_fields<SPECIAL, R, C>(Ein, Eout, H, J, t, cf, El, Hl, Er, nchh, p, flag, k0, g, nloc, owner);
-    El = __shfl_up_sync(0xffffffffu, Eout[C - 1], 1);
-    Hl = __shfl_up_sync(0xffffffffu, H[C - 1], 1);
-    Er = __shfl_down_sync(0xffffffffu, Eout[0], 1);
-    step_current<R, C>(J, Eout, t, cf);
-    if (SPECIAL) ++nloc;
-  };
   int left = nsteps;
   for (; left >= 2; left -= 2) {
-    one_step(E, Eb);
-    one_step(Eb, E);
+    warp_step<SPECIAL, R, C>(E, Eb, H, G, cf, Er, nchh, p, flag, k0, g, nloc, owner);
+    warp_step<SPECIAL, R, C>(Eb, E, H, G, cf, Er, nchh, p, flag, k0, g, nloc + 1, owner);
+    nloc += 2;
   }
   if (left) {
-    one_step(E, Eb);
+    warp_step<SPECIAL, R, C>(E, Eb, H, G, cf, Er, nchh, p, flag, k0, g, nloc, owner);
 #pragma unroll
     for (int i = 0; i < C; ++i) E[i] = Eb[i];
   }
 }
 
-template <typename R, int NW, int MINB>
+// DIRECT = false: results leave through a shared-memory stage and TMA stores (10 x 2 KB of shared memory
+// per warp).  DIRECT = true: every owner lane writes its 64-B rows with 256-bit global stores (full 32-B
+// sectors); 7 x 2 KB per warp, which lets 12 warps (3 per scheduler) share an SM.
+template <typename R, int NW, int MINB, bool DIRECT>
 __global__ void __launch_bounds__(NW * 32, MINB) k2_wtile(const __grid_constant__ K2Maps maps,
-                                                          const __grid_constant__ StepParams<R> p, K2Args q) {
+                                                          const __grid_constant__ StepParams<R> p, K2Args q,
+                                                          RowPtrs<R> dst) {
   constexpr int C = kRowBytes / sizeof(R);
   typedef Geom<R, C> G;
-  constexpr uint32_t kArrayBytes = 32 * kRowBytes;      // one array of one warp tile: 2 KB
-  constexpr uint32_t kWarpBytes = 12 * kArrayBytes;     // 9 input + 3 output arrays
-  typedef typename Arith<R>::Vec Vec;
+  constexpr uint32_t kArrayBytes = 32 * kRowBytes;                      // one array of one warp tile: 2 KB
+  constexpr uint32_t kWarpBytes = (kNumIn + (DIRECT ? 0 : 3)) * kArrayBytes;
 
   __shared__ __align__(8) uint64_t mbars[NW];
   extern __shared__ uint8_t smem_raw[];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  uint8_t *sin = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023)) +
-                 warp * kWarpBytes;
-  uint8_t *sout = sin + 9 * kArrayBytes;
+  const uint32_t base = smem_u32(smem_raw);
+  const uint32_t sin = base + ((1024u - (base & 1023u)) & 1023u) + warp * kWarpBytes;
+  const uint32_t sout = sin + kNumIn * kArrayBytes;
   uint64_t *mbar = &mbars[warp];
 
   auto issue_loads = [&](int64_t tile) {   // lane 0
     const int64_t g = tile / q.tiles_per_grid, ti = tile - g * q.tiles_per_grid;
     const int row0 = (int)(ti * q.rows_out - q.HR);
-    mbar_expect_tx(mbar, 9u * kArrayBytes);
+    mbar_expect_tx(mbar, (uint32_t)kNumIn * kArrayBytes);
 #pragma unroll 1
-    for (int a = 0; a < 9; ++a) tma_load_3d(sin + a * kArrayBytes, &maps.ld[a], mbar, 0, row0, (int)g);
+    for (int a = 0; a < kNumIn; ++a) tma_load_3d(sin + a * kArrayBytes, &maps.ld[a], mbar, 0, row0, (int)g);
+  };
+  auto row_flag = [&](int64_t tile) -> uint32_t {
+    if (tile >= q.total_tiles) return 0u;
+    const int64_t g = tile / q.tiles_per_grid, ti = tile - g * q.tiles_per_grid;
+    const int64_t rowg = ti * q.rows_out - q.HR + lane;
+    return (rowg >= 0 && rowg < q.nrows) ? p.rowflag[rowg] : 0u;
   };
 
   if (lane == 0) {
@@ -346,9 +367,12 @@ __global__ void __launch_bounds__(NW * 32, MINB) k2_wtile(const __grid_constant_
   }
   __syncwarp();
   const int64_t stride = (int64_t)gridDim.x * NW;
+  // the warps of a CTA work on consecutive tiles, so that the tiles in flight at any time are neighbours
+  // in memory and the halo rows two tiles share are served by L2
   int64_t tile = (int64_t)blockIdx.x * NW + warp;
   if (lane == 0 && tile < q.total_tiles) issue_loads(tile);
   uint32_t phase = 0;
+  uint32_t flag = row_flag(tile);
 
   const int r_out = lane - q.HR;
   const bool owner = r_out >= 0 && r_out < q.rows_out;
@@ -368,49 +392,42 @@ __global__ void __launch_bounds__(NW * 32, MINB) k2_wtile(const __grid_constant_
 
     R E[C], H[C], J[C];
     CoefRegs<R, C> cf;
-#pragma unroll
-    for (int j = 0; j < G::NCH; ++j) {
-      const uint8_t *my = sin + off_in[j];
-      vec_to_regs<R, C>(*reinterpret_cast<const Vec *>(my + 0 * kArrayBytes), E, j);
-      vec_to_regs<R, C>(*reinterpret_cast<const Vec *>(my + 1 * kArrayBytes), H, j);
-      vec_to_regs<R, C>(*reinterpret_cast<const Vec *>(my + 2 * kArrayBytes), J, j);
-#pragma unroll
-      for (int a = 0; a < 6; ++a)
-        vec_to_regs<R, C>(*reinterpret_cast<const Vec *>(my + (3 + a) * kArrayBytes), cf.c[a], j);
-    }
-    const uint32_t flag = (rowg >= 0 && rowg < q.nrows) ? p.rowflag[rowg] : 0u;
+    tile_to_regs<R, C>(sin, off_in, kArrayBytes, E, H, J, cf);
     const bool special = __any_sync(0xffffffffu, flag != 0u);   // also: every lane has left the input stage
+    const uint32_t myflag = flag;
     if (lane == 0) {
       const int64_t next = tile + stride;
       if (next < q.total_tiles) issue_loads(next);   // overlaps with the T steps below
-      tma_wait_read0();                              // previous tile's stores have drained the output stage
+      if (!DIRECT) tma_wait_read0();                 // previous tile's stores have drained the output stage
     }
+    flag = row_flag(tile + stride);                  // next tile's flags: the load latency hides behind the steps
 
     if (special)
-      warp_time_loop<true, R, C>(E, H, J, cf, p, flag, rowg * C, g, owner, q.T);
+      warp_time_loop<true, R, C>(E, H, J, cf, p, myflag, rowg * C, g, owner, q.T);
     else
       warp_time_loop<false, R, C>(E, H, J, cf, p, 0u, 0, g, false, q.T);
 
-    __syncwarp();                                    // orders lane 0's tma_wait_read0 before the writes below
-    if (owner) {
-#pragma unroll
-      for (int j = 0; j < G::NCH; ++j) {
-        uint8_t *my = sout + off_out[j];
-        *reinterpret_cast<Vec *>(my + 0 * kArrayBytes) = regs_to_vec<R, C>(E, j);
-        *reinterpret_cast<Vec *>(my + 1 * kArrayBytes) = regs_to_vec<R, C>(H, j);
-        *reinterpret_cast<Vec *>(my + 2 * kArrayBytes) = regs_to_vec<R, C>(J, j);
+    if constexpr (DIRECT) {
+      if (owner && rowg < q.nrows) {
+        const int64_t first = (g * q.nrows + rowg) * C;
+        store_nodes_global<R, C>(dst.E, first, E);
+        store_nodes_global<R, C>(dst.H, first, H);
+        store_nodes_global<R, C>(dst.J, first, J);
+      }
+    } else {
+      __syncwarp();                                    // orders lane 0's tma_wait_read0 before the writes below
+      if (owner) regs_to_tile<R, C>(sout, off_out, kArrayBytes, E, H, J);
+      fence_proxy_async_smem();
+      __syncwarp();
+      if (lane == 0) {
+        const int row_out0 = (int)(ti * q.rows_out);
+#pragma unroll 1
+        for (int a = 0; a < 3; ++a) tma_store_3d(&maps.st[a], sout + a * kArrayBytes, 0, row_out0, (int)g);
+        tma_commit();
       }
     }
-    fence_proxy_async_smem();
-    __syncwarp();
-    if (lane == 0) {
-      const int row_out0 = (int)(ti * q.rows_out);
-#pragma unroll 1
-      for (int a = 0; a < 3; ++a) tma_store_3d(&maps.st[a], sout + a * kArrayBytes, 0, row_out0, (int)g);
-      tma_commit();
-    }
   }
-  if (lane == 0) tma_wait0();
+  if (!DIRECT && lane == 0) tma_wait0();
 }
 
 // ------------------------------------------------------------------------------------ launchers
@@ -429,21 +446,21 @@ static StepParams<R> make_params(const StepCommon &sc) {
   return p;
 }
 template <typename R> static RowPtrs<R> rp(FieldPtrs f) { return RowPtrs<R>{(R *)f.E, (R *)f.H, (R *)f.J}; }
-template <typename R> static CoefPtrs<R> cpz(void *const coef[6]) {
+template <typename R> static CoefPtrs<R> cpz(void *const coef[kNumCoef]) {
   CoefPtrs<R> c;
-  for (int a = 0; a < 6; ++a) c.c[a] = (const R *)coef[a];
+  for (int a = 0; a < kNumCoef; ++a) c.c[a] = (const R *)coef[a];
   return c;
 }
 
 template <typename R>
-static cudaError_t launch_k1_t(const Layout &L, FieldPtrs src, FieldPtrs dst, void *const coef[6],
+static cudaError_t launch_k1_t(const Layout &L, FieldPtrs src, FieldPtrs dst, void *const coef[kNumCoef],
                                const StepCommon &sc, cudaStream_t st) {
   const int64_t total = L.nrows * L.nbatch;
   const int64_t blocks = (total + 127) / 128;
   k1_step<R><<<(unsigned)blocks, 128, 0, st>>>(rp<R>(src), rp<R>(dst), cpz<R>(coef), make_params<R>(sc), L.nrows, total);
   return cudaGetLastError();
 }
-cudaError_t launch_k1(int dtype, const Layout &L, FieldPtrs src, FieldPtrs dst, void *const coef[6],
+cudaError_t launch_k1(int dtype, const Layout &L, FieldPtrs src, FieldPtrs dst, void *const coef[kNumCoef],
                       const StepCommon &sc, cudaStream_t st) {
   return dtype == 0 ? launch_k1_t<double>(L, src, dst, coef, sc, st) : launch_k1_t<float>(L, src, dst, coef, sc, st);
 }
@@ -462,10 +479,10 @@ int k3_threads_for_rows(int, int64_t nrows, int variant) {
 }
 
 template <typename R, int C, int NT, bool CSM, int MINB>
-static cudaError_t launch_k3_v(const Layout &L, FieldPtrs f, void *const coef[6], const StepCommon &sc,
+static cudaError_t launch_k3_v(const Layout &L, FieldPtrs f, void *const coef[kNumCoef], const StepCommon &sc,
                                int64_t nsteps, cudaStream_t st) {
   auto kern = k3_resident<R, C, NT, CSM, MINB>;
-  const size_t smem = CSM ? (size_t)6 * (NT / Geom<R, C>::TPR) * kRowBytes + 1024 : 0;
+  const size_t smem = CSM ? (size_t)kNumCoef * (NT / Geom<R, C>::TPR) * kRowBytes + 1024 : 0;
   if (smem > 48 * 1024) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
@@ -474,7 +491,7 @@ static cudaError_t launch_k3_v(const Layout &L, FieldPtrs f, void *const coef[6]
   return cudaGetLastError();
 }
 template <typename R>
-static cudaError_t launch_k3_t(const Layout &L, FieldPtrs f, void *const coef[6], const StepCommon &sc,
+static cudaError_t launch_k3_t(const Layout &L, FieldPtrs f, void *const coef[kNumCoef], const StepCommon &sc,
                                int64_t nsteps, int NT, int variant, cudaStream_t st) {
   constexpr int CF = kRowBytes / sizeof(R), CH = CF / 2;
   if (variant == 0) switch (NT) {
@@ -492,20 +509,23 @@ static cudaError_t launch_k3_t(const Layout &L, FieldPtrs f, void *const coef[6]
   }
   return cudaErrorInvalidValue;
 }
-cudaError_t launch_k3(int dtype, const Layout &L, FieldPtrs f, void *const coef[6], const StepCommon &sc,
+cudaError_t launch_k3(int dtype, const Layout &L, FieldPtrs f, void *const coef[kNumCoef], const StepCommon &sc,
                       int64_t nsteps, int NT, int variant, cudaStream_t st) {
   return dtype == 0 ? launch_k3_t<double>(L, f, coef, sc, nsteps, NT, variant, st)
                     : launch_k3_t<float>(L, f, coef, sc, nsteps, NT, variant, st);
 }
 
 // K2 variants: {nodes per thread, threads per CTA, CTAs per SM aimed at}
-//   0: full row, 128 threads, 2 CTAs/SM     1: half row, 256 threads, 2 CTAs/SM
-//   2: full row, 256 threads, 1 CTA/SM      3: half row, 512 threads, 1 CTA/SM
-//   4: warp tiles (32 rows per warp), 8 warps, 1 CTA/SM      5: warp tiles, 4 warps, 2 CTAs/SM
-int k2_tile_rows(int variant) { const int r[] = {128, 128, 256, 256, 32, 32}; return (variant >= 0 && variant < 6) ? r[variant] : 0; }
-int k2_tiles_per_cta(int variant) { return variant == 4 ? 8 : variant == 5 ? 4 : 1; }
+//   0: CTA tile, full row, 128 threads, 2 CTAs/SM     1: CTA tile, half row, 256 threads, 2 CTAs/SM
+//   2: CTA tile, full row, 256 threads, 1 CTA/SM      3: CTA tile, half row, 512 threads, 1 CTA/SM
+//   4: warp tiles, 8 warps, 1 CTA/SM, TMA stores      5: warp tiles, 4 warps, 2 CTAs/SM, TMA stores
+//   6: warp tiles, 12 warps, 1 CTA/SM, 256-bit global stores
+//   7: warp tiles, 8 warps, 1 CTA/SM, 256-bit global stores
+int k2_tile_rows(int variant) { const int r[] = {128, 128, 256, 256, 32, 32, 32, 32}; return (variant >= 0 && variant < kK2Variants) ? r[variant] : 0; }
+int k2_tiles_per_cta(int variant) { const int t[] = {1, 1, 1, 1, 8, 4, 12, 8}; return (variant >= 0 && variant < kK2Variants) ? t[variant] : 0; }
 size_t k2_smem_bytes(int variant) {
-  return (size_t)12 * k2_tile_rows(variant) * k2_tiles_per_cta(variant) * kRowBytes + 1024;
+  const int arrays = variant >= 6 ? kNumIn : kNumIn + 3;
+  return (size_t)arrays * k2_tile_rows(variant) * k2_tiles_per_cta(variant) * kRowBytes + 1024;
 }
 
 template <typename R, int V> struct K2Variant;
@@ -532,8 +552,10 @@ static cudaError_t k2_configure_t(int variant, int *ctas) {
     case 1: return k2_configure_v<R, 1>(ctas);
     case 2: return k2_configure_v<R, 2>(ctas);
     case 3: return k2_configure_v<R, 3>(ctas);
-    case 4: return k2_configure_k(k2_wtile<R, 8, 1>, 4, 256, ctas);
-    case 5: return k2_configure_k(k2_wtile<R, 4, 2>, 5, 128, ctas);
+    case 4: return k2_configure_k(k2_wtile<R, 8, 1, false>, 4, 256, ctas);
+    case 5: return k2_configure_k(k2_wtile<R, 4, 2, false>, 5, 128, ctas);
+    case 6: return k2_configure_k(k2_wtile<R, 12, 1, true>, 6, 384, ctas);
+    case 7: return k2_configure_k(k2_wtile<R, 8, 1, true>, 7, 256, ctas);
   }
   return cudaErrorInvalidValue;
 }
@@ -542,42 +564,36 @@ cudaError_t k2_configure(int dtype, int variant, int *ctas) {
 }
 
 template <typename R, int V>
-static cudaError_t launch_k2_v(const Layout &L, const K2Plan &plan, int src_buf, const StepCommon &sc, int steps,
-                               cudaStream_t st) {
+static cudaError_t launch_k2_v(const K2Plan &plan, int src_buf, const StepParams<R> &sp, const K2Args &q, cudaStream_t st) {
   typedef K2Variant<R, V> KV;
-  K2Args q;
-  q.T = steps; q.HR = plan.HR; q.rows_out = plan.rows_out;
-  q.tiles_per_grid = plan.tiles_per_grid; q.total_tiles = plan.total_tiles; q.nrows = L.nrows;
-  k2_tblock<R, KV::C, KV::NT, KV::MINB><<<plan.grid, KV::NT, plan.smem_bytes, st>>>(plan.maps[src_buf],
-                                                                                   make_params<R>(sc), q);
+  k2_tblock<R, KV::C, KV::NT, KV::MINB><<<plan.grid, KV::NT, plan.smem_bytes, st>>>(plan.maps[src_buf], sp, q);
   return cudaGetLastError();
 }
 template <typename R>
-static cudaError_t launch_k2_t(const Layout &L, const K2Plan &plan, int src_buf, const StepCommon &sc, int steps,
-                               cudaStream_t st) {
+static cudaError_t launch_k2_t(const Layout &L, const K2Plan &plan, int src_buf, FieldPtrs dst, const StepCommon &sc,
+                               int steps, cudaStream_t st) {
+  K2Args q;
+  q.T = steps; q.HR = plan.HR; q.rows_out = plan.rows_out;
+  q.tiles_per_grid = plan.tiles_per_grid; q.total_tiles = plan.total_tiles; q.nrows = L.nrows;
+  const StepParams<R> sp = make_params<R>(sc);
+  const K2Maps &m = plan.maps[src_buf];
   switch (plan.variant) {
-    case 0: return launch_k2_v<R, 0>(L, plan, src_buf, sc, steps, st);
-    case 1: return launch_k2_v<R, 1>(L, plan, src_buf, sc, steps, st);
-    case 2: return launch_k2_v<R, 2>(L, plan, src_buf, sc, steps, st);
-    case 3: return launch_k2_v<R, 3>(L, plan, src_buf, sc, steps, st);
-    case 4:
-    case 5: {
-      K2Args q;
-      q.T = steps; q.HR = plan.HR; q.rows_out = plan.rows_out;
-      q.tiles_per_grid = plan.tiles_per_grid; q.total_tiles = plan.total_tiles; q.nrows = L.nrows;
-      if (plan.variant == 4)
-        k2_wtile<R, 8, 1><<<plan.grid, 256, plan.smem_bytes, st>>>(plan.maps[src_buf], make_params<R>(sc), q);
-      else
-        k2_wtile<R, 4, 2><<<plan.grid, 128, plan.smem_bytes, st>>>(plan.maps[src_buf], make_params<R>(sc), q);
-      return cudaGetLastError();
-    }
+    case 0: return launch_k2_v<R, 0>(plan, src_buf, sp, q, st);
+    case 1: return launch_k2_v<R, 1>(plan, src_buf, sp, q, st);
+    case 2: return launch_k2_v<R, 2>(plan, src_buf, sp, q, st);
+    case 3: return launch_k2_v<R, 3>(plan, src_buf, sp, q, st);
+    case 4: k2_wtile<R, 8, 1, false><<<plan.grid, 256, plan.smem_bytes, st>>>(m, sp, q, rp<R>(dst)); break;
+    case 5: k2_wtile<R, 4, 2, false><<<plan.grid, 128, plan.smem_bytes, st>>>(m, sp, q, rp<R>(dst)); break;
+    case 6: k2_wtile<R, 12, 1, true><<<plan.grid, 384, plan.smem_bytes, st>>>(m, sp, q, rp<R>(dst)); break;
+    case 7: k2_wtile<R, 8, 1, true><<<plan.grid, 256, plan.smem_bytes, st>>>(m, sp, q, rp<R>(dst)); break;
+    default: return cudaErrorInvalidValue;
   }
-  return cudaErrorInvalidValue;
+  return cudaGetLastError();
 }
-cudaError_t launch_k2(int dtype, const Layout &L, const K2Plan &plan, int src_buf, const StepCommon &sc, int steps,
-                      cudaStream_t st) {
-  return dtype == 0 ? launch_k2_t<double>(L, plan, src_buf, sc, steps, st)
-                    : launch_k2_t<float>(L, plan, src_buf, sc, steps, st);
+cudaError_t launch_k2(int dtype, const Layout &L, const K2Plan &plan, int src_buf, FieldPtrs dst, const StepCommon &sc,
+                      int steps, cudaStream_t st) {
+  return dtype == 0 ? launch_k2_t<double>(L, plan, src_buf, dst, sc, steps, st)
+                    : launch_k2_t<float>(L, plan, src_buf, dst, sc, steps, st);
 }
 
 }  // namespace rketd

@@ -25,7 +25,7 @@ CTR_LAUNCHES, CTR_STEP_LAUNCHES, CTR_KERNEL_USED, CTR_DEPTH_USED, CTR_STEPS_DONE
 
 EXPORTS = ["rketd_create", "rketd_set_media", "rketd_set_source", "rketd_set_probes", "rketd_set_probe_dft",
            "rketd_set_fields", "rketd_reset", "rketd_discard_records", "rketd_set_plan", "rketd_run", "rketd_read_probes",
-           "rketd_get_fields", "rketd_get_coefficients", "rketd_get_counter", "rketd_destroy", "rketd_last_error"]
+           "rketd_get_fields", "rketd_get_coefficients", "rketd_get_kernel_coefficients", "rketd_get_counter", "rketd_destroy", "rketd_last_error"]
 
 if not os.path.exists(LIB_PATH):
     raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_1709_00821_b200.build` "
@@ -46,13 +46,14 @@ _lib.rketd_run.argtypes = [_vp, _i64]
 _lib.rketd_read_probes.argtypes = [_vp, _vp, _i64, ctypes.POINTER(_i64)]
 _lib.rketd_get_fields.argtypes = [_vp, _vp, _vp, _vp]
 _lib.rketd_get_coefficients.argtypes = [_vp, _vp, _vp]
+_lib.rketd_get_kernel_coefficients.argtypes = [_vp, _vp]
 _lib.rketd_get_counter.argtypes = [_vp, _i32]
 _lib.rketd_get_counter.restype = _i64
 _lib.rketd_destroy.argtypes = [_vp]
 _lib.rketd_destroy.restype = None
 _lib.rketd_last_error.argtypes = [_vp]
 _lib.rketd_last_error.restype = ctypes.c_char_p
-for _n in EXPORTS[:13]:
+for _n in EXPORTS[:14]:
     getattr(_lib, _n).restype = _i32
 
 
@@ -142,6 +143,10 @@ def rketd_get_coefficients(h, out, chh_m=None):
     _check(h, _lib.rketd_get_coefficients(h, _ptr(out), _ptr(chh_m)))
 
 
+def rketd_get_kernel_coefficients(h, out):
+    _check(h, _lib.rketd_get_kernel_coefficients(h, _ptr(out)))
+
+
 def rketd_get_counter(h, which: int) -> int:
     return _lib.rketd_get_counter(h, which)
 
@@ -219,6 +224,11 @@ class Sim:
         d = {k: out[i] for i, k in enumerate(("ca", "cj", "ch", "ka", "kb", "kc"))}
         d["chh"], d["m"] = float(cm[0]), float(cm[1])
         return d
+
+    def get_kernel_coefficients(self):
+        out = np.empty((4, self.nbatch, self.ncells), np.float64)
+        rketd_get_kernel_coefficients(self.h, out)
+        return {k: out[i] for i, k in enumerate(("P", "ch", "ka", "Q"))}
 
     def close(self):
         if self.h is not None:

@@ -65,8 +65,8 @@ def check_fields(gpu, st, tol, peak=0.0, wp_max=0.0):
             assert np.max(np.abs(np.asarray(gpu[k], np.float64) - ref)) <= tol * scale, k
 
 
-ALL_PLANS = [(1, 0, -1), (3, 0, 0), (3, 0, 1)] + [(2, 0, v) for v in range(6)] + [(2, d, 4) for d in (1, 7, 16, 33)] + \
-            [(2, 5, 0), (2, 40, 2)]
+ALL_PLANS = [(1, 0, -1), (3, 0, 0), (3, 0, 1)] + [(2, 0, v) for v in range(8)] + [(2, d, 4) for d in (1, 7, 16, 33)] + \
+            [(2, d, 6) for d in (1, 2, 9, 32, 40)] + [(2, 5, 0), (2, 40, 2)]
 
 
 # ------------------------------------------------------------------------------------------ config 1
@@ -111,14 +111,59 @@ def test_coefficients_match_oracle_in_ulps(rk):
         # exp / expm1 between glibc and CUDA is amplified
         assert np.all(np.abs(c[k] - o[k])[~small] <= 1e-12 * np.abs(o[k])[~small]), k
     assert c["chh"] == o["chh"] and c["m"] == o["m"]
+    # the four arrays the kernels read: P = ca - cj kc, ch, ka, Q = ka cj kc + cj kb (rketd_device.cuh)
+    kc4 = s.get_kernel_coefficients()
     s.close()
-    # fp32 mode: fp64 values rounded once
+    kcp = o["cj"] * o["kc"]
+    want = {"P": o["ca"] - kcp, "ch": o["ch"], "ka": o["ka"], "Q": o["ka"] * kcp + o["cj"] * o["kb"]}
+    for k in ("P", "ch", "ka", "Q"):
+        ulp = np.abs(kc4[k] - want[k]) / np.maximum(np.spacing(np.abs(want[k])), 1e-300)
+        assert ulp[small].max() <= (8.0 if k == "Q" else 2.0), (k, ulp[small].max())
+        assert np.all(np.abs(kc4[k] - want[k])[~small] <= 1e-12 * np.abs(want[k])[~small] + 1e-300), k
+    # fp32 mode: the fp64 values rounded once; the six reported coefficients stay fp64
     s = rk.Sim(n, 3, wl.DZ, wl.DT, "f32")
     s.set_media(wp, nu)
     c32 = s.get_coefficients()
     for k in ("ca", "cj", "ch", "ka", "kb", "kc"):
-        assert np.array_equal(c32[k], c[k].astype(np.float32).astype(np.float64)), k
+        assert np.array_equal(c32[k], c[k]), k
+    k32 = s.get_kernel_coefficients()
+    for k in ("P", "ch", "ka", "Q"):
+        assert np.array_equal(k32[k], kc4[k].astype(np.float32).astype(np.float64)), k
     s.close()
+
+
+def test_media_and_fields_in_any_order(rk):
+    """The kernels carry G = cj J - cj kc E: set_fields before set_media, and a change of media with live
+    fields, must both keep E, H, J (checked against the oracle, which is called once per media)."""
+    rng = np.random.default_rng(11)
+    n, nb = 777, 2
+    wpA, wpB = (rng.uniform(0, 2 * np.pi * 40e9, (nb, n)) for _ in range(2))
+    nuA, nuB = (rng.uniform(0, 5e10, (nb, n)) for _ in range(2))
+    E0, H0, J0 = (rng.uniform(-1, 1, (nb, n)) for _ in range(3))
+    H0 /= 376.73
+    H0[:, -1] = 0.0
+    st = oracle.State(n, nb, E0, H0, J0)
+    rec1, _ = oracle.run(st, wpA, nuA, wl.DZ, wl.DT, 150, probes=[5, 700])
+    rec2, _ = oracle.run(st, wpB, nuB, wl.DZ, wl.DT, 150, probes=[5, 700])
+    ref = np.concatenate([rec1, rec2], axis=2)
+    for kernel in (1, 2, 3):
+        s = rk.Sim(n, nb, wl.DZ, wl.DT, "f64")
+        s.set_fields(E0, H0, J0)              # before the media
+        E, H, J = s.get_fields()
+        assert np.array_equal(J, J0) and np.array_equal(E, E0)
+        s.set_media(wpA, nuA)
+        E, H, J = s.get_fields()              # J -> G -> J round trip
+        assert np.max(np.abs(J - J0)) <= 4e-16 * np.max(np.abs(J0)) + 4e-16 * np.abs(E0).max() * 1e-2
+        s.set_probes([5, 700])
+        s.set_plan(kernel, 0, -1)
+        s.run(150)
+        s.set_media(wpB, nuB)                 # live fields: J is kept, G is re-derived
+        s.run(150)
+        assert grid_err(s.read_probes(), ref) <= 1e-12
+        E, H, J = s.get_fields()
+        assert np.max(np.abs(J - st.J)) <= 1e-12 * np.max(np.abs(st.J))
+        assert np.max(np.abs(E - st.E)) <= 1e-12 * np.max(np.abs(st.E))
+        s.close()
 
 
 # ------------------------------------------------------------------------------------------ reduced configs 2-5
