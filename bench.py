@@ -73,6 +73,7 @@ class ClockSampler:
     def __init__(self, index: int):
         self.index = index
         self.samples = []
+        self.power = []
         self.reasons = set()
         self.max_mhz = None
         self._stop = threading.Event()
@@ -97,6 +98,7 @@ class ClockSampler:
         while not self._stop.is_set():
             try:
                 self.samples.append(p.nvmlDeviceGetClockInfo(self._h, p.NVML_CLOCK_SM))
+                self.power.append(p.nvmlDeviceGetPowerUsage(self._h) / 1000.0)
                 r = p.nvmlDeviceGetCurrentClocksThrottleReasons(self._h)
                 for k, bit in names.items():
                     if r & bit:
@@ -134,8 +136,10 @@ class ClockSampler:
 
     def summary(self):
         s = sorted(self.samples)
+        w = sorted(self.power)
         return {"sm_mhz": s[len(s) // 2] if s else None, "sm_min_mhz": s[0] if s else None,
-                "sm_max_mhz": self.max_mhz, "samples": len(s), "reasons": sorted(self.reasons)}
+                "sm_max_mhz": self.max_mhz, "samples": len(s), "reasons": sorted(self.reasons),
+                "power_w": round(w[len(w) // 2], 1) if w else None}
 
 
 def measured_peaks():

@@ -175,7 +175,7 @@ int make_map(rketd_sim *s, CUtensorMap *m, void *base, int box_rows) {
   return RKETD_OK;
 }
 
-int default_depth(const rketd_sim *s) { return s->dtype == RKETD_F64 ? 24 : 32; }
+int default_depth(const rketd_sim *s) { return s->dtype == RKETD_F64 ? 16 : 32; }
 int default_k2_variant(const rketd_sim *) { return 6; }
 int default_k3_variant(const rketd_sim *) { return 0; }
 int max_depth(const rketd_sim *s, int variant) { return (k2_tile_rows(variant) / 2 - 1) * s->L.C; }
@@ -190,6 +190,7 @@ int build_k2_plan(rketd_sim *s, int depth, int variant) {
   P.variant = variant; P.rows = rows; P.HR = HR; P.rows_out = rows - 2 * HR; P.depth = depth;
   P.tiles_per_grid = (L.nrows + P.rows_out - 1) / P.rows_out;
   P.total_tiles = P.tiles_per_grid * L.nbatch;
+  if (P.total_tiles >= (int64_t)1 << 31) return fail(s, RKETD_EINVAL, "too many tiles for the temporal-blocking kernel");
   P.smem_bytes = k2_smem_bytes(variant);
   int ctas = 0, dev = 0, sms = 0;
   CU_TRY(s, k2_configure(s->dtype, variant, &ctas));

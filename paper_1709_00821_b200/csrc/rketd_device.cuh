@@ -9,7 +9,7 @@
 // define the scaled, shifted current  G := cj J - (cj kc) E.  Then, exactly:
 //   H'[k] = fma(-chh, E[k+1] - E[k], H[k])                                  2 flop-instr   eq. (14)
 //   E'[k] = fma(-ch, H'[k] - H'[k-1], fma(P, E[k], -G[k])),  P = ca - cj kc  3              eq. (12)+(11)
-//   G'[k] = fma(Q, E[k], ka * G[k]),                         Q = ka cj kc + cj kb   2       eq. (11)
+//   G'[k] = fma(ka, G[k], Q * E[k]),                         Q = ka cj kc + cj kb   2       eq. (11)
 // G' needs only OLD values, so Mur, the source and the probes (which change E') do not touch it, and
 // J is recovered on read-out as J = (G + cj kc E)/cj.  7 instructions and 4 per-node coefficients
 // (P, ch, ka, Q) per node and step instead of 9 and 6.
@@ -270,7 +270,7 @@ __device__ __forceinline__ void step_fields(const R (&E)[C], R (&En)[C], R (&H)[
   }
 }
 
-// a5 — eq. (11) in the G form: G' = Q E + ka G with the OLD E (independent of E').
+// a5 — eq. (11) in the G form: G' = ka G + Q E with the OLD E (independent of E').
 template <typename R, int C, typename CF>
 __device__ __forceinline__ void step_current(R (&G)[C], const R (&E)[C], const CF &cf) {
   typedef Arith<R> A;
@@ -281,7 +281,7 @@ __device__ __forceinline__ void step_current(R (&G)[C], const R (&E)[C], const C
     cf.template chunk<COEF_KA>(j, ka);
     cf.template chunk<COEF_Q>(j, cq);
 #pragma unroll
-    for (int u = 0; u < V; ++u) G[j * V + u] = A::fma(cq[u], E[j * V + u], A::mul(ka[u], G[j * V + u]));
+    for (int u = 0; u < V; ++u) G[j * V + u] = A::fma(ka[u], G[j * V + u], A::mul(cq[u], E[j * V + u]));
   }
 }
 

@@ -161,7 +161,8 @@ struct K2Args {
   int T;                  // steps this pass
   int HR;                 // halo rows
   int rows_out;           // ROWS - 2 HR
-  int64_t tiles_per_grid, total_tiles, nrows;
+  uint32_t tiles_per_grid, total_tiles;   // 32-bit on purpose: tile index arithmetic sits between two tiles
+  int64_t nrows;
 };
 constexpr int kNumIn = 3 + kNumCoef;      // arrays a tile loads: E, H, G, P, ch, ka, Q
 
@@ -215,11 +216,11 @@ __global__ void __launch_bounds__(NT, MINB) k2_tblock(const __grid_constant__ K2
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int row = tid / G::TPR, sub = tid % G::TPR;
 
-  auto issue_loads = [&](int64_t tile) {   // one elected thread
-    const int64_t g = tile / q.tiles_per_grid, ti = tile - g * q.tiles_per_grid;
-    const int row0 = (int)(ti * q.rows_out - q.HR);
+  auto issue_loads = [&](uint32_t tile) {   // one elected thread
+    const uint32_t g = tile / q.tiles_per_grid, ti = tile - g * q.tiles_per_grid;
+    const int row0 = (int)(ti * q.rows_out) - q.HR;
     mbar_expect_tx(&mbar, (uint32_t)kNumIn * kArrayBytes);
-#pragma unroll 1
+#pragma unroll
     for (int a = 0; a < kNumIn; ++a) tma_load_3d(sin + a * kArrayBytes, &maps.ld[a], &mbar, 0, row0, (int)g);
   };
 
@@ -229,7 +230,7 @@ __global__ void __launch_bounds__(NT, MINB) k2_tblock(const __grid_constant__ K2
     fence_barrier_init();
   }
   __syncthreads();
-  int64_t tile = blockIdx.x;
+  uint32_t tile = blockIdx.x;
   if (tid == 0 && tile < q.total_tiles) issue_loads(tile);
   uint32_t phase = 0;
 
@@ -243,8 +244,8 @@ __global__ void __launch_bounds__(NT, MINB) k2_tblock(const __grid_constant__ K2
   }
 
   for (; tile < q.total_tiles; tile += gridDim.x) {
-    const int64_t g = tile / q.tiles_per_grid, ti = tile - g * q.tiles_per_grid;
-    const int64_t rowg = ti * q.rows_out - q.HR + row;     // this thread's row in the grid
+    const uint32_t g = tile / q.tiles_per_grid, ti = tile - g * q.tiles_per_grid;
+    const int64_t rowg = (int64_t)ti * q.rows_out - q.HR + row;     // this thread's row in the grid
     const uint32_t flag = (rowg >= 0 && rowg < q.nrows) ? p.rowflag[rowg] : 0u;
 
     mbar_wait(&mbar, phase);
@@ -255,7 +256,7 @@ __global__ void __launch_bounds__(NT, MINB) k2_tblock(const __grid_constant__ K2
     tile_to_regs<R, C>(sin, off_in, kArrayBytes, E, H, J, cf);
     const bool special = __syncthreads_or(flag != 0u);   // barrier: everyone has left the input stage
     if (tid == 0) {
-      const int64_t next = tile + gridDim.x;
+      const uint32_t next = tile + gridDim.x;
       if (next < q.total_tiles) issue_loads(next);   // overlaps with the T steps below
       tma_wait_read0();                    // previous tile's stores have drained the output stage
     }
@@ -290,27 +291,31 @@ __device__ __forceinline__ void warp_step(const R (&E)[C], R (&En)[C], R (&H)[C]
                                           R &Er, R nchh, const StepParams<R> &p, uint32_t flag, int64_t k0, int64_t g,
                                           int64_t nloc, bool owner) {
   typedef Arith<R> A;
+  // Issue cost of an FP64 instruction on sm_100 = max(2, distinct 64-bit register operands) cycles per
+  // scheduler (measured): the two FMAs that multiply E[i] sit next to each other so that the
+  // second one finds E[i] in the operand-reuse cache, and nchh comes from the constant bank.
   H[C - 1] = A::fma(nchh, A::sub(Er, E[C - 1]), H[C - 1]);                    // a1, last node first
   const R Hl = __shfl_up_sync(0xffffffffu, H[C - 1], 1);
 #pragma unroll
   for (int i = 0; i < C - 1; ++i) H[i] = A::fma(nchh, A::sub(E[i + 1], E[i]), H[i]);
 #pragma unroll
-  for (int i = C - 1; i >= 1; --i)                                            // a2
-    En[i] = A::fma(-cf.c[COEF_CH][i], A::sub(H[i], H[i - 1]), A::fma(cf.c[COEF_P][i], E[i], -G[i]));
-  En[0] = A::fma(-cf.c[COEF_CH][0], A::sub(H[0], Hl), A::fma(cf.c[COEF_P][0], E[0], -G[0]));
+  for (int i = C - 1; i >= 0; --i) {
+    const R w = A::mul(cf.c[COEF_Q][i], E[i]);
+    const R t = A::fma(cf.c[COEF_P][i], E[i], -G[i]);
+    G[i] = A::fma(cf.c[COEF_KA][i], G[i], w);                                 // a5 (old E, old G)
+    En[i] = A::fma(-cf.c[COEF_CH][i], A::sub(H[i], i ? H[i - 1] : Hl), t);    // a2
+  }
   if constexpr (SPECIAL) {
     if (flag) step_special<R, C>(E, En, H, p, flag, k0, g, nloc, owner);       // a3, a4, a6
   }
   Er = __shfl_down_sync(0xffffffffu, En[0], 1);
-#pragma unroll
-  for (int i = 0; i < C; ++i) G[i] = A::fma(cf.c[COEF_Q][i], E[i], A::mul(cf.c[COEF_KA][i], G[i]));   // a5
 }
 
 template <bool SPECIAL, typename R, int C>
 __device__ __forceinline__ void warp_time_loop(R (&E)[C], R (&H)[C], R (&G)[C], const CoefRegs<R, C> &cf,
                                                const StepParams<R> &p, uint32_t flag, int64_t k0, int64_t g, bool owner,
                                                int nsteps) {
-  const R nchh = pin_register(p.nchh);
+  const R nchh = p.nchh;       // stays a constant-bank operand of the FMAs (one register read less each)
   int64_t nloc = p.n0;
   R Er = __shfl_down_sync(0xffffffffu, E[0], 1);
   R Eb[C];
@@ -347,17 +352,19 @@ __global__ void __launch_bounds__(NW * 32, MINB) k2_wtile(const __grid_constant_
   const uint32_t sout = sin + kNumIn * kArrayBytes;
   uint64_t *mbar = &mbars[warp];
 
-  auto issue_loads = [&](int64_t tile) {   // lane 0
-    const int64_t g = tile / q.tiles_per_grid, ti = tile - g * q.tiles_per_grid;
-    const int row0 = (int)(ti * q.rows_out - q.HR);
+  // (g, ti, first row) of a tile; 32-bit arithmetic: this sits on the serial path between two tiles
+  auto locate = [&](uint32_t tile, uint32_t &g, uint32_t &ti, int &row0) {
+    g = tile / q.tiles_per_grid;
+    ti = tile - g * q.tiles_per_grid;
+    row0 = (int)(ti * q.rows_out) - q.HR;
+  };
+  auto issue_loads = [&](uint32_t g, int row0) {   // lane 0
     mbar_expect_tx(mbar, (uint32_t)kNumIn * kArrayBytes);
-#pragma unroll 1
+#pragma unroll
     for (int a = 0; a < kNumIn; ++a) tma_load_3d(sin + a * kArrayBytes, &maps.ld[a], mbar, 0, row0, (int)g);
   };
-  auto row_flag = [&](int64_t tile) -> uint32_t {
-    if (tile >= q.total_tiles) return 0u;
-    const int64_t g = tile / q.tiles_per_grid, ti = tile - g * q.tiles_per_grid;
-    const int64_t rowg = ti * q.rows_out - q.HR + lane;
+  auto row_flag = [&](int row0) -> uint32_t {
+    const int64_t rowg = (int64_t)row0 + lane;
     return (rowg >= 0 && rowg < q.nrows) ? p.rowflag[rowg] : 0u;
   };
 
@@ -366,13 +373,18 @@ __global__ void __launch_bounds__(NW * 32, MINB) k2_wtile(const __grid_constant_
     fence_barrier_init();
   }
   __syncwarp();
-  const int64_t stride = (int64_t)gridDim.x * NW;
+  const uint32_t stride = gridDim.x * NW;
   // the warps of a CTA work on consecutive tiles, so that the tiles in flight at any time are neighbours
   // in memory and the halo rows two tiles share are served by L2
-  int64_t tile = (int64_t)blockIdx.x * NW + warp;
-  if (lane == 0 && tile < q.total_tiles) issue_loads(tile);
+  uint32_t tile = blockIdx.x * NW + warp;
+  uint32_t g = 0, ti = 0, flag = 0;
+  int row0 = 0;
+  if (tile < q.total_tiles) {
+    locate(tile, g, ti, row0);
+    if (lane == 0) issue_loads(g, row0);
+    flag = row_flag(row0);
+  }
   uint32_t phase = 0;
-  uint32_t flag = row_flag(tile);
 
   const int r_out = lane - q.HR;
   const bool owner = r_out >= 0 && r_out < q.rows_out;
@@ -384,8 +396,8 @@ __global__ void __launch_bounds__(NW * 32, MINB) k2_wtile(const __grid_constant_
   }
 
   for (; tile < q.total_tiles; tile += stride) {
-    const int64_t g = tile / q.tiles_per_grid, ti = tile - g * q.tiles_per_grid;
-    const int64_t rowg = ti * q.rows_out - q.HR + lane;
+    const int64_t rowg = (int64_t)row0 + lane;       // this lane's row in grid g
+    const uint32_t g_cur = g, ti_cur = ti;
 
     mbar_wait(mbar, phase);
     phase ^= 1u;
@@ -395,21 +407,22 @@ __global__ void __launch_bounds__(NW * 32, MINB) k2_wtile(const __grid_constant_
     tile_to_regs<R, C>(sin, off_in, kArrayBytes, E, H, J, cf);
     const bool special = __any_sync(0xffffffffu, flag != 0u);   // also: every lane has left the input stage
     const uint32_t myflag = flag;
-    if (lane == 0) {
-      const int64_t next = tile + stride;
-      if (next < q.total_tiles) issue_loads(next);   // overlaps with the T steps below
-      if (!DIRECT) tma_wait_read0();                 // previous tile's stores have drained the output stage
+    flag = 0u;
+    if (tile + stride < q.total_tiles) {             // next tile: loads and flags fly behind the steps below
+      locate(tile + stride, g, ti, row0);
+      if (lane == 0) issue_loads(g, row0);
+      flag = row_flag(row0);
     }
-    flag = row_flag(tile + stride);                  // next tile's flags: the load latency hides behind the steps
+    if (!DIRECT && lane == 0) tma_wait_read0();      // previous tile's stores have drained the output stage
 
     if (special)
-      warp_time_loop<true, R, C>(E, H, J, cf, p, myflag, rowg * C, g, owner, q.T);
+      warp_time_loop<true, R, C>(E, H, J, cf, p, myflag, rowg * C, g_cur, owner, q.T);
     else
-      warp_time_loop<false, R, C>(E, H, J, cf, p, 0u, 0, g, false, q.T);
+      warp_time_loop<false, R, C>(E, H, J, cf, p, 0u, 0, g_cur, false, q.T);
 
     if constexpr (DIRECT) {
       if (owner && rowg < q.nrows) {
-        const int64_t first = (g * q.nrows + rowg) * C;
+        const int64_t first = ((int64_t)g_cur * q.nrows + rowg) * C;
         store_nodes_global<R, C>(dst.E, first, E);
         store_nodes_global<R, C>(dst.H, first, H);
         store_nodes_global<R, C>(dst.J, first, J);
@@ -420,9 +433,9 @@ __global__ void __launch_bounds__(NW * 32, MINB) k2_wtile(const __grid_constant_
       fence_proxy_async_smem();
       __syncwarp();
       if (lane == 0) {
-        const int row_out0 = (int)(ti * q.rows_out);
-#pragma unroll 1
-        for (int a = 0; a < 3; ++a) tma_store_3d(&maps.st[a], sout + a * kArrayBytes, 0, row_out0, (int)g);
+        const int row_out0 = (int)(ti_cur * q.rows_out);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) tma_store_3d(&maps.st[a], sout + a * kArrayBytes, 0, row_out0, (int)g_cur);
         tma_commit();
       }
     }
@@ -574,7 +587,7 @@ static cudaError_t launch_k2_t(const Layout &L, const K2Plan &plan, int src_buf,
                                int steps, cudaStream_t st) {
   K2Args q;
   q.T = steps; q.HR = plan.HR; q.rows_out = plan.rows_out;
-  q.tiles_per_grid = plan.tiles_per_grid; q.total_tiles = plan.total_tiles; q.nrows = L.nrows;
+  q.tiles_per_grid = (uint32_t)plan.tiles_per_grid; q.total_tiles = (uint32_t)plan.total_tiles; q.nrows = L.nrows;
   const StepParams<R> sp = make_params<R>(sc);
   const K2Maps &m = plan.maps[src_buf];
   switch (plan.variant) {
