@@ -183,6 +183,24 @@ def cpu_baseline(w, target_updates_serial=6e8, target_updates_omp=2.5e9):
             "serial_sample": out["serial"][1] + f" (serial build, 1 thread, {out['serial'][2]:.1f} s)"}
 
 
+def max_over_ranks(x: float, world: int, device: str = "cuda") -> float:
+    """Multi-GPU timing rule: a job is as slow as its slowest rank (all-reduce MAX over the process group;
+    NCCL on the GPU box, gloo in the CPU test of this host logic)."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_gcells(world: int, units_per_replica_step: int, steps: int, seconds: float) -> float:
+    """The path does not shard (BASELINE: "no multi-GPU sharding"): N ranks = N independent replicas of the
+    same workload, no collective on the data path; whole-job throughput = N x replica work / slowest rank."""
+    return world * units_per_replica_step * steps / seconds / 1e9
+
+
 def run_reference(args):
     """--impl reference: the CPU oracle on this host's cores, same metric/config, bounded sample per step."""
     rank = int(os.environ.get("RANK", "0"))
@@ -306,11 +324,8 @@ def main():
     kernel_used = sim.counter(rketd.CTR_KERNEL_USED)
     depth = sim.counter(rketd.CTR_DEPTH_USED)
     tile_cells, halo_cells = sim.counter(rketd.CTR_TILE_CELLS), sim.counter(rketd.CTR_HALO_CELLS)
-    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms = float(t.item())
-    value = world * units_per_step * args.steps / (ms * 1e-3) / 1e9
+    ms = max_over_ranks(ms, world)
+    value = whole_job_gcells(world, units_per_step, args.steps, ms * 1e-3)
 
     # ---- roofline of the dominant kernel (the stencil kernel: K2 / K3 / K1) -----------------------------------
     hbm_gbs, peak_src, sm_max = measured_peaks()
@@ -366,11 +381,8 @@ def main():
             e2e_step()
         barrier()
         dt = time.perf_counter() - t0
-        tt = torch.tensor([dt], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        dt = float(tt.item())
-        e2e = {"value": world * units_per_step * nrep / dt / 1e9, "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+        dt = max_over_ranks(dt, world)
+        e2e = {"value": whole_job_gcells(world, units_per_step, nrep, dt), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                "d2h_bytes_per_step": int(d2h), "steps": nrep,
                "note": "set_media(wp, nu) + set_fields(E0) from pinned host, rketd_run, read_probes to pinned host"}
         del wp_h, nu_h, E0_h, out_h

@@ -191,7 +191,7 @@ def config4(ncells: int = 1 << 28, nsteps: int = 1000, noise: bool = True) -> Wo
             return None
         return _block_noise(4, 1, lo, hi, 1e-3)[None, :].copy()
 
-    probes = [((2 * i + 1) * N) // 32 for i in range(16)] + [N // 2 - 256, N // 2 + 256]
+    probes = [((2 * i + 1) * N) // 32 for i in range(16)] + [N // 2 - 256, N // 2, N // 2 + 256]   # N/2: the source node
     probes += [int(v) for v in _rng(4, 2).integers(0, N, 16)]
     return Workload("config4_line_2p28" if N == 1 << 28 else f"config4_line_{N}", 4, N, 1, nsteps, DZ, DT,
                     SRC_GAUSS_DERIV, _SRC, N // 2, np.array(sorted(set(probes)), np.int64), None,

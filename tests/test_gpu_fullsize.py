@@ -15,6 +15,7 @@ from paper_1709_00821_b200 import workloads as wl
 
 pytestmark = pytest.mark.gpu
 TOL = {"f64": 1e-12, "f32": 1e-5}
+UNIT_ROUNDOFF = {"f64": 2.0 ** -53, "f32": 2.0 ** -24}
 
 
 @pytest.fixture(scope="module")
@@ -37,18 +38,25 @@ def _line_parity(rk, w, dtype, nwindows=64, wlen=4096):
     # every probe record against a windowed oracle run (light cone of n steps + 1)
     worst = 0.0
     peak = 0.0
+    worst_rel = 0.0
     for i, p in enumerate(w.probes):
         lo, hi = max(0, int(p) - n - 1), min(w.ncells, int(p) + n + 2)
         o = oracle.run_workload(w, cells=(lo, hi))
         j = o["probe_cells"].index(int(p))
-        peak = max(peak, np.max(np.abs(o["rec"][0][j])))
-        worst = max(worst, np.max(np.abs(rec[0][i] - o["rec"][0][j])))
-    assert peak > 0 and worst <= TOL[dtype] * peak, (worst, peak)
+        pk = np.max(np.abs(o["rec"][0][j]))
+        d = np.max(np.abs(rec[0][i] - o["rec"][0][j]))
+        assert pk > 0, ("vacuous: oracle record identically zero at probe", int(p))
+        peak, worst, worst_rel = max(peak, pk), max(worst, d), max(worst_rel, d / pk)
+    # north_star tolerance: error over every probe sample against the field peak of the grid (SURVEY §8(c)
+    # tolerance rule; the source node is a probe of config 4, so the peak is the driven field, ~1)
+    assert worst <= TOL[dtype] * peak, (worst, peak)
+    # per-probe figure, held to the drift bound DESIGN.md derives: one unit roundoff per step
+    assert worst_rel <= n * UNIT_ROUNDOFF[dtype], worst_rel
     # random windows of the final state
     rng = np.random.default_rng(99)
     starts = list(rng.integers(0, w.ncells - wlen, nwindows - 3)) + [0, w.ncells - wlen, w.src_cell - wlen // 2]
     for a in starts:
-        a = int(a)
+        a = min(max(int(a), 0), w.ncells - wlen)
         lo, hi = max(0, a - n - 1), min(w.ncells, a + wlen + n + 1)
         st = oracle.run_workload(w, cells=(lo, hi))["state"]
         for name, dev, ref in (("E", E, st.E), ("H", H, st.H), ("J", J, st.J)):
