@@ -48,6 +48,11 @@ FP64_LANES_PER_SM = 64        # DFMA per SM per clock (B200: 40 TFLOP/s fp64 / 1
 FP32_LANES_PER_SM = 128
 FP_INSTR_PER_CELL_STEP = 7    # kernel form (rketd_device.cuh): H 2, E 3, G 2  (SURVEY §8(d) counts 9 for the plain form)
 ARRAYS_PER_PASS = 10          # read E, H, G, P, ch, ka, Q; write E, H, G
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+# `ncu --set full` captures (profiles/*.md name the command); key = (workload, dtype, depth T, K2 variant)
+NCU_TRAFFIC_BYTES = {
+    ("config4_line_2p28", "f64", 16, 6): 22.86e9,    # profiles/r01_ncu_full_k2_wtile_config4_f64.md
+}
 
 
 def make_workload(name: str):
@@ -343,8 +348,9 @@ def main():
     else:
         alg_bytes = ARRAYS_PER_PASS * esize * ncell_total                                        # per launch (one pass)
         achieved = alg_bytes / (ms_per_launch * 1e-3) / 1e9
+        variant_used = args.variant if args.variant >= 0 else 6
         roof = {"bound": "hbm", "achieved": achieved, "peak": hbm_gbs, "unit": "GB/s", "frac": achieved / hbm_gbs,
-                "traffic": None, "peak_source": peak_src,
+                "traffic": NCU_TRAFFIC_BYTES.get((w.name, args.dtype, int(depth), variant_used)), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": alg_bytes, "ms_per_launch": ms_per_launch,
                 "depth_T": depth, "tile_cells": tile_cells, "halo_cells": halo_cells,
                 "frac_vs_8TBps_nominal": achieved / 8000.0,

@@ -194,13 +194,46 @@ struct CoefSmem {
   }
 };
 
+// ---- source samples (a4) without a global load on the time loop's critical path: a warp that holds the
+// source node keeps 32 consecutive samples of the table in one register per lane (lane i <-> step base + i), with
+// the next 32 already in flight, and picks the sample of the current step by shuffle.  Every call is warp-uniform.
+template <typename R>
+struct SourceStream {
+  R cur, nxt;
+  int64_t base;
+  bool on;
+  __device__ __forceinline__ R fetch(const StepParams<R> &p, int64_t idx) const {
+    return (p.src_tab != nullptr && idx < p.rec_stride) ? p.src_tab[idx] : R(0);
+  }
+  // on: some lane of this warp holds the source node (warp-uniform)
+  __device__ __forceinline__ void start(const StepParams<R> &p, bool warp_has_source, int64_t n0, int lane) {
+    on = warp_has_source;
+    base = n0;
+    cur = R(0);
+    nxt = R(0);
+    if (on) {
+      cur = fetch(p, base + lane);
+      nxt = fetch(p, base + 32 + lane);
+    }
+  }
+  __device__ __forceinline__ R sample(const StepParams<R> &p, int64_t nloc, int lane) {
+    if (!on) return R(0);
+    if (nloc - base >= 32) {
+      cur = nxt;
+      base += 32;
+      nxt = fetch(p, base + 32 + lane);
+    }
+    return __shfl_sync(0xffffffffu, cur, (int)(nloc - base));
+  }
+};
+
 // ---- Mur (a3), soft source (a4), probe record (a6) and padding hygiene for the threads whose
 // nodes include a boundary, the source or a probe.  E: old values, En: new values (modified), H: new
 // values (padding zeroed).  k0: physical in-grid index of the thread's first node; g: grid; nloc:
 // local step index; owner: this thread records probes among its nodes.
 template <typename R, int C>
 __device__ __forceinline__ void step_special(const R (&E)[C], R (&En)[C], R (&H)[C], const StepParams<R> &p,
-                                             uint32_t flag, int64_t k0, int64_t g, int64_t nloc, bool owner) {
+                                             uint32_t flag, int64_t k0, int64_t g, int64_t nloc, bool owner, R src_now) {
   typedef Arith<R> A;
   if (flag & F_MURL) {   // a3, left end.  The layout guarantees node 1 is held by the same thread.
 #pragma unroll
@@ -218,11 +251,10 @@ __device__ __forceinline__ void step_special(const R (&E)[C], R (&En)[C], R (&H)
     for (int i = 0; i < C; ++i)
       if (k0 + i >= p.cellR) H[i] = R(0);     // H[ncells-1] and padding
   }
-  if (flag & F_SRC) {    // a4: soft source
-    const R s = p.src_tab[nloc];
+  if (flag & F_SRC) {    // a4: soft source (sample of this step, streamed by SourceStream)
 #pragma unroll
     for (int i = 0; i < C; ++i)
-      if (k0 + i == p.cellS) En[i] = A::add(En[i], s);
+      if (k0 + i == p.cellS) En[i] = A::add(En[i], src_now);
   }
   if ((flag & F_PROBE) && owner && p.rec) {   // a6: probe record
     for (int q = 0; q < p.nprobes; ++q) {
@@ -246,7 +278,7 @@ __device__ __forceinline__ void step_special(const R (&E)[C], R (&En)[C], R (&H)
 template <bool SPECIAL, typename R, int C, typename CF>
 __device__ __forceinline__ void step_fields(const R (&E)[C], R (&En)[C], R (&H)[C], const R (&G)[C], const CF &cf, R El,
                                             R Hl, R Er, R nchh, const StepParams<R> &p, uint32_t flag, int64_t k0,
-                                            int64_t g, int64_t nloc, bool owner) {
+                                            int64_t g, int64_t nloc, bool owner, R src_now) {
   typedef Arith<R> A;
   constexpr int V = 16 / sizeof(R);
   // a1: H update, eq. (14)
@@ -266,7 +298,7 @@ __device__ __forceinline__ void step_fields(const R (&E)[C], R (&En)[C], R (&H)[
     }
   }
   if constexpr (SPECIAL) {
-    if (flag) step_special<R, C>(E, En, H, p, flag, k0, g, nloc, owner);
+    if (flag) step_special<R, C>(E, En, H, p, flag, k0, g, nloc, owner, src_now);
   }
 }
 

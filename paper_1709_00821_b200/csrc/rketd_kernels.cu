@@ -47,7 +47,8 @@ __global__ void __launch_bounds__(128) k1_step(RowPtrs<R> src, RowPtrs<R> dst, C
   const R Hl = row > 0 ? src.H[r * C - 1] : R(0);
   const R Er = row < nrows - 1 ? src.E[(r + 1) * C] : R(0);
   const uint32_t flag = p.rowflag[row];
-  step_fields<true, R, C>(E, En, H, G, cf, El, Hl, Er, p.nchh, p, flag, row * C, g, p.n0, true);
+  const R src_now = (flag & F_SRC) ? p.src_tab[p.n0] : R(0);
+  step_fields<true, R, C>(E, En, H, G, cf, El, Hl, Er, p.nchh, p, flag, row * C, g, p.n0, true, src_now);
   step_current<R, C>(G, E, cf);
   store_nodes_global<R, C>(dst.E, r * C, En);
   store_nodes_global<R, C>(dst.H, r * C, H);
@@ -68,8 +69,11 @@ __device__ __forceinline__ void time_loop(R (&E)[C], R (&H)[C], R (&J)[C], const
   __syncthreads();
   recv_halo<R, NW>(hs, 0, warp, lane, El, Hl, Er);
   R Eb[C];
+  SourceStream<R> src;
+  src.start(p, SPECIAL && __any_sync(0xffffffffu, (flag & F_SRC) != 0u), nloc, lane);
   auto one_step = [&](const R (&Ein)[C], R (&Eout)[C], int par) {
-    step_fields<SPECIAL, R, C>(Ein, Eout, H, J, cf, El, Hl, Er, nchh, p, flag, k0, g, nloc, owner);
+    const R src_now = SPECIAL ? src.sample(p, nloc, lane) : R(0);
+    step_fields<SPECIAL, R, C>(Ein, Eout, H, J, cf, El, Hl, Er, nchh, p, flag, k0, g, nloc, owner, src_now);
     send_halo<R, C, NW>(Eout, H, hs, par, warp, lane, El, Hl, Er);     // for the next step
     step_current<R, C>(J, Ein, cf);
     __syncthreads();
@@ -289,7 +293,7 @@ __global__ void __launch_bounds__(NT, MINB) k2_tblock(const __grid_constant__ K2
 template <bool SPECIAL, typename R, int C>
 __device__ __forceinline__ void warp_step(const R (&E)[C], R (&En)[C], R (&H)[C], R (&G)[C], const CoefRegs<R, C> &cf,
                                           R &Er, R nchh, const StepParams<R> &p, uint32_t flag, int64_t k0, int64_t g,
-                                          int64_t nloc, bool owner) {
+                                          int64_t nloc, bool owner, R src_now) {
   typedef Arith<R> A;
   // Issue cost of an FP64 instruction on sm_100 = max(2, distinct 64-bit register operands) cycles per
   // scheduler (measured): the two FMAs that multiply E[i] sit next to each other so that the
@@ -306,7 +310,7 @@ __device__ __forceinline__ void warp_step(const R (&E)[C], R (&En)[C], R (&H)[C]
     En[i] = A::fma(-cf.c[COEF_CH][i], A::sub(H[i], i ? H[i - 1] : Hl), t);    // a2
   }
   if constexpr (SPECIAL) {
-    if (flag) step_special<R, C>(E, En, H, p, flag, k0, g, nloc, owner);       // a3, a4, a6
+    if (flag) step_special<R, C>(E, En, H, p, flag, k0, g, nloc, owner, src_now);       // a3, a4, a6
   }
   Er = __shfl_down_sync(0xffffffffu, En[0], 1);
 }
@@ -319,14 +323,20 @@ __device__ __forceinline__ void warp_time_loop(R (&E)[C], R (&H)[C], R (&G)[C], 
   int64_t nloc = p.n0;
   R Er = __shfl_down_sync(0xffffffffu, E[0], 1);
   R Eb[C];
+  const int lane = threadIdx.x & 31;
+  SourceStream<R> src;
+  src.start(p, SPECIAL && __any_sync(0xffffffffu, (flag & F_SRC) != 0u), nloc, lane);
   int left = nsteps;
   for (; left >= 2; left -= 2) {
-    warp_step<SPECIAL, R, C>(E, Eb, H, G, cf, Er, nchh, p, flag, k0, g, nloc, owner);
-    warp_step<SPECIAL, R, C>(Eb, E, H, G, cf, Er, nchh, p, flag, k0, g, nloc + 1, owner);
+    const R s0 = SPECIAL ? src.sample(p, nloc, lane) : R(0);
+    warp_step<SPECIAL, R, C>(E, Eb, H, G, cf, Er, nchh, p, flag, k0, g, nloc, owner, s0);
+    const R s1 = SPECIAL ? src.sample(p, nloc + 1, lane) : R(0);
+    warp_step<SPECIAL, R, C>(Eb, E, H, G, cf, Er, nchh, p, flag, k0, g, nloc + 1, owner, s1);
     nloc += 2;
   }
   if (left) {
-    warp_step<SPECIAL, R, C>(E, Eb, H, G, cf, Er, nchh, p, flag, k0, g, nloc, owner);
+    const R s0 = SPECIAL ? src.sample(p, nloc, lane) : R(0);
+    warp_step<SPECIAL, R, C>(E, Eb, H, G, cf, Er, nchh, p, flag, k0, g, nloc, owner, s0);
 #pragma unroll
     for (int i = 0; i < C; ++i) E[i] = Eb[i];
   }
