@@ -69,6 +69,9 @@ def make_workload(name: str):
         return wl.config1()
     if name.startswith("config4:"):          # config4:<log2 cells> (development aid)
         return wl.config4(ncells=1 << int(name.split(":")[1]))
+    if name.startswith(("config3:", "config5:")):   # config3:<nbatch>:<nsteps> (development aid, e.g. short ncu captures)
+        f = name.split(":")
+        return (wl.config3 if f[0] == "config3" else wl.config5)(nbatch=int(f[1]), nsteps=int(f[2]))
     raise SystemExit(f"unknown workload {name}")
 
 

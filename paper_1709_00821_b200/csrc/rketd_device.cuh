@@ -17,6 +17,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <type_traits>
+
 namespace rketd {
 
 constexpr int kRowBytes = 64;       // one thread owns 64 B (or 32 B) of every array
@@ -172,6 +174,23 @@ struct CoefRegs {
   }
 };
 
+// Coefficients of a thread whose C nodes all carry the same four values (piecewise-constant media: every row that
+// does not straddle a media interface): one register per array.
+template <typename R, int C>
+struct CoefUniform {
+  static constexpr int V = 16 / sizeof(R);
+  R v[kNumCoef];
+  template <int a>
+  __device__ __forceinline__ void chunk(int, R (&out)[V]) const {
+#pragma unroll
+    for (int u = 0; u < V; ++u) out[u] = v[a];
+  }
+};
+
+// Block barrier by PTX: warps of one CTA may reach it from different instantiations of the time loop (K3 picks the
+// coefficient source per warp); bar.sync counts arriving warps, not program counters.
+__device__ __forceinline__ void cta_barrier() { asm volatile("bar.sync 0;" ::: "memory"); }
+
 // Coefficients held in shared memory: kNumCoef arrays of ROWS swizzled 64-B rows.
 template <typename R, int C, int ROWS>
 struct CoefSmem {
@@ -227,44 +246,81 @@ struct SourceStream {
   }
 };
 
-// ---- Mur (a3), soft source (a4), probe record (a6) and padding hygiene for the threads whose
-// nodes include a boundary, the source or a probe.  E: old values, En: new values (modified), H: new
-// values (padding zeroed).  k0: physical in-grid index of the thread's first node; g: grid; nloc:
-// local step index; owner: this thread records probes among its nodes.
+// ---- Mur (a3), soft source (a4), probe record (a6) and padding hygiene for the threads whose nodes include a
+// boundary, the source or a probe.  These threads run alone in their warp (divergent), so what counts is the
+// number of instructions on that path: everything that does not change from step to step is worked out once
+// per tile (SpecialIdx, 32-bit local indices) and the time loop only dispatches on small integers.
+struct SpecialIdx {
+  int iL = -1, iR = -1, iS = -1;   // local index (0..C-1) of node 0 / node ncells-1 / the source node, or -1
+  int np = 0;                      // probes among this thread's nodes that it records: 0, 1, 2; 3 = more (generic loop)
+  int pi0 = -1, pi1 = -1;          // local indices of the first two
+  int64_t pr0 = 0, pr1 = 0;        // their record offsets (grid * nprobes + q) * rec_stride; np == 3: k0 and grid
+  bool any = false;
+};
+
+// k0: physical in-grid index of the thread's first node; g: grid; owner: this thread records the probes among
+// its nodes (halo threads of a K2 tile do not).
 template <typename R, int C>
-__device__ __forceinline__ void step_special(const R (&E)[C], R (&En)[C], R (&H)[C], const StepParams<R> &p,
-                                             uint32_t flag, int64_t k0, int64_t g, int64_t nloc, bool owner, R src_now) {
-  typedef Arith<R> A;
-  if (flag & F_MURL) {   // a3, left end.  The layout guarantees node 1 is held by the same thread.
-#pragma unroll
-    for (int i = 0; i < C - 1; ++i)
-      if (k0 + i == p.cellL) En[i] = A::fma(p.mur_m, A::sub(En[i + 1], E[i]), E[i + 1]);
-#pragma unroll
-    for (int i = 0; i < C; ++i)
-      if (k0 + i < p.cellL) H[i] = R(0);      // padding left of node 0
-  }
-  if (flag & F_MURR) {   // a3, right end.  Node ncells-2 is held by the same thread.
-#pragma unroll
-    for (int i = 1; i < C; ++i)
-      if (k0 + i == p.cellR) En[i] = A::fma(p.mur_m, A::sub(En[i - 1], E[i]), E[i - 1]);
-#pragma unroll
-    for (int i = 0; i < C; ++i)
-      if (k0 + i >= p.cellR) H[i] = R(0);     // H[ncells-1] and padding
-  }
-  if (flag & F_SRC) {    // a4: soft source (sample of this step, streamed by SourceStream)
-#pragma unroll
-    for (int i = 0; i < C; ++i)
-      if (k0 + i == p.cellS) En[i] = A::add(En[i], src_now);
-  }
-  if ((flag & F_PROBE) && owner && p.rec) {   // a6: probe record
+__device__ __forceinline__ SpecialIdx make_special(const StepParams<R> &p, uint32_t flag, int64_t k0, int64_t g, bool owner) {
+  SpecialIdx sx;
+  if (!flag) return sx;
+  if (flag & F_MURL) { const int64_t d = p.cellL - k0; if (d >= 0 && d < C) sx.iL = (int)d; }
+  if (flag & F_MURR) { const int64_t d = p.cellR - k0; if (d >= 0 && d < C) sx.iR = (int)d; }
+  if (flag & F_SRC)  { const int64_t d = p.cellS - k0; if (d >= 0 && d < C) sx.iS = (int)d; }
+  if ((flag & F_PROBE) && owner && p.rec) {
     for (int q = 0; q < p.nprobes; ++q) {
       const int64_t d = p.probe_cell[q] - k0;
       if (d >= 0 && d < C) {
-        R v = En[0];
+        const int64_t off = (g * p.nprobes + q) * p.rec_stride;
+        if (sx.np == 0) { sx.pi0 = (int)d; sx.pr0 = off; }
+        else if (sx.np == 1) { sx.pi1 = (int)d; sx.pr1 = off; }
+        sx.np = sx.np < 3 ? sx.np + 1 : 3;
+      }
+    }
+  }
+  if (sx.np == 3) { sx.pr0 = k0; sx.pr1 = g; }
+  sx.any = sx.iL >= 0 || sx.iR >= 0 || sx.iS >= 0 || sx.np > 0;
+  return sx;
+}
+
+// f(integral_constant<int, i>) for the i in [I, C) that equals idx: an else-if chain over compile-time indices,
+// so that register arrays are indexed statically and the chain stops at the hit
+template <int I, int C, typename F>
+__device__ __forceinline__ void at_index(int idx, F &&f) {
+  if constexpr (I < C) {
+    if (idx == I) f(std::integral_constant<int, I>{});
+    else at_index<I + 1, C>(idx, f);
+  }
+}
+
+// E: old values, En: new values (modified), H: new values (padding zeroed).
+template <typename R, int C>
+__device__ __forceinline__ void step_special(const R (&E)[C], R (&En)[C], R (&H)[C], const StepParams<R> &p,
+                                             const SpecialIdx &sx, int64_t nloc, R src_now) {
+  typedef Arith<R> A;
+  if (sx.iL >= 0) {   // a3, left end.  The layout puts node 0 at local index 0 or 1, node 1 in the same thread.
+    if (sx.iL == 0) En[0] = A::fma(p.mur_m, A::sub(En[1], E[0]), E[1]);
+    else { En[1] = A::fma(p.mur_m, A::sub(En[2], E[1]), E[2]); H[0] = R(0); }      // H[0]: padding left of node 0
+  }
+  if (sx.iR >= 0) {   // a3, right end.  Node ncells-2 is held by the same thread.
+    at_index<1, C>(sx.iR, [&](auto ic) {
+      constexpr int i = decltype(ic)::value;
+      En[i] = A::fma(p.mur_m, A::sub(En[i - 1], E[i]), E[i - 1]);
 #pragma unroll
-        for (int i = 1; i < C; ++i)
-          if (d == i) v = En[i];
-        p.rec[(g * p.nprobes + q) * p.rec_stride + nloc] = v;
+      for (int j = i; j < C; ++j) H[j] = R(0);                                     // H[ncells-1] and padding
+    });
+  }
+  if (sx.iS >= 0)     // a4: soft source (sample of this step, streamed by SourceStream)
+    at_index<0, C>(sx.iS, [&](auto ic) { En[decltype(ic)::value] = A::add(En[decltype(ic)::value], src_now); });
+  if (sx.np > 0) {    // a6: probe record
+    if (sx.np <= 2) {
+      at_index<0, C>(sx.pi0, [&](auto ic) { p.rec[sx.pr0 + nloc] = En[decltype(ic)::value]; });
+      if (sx.np == 2) at_index<0, C>(sx.pi1, [&](auto ic) { p.rec[sx.pr1 + nloc] = En[decltype(ic)::value]; });
+    } else {          // more than two probes in one thread's nodes: generic loop
+      for (int q = 0; q < p.nprobes; ++q) {
+        const int64_t d = p.probe_cell[q] - sx.pr0;
+        if (d >= 0 && d < C)
+          at_index<0, C>((int)d, [&](auto ic) { p.rec[(sx.pr1 * p.nprobes + q) * p.rec_stride + nloc] = En[decltype(ic)::value]; });
       }
     }
   }
@@ -277,8 +333,8 @@ __device__ __forceinline__ void step_special(const R (&E)[C], R (&En)[C], R (&H)
 // SPECIAL = false compiles the boundary/source/probe handling out (tiles without such rows).
 template <bool SPECIAL, typename R, int C, typename CF>
 __device__ __forceinline__ void step_fields(const R (&E)[C], R (&En)[C], R (&H)[C], const R (&G)[C], const CF &cf, R El,
-                                            R Hl, R Er, R nchh, const StepParams<R> &p, uint32_t flag, int64_t k0,
-                                            int64_t g, int64_t nloc, bool owner, R src_now) {
+                                            R Hl, R Er, R nchh, const StepParams<R> &p, const SpecialIdx &sx,
+                                            int64_t nloc, R src_now) {
   typedef Arith<R> A;
   constexpr int V = 16 / sizeof(R);
   // a1: H update, eq. (14)
@@ -298,7 +354,7 @@ __device__ __forceinline__ void step_fields(const R (&E)[C], R (&En)[C], R (&H)[
     }
   }
   if constexpr (SPECIAL) {
-    if (flag) step_special<R, C>(E, En, H, p, flag, k0, g, nloc, owner, src_now);
+    if (sx.any) step_special<R, C>(E, En, H, p, sx, nloc, src_now);
   }
 }
 

@@ -48,7 +48,8 @@ __global__ void __launch_bounds__(128) k1_step(RowPtrs<R> src, RowPtrs<R> dst, C
   const R Er = row < nrows - 1 ? src.E[(r + 1) * C] : R(0);
   const uint32_t flag = p.rowflag[row];
   const R src_now = (flag & F_SRC) ? p.src_tab[p.n0] : R(0);
-  step_fields<true, R, C>(E, En, H, G, cf, El, Hl, Er, p.nchh, p, flag, row * C, g, p.n0, true, src_now);
+  const SpecialIdx sx = make_special<R, C>(p, flag, row * C, g, true);
+  step_fields<true, R, C>(E, En, H, G, cf, El, Hl, Er, p.nchh, p, sx, p.n0, src_now);
   step_current<R, C>(G, E, cf);
   store_nodes_global<R, C>(dst.E, r * C, En);
   store_nodes_global<R, C>(dst.H, r * C, H);
@@ -66,17 +67,18 @@ __device__ __forceinline__ void time_loop(R (&E)[C], R (&H)[C], R (&J)[C], const
   int64_t nloc = p.n0;
   R El, Hl, Er;
   send_halo<R, C, NW>(E, H, hs, 0, warp, lane, El, Hl, Er);
-  __syncthreads();
+  cta_barrier();
   recv_halo<R, NW>(hs, 0, warp, lane, El, Hl, Er);
   R Eb[C];
   SourceStream<R> src;
   src.start(p, SPECIAL && __any_sync(0xffffffffu, (flag & F_SRC) != 0u), nloc, lane);
+  const SpecialIdx sx = SPECIAL ? make_special<R, C>(p, flag, k0, g, owner) : SpecialIdx();
   auto one_step = [&](const R (&Ein)[C], R (&Eout)[C], int par) {
     const R src_now = SPECIAL ? src.sample(p, nloc, lane) : R(0);
-    step_fields<SPECIAL, R, C>(Ein, Eout, H, J, cf, El, Hl, Er, nchh, p, flag, k0, g, nloc, owner, src_now);
+    step_fields<SPECIAL, R, C>(Ein, Eout, H, J, cf, El, Hl, Er, nchh, p, sx, nloc, src_now);
     send_halo<R, C, NW>(Eout, H, hs, par, warp, lane, El, Hl, Er);     // for the next step
     step_current<R, C>(J, Ein, cf);
-    __syncthreads();
+    cta_barrier();
     recv_halo<R, NW>(hs, par, warp, lane, El, Hl, Er);
     if (SPECIAL) ++nloc;
   };
@@ -110,16 +112,16 @@ __global__ void __launch_bounds__(NT, MINB) k3_resident(RowPtrs<R> f, CoefPtrs<R
   const int row = tid / G::TPR;
   const bool valid = row < nrows;
   const int64_t k0 = (int64_t)tid * C;                       // physical in-grid index of the first node
-  const int64_t first = g * nrows * G::CR + k0;
+  const int64_t first_node = g * nrows * G::CR + k0;
   hs.clear(tid);
 
   R E[C], H[C], J[C];
 #pragma unroll
   for (int i = 0; i < C; ++i) { E[i] = R(0); H[i] = R(0); J[i] = R(0); }
   if (valid) {
-    load_nodes_global<R, C>(f.E, first, E);
-    load_nodes_global<R, C>(f.H, first, H);
-    load_nodes_global<R, C>(f.J, first, J);
+    load_nodes_global<R, C>(f.E, first_node, E);
+    load_nodes_global<R, C>(f.H, first_node, H);
+    load_nodes_global<R, C>(f.J, first_node, J);
   }
   const uint32_t flag = valid ? p.rowflag[row] : 0u;
   __syncthreads();
@@ -128,35 +130,52 @@ __global__ void __launch_bounds__(NT, MINB) k3_resident(RowPtrs<R> f, CoefPtrs<R
     const uint32_t base = smem_u32(smem_raw);
     CoefSmem<R, C, ROWS> cf;
     cf.init(base + ((1024u - (base & 1023u)) & 1023u), tid);
-    // each thread stages its own coefficient chunks (only it reads them back: no barrier needed)
+    // each thread stages its own coefficient chunks (only it reads them back: no barrier needed) and notes
+    // whether its C nodes all carry the same values
+    R first[kNumCoef];
+    bool uniform = true;
     auto stage = [&](auto ac) {
       constexpr int a = decltype(ac)::value;
 #pragma unroll
       for (int j = 0; j < G::NCH; ++j) {
         R z[G::V] = {};
         Vec v = vec_pack(z);
-        if (valid) v = reinterpret_cast<const Vec *>(cp.c[a] + first)[j];
+        if (valid) v = reinterpret_cast<const Vec *>(cp.c[a] + first_node)[j];
         cf.template store_chunk<a>(j, v);
+        vec_unpack(v, z);
+        if (j == 0) first[a] = z[0];
+#pragma unroll
+        for (int u = 0; u < G::V; ++u) uniform = uniform && (z[u] == first[a]);
       }
     };
     stage(std::integral_constant<int, 0>{}); stage(std::integral_constant<int, 1>{});
     stage(std::integral_constant<int, 2>{}); stage(std::integral_constant<int, 3>{});
-    time_loop<true, R, C, NW>(E, H, J, cf, hs, p, flag, k0, g, true, nsteps, warp, lane);
+    // piecewise-constant media: a warp whose rows are all uniform reads its coefficients from four registers and
+    // leaves shared memory alone (one 512-row grid would otherwise read 128 KB of coefficients per step: the
+    // shared-memory roofline, profiles/r01_ncu_k3_config3.md); warps on a media interface keep the general path
+    if (__all_sync(0xffffffffu, uniform)) {
+      CoefUniform<R, C> cu;
+#pragma unroll
+      for (int a = 0; a < kNumCoef; ++a) cu.v[a] = first[a];
+      time_loop<true, R, C, NW>(E, H, J, cu, hs, p, flag, k0, g, true, nsteps, warp, lane);
+    } else {
+      time_loop<true, R, C, NW>(E, H, J, cf, hs, p, flag, k0, g, true, nsteps, warp, lane);
+    }
   } else {
     CoefRegs<R, C> cf;
 #pragma unroll
     for (int a = 0; a < kNumCoef; ++a) {
 #pragma unroll
       for (int i = 0; i < C; ++i) cf.c[a][i] = R(0);
-      if (valid) load_nodes_global<R, C>(cp.c[a], first, cf.c[a]);
+      if (valid) load_nodes_global<R, C>(cp.c[a], first_node, cf.c[a]);
     }
     time_loop<true, R, C, NW>(E, H, J, cf, hs, p, flag, k0, g, true, nsteps, warp, lane);
   }
 
   if (valid) {
-    store_nodes_global<R, C>(f.E, first, E);
-    store_nodes_global<R, C>(f.H, first, H);
-    store_nodes_global<R, C>(f.J, first, J);
+    store_nodes_global<R, C>(f.E, first_node, E);
+    store_nodes_global<R, C>(f.H, first_node, H);
+    store_nodes_global<R, C>(f.J, first_node, J);
   }
 }
 
@@ -292,8 +311,8 @@ __global__ void __launch_bounds__(NT, MINB) k2_tblock(const __grid_constant__ K2
 // away (garbage moves inwards one node per step; the halo is >= T nodes wide).
 template <bool SPECIAL, typename R, int C>
 __device__ __forceinline__ void warp_step(const R (&E)[C], R (&En)[C], R (&H)[C], R (&G)[C], const CoefRegs<R, C> &cf,
-                                          R &Er, R nchh, const StepParams<R> &p, uint32_t flag, int64_t k0, int64_t g,
-                                          int64_t nloc, bool owner, R src_now) {
+                                          R &Er, R nchh, const StepParams<R> &p, const SpecialIdx &sx, int64_t nloc,
+                                          R src_now) {
   typedef Arith<R> A;
   // Issue cost of an FP64 instruction on sm_100 = max(2, distinct 64-bit register operands) cycles per
   // scheduler (measured): the two FMAs that multiply E[i] sit next to each other so that the
@@ -310,7 +329,7 @@ __device__ __forceinline__ void warp_step(const R (&E)[C], R (&En)[C], R (&H)[C]
     En[i] = A::fma(-cf.c[COEF_CH][i], A::sub(H[i], i ? H[i - 1] : Hl), t);    // a2
   }
   if constexpr (SPECIAL) {
-    if (flag) step_special<R, C>(E, En, H, p, flag, k0, g, nloc, owner, src_now);       // a3, a4, a6
+    if (sx.any) step_special<R, C>(E, En, H, p, sx, nloc, src_now);       // a3, a4, a6
   }
   Er = __shfl_down_sync(0xffffffffu, En[0], 1);
 }
@@ -326,17 +345,18 @@ __device__ __forceinline__ void warp_time_loop(R (&E)[C], R (&H)[C], R (&G)[C], 
   const int lane = threadIdx.x & 31;
   SourceStream<R> src;
   src.start(p, SPECIAL && __any_sync(0xffffffffu, (flag & F_SRC) != 0u), nloc, lane);
+  const SpecialIdx sx = SPECIAL ? make_special<R, C>(p, flag, k0, g, owner) : SpecialIdx();
   int left = nsteps;
   for (; left >= 2; left -= 2) {
     const R s0 = SPECIAL ? src.sample(p, nloc, lane) : R(0);
-    warp_step<SPECIAL, R, C>(E, Eb, H, G, cf, Er, nchh, p, flag, k0, g, nloc, owner, s0);
+    warp_step<SPECIAL, R, C>(E, Eb, H, G, cf, Er, nchh, p, sx, nloc, s0);
     const R s1 = SPECIAL ? src.sample(p, nloc + 1, lane) : R(0);
-    warp_step<SPECIAL, R, C>(Eb, E, H, G, cf, Er, nchh, p, flag, k0, g, nloc + 1, owner, s1);
+    warp_step<SPECIAL, R, C>(Eb, E, H, G, cf, Er, nchh, p, sx, nloc + 1, s1);
     nloc += 2;
   }
   if (left) {
     const R s0 = SPECIAL ? src.sample(p, nloc, lane) : R(0);
-    warp_step<SPECIAL, R, C>(E, Eb, H, G, cf, Er, nchh, p, flag, k0, g, nloc, owner, s0);
+    warp_step<SPECIAL, R, C>(E, Eb, H, G, cf, Er, nchh, p, sx, nloc, s0);
 #pragma unroll
     for (int i = 0; i < C; ++i) E[i] = Eb[i];
   }
@@ -519,8 +539,8 @@ static cudaError_t launch_k3_t(const Layout &L, FieldPtrs f, void *const coef[kN
   constexpr int CF = kRowBytes / sizeof(R), CH = CF / 2;
   if (variant == 0) switch (NT) {
     case 32: return launch_k3_v<R, CF, 32, false, 8>(L, f, coef, sc, nsteps, st);
-    case 64: return launch_k3_v<R, CF, 64, false, 4>(L, f, coef, sc, nsteps, st);
-    case 128: return launch_k3_v<R, CF, 128, false, 2>(L, f, coef, sc, nsteps, st);
+    case 64: return launch_k3_v<R, CF, 64, false, 6>(L, f, coef, sc, nsteps, st);
+    case 128: return launch_k3_v<R, CF, 128, false, 3>(L, f, coef, sc, nsteps, st);
     case 256: return launch_k3_v<R, CF, 256, false, 1>(L, f, coef, sc, nsteps, st);
     case 512: return launch_k3_v<R, CF, 512, true, 1>(L, f, coef, sc, nsteps, st);
   }
