@@ -249,6 +249,55 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+PAPER_TABLE2_MS = {1024: (33, 114, 279), 5120: (33, 122, 379), 10240: (33, 138, 504), 20480: (34, 148, 753),
+                   30720: (46, 175, 982), 40960: (53, 231, 1231), 51200: (61, 299, 1467), 61440: (64, 309, 1701)}
+# ^ PAPER.md:155-162, Table 2: (GPU GTX 1080, OpenMP i7-6700, serial) ms per 1000 steps — context, other hardware
+
+
+def run_table2(args):
+    """--table2: the paper's Table 2 sweep on this GPU and this host.
+    One rketd_run of 1000 steps per line length, CUDA events, median of 7 after 3 warm-ups; the oracle (serial
+    and OpenMP builds) timed on the same inputs.  Prints one JSON line; not the headline metric."""
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: librketd has no CPU fallback")
+    from paper_1709_00821_b200 import rketd, workloads as wl
+    import oracle
+    oracle.build()
+    stream = torch.cuda.current_stream()
+    rows = []
+    for n in wl.PAPER_TABLE2_CELLS:
+        w = wl.paper_table2(n)
+        sim = rketd.Sim.from_workload(w, args.dtype, stream=stream.cuda_stream)
+        times = []
+        for it in range(10):
+            sim.reset()
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            sim.run(w.nsteps)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            if it >= 3:
+                times.append(e0.elapsed_time(e1))
+        kernel = sim.counter(rketd.CTR_KERNEL_USED)
+        sim.close()
+        cpu = {}
+        for omp in (False, True):
+            t0 = time.perf_counter()
+            oracle.run_workload(w, omp=omp)
+            cpu[omp] = (time.perf_counter() - t0) * 1e3
+        ms = sorted(times)[len(times) // 2]
+        pg, po, ps = PAPER_TABLE2_MS[n]
+        rows.append({"cells": n, "steps": w.nsteps, "kernel": int(kernel), "gpu_ms": round(ms, 4), "gpu_ms_min": round(min(times), 4),
+                     "gcells": round(n * w.nsteps / ms / 1e6, 3), "oracle_serial_ms": round(cpu[False], 2),
+                     "oracle_omp_ms": round(cpu[True], 2), "paper_gtx1080_ms": pg, "paper_openmp_ms": po,
+                     "paper_serial_ms": ps})
+    print(json.dumps({"table2": rows, "dtype": args.dtype, "cores": os.cpu_count(),
+                      "note": "paper columns are another machine's (GTX 1080 / i7-6700, PAPER.md:109-162): context only; "
+                              "Mur-1 ends here, 5-cell PML there"}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -262,7 +311,10 @@ def main():
     ap.add_argument("--variant", type=int, default=-1)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--table2", action="store_true", help="time the paper's Table 2 sweep instead of the headline workload")
     args = ap.parse_args()
+    if args.table2:
+        return run_table2(args)
     if args.impl == "reference":
         return run_reference(args)
 

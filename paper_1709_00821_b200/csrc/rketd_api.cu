@@ -175,9 +175,24 @@ int make_map(rketd_sim *s, CUtensorMap *m, void *base, int box_rows) {
   return RKETD_OK;
 }
 
-int default_depth(const rketd_sim *s) { return s->dtype == RKETD_F64 ? 16 : 32; }
+// Temporal depth T of K2.  Large problems: 16 (fp64) / 32 (fp32) steps per pass, the deepest setting that still
+// sits on the HBM roofline.  Problems whose tiles do not even fill one wave of warps (148 SMs x 12
+// warp tiles) are launch-latency bound (the paper's Table 2 sizes): there the deepest pass that still fits one
+// wave wins, because it divides the number of launches.
+int default_depth(const rketd_sim *s) {
+  const int base = s->dtype == RKETD_F64 ? 16 : 32;
+  const int64_t one_wave = 148 * 12;
+  for (int T = 4 * base; T > base; T -= base) {
+    const int HR = (T + s->L.C - 1) / s->L.C, rows_out = 32 - 2 * HR;
+    if (rows_out < 8) continue;
+    if (((s->L.nrows + rows_out - 1) / rows_out) * s->L.nbatch <= one_wave) return T;
+  }
+  return base;
+}
 int default_k2_variant(const rketd_sim *) { return 6; }
-int default_k3_variant(const rketd_sim *) { return 0; }
+// fp64 grids of up to 256 rows: half-row threads (twice the warps hide the per-step barrier better: config 5 fp64
+// 630 -> 700 Gcell/s); fp32 is faster with whole rows (1104 vs 931)
+int default_k3_variant(const rketd_sim *s) { return (s->dtype == RKETD_F64 && s->L.nrows <= 256) ? 1 : 0; }
 int max_depth(const rketd_sim *s, int variant) { return (k2_tile_rows(variant) / 2 - 1) * s->L.C; }
 
 int build_k2_plan(rketd_sim *s, int depth, int variant) {
@@ -200,6 +215,11 @@ int build_k2_plan(rketd_sim *s, int depth, int variant) {
   P.ctas_per_sm = ctas;
   const int tpc = k2_tiles_per_cta(variant);
   P.grid = (int)std::min<int64_t>((P.total_tiles + tpc - 1) / tpc, (int64_t)sms * ctas);
+  P.spread = 0;
+  if (tpc > 1 && P.total_tiles < (int64_t)sms * ctas * tpc) {   // less than one wave of warp tiles
+    P.spread = 1;
+    P.grid = (int)std::min<int64_t>(P.total_tiles, (int64_t)sms * ctas);
+  }
   for (int b = 0; b < 2; ++b) {
     for (int a = 0; a < 3; ++a) {
       int rc = make_map(s, &P.maps[b].ld[a], s->fld[b][a], rows);

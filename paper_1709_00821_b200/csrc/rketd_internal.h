@@ -51,6 +51,7 @@ struct K2Plan {
   int64_t tiles_per_grid = 0, total_tiles = 0;
   int grid = 0;            // CTAs launched (persistent)
   int ctas_per_sm = 0;
+  int spread = 0;          // warp tiles dealt out across the SMs first (fewer tiles than one wave of warps)
   size_t smem_bytes = 0;
   K2Maps maps[2];          // maps[s]: read buffer s, write buffer 1-s
 };

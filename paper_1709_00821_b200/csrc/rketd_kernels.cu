@@ -186,6 +186,7 @@ struct K2Args {
   int rows_out;           // ROWS - 2 HR
   uint32_t tiles_per_grid, total_tiles;   // 32-bit on purpose: tile index arithmetic sits between two tiles
   int64_t nrows;
+  int spread;             // warp tiles: 1 = fewer tiles than one wave of warps: deal them out across the SMs first
 };
 constexpr int kNumIn = 3 + kNumCoef;      // arrays a tile loads: E, H, G, P, ch, ka, Q
 
@@ -406,7 +407,8 @@ __global__ void __launch_bounds__(NW * 32, MINB) k2_wtile(const __grid_constant_
   const uint32_t stride = gridDim.x * NW;
   // the warps of a CTA work on consecutive tiles, so that the tiles in flight at any time are neighbours
   // in memory and the halo rows two tiles share are served by L2
-  uint32_t tile = blockIdx.x * NW + warp;
+  // (a problem smaller than one wave is latency bound: there one warp per SM beats twelve warps sharing an SM)
+  uint32_t tile = q.spread ? warp * gridDim.x + blockIdx.x : blockIdx.x * NW + warp;
   uint32_t g = 0, ti = 0, flag = 0;
   int row0 = 0;
   if (tile < q.total_tiles) {
@@ -618,6 +620,7 @@ static cudaError_t launch_k2_t(const Layout &L, const K2Plan &plan, int src_buf,
   K2Args q;
   q.T = steps; q.HR = plan.HR; q.rows_out = plan.rows_out;
   q.tiles_per_grid = (uint32_t)plan.tiles_per_grid; q.total_tiles = (uint32_t)plan.total_tiles; q.nrows = L.nrows;
+  q.spread = plan.spread;
   const StepParams<R> sp = make_params<R>(sc);
   const K2Maps &m = plan.maps[src_buf];
   switch (plan.variant) {

@@ -237,4 +237,52 @@ def config5(ncells: int = 1024, nbatch: int = 65_536, nsteps: int = 5000, dft: b
                     notes="random multilayer; probes reduced on device to |DFT| at 64 frequencies")
 
 
+# ----------------------------------------------------------------------------
+# The paper's own two workloads
+# ----------------------------------------------------------------------------
+PAPER_DT = 125e-15           # "a single time step is taken to be 125 fs"; S = c dt/dz = 0.49965
+PAPER_TABLE2_CELLS = (1024, 5120, 10240, 20480, 30720, 40960, 51200, 61440)
+
+
+def _paper_slab(name: str, cfg: int, ncells: int, nsteps: int, src_cell: int, probes) -> Workload:
+    """A slab on the middle 1200/4096 of the line, wp = 2 pi 28.7e9 rad/s, nu = 20e9 1/s, vacuum elsewhere,
+    Gaussian-derivative pulse with tau = 15 dt, delay 5 tau.  The paper ends the line in 5-cell
+    PMLs whose parameters it does not give; here the ends are Mur-1 like everywhere else (DESIGN.md §2 G10)."""
+    m = (ncells * 1200) // 4096
+    slab_lo = (ncells - m) // 2
+    wp0, nu0 = 2.0 * math.pi * 28.7e9, 2.0e10
+    tau = 15.0 * PAPER_DT
+
+    def media(lo=0, hi=ncells, b0=0, b1=1):
+        k = np.arange(lo, hi)
+        inside = (k >= slab_lo) & (k < slab_lo + m)
+        wp = np.where(inside, wp0, 0.0)[None, :].repeat(b1 - b0, 0)
+        nu = np.where(inside, nu0, 0.0)[None, :].repeat(b1 - b0, 0)
+        return np.ascontiguousarray(wp), np.ascontiguousarray(nu)
+
+    def initial_E(lo=0, hi=ncells, b0=0, b1=1):
+        return None
+
+    w = Workload(name, cfg, ncells, 1, nsteps, DZ, PAPER_DT, SRC_GAUSS_DERIV, (tau, 5.0 * tau, 1.0), src_cell,
+                 np.array(sorted(probes), np.int64), None, media, initial_E,
+                 notes="paper's own workload (PAPER.md:123-128); Mur instead of the unspecified PML")
+    w.slab = (slab_lo, m)
+    return w
+
+
+def paper_exp_a(nsteps: int = 16384) -> Workload:
+    """Experiment A (Figs. 2-3): 4096 cells, slab = middle 1200 cells (9 cm), R and T by FFT.
+    The paper gives neither source nor probe positions nor the run length: source 300, reflected probe 800,
+    transmitted probe 3300, 16 384 steps (both records have decayed to < 1e-6 of their peak by then)."""
+    return _paper_slab("paper_expA_4096", 11, 4096, nsteps, 300, (800, 3300))
+
+
+def paper_table2(ncells: int, nsteps: int = 1000) -> Workload:
+    """One row of Table 2: `ncells` Yee cells x 1000 steps; the same slab geometry scaled to the
+    line (the paper does not say what fills the longer lines, nor where it records)."""
+    src = max(2, (ncells * 300) // 4096)
+    # the pulse travels 500 cells in 1000 steps (S = 1/2): probes 128 and 400 cells behind the source see it
+    return _paper_slab(f"paper_table2_{ncells}", 12, ncells, nsteps, src, (src + 128, src + 400))
+
+
 CONFIGS = {1: config1, 2: config2, 3: config3, 4: config4, 5: config5}

@@ -352,3 +352,31 @@ def test_mur_reflection_is_small_at_half_courant():
     z = np.zeros((1, N))
     oracle.run(st, z, z, DZ, DT, 2000)
     assert np.max(np.abs(st.E)) < 1e-3
+
+
+# ----------------------------------------------------------------------------- paper experiment A (NEXT-1)
+def test_paper_experiment_A_reflection_transmission():
+    """The paper's own experiment (Figs. 2-3): 4096 cells, 9 cm slab (1200 cells), dt = 125 fs,
+    tau = 15 dt.  |R|, |T| by FFT against the closed form.  T holds to 1e-3 over the whole pulse band
+    (1-300 GHz); R to 1e-2 up to 150 GHz and 2e-2 above, where the line has < 27 cells per wavelength and the
+    first-order Mur end reflects about 1 % (the paper used PML there)."""
+    w = wl.paper_exp_a()
+    assert w.ncells == 4096 and w.slab == (1448, 1200) and abs(w.src_params[0] - 15 * 125e-15) < 1e-25
+    tot = oracle.run_workload(w)["rec"][0]
+    wv = wl.paper_exp_a()
+    wv.media = lambda lo=0, hi=w.ncells, b0=0, b1=1: (np.zeros((b1 - b0, hi - lo)), np.zeros((b1 - b0, hi - lo)))
+    inc = oracle.run_workload(wv)["rec"][0]
+    assert np.max(np.abs(tot[:, -200:])) < 1e-5 * np.max(np.abs(tot))          # records have decayed
+    freqs = np.fft.rfftfreq(w.nsteps, w.dt)
+    Ir, It = np.fft.rfft(inc[0]), np.fft.rfft(inc[1])
+    R = np.abs(np.fft.rfft(tot[0] - inc[0])) / np.abs(Ir)
+    T = np.abs(np.fft.rfft(tot[1])) / np.abs(It)
+    band = np.abs(Ir) >= 1e-2 * np.max(np.abs(Ir))
+    assert freqs[band].min() < 2e9 and freqs[band].max() > 250e9
+    Ra, Ta = _slab_rt_analytic(freqs[band], 2 * math.pi * 28.7e9, 2.0e10, 1200 * w.dz)
+    low = freqs[band] <= 150e9
+    assert np.max(np.abs(T[band] - Ta)) < 1e-3
+    assert np.max(np.abs(R[band][low] - Ra[low])) < 1e-2
+    assert np.max(np.abs(R[band] - Ra)) < 2e-2
+    # opaque below the plasma frequency, transparent far above it
+    assert T[band][freqs[band] < 25e9].max() < 1e-5 and T[band][freqs[band] > 200e9].min() > 0.9
