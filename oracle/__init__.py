@@ -30,6 +30,8 @@ BOUNDARY_PEC = 1
 SRC_NONE = -1
 SRC_GAUSS_DERIV = 0
 SRC_TABLE = 1
+SCHEME_ETD2 = 0      # eq. (11) PAPER.md:68 — the paper's method
+SCHEME_ETD1 = 1      # eq. (9) PAPER.md:59 — first-order ETD
 
 
 def build(force: bool = False) -> None:
@@ -58,6 +60,8 @@ def _lib(omp: bool = False) -> ctypes.CDLL:
         lib.oracle_phi.restype = None
         lib.oracle_coefficients.argtypes = [ctypes.c_int64, _D, _D, ctypes.c_double, ctypes.c_double] + [_D] * 8
         lib.oracle_coefficients.restype = ctypes.c_int
+        lib.oracle_coefficients_scheme.argtypes = lib.oracle_coefficients.argtypes + [ctypes.c_int]
+        lib.oracle_coefficients_scheme.restype = ctypes.c_int
         lib.oracle_source.argtypes = [ctypes.c_int, _D, ctypes.c_int64, ctypes.c_int64, ctypes.c_double]
         lib.oracle_source.restype = ctypes.c_double
         lib.oracle_run.argtypes = [ctypes.c_int64, ctypes.c_int64, ctypes.c_double, ctypes.c_double,
@@ -66,6 +70,8 @@ def _lib(omp: bool = False) -> ctypes.CDLL:
                                    _I64, ctypes.c_int, ctypes.c_int64, ctypes.c_int64,
                                    _D, _D, _D, ctypes.c_int, _D, _D, ctypes.c_int]
         lib.oracle_run.restype = ctypes.c_int
+        lib.oracle_run_scheme.argtypes = lib.oracle_run.argtypes + [ctypes.c_int]
+        lib.oracle_run_scheme.restype = ctypes.c_int
         _loaded[omp] = lib
     return _loaded[omp]
 
@@ -87,14 +93,15 @@ def phi(x: float):
     return p1.value, p2.value
 
 
-def coefficients(wp: np.ndarray, nu: np.ndarray, dz: float, dt: float):
+def coefficients(wp: np.ndarray, nu: np.ndarray, dz: float, dt: float, scheme: int = SCHEME_ETD2):
     """S0: returns dict(ca, cj, ch, ka, kb, kc [same shape as wp], chh, m)."""
     wp = np.ascontiguousarray(wp, np.float64)
     nu = np.ascontiguousarray(nu, np.float64)
     out = {k: np.empty_like(wp) for k in ("ca", "cj", "ch", "ka", "kb", "kc")}
     chh, m = ctypes.c_double(), ctypes.c_double()
-    rc = _lib().oracle_coefficients(wp.size, _p(wp), _p(nu), dz, dt, *[_p(out[k]) for k in
-                                    ("ca", "cj", "ch", "ka", "kb", "kc")], ctypes.byref(chh), ctypes.byref(m))
+    rc = _lib().oracle_coefficients_scheme(wp.size, _p(wp), _p(nu), dz, dt, *[_p(out[k]) for k in
+                                           ("ca", "cj", "ch", "ka", "kb", "kc")], ctypes.byref(chh), ctypes.byref(m),
+                                           scheme)
     if rc:
         raise ValueError("oracle_coefficients: invalid argument")
     out["chh"], out["m"] = chh.value, m.value
@@ -119,7 +126,8 @@ class State:
 
 def run(state: State, wp, nu, dz: float, dt: float, nsteps: int, *, src_kind: int = SRC_NONE,
         src_params: Sequence[float] = (), src_cell: int = 0, probes: Sequence[int] = (),
-        freqs=None, dft=None, record_J: bool = False, boundary: int = BOUNDARY_MUR, omp: bool = False):
+        freqs=None, dft=None, record_J: bool = False, boundary: int = BOUNDARY_MUR, omp: bool = False,
+        scheme: int = SCHEME_ETD2):
     """Advance ``state`` by nsteps.  Returns (rec, recJ) with rec[nbatch][nprobes][nsteps]
     (recJ None unless record_J).  ``dft`` = (re, im) accumulator arrays [nbatch][nprobes][nfreq],
     updated in place when ``freqs`` is given."""
@@ -135,10 +143,10 @@ def run(state: State, wp, nu, dz: float, dt: float, nsteps: int, *, src_kind: in
     if fr is not None:
         re, im = dft
         assert re.shape == (nbatch, prb.size, fr.size) and re.flags.c_contiguous and im.flags.c_contiguous
-    rc = _lib(omp).oracle_run(ncells, nbatch, dz, dt, _p(wp), _p(nu), _p(state.E), _p(state.H), _p(state.J),
+    rc = _lib(omp).oracle_run_scheme(ncells, nbatch, dz, dt, _p(wp), _p(nu), _p(state.E), _p(state.H), _p(state.J),
                               src_kind, _p(prm) if prm.size else None, prm.size, src_cell,
                               prb.ctypes.data_as(_I64) if prb.size else None, prb.size, state.step, nsteps,
-                              _p(rec), _p(recJ), _p(fr), 0 if fr is None else fr.size, _p(re), _p(im), boundary)
+                              _p(rec), _p(recJ), _p(fr), 0 if fr is None else fr.size, _p(re), _p(im), boundary, scheme)
     if rc:
         raise ValueError("oracle_run: invalid argument")
     state.step += nsteps
@@ -146,7 +154,7 @@ def run(state: State, wp, nu, dz: float, dt: float, nsteps: int, *, src_kind: in
 
 
 def run_workload(w, nsteps: Optional[int] = None, b0: int = 0, b1: Optional[int] = None, omp: bool = False,
-                 cells: Optional[tuple] = None):
+                 cells: Optional[tuple] = None, scheme: int = SCHEME_ETD2):
     """Run a ``workloads.Workload`` (duck-typed: only its data attributes are used) on grids
     b0..b1-1.  ``cells=(lo, hi)`` runs the window lo..hi-1 only, with Mur at the window ends
     (pin P7: exact for probes at distance > nsteps from both window ends).
@@ -164,6 +172,6 @@ def run_workload(w, nsteps: Optional[int] = None, b0: int = 0, b1: Optional[int]
         dft = (np.zeros((b1 - b0, len(probes), len(w.dft_freqs))), np.zeros((b1 - b0, len(probes), len(w.dft_freqs))))
     rec, _ = run(st, wp, nu, w.dz, w.dt, nsteps, src_kind=w.src_kind if in_src else SRC_NONE,
                  src_params=w.src_params, src_cell=w.src_cell - lo if in_src else 0, probes=probes,
-                 freqs=w.dft_freqs, dft=dft, omp=omp)
+                 freqs=w.dft_freqs, dft=dft, omp=omp, scheme=scheme)
     mag = None if dft is None else np.hypot(dft[0], dft[1])
     return {"rec": rec, "dft_mag": mag, "state": st, "probe_cells": [p + lo for p in probes]}

@@ -68,10 +68,28 @@ struct Coef {
 // S0 — the six per-cell coefficients of SURVEY §8(a) row a0.  Derivation:
 // write (11) as J' = a J + (b-c) E + c E', put it into (12), collect E'
 // (this is eq. (13) with the 1/D the print drops restored — SURVEY G1).
+//
+// scheme 1 — the first-order ETD variant the paper derives but does not use (eqs. (8)-(9), PAPER.md:55-60;
+// SURVEY §8(f) NEXT-4): F held at F_n over the step, J' = a J + b E.  Put into (12): D = 1,
+// ca = 1 - wp^2 beta dt/2, cj = (dt/2 eps0)(1 + a), ch = dt/(eps0 dz), ka = a, kb = b, kc = 0.
 void coefficients(int64_t n, const double* wp, const double* nu, double dz, double dt,
                   double* ca, double* cj, double* ch, double* ka, double* kb, double* kc,
-                  double* chh, double* m) {
-  for (int64_t k = 0; k < n; ++k) {
+                  double* chh, double* m, int scheme = 0) {
+  for (int64_t k = 0; k < n && scheme == 1; ++k) {
+    const double x = nu[k] * dt;
+    const double a = std::exp(-x);
+    double p1, p2;
+    phi(x, &p1, &p2);
+    const double beta = dt * p1;                 // (1 - a)/nu
+    const double wp2 = wp[k] * wp[k];
+    ca[k] = 1.0 - wp2 * beta * dt / 2.0;
+    cj[k] = (dt / (2.0 * kEps0)) * (1.0 + a);
+    ch[k] = dt / (kEps0 * dz);
+    ka[k] = a;
+    kb[k] = kEps0 * wp2 * beta;                  // eq. (9): F_n (1 - a)/nu
+    kc[k] = 0.0;
+  }
+  for (int64_t k = 0; k < n && scheme == 0; ++k) {
     const double x = nu[k] * dt;
     const double a = std::exp(-x);
     double p1, p2;
@@ -119,12 +137,19 @@ void oracle_constants(double* c0, double* mu0, double* eps0) {
 
 void oracle_phi(double x, double* phi1, double* phi2) { phi(x, phi1, phi2); }
 
+// scheme: 0 = second-order ETD, eq. (11) (the paper's method); 1 = first-order ETD, eq. (9)
+int oracle_coefficients_scheme(int64_t n, const double* wp, const double* nu, double dz, double dt,
+                               double* ca, double* cj, double* ch, double* ka, double* kb, double* kc,
+                               double* chh, double* m, int scheme) {
+  if (n < 0 || dz <= 0 || dt <= 0 || scheme < 0 || scheme > 1) return 1;
+  coefficients(n, wp, nu, dz, dt, ca, cj, ch, ka, kb, kc, chh, m, scheme);
+  return 0;
+}
+
 int oracle_coefficients(int64_t n, const double* wp, const double* nu, double dz, double dt,
                         double* ca, double* cj, double* ch, double* ka, double* kb, double* kc,
                         double* chh, double* m) {
-  if (n < 0 || dz <= 0 || dt <= 0) return 1;
-  coefficients(n, wp, nu, dz, dt, ca, cj, ch, ka, kb, kc, chh, m);
-  return 0;
+  return oracle_coefficients_scheme(n, wp, nu, dz, dt, ca, cj, ch, ka, kb, kc, chh, m, 0);
 }
 
 double oracle_source(int kind, const double* params, int64_t nparams, int64_t step_index, double dt) {
@@ -140,15 +165,16 @@ double oracle_source(int kind, const double* params, int64_t nparams, int64_t st
 //                   (step0+n+1) dt; either may be NULL
 //   freqs           [nfreq] Hz; dft_re/dft_im [nbatch][nprobes][nfreq] accumulators (in/out), NULL = off
 //   boundary        0 = Mur first order (a3), 1 = PEC (E[0] = E[N-1] = 0; oracle-only, for pin P3)
-int oracle_run(int64_t ncells, int64_t nbatch, double dz, double dt,
-               const double* wp, const double* nu, double* E, double* H, double* J,
-               int src_kind, const double* src_params, int64_t nparams, int64_t src_cell,
-               const int64_t* probes, int nprobes, int64_t step0, int64_t nsteps,
-               double* rec, double* recJ,
-               const double* freqs, int nfreq, double* dft_re, double* dft_im,
-               int boundary) {
+//   scheme          0 = eq. (11) (second-order ETD), 1 = eq. (9) (first-order ETD): only S0 differs
+int oracle_run_scheme(int64_t ncells, int64_t nbatch, double dz, double dt,
+                      const double* wp, const double* nu, double* E, double* H, double* J,
+                      int src_kind, const double* src_params, int64_t nparams, int64_t src_cell,
+                      const int64_t* probes, int nprobes, int64_t step0, int64_t nsteps,
+                      double* rec, double* recJ,
+                      const double* freqs, int nfreq, double* dft_re, double* dft_im,
+                      int boundary, int scheme) {
   const int64_t N = ncells;
-  if (N < 3 || nbatch < 1 || nsteps < 0 || dz <= 0 || dt <= 0) return 1;
+  if (N < 3 || nbatch < 1 || nsteps < 0 || dz <= 0 || dt <= 0 || scheme < 0 || scheme > 1) return 1;
   if (src_kind >= 0 && (src_cell < 0 || src_cell >= N)) return 1;
   for (int p = 0; p < nprobes; ++p)
     if (probes[p] < 0 || probes[p] >= N) return 1;
@@ -169,7 +195,7 @@ int oracle_run(int64_t ncells, int64_t nbatch, double dz, double dt,
     Coef cf;
     cf.ca.resize(N); cf.cj.resize(N); cf.ch.resize(N); cf.ka.resize(N); cf.kb.resize(N); cf.kc.resize(N);
     coefficients(N, wpg, nug, dz, dt, cf.ca.data(), cf.cj.data(), cf.ch.data(), cf.ka.data(),
-                 cf.kb.data(), cf.kc.data(), &cf.chh, &cf.m);
+                 cf.kb.data(), cf.kc.data(), &cf.chh, &cf.m, scheme);
     const double* ca = cf.ca.data(); const double* cj = cf.cj.data(); const double* ch = cf.ch.data();
     const double* ka = cf.ka.data(); const double* kb = cf.kb.data(); const double* kc = cf.kc.data();
     const double chh = cf.chh, m = cf.m;
@@ -222,6 +248,17 @@ int oracle_run(int64_t ncells, int64_t nbatch, double dz, double dt,
     }
   }
   return 0;
+}
+
+int oracle_run(int64_t ncells, int64_t nbatch, double dz, double dt,
+               const double* wp, const double* nu, double* E, double* H, double* J,
+               int src_kind, const double* src_params, int64_t nparams, int64_t src_cell,
+               const int64_t* probes, int nprobes, int64_t step0, int64_t nsteps,
+               double* rec, double* recJ,
+               const double* freqs, int nfreq, double* dft_re, double* dft_im,
+               int boundary) {
+  return oracle_run_scheme(ncells, nbatch, dz, dt, wp, nu, E, H, J, src_kind, src_params, nparams, src_cell, probes,
+                           nprobes, step0, nsteps, rec, recJ, freqs, nfreq, dft_re, dft_im, boundary, 0);
 }
 
 }  // extern "C"

@@ -380,3 +380,70 @@ def test_paper_experiment_A_reflection_transmission():
     assert np.max(np.abs(R[band] - Ra)) < 2e-2
     # opaque below the plasma frequency, transparent far above it
     assert T[band][freqs[band] < 25e9].max() < 1e-5 and T[band][freqs[band] > 200e9].min() > 0.9
+
+
+# ----------------------------------------------------------------------------- first-order ETD, eq. (9) (NEXT-4)
+@pytest.mark.parametrize("nu", [2.4e12, 8e12, 2e10])
+def test_ETD1_residual_of_literal_eq9_and_eq12(nu):
+    """scheme 1: after each step the state satisfies eq. (9) and eq. (12) as PRINTED."""
+    N = 64
+    rng = np.random.default_rng(4)
+    wp = np.full((1, N), 2 * math.pi * 40e9)
+    nuv = np.full((1, N), nu)
+    st = oracle.State(N, 1, E0=rng.uniform(-1, 1, N), H0=rng.uniform(-1, 1, N) / ETA0, J0=rng.uniform(-1, 1, N) * 1e3)
+    a = math.exp(-nu * DT)
+    for _ in range(20):
+        E0, J0 = st.E[0].copy(), st.J[0].copy()
+        oracle.run(st, wp, nuv, DZ, DT, 1, scheme=oracle.SCHEME_ETD1)
+        E1, J1, H = st.E[0], st.J[0], st.H[0]
+        Fn = EPS0 * wp[0] ** 2 * E0
+        j9 = J0 * a - Fn * (a - 1) / nu                                   # eq. (9) as printed
+        assert np.max(np.abs(J1 - j9)) <= 1e-11 * np.max(np.abs(J1))       # (a - 1)/nu cancels 3 digits at nu = 2e10
+        k = np.arange(1, N - 1)
+        e12 = E0[k] - DT / (EPS0 * DZ) * (H[k] - H[k - 1]) - DT / (2 * EPS0) * (J1[k] + J0[k])
+        assert np.max(np.abs(E1[k] - e12)) <= 1e-12 * np.max(np.abs(E1))
+
+
+@pytest.mark.parametrize("nu", [0.0, 2e10, 1e11])
+def test_ETD1_J_is_exact_solution_of_eq6_for_piecewise_constant_E(nu):
+    """Brute force for eq. (9): RK4 (64 sub-steps per dt) of dJ/dt + nu J = eps0 wp^2 E^n, E HELD at its value at
+    the start of each step (eq. (8): F = F_n) reproduces the scheme-1 J series; and the two schemes differ at first
+    order in dt (they are not the same recurrence)."""
+    N, nsteps, cell = 200, 400, 100
+    wpv = 2 * math.pi * 28.7e9
+    wp = np.zeros((1, N)); nuv = np.zeros((1, N))
+    wp[0, 80:130] = wpv; nuv[0, 80:130] = nu
+    kw = dict(src_kind=0, src_params=(20e-12, 80e-12, 1.0), src_cell=40, probes=[cell], record_J=True)
+    rec, recJ = oracle.run(oracle.State(N, 1), wp, nuv, DZ, DT, nsteps, scheme=oracle.SCHEME_ETD1, **kw)
+    Es = np.concatenate([[0.0], rec[0, 0]])
+    Js = np.concatenate([[0.0], recJ[0, 0]])
+    nsub, J, Jref = 64, 0.0, [0.0]
+    h = DT / nsub
+    for n in range(nsteps):
+        f = lambda j: -nu * j + EPS0 * wpv ** 2 * Es[n]
+        for s in range(nsub):
+            k1 = f(J); k2 = f(J + h / 2 * k1); k3 = f(J + h / 2 * k2); k4 = f(J + h * k3)
+            J += h / 6 * (k1 + 2 * k2 + 2 * k3 + k4)
+        Jref.append(J)
+    Jref = np.array(Jref)
+    assert np.max(np.abs(Jref)) > 0 and np.max(np.abs(Js - Jref)) < 5e-13 * np.max(np.abs(Jref))
+    rec2, _ = oracle.run(oracle.State(N, 1), wp, nuv, DZ, DT, nsteps, **kw)
+    d = np.max(np.abs(rec2 - rec)) / np.max(np.abs(rec2))
+    assert 1e-5 < d < 5e-2, d
+
+
+def test_ETD1_coefficients_closed_form_and_vacuum():
+    wp = np.array([0.0, 2 * math.pi * 28.7e9, 2 * math.pi * 60e9])
+    nu = np.array([0.0, 2e10, 0.0])
+    c = oracle.coefficients(wp, nu, DZ, DT, oracle.SCHEME_ETD1)
+    mpmath.mp.dps = 50
+    for i in range(3):
+        x = mpmath.mpf(nu[i]) * mpmath.mpf(DT)
+        a = mpmath.exp(-x)
+        beta = mpmath.mpf(DT) if nu[i] == 0 else (1 - a) / mpmath.mpf(nu[i])
+        w2 = mpmath.mpf(wp[i]) ** 2
+        ref = {"ca": 1 - w2 * beta * mpmath.mpf(DT) / 2, "cj": mpmath.mpf(DT) / (2 * mpmath.mpf(EPS0)) * (1 + a),
+               "ch": mpmath.mpf(DT) / (mpmath.mpf(EPS0) * mpmath.mpf(DZ)), "ka": a, "kb": mpmath.mpf(EPS0) * w2 * beta,
+               "kc": mpmath.mpf(0)}
+        for k, v in ref.items():
+            assert abs(c[k][i] - float(v)) <= 4e-16 * abs(float(v)), (k, i)
