@@ -34,6 +34,11 @@ typedef struct rketd_sim rketd_sim; /* opaque */
 enum { RKETD_F64 = 0, RKETD_F32 = 1 };
 enum { RKETD_OK = 0, RKETD_EINVAL = 1, RKETD_ENOMEM = 2, RKETD_ECUDA = 3, RKETD_ESTATE = 4 };
 enum { RKETD_SRC_NONE = -1, RKETD_SRC_GAUSS_DERIV = 0, RKETD_SRC_TABLE = 1 };
+/* current-density recurrence for rketd_set_scheme */
+enum {
+  RKETD_SCHEME_ETD2 = 0,     /* eq. (11): second-order ETD ("RKETD"), the paper's method; the default   */
+  RKETD_SCHEME_ETD1 = 1      /* eq. (9)  PAPER.md:59: first-order ETD, F held at F_n over the step   */
+};
 /* kernel selection for rketd_set_plan */
 enum {
   RKETD_KERNEL_AUTO = 0,     /* resident (K3) when a grid fits one CTA, else temporal blocking (K2) */
@@ -71,6 +76,11 @@ int rketd_create(rketd_sim **out, int64_t ncells, int64_t nbatch, double dz, dou
  * and from them the four arrays the kernels read (rketd_get_kernel_coefficients).
  * The current fields E, H, J are kept.  EINVAL: any wp or nu negative or non-finite.  Synchronises. */
 int rketd_set_media(rketd_sim *s, const double *wp, const double *nu);
+
+/* Choose the recurrence that advances J (RKETD_SCHEME_*).  Only the coefficient precompute differs: with eq. (9),
+ * J' = ka J + kb E (kc = 0) and eq. (12) solved for E' has D = 1.  Takes effect at the next rketd_set_media, which
+ * derives the coefficients; call it before.  EINVAL: unknown scheme. */
+int rketd_set_scheme(rketd_sim *s, int scheme);
 
 /* Soft source added to E^{n+1}[cell] in every grid (eq. (15)).
  * kind RKETD_SRC_GAUSS_DERIV: params = {tau, t0, amplitude},

@@ -19,6 +19,7 @@ std::string g_create_error;
 struct Chunk {
   void *buf;
   int64_t nsteps;
+  size_t bytes;
 };
 }  // namespace
 
@@ -26,6 +27,7 @@ struct rketd_sim {
   Layout L;
   double dz = 0, dt = 0;
   int dtype = 0;
+  int scheme = RKETD_SCHEME_ETD2, media_scheme = RKETD_SCHEME_ETD2;   // requested / the one the live coefficients use
   cudaStream_t stream = nullptr;
   void *fld[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};
   int cur = 0;
@@ -46,6 +48,8 @@ struct rketd_sim {
   std::vector<double> freqs;
   double *d_freqs = nullptr, *dft_re = nullptr, *dft_im = nullptr;
   std::vector<Chunk> chunks;
+  void *spare_buf = nullptr;     // one discarded record buffer kept for the next rketd_run (no cudaMalloc per run)
+  size_t spare_bytes = 0;
   int64_t nsamples = 0;
   int64_t step = 0;
   int plan_kernel = RKETD_KERNEL_AUTO, plan_depth = 0, plan_variant = -1;
@@ -93,7 +97,14 @@ cudaError_t copy_out(const rketd_sim *s, void *dst_user, const void *src_phys) {
 }
 
 void discard_records(rketd_sim *s) {
-  for (auto &c : s->chunks) cudaFree(c.buf);
+  for (auto &c : s->chunks) {
+    if (c.bytes > s->spare_bytes) {
+      if (s->spare_buf) cudaFree(s->spare_buf);
+      s->spare_buf = c.buf; s->spare_bytes = c.bytes;
+    } else {
+      cudaFree(c.buf);
+    }
+  }
   s->chunks.clear();
   s->nsamples = 0;
   if (s->dft_re) {
@@ -253,6 +264,7 @@ int run_segment(rketd_sim *s, int64_t nsteps, void *rec) {
       CU_TRY(s, cudaMalloc(&s->d_srctab, (size_t)nsteps * L.esize));
       s->srctab_cap = nsteps;
     }
+    // (pageable source: cudaMemcpyAsync stages it before returning, so the local vector may die at once)
     if (s->dtype == RKETD_F64) {
       std::vector<double> tab((size_t)nsteps);
       for (int64_t n = 0; n < nsteps; ++n) tab[(size_t)n] = source_sample(s, s->step + n);
@@ -379,7 +391,7 @@ int rketd_set_media(rketd_sim *s, const double *wp, const double *nu) {
   const bool reconvert = s->have_media && !s->fields_zero && !s->third_is_J;
   if (reconvert) {
     SM_TRY(cudaMalloc(&tJ, (size_t)L.ncells * L.nbatch * L.esize));
-    SM_TRY(launch_G_to_current(s->dtype, L, s->wp_p, s->nu_p, s->dz, s->dt, s->fld[s->cur][0], s->fld[s->cur][2], tJ,
+    SM_TRY(launch_G_to_current(s->dtype, L, s->wp_p, s->nu_p, s->dz, s->dt, s->media_scheme, s->fld[s->cur][0], s->fld[s->cur][2], tJ,
                                s->stream));
     ++s->ctr_launches;
   }
@@ -394,7 +406,7 @@ int rketd_set_media(rketd_sim *s, const double *wp, const double *nu) {
     dnu = (const double *)tnu;
   }
   SM_TRY(cudaMemsetAsync(s->d_bad, 0, sizeof(int), s->stream));
-  SM_TRY(launch_coefficients(s->dtype, L, dwp, dnu, s->dz, s->dt, s->wp_p, s->nu_p, s->coef, s->d_bad, s->stream));
+  SM_TRY(launch_coefficients(s->dtype, L, dwp, dnu, s->dz, s->dt, s->scheme, s->wp_p, s->nu_p, s->coef, s->d_bad, s->stream));
   ++s->ctr_launches;
   int bad = 0;
   SM_TRY(cudaMemcpyAsync(&bad, s->d_bad, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
@@ -404,13 +416,14 @@ int rketd_set_media(rketd_sim *s, const double *wp, const double *nu) {
     s->have_media = false;
     return fail(s, RKETD_EINVAL, "rketd_set_media: wp and nu must be finite and non-negative");
   }
+  s->media_scheme = s->scheme;
   if (reconvert) {
     SM_TRY(cudaMemsetAsync(s->fld[s->cur][2], 0, arr_bytes(L), s->stream));
     SM_TRY(copy_in(s, s->fld[s->cur][2], tJ));
   }
   if (reconvert || s->third_is_J) {
-    SM_TRY(launch_current_to_G(s->dtype, L, s->wp_p, s->nu_p, s->dz, s->dt, s->fld[s->cur][0], s->fld[s->cur][2],
-                               s->stream));
+    SM_TRY(launch_current_to_G(s->dtype, L, s->wp_p, s->nu_p, s->dz, s->dt, s->media_scheme, s->fld[s->cur][0],
+                               s->fld[s->cur][2], s->stream));
     ++s->ctr_launches;
     SM_TRY(cudaStreamSynchronize(s->stream));
   }
@@ -418,6 +431,13 @@ int rketd_set_media(rketd_sim *s, const double *wp, const double *nu) {
   cleanup();
   s->third_is_J = false;
   s->have_media = true;
+  return RKETD_OK;
+}
+
+int rketd_set_scheme(rketd_sim *s, int scheme) {
+  if (!s) return RKETD_EINVAL;
+  if (scheme != RKETD_SCHEME_ETD2 && scheme != RKETD_SCHEME_ETD1) return fail(s, RKETD_EINVAL, "rketd_set_scheme: unknown scheme");
+  s->scheme = scheme;
   return RKETD_OK;
 }
 
@@ -466,8 +486,8 @@ int rketd_set_fields(rketd_sim *s, const void *E, const void *H, const void *J) 
   s->third_is_J = false;
   if (E || J) {   // the kernels carry G = cj J - cj kc E in the third array (rketd_device.cuh)
     if (s->have_media) {
-      CU_TRY(s, launch_current_to_G(s->dtype, s->L, s->wp_p, s->nu_p, s->dz, s->dt, s->fld[s->cur][0], s->fld[s->cur][2],
-                                    s->stream));
+      CU_TRY(s, launch_current_to_G(s->dtype, s->L, s->wp_p, s->nu_p, s->dz, s->dt, s->media_scheme, s->fld[s->cur][0],
+                                    s->fld[s->cur][2], s->stream));
       ++s->ctr_launches;
     } else {
       s->third_is_J = true;   // converted by rketd_set_media
@@ -522,8 +542,14 @@ int rketd_run(rketd_sim *s, int64_t nsteps) {
   if (nseries == 0) return run_segment(s, nsteps, nullptr);
   if (s->freqs.empty()) {   // time-series mode: one record chunk per call
     void *buf = nullptr;
-    CU_TRY(s, cudaMalloc(&buf, (size_t)nseries * nsteps * L.esize));
-    s->chunks.push_back(Chunk{buf, nsteps});
+    size_t bytes = (size_t)nseries * nsteps * L.esize;
+    if (s->spare_buf && s->spare_bytes >= bytes) {
+      buf = s->spare_buf; bytes = s->spare_bytes;
+      s->spare_buf = nullptr; s->spare_bytes = 0;
+    } else {
+      CU_TRY(s, cudaMalloc(&buf, bytes));
+    }
+    s->chunks.push_back(Chunk{buf, nsteps, bytes});
     int rc = run_segment(s, nsteps, buf);
     if (rc) return rc;
     s->nsamples += nsteps;
@@ -599,8 +625,8 @@ int rketd_get_fields(rketd_sim *s, void *E, void *H, void *J) {
       const size_t n = (size_t)s->L.ncells * s->L.nbatch * s->L.esize;
       void *dst = J;
       if (!is_device_ptr(J)) { CU_TRY(s, cudaMalloc(&tmp, n)); dst = tmp; }
-      cudaError_t e = launch_G_to_current(s->dtype, s->L, s->wp_p, s->nu_p, s->dz, s->dt, s->fld[s->cur][0],
-                                          s->fld[s->cur][2], dst, s->stream);
+      cudaError_t e = launch_G_to_current(s->dtype, s->L, s->wp_p, s->nu_p, s->dz, s->dt, s->media_scheme,
+                                          s->fld[s->cur][0], s->fld[s->cur][2], dst, s->stream);
       ++s->ctr_launches;
       if (e == cudaSuccess && tmp) e = cudaMemcpyAsync(J, tmp, n, cudaMemcpyDefault, s->stream);
       if (e != cudaSuccess) { if (tmp) cudaFree(tmp); CU_TRY(s, e); }
@@ -618,7 +644,7 @@ int rketd_get_coefficients(rketd_sim *s, double *out, double *chh_m) {
   const size_t n = (size_t)6 * s->L.ncells * s->L.nbatch * sizeof(double);
   void *tmp = nullptr;
   CU_TRY(s, cudaMalloc(&tmp, n));
-  cudaError_t e = launch_six_coefficients(s->L, s->wp_p, s->nu_p, s->dz, s->dt, (double *)tmp, s->stream);
+  cudaError_t e = launch_six_coefficients(s->L, s->wp_p, s->nu_p, s->dz, s->dt, s->media_scheme, (double *)tmp, s->stream);
   ++s->ctr_launches;
   if (e == cudaSuccess) e = cudaMemcpyAsync(out, tmp, n, cudaMemcpyDefault, s->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
@@ -676,6 +702,7 @@ void rketd_destroy(rketd_sim *s) {
   if (s->d_bad) cudaFree(s->d_bad);
   if (s->d_srctab) cudaFree(s->d_srctab);
   for (auto &c : s->chunks) cudaFree(c.buf);
+  if (s->spare_buf) cudaFree(s->spare_buf);
   if (s->dft_re) cudaFree(s->dft_re);
   if (s->dft_im) cudaFree(s->dft_im);
   if (s->d_freqs) cudaFree(s->d_freqs);

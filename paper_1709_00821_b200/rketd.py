@@ -25,7 +25,9 @@ CTR_LAUNCHES, CTR_STEP_LAUNCHES, CTR_KERNEL_USED, CTR_DEPTH_USED, CTR_STEPS_DONE
 
 EXPORTS = ["rketd_create", "rketd_set_media", "rketd_set_source", "rketd_set_probes", "rketd_set_probe_dft",
            "rketd_set_fields", "rketd_reset", "rketd_discard_records", "rketd_set_plan", "rketd_run", "rketd_read_probes",
-           "rketd_get_fields", "rketd_get_coefficients", "rketd_get_kernel_coefficients", "rketd_get_counter", "rketd_destroy", "rketd_last_error"]
+           "rketd_get_fields", "rketd_get_coefficients", "rketd_get_kernel_coefficients", "rketd_set_scheme",
+           "rketd_get_counter", "rketd_destroy", "rketd_last_error"]
+SCHEME_ETD2, SCHEME_ETD1 = 0, 1
 
 if not os.path.exists(LIB_PATH):
     raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_1709_00821_b200.build` "
@@ -47,13 +49,14 @@ _lib.rketd_read_probes.argtypes = [_vp, _vp, _i64, ctypes.POINTER(_i64)]
 _lib.rketd_get_fields.argtypes = [_vp, _vp, _vp, _vp]
 _lib.rketd_get_coefficients.argtypes = [_vp, _vp, _vp]
 _lib.rketd_get_kernel_coefficients.argtypes = [_vp, _vp]
+_lib.rketd_set_scheme.argtypes = [_vp, _i32]
 _lib.rketd_get_counter.argtypes = [_vp, _i32]
 _lib.rketd_get_counter.restype = _i64
 _lib.rketd_destroy.argtypes = [_vp]
 _lib.rketd_destroy.restype = None
 _lib.rketd_last_error.argtypes = [_vp]
 _lib.rketd_last_error.restype = ctypes.c_char_p
-for _n in EXPORTS[:14]:
+for _n in EXPORTS[:15]:
     getattr(_lib, _n).restype = _i32
 
 
@@ -121,6 +124,10 @@ def rketd_discard_records(h):
     _check(h, _lib.rketd_discard_records(h))
 
 
+def rketd_set_scheme(h, scheme: int):
+    _check(h, _lib.rketd_set_scheme(h, scheme))
+
+
 def rketd_set_plan(h, kernel: int = KERNEL_AUTO, depth: int = 0, variant: int = -1):
     _check(h, _lib.rketd_set_plan(h, kernel, depth, variant))
 
@@ -172,9 +179,11 @@ class Sim:
         self.h = rketd_create(ncells, nbatch, dz, dt, F64 if dtype == "f64" else F32, stream)
 
     @classmethod
-    def from_workload(cls, w, dtype: str = "f64", stream: int = 0, b0: int = 0, b1: Optional[int] = None):
+    def from_workload(cls, w, dtype: str = "f64", stream: int = 0, b0: int = 0, b1: Optional[int] = None,
+                      scheme: int = SCHEME_ETD2):
         b1 = w.nbatch if b1 is None else b1
         s = cls(w.ncells, b1 - b0, w.dz, w.dt, dtype, stream)
+        s.set_scheme(scheme)
         wp, nu = w.media(0, w.ncells, b0, b1)
         s.set_media(np.ascontiguousarray(wp), np.ascontiguousarray(nu))
         E0 = w.initial_E(0, w.ncells, b0, b1)
@@ -201,6 +210,8 @@ class Sim:
     def reset(self): rketd_reset(self.h)
     def discard_records(self): rketd_discard_records(self.h)
     def set_plan(self, kernel=KERNEL_AUTO, depth=0, variant=-1): rketd_set_plan(self.h, kernel, depth, variant)
+
+    def set_scheme(self, scheme): rketd_set_scheme(self.h, scheme)
     def run(self, nsteps): rketd_run(self.h, nsteps)
     def counter(self, which): return rketd_get_counter(self.h, which)
 

@@ -359,3 +359,59 @@ def test_error_codes(rk):
         big.set_plan(rk.KERNEL_RESIDENT, 0, -1)          # 5000 fp64 nodes do not fit one CTA
     big.close()
     s.close()
+
+
+# ---- first-order ETD, eq. (9): only the coefficient precompute differs
+def test_ETD1_coefficients_and_parity_all_kernels(rk):
+    rng = np.random.default_rng(9)
+    n = 3000
+    wp = rng.uniform(0, 2 * np.pi * 60e9, (2, n))
+    nu = rng.uniform(0, 1e11, (2, n))
+    wp[0, :50] = 0.0
+    nu[1, :50] = 0.0
+    s = rk.Sim(n, 2, wl.DZ, wl.DT, "f64")
+    s.set_scheme(rk.SCHEME_ETD1)
+    s.set_media(wp, nu)
+    c = s.get_coefficients()
+    s.close()
+    o = oracle.coefficients(wp, nu, wl.DZ, wl.DT, oracle.SCHEME_ETD1)
+    assert np.all(c["kc"] == 0.0)
+    for k in ("ca", "cj", "ch", "ka", "kb"):
+        ulp = np.abs(c[k] - o[k]) / np.maximum(np.spacing(np.abs(o[k])), 1e-300)
+        # kb = eps0 wp^2 dt phi1(x): expm1 of glibc vs CUDA (1 ulp each way) plus two products
+        assert ulp.max() <= (4.0 if k == "kb" else 2.0), (k, ulp.max())
+    # config 1 at full size through K1, K2, K3: parity with the scheme-1 oracle, bit-identical among the kernels,
+    # and NOT equal to the scheme-0 result (the switch really changes the recurrence)
+    w = wl.config1()
+    ref = oracle.run_workload(w, scheme=oracle.SCHEME_ETD1)
+    ref0 = oracle.run_workload(w)["rec"]
+    assert np.max(np.abs(ref["rec"] - ref0)) > 1e-6 * np.max(np.abs(ref0))
+    first = None
+    for kernel in (rk.KERNEL_STEP, rk.KERNEL_TBLOCK, rk.KERNEL_RESIDENT):
+        s = rk.Sim.from_workload(w, "f64", scheme=rk.SCHEME_ETD1)
+        s.set_plan(kernel, 0, -1)
+        s.run(w.nsteps)
+        rec = s.read_probes()
+        s.close()
+        assert grid_err(rec, ref["rec"]) <= 1e-12, kernel
+        if first is None:
+            first = rec
+        else:
+            assert np.array_equal(first, rec), kernel
+    # fields (J through the G <-> J conversion with kc = 0) while the pulse is still on the line
+    ref = oracle.run_workload(w, nsteps=1500, scheme=oracle.SCHEME_ETD1)["state"]
+    s = rk.Sim.from_workload(w, "f64", scheme=rk.SCHEME_ETD1)
+    s.set_plan(rk.KERNEL_TBLOCK, 0, -1)
+    s.run(1500)
+    E, H, J = s.get_fields()
+    s.close()
+    for g, r in ((E, ref.E), (H, ref.H), (J, ref.J)):
+        assert np.max(np.abs(r)) > 0 and np.max(np.abs(g - r)) <= 1e-12 * np.max(np.abs(r))
+
+
+def test_set_scheme_errors(rk):
+    s = rk.Sim(64, 1, wl.DZ, wl.DT, "f64")
+    with pytest.raises(rk.RketdError) as e:
+        s.set_scheme(7)
+    assert e.value.code == 1
+    s.close()
