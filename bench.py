@@ -322,7 +322,14 @@ def main():
     import torch.distributed as dist
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: librketd has no CPU fallback")
-    from paper_1709_00821_b200 import rketd      # raises if librketd.so is missing
+    from paper_1709_00821_b200 import build as lib_build
+    if int(os.environ.get("LOCAL_RANK", "0")) == 0:
+        lib_build.build_library()                # no-op when the in-tree librketd.so is newer than its sources
+    else:                                        # the other ranks of the node wait for local rank 0's build
+        t_wait = time.time()
+        while lib_build._stale() and time.time() - t_wait < 900:
+            time.sleep(1.0)
+    from paper_1709_00821_b200 import rketd      # raises if librketd.so is missing (there is no CPU fallback)
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

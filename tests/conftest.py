@@ -24,3 +24,13 @@ def pytest_collection_modifyitems(config, items):
     for item in items:
         if "gpu" in item.keywords:
             item.add_marker(skip)
+
+
+@pytest.fixture(scope="session", autouse=True)
+def _built_library():
+    """librketd.so and the oracle are build artefacts (git-ignored): compile them once per session if they are
+    missing or older than their sources (nvcc cross-compiles without a GPU)."""
+    from paper_1709_00821_b200 import build
+    build.build_library()
+    import oracle
+    oracle.build()
