@@ -27,6 +27,7 @@ _loaded = {}
 
 BOUNDARY_MUR = 0
 BOUNDARY_PEC = 1
+BOUNDARY_PML = 2     # Berenger layer + PEC (reading in DESIGN.md §12): pml = (npml, m, R0)
 SRC_NONE = -1
 SRC_GAUSS_DERIV = 0
 SRC_TABLE = 1
@@ -72,6 +73,8 @@ def _lib(omp: bool = False) -> ctypes.CDLL:
         lib.oracle_run.restype = ctypes.c_int
         lib.oracle_run_scheme.argtypes = lib.oracle_run.argtypes + [ctypes.c_int]
         lib.oracle_run_scheme.restype = ctypes.c_int
+        lib.oracle_run_bc.argtypes = lib.oracle_run_scheme.argtypes + [ctypes.c_int, ctypes.c_double, ctypes.c_double]
+        lib.oracle_run_bc.restype = ctypes.c_int
         _loaded[omp] = lib
     return _loaded[omp]
 
@@ -127,7 +130,7 @@ class State:
 def run(state: State, wp, nu, dz: float, dt: float, nsteps: int, *, src_kind: int = SRC_NONE,
         src_params: Sequence[float] = (), src_cell: int = 0, probes: Sequence[int] = (),
         freqs=None, dft=None, record_J: bool = False, boundary: int = BOUNDARY_MUR, omp: bool = False,
-        scheme: int = SCHEME_ETD2):
+        scheme: int = SCHEME_ETD2, pml: Sequence[float] = (0, 0.0, 1.0)):
     """Advance ``state`` by nsteps.  Returns (rec, recJ) with rec[nbatch][nprobes][nsteps]
     (recJ None unless record_J).  ``dft`` = (re, im) accumulator arrays [nbatch][nprobes][nfreq],
     updated in place when ``freqs`` is given."""
@@ -143,10 +146,11 @@ def run(state: State, wp, nu, dz: float, dt: float, nsteps: int, *, src_kind: in
     if fr is not None:
         re, im = dft
         assert re.shape == (nbatch, prb.size, fr.size) and re.flags.c_contiguous and im.flags.c_contiguous
-    rc = _lib(omp).oracle_run_scheme(ncells, nbatch, dz, dt, _p(wp), _p(nu), _p(state.E), _p(state.H), _p(state.J),
+    rc = _lib(omp).oracle_run_bc(ncells, nbatch, dz, dt, _p(wp), _p(nu), _p(state.E), _p(state.H), _p(state.J),
                               src_kind, _p(prm) if prm.size else None, prm.size, src_cell,
                               prb.ctypes.data_as(_I64) if prb.size else None, prb.size, state.step, nsteps,
-                              _p(rec), _p(recJ), _p(fr), 0 if fr is None else fr.size, _p(re), _p(im), boundary, scheme)
+                              _p(rec), _p(recJ), _p(fr), 0 if fr is None else fr.size, _p(re), _p(im), boundary, scheme,
+                                 int(pml[0]), float(pml[1]), float(pml[2]))
     if rc:
         raise ValueError("oracle_run: invalid argument")
     state.step += nsteps
@@ -154,7 +158,8 @@ def run(state: State, wp, nu, dz: float, dt: float, nsteps: int, *, src_kind: in
 
 
 def run_workload(w, nsteps: Optional[int] = None, b0: int = 0, b1: Optional[int] = None, omp: bool = False,
-                 cells: Optional[tuple] = None, scheme: int = SCHEME_ETD2):
+                 cells: Optional[tuple] = None, scheme: int = SCHEME_ETD2, boundary: int = BOUNDARY_MUR,
+                 pml: Sequence[float] = (0, 0.0, 1.0)):
     """Run a ``workloads.Workload`` (duck-typed: only its data attributes are used) on grids
     b0..b1-1.  ``cells=(lo, hi)`` runs the window lo..hi-1 only, with Mur at the window ends
     (pin P7: exact for probes at distance > nsteps from both window ends).
@@ -172,6 +177,6 @@ def run_workload(w, nsteps: Optional[int] = None, b0: int = 0, b1: Optional[int]
         dft = (np.zeros((b1 - b0, len(probes), len(w.dft_freqs))), np.zeros((b1 - b0, len(probes), len(w.dft_freqs))))
     rec, _ = run(st, wp, nu, w.dz, w.dt, nsteps, src_kind=w.src_kind if in_src else SRC_NONE,
                  src_params=w.src_params, src_cell=w.src_cell - lo if in_src else 0, probes=probes,
-                 freqs=w.dft_freqs, dft=dft, omp=omp, scheme=scheme)
+                 freqs=w.dft_freqs, dft=dft, omp=omp, scheme=scheme, boundary=boundary, pml=pml)
     mag = None if dft is None else np.hypot(dft[0], dft[1])
     return {"rec": rec, "dft_mag": mag, "state": st, "probe_cells": [p + lo for p in probes]}

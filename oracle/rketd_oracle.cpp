@@ -166,15 +166,42 @@ double oracle_source(int kind, const double* params, int64_t nparams, int64_t st
 //   freqs           [nfreq] Hz; dft_re/dft_im [nbatch][nprobes][nfreq] accumulators (in/out), NULL = off
 //   boundary        0 = Mur first order (a3), 1 = PEC (E[0] = E[N-1] = 0; oracle-only, for pin P3)
 //   scheme          0 = eq. (11) (second-order ETD), 1 = eq. (9) (first-order ETD): only S0 differs
-int oracle_run_scheme(int64_t ncells, int64_t nbatch, double dz, double dt,
-                      const double* wp, const double* nu, double* E, double* H, double* J,
-                      int src_kind, const double* src_params, int64_t nparams, int64_t src_cell,
-                      const int64_t* probes, int nprobes, int64_t step0, int64_t nsteps,
-                      double* rec, double* recJ,
-                      const double* freqs, int nfreq, double* dft_re, double* dft_im,
-                      int boundary, int scheme) {
+//   boundary 2      PML (the paper's choice: "PML absorbing boundary conditions [29] ... at both
+//                   ends of 5 cells").  The paper gives no conductivity profile; the reading
+//                    is Berenger's layer at normal incidence with polynomial grading:
+//                     E nodes k < npml (and mirrored at the right end): depth rho = (npml - k)/npml,
+//                     H nodes k + 1/2, k < npml:                        depth rho = (npml - k - 1/2)/npml,
+//                     sigma(rho) = sigma_max rho^m,  sigma_max = -(m + 1) eps0 c ln(R0) / (2 npml dz),
+//                     matched magnetic conductivity sigma* = sigma mu0/eps0; with s = sigma dt / (2 eps0):
+//                       E'[k] = ((1 - s)/(1 + s)) E[k] - ((dt/(eps0 dz))/(1 + s)) (H[k] - H[k-1])     (PML E nodes: vacuum,
+//                       H'[k] = ((1 - s)/(1 + s)) H[k] - ((dt/(mu0 dz))/(1 + s)) (E[k+1] - E[k])       media there ignored)
+//                   and a perfect conductor behind the layer: E[0] = E[N-1] = 0.  In 1-D the split fields of [29]
+//                   have one non-trivial part each, so "split" and "unsplit" coincide.
+int oracle_run_bc(int64_t ncells, int64_t nbatch, double dz, double dt,
+                  const double* wp, const double* nu, double* E, double* H, double* J,
+                  int src_kind, const double* src_params, int64_t nparams, int64_t src_cell,
+                  const int64_t* probes, int nprobes, int64_t step0, int64_t nsteps,
+                  double* rec, double* recJ,
+                  const double* freqs, int nfreq, double* dft_re, double* dft_im,
+                  int boundary, int scheme, int npml, double pml_m, double pml_R0) {
   const int64_t N = ncells;
   if (N < 3 || nbatch < 1 || nsteps < 0 || dz <= 0 || dt <= 0 || scheme < 0 || scheme > 1) return 1;
+  if (boundary == 2 && (npml < 1 || 2 * (int64_t)npml + 1 > N || !(pml_R0 > 0.0) || pml_R0 > 1.0 || pml_m < 0.0)) return 1;
+  // PML profile (the same for every grid): index j = distance in nodes from the outer end
+  std::vector<double> pe_a(npml > 0 ? npml : 0), pe_b(npml > 0 ? npml : 0), ph_a(npml > 0 ? npml : 0), ph_b(npml > 0 ? npml : 0);
+  if (boundary == 2) {
+    const double smax = -(pml_m + 1.0) * kEps0 * kC0 * std::log(pml_R0) / (2.0 * double(npml) * dz);
+    for (int j = 0; j < npml; ++j) {
+      const double rho_e = double(npml - j) / double(npml);
+      const double rho_h = (double(npml - j) - 0.5) / double(npml);
+      const double se = smax * std::pow(rho_e, pml_m) * dt / (2.0 * kEps0);
+      const double sh = smax * std::pow(rho_h, pml_m) * dt / (2.0 * kEps0);      // sigma* dt/(2 mu0) = sigma dt/(2 eps0)
+      pe_a[j] = (1.0 - se) / (1.0 + se);
+      pe_b[j] = (dt / (kEps0 * dz)) / (1.0 + se);
+      ph_a[j] = (1.0 - sh) / (1.0 + sh);
+      ph_b[j] = (dt / (kMu0 * dz)) / (1.0 + sh);
+    }
+  }
   if (src_kind >= 0 && (src_cell < 0 || src_cell >= N)) return 1;
   for (int p = 0; p < nprobes; ++p)
     if (probes[p] < 0 || probes[p] >= N) return 1;
@@ -196,6 +223,14 @@ int oracle_run_scheme(int64_t ncells, int64_t nbatch, double dz, double dt,
     cf.ca.resize(N); cf.cj.resize(N); cf.ch.resize(N); cf.ka.resize(N); cf.kb.resize(N); cf.kc.resize(N);
     coefficients(N, wpg, nug, dz, dt, cf.ca.data(), cf.cj.data(), cf.ch.data(), cf.ka.data(),
                  cf.kb.data(), cf.kc.data(), &cf.chh, &cf.m, scheme);
+    if (boundary == 2) {   // PML E nodes: vacuum with electric conductivity (media there are ignored)
+      for (int j = 0; j < npml; ++j) {
+        const int64_t kk[2] = {int64_t(j), N - 1 - int64_t(j)};
+        for (int64_t k : kk) {
+          cf.ca[k] = pe_a[j]; cf.ch[k] = pe_b[j]; cf.cj[k] = 0.0; cf.ka[k] = 1.0; cf.kb[k] = 0.0; cf.kc[k] = 0.0;
+        }
+      }
+    }
     const double* ca = cf.ca.data(); const double* cj = cf.cj.data(); const double* ch = cf.ch.data();
     const double* ka = cf.ka.data(); const double* kb = cf.kb.data(); const double* kc = cf.kc.data();
     const double chh = cf.chh, m = cf.m;
@@ -207,7 +242,11 @@ int oracle_run_scheme(int64_t ncells, int64_t nbatch, double dz, double dt,
 
       // S1: H update, eq. (14)
 #pragma omp parallel for schedule(static) if (par_cells)
-      for (int64_t k = 0; k <= N - 2; ++k) Hg[k] = Hg[k] - chh * (Eg[k + 1] - Eg[k]);
+      for (int64_t k = 0; k <= N - 2; ++k) {
+        if (boundary == 2 && k < npml) Hg[k] = ph_a[k] * Hg[k] - ph_b[k] * (Eg[k + 1] - Eg[k]);
+        else if (boundary == 2 && k > N - 2 - npml) Hg[k] = ph_a[N - 2 - k] * Hg[k] - ph_b[N - 2 - k] * (Eg[k + 1] - Eg[k]);
+        else Hg[k] = Hg[k] - chh * (Eg[k + 1] - Eg[k]);
+      }
 
       // S2: E update, eq. (12) with (11) substituted
 #pragma omp parallel for schedule(static) if (par_cells)
@@ -248,6 +287,18 @@ int oracle_run_scheme(int64_t ncells, int64_t nbatch, double dz, double dt,
     }
   }
   return 0;
+}
+
+int oracle_run_scheme(int64_t ncells, int64_t nbatch, double dz, double dt,
+                      const double* wp, const double* nu, double* E, double* H, double* J,
+                      int src_kind, const double* src_params, int64_t nparams, int64_t src_cell,
+                      const int64_t* probes, int nprobes, int64_t step0, int64_t nsteps,
+                      double* rec, double* recJ,
+                      const double* freqs, int nfreq, double* dft_re, double* dft_im,
+                      int boundary, int scheme) {
+  if (boundary == 2) return 1;     // PML needs its parameters: oracle_run_bc
+  return oracle_run_bc(ncells, nbatch, dz, dt, wp, nu, E, H, J, src_kind, src_params, nparams, src_cell, probes,
+                       nprobes, step0, nsteps, rec, recJ, freqs, nfreq, dft_re, dft_im, boundary, scheme, 0, 0.0, 1.0);
 }
 
 int oracle_run(int64_t ncells, int64_t nbatch, double dz, double dt,

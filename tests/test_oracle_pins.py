@@ -447,3 +447,64 @@ def test_ETD1_coefficients_closed_form_and_vacuum():
                "kc": mpmath.mpf(0)}
         for k, v in ref.items():
             assert abs(c[k][i] - float(v)) <= 4e-16 * abs(float(v)), (k, i)
+
+
+# ----------------------------------------------------------------------------- PML (NEXT-2)
+def _end_reflection(boundary, pml=(0, 0.0, 1.0), tau=20e-12, N=2000):
+    """Peak of what comes back from the left end / peak of what went in, seen at node 600 (source at node 1000)."""
+    z = np.zeros((1, N))
+    st = oracle.State(N, 1)
+    tc = int(4 * tau / DT)
+    rec, _ = oracle.run(st, z, z, DZ, DT, tc + 4400, src_kind=0, src_params=(tau, 4 * tau, 1.0), src_cell=1000,
+                        probes=[600], boundary=boundary, pml=pml)
+    r = rec[0, 0]
+    cut = tc + 2000                      # incident passes by step tc + 800, the echo arrives at step tc + 3200
+    return np.abs(r[cut:]).max() / np.abs(r[:cut]).max()
+
+
+def test_PML_with_R0_1_is_the_PEC_run_bit_for_bit():
+    """sigma = 0 (R0 = 1): the layer is vacuum and the run must equal the PEC-terminated one bit for bit (indexing of
+    the layer, of the mirrored right end and of the conductor behind it)."""
+    w = wl.config1(nsteps=3000)
+    a = oracle.run_workload(w, boundary=oracle.BOUNDARY_PEC)
+    b = oracle.run_workload(w, boundary=oracle.BOUNDARY_PML, pml=(5, 3.0, 1.0))
+    assert np.array_equal(a["rec"], b["rec"]) and np.array_equal(a["state"].H, b["state"].H)
+    assert _end_reflection(oracle.BOUNDARY_PEC) > 0.99
+
+
+def test_PML_matched_layer_attenuates_by_R0_per_round_trip():
+    """Constant profile (m = 0): a matched lossy medium is dispersion-free, a pulse keeps its shape and decays as
+    exp(-sigma eta0 x) = R0^(x / 2d).  Pins sigma_max, the matching sigma* = sigma mu0/eps0 and the signs."""
+    N, npml, R0 = 1400, 600, 1e-3
+    z = np.zeros((1, N))
+    st = oracle.State(N, 1)
+    probes = [500, 400, 300]                           # 100, 200, 300 nodes inside the left layer (interface at 600)
+    rec, _ = oracle.run(st, z, z, DZ, DT, 1800, src_kind=0, src_params=(20e-12, 80e-12, 1.0), src_cell=700,
+                        probes=probes, boundary=oracle.BOUNDARY_PML, pml=(npml, 0.0, R0))
+    pk = np.abs(rec[0]).max(1)
+    want = R0 ** (100.0 / (2 * npml))
+    assert abs(pk[1] / pk[0] - want) < 2e-3 * want and abs(pk[2] / pk[1] - want) < 2e-3 * want
+
+
+def test_PML_reflection_floor_against_Mur():
+    """What the paper's 5-cell layer buys (reading: cubic grading, R0 = 1e-6).  For the paper's own pulse
+    (tau = 15 dt, content to 300 GHz) it reflects 7 x less than first-order Mur at S = 1/2, 10 cells 30 x less;
+    for the slow BASELINE pulse (tau = 20 ps) first-order Mur is already at 5e-5 and the 5-cell layer is not better."""
+    tau_paper = 15 * 125e-15
+    mur, pml5, pml10 = (_end_reflection(oracle.BOUNDARY_MUR, tau=tau_paper),
+                        _end_reflection(oracle.BOUNDARY_PML, (5, 3.0, 1e-6), tau=tau_paper),
+                        _end_reflection(oracle.BOUNDARY_PML, (10, 3.0, 1e-6), tau=tau_paper))
+    assert 1e-3 < mur < 3e-3 and pml5 < mur / 5 and pml10 < mur / 25
+    assert _end_reflection(oracle.BOUNDARY_MUR) < 1e-4 and _end_reflection(oracle.BOUNDARY_PML, (5, 3.0, 1e-6)) < 1e-3
+
+
+def test_PML_is_mirror_symmetric():
+    """Source on the centre node of an odd grid: E is even about it, so mirrored probes record the same series
+    (the right layer's H index N-2-j and E index N-1-j)."""
+    N = 401
+    z = np.zeros((1, N))
+    rec, _ = oracle.run(oracle.State(N, 1), z, z, DZ, DT, 1500, src_kind=0, src_params=(1.875e-12, 7.5e-12, 1.0), src_cell=200,
+                        probes=[2, 398, 0, 400, 4, 396], boundary=oracle.BOUNDARY_PML, pml=(5, 3.0, 1e-6))
+    r = rec[0]
+    assert np.abs(r[0]).max() > 1e-4
+    assert np.array_equal(r[0], r[1]) and np.array_equal(r[4], r[5]) and not r[2].any() and not r[3].any()
