@@ -39,6 +39,11 @@ enum {
   RKETD_SCHEME_ETD2 = 0,     /* eq. (11): second-order ETD ("RKETD"), the paper's method; the default   */
   RKETD_SCHEME_ETD1 = 1      /* eq. (9)  PAPER.md:59: first-order ETD, F held at F_n over the step   */
 };
+/* grid ends for rketd_set_boundary */
+enum {
+  RKETD_BC_MUR = 0,          /* first-order Mur at both ends (BASELINE north_star); the default                    */
+  RKETD_BC_PML = 1           /* absorbing layer + conductor, the paper's choice   */
+};
 /* kernel selection for rketd_set_plan */
 enum {
   RKETD_KERNEL_AUTO = 0,     /* resident (K3) when a grid fits one CTA, else temporal blocking (K2) */
@@ -81,6 +86,17 @@ int rketd_set_media(rketd_sim *s, const double *wp, const double *nu);
  * J' = ka J + kb E (kc = 0) and eq. (12) solved for E' has D = 1.  Takes effect at the next rketd_set_media, which
  * derives the coefficients; call it before.  EINVAL: unknown scheme. */
 int rketd_set_scheme(rketd_sim *s, int scheme);
+
+/* Ends of every grid.  RKETD_BC_PML: Berenger's layer of npml nodes (paper: 5) at both ends, a perfect conductor
+ * behind it (E[0] = E[ncells-1] = 0).  The paper gives no conductivity profile; the reading built:
+ * sigma(rho) = sigma_max rho^grading at relative depth rho (E nodes at (npml-k)/npml, H nodes half a node less),
+ * sigma_max = -(grading+1) eps0 c ln(R0) / (2 npml dz) (R0 = design reflection at normal incidence), matched magnetic
+ * conductivity; layer nodes are vacuum: the media given for them are ignored and J stays 0 there.
+ *   E'[k] = ((1-s)/(1+s)) E[k] - ((dt/(eps0 dz))/(1+s)) (H[k]-H[k-1]),  H likewise,  s = sigma dt/(2 eps0).
+ * Takes effect at the next rketd_set_media (which derives the coefficients); call it before.  npml, grading, R0
+ * are ignored for RKETD_BC_MUR.  EINVAL: unknown kind, npml outside 1..32, 2 npml + 1 > ncells, R0 outside (0, 1],
+ * grading < 0. */
+int rketd_set_boundary(rketd_sim *s, int kind, int npml, double grading, double R0);
 
 /* Soft source added to E^{n+1}[cell] in every grid (eq. (15)).
  * kind RKETD_SRC_GAUSS_DERIV: params = {tau, t0, amplitude},

@@ -28,6 +28,10 @@ struct rketd_sim {
   double dz = 0, dt = 0;
   int dtype = 0;
   int scheme = RKETD_SCHEME_ETD2, media_scheme = RKETD_SCHEME_ETD2;   // requested / the one the live coefficients use
+  int bc_npml = 0;                 // requested boundary: 0 = first-order Mur, > 0 = absorbing layer of that many nodes
+  double bc_m = 3.0, bc_R0 = 1e-6;
+  PmlE pml{};                      // the layer the live coefficients use (npml = 0: Mur)
+  double pml_ha[kMaxPml] = {}, pml_hd[kMaxPml] = {};
   cudaStream_t stream = nullptr;
   void *fld[2][3] = {{nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr}};
   int cur = 0;
@@ -137,6 +141,10 @@ int rebuild_rowflags(rketd_sim *s) {
   f[(size_t)((L.off + L.ncells - 1) / L.C)] |= F_MURR;
   if (s->src_kind != RKETD_SRC_NONE) f[(size_t)((L.off + s->src_cell) / L.C)] |= F_SRC;
   for (int64_t c : s->probes) f[(size_t)((L.off + c) / L.C)] |= F_PROBE;
+  for (int j = 0; j <= s->pml.npml && s->pml.npml > 0; ++j) {   // rows with H nodes of a layer, and the node right of the left layer
+    f[(size_t)((L.off + j) / L.C)] |= F_PML;
+    f[(size_t)((L.off + L.ncells - 1 - j) / L.C)] |= F_PML;
+  }
   CU_TRY(s, cudaMemcpyAsync(s->rowflag, f.data(), f.size(), cudaMemcpyHostToDevice, s->stream));
   CU_TRY(s, cudaStreamSynchronize(s->stream));   // f is a local
   s->flags_dirty = false;
@@ -286,6 +294,9 @@ int run_segment(rketd_sim *s, int64_t nsteps, void *rec) {
   sc.nprobes = (int)s->probes.size();
   for (size_t i = 0; i < s->probes.size(); ++i) sc.probe_cell[i] = L.off + s->probes[i];
   sc.rec_stride = nsteps; sc.n0 = 0; sc.src_tab = d_src; sc.rec = rec; sc.rowflag = s->rowflag;
+  sc.npml = s->pml.npml;
+  std::memcpy(sc.pml_ha, s->pml_ha, sizeof(sc.pml_ha));
+  std::memcpy(sc.pml_hd, s->pml_hd, sizeof(sc.pml_hd));
 
   const int kern = resolve_kernel(s);
   s->ctr_kernel_used = kern;
@@ -391,7 +402,7 @@ int rketd_set_media(rketd_sim *s, const double *wp, const double *nu) {
   const bool reconvert = s->have_media && !s->fields_zero && !s->third_is_J;
   if (reconvert) {
     SM_TRY(cudaMalloc(&tJ, (size_t)L.ncells * L.nbatch * L.esize));
-    SM_TRY(launch_G_to_current(s->dtype, L, s->wp_p, s->nu_p, s->dz, s->dt, s->media_scheme, s->fld[s->cur][0], s->fld[s->cur][2], tJ,
+    SM_TRY(launch_G_to_current(s->dtype, L, s->wp_p, s->nu_p, s->dz, s->dt, s->media_scheme, s->pml, s->fld[s->cur][0], s->fld[s->cur][2], tJ,
                                s->stream));
     ++s->ctr_launches;
   }
@@ -405,8 +416,28 @@ int rketd_set_media(rketd_sim *s, const double *wp, const double *nu) {
     SM_TRY(cudaMemcpyAsync(tnu, nu, n, cudaMemcpyDefault, s->stream));
     dnu = (const double *)tnu;
   }
+  // absorbing layer requested by rketd_set_boundary: tables of the E nodes (into the coefficient arrays) and of the
+  // H nodes (kernel parameters).  Reading of PAPER.md:93, :123 in DESIGN.md §12: sigma(rho) = sigma_max rho^m,
+  // sigma_max = -(m+1) eps0 c ln(R0) / (2 npml dz), rho = depth / thickness, matched sigma* = sigma mu0/eps0.
+  PmlE new_pml{};
+  double new_ha[kMaxPml] = {}, new_hd[kMaxPml] = {};
+  new_pml.npml = s->bc_npml;
+  if (s->bc_npml > 0) {
+    const int np = s->bc_npml;
+    const double smax = -(s->bc_m + 1.0) * kEps0 * kC0 * std::log(s->bc_R0) / (2.0 * (double)np * s->dz);
+    const double nchh = -(s->dt / (kMu0 * s->dz));
+    for (int j = 0; j < np; ++j) {
+      const double rho_e = (double)(np - j) / (double)np, rho_h = ((double)(np - j) - 0.5) / (double)np;
+      const double se = smax * std::pow(rho_e, s->bc_m) * s->dt / (2.0 * kEps0);
+      const double sh = smax * std::pow(rho_h, s->bc_m) * s->dt / (2.0 * kEps0);
+      new_pml.a[j] = (1.0 - se) / (1.0 + se);
+      new_pml.b[j] = (s->dt / (kEps0 * s->dz)) / (1.0 + se);
+      new_ha[j] = (1.0 - sh) / (1.0 + sh);
+      new_hd[j] = nchh / (1.0 + sh) - nchh;
+    }
+  }
   SM_TRY(cudaMemsetAsync(s->d_bad, 0, sizeof(int), s->stream));
-  SM_TRY(launch_coefficients(s->dtype, L, dwp, dnu, s->dz, s->dt, s->scheme, s->wp_p, s->nu_p, s->coef, s->d_bad, s->stream));
+  SM_TRY(launch_coefficients(s->dtype, L, dwp, dnu, s->dz, s->dt, s->scheme, new_pml, s->wp_p, s->nu_p, s->coef, s->d_bad, s->stream));
   ++s->ctr_launches;
   int bad = 0;
   SM_TRY(cudaMemcpyAsync(&bad, s->d_bad, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
@@ -417,12 +448,16 @@ int rketd_set_media(rketd_sim *s, const double *wp, const double *nu) {
     return fail(s, RKETD_EINVAL, "rketd_set_media: wp and nu must be finite and non-negative");
   }
   s->media_scheme = s->scheme;
+  s->pml = new_pml;
+  std::memcpy(s->pml_ha, new_ha, sizeof(new_ha));
+  std::memcpy(s->pml_hd, new_hd, sizeof(new_hd));
+  s->flags_dirty = true;
   if (reconvert) {
     SM_TRY(cudaMemsetAsync(s->fld[s->cur][2], 0, arr_bytes(L), s->stream));
     SM_TRY(copy_in(s, s->fld[s->cur][2], tJ));
   }
   if (reconvert || s->third_is_J) {
-    SM_TRY(launch_current_to_G(s->dtype, L, s->wp_p, s->nu_p, s->dz, s->dt, s->media_scheme, s->fld[s->cur][0],
+    SM_TRY(launch_current_to_G(s->dtype, L, s->wp_p, s->nu_p, s->dz, s->dt, s->media_scheme, s->pml, s->fld[s->cur][0],
                                s->fld[s->cur][2], s->stream));
     ++s->ctr_launches;
     SM_TRY(cudaStreamSynchronize(s->stream));
@@ -438,6 +473,16 @@ int rketd_set_scheme(rketd_sim *s, int scheme) {
   if (!s) return RKETD_EINVAL;
   if (scheme != RKETD_SCHEME_ETD2 && scheme != RKETD_SCHEME_ETD1) return fail(s, RKETD_EINVAL, "rketd_set_scheme: unknown scheme");
   s->scheme = scheme;
+  return RKETD_OK;
+}
+
+int rketd_set_boundary(rketd_sim *s, int kind, int npml, double grading, double R0) {
+  if (!s) return RKETD_EINVAL;
+  if (kind == RKETD_BC_MUR) { s->bc_npml = 0; return RKETD_OK; }
+  if (kind != RKETD_BC_PML) return fail(s, RKETD_EINVAL, "rketd_set_boundary: unknown kind");
+  if (npml < 1 || npml > kMaxPml || 2 * (int64_t)npml + 1 > s->L.ncells || !(R0 > 0.0) || R0 > 1.0 || !(grading >= 0.0))
+    return fail(s, RKETD_EINVAL, "rketd_set_boundary: need 1 <= npml <= 32, 2 npml + 1 <= ncells, 0 < R0 <= 1, grading >= 0");
+  s->bc_npml = npml; s->bc_m = grading; s->bc_R0 = R0;
   return RKETD_OK;
 }
 
@@ -486,7 +531,7 @@ int rketd_set_fields(rketd_sim *s, const void *E, const void *H, const void *J) 
   s->third_is_J = false;
   if (E || J) {   // the kernels carry G = cj J - cj kc E in the third array (rketd_device.cuh)
     if (s->have_media) {
-      CU_TRY(s, launch_current_to_G(s->dtype, s->L, s->wp_p, s->nu_p, s->dz, s->dt, s->media_scheme, s->fld[s->cur][0],
+      CU_TRY(s, launch_current_to_G(s->dtype, s->L, s->wp_p, s->nu_p, s->dz, s->dt, s->media_scheme, s->pml, s->fld[s->cur][0],
                                     s->fld[s->cur][2], s->stream));
       ++s->ctr_launches;
     } else {
@@ -625,7 +670,7 @@ int rketd_get_fields(rketd_sim *s, void *E, void *H, void *J) {
       const size_t n = (size_t)s->L.ncells * s->L.nbatch * s->L.esize;
       void *dst = J;
       if (!is_device_ptr(J)) { CU_TRY(s, cudaMalloc(&tmp, n)); dst = tmp; }
-      cudaError_t e = launch_G_to_current(s->dtype, s->L, s->wp_p, s->nu_p, s->dz, s->dt, s->media_scheme,
+      cudaError_t e = launch_G_to_current(s->dtype, s->L, s->wp_p, s->nu_p, s->dz, s->dt, s->media_scheme, s->pml,
                                           s->fld[s->cur][0], s->fld[s->cur][2], dst, s->stream);
       ++s->ctr_launches;
       if (e == cudaSuccess && tmp) e = cudaMemcpyAsync(J, tmp, n, cudaMemcpyDefault, s->stream);
@@ -644,7 +689,7 @@ int rketd_get_coefficients(rketd_sim *s, double *out, double *chh_m) {
   const size_t n = (size_t)6 * s->L.ncells * s->L.nbatch * sizeof(double);
   void *tmp = nullptr;
   CU_TRY(s, cudaMalloc(&tmp, n));
-  cudaError_t e = launch_six_coefficients(s->L, s->wp_p, s->nu_p, s->dz, s->dt, s->media_scheme, (double *)tmp, s->stream);
+  cudaError_t e = launch_six_coefficients(s->L, s->wp_p, s->nu_p, s->dz, s->dt, s->media_scheme, s->pml, (double *)tmp, s->stream);
   ++s->ctr_launches;
   if (e == cudaSuccess) e = cudaMemcpyAsync(out, tmp, n, cudaMemcpyDefault, s->stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);

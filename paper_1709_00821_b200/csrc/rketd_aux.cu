@@ -69,11 +69,25 @@ __device__ __forceinline__ Six six_coefficients(double w, double v, double dz, d
   return s;
 }
 
+// index of E node k inside an absorbing layer (distance in nodes from the outer end), or -1
+__device__ __forceinline__ int pml_index(const PmlE &pml, int64_t k, int64_t ncells) {
+  if (pml.npml <= 0) return -1;
+  if (k < pml.npml) return (int)k;
+  if (k > ncells - 1 - pml.npml) return (int)(ncells - 1 - k);
+  return -1;
+}
+// layer nodes are vacuum with an electric conductivity (media there are ignored): E' = a E - b dH, J = 0
+__device__ __forceinline__ Six pml_six(const PmlE &pml, int j) {
+  Six s;
+  s.ca = pml.a[j]; s.cj = 0.0; s.ch = pml.b[j]; s.ka = 1.0; s.kb = 0.0; s.kc = 0.0;
+  return s;
+}
+
 // a0: pads the media into the physical layout and derives the four per-node coefficients the stencil
 // kernels use (rketd_device.cuh): P = ca - cj kc, ch, ka, Q = ka (cj kc) + cj kb; padding nodes get zeros.
 template <typename R>
 __global__ void coefficients_kernel(Layout L, const double *__restrict__ wp, const double *__restrict__ nu,
-                                    double dz, double dt, double eps0, int scheme, double *wp_p, double *nu_p, R *cP, R *cch, R *cka,
+                                    double dz, double dt, double eps0, int scheme, PmlE pml, double *wp_p, double *nu_p, R *cP, R *cch, R *cka,
                                     R *cQ, int *bad) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= L.gstride * L.nbatch) return;
@@ -83,7 +97,8 @@ __global__ void coefficients_kernel(Layout L, const double *__restrict__ wp, con
     w = wp[g * L.ncells + k];
     v = nu[g * L.ncells + k];
     if (!(w >= 0.0) || !(v >= 0.0) || isinf(w) || isinf(v)) atomicOr(bad, 1);
-    const Six s = six_coefficients(w, v, dz, dt, eps0, scheme);
+    const int jp = pml_index(pml, k, L.ncells);
+    const Six s = jp >= 0 ? pml_six(pml, jp) : six_coefficients(w, v, dz, dt, eps0, scheme);
     const double kcp = __dmul_rn(s.cj, s.kc), kbp = __dmul_rn(s.cj, s.kb);
     vP = __dsub_rn(s.ca, kcp);
     vch = s.ch;
@@ -95,33 +110,34 @@ __global__ void coefficients_kernel(Layout L, const double *__restrict__ wp, con
 }
 
 cudaError_t launch_coefficients(int dtype, const Layout &L, const double *wp, const double *nu, double dz,
-                                double dt, int scheme, double *wp_p, double *nu_p, void *const coef[kNumCoefArrays], int *d_bad,
-                                cudaStream_t st) {
+                                double dt, int scheme, const PmlE &pml, double *wp_p, double *nu_p, void *const coef[kNumCoefArrays],
+                                int *d_bad, cudaStream_t st) {
   const int64_t total = L.gstride * L.nbatch;
   const unsigned blocks = (unsigned)((total + 255) / 256);
   if (dtype == 0)
-    coefficients_kernel<double><<<blocks, 256, 0, st>>>(L, wp, nu, dz, dt, kEps0, scheme, wp_p, nu_p, (double *)coef[0],
+    coefficients_kernel<double><<<blocks, 256, 0, st>>>(L, wp, nu, dz, dt, kEps0, scheme, pml, wp_p, nu_p, (double *)coef[0],
                                                         (double *)coef[1], (double *)coef[2], (double *)coef[3], d_bad);
   else
-    coefficients_kernel<float><<<blocks, 256, 0, st>>>(L, wp, nu, dz, dt, kEps0, scheme, wp_p, nu_p, (float *)coef[0],
+    coefficients_kernel<float><<<blocks, 256, 0, st>>>(L, wp, nu, dz, dt, kEps0, scheme, pml, wp_p, nu_p, (float *)coef[0],
                                                        (float *)coef[1], (float *)coef[2], (float *)coef[3], d_bad);
   return cudaGetLastError();
 }
 
 __global__ void six_coefficients_kernel(Layout L, const double *__restrict__ wp_p, const double *__restrict__ nu_p,
-                                        double dz, double dt, double eps0, int scheme, double *out) {
+                                        double dz, double dt, double eps0, int scheme, PmlE pml, double *out) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const int64_t n = L.ncells * L.nbatch;
   if (idx >= n) return;
   const int64_t g = idx / L.ncells, k = idx - g * L.ncells, src = g * L.gstride + L.off + k;
-  const Six s = six_coefficients(wp_p[src], nu_p[src], dz, dt, eps0, scheme);
+  const int jp = pml_index(pml, k, L.ncells);
+  const Six s = jp >= 0 ? pml_six(pml, jp) : six_coefficients(wp_p[src], nu_p[src], dz, dt, eps0, scheme);
   out[0 * n + idx] = s.ca; out[1 * n + idx] = s.cj; out[2 * n + idx] = s.ch;
   out[3 * n + idx] = s.ka; out[4 * n + idx] = s.kb; out[5 * n + idx] = s.kc;
 }
 cudaError_t launch_six_coefficients(const Layout &L, const double *wp_p, const double *nu_p, double dz, double dt,
-                                    int scheme, double *out, cudaStream_t st) {
+                                    int scheme, const PmlE &pml, double *out, cudaStream_t st) {
   const int64_t n = L.ncells * L.nbatch;
-  six_coefficients_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(L, wp_p, nu_p, dz, dt, kEps0, scheme, out);
+  six_coefficients_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(L, wp_p, nu_p, dz, dt, kEps0, scheme, pml, out);
   return cudaGetLastError();
 }
 
@@ -152,46 +168,47 @@ cudaError_t launch_unpack_coefficients(int dtype, const Layout &L, void *const c
 // fp64 and round once to the storage type.  Padding nodes: G = 0.
 template <typename R>
 __global__ void current_to_G_kernel(Layout L, const double *__restrict__ wp_p, const double *__restrict__ nu_p, double dz,
-                                    double dt, double eps0, int scheme, const R *__restrict__ E, R *JG) {
+                                    double dt, double eps0, int scheme, PmlE pml, const R *__restrict__ E, R *JG) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= L.gstride * L.nbatch) return;
   const int64_t kp = idx % L.gstride, k = kp - L.off;
   double G = 0.0;
-  if (k >= 0 && k < L.ncells) {
+  if (k >= 0 && k < L.ncells && pml_index(pml, k, L.ncells) < 0) {     // layer nodes carry no current: G = 0
     const Six s = six_coefficients(wp_p[idx], nu_p[idx], dz, dt, eps0, scheme);
     G = __fma_rn(-__dmul_rn(s.cj, s.kc), (double)E[idx], __dmul_rn(s.cj, (double)JG[idx]));
   }
   JG[idx] = (R)G;
 }
 cudaError_t launch_current_to_G(int dtype, const Layout &L, const double *wp_p, const double *nu_p, double dz,
-                                double dt, int scheme, const void *E, void *JG, cudaStream_t st) {
+                                double dt, int scheme, const PmlE &pml, const void *E, void *JG, cudaStream_t st) {
   const int64_t total = L.gstride * L.nbatch;
   const unsigned blocks = (unsigned)((total + 255) / 256);
-  if (dtype == 0) current_to_G_kernel<double><<<blocks, 256, 0, st>>>(L, wp_p, nu_p, dz, dt, kEps0, scheme, (const double *)E, (double *)JG);
-  else current_to_G_kernel<float><<<blocks, 256, 0, st>>>(L, wp_p, nu_p, dz, dt, kEps0, scheme, (const float *)E, (float *)JG);
+  if (dtype == 0) current_to_G_kernel<double><<<blocks, 256, 0, st>>>(L, wp_p, nu_p, dz, dt, kEps0, scheme, pml, (const double *)E, (double *)JG);
+  else current_to_G_kernel<float><<<blocks, 256, 0, st>>>(L, wp_p, nu_p, dz, dt, kEps0, scheme, pml, (const float *)E, (float *)JG);
   return cudaGetLastError();
 }
 
 // J = (G + cj kc E)/cj, written in the user's [nbatch][ncells] layout
 template <typename R>
 __global__ void G_to_current_kernel(Layout L, const double *__restrict__ wp_p, const double *__restrict__ nu_p, double dz,
-                                    double dt, double eps0, int scheme, const R *__restrict__ E, const R *__restrict__ G, R *J_user) {
+                                    double dt, double eps0, int scheme, PmlE pml, const R *__restrict__ E, const R *__restrict__ G, R *J_user) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const int64_t n = L.ncells * L.nbatch;
   if (idx >= n) return;
   const int64_t g = idx / L.ncells, k = idx - g * L.ncells, src = g * L.gstride + L.off + k;
+  if (pml_index(pml, k, L.ncells) >= 0) { J_user[idx] = R(0); return; }     // layer nodes carry no current
   const Six s = six_coefficients(wp_p[src], nu_p[src], dz, dt, eps0, scheme);
   const double J = __ddiv_rn(__fma_rn(__dmul_rn(s.cj, s.kc), (double)E[src], (double)G[src]), s.cj);
   J_user[idx] = (R)J;
 }
 cudaError_t launch_G_to_current(int dtype, const Layout &L, const double *wp_p, const double *nu_p, double dz,
-                                double dt, int scheme, const void *E, const void *G, void *J_user, cudaStream_t st) {
+                                double dt, int scheme, const PmlE &pml, const void *E, const void *G, void *J_user, cudaStream_t st) {
   const int64_t n = L.ncells * L.nbatch;
   const unsigned blocks = (unsigned)((n + 255) / 256);
   if (dtype == 0)
-    G_to_current_kernel<double><<<blocks, 256, 0, st>>>(L, wp_p, nu_p, dz, dt, kEps0, scheme, (const double *)E, (const double *)G, (double *)J_user);
+    G_to_current_kernel<double><<<blocks, 256, 0, st>>>(L, wp_p, nu_p, dz, dt, kEps0, scheme, pml, (const double *)E, (const double *)G, (double *)J_user);
   else
-    G_to_current_kernel<float><<<blocks, 256, 0, st>>>(L, wp_p, nu_p, dz, dt, kEps0, scheme, (const float *)E, (const float *)G, (float *)J_user);
+    G_to_current_kernel<float><<<blocks, 256, 0, st>>>(L, wp_p, nu_p, dz, dt, kEps0, scheme, pml, (const float *)E, (const float *)G, (float *)J_user);
   return cudaGetLastError();
 }
 

@@ -26,7 +26,8 @@ constexpr int kMaxProbes = 64;
 constexpr int kNumCoef = 4;         // P, ch, ka, Q
 enum { COEF_P = 0, COEF_CH = 1, COEF_KA = 2, COEF_Q = 3 };
 
-enum : uint32_t { F_MURL = 1u, F_MURR = 2u, F_SRC = 4u, F_PROBE = 8u };
+enum : uint32_t { F_MURL = 1u, F_MURR = 2u, F_SRC = 4u, F_PROBE = 8u, F_PML = 16u };
+constexpr int kMaxPml = 32;         // deepest absorbing layer, in nodes
 
 template <typename R> struct Arith;
 template <> struct Arith<double> {
@@ -59,6 +60,11 @@ struct StepParams {
   R *rec;                    // [nbatch][nprobes][rec_stride] (a6), or nullptr
   const uint8_t *rowflag;    // [nrows] F_* bits per row
   int64_t probe_cell[kMaxProbes];
+  // PML (rketd_set_boundary): npml = 0 means first-order Mur ends.  H node j nodes from an outer
+  // end updates as H' = ha[j] H + (nchh/(1+s_j)) dE; the kernels apply it as a pre-step H <- ha[j] H + hd[j] dE,
+  // hd[j] = nchh/(1+s_j) - nchh, followed by the ordinary update H <- H + nchh dE.
+  int npml;
+  R pml_ha[kMaxPml], pml_hd[kMaxPml];
 };
 
 // 16-B vector <-> scalars
@@ -255,12 +261,19 @@ struct SpecialIdx {
   int np = 0;                      // probes among this thread's nodes that it records: 0, 1, 2; 3 = more (generic loop)
   int pi0 = -1, pi1 = -1;          // local indices of the first two
   int64_t pr0 = 0, pr1 = 0;        // their record offsets (grid * nprobes + q) * rec_stride; np == 3: k0 and grid
+  // absorbing layer, packed into two registers: pml_mask bit i (left layer) / bit 16+i (right layer): local node i is
+  // an H node of that layer; pml_j = (jL0 + 64) | (jR0 + 64) << 8 | (jN + 1) << 16, where the layer index of local
+  // node i is jL0 + i (left) or jR0 - i (right) and jN is that of the node left of the thread's nodes (-1: none)
+  uint32_t pml_mask = 0, pml_j = 0;
+  __device__ __forceinline__ int jL0() const { return (int)(pml_j & 255u) - 64; }
+  __device__ __forceinline__ int jR0() const { return (int)((pml_j >> 8) & 255u) - 64; }
+  __device__ __forceinline__ int jN() const { return (int)((pml_j >> 16) & 255u) - 1; }
   bool any = false;
 };
 
 // k0: physical in-grid index of the thread's first node; g: grid; owner: this thread records the probes among
 // its nodes (halo threads of a K2 tile do not).
-template <typename R, int C>
+template <typename R, int C, bool PML>
 __device__ __forceinline__ SpecialIdx make_special(const StepParams<R> &p, uint32_t flag, int64_t k0, int64_t g, bool owner) {
   SpecialIdx sx;
   if (!flag) return sx;
@@ -279,7 +292,21 @@ __device__ __forceinline__ SpecialIdx make_special(const StepParams<R> &p, uint3
     }
   }
   if (sx.np == 3) { sx.pr0 = k0; sx.pr1 = g; }
-  sx.any = sx.iL >= 0 || sx.iR >= 0 || sx.iS >= 0 || sx.np > 0;
+  if constexpr (PML) if ((flag & F_PML) && p.npml > 0) {
+    const int64_t jl = k0 - p.cellL, jr = p.cellR - 1 - k0;      // H node k0+i: jl + i from the left end, jr - i from the right
+    uint32_t mL = 0, mR = 0;
+#pragma unroll
+    for (int i = 0; i < C; ++i) {
+      if (jl + i >= 0 && jl + i < p.npml) mL |= 1u << i;
+      if (jr - i >= 0 && jr - i < p.npml) mR |= 1u << i;
+    }
+    int jn = -1;
+    if (jl - 1 >= 0 && jl - 1 < p.npml) jn = (int)(jl - 1);
+    else if (jr + 1 >= 0 && jr + 1 < p.npml) jn = (int)(jr + 1);
+    sx.pml_mask = mL | (mR << 16);
+    sx.pml_j = (uint32_t)((mL ? (int)jl : 0) + 64) | ((uint32_t)((mR ? (int)jr : 0) + 64) << 8) | ((uint32_t)(jn + 1) << 16);
+  }
+  sx.any = (PML && (sx.pml_mask != 0u || sx.jN() >= 0)) || sx.iL >= 0 || sx.iR >= 0 || sx.iS >= 0 || sx.np > 0;
   return sx;
 }
 
@@ -293,19 +320,36 @@ __device__ __forceinline__ void at_index(int idx, F &&f) {
   }
 }
 
-// E: old values, En: new values (modified), H: new values (padding zeroed).
+// Pre-step of the H nodes inside an absorbing layer (see StepParams): runs BEFORE the ordinary H update, on old E.
+// Er: old E of the node right of the thread's nodes.
 template <typename R, int C>
+__device__ __forceinline__ void pml_pre(const R (&E)[C], R Er, R (&H)[C], const StepParams<R> &p, const SpecialIdx &sx) {
+  typedef Arith<R> A;
+#pragma unroll
+  for (int i = 0; i < C; ++i) {
+    const bool l = (sx.pml_mask >> i) & 1u, r = (sx.pml_mask >> (16 + i)) & 1u;
+    if (l || r) {
+      const int j = l ? sx.jL0() + i : sx.jR0() - i;
+      const R dE = A::sub(i + 1 < C ? E[i + 1] : Er, E[i]);
+      H[i] = A::fma(p.pml_ha[j], H[i], A::mul(p.pml_hd[j], dE));
+    }
+  }
+}
+
+// E: old values, En: new values (modified), H: new values (padding zeroed).
+template <typename R, int C, bool PML>
 __device__ __forceinline__ void step_special(const R (&E)[C], R (&En)[C], R (&H)[C], const StepParams<R> &p,
                                              const SpecialIdx &sx, int64_t nloc, R src_now) {
   typedef Arith<R> A;
+  constexpr bool pec = PML;       // a conductor behind the absorbing layer instead of Mur
   if (sx.iL >= 0) {   // a3, left end.  The layout puts node 0 at local index 0 or 1, node 1 in the same thread.
-    if (sx.iL == 0) En[0] = A::fma(p.mur_m, A::sub(En[1], E[0]), E[1]);
-    else { En[1] = A::fma(p.mur_m, A::sub(En[2], E[1]), E[2]); H[0] = R(0); }      // H[0]: padding left of node 0
+    if (sx.iL == 0) En[0] = pec ? R(0) : A::fma(p.mur_m, A::sub(En[1], E[0]), E[1]);
+    else { En[1] = pec ? R(0) : A::fma(p.mur_m, A::sub(En[2], E[1]), E[2]); H[0] = R(0); }      // H[0]: padding left of node 0
   }
   if (sx.iR >= 0) {   // a3, right end.  Node ncells-2 is held by the same thread.
     at_index<1, C>(sx.iR, [&](auto ic) {
       constexpr int i = decltype(ic)::value;
-      En[i] = A::fma(p.mur_m, A::sub(En[i - 1], E[i]), E[i - 1]);
+      En[i] = pec ? R(0) : A::fma(p.mur_m, A::sub(En[i - 1], E[i]), E[i - 1]);
 #pragma unroll
       for (int j = i; j < C; ++j) H[j] = R(0);                                     // H[ncells-1] and padding
     });
@@ -331,14 +375,21 @@ __device__ __forceinline__ void step_special(const R (&E)[C], R (&En)[C], R (&H)
 // The left neighbour's new H is recomputed here from old values (same expression, same bits as the
 // neighbour's own), so that one exchange of old values per step is enough.
 // SPECIAL = false compiles the boundary/source/probe handling out (tiles without such rows).
-template <bool SPECIAL, typename R, int C, typename CF>
+template <bool SPECIAL, bool PML, typename R, int C, typename CF>
 __device__ __forceinline__ void step_fields(const R (&E)[C], R (&En)[C], R (&H)[C], const R (&G)[C], const CF &cf, R El,
                                             R Hl, R Er, R nchh, const StepParams<R> &p, const SpecialIdx &sx,
                                             int64_t nloc, R src_now) {
   typedef Arith<R> A;
   constexpr int V = 16 / sizeof(R);
+  R Hl_old = Hl;
+  if constexpr (SPECIAL && PML) {
+    if (sx.pml_mask) pml_pre<R, C>(E, Er, H, p, sx);
+    // the left neighbour's new H is recomputed below from old values: a layer node needs the same pre-step first
+    const int jn = sx.jN();
+    if (jn >= 0) Hl_old = A::fma(p.pml_ha[jn], Hl, A::mul(p.pml_hd[jn], A::sub(E[0], El)));
+  }
   // a1: H update, eq. (14)
-  const R Hl_new = A::fma(nchh, A::sub(E[0], El), Hl);
+  const R Hl_new = A::fma(nchh, A::sub(E[0], El), Hl_old);
 #pragma unroll
   for (int i = 0; i < C; ++i) H[i] = A::fma(nchh, A::sub(i + 1 < C ? E[i + 1] : Er, E[i]), H[i]);
   // a2: E update, eq. (12) with (11) substituted, in the (P, G) form
@@ -354,7 +405,7 @@ __device__ __forceinline__ void step_fields(const R (&E)[C], R (&En)[C], R (&H)[
     }
   }
   if constexpr (SPECIAL) {
-    if (sx.any) step_special<R, C>(E, En, H, p, sx, nloc, src_now);
+    if (sx.any) step_special<R, C, PML>(E, En, H, p, sx, nloc, src_now);
   }
 }
 

@@ -25,6 +25,12 @@ struct Layout {
 
 struct FieldPtrs { void *E, *H, *J; };
 
+// E-node coefficients of the absorbing layer, index = distance in nodes from the outer end (npml = 0: none)
+struct PmlE {
+  int npml;
+  double a[32], b[32];     // E' = a E - b (H[k] - H[k-1])
+};
+
 // dtype-agnostic description of what a step needs (converted to StepParams<R> by the launchers)
 struct StepCommon {
   double nchh, mur_m;
@@ -35,6 +41,8 @@ struct StepCommon {
   void *rec;
   const uint8_t *rowflag;
   int64_t probe_cell[64];
+  int npml;                      // 0 = Mur ends
+  double pml_ha[32], pml_hd[32]; // H pre-step coefficients of the absorbing layer (rketd_device.cuh StepParams)
 };
 
 // K2 (temporal blocking) plan: tiling + the TMA descriptors for one ping-pong direction.
@@ -74,19 +82,20 @@ cudaError_t k2_configure(int dtype, int variant, int *ctas_per_sm);   // sets sm
 // auxiliary kernels (rketd_aux.cu)
 // media: user wp, nu [nbatch][ncells] -> padded fp64 copies wp_p, nu_p + the four kernel coefficients
 cudaError_t launch_coefficients(int dtype, const Layout &L, const double *wp, const double *nu, double dz,
-                                double dt, int scheme, double *wp_p, double *nu_p, void *const coef[kNumCoefArrays], int *d_bad,
+                                double dt, int scheme, const PmlE &pml, double *wp_p, double *nu_p, void *const coef[kNumCoefArrays],
+                                int *d_bad,
                                 cudaStream_t st);
 // the six coefficients of SURVEY a0 (ca, cj, ch, ka, kb, kc), recomputed in fp64 from the padded media
 cudaError_t launch_six_coefficients(const Layout &L, const double *wp_p, const double *nu_p, double dz, double dt,
-                                    int scheme, double *out, cudaStream_t st);
+                                    int scheme, const PmlE &pml, double *out, cudaStream_t st);
 // the four kernel coefficients as stored (P, ch, ka, Q), converted to fp64, user layout
 cudaError_t launch_unpack_coefficients(int dtype, const Layout &L, void *const coef[kNumCoefArrays], double *out,
                                        cudaStream_t st);
 // J <-> G = cj J - cj kc E on the padded arrays (in place on the third field array)
 cudaError_t launch_current_to_G(int dtype, const Layout &L, const double *wp_p, const double *nu_p, double dz,
-                                double dt, int scheme, const void *E, void *JG, cudaStream_t st);
+                                double dt, int scheme, const PmlE &pml, const void *E, void *JG, cudaStream_t st);
 cudaError_t launch_G_to_current(int dtype, const Layout &L, const double *wp_p, const double *nu_p, double dz,
-                                double dt, int scheme, const void *E, const void *G, void *J_user, cudaStream_t st);
+                                double dt, int scheme, const PmlE &pml, const void *E, const void *G, void *J_user, cudaStream_t st);
 cudaError_t launch_twiddles(const double *d_freqs, int nfreq, int64_t step0, int64_t nsteps, double dt,
                             double2 *tw, cudaStream_t st);
 cudaError_t launch_dft_accumulate(int dtype, const void *rec, int64_t nseries, int64_t nsteps, const double2 *tw,

@@ -28,7 +28,7 @@ template <typename R> struct RowPtrs { R *E, *H, *J; };
 template <typename R> struct CoefPtrs { const R *c[kNumCoef]; };
 
 // ------------------------------------------------------------------------------------ K1
-template <typename R>
+template <typename R, bool PML>
 __global__ void __launch_bounds__(128) k1_step(RowPtrs<R> src, RowPtrs<R> dst, CoefPtrs<R> cp,
                                                const __grid_constant__ StepParams<R> p, int64_t nrows,
                                                int64_t total_rows) {
@@ -48,8 +48,8 @@ __global__ void __launch_bounds__(128) k1_step(RowPtrs<R> src, RowPtrs<R> dst, C
   const R Er = row < nrows - 1 ? src.E[(r + 1) * C] : R(0);
   const uint32_t flag = p.rowflag[row];
   const R src_now = (flag & F_SRC) ? p.src_tab[p.n0] : R(0);
-  const SpecialIdx sx = make_special<R, C>(p, flag, row * C, g, true);
-  step_fields<true, R, C>(E, En, H, G, cf, El, Hl, Er, p.nchh, p, sx, p.n0, src_now);
+  const SpecialIdx sx = make_special<R, C, PML>(p, flag, row * C, g, true);
+  step_fields<true, PML, R, C>(E, En, H, G, cf, El, Hl, Er, p.nchh, p, sx, p.n0, src_now);
   step_current<R, C>(G, E, cf);
   store_nodes_global<R, C>(dst.E, r * C, En);
   store_nodes_global<R, C>(dst.H, r * C, H);
@@ -59,7 +59,7 @@ __global__ void __launch_bounds__(128) k1_step(RowPtrs<R> src, RowPtrs<R> dst, C
 // The time loop shared by K2 and K3: nsteps leapfrog steps of this thread's nodes, halos
 // exchanged inside the CTA.  One __syncthreads per step, placed after phase 2.  The loop is
 // unrolled by two so that E ping-pongs between two register arrays without copies.
-template <bool SPECIAL, typename R, int C, int NW, typename CF>
+template <bool SPECIAL, bool PML, typename R, int C, int NW, typename CF>
 __device__ __forceinline__ void time_loop(R (&E)[C], R (&H)[C], R (&J)[C], const CF &cf, HaloSlots<R, NW> &hs,
                                           const StepParams<R> &p, uint32_t flag, int64_t k0, int64_t g, bool owner,
                                           int64_t nsteps, int warp, int lane) {
@@ -72,10 +72,10 @@ __device__ __forceinline__ void time_loop(R (&E)[C], R (&H)[C], R (&J)[C], const
   R Eb[C];
   SourceStream<R> src;
   src.start(p, SPECIAL && __any_sync(0xffffffffu, (flag & F_SRC) != 0u), nloc, lane);
-  const SpecialIdx sx = SPECIAL ? make_special<R, C>(p, flag, k0, g, owner) : SpecialIdx();
+  const SpecialIdx sx = SPECIAL ? make_special<R, C, PML>(p, flag, k0, g, owner) : SpecialIdx();
   auto one_step = [&](const R (&Ein)[C], R (&Eout)[C], int par) {
     const R src_now = SPECIAL ? src.sample(p, nloc, lane) : R(0);
-    step_fields<SPECIAL, R, C>(Ein, Eout, H, J, cf, El, Hl, Er, nchh, p, sx, nloc, src_now);
+    step_fields<SPECIAL, PML, R, C>(Ein, Eout, H, J, cf, El, Hl, Er, nchh, p, sx, nloc, src_now);
     send_halo<R, C, NW>(Eout, H, hs, par, warp, lane, El, Hl, Er);     // for the next step
     step_current<R, C>(J, Ein, cf);
     cta_barrier();
@@ -96,7 +96,7 @@ __device__ __forceinline__ void time_loop(R (&E)[C], R (&H)[C], R (&J)[C], const
 
 // ------------------------------------------------------------------------------------ K3
 // One CTA per grid; NT threads x C nodes cover the grid (NT * C >= physical nodes per grid).
-template <typename R, int C, int NT, bool CSM, int MINB>
+template <typename R, int C, int NT, bool CSM, int MINB, bool PML>
 __global__ void __launch_bounds__(NT, MINB) k3_resident(RowPtrs<R> f, CoefPtrs<R> cp,
                                                         const __grid_constant__ StepParams<R> p, int64_t nrows,
                                                         int64_t nsteps) {
@@ -157,9 +157,9 @@ __global__ void __launch_bounds__(NT, MINB) k3_resident(RowPtrs<R> f, CoefPtrs<R
       CoefUniform<R, C> cu;
 #pragma unroll
       for (int a = 0; a < kNumCoef; ++a) cu.v[a] = first[a];
-      time_loop<true, R, C, NW>(E, H, J, cu, hs, p, flag, k0, g, true, nsteps, warp, lane);
+      time_loop<true, PML, R, C, NW>(E, H, J, cu, hs, p, flag, k0, g, true, nsteps, warp, lane);
     } else {
-      time_loop<true, R, C, NW>(E, H, J, cf, hs, p, flag, k0, g, true, nsteps, warp, lane);
+      time_loop<true, PML, R, C, NW>(E, H, J, cf, hs, p, flag, k0, g, true, nsteps, warp, lane);
     }
   } else {
     CoefRegs<R, C> cf;
@@ -169,7 +169,7 @@ __global__ void __launch_bounds__(NT, MINB) k3_resident(RowPtrs<R> f, CoefPtrs<R
       for (int i = 0; i < C; ++i) cf.c[a][i] = R(0);
       if (valid) load_nodes_global<R, C>(cp.c[a], first_node, cf.c[a]);
     }
-    time_loop<true, R, C, NW>(E, H, J, cf, hs, p, flag, k0, g, true, nsteps, warp, lane);
+    time_loop<true, PML, R, C, NW>(E, H, J, cf, hs, p, flag, k0, g, true, nsteps, warp, lane);
   }
 
   if (valid) {
@@ -222,7 +222,7 @@ __device__ __forceinline__ void regs_to_tile(uint32_t sout, const uint32_t (&off
 }
 
 // Persistent CTAs; tile = ROWS = NT / TPR rows of 64 B (halo of HR rows on each side included).
-template <typename R, int C, int NT, int MINB>
+template <typename R, int C, int NT, int MINB, bool PML>
 __global__ void __launch_bounds__(NT, MINB) k2_tblock(const __grid_constant__ K2Maps maps,
                                                       const __grid_constant__ StepParams<R> p, K2Args q) {
   typedef Geom<R, C> G;
@@ -286,9 +286,9 @@ __global__ void __launch_bounds__(NT, MINB) k2_tblock(const __grid_constant__ K2
     }
 
     if (special)   // tile holds a boundary, source or probe row (a handful of tiles per grid)
-      time_loop<true, R, C, NW>(E, H, J, cf, hs, p, flag, rowg * G::CR + sub * C, g, owner, q.T, warp, lane);
+      time_loop<true, PML, R, C, NW>(E, H, J, cf, hs, p, flag, rowg * G::CR + sub * C, g, owner, q.T, warp, lane);
     else
-      time_loop<false, R, C, NW>(E, H, J, cf, hs, p, 0u, 0, g, false, q.T, warp, lane);
+      time_loop<false, false, R, C, NW>(E, H, J, cf, hs, p, 0u, 0, g, false, q.T, warp, lane);
 
     // (the barriers of the time loop order tma_wait_read0 before the writes below)
     if (owner) regs_to_tile<R, C>(sout, off_out, kArrayBytes, E, H, J);
@@ -310,7 +310,7 @@ __global__ void __launch_bounds__(NT, MINB) k2_tblock(const __grid_constant__ K2
 // next step's H'[C-1] needs).  Two 64-bit shuffles per step and no redundant arithmetic.  Lanes 0 and 31
 // receive their own values at the tile edge, which is fine: those nodes are in the halo that is thrown
 // away (garbage moves inwards one node per step; the halo is >= T nodes wide).
-template <bool SPECIAL, typename R, int C>
+template <bool SPECIAL, bool PML, typename R, int C>
 __device__ __forceinline__ void warp_step(const R (&E)[C], R (&En)[C], R (&H)[C], R (&G)[C], const CoefRegs<R, C> &cf,
                                           R &Er, R nchh, const StepParams<R> &p, const SpecialIdx &sx, int64_t nloc,
                                           R src_now) {
@@ -318,6 +318,9 @@ __device__ __forceinline__ void warp_step(const R (&E)[C], R (&En)[C], R (&H)[C]
   // Issue cost of an FP64 instruction on sm_100 = max(2, distinct 64-bit register operands) cycles per
   // scheduler (measured): the two FMAs that multiply E[i] sit next to each other so that the
   // second one finds E[i] in the operand-reuse cache, and nchh comes from the constant bank.
+  if constexpr (SPECIAL && PML) {
+    if (sx.pml_mask) pml_pre<R, C>(E, Er, H, p, sx);                           // absorbing-layer H nodes, on old E
+  }
   H[C - 1] = A::fma(nchh, A::sub(Er, E[C - 1]), H[C - 1]);                    // a1, last node first
   const R Hl = __shfl_up_sync(0xffffffffu, H[C - 1], 1);
 #pragma unroll
@@ -330,12 +333,12 @@ __device__ __forceinline__ void warp_step(const R (&E)[C], R (&En)[C], R (&H)[C]
     En[i] = A::fma(-cf.c[COEF_CH][i], A::sub(H[i], i ? H[i - 1] : Hl), t);    // a2
   }
   if constexpr (SPECIAL) {
-    if (sx.any) step_special<R, C>(E, En, H, p, sx, nloc, src_now);       // a3, a4, a6
+    if (sx.any) step_special<R, C, PML>(E, En, H, p, sx, nloc, src_now);       // a3, a4, a6
   }
   Er = __shfl_down_sync(0xffffffffu, En[0], 1);
 }
 
-template <bool SPECIAL, typename R, int C>
+template <bool SPECIAL, bool PML, typename R, int C>
 __device__ __forceinline__ void warp_time_loop(R (&E)[C], R (&H)[C], R (&G)[C], const CoefRegs<R, C> &cf,
                                                const StepParams<R> &p, uint32_t flag, int64_t k0, int64_t g, bool owner,
                                                int nsteps) {
@@ -346,18 +349,18 @@ __device__ __forceinline__ void warp_time_loop(R (&E)[C], R (&H)[C], R (&G)[C], 
   const int lane = threadIdx.x & 31;
   SourceStream<R> src;
   src.start(p, SPECIAL && __any_sync(0xffffffffu, (flag & F_SRC) != 0u), nloc, lane);
-  const SpecialIdx sx = SPECIAL ? make_special<R, C>(p, flag, k0, g, owner) : SpecialIdx();
+  const SpecialIdx sx = SPECIAL ? make_special<R, C, PML>(p, flag, k0, g, owner) : SpecialIdx();
   int left = nsteps;
   for (; left >= 2; left -= 2) {
     const R s0 = SPECIAL ? src.sample(p, nloc, lane) : R(0);
-    warp_step<SPECIAL, R, C>(E, Eb, H, G, cf, Er, nchh, p, sx, nloc, s0);
+    warp_step<SPECIAL, PML, R, C>(E, Eb, H, G, cf, Er, nchh, p, sx, nloc, s0);
     const R s1 = SPECIAL ? src.sample(p, nloc + 1, lane) : R(0);
-    warp_step<SPECIAL, R, C>(Eb, E, H, G, cf, Er, nchh, p, sx, nloc + 1, s1);
+    warp_step<SPECIAL, PML, R, C>(Eb, E, H, G, cf, Er, nchh, p, sx, nloc + 1, s1);
     nloc += 2;
   }
   if (left) {
     const R s0 = SPECIAL ? src.sample(p, nloc, lane) : R(0);
-    warp_step<SPECIAL, R, C>(E, Eb, H, G, cf, Er, nchh, p, sx, nloc, s0);
+    warp_step<SPECIAL, PML, R, C>(E, Eb, H, G, cf, Er, nchh, p, sx, nloc, s0);
 #pragma unroll
     for (int i = 0; i < C; ++i) E[i] = Eb[i];
   }
@@ -366,7 +369,7 @@ __device__ __forceinline__ void warp_time_loop(R (&E)[C], R (&H)[C], R (&G)[C], 
 // DIRECT = false: results leave through a shared-memory stage and TMA stores (10 x 2 KB of shared memory
 // per warp).  DIRECT = true: every owner lane writes its 64-B rows with 256-bit global stores (full 32-B
 // sectors); 7 x 2 KB per warp, which lets 12 warps (3 per scheduler) share an SM.
-template <typename R, int NW, int MINB, bool DIRECT>
+template <typename R, int NW, int MINB, bool DIRECT, bool PML>
 __global__ void __launch_bounds__(NW * 32, MINB) k2_wtile(const __grid_constant__ K2Maps maps,
                                                           const __grid_constant__ StepParams<R> p, K2Args q,
                                                           RowPtrs<R> dst) {
@@ -448,9 +451,9 @@ __global__ void __launch_bounds__(NW * 32, MINB) k2_wtile(const __grid_constant_
     if (!DIRECT && lane == 0) tma_wait_read0();      // previous tile's stores have drained the output stage
 
     if (special)
-      warp_time_loop<true, R, C>(E, H, J, cf, p, myflag, rowg * C, g_cur, owner, q.T);
+      warp_time_loop<true, PML, R, C>(E, H, J, cf, p, myflag, rowg * C, g_cur, owner, q.T);
     else
-      warp_time_loop<false, R, C>(E, H, J, cf, p, 0u, 0, g_cur, false, q.T);
+      warp_time_loop<false, false, R, C>(E, H, J, cf, p, 0u, 0, g_cur, false, q.T);
 
     if constexpr (DIRECT) {
       if (owner && rowg < q.nrows) {
@@ -488,6 +491,8 @@ static StepParams<R> make_params(const StepCommon &sc) {
   p.rec = (R *)sc.rec;
   p.rowflag = sc.rowflag;
   for (int i = 0; i < kMaxProbes; ++i) p.probe_cell[i] = sc.probe_cell[i];
+  p.npml = sc.npml;
+  for (int j = 0; j < kMaxPml; ++j) { p.pml_ha[j] = (R)sc.pml_ha[j]; p.pml_hd[j] = (R)sc.pml_hd[j]; }
   return p;
 }
 template <typename R> static RowPtrs<R> rp(FieldPtrs f) { return RowPtrs<R>{(R *)f.E, (R *)f.H, (R *)f.J}; }
@@ -497,12 +502,17 @@ template <typename R> static CoefPtrs<R> cpz(void *const coef[kNumCoef]) {
   return c;
 }
 
+// Every stencil kernel exists twice: PML = false (first-order Mur ends; exactly the code without any trace of the
+// absorbing layer) and PML = true (rketd_set_boundary: layer pre-step of H, conductor behind the layer).
 template <typename R>
 static cudaError_t launch_k1_t(const Layout &L, FieldPtrs src, FieldPtrs dst, void *const coef[kNumCoef],
                                const StepCommon &sc, cudaStream_t st) {
   const int64_t total = L.nrows * L.nbatch;
   const int64_t blocks = (total + 127) / 128;
-  k1_step<R><<<(unsigned)blocks, 128, 0, st>>>(rp<R>(src), rp<R>(dst), cpz<R>(coef), make_params<R>(sc), L.nrows, total);
+  if (sc.npml > 0)
+    k1_step<R, true><<<(unsigned)blocks, 128, 0, st>>>(rp<R>(src), rp<R>(dst), cpz<R>(coef), make_params<R>(sc), L.nrows, total);
+  else
+    k1_step<R, false><<<(unsigned)blocks, 128, 0, st>>>(rp<R>(src), rp<R>(dst), cpz<R>(coef), make_params<R>(sc), L.nrows, total);
   return cudaGetLastError();
 }
 cudaError_t launch_k1(int dtype, const Layout &L, FieldPtrs src, FieldPtrs dst, void *const coef[kNumCoef],
@@ -523,10 +533,10 @@ int k3_threads_for_rows(int, int64_t nrows, int variant) {
   return 0;
 }
 
-template <typename R, int C, int NT, bool CSM, int MINB>
-static cudaError_t launch_k3_v(const Layout &L, FieldPtrs f, void *const coef[kNumCoef], const StepCommon &sc,
+template <typename R, int C, int NT, bool CSM, int MINB, bool PML>
+static cudaError_t launch_k3_p(const Layout &L, FieldPtrs f, void *const coef[kNumCoef], const StepCommon &sc,
                                int64_t nsteps, cudaStream_t st) {
-  auto kern = k3_resident<R, C, NT, CSM, MINB>;
+  auto kern = k3_resident<R, C, NT, CSM, MINB, PML>;
   const size_t smem = CSM ? (size_t)kNumCoef * (NT / Geom<R, C>::TPR) * kRowBytes + 1024 : 0;
   if (smem > 48 * 1024) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -534,6 +544,12 @@ static cudaError_t launch_k3_v(const Layout &L, FieldPtrs f, void *const coef[kN
   }
   kern<<<(unsigned)L.nbatch, NT, smem, st>>>(rp<R>(f), cpz<R>(coef), make_params<R>(sc), L.nrows, nsteps);
   return cudaGetLastError();
+}
+template <typename R, int C, int NT, bool CSM, int MINB>
+static cudaError_t launch_k3_v(const Layout &L, FieldPtrs f, void *const coef[kNumCoef], const StepCommon &sc,
+                               int64_t nsteps, cudaStream_t st) {
+  return sc.npml > 0 ? launch_k3_p<R, C, NT, CSM, MINB, true>(L, f, coef, sc, nsteps, st)
+                     : launch_k3_p<R, C, NT, CSM, MINB, false>(L, f, coef, sc, nsteps, st);
 }
 template <typename R>
 static cudaError_t launch_k3_t(const Layout &L, FieldPtrs f, void *const coef[kNumCoef], const StepCommon &sc,
@@ -579,16 +595,18 @@ template <typename R> struct K2Variant<R, 1> { static constexpr int C = kRowByte
 template <typename R> struct K2Variant<R, 2> { static constexpr int C = kRowBytes / sizeof(R), NT = 256, MINB = 1; };
 template <typename R> struct K2Variant<R, 3> { static constexpr int C = kRowBytes / sizeof(R) / 2, NT = 512, MINB = 1; };
 
-template <typename K>
-static cudaError_t k2_configure_k(K kern, int variant, int threads, int *ctas) {
+template <typename K, typename KP>
+static cudaError_t k2_configure_k(K kern, KP kern_pml, int variant, int threads, int *ctas) {
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k2_smem_bytes(variant));
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(kern_pml, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k2_smem_bytes(variant));
   if (e != cudaSuccess) return e;
   return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas, kern, threads, k2_smem_bytes(variant));
 }
 template <typename R, int V>
 static cudaError_t k2_configure_v(int *ctas) {
   typedef K2Variant<R, V> KV;
-  return k2_configure_k(k2_tblock<R, KV::C, KV::NT, KV::MINB>, V, KV::NT, ctas);
+  return k2_configure_k(k2_tblock<R, KV::C, KV::NT, KV::MINB, false>, k2_tblock<R, KV::C, KV::NT, KV::MINB, true>, V, KV::NT, ctas);
 }
 template <typename R>
 static cudaError_t k2_configure_t(int variant, int *ctas) {
@@ -597,10 +615,10 @@ static cudaError_t k2_configure_t(int variant, int *ctas) {
     case 1: return k2_configure_v<R, 1>(ctas);
     case 2: return k2_configure_v<R, 2>(ctas);
     case 3: return k2_configure_v<R, 3>(ctas);
-    case 4: return k2_configure_k(k2_wtile<R, 8, 1, false>, 4, 256, ctas);
-    case 5: return k2_configure_k(k2_wtile<R, 4, 2, false>, 5, 128, ctas);
-    case 6: return k2_configure_k(k2_wtile<R, 12, 1, true>, 6, 384, ctas);
-    case 7: return k2_configure_k(k2_wtile<R, 8, 1, true>, 7, 256, ctas);
+    case 4: return k2_configure_k(k2_wtile<R, 8, 1, false, false>, k2_wtile<R, 8, 1, false, true>, 4, 256, ctas);
+    case 5: return k2_configure_k(k2_wtile<R, 4, 2, false, false>, k2_wtile<R, 4, 2, false, true>, 5, 128, ctas);
+    case 6: return k2_configure_k(k2_wtile<R, 12, 1, true, false>, k2_wtile<R, 12, 1, true, true>, 6, 384, ctas);
+    case 7: return k2_configure_k(k2_wtile<R, 8, 1, true, false>, k2_wtile<R, 8, 1, true, true>, 7, 256, ctas);
   }
   return cudaErrorInvalidValue;
 }
@@ -611,8 +629,17 @@ cudaError_t k2_configure(int dtype, int variant, int *ctas) {
 template <typename R, int V>
 static cudaError_t launch_k2_v(const K2Plan &plan, int src_buf, const StepParams<R> &sp, const K2Args &q, cudaStream_t st) {
   typedef K2Variant<R, V> KV;
-  k2_tblock<R, KV::C, KV::NT, KV::MINB><<<plan.grid, KV::NT, plan.smem_bytes, st>>>(plan.maps[src_buf], sp, q);
+  if (sp.npml > 0)
+    k2_tblock<R, KV::C, KV::NT, KV::MINB, true><<<plan.grid, KV::NT, plan.smem_bytes, st>>>(plan.maps[src_buf], sp, q);
+  else
+    k2_tblock<R, KV::C, KV::NT, KV::MINB, false><<<plan.grid, KV::NT, plan.smem_bytes, st>>>(plan.maps[src_buf], sp, q);
   return cudaGetLastError();
+}
+template <typename R, int NW, int MINB, bool DIRECT>
+static void launch_k2_w(const K2Plan &plan, const K2Maps &m, const StepParams<R> &sp, const K2Args &q, RowPtrs<R> dst,
+                        cudaStream_t st) {
+  if (sp.npml > 0) k2_wtile<R, NW, MINB, DIRECT, true><<<plan.grid, NW * 32, plan.smem_bytes, st>>>(m, sp, q, dst);
+  else k2_wtile<R, NW, MINB, DIRECT, false><<<plan.grid, NW * 32, plan.smem_bytes, st>>>(m, sp, q, dst);
 }
 template <typename R>
 static cudaError_t launch_k2_t(const Layout &L, const K2Plan &plan, int src_buf, FieldPtrs dst, const StepCommon &sc,
@@ -628,10 +655,10 @@ static cudaError_t launch_k2_t(const Layout &L, const K2Plan &plan, int src_buf,
     case 1: return launch_k2_v<R, 1>(plan, src_buf, sp, q, st);
     case 2: return launch_k2_v<R, 2>(plan, src_buf, sp, q, st);
     case 3: return launch_k2_v<R, 3>(plan, src_buf, sp, q, st);
-    case 4: k2_wtile<R, 8, 1, false><<<plan.grid, 256, plan.smem_bytes, st>>>(m, sp, q, rp<R>(dst)); break;
-    case 5: k2_wtile<R, 4, 2, false><<<plan.grid, 128, plan.smem_bytes, st>>>(m, sp, q, rp<R>(dst)); break;
-    case 6: k2_wtile<R, 12, 1, true><<<plan.grid, 384, plan.smem_bytes, st>>>(m, sp, q, rp<R>(dst)); break;
-    case 7: k2_wtile<R, 8, 1, true><<<plan.grid, 256, plan.smem_bytes, st>>>(m, sp, q, rp<R>(dst)); break;
+    case 4: launch_k2_w<R, 8, 1, false>(plan, m, sp, q, rp<R>(dst), st); break;
+    case 5: launch_k2_w<R, 4, 2, false>(plan, m, sp, q, rp<R>(dst), st); break;
+    case 6: launch_k2_w<R, 12, 1, true>(plan, m, sp, q, rp<R>(dst), st); break;
+    case 7: launch_k2_w<R, 8, 1, true>(plan, m, sp, q, rp<R>(dst), st); break;
     default: return cudaErrorInvalidValue;
   }
   return cudaGetLastError();

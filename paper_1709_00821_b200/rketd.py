@@ -26,8 +26,10 @@ CTR_LAUNCHES, CTR_STEP_LAUNCHES, CTR_KERNEL_USED, CTR_DEPTH_USED, CTR_STEPS_DONE
 EXPORTS = ["rketd_create", "rketd_set_media", "rketd_set_source", "rketd_set_probes", "rketd_set_probe_dft",
            "rketd_set_fields", "rketd_reset", "rketd_discard_records", "rketd_set_plan", "rketd_run", "rketd_read_probes",
            "rketd_get_fields", "rketd_get_coefficients", "rketd_get_kernel_coefficients", "rketd_set_scheme",
+           "rketd_set_boundary",
            "rketd_get_counter", "rketd_destroy", "rketd_last_error"]
 SCHEME_ETD2, SCHEME_ETD1 = 0, 1
+BC_MUR, BC_PML = 0, 1
 
 if not os.path.exists(LIB_PATH):
     raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_1709_00821_b200.build` "
@@ -50,13 +52,14 @@ _lib.rketd_get_fields.argtypes = [_vp, _vp, _vp, _vp]
 _lib.rketd_get_coefficients.argtypes = [_vp, _vp, _vp]
 _lib.rketd_get_kernel_coefficients.argtypes = [_vp, _vp]
 _lib.rketd_set_scheme.argtypes = [_vp, _i32]
+_lib.rketd_set_boundary.argtypes = [_vp, _i32, _i32, _dbl, _dbl]
 _lib.rketd_get_counter.argtypes = [_vp, _i32]
 _lib.rketd_get_counter.restype = _i64
 _lib.rketd_destroy.argtypes = [_vp]
 _lib.rketd_destroy.restype = None
 _lib.rketd_last_error.argtypes = [_vp]
 _lib.rketd_last_error.restype = ctypes.c_char_p
-for _n in EXPORTS[:15]:
+for _n in EXPORTS[:16]:
     getattr(_lib, _n).restype = _i32
 
 
@@ -128,6 +131,10 @@ def rketd_set_scheme(h, scheme: int):
     _check(h, _lib.rketd_set_scheme(h, scheme))
 
 
+def rketd_set_boundary(h, kind: int, npml: int = 5, grading: float = 3.0, R0: float = 1e-6):
+    _check(h, _lib.rketd_set_boundary(h, kind, npml, grading, R0))
+
+
 def rketd_set_plan(h, kernel: int = KERNEL_AUTO, depth: int = 0, variant: int = -1):
     _check(h, _lib.rketd_set_plan(h, kernel, depth, variant))
 
@@ -180,10 +187,12 @@ class Sim:
 
     @classmethod
     def from_workload(cls, w, dtype: str = "f64", stream: int = 0, b0: int = 0, b1: Optional[int] = None,
-                      scheme: int = SCHEME_ETD2):
+                      scheme: int = SCHEME_ETD2, pml=None):
         b1 = w.nbatch if b1 is None else b1
         s = cls(w.ncells, b1 - b0, w.dz, w.dt, dtype, stream)
         s.set_scheme(scheme)
+        if pml is not None:                      # (npml, grading, R0)
+            s.set_boundary(BC_PML, int(pml[0]), float(pml[1]), float(pml[2]))
         wp, nu = w.media(0, w.ncells, b0, b1)
         s.set_media(np.ascontiguousarray(wp), np.ascontiguousarray(nu))
         E0 = w.initial_E(0, w.ncells, b0, b1)
@@ -212,6 +221,8 @@ class Sim:
     def set_plan(self, kernel=KERNEL_AUTO, depth=0, variant=-1): rketd_set_plan(self.h, kernel, depth, variant)
 
     def set_scheme(self, scheme): rketd_set_scheme(self.h, scheme)
+
+    def set_boundary(self, kind, npml=5, grading=3.0, R0=1e-6): rketd_set_boundary(self.h, kind, npml, grading, R0)
     def run(self, nsteps): rketd_run(self.h, nsteps)
     def counter(self, which): return rketd_get_counter(self.h, which)
 
