@@ -51,7 +51,7 @@ ARRAYS_PER_PASS = 10          # read E, H, G, P, ch, ka, Q; write E, H, G
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` captures (profiles/*.md name the command); key = (workload, dtype, depth T, K2 variant)
 NCU_TRAFFIC_BYTES = {
-    ("config4_line_2p28", "f64", 16, 6): 22.86e9,    # profiles/r01_ncu_full_k2_wtile_config4_f64.md
+    ("config4_line_2p28", "f64", 16, 6): 22.24e9,    # profiles/r01_ncu_full_k2_wtile_config4_f64.md
 }
 
 
