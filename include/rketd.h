@@ -144,6 +144,12 @@ int rketd_run(rketd_sim *s, int64_t nsteps);
  * *nsamples = nfreq.  out may be NULL to query *nsamples.  EINVAL if out_bytes is too small. */
 int rketd_read_probes(rketd_sim *s, void *out, int64_t out_bytes, int64_t *nsamples);
 
+/* DFT mode only: the complex accumulators themselves, X = re + j im, each [nbatch][nprobes][nfreq] fp64 (host or
+ * device), count = elements each buffer can hold.  Linear in the records, so reflection and transmission of a sweep
+ * follow from two runs as |X_slab - X_vacuum| / |X_vacuum| and |X_slab| / |X_vacuum|.
+ * Synchronises.  ESTATE outside DFT mode; EINVAL if count is too small. */
+int rketd_read_probe_dft(rketd_sim *s, double *re, double *im, int64_t count);
+
 /* Copy the fields out ([nbatch][ncells], handle's dtype, host or device; any may be NULL).
  * Synchronises. */
 int rketd_get_fields(rketd_sim *s, void *E, void *H, void *J);

@@ -163,7 +163,7 @@ def run_workload(w, nsteps: Optional[int] = None, b0: int = 0, b1: Optional[int]
     """Run a ``workloads.Workload`` (duck-typed: only its data attributes are used) on grids
     b0..b1-1.  ``cells=(lo, hi)`` runs the window lo..hi-1 only, with Mur at the window ends
     (pin P7: exact for probes at distance > nsteps from both window ends).
-    Returns dict(rec, dft_mag, state)."""
+    Returns dict(rec, dft_mag, dft (complex accumulators), state)."""
     b1 = w.nbatch if b1 is None else b1
     lo, hi = (0, w.ncells) if cells is None else cells
     nsteps = w.nsteps if nsteps is None else nsteps
@@ -179,4 +179,5 @@ def run_workload(w, nsteps: Optional[int] = None, b0: int = 0, b1: Optional[int]
                  src_params=w.src_params, src_cell=w.src_cell - lo if in_src else 0, probes=probes,
                  freqs=w.dft_freqs, dft=dft, omp=omp, scheme=scheme, boundary=boundary, pml=pml)
     mag = None if dft is None else np.hypot(dft[0], dft[1])
-    return {"rec": rec, "dft_mag": mag, "state": st, "probe_cells": [p + lo for p in probes]}
+    cplx = None if dft is None else dft[0] + 1j * dft[1]
+    return {"rec": rec, "dft_mag": mag, "dft": cplx, "state": st, "probe_cells": [p + lo for p in probes]}

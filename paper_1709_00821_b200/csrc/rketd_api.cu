@@ -658,6 +658,19 @@ int rketd_read_probes(rketd_sim *s, void *out, int64_t out_bytes, int64_t *nsamp
   return RKETD_OK;
 }
 
+int rketd_read_probe_dft(rketd_sim *s, double *re, double *im, int64_t count) {
+  if (!s) return RKETD_EINVAL;
+  if (s->freqs.empty()) return fail(s, RKETD_ESTATE, "rketd_read_probe_dft: not in DFT mode (rketd_set_probe_dft)");
+  const int64_t n = s->L.nbatch * (int64_t)s->probes.size() * (int64_t)s->freqs.size();
+  if (count < n || (n > 0 && (!re || !im))) return fail(s, RKETD_EINVAL, "rketd_read_probe_dft: buffers too small");
+  if (n > 0) {
+    CU_TRY(s, cudaMemcpyAsync(re, s->dft_re, (size_t)n * sizeof(double), cudaMemcpyDefault, s->stream));
+    CU_TRY(s, cudaMemcpyAsync(im, s->dft_im, (size_t)n * sizeof(double), cudaMemcpyDefault, s->stream));
+  }
+  CU_TRY(s, cudaStreamSynchronize(s->stream));
+  return RKETD_OK;
+}
+
 int rketd_get_fields(rketd_sim *s, void *E, void *H, void *J) {
   if (!s) return RKETD_EINVAL;
   if (E) CU_TRY(s, copy_out(s, E, s->fld[s->cur][0]));

@@ -26,7 +26,7 @@ CTR_LAUNCHES, CTR_STEP_LAUNCHES, CTR_KERNEL_USED, CTR_DEPTH_USED, CTR_STEPS_DONE
 EXPORTS = ["rketd_create", "rketd_set_media", "rketd_set_source", "rketd_set_probes", "rketd_set_probe_dft",
            "rketd_set_fields", "rketd_reset", "rketd_discard_records", "rketd_set_plan", "rketd_run", "rketd_read_probes",
            "rketd_get_fields", "rketd_get_coefficients", "rketd_get_kernel_coefficients", "rketd_set_scheme",
-           "rketd_set_boundary",
+           "rketd_set_boundary", "rketd_read_probe_dft",
            "rketd_get_counter", "rketd_destroy", "rketd_last_error"]
 SCHEME_ETD2, SCHEME_ETD1 = 0, 1
 BC_MUR, BC_PML = 0, 1
@@ -53,13 +53,14 @@ _lib.rketd_get_coefficients.argtypes = [_vp, _vp, _vp]
 _lib.rketd_get_kernel_coefficients.argtypes = [_vp, _vp]
 _lib.rketd_set_scheme.argtypes = [_vp, _i32]
 _lib.rketd_set_boundary.argtypes = [_vp, _i32, _i32, _dbl, _dbl]
+_lib.rketd_read_probe_dft.argtypes = [_vp, _vp, _vp, _i64]
 _lib.rketd_get_counter.argtypes = [_vp, _i32]
 _lib.rketd_get_counter.restype = _i64
 _lib.rketd_destroy.argtypes = [_vp]
 _lib.rketd_destroy.restype = None
 _lib.rketd_last_error.argtypes = [_vp]
 _lib.rketd_last_error.restype = ctypes.c_char_p
-for _n in EXPORTS[:16]:
+for _n in EXPORTS[:17]:
     getattr(_lib, _n).restype = _i32
 
 
@@ -129,6 +130,10 @@ def rketd_discard_records(h):
 
 def rketd_set_scheme(h, scheme: int):
     _check(h, _lib.rketd_set_scheme(h, scheme))
+
+
+def rketd_read_probe_dft(h, re, im):
+    _check(h, _lib.rketd_read_probe_dft(h, _ptr(re), _ptr(im), re.size if isinstance(re, np.ndarray) else re.numel()))
 
 
 def rketd_set_boundary(h, kind: int, npml: int = 5, grading: float = 3.0, R0: float = 1e-6):
@@ -233,6 +238,14 @@ class Sim:
         nbytes = out.nbytes if isinstance(out, np.ndarray) else out.numel() * out.element_size()
         rketd_read_probes(self.h, out, nbytes)
         return out
+
+    def read_probe_dft(self):
+        """complex [nbatch][nprobes][nfreq] accumulators of the device DFT"""
+        nf = rketd_read_probes(self.h)
+        re = np.empty((self.nbatch, self.nprobes, nf), np.float64)
+        im = np.empty_like(re)
+        rketd_read_probe_dft(self.h, re, im)
+        return re + 1j * im
 
     def get_fields(self):
         E, H, J = (np.empty((self.nbatch, self.ncells), self.np_dtype) for _ in range(3))

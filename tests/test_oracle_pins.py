@@ -508,3 +508,25 @@ def test_PML_is_mirror_symmetric():
     r = rec[0]
     assert np.abs(r[0]).max() > 1e-4
     assert np.array_equal(r[0], r[1]) and np.array_equal(r[4], r[5]) and not r[2].any() and not r[3].any()
+
+
+# ----------------------------------------------------------------------------- R/T sweep from DFT accumulators (NEXT-4)
+def test_sweep_RT_from_running_dft_matches_analytic():
+    """Config-3 slabs (12 grids: drawn thickness, wp, nu): |R|, |T| from the oracle's running DFT (row a7) of a slab
+    run and of one vacuum run, against the closed form.  Pins the DFT sign/phase convention (a wrong sign of the
+    exponent or an off-by-one in the sample time would not cancel in X_slab - X_vac)."""
+    nb, freqs = 12, np.linspace(2e9, 26e9, 13)
+    w = wl.config3(nbatch=nb)
+    w.dft_freqs = freqs
+    wv = wl.config3(nbatch=1)
+    wv.dft_freqs = freqs
+    wv.media = lambda lo=0, hi=w.ncells, b0=0, b1=1: (np.zeros((b1 - b0, hi - lo)), np.zeros((b1 - b0, hi - lo)))
+    X = oracle.run_workload(w, omp=True)["dft"]
+    inc = oracle.run_workload(wv)["dft"][0]
+    R = np.abs(X[:, 0] - inc[0]) / np.abs(inc[0])
+    T = np.abs(X[:, 1]) / np.abs(inc[1])
+    wp, nu = w.media(2000, 2001, 0, nb)
+    thick = (w.media(0, w.ncells, 0, nb)[0] > 0).sum(1)
+    for g in range(nb):
+        Ra, Ta = _slab_rt_analytic(freqs, wp[g, 0], nu[g, 0], thick[g] * w.dz)
+        assert np.abs(R[g] - Ra).max() < 1e-3 and np.abs(T[g] - Ta).max() < 1e-3, g
