@@ -129,7 +129,7 @@ int rketd_discard_records(rketd_sim *s);
 
 /* Choose the kernel (RKETD_KERNEL_*), for K2 the temporal depth T (0 = default), and the launch
  * variant of K2/K3 (-1 = default; K2: 0..3 = CTA tiles with {nodes per thread, threads per CTA} combinations, 4..7 = warp tiles,
- * K3: 0 = a thread owns a 64-B row, 1 = half a row).  All choices compute identical bits.
+ * K3: 0 = a thread owns a 64-B row, 1 = half a row, 2 = a row with the coefficients in shared memory).  All choices compute identical bits.
  * EINVAL if the choice cannot run this grid (e.g. RESIDENT with a grid larger than one CTA). */
 int rketd_set_plan(rketd_sim *s, int kernel, int depth, int variant);
 

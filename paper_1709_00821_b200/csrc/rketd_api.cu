@@ -209,9 +209,10 @@ int default_depth(const rketd_sim *s) {
   return base;
 }
 int default_k2_variant(const rketd_sim *) { return 6; }
-// fp64 grids of up to 256 rows: half-row threads (twice the warps hide the per-step barrier better: config 5 fp64
-// 630 -> 700 Gcell/s); fp32 is faster with whole rows (1104 vs 931)
-int default_k3_variant(const rketd_sim *s) { return (s->dtype == RKETD_F64 && s->L.nrows <= 256) ? 1 : 0; }
+// Grids of 33..256 rows: whole-row threads with the coefficients in shared memory (128 registers: 4 CTAs of 128
+// threads per SM instead of 3, and warps whose rows carry one coefficient set read nothing per step).  Measured on
+// config 5: fp64 860 Gcell/s against 630 (coefficients in registers) and 670 (half-row threads); fp32 1271 against 965.
+int default_k3_variant(const rketd_sim *s) { return (s->L.nrows > 32 && s->L.nrows <= 256) ? 2 : 0; }
 int max_depth(const rketd_sim *s, int variant) { return (k2_tile_rows(variant) / 2 - 1) * s->L.C; }
 
 int build_k2_plan(rketd_sim *s, int depth, int variant) {

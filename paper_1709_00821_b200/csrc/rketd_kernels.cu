@@ -522,12 +522,14 @@ cudaError_t launch_k1(int dtype, const Layout &L, FieldPtrs src, FieldPtrs dst, 
 
 // K3 variants.  variant 0: a thread owns a whole 64-B row (ROWS = NT); coefficients in registers
 // up to 256 rows, in shared memory at 512 rows.  variant 1: a thread owns half a row (twice the
-// warps per grid, half the registers per thread); up to 256 rows.
+// warps per grid, half the registers per thread); up to 256 rows.  variant 2: whole rows with the
+// coefficients in shared memory at every size (fewer registers: more CTAs per SM); 64 rows and up.
 int k3_threads_for_rows(int, int64_t nrows, int variant) {
   const int opts[] = {32, 64, 128, 256, 512};
   for (int o : opts)
     if (nrows <= o) {
       if (variant == 1) return o <= 256 ? 2 * o : 0;
+      if (variant == 2) return o >= 64 ? o : 0;
       return o;
     }
   return 0;
@@ -560,6 +562,12 @@ static cudaError_t launch_k3_t(const Layout &L, FieldPtrs f, void *const coef[kN
     case 64: return launch_k3_v<R, CF, 64, false, 6>(L, f, coef, sc, nsteps, st);
     case 128: return launch_k3_v<R, CF, 128, false, 3>(L, f, coef, sc, nsteps, st);
     case 256: return launch_k3_v<R, CF, 256, false, 1>(L, f, coef, sc, nsteps, st);
+    case 512: return launch_k3_v<R, CF, 512, true, 1>(L, f, coef, sc, nsteps, st);
+  }
+  else if (variant == 2) switch (NT) {   // whole rows, coefficients in shared memory (warps of uniform rows: registers)
+    case 64: return launch_k3_v<R, CF, 64, true, 8>(L, f, coef, sc, nsteps, st);
+    case 128: return launch_k3_v<R, CF, 128, true, 4>(L, f, coef, sc, nsteps, st);
+    case 256: return launch_k3_v<R, CF, 256, true, 2>(L, f, coef, sc, nsteps, st);
     case 512: return launch_k3_v<R, CF, 512, true, 1>(L, f, coef, sc, nsteps, st);
   }
   else switch (NT) {

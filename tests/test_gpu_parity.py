@@ -65,7 +65,7 @@ def check_fields(gpu, st, tol, peak=0.0, wp_max=0.0):
             assert np.max(np.abs(np.asarray(gpu[k], np.float64) - ref)) <= tol * scale, k
 
 
-ALL_PLANS = [(1, 0, -1), (3, 0, 0), (3, 0, 1)] + [(2, 0, v) for v in range(8)] + [(2, d, 4) for d in (1, 7, 16, 33)] + \
+ALL_PLANS = [(1, 0, -1), (3, 0, 0), (3, 0, 1), (3, 0, 2)] + [(2, 0, v) for v in range(8)] + [(2, d, 4) for d in (1, 7, 16, 33)] + \
             [(2, d, 6) for d in (1, 2, 9, 32, 40)] + [(2, 5, 0), (2, 40, 2)]
 
 

@@ -39,7 +39,7 @@ def _err(gpu, ref):
     return float(np.max(d / sc))
 
 
-PLANS = [(1, 0, -1), (3, 0, 0), (3, 0, 1), (2, 0, 6), (2, 7, 6), (2, 16, 4), (2, 16, 0), (2, 9, 2), (2, 40, 6)]
+PLANS = [(1, 0, -1), (3, 0, 0), (3, 0, 1), (3, 0, 2), (2, 0, 6), (2, 7, 6), (2, 16, 4), (2, 16, 0), (2, 9, 2), (2, 40, 6)]
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
