@@ -75,6 +75,14 @@ def _lib(omp: bool = False) -> ctypes.CDLL:
         lib.oracle_run_scheme.restype = ctypes.c_int
         lib.oracle_run_bc.argtypes = lib.oracle_run_scheme.argtypes + [ctypes.c_int, ctypes.c_double, ctypes.c_double]
         lib.oracle_run_bc.restype = ctypes.c_int
+        lib.oracle2d_coefficients.argtypes = [ctypes.c_int64, _D, _D, ctypes.c_double, ctypes.c_double, ctypes.c_double,
+                                              ctypes.c_int] + [_D] * 8
+        lib.oracle2d_coefficients.restype = ctypes.c_int
+        lib.oracle2d_run.argtypes = [ctypes.c_int64, ctypes.c_int64, ctypes.c_double, ctypes.c_double, ctypes.c_double,
+                                     _D, _D, _D, _D, _D, _D,
+                                     ctypes.c_int, _D, ctypes.c_int64, ctypes.c_int64, ctypes.c_int64,
+                                     _I64, ctypes.c_int, ctypes.c_int64, ctypes.c_int64, _D, _D, ctypes.c_int, ctypes.c_int]
+        lib.oracle2d_run.restype = ctypes.c_int
         _loaded[omp] = lib
     return _loaded[omp]
 
@@ -181,3 +189,66 @@ def run_workload(w, nsteps: Optional[int] = None, b0: int = 0, b1: Optional[int]
     mag = None if dft is None else np.hypot(dft[0], dft[1])
     cplx = None if dft is None else dft[0] + 1j * dft[1]
     return {"rec": rec, "dft_mag": mag, "dft": cplx, "state": st, "probe_cells": [p + lo for p in probes]}
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# 2-D TMz: see the second half of rketd_oracle.cpp
+# ----------------------------------------------------------------------------------------------------------------
+class State2D:
+    """Ez, Hx, Hy, Jz [ny][nx] fp64 plus the global step counter; advanced in place by run2d()."""
+
+    def __init__(self, nx: int, ny: int, Ez0=None, Hx0=None, Hy0=None, Jz0=None):
+        shp = (ny, nx)
+        mk = lambda a: np.zeros(shp) if a is None else np.array(a, np.float64).reshape(shp).copy()
+        self.Ez, self.Hx, self.Hy, self.Jz = mk(Ez0), mk(Hx0), mk(Hy0), mk(Jz0)
+        self.step = 0
+
+
+def coefficients2d(wp, nu, dx: float, dy: float, dt: float, scheme: int = SCHEME_ETD2):
+    """dict(ca, cj, cex, cey, ka, kb, kc [same shape as wp], chx, chy, mx, my)."""
+    wp = np.ascontiguousarray(wp, np.float64)
+    nu = np.ascontiguousarray(nu, np.float64)
+    names = ("ca", "cj", "cex", "cey", "ka", "kb", "kc")
+    out = {k: np.empty_like(wp) for k in names}
+    g = np.zeros(4)
+    if _lib().oracle2d_coefficients(wp.size, _p(wp), _p(nu), dx, dy, dt, scheme, *[_p(out[k]) for k in names], _p(g)):
+        raise ValueError("oracle2d_coefficients: invalid argument")
+    out["chx"], out["chy"], out["mx"], out["my"] = (float(v) for v in g)
+    return out
+
+
+def run2d(state: State2D, wp, nu, dx: float, dy: float, dt: float, nsteps: int, *, src_kind: int = SRC_NONE,
+          src_params: Sequence[float] = (), src_ij=(0, 0), probes=(), record_J: bool = False,
+          boundary: int = BOUNDARY_MUR, omp: bool = False, scheme: int = SCHEME_ETD2):
+    """Advance ``state`` by nsteps.  probes = sequence of (i, j).  Returns (rec, recJ), each [nprobes][nsteps]."""
+    ny, nx = state.Ez.shape
+    wp = np.ascontiguousarray(wp, np.float64).reshape(ny, nx)
+    nu = np.ascontiguousarray(nu, np.float64).reshape(ny, nx)
+    prm = np.ascontiguousarray(src_params, np.float64)
+    prb = np.ascontiguousarray(probes, np.int64).reshape(-1, 2)
+    rec = np.zeros((prb.shape[0], nsteps))
+    recJ = np.zeros((prb.shape[0], nsteps)) if record_J else None
+    rc = _lib(omp).oracle2d_run(nx, ny, dx, dy, dt, _p(wp), _p(nu), _p(state.Ez), _p(state.Hx), _p(state.Hy),
+                                _p(state.Jz), src_kind, _p(prm) if prm.size else None, prm.size, int(src_ij[0]),
+                                int(src_ij[1]), prb.ctypes.data_as(_I64) if prb.size else None, prb.shape[0],
+                                state.step, nsteps, _p(rec), _p(recJ), boundary, scheme)
+    if rc:
+        raise ValueError("oracle2d_run: invalid argument")
+    state.step += nsteps
+    return rec, recJ
+
+
+def run_workload2d(w, nsteps: Optional[int] = None, window=None, omp: bool = False, boundary: Optional[int] = None):
+    """Run a ``workloads.Workload2D`` (duck-typed).  window = (i0, i1, j0, j1) runs nodes i0..i1-1 x j0..j1-1 only,
+    with the edge rule at the window edges (pin Q7: exact for probes farther than nsteps from every window edge).
+    Returns dict(rec [nprobes][nsteps], probe_ij, state)."""
+    i0, i1, j0, j1 = (0, w.nx, 0, w.ny) if window is None else window
+    nsteps = w.nsteps if nsteps is None else nsteps
+    wp, nu = w.media(i0, i1, j0, j1)
+    st = State2D(i1 - i0, j1 - j0, w.initial_E(i0, i1, j0, j1))
+    probes = [(int(i) - i0, int(j) - j0) for i, j in w.probes if i0 <= i < i1 and j0 <= j < j1]
+    in_src = i0 <= w.src_ij[0] < i1 and j0 <= w.src_ij[1] < j1
+    rec, _ = run2d(st, wp, nu, w.dx, w.dy, w.dt, nsteps, src_kind=w.src_kind if in_src else SRC_NONE,
+                   src_params=w.src_params, src_ij=(w.src_ij[0] - i0, w.src_ij[1] - j0) if in_src else (0, 0),
+                   probes=probes, omp=omp, boundary=w.boundary if boundary is None else boundary)
+    return {"rec": rec, "probe_ij": [(i + i0, j + j0) for i, j in probes], "state": st}

@@ -20,7 +20,8 @@
 // residual with eq.(11) literal, P3 discrete energy, P4 RK4 brute force of
 // eq.(6), P5 analytic slab R/T, P6 stability, P7 domain of dependence, P8 DFT,
 // P9 OpenMP == serial, and the phi-functions against 50-digit arithmetic.
-// Nothing in this file is "parity unpinned".
+// The 2-D TMz generalisation at the end of the file has its own pins Q1-Q9
+// (tests/test_oracle2d_pins.py), listed above it.  Nothing in this file is "parity unpinned".
 //
 // Notation: N E-nodes k = 0..N-1; E[k] = Ex(k dz) at integer steps;
 // H[k] = Hy((k+1/2) dz) at half steps, k = 0..N-2 (H[N-1] is padding, kept 0);
@@ -310,6 +311,116 @@ int oracle_run(int64_t ncells, int64_t nbatch, double dz, double dt,
                int boundary) {
   return oracle_run_scheme(ncells, nbatch, dz, dt, wp, nu, E, H, J, src_kind, src_params, nparams, src_cell, probes,
                            nprobes, step0, nsteps, rec, recJ, freqs, nfreq, dft_re, dft_im, boundary, 0);
+}
+
+
+// ============================================================================
+// 2-D TMz generalisation (the paper's stated next step).
+// The paper writes the method for vector fields — eqs. (1)-(3), PAPER.md:33-37 — and then keeps one component
+// pair.  Keeping the components (Ez, Hx, Hy, Jz) of fields that do not vary along z gives
+//     mu0 dHx/dt = -dEz/dy,   mu0 dHy/dt = +dEz/dx,   eps0 dEz/dt + Jz = dHy/dx - dHx/dy,   dJz/dt + nu Jz = eps0 wp^2 Ez.
+// J is advanced by the same recurrence, eq. (11), node by node, and E by eq. (12) PAPER.md:74 with the
+// 1-D difference of H replaced by the z component of the discrete curl; substituting (11) into (12) as in 1-D gives
+// the same D and the same six coefficients, with ch once per axis (cex with dx, cey with dy).
+//
+// Notation.  nx x ny Ez nodes (i, j), arrays row-major [ny][nx] (i fastest).  Ez[j][i] = Ez(i dx, j dy) and Jz at
+// integer steps; Hx[j][i] = Hx(i dx, (j+1/2) dy), j <= ny-2 (row ny-1 is padding, kept 0); Hy[j][i] =
+// Hy((i+1/2) dx, j dy), i <= nx-2 (column nx-1 is padding, kept 0); both at half steps.
+// One step, in the order of the 1-D S1-S6:
+//   S1  Hx[j][i] -= chy (Ez[j+1][i] - Ez[j][i])   chy = dt/(mu0 dy);   Hy[j][i] += chx (Ez[j][i+1] - Ez[j][i])   chx = dt/(mu0 dx)
+//   S2  interior 1 <= i <= nx-2, 1 <= j <= ny-2:
+//       Ez'[j][i] = ca Ez - cj Jz + cex (Hy[j][i] - Hy[j][i-1]) - cey (Hx[j][i] - Hx[j-1][i])
+//   S3  edges: boundary 0 = first-order Mur normal to each edge, e.g. Ez'[j][0] = Ez[j][1] + mx (Ez'[j][1] - Ez[j][0]),
+//       mx = (c dt - dx)/(c dt + dx), my likewise (the 1-D a3 applied along the normal; reading: the paper's PML has
+//       no parameters); boundary 1 = perfect conductor, Ez' = 0 on the four edges.  The four corner
+//       nodes are set to 0 in both cases: no interior update reads them (only edge H values do, and those feed
+//       nothing), so the choice is unobservable.
+//   S4  soft source Ez'[js][is] += s((n+1) dt);   S5  Jz' = ka Jz + kb Ez + kc Ez' at every node;   S6  probes.
+// Pins (tests/test_oracle2d_pins.py): Q1 fields uniform along one axis reproduce the 1-D oracle bit for bit (both axes),
+// Q2 discrete energy in a conducting box, Q3 cavity eigenmode against the scalar three-term recurrence of the Yee
+// dispersion relation with dx != dy, Q4 RK4 brute force of eq. (6) on a recorded node, Q5 transposed problem gives the
+// transposed result, Q7 domain of dependence (windowed run), Q8 OpenMP == serial.
+// ============================================================================
+int oracle2d_coefficients(int64_t n, const double* wp, const double* nu, double dx, double dy, double dt, int scheme,
+                          double* ca, double* cj, double* cex, double* cey, double* ka, double* kb, double* kc,
+                          double* chx_chy_mx_my) {
+  if (n < 0 || dx <= 0 || dy <= 0 || dt <= 0 || scheme < 0 || scheme > 1) return 1;
+  double chx, chy, mx, my;
+  coefficients(n, wp, nu, dy, dt, ca, cj, cey, ka, kb, kc, &chy, &my, scheme);
+  coefficients(n, wp, nu, dx, dt, ca, cj, cex, ka, kb, kc, &chx, &mx, scheme);
+  chx_chy_mx_my[0] = chx; chx_chy_mx_my[1] = chy; chx_chy_mx_my[2] = mx; chx_chy_mx_my[3] = my;
+  return 0;
+}
+
+//   wp, nu, Ez, Hx, Hy, Jz   [ny][nx]
+//   probes                   [nprobes][2] = (i, j);  rec, recJ [nprobes][nsteps] (either may be NULL)
+int oracle2d_run(int64_t nx, int64_t ny, double dx, double dy, double dt,
+                 const double* wp, const double* nu, double* Ez, double* Hx, double* Hy, double* Jz,
+                 int src_kind, const double* src_params, int64_t nparams, int64_t src_i, int64_t src_j,
+                 const int64_t* probes, int nprobes, int64_t step0, int64_t nsteps,
+                 double* rec, double* recJ, int boundary, int scheme) {
+  if (nx < 3 || ny < 3 || nsteps < 0 || dx <= 0 || dy <= 0 || dt <= 0 || scheme < 0 || scheme > 1) return 1;
+  if (boundary < 0 || boundary > 1) return 1;
+  if (src_kind >= 0 && (src_i < 0 || src_i >= nx || src_j < 0 || src_j >= ny)) return 1;
+  for (int p = 0; p < nprobes; ++p)
+    if (probes[2 * p] < 0 || probes[2 * p] >= nx || probes[2 * p + 1] < 0 || probes[2 * p + 1] >= ny) return 1;
+  const int64_t n = nx * ny;
+  std::vector<double> ca(n), cj(n), cex(n), cey(n), ka(n), kb(n), kc(n), Eold(n);
+  double g[4];
+  oracle2d_coefficients(n, wp, nu, dx, dy, dt, scheme, ca.data(), cj.data(), cex.data(), cey.data(), ka.data(),
+                        kb.data(), kc.data(), g);
+  const double chx = g[0], chy = g[1], mx = g[2], my = g[3];
+#define AT(j, i) ((j) * nx + (i))
+  for (int64_t s = 0; s < nsteps; ++s) {
+    const int64_t ng = step0 + s;
+    // S1: H from the curl of E (eq. (2), discretised as eq. (14) PAPER.md:84 along each axis)
+#pragma omp parallel for schedule(static)
+    for (int64_t j = 0; j < ny; ++j)
+      for (int64_t i = 0; i < nx; ++i) {
+        if (j <= ny - 2) Hx[AT(j, i)] = Hx[AT(j, i)] - chy * (Ez[AT(j + 1, i)] - Ez[AT(j, i)]);
+        if (i <= nx - 2) Hy[AT(j, i)] = Hy[AT(j, i)] + chx * (Ez[AT(j, i + 1)] - Ez[AT(j, i)]);
+      }
+    // S2: E from the curl of H and J (eq. (12) PAPER.md:74 with (11) substituted)
+#pragma omp parallel for schedule(static)
+    for (int64_t k = 0; k < n; ++k) Eold[k] = Ez[k];
+#pragma omp parallel for schedule(static)
+    for (int64_t j = 1; j <= ny - 2; ++j)
+      for (int64_t i = 1; i <= nx - 2; ++i) {
+        const int64_t k = AT(j, i);
+        Ez[k] = ca[k] * Eold[k] - cj[k] * Jz[k] + cex[k] * (Hy[k] - Hy[AT(j, i - 1)]) - cey[k] * (Hx[k] - Hx[AT(j - 1, i)]);
+      }
+    // S3: the four edges, then the corners
+    for (int64_t j = 1; j <= ny - 2; ++j) {
+      if (boundary == 0) {
+        Ez[AT(j, 0)] = Eold[AT(j, 1)] + mx * (Ez[AT(j, 1)] - Eold[AT(j, 0)]);
+        Ez[AT(j, nx - 1)] = Eold[AT(j, nx - 2)] + mx * (Ez[AT(j, nx - 2)] - Eold[AT(j, nx - 1)]);
+      } else {
+        Ez[AT(j, 0)] = 0.0; Ez[AT(j, nx - 1)] = 0.0;
+      }
+    }
+    for (int64_t i = 1; i <= nx - 2; ++i) {
+      if (boundary == 0) {
+        Ez[AT(0, i)] = Eold[AT(1, i)] + my * (Ez[AT(1, i)] - Eold[AT(0, i)]);
+        Ez[AT(ny - 1, i)] = Eold[AT(ny - 2, i)] + my * (Ez[AT(ny - 2, i)] - Eold[AT(ny - 1, i)]);
+      } else {
+        Ez[AT(0, i)] = 0.0; Ez[AT(ny - 1, i)] = 0.0;
+      }
+    }
+    Ez[AT(0, 0)] = 0.0; Ez[AT(0, nx - 1)] = 0.0; Ez[AT(ny - 1, 0)] = 0.0; Ez[AT(ny - 1, nx - 1)] = 0.0;
+    // S4: soft source, eq. (15)
+    if (src_kind >= 0) Ez[AT(src_j, src_i)] += source_sample(src_kind, src_params, nparams, ng, dt);
+    // S5: J, eq. (11), every node, with the final E'
+#pragma omp parallel for schedule(static)
+    for (int64_t k = 0; k < n; ++k) Jz[k] = ka[k] * Jz[k] + kb[k] * Eold[k] + kc[k] * Ez[k];
+    // S6: probes
+    for (int p = 0; p < nprobes; ++p) {
+      const int64_t k = AT(probes[2 * p + 1], probes[2 * p]);
+      if (rec) rec[int64_t(p) * nsteps + s] = Ez[k];
+      if (recJ) recJ[int64_t(p) * nsteps + s] = Jz[k];
+    }
+  }
+#undef AT
+  return 0;
 }
 
 }  // extern "C"

@@ -286,3 +286,79 @@ def paper_table2(ncells: int, nsteps: int = 1000) -> Workload:
 
 
 CONFIGS = {1: config1, 2: config2, 3: config3, 4: config4, 5: config5}
+
+
+# ----------------------------------------------------------------------------
+# 2-D TMz (the paper's stated next step): a plasma column in vacuum
+# ----------------------------------------------------------------------------
+BC_MUR = 0
+BC_PEC = 1
+
+
+@dataclasses.dataclass
+class Workload2D:
+    """One 2-D TMz problem instance as plain data (arrays are [ny][nx], x fastest)."""
+    name: str
+    cfg: int
+    nx: int
+    ny: int
+    nsteps: int
+    dx: float
+    dy: float
+    dt: float
+    src_kind: int
+    src_params: Tuple[float, ...]
+    src_ij: Tuple[int, int]
+    probes: np.ndarray                  # int64 [nprobes][2] = (i, j)
+    boundary: int
+    # media(i0, i1, j0, j1) -> (wp, nu) float64 [j1-j0][i1-i0];  initial_E(i0, i1, j0, j1) -> same shape or None
+    media: Callable[..., Tuple[np.ndarray, np.ndarray]]
+    initial_E: Callable[..., Optional[np.ndarray]]
+    dtypes: Tuple[str, ...] = ("f64", "f32")
+    notes: str = ""
+
+    @property
+    def cell_updates(self) -> int:
+        return self.nx * self.ny * self.nsteps
+
+
+def _row_noise(cfg: int, tag: int, i0: int, i1: int, j0: int, j1: int, nx: int, amp: float) -> np.ndarray:
+    """amp * U(-1,1) per node, one stream per grid row, so that any window regenerates bit for bit."""
+    out = np.empty((j1 - j0, i1 - i0))
+    for j in range(j0, j1):
+        out[j - j0] = amp * _rng(cfg, tag, j).uniform(-1.0, 1.0, nx)[i0:i1]
+    return out
+
+
+def tm2d_column(nx: int = 16384, ny: int = 16384, nsteps: int = 1000, noise: bool = True, dy_over_dx: float = 1.0,
+                boundary: int = BC_MUR, nprobes: int = 16) -> Workload2D:
+    """The 2-D counterpart of config 4: a plasma column with a tanh (Epstein) edge in the middle of an nx x ny grid,
+    wp^2(r) = (2 pi 50e9)^2 * 1/2 [1 - tanh((r - 0.15 nx)/(0.025 nx))] (r in nodes of dx, measured in physical
+    distance / dx), nu = 1e10; per-node coefficient arrays.  Source: the same Gaussian-derivative pulse as the 1-D
+    configs, at (nx/4, ny/2), outside the column.  Probes: the source node, nodes around it, on a ring through the
+    column and seeded random nodes.  dx = 75 um, dt = dx/(2c) (Courant number 1/2 per axis, 0.707 of the 2-D limit
+    when dy = dx).  Initial E: 1e-3 U(-1,1) so that probes the pulse has not reached yet carry a signal."""
+    dx, dy = DZ, DZ * dy_over_dx
+    dt = DZ * min(1.0, dy_over_dx) / (2.0 * C0)
+    wp0, nu0 = 2.0 * math.pi * 50e9, 1.0e10
+    ci, cj, R, wd = nx / 2.0, ny / 2.0, 0.15 * nx, 0.025 * nx
+
+    def media(i0=0, i1=nx, j0=0, j1=ny):
+        i = np.arange(i0, i1)[None, :] - ci
+        j = (np.arange(j0, j1)[:, None] - cj) * dy_over_dx
+        r = np.sqrt(i * i + j * j)
+        wp = wp0 * np.sqrt(np.clip(0.5 * (1.0 - np.tanh((r - R) / wd)), 0.0, None))
+        return np.ascontiguousarray(wp), np.full(wp.shape, nu0)
+
+    def initial_E(i0=0, i1=nx, j0=0, j1=ny):
+        return _row_noise(21, 1, i0, i1, j0, j1, nx, 1e-3) if noise else None
+
+    src = (nx // 4, ny // 2)
+    pr = [src, (src[0] + 3, src[1]), (src[0], src[1] + 5), (src[0] - 7, src[1] - 2), (nx // 2, ny // 2), (1, ny // 3),
+          (nx - 2, ny // 3), (nx // 3, 1), (nx // 3, ny - 2), (0, ny // 2), (nx // 2, 0)]
+    rng = _rng(21, 2)
+    while len(pr) < nprobes:
+        pr.append((int(rng.integers(0, nx)), int(rng.integers(0, ny))))
+    pr = np.array(pr[:max(nprobes, 1)], np.int64)
+    return Workload2D(f"tm2d_column_{nx}x{ny}", 21, nx, ny, nsteps, dx, dy, dt, SRC_GAUSS_DERIV, _SRC, src, pr, boundary,
+                      media, initial_E, notes="2-D TMz plasma column, per-node coefficients")
