@@ -1,0 +1,877 @@
+// rketd2d.cu — the 2-D TMz generalisation of the RKETD-FDTD leapfrog (include/rketd2d.h; SURVEY.md §8(f) NEXT-3,
+// PAPER.md:164): C ABI, setup kernels and the two stencil kernels
+//   k1_2d   one fused H/E/J launch per time step (HBM-bound baseline and cross-check),
+//   k2_2d   temporal blocking by streaming: a CTA owns a strip of columns, rows enter one per iteration and pass
+//           through T pipeline stages held in registers, so every HBM byte serves T steps.
+// Both run the same sequence of correctly rounded operations per node (struct Ops) and agree bit for bit.
+//
+// The form computed (the 2-D twin of rketd_device.cuh's 7-operation form).  With the six coefficients of SURVEY a0
+// (Ez' = ca Ez - cj Jz + cex dHy - cey dHx,  Jz' = ka Jz + kb Ez + kc Ez') and G := cj Jz - (cj kc) Ez, exactly:
+//   Hx'[j][i] = fma(-chy, Ez[j+1][i] - Ez[j][i], Hx[j][i])                                   eq. (14), y axis
+//   Hy'[j][i] = fma(+chx, Ez[j][i+1] - Ez[j][i], Hy[j][i])                                   eq. (14), x axis
+//   Ez'[j][i] = fma(ce, fma(-r, Hx'[j][i] - Hx'[j-1][i], Hy'[j][i] - Hy'[j][i-1]), fma(P, Ez, -G))    eq. (12)+(11)
+//   G'[j][i]  = fma(ka, G, Q Ez)                                                            eq. (11)
+// P = ca - cj kc, ce = cex, r = dx/dy (cey = cex r), Q = ka cj kc + cj kb: 11 FP instructions and 4 per-node
+// coefficients per node and step.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/rketd2d.h"
+#include "rketd_coef.cuh"
+#include "rketd_device.cuh"
+#include "rketd_internal.h"
+
+using rketd::Arith;
+using rketd::kC0;
+using rketd::kEps0;
+using rketd::kMu0;
+
+namespace {
+
+constexpr int kMaxProbes2 = 64;
+constexpr int kMaxT = 16;
+constexpr int kNT = 256;       // threads per CTA of the streaming kernel = columns of a strip, one per thread
+constexpr int kPF = 3;         // rows in flight (cp.async) ahead of the row entering the pipeline
+constexpr int kK1Rows = 4;     // rows a K1 thread walks
+
+enum : uint8_t { RF_SPECIAL = 1, RF_PROBE = 2 };
+
+template <typename R>
+struct P2 {
+  int nx, ny;
+  int64_t pitch;
+  R chx, nchy, nr;             // dt/(mu0 dx), -dt/(mu0 dy), -(dx/dy)
+  R mx, my;                    // first-order Mur (S-1)/(S+1) per axis
+  int bc;
+  int src_i, src_j;            // -1: none
+  int nprobes;
+  int probe_i[kMaxProbes2], probe_j[kMaxProbes2];
+  R *rec;                      // [nprobes][rec_stride]
+  int64_t rec_stride, n0;      // samples per probe in rec; local index of the first step of this launch
+  R src[kMaxT];                // source sample of each level of this launch (a4)
+  const uint8_t *rowflag;      // [ny] RF_* bits
+  // streaming plan
+  int HP, Wv, nstrips, nsegs, Sy, dlast;
+};
+
+template <typename R>
+struct Arrays {
+  const R *E, *Hx, *Hy, *G, *cP, *cce, *cka, *cQ;
+  R *E2, *Hx2, *Hy2, *G2;
+};
+
+// The per-node operations, shared by both kernels.
+template <typename R>
+struct Ops {
+  typedef Arith<R> A;
+  static __device__ __forceinline__ R hx_new(R nchy_j, R e, R e_up, R hx) { return A::fma(nchy_j, A::sub(e_up, e), hx); }
+  static __device__ __forceinline__ R hy_new(R chx_i, R e, R e_rt, R hy) { return A::fma(chx_i, A::sub(e_rt, e), hy); }
+  static __device__ __forceinline__ R e_new(R P, R ce, R nr, R e, R g, R hyn, R hyn_l, R hxn, R hxn_d) {
+    const R t = A::fma(nr, A::sub(hxn, hxn_d), A::sub(hyn, hyn_l));
+    return A::fma(ce, t, A::fma(P, e, -g));
+  }
+  static __device__ __forceinline__ R g_new(R ka, R Q, R g, R e) { return A::fma(ka, g, A::mul(Q, e)); }
+  // first-order Mur along the inward normal: E'[edge] = Eold[in] + m (E'[in] - Eold[edge])
+  static __device__ __forceinline__ R mur(R m, R eold_in, R enew_in, R eold_self) {
+    return A::fma(m, A::sub(enew_in, eold_self), eold_in);
+  }
+};
+
+// ------------------------------------------------------------------------------------------------ K1
+// Interior formula of Ez' at node (i, j), everything read from global memory (neighbours outside the grid count as 0);
+// also returns the node's own new Hx, Hy.
+template <typename R>
+__device__ __forceinline__ R interior_e(const P2<R> &p, const Arrays<R> &a, int i, int j, R &hxn, R &hyn) {
+  typedef Ops<R> O;
+  const int64_t idx = (int64_t)j * p.pitch + i;
+  const R e = a.E[idx];
+  const R e_rt = (i + 1 < p.nx) ? a.E[idx + 1] : R(0);
+  const R e_up = (j + 1 < p.ny) ? a.E[idx + p.pitch] : R(0);
+  const R chx_i = (i <= p.nx - 2) ? p.chx : R(0);
+  const R nchy_j = (j <= p.ny - 2) ? p.nchy : R(0);
+  hxn = O::hx_new(nchy_j, e, e_up, a.Hx[idx]);
+  hyn = O::hy_new(chx_i, e, e_rt, a.Hy[idx]);
+  R hyn_l = R(0), hxn_d = R(0);
+  if (i >= 1) hyn_l = O::hy_new(p.chx, a.E[idx - 1], e, a.Hy[idx - 1]);
+  if (j >= 1) hxn_d = O::hx_new(p.nchy, a.E[idx - p.pitch], e, a.Hx[idx - p.pitch]);
+  return O::e_new(a.cP[idx], a.cce[idx], p.nr, e, a.G[idx], hyn, hyn_l, hxn, hxn_d);
+}
+
+template <typename R>
+__global__ void __launch_bounds__(128) k1_2d(const P2<R> p, const Arrays<R> a) {
+  typedef Ops<R> O;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= p.nx) return;
+  const int j0 = blockIdx.y * kK1Rows, j1 = min(p.ny, j0 + kK1Rows);
+  const bool xe = (i == 0 || i == p.nx - 1);
+  for (int j = j0; j < j1; ++j) {
+    const int64_t idx = (int64_t)j * p.pitch + i;
+    const bool ye = (j == 0 || j == p.ny - 1);
+    R hxn, hyn;
+    R en = interior_e(p, a, i, j, hxn, hyn);
+    const R e = a.E[idx];
+    if (xe && ye) {
+      en = R(0);
+    } else if (xe || ye) {
+      if (p.bc == RKETD2D_BC_MUR) {
+        const int ii = xe ? (i == 0 ? 1 : p.nx - 2) : i, jj = ye ? (j == 0 ? 1 : p.ny - 2) : j;
+        R d1, d2;
+        const R en_in = interior_e(p, a, ii, jj, d1, d2);
+        en = O::mur(xe ? p.mx : p.my, a.E[(int64_t)jj * p.pitch + ii], en_in, e);
+      } else {
+        en = R(0);
+      }
+    }
+    if (i == p.src_i && j == p.src_j) en = Arith<R>::add(en, p.src[0]);
+    a.Hx2[idx] = hxn;
+    a.Hy2[idx] = hyn;
+    a.G2[idx] = O::g_new(a.cka[idx], a.cQ[idx], a.G[idx], e);
+    a.E2[idx] = en;
+    if (p.rowflag[j] & RF_PROBE)
+      for (int q = 0; q < p.nprobes; ++q)
+        if (p.probe_i[q] == i && p.probe_j[q] == j) p.rec[(int64_t)q * p.rec_stride + p.n0] = en;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ K2
+template <typename R>
+__device__ __forceinline__ void cp_async_val(R *smem_dst, const R *gsrc, bool valid) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
+  const int sz = valid ? (int)sizeof(R) : 0;          // 0 source bytes: the destination is zero-filled
+  asm volatile("cp.async.ca.shared.global [%0], [%1], %2, %3;\n" ::"r"(sa), "l"(gsrc), "n"((int)sizeof(R)), "r"(sz) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
+
+template <typename R>
+__device__ __forceinline__ R shfl_down1(R v) { return __shfl_down_sync(0xffffffffu, v, 1); }
+template <typename R>
+__device__ __forceinline__ R shfl_up1(R v) { return __shfl_up_sync(0xffffffffu, v, 1); }
+
+constexpr int kFieldRing = kPF + 1;
+template <typename R, int T>
+struct K2Shape {
+  static constexpr int CR = T + kPF + 1;            // coefficient ring: rows Y-T .. Y+kPF are alive at once
+  static constexpr size_t smem = sizeof(R) * ((size_t)kFieldRing * 4 * kNT + (size_t)CR * 4 * kNT + (size_t)2 * T * 3 * (kNT / 32));
+};
+
+// Streaming temporal blocking.  Job = (strip of kNT columns, halo HP (+ dlast) on each side) x (segment of Sy rows, T
+// halo rows on each side).  Iteration `it` lets row Y = ya + it enter; stage s (s = 0..T-1) then holds row Y-1-s at
+// level s (E, G at step n0+s, H half a step earlier) in registers, receives row Y-s at level s from stage s-1 (from
+// shared memory for s = 0), and produces level s+1 of its held row, which is what stage s+1 receives.  The last stage
+// writes row Y-T at level T to the other field buffer.  Per stage a thread keeps E, Hx, Hy, G of the held row, the new
+// Hx of the row before, and one spare value for the y edges; the four coefficients of a row wait in a shared-memory
+// ring (written once by cp.async, read by each stage in turn; every thread touches its own column only).  Between
+// lanes new Hy and old E travel by shuffle; between warps old E and old Hy of the warp-edge columns are posted to
+// shared memory at the end of an iteration (one CTA barrier per row).
+template <typename R, int T>
+__global__ void __launch_bounds__(kNT, 1) k2_2d(const P2<R> p, const Arrays<R> a) {
+  typedef Ops<R> O;
+  constexpr int NW = kNT / 32;
+  constexpr int CR = K2Shape<R, T>::CR;
+  constexpr int FR = kFieldRing;
+  extern __shared__ __align__(16) uint8_t smem_raw[];
+  R *fring = reinterpret_cast<R *>(smem_raw);                 // [FR][4][kNT]
+  R *cring = fring + FR * 4 * kNT;                            // [CR][4][kNT]
+  R *xch = cring + CR * 4 * kNT;                              // [2][T][3][NW]: E of lane 0, E of lane 31, Hy of lane 31
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const bool is_mur = (p.bc == RKETD2D_BC_MUR);
+
+  for (int q = tid; q < 2 * T * 3 * NW; q += kNT) xch[q] = R(0);
+  for (int q = 0; q < CR * 4; ++q) cring[q * kNT + tid] = R(0);
+
+  const int njobs = p.nstrips * p.nsegs;
+  for (int job = blockIdx.x; job < njobs; job += gridDim.x) {
+    const int strip = job % p.nstrips, seg = job / p.nstrips;
+    const int x0 = strip * p.Wv - p.HP - (strip == p.nstrips - 1 ? p.dlast : 0);
+    const int i = x0 + tid;
+    const bool incol = (i >= 0 && i < p.nx);
+    const bool own_col = incol && i >= strip * p.Wv && i < (strip + 1) * p.Wv;
+    const int y_out0 = seg * p.Sy, y_out1 = min(p.ny, y_out0 + p.Sy);
+    const int ya = y_out0 - T;
+    const int niter = (y_out1 - y_out0) + 2 * T;
+    const R chx_i = (i >= 0 && i <= p.nx - 2) ? p.chx : R(0);
+    const R chx_im1 = (i >= 1 && i <= p.nx - 1) ? p.chx : R(0);
+    const bool xl = (i == 0), xr = (i == p.nx - 1), xin = (i >= 1 && i <= p.nx - 2);
+    const bool xw = __any_sync(0xffffffffu, xl || xr);
+    const bool src_col = (i == p.src_i);
+
+    R e[T], hx[T], hy[T], g[T], hxp[T], xs[T];
+#pragma unroll
+    for (int s = 0; s < T; ++s) e[s] = hx[s] = hy[s] = g[s] = hxp[s] = xs[s] = R(0);
+    uint32_t fq = 0;
+
+    __syncthreads();                       // xch zeroed / the previous job is done with it
+
+    auto issue_row = [&](int ridx) {       // ridx = row index relative to ya
+      const int Y = ya + ridx;
+      const bool valid = incol && Y >= 0 && Y < p.ny && ridx < niter;
+      const int64_t idx = valid ? (int64_t)Y * p.pitch + i : 0;
+      R *fd = fring + (ridx % FR) * 4 * kNT + tid;
+      R *cd = cring + (ridx % CR) * 4 * kNT + tid;
+      cp_async_val(fd, a.E + idx, valid);
+      cp_async_val(fd + kNT, a.Hx + idx, valid);
+      cp_async_val(fd + 2 * kNT, a.Hy + idx, valid);
+      cp_async_val(fd + 3 * kNT, a.G + idx, valid);
+      cp_async_val(cd, a.cP + idx, valid);
+      cp_async_val(cd + kNT, a.cce + idx, valid);
+      cp_async_val(cd + 2 * kNT, a.cka + idx, valid);
+      cp_async_val(cd + 3 * kNT, a.cQ + idx, valid);
+      cp_async_commit();
+    };
+#pragma unroll
+    for (int r = 0; r < kPF; ++r) issue_row(r);
+
+    int cbase = 0;                         // it % CR
+    for (int it = 0; it < niter; ++it) {
+      const int Y = ya + it;
+      issue_row(it + kPF);
+      cp_async_wait<kPF>();
+      fq = (fq << 1) | ((Y >= 0 && Y < p.ny) ? (uint32_t)(p.rowflag[Y] & RF_SPECIAL) : 0u);
+      __syncthreads();                     // the warp-edge values posted at the end of the previous iteration
+      const R *fs = fring + (it % FR) * 4 * kNT + tid;
+      R ein = fs[0], hxin = fs[kNT], hyin = fs[2 * kNT], gin = fs[3 * kNT];
+      const R *xr_ = xch + ((it + 1) & 1) * (T * 3 * NW);      // read buffer of this iteration
+#pragma unroll
+      for (int s = 0; s < T; ++s) {
+        const int y = Y - 1 - s;
+        int slot = cbase - 1 - s;
+        if (slot < 0) slot += CR;
+        if (slot < 0) slot += CR;
+        const R *c = cring + slot * 4 * kNT + tid;
+        const R cP = c[0], cce = c[kNT], cka = c[2 * kNT], cQ = c[3 * kNT];
+        const R nchy_y = (y >= 0 && y <= p.ny - 2) ? p.nchy : R(0);
+        R e_rt = shfl_down1(e[s]);
+        if (lane == 31) e_rt = (warp + 1 < NW) ? xr_[(s * 3 + 0) * NW + warp + 1] : R(0);
+        const R hyn = O::hy_new(chx_i, e[s], e_rt, hy[s]);
+        R hyn_l = shfl_up1(hyn);
+        if (lane == 0)
+          hyn_l = (warp > 0) ? O::hy_new(chx_im1, xr_[(s * 3 + 1) * NW + warp - 1], e[s], xr_[(s * 3 + 2) * NW + warp - 1]) : R(0);
+        const R hxn = O::hx_new(nchy_y, e[s], ein, hx[s]);
+        R en = O::e_new(cP, cce, p.nr, e[s], g[s], hyn, hyn_l, hxn, hxp[s]);
+        const R gn = O::g_new(cka, cQ, g[s], e[s]);
+        R xs_new = e[s];
+        if (xw) {                          // this warp holds column 0 or nx-1: x edges of the rows 1..ny-2
+          const R en_rt = shfl_down1(en), en_lf = shfl_up1(en), e_lf = shfl_up1(e[s]);
+          if (y >= 1 && y <= p.ny - 2) {
+            if (xl) en = is_mur ? O::mur(p.mx, e_rt, en_rt, e[s]) : R(0);
+            if (xr) en = is_mur ? O::mur(p.mx, e_lf, en_lf, e[s]) : R(0);
+          }
+        }
+        if ((fq >> (s + 1)) & 1u) {        // rows 0, 1, ny-2, ny-1, the source row, rows with probes (CTA-uniform)
+          const bool own = own_col && y >= y_out0 && y < y_out1;
+          if (y == p.ny - 1) en = xs[s];   // computed one iteration ago from rows ny-2 (new) and ny-1 (old)
+          if (y == 0) en = R(0);           // set one iteration later, when E'[1] exists
+          if (y == p.ny - 2) xs_new = (xin && is_mur) ? O::mur(p.my, e[s], en, ein) : R(0);
+          if (y == 1) {                    // row 0 at level s+1: stage s+1 holds it by now (or it has been stored)
+            R e0 = (xin && is_mur) ? O::mur(p.my, e[s], en, xs[s]) : R(0);
+            if (p.src_j == 0 && src_col) e0 = Arith<R>::add(e0, p.src[s]);
+            if (own_col && y_out0 == 0 && (p.rowflag[0] & RF_PROBE))
+              for (int q = 0; q < p.nprobes; ++q)
+                if (p.probe_j[q] == 0 && p.probe_i[q] == i) p.rec[(int64_t)q * p.rec_stride + p.n0 + s] = e0;
+            if (s + 1 < T) {
+              e[s + 1 < T ? s + 1 : s] = e0;
+              R *xw_ = const_cast<R *>(xr_);
+              if (lane == 0) xw_[((s + 1) * 3 + 0) * NW + warp] = e0;
+              if (lane == 31) xw_[((s + 1) * 3 + 1) * NW + warp] = e0;
+              __syncthreads();
+            } else if (own_col && y_out0 == 0) {
+              a.E2[i] = e0;
+            }
+          }
+          if (y == p.src_j && src_col && y != 0) en = Arith<R>::add(en, p.src[s]);
+          if (own && y != 0 && (p.rowflag[y] & RF_PROBE))
+            for (int q = 0; q < p.nprobes; ++q)
+              if (p.probe_j[q] == y && p.probe_i[q] == i) p.rec[(int64_t)q * p.rec_stride + p.n0 + s] = en;
+        }
+        hxp[s] = hxn;
+        xs[s] = xs_new;
+        e[s] = ein; hx[s] = hxin; hy[s] = hyin; g[s] = gin;
+        ein = en; hxin = hxn; hyin = hyn; gin = gn;
+      }
+      {                                    // (ein, hxin, hyin, gin) is now row Y-T at level T
+        const int y = Y - T;
+        if (own_col && y >= y_out0 && y < y_out1) {
+          const int64_t idx = (int64_t)y * p.pitch + i;
+          a.E2[idx] = ein; a.Hx2[idx] = hxin; a.Hy2[idx] = hyin; a.G2[idx] = gin;
+        }
+      }
+      R *xp = xch + (it & 1) * (T * 3 * NW);                   // read in the next iteration
+      if (lane == 0) {
+#pragma unroll
+        for (int s = 0; s < T; ++s) xp[(s * 3 + 0) * NW + warp] = e[s];
+      }
+      if (lane == 31) {
+#pragma unroll
+        for (int s = 0; s < T; ++s) { xp[(s * 3 + 1) * NW + warp] = e[s]; xp[(s * 3 + 2) * NW + warp] = hy[s]; }
+      }
+      cbase = (cbase + 1 == CR) ? 0 : cbase + 1;
+    }
+    cp_async_wait<0>();
+    __syncthreads();
+    for (int q = tid; q < 2 * T * 3 * NW; q += kNT) xch[q] = R(0);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------ setup kernels
+// media -> pitch layout (fp64) + the four kernel coefficients; padding columns get zeros
+template <typename R>
+__global__ void coef2d_kernel(int nx, int ny, int64_t pitch, const double *__restrict__ wp, const double *__restrict__ nu,
+                              double dx, double dt, double eps0, double *wp_p, double *nu_p, R *cP, R *cce, R *cka, R *cQ,
+                              int *bad) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= pitch * ny) return;
+  const int64_t j = idx / pitch, i = idx - j * pitch;
+  double vP = 0, vce = 0, vka = 0, vQ = 0, w = 0, v = 0;
+  if (i < nx) {
+    w = wp[j * nx + i];
+    v = nu[j * nx + i];
+    if (!(w >= 0.0) || !(v >= 0.0) || isinf(w) || isinf(v)) atomicOr(bad, 1);
+    const rketd::Six s = rketd::six_coefficients(w, v, dx, dt, eps0, 0);
+    const double kcp = __dmul_rn(s.cj, s.kc), kbp = __dmul_rn(s.cj, s.kb);
+    vP = __dsub_rn(s.ca, kcp);
+    vce = s.ch;
+    vka = s.ka;
+    vQ = __dadd_rn(__dmul_rn(s.ka, kcp), kbp);
+  }
+  wp_p[idx] = w; nu_p[idx] = v;
+  cP[idx] = (R)vP; cce[idx] = (R)vce; cka[idx] = (R)vka; cQ[idx] = (R)vQ;
+}
+
+// G = cj J - cj kc E (in place on the array holding J), fp64 arithmetic, one rounding to R
+template <typename R>
+__global__ void j_to_g_kernel(int nx, int ny, int64_t pitch, const double *__restrict__ wp_p, const double *__restrict__ nu_p,
+                              double dx, double dt, double eps0, const R *__restrict__ E, R *JG) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= pitch * ny) return;
+  const int64_t i = idx % pitch;
+  double G = 0.0;
+  if (i < nx) {
+    const rketd::Six s = rketd::six_coefficients(wp_p[idx], nu_p[idx], dx, dt, eps0, 0);
+    G = __fma_rn(-__dmul_rn(s.cj, s.kc), (double)E[idx], __dmul_rn(s.cj, (double)JG[idx]));
+  }
+  JG[idx] = (R)G;
+}
+// J = (G + cj kc E)/cj
+template <typename R>
+__global__ void g_to_j_kernel(int nx, int ny, int64_t pitch, const double *__restrict__ wp_p, const double *__restrict__ nu_p,
+                              double dx, double dt, double eps0, const R *__restrict__ E, const R *__restrict__ G, R *J) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= pitch * ny) return;
+  const int64_t i = idx % pitch;
+  double v = 0.0;
+  if (i < nx) {
+    const rketd::Six s = rketd::six_coefficients(wp_p[idx], nu_p[idx], dx, dt, eps0, 0);
+    v = __ddiv_rn(__fma_rn(__dmul_rn(s.cj, s.kc), (double)E[idx], (double)G[idx]), s.cj);
+  }
+  J[idx] = (R)v;
+}
+template <typename R>
+__global__ void unpack2d_kernel(int nx, int ny, int64_t pitch, const R *c0, const R *c1, const R *c2, const R *c3, double *out) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t n = (int64_t)nx * ny;
+  if (idx >= n) return;
+  const int64_t j = idx / nx, i = idx - j * nx, src = j * pitch + i;
+  out[idx] = (double)c0[src]; out[n + idx] = (double)c1[src]; out[2 * n + idx] = (double)c2[src]; out[3 * n + idx] = (double)c3[src];
+}
+
+std::string g_create_error2;
+
+struct Chunk2 { void *buf; int64_t nsteps; };
+
+struct Plan2 { int HP, Wv, nstrips, nsegs, Sy, dlast; };
+
+}  // namespace
+
+struct rketd2d_sim {
+  int nx = 0, ny = 0, dtype = 0, esize = 8;
+  int64_t pitch = 0;
+  double dx = 0, dy = 0, dt = 0;
+  cudaStream_t stream = nullptr;
+  void *fld[2][4] = {{nullptr, nullptr, nullptr, nullptr}, {nullptr, nullptr, nullptr, nullptr}};   // E, Hx, Hy, G
+  int cur = 0;
+  void *coef[4] = {nullptr, nullptr, nullptr, nullptr};                                              // P, ce, ka, Q
+  double *wp_p = nullptr, *nu_p = nullptr;
+  uint8_t *rowflag = nullptr;
+  int *d_bad = nullptr;
+  bool flags_dirty = true, have_media = false, fields_zero = true, third_is_J = false;
+  int bc = RKETD2D_BC_MUR;
+  int src_kind = RKETD_SRC_NONE;
+  std::vector<double> src_params;
+  int src_i = -1, src_j = -1;
+  std::vector<int> probe_i, probe_j;
+  std::vector<Chunk2> chunks;
+  int64_t nsamples = 0, step = 0;
+  int plan_kernel = RKETD2D_KERNEL_AUTO, plan_depth = 0;
+  int num_sms = 148;
+  int64_t ctr_launches = 0, ctr_step_launches = 0, ctr_kernel_used = 0, ctr_depth_used = 0, ctr_strip = 0, ctr_halo = 0,
+          ctr_seg = 0, state_bytes = 0;
+  std::string err;
+};
+
+namespace {
+
+int fail2(rketd2d_sim *s, int code, const std::string &msg) {
+  if (s) s->err = msg; else g_create_error2 = msg;
+  return code;
+}
+#define CU_TRY2(s, expr)                                                                         \
+  do {                                                                                           \
+    cudaError_t e__ = (expr);                                                                    \
+    if (e__ != cudaSuccess)                                                                      \
+      return fail2(s, e__ == cudaErrorMemoryAllocation ? RKETD_ENOMEM : RKETD_ECUDA,             \
+                   std::string(#expr) + ": " + cudaGetErrorString(e__));                         \
+  } while (0)
+
+size_t arr_bytes2(const rketd2d_sim *s) { return (size_t)s->pitch * s->ny * s->esize; }
+unsigned blocks_for(int64_t n) { return (unsigned)((n + 255) / 256); }
+
+cudaError_t copy_in2(const rketd2d_sim *s, void *dst, const void *src, size_t es) {
+  return cudaMemcpy2DAsync(dst, (size_t)s->pitch * es, src, (size_t)s->nx * es, (size_t)s->nx * es, (size_t)s->ny,
+                           cudaMemcpyDefault, s->stream);
+}
+cudaError_t copy_out2(const rketd2d_sim *s, void *dst, const void *src, size_t es) {
+  return cudaMemcpy2DAsync(dst, (size_t)s->nx * es, src, (size_t)s->pitch * es, (size_t)s->nx * es, (size_t)s->ny,
+                           cudaMemcpyDefault, s->stream);
+}
+
+void discard_records2(rketd2d_sim *s) {
+  for (auto &c : s->chunks) cudaFree(c.buf);
+  s->chunks.clear();
+  s->nsamples = 0;
+}
+
+double source_sample2(const rketd2d_sim *s, int64_t step_index) {
+  if (s->src_kind == RKETD_SRC_GAUSS_DERIV) {
+    const double tau = s->src_params[0], t0 = s->src_params[1], A = s->src_params[2];
+    const double t = double(step_index + 1) * s->dt;
+    const double u = (t - t0) / tau;
+    return A * u * std::exp(0.5 - 0.5 * u * u);
+  }
+  if (s->src_kind == RKETD_SRC_TABLE)
+    return (step_index >= 0 && step_index < (int64_t)s->src_params.size()) ? s->src_params[(size_t)step_index] : 0.0;
+  return 0.0;
+}
+
+int build_rowflags(rketd2d_sim *s) {
+  std::vector<uint8_t> rf((size_t)s->ny, 0);
+  rf[0] |= RF_SPECIAL; rf[1] |= RF_SPECIAL; rf[(size_t)s->ny - 2] |= RF_SPECIAL; rf[(size_t)s->ny - 1] |= RF_SPECIAL;
+  if (s->src_kind != RKETD_SRC_NONE && s->src_j >= 0) {
+    rf[(size_t)s->src_j] |= RF_SPECIAL;
+    if (s->src_j == 0) rf[1] |= RF_SPECIAL;
+  }
+  for (size_t q = 0; q < s->probe_j.size(); ++q) rf[(size_t)s->probe_j[q]] |= RF_SPECIAL | RF_PROBE;
+  CU_TRY2(s, cudaMemcpyAsync(s->rowflag, rf.data(), rf.size(), cudaMemcpyHostToDevice, s->stream));
+  CU_TRY2(s, cudaStreamSynchronize(s->stream));      // rf is a local
+  s->flags_dirty = false;
+  return RKETD_OK;
+}
+
+// strips and segments of the streaming kernel for depth T
+Plan2 make_plan(const rketd2d_sim *s, int T) {
+  Plan2 pl;
+  pl.HP = std::max(8, (T + 7) / 8 * 8);
+  pl.Wv = kNT - 2 * pl.HP;
+  while ((s->nx % pl.Wv) == 1 && pl.Wv > 16) pl.Wv -= 8;      // the last strip owns at least two columns (x Mur)
+  pl.nstrips = (s->nx + pl.Wv - 1) / pl.Wv;
+  const int x0_last = (pl.nstrips - 1) * pl.Wv - pl.HP;
+  pl.dlast = (((s->nx - 1 - x0_last) % 32) == 0) ? 8 : 0;      // column nx-1 must not be lane 0 of its warp
+  // segments: fewest iterations per SM, whole waves; first and last segment own at least two rows
+  double best = 1e300;
+  pl.nsegs = 1; pl.Sy = s->ny;
+  const int max_segs = std::max(1, std::min(s->ny / 2, 4096));
+  for (int ns = 1; ns <= max_segs; ++ns) {
+    const int Sy = (s->ny + ns - 1) / ns;
+    const int nsr = (s->ny + Sy - 1) / Sy;
+    if (Sy < 2 || s->ny - (nsr - 1) * Sy < 2) continue;
+    const int64_t jobs = (int64_t)pl.nstrips * nsr;
+    const double cost = (double)((jobs + s->num_sms - 1) / s->num_sms) * (Sy + 2 * T + 8);
+    if (cost < best - 1e-9) { best = cost; pl.nsegs = nsr; pl.Sy = Sy; }
+  }
+  return pl;
+}
+
+template <typename R>
+void fill_params(const rketd2d_sim *s, P2<R> &p, void *rec, int64_t rec_stride, int64_t n0, int nlev) {
+  p.nx = s->nx; p.ny = s->ny; p.pitch = s->pitch;
+  p.chx = (R)(s->dt / (kMu0 * s->dx));
+  p.nchy = (R)(-(s->dt / (kMu0 * s->dy)));
+  p.nr = (R)(-(s->dx / s->dy));
+  const double Sx = kC0 * s->dt / s->dx, Sy = kC0 * s->dt / s->dy;
+  p.mx = (R)((Sx - 1.0) / (Sx + 1.0));
+  p.my = (R)((Sy - 1.0) / (Sy + 1.0));
+  p.bc = s->bc;
+  const bool has_src = s->src_kind != RKETD_SRC_NONE;
+  p.src_i = has_src ? s->src_i : -1;
+  p.src_j = has_src ? s->src_j : -1;
+  p.nprobes = (int)s->probe_i.size();
+  for (int q = 0; q < p.nprobes; ++q) { p.probe_i[q] = s->probe_i[(size_t)q]; p.probe_j[q] = s->probe_j[(size_t)q]; }
+  p.rec = (R *)rec; p.rec_stride = rec_stride; p.n0 = n0;
+  for (int l = 0; l < kMaxT; ++l) p.src[l] = (l < nlev && has_src) ? (R)source_sample2(s, s->step + l) : R(0);
+  p.rowflag = s->rowflag;
+  p.HP = p.Wv = p.nstrips = p.nsegs = p.Sy = p.dlast = 0;
+}
+
+template <typename R>
+Arrays<R> arrays_of(const rketd2d_sim *s) {
+  Arrays<R> a;
+  const int c = s->cur, d = 1 - s->cur;
+  a.E = (const R *)s->fld[c][0]; a.Hx = (const R *)s->fld[c][1]; a.Hy = (const R *)s->fld[c][2]; a.G = (const R *)s->fld[c][3];
+  a.cP = (const R *)s->coef[0]; a.cce = (const R *)s->coef[1]; a.cka = (const R *)s->coef[2]; a.cQ = (const R *)s->coef[3];
+  a.E2 = (R *)s->fld[d][0]; a.Hx2 = (R *)s->fld[d][1]; a.Hy2 = (R *)s->fld[d][2]; a.G2 = (R *)s->fld[d][3];
+  return a;
+}
+
+template <typename R, int T>
+cudaError_t launch_k2_T(rketd2d_sim *s, P2<R> &p) {
+  const Plan2 pl = make_plan(s, T);
+  p.HP = pl.HP; p.Wv = pl.Wv; p.nstrips = pl.nstrips; p.nsegs = pl.nsegs; p.Sy = pl.Sy; p.dlast = pl.dlast;
+  s->ctr_strip = kNT; s->ctr_halo = pl.HP; s->ctr_seg = pl.Sy;
+  constexpr size_t smem = K2Shape<R, T>::smem;
+  static bool configured = false;
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(k2_2d<R, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  const int grid = pl.nstrips * pl.nsegs;
+  k2_2d<R, T><<<grid, kNT, smem, s->stream>>>(p, arrays_of<R>(s));
+  return cudaGetLastError();
+}
+
+template <typename R>
+cudaError_t launch_k2(rketd2d_sim *s, P2<R> &p, int T) {
+  switch (T) {
+    case 1: return launch_k2_T<R, 1>(s, p);
+    case 2: return launch_k2_T<R, 2>(s, p);
+    case 4: return launch_k2_T<R, 4>(s, p);
+    case 8: return launch_k2_T<R, 8>(s, p);
+    case 16: return launch_k2_T<R, 16>(s, p);
+  }
+  return cudaErrorInvalidValue;
+}
+
+template <typename R>
+int run_typed(rketd2d_sim *s, int64_t nsteps, void *rec) {
+  const bool stream_kernel = s->plan_kernel != RKETD2D_KERNEL_STEP;
+  const int Tdef = s->plan_depth > 0 ? s->plan_depth : (s->dtype == RKETD_F64 ? 8 : 16);
+  s->ctr_kernel_used = stream_kernel ? RKETD2D_KERNEL_STREAM : RKETD2D_KERNEL_STEP;
+  s->ctr_depth_used = stream_kernel ? Tdef : 1;
+  int64_t done = 0;
+  while (done < nsteps) {
+    int T = 1;
+    if (stream_kernel) {
+      T = Tdef;
+      while ((int64_t)T > nsteps - done) T >>= 1;
+    }
+    P2<R> p;
+    fill_params<R>(s, p, rec, nsteps, done, T);
+    if (stream_kernel) {
+      CU_TRY2(s, launch_k2<R>(s, p, T));
+    } else {
+      dim3 grid((unsigned)((s->nx + 127) / 128), (unsigned)((s->ny + kK1Rows - 1) / kK1Rows));
+      k1_2d<R><<<grid, 128, 0, s->stream>>>(p, arrays_of<R>(s));
+      CU_TRY2(s, cudaGetLastError());
+    }
+    s->cur = 1 - s->cur;
+    s->step += T;
+    done += T;
+    s->ctr_launches++; s->ctr_step_launches++;
+  }
+  return RKETD_OK;
+}
+
+// the array holding G (or J before the first media) <-> J
+template <typename R>
+int convert_current(rketd2d_sim *s, bool to_G, void *dstJ) {
+  const int64_t n = s->pitch * s->ny;
+  if (to_G)
+    j_to_g_kernel<R><<<blocks_for(n), 256, 0, s->stream>>>(s->nx, s->ny, s->pitch, s->wp_p, s->nu_p, s->dx, s->dt, kEps0,
+                                                           (const R *)s->fld[s->cur][0], (R *)s->fld[s->cur][3]);
+  else
+    g_to_j_kernel<R><<<blocks_for(n), 256, 0, s->stream>>>(s->nx, s->ny, s->pitch, s->wp_p, s->nu_p, s->dx, s->dt, kEps0,
+                                                           (const R *)s->fld[s->cur][0], (const R *)s->fld[s->cur][3], (R *)dstJ);
+  CU_TRY2(s, cudaGetLastError());
+  s->ctr_launches++;
+  return RKETD_OK;
+}
+int convert_current_any(rketd2d_sim *s, bool to_G, void *dstJ) {
+  return s->dtype == RKETD_F64 ? convert_current<double>(s, to_G, dstJ) : convert_current<float>(s, to_G, dstJ);
+}
+
+}  // namespace
+
+extern "C" {
+
+int rketd2d_create(rketd2d_sim **out, int64_t nx, int64_t ny, double dx, double dy, double dt, int dtype, void *cuda_stream) {
+  if (!out) return fail2(nullptr, RKETD_EINVAL, "out is NULL");
+  *out = nullptr;
+  if (nx < 3 || ny < 3 || nx > (1 << 30) || ny > (1 << 30)) return fail2(nullptr, RKETD_EINVAL, "nx, ny must be in 3..2^30");
+  if (!(dx > 0) || !(dy > 0) || !(dt > 0)) return fail2(nullptr, RKETD_EINVAL, "dx, dy, dt must be positive");
+  if (kC0 * dt * std::sqrt(1.0 / (dx * dx) + 1.0 / (dy * dy)) > 1.0 + 1e-12)
+    return fail2(nullptr, RKETD_EINVAL, "c dt sqrt(1/dx^2 + 1/dy^2) > 1: unstable");
+  if (dtype != RKETD_F64 && dtype != RKETD_F32) return fail2(nullptr, RKETD_EINVAL, "unknown dtype");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+    cudaGetLastError();
+    return fail2(nullptr, RKETD_ECUDA, "no usable CUDA device; librketd has no CPU fallback");
+  }
+  rketd2d_sim *s = new rketd2d_sim();
+  s->nx = (int)nx; s->ny = (int)ny; s->dx = dx; s->dy = dy; s->dt = dt; s->dtype = dtype;
+  s->esize = dtype == RKETD_F64 ? 8 : 4;
+  s->pitch = (nx + 31) / 32 * 32;
+  s->stream = (cudaStream_t)cuda_stream;
+  int dev = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&s->num_sms, cudaDevAttrMultiProcessorCount, dev);
+  const size_t ab = arr_bytes2(s);
+  auto alloc = [&](void **p, size_t bytes) {
+    cudaError_t e = cudaMalloc(p, bytes);
+    if (e == cudaSuccess) { e = cudaMemsetAsync(*p, 0, bytes, s->stream); s->state_bytes += (int64_t)bytes; }
+    return e;
+  };
+  cudaError_t e = cudaSuccess;
+  for (int b = 0; b < 2 && e == cudaSuccess; ++b)
+    for (int f = 0; f < 4 && e == cudaSuccess; ++f) e = alloc(&s->fld[b][f], ab);
+  for (int c = 0; c < 4 && e == cudaSuccess; ++c) e = alloc(&s->coef[c], ab);
+  if (e == cudaSuccess) e = alloc((void **)&s->wp_p, (size_t)s->pitch * s->ny * 8);
+  if (e == cudaSuccess) e = alloc((void **)&s->nu_p, (size_t)s->pitch * s->ny * 8);
+  if (e == cudaSuccess) e = alloc((void **)&s->rowflag, (size_t)s->ny);
+  if (e == cudaSuccess) e = alloc((void **)&s->d_bad, sizeof(int));
+  if (e != cudaSuccess) {
+    const int code = e == cudaErrorMemoryAllocation ? RKETD_ENOMEM : RKETD_ECUDA;
+    const std::string msg = std::string("device allocation: ") + cudaGetErrorString(e);
+    cudaGetLastError();
+    rketd2d_destroy(s);
+    return fail2(nullptr, code, msg);
+  }
+  *out = s;
+  return RKETD_OK;
+}
+
+int rketd2d_set_media(rketd2d_sim *s, const double *wp, const double *nu) {
+  if (!s) return RKETD_EINVAL;
+  if (!wp || !nu) return fail2(s, RKETD_EINVAL, "wp and nu must not be NULL");
+  // live fields under the old media: back to J first
+  const bool live = s->have_media && !s->fields_zero;
+  if (live) { const int rc = convert_current_any(s, false, s->fld[s->cur][3]); if (rc) return rc; }
+  const int64_t n = s->pitch * s->ny, nu_n = (int64_t)s->nx * s->ny;
+  double *d_wp = nullptr, *d_nu = nullptr;      // user layout on the device
+  CU_TRY2(s, cudaMalloc((void **)&d_wp, (size_t)nu_n * 8));
+  cudaError_t e = cudaMalloc((void **)&d_nu, (size_t)nu_n * 8);
+  if (e != cudaSuccess) { cudaFree(d_wp); CU_TRY2(s, e); }
+  e = cudaMemcpyAsync(d_wp, wp, (size_t)nu_n * 8, cudaMemcpyDefault, s->stream);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(d_nu, nu, (size_t)nu_n * 8, cudaMemcpyDefault, s->stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(s->d_bad, 0, sizeof(int), s->stream);
+  if (e == cudaSuccess) {
+    if (s->dtype == RKETD_F64)
+      coef2d_kernel<double><<<blocks_for(n), 256, 0, s->stream>>>(s->nx, s->ny, s->pitch, d_wp, d_nu, s->dx, s->dt, kEps0, s->wp_p,
+                                                                  s->nu_p, (double *)s->coef[0], (double *)s->coef[1],
+                                                                  (double *)s->coef[2], (double *)s->coef[3], s->d_bad);
+    else
+      coef2d_kernel<float><<<blocks_for(n), 256, 0, s->stream>>>(s->nx, s->ny, s->pitch, d_wp, d_nu, s->dx, s->dt, kEps0, s->wp_p,
+                                                                 s->nu_p, (float *)s->coef[0], (float *)s->coef[1],
+                                                                 (float *)s->coef[2], (float *)s->coef[3], s->d_bad);
+    e = cudaGetLastError();
+    s->ctr_launches++;
+  }
+  int bad = 0;
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&bad, s->d_bad, sizeof(int), cudaMemcpyDeviceToHost, s->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+  cudaFree(d_wp); cudaFree(d_nu);
+  CU_TRY2(s, e);
+  if (bad) { s->have_media = false; return fail2(s, RKETD_EINVAL, "wp and nu must be finite and non-negative"); }
+  s->have_media = true;
+  if (live || s->third_is_J) { const int rc = convert_current_any(s, true, nullptr); if (rc) return rc; }
+  s->third_is_J = false;
+  CU_TRY2(s, cudaStreamSynchronize(s->stream));
+  return RKETD_OK;
+}
+
+int rketd2d_set_boundary(rketd2d_sim *s, int kind) {
+  if (!s) return RKETD_EINVAL;
+  if (kind != RKETD2D_BC_MUR && kind != RKETD2D_BC_PEC) return fail2(s, RKETD_EINVAL, "unknown boundary kind");
+  s->bc = kind;
+  return RKETD_OK;
+}
+
+int rketd2d_set_source(rketd2d_sim *s, int kind, const double *params, int64_t nparams, int64_t i, int64_t j) {
+  if (!s) return RKETD_EINVAL;
+  if (kind == RKETD_SRC_NONE) { s->src_kind = kind; s->src_i = s->src_j = -1; s->flags_dirty = true; return RKETD_OK; }
+  if (kind != RKETD_SRC_GAUSS_DERIV && kind != RKETD_SRC_TABLE) return fail2(s, RKETD_EINVAL, "unknown source kind");
+  if (i < 0 || i >= s->nx || j < 0 || j >= s->ny) return fail2(s, RKETD_EINVAL, "source node outside the grid");
+  if (kind == RKETD_SRC_GAUSS_DERIV && (nparams != 3 || !params || !(params[0] > 0)))
+    return fail2(s, RKETD_EINVAL, "GAUSS_DERIV needs params = {tau > 0, t0, amplitude}");
+  if (kind == RKETD_SRC_TABLE && (nparams < 0 || (nparams > 0 && !params))) return fail2(s, RKETD_EINVAL, "bad table");
+  s->src_kind = kind;
+  s->src_params.assign(params, params + nparams);
+  s->src_i = (int)i; s->src_j = (int)j;
+  s->flags_dirty = true;
+  return RKETD_OK;
+}
+
+int rketd2d_set_probes(rketd2d_sim *s, const int64_t *ij, int nprobes) {
+  if (!s) return RKETD_EINVAL;
+  if (nprobes < 0 || nprobes > kMaxProbes2 || (nprobes > 0 && !ij)) return fail2(s, RKETD_EINVAL, "0..64 probes");
+  for (int q = 0; q < nprobes; ++q)
+    if (ij[2 * q] < 0 || ij[2 * q] >= s->nx || ij[2 * q + 1] < 0 || ij[2 * q + 1] >= s->ny)
+      return fail2(s, RKETD_EINVAL, "probe node outside the grid");
+  CU_TRY2(s, cudaStreamSynchronize(s->stream));
+  discard_records2(s);
+  s->probe_i.clear(); s->probe_j.clear();
+  for (int q = 0; q < nprobes; ++q) { s->probe_i.push_back((int)ij[2 * q]); s->probe_j.push_back((int)ij[2 * q + 1]); }
+  s->flags_dirty = true;
+  return RKETD_OK;
+}
+
+int rketd2d_set_fields(rketd2d_sim *s, const void *Ez, const void *Hx, const void *Hy, const void *Jz) {
+  if (!s) return RKETD_EINVAL;
+  const void *src[4] = {Ez, Hx, Hy, Jz};
+  for (int f = 0; f < 4; ++f) {
+    if (src[f]) CU_TRY2(s, copy_in2(s, s->fld[s->cur][f], src[f], (size_t)s->esize));
+    else CU_TRY2(s, cudaMemsetAsync(s->fld[s->cur][f], 0, arr_bytes2(s), s->stream));
+  }
+  s->fields_zero = !Ez && !Hx && !Hy && !Jz;
+  if (s->have_media) { const int rc = convert_current_any(s, true, nullptr); if (rc) return rc; s->third_is_J = false; }
+  else s->third_is_J = true;
+  CU_TRY2(s, cudaStreamSynchronize(s->stream));
+  return RKETD_OK;
+}
+
+int rketd2d_get_fields(rketd2d_sim *s, void *Ez, void *Hx, void *Hy, void *Jz) {
+  if (!s) return RKETD_EINVAL;
+  void *dst[3] = {Ez, Hx, Hy};
+  for (int f = 0; f < 3; ++f)
+    if (dst[f]) CU_TRY2(s, copy_out2(s, dst[f], s->fld[s->cur][f], (size_t)s->esize));
+  if (Jz) {
+    const void *srcJ = s->fld[s->cur][3];
+    if (s->have_media && !s->third_is_J) {       // the other buffer's G array is scratch between runs
+      const int rc = convert_current_any(s, false, s->fld[1 - s->cur][3]);
+      if (rc) return rc;
+      srcJ = s->fld[1 - s->cur][3];
+    }
+    CU_TRY2(s, copy_out2(s, Jz, srcJ, (size_t)s->esize));
+  }
+  CU_TRY2(s, cudaStreamSynchronize(s->stream));
+  return RKETD_OK;
+}
+
+int rketd2d_reset(rketd2d_sim *s) {
+  if (!s) return RKETD_EINVAL;
+  CU_TRY2(s, cudaStreamSynchronize(s->stream));
+  for (int f = 0; f < 4; ++f) CU_TRY2(s, cudaMemsetAsync(s->fld[s->cur][f], 0, arr_bytes2(s), s->stream));
+  discard_records2(s);
+  s->step = 0;
+  s->fields_zero = true;
+  s->third_is_J = false;
+  return RKETD_OK;
+}
+
+int rketd2d_set_plan(rketd2d_sim *s, int kernel, int depth) {
+  if (!s) return RKETD_EINVAL;
+  if (kernel < RKETD2D_KERNEL_AUTO || kernel > RKETD2D_KERNEL_STREAM) return fail2(s, RKETD_EINVAL, "unknown kernel");
+  if (depth != 0 && depth != 1 && depth != 2 && depth != 4 && depth != 8 && depth != 16)
+    return fail2(s, RKETD_EINVAL, "depth must be 0, 1, 2, 4, 8 or 16");
+  s->plan_kernel = kernel;
+  s->plan_depth = depth;
+  return RKETD_OK;
+}
+
+int rketd2d_run(rketd2d_sim *s, int64_t nsteps) {
+  if (!s) return RKETD_EINVAL;
+  if (nsteps < 0) return fail2(s, RKETD_EINVAL, "nsteps < 0");
+  if (!s->have_media) return fail2(s, RKETD_ESTATE, "rketd2d_run before rketd2d_set_media");
+  if (nsteps == 0) return RKETD_OK;
+  if (s->flags_dirty) { const int rc = build_rowflags(s); if (rc) return rc; }
+  void *rec = nullptr;
+  if (!s->probe_i.empty()) {
+    CU_TRY2(s, cudaMalloc(&rec, (size_t)s->probe_i.size() * (size_t)nsteps * s->esize));
+    s->chunks.push_back({rec, nsteps});
+  }
+  s->fields_zero = false;
+  const int rc = s->dtype == RKETD_F64 ? run_typed<double>(s, nsteps, rec) : run_typed<float>(s, nsteps, rec);
+  if (rc) return rc;
+  s->nsamples += s->probe_i.empty() ? 0 : nsteps;
+  return RKETD_OK;
+}
+
+int rketd2d_read_probes(rketd2d_sim *s, void *out, int64_t out_bytes, int64_t *nsamples) {
+  if (!s) return RKETD_EINVAL;
+  CU_TRY2(s, cudaStreamSynchronize(s->stream));
+  if (nsamples) *nsamples = s->nsamples;
+  if (!out) return RKETD_OK;
+  const int64_t np = (int64_t)s->probe_i.size();
+  if (out_bytes < np * s->nsamples * s->esize) return fail2(s, RKETD_EINVAL, "out_bytes too small");
+  int64_t off = 0;
+  for (auto &c : s->chunks) {
+    CU_TRY2(s, cudaMemcpy2DAsync((char *)out + off * s->esize, (size_t)s->nsamples * s->esize, c.buf, (size_t)c.nsteps * s->esize,
+                                 (size_t)c.nsteps * s->esize, (size_t)np, cudaMemcpyDefault, s->stream));
+    off += c.nsteps;
+  }
+  CU_TRY2(s, cudaStreamSynchronize(s->stream));
+  return RKETD_OK;
+}
+
+int rketd2d_get_kernel_coefficients(rketd2d_sim *s, double *out, double *globals) {
+  if (!s) return RKETD_EINVAL;
+  if (!s->have_media) return fail2(s, RKETD_ESTATE, "no media yet");
+  if (globals) {
+    const double Sx = kC0 * s->dt / s->dx, Sy = kC0 * s->dt / s->dy;
+    globals[0] = s->dt / (kMu0 * s->dx); globals[1] = s->dt / (kMu0 * s->dy);
+    globals[2] = (Sx - 1.0) / (Sx + 1.0); globals[3] = (Sy - 1.0) / (Sy + 1.0);
+  }
+  if (!out) return RKETD_OK;
+  const int64_t n = (int64_t)s->nx * s->ny;
+  double *d = nullptr;
+  CU_TRY2(s, cudaMalloc((void **)&d, (size_t)n * 4 * 8));
+  if (s->dtype == RKETD_F64)
+    unpack2d_kernel<double><<<blocks_for(n), 256, 0, s->stream>>>(s->nx, s->ny, s->pitch, (double *)s->coef[0], (double *)s->coef[1],
+                                                                  (double *)s->coef[2], (double *)s->coef[3], d);
+  else
+    unpack2d_kernel<float><<<blocks_for(n), 256, 0, s->stream>>>(s->nx, s->ny, s->pitch, (float *)s->coef[0], (float *)s->coef[1],
+                                                                 (float *)s->coef[2], (float *)s->coef[3], d);
+  cudaError_t e = cudaGetLastError();
+  if (e == cudaSuccess) e = cudaMemcpyAsync(out, d, (size_t)n * 4 * 8, cudaMemcpyDefault, s->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+  cudaFree(d);
+  CU_TRY2(s, e);
+  s->ctr_launches++;
+  return RKETD_OK;
+}
+
+int64_t rketd2d_get_counter(const rketd2d_sim *s, int which) {
+  if (!s) return -1;
+  switch (which) {
+    case RKETD2D_CTR_LAUNCHES: return s->ctr_launches;
+    case RKETD2D_CTR_STEP_LAUNCHES: return s->ctr_step_launches;
+    case RKETD2D_CTR_KERNEL_USED: return s->ctr_kernel_used;
+    case RKETD2D_CTR_DEPTH_USED: return s->ctr_depth_used;
+    case RKETD2D_CTR_STEPS_DONE: return s->step;
+    case RKETD2D_CTR_STRIP_COLS: return s->ctr_strip;
+    case RKETD2D_CTR_HALO_COLS: return s->ctr_halo;
+    case RKETD2D_CTR_SEG_ROWS: return s->ctr_seg;
+    case RKETD2D_CTR_STATE_BYTES: return s->state_bytes;
+  }
+  return -1;
+}
+
+void rketd2d_destroy(rketd2d_sim *s) {
+  if (!s) return;
+  cudaStreamSynchronize(s->stream);
+  for (int b = 0; b < 2; ++b)
+    for (int f = 0; f < 4; ++f) cudaFree(s->fld[b][f]);
+  for (int c = 0; c < 4; ++c) cudaFree(s->coef[c]);
+  cudaFree(s->wp_p); cudaFree(s->nu_p); cudaFree(s->rowflag); cudaFree(s->d_bad);
+  for (auto &c : s->chunks) cudaFree(c.buf);
+  cudaGetLastError();
+  delete s;
+}
+
+const char *rketd2d_last_error(const rketd2d_sim *s) { return s ? s->err.c_str() : g_create_error2.c_str(); }
+
+}  // extern "C"

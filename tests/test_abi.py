@@ -92,3 +92,52 @@ def test_no_cpu_fallback_without_a_device(lib_path):
             "    print('OK')\n" % ROOT)
     out = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True)
     assert out.stdout.strip() == "OK", out.stdout + out.stderr
+
+
+# ---- the 2-D TMz entry points (include/rketd2d.h) ---------------------------------------------
+HEADER2D = os.path.join(ROOT, "include", "rketd2d.h")
+
+
+def declared_functions_2d():
+    src = re.sub(r"/\*.*?\*/", "", open(HEADER2D).read(), flags=re.S)
+    return sorted(set(re.findall(r"\b(rketd2d_[a-z_]+)\s*\(", src)))
+
+
+def test_library_exports_every_declared_2d_symbol(lib_path):
+    dll = ctypes.CDLL(lib_path)
+    names = declared_functions_2d()
+    assert "rketd2d_create" in names and "rketd2d_run" in names and "rketd2d_read_probes" in names
+    for n in names:
+        assert hasattr(dll, n), n
+    out = subprocess.run(["nm", "-D", "--defined-only", lib_path], capture_output=True, text=True, check=True).stdout
+    assert sorted(set(re.findall(r" T (rketd2d_[a-z_]+)$", out, flags=re.M))) == names
+
+
+def test_2d_binding_has_the_same_names(lib_path):
+    from paper_1709_00821_b200 import rketd2d
+    assert sorted(rketd2d.EXPORTS) == declared_functions_2d()
+    for n in rketd2d.EXPORTS:
+        assert callable(getattr(rketd2d, n)), n
+
+
+def test_2d_header_compiles_as_plain_c(tmp_path):
+    c = tmp_path / "t.c"
+    c.write_text('#include "rketd2d.h"\nint main(void) { rketd2d_sim *s = 0; (void)s; return RKETD2D_BC_MUR; }\n')
+    subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"), "-c", str(c),
+                    "-o", str(tmp_path / "t.o")], check=True)
+
+
+def test_2d_has_no_cpu_fallback_without_a_device(lib_path):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    code = ("import sys; sys.path.insert(0, %r)\n"
+            "from paper_1709_00821_b200 import rketd2d, rketd\n"
+            "try:\n"
+            "    rketd2d.Sim2D(100, 100, 75e-6, 75e-6, 1.25e-13)\n"
+            "except rketd.RketdError as e:\n"
+            "    assert e.code == rketd.ECUDA, e.code\n"
+            "    assert 'no CPU fallback' in str(e)\n"
+            "    print('OK')\n" % ROOT)
+    out = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True)
+    assert out.stdout.strip() == "OK", out.stdout + out.stderr

@@ -1,0 +1,266 @@
+"""GPU parity of the 2-D TMz path (include/rketd2d.h) against the CPU oracle (oracle2d_*), through
+the C ABI.  fp64: max |gpu - oracle| / max |oracle| <= 1e-12 over every probe sample and over the final fields;
+fp32: <= 1e-5.  The one-step kernel (K1) and the streaming kernel (K2, every depth) must agree bit for bit."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1709_00821_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"f64": 1e-12, "f32": 1e-5}
+C0 = 299792458.0
+DX = 75e-6
+DT = DX / (2 * C0)
+SRC = (20e-12, 80e-12, 1.0)
+
+
+def _mod():
+    from paper_1709_00821_b200 import rketd2d
+    return rketd2d
+
+
+def _gpu_run(w, dtype="f64", kernel=None, depth=0, nsteps=None, splits=None, fields=None):
+    m = _mod()
+    sim = m.Sim2D.from_workload(w, dtype)
+    if fields is not None:
+        sim.set_fields(*[None if f is None else np.ascontiguousarray(f, sim.np_dtype) for f in fields])
+    sim.set_plan(m.KERNEL_AUTO if kernel is None else kernel, depth)
+    n = w.nsteps if nsteps is None else nsteps
+    for part in (splits or [n]):
+        sim.run(part)
+    rec = sim.read_probes()
+    out = dict(rec=rec, fields=sim.get_fields(), launches=sim.counter(m.CTR_STEP_LAUNCHES),
+               kernel=sim.counter(m.CTR_KERNEL_USED))
+    sim.close()
+    return out
+
+
+def _oracle_run(w, nsteps=None, fields=None):
+    n = w.nsteps if nsteps is None else nsteps
+    wp, nu = w.media()
+    if fields is None:
+        st = oracle.State2D(w.nx, w.ny, Ez0=w.initial_E())
+    else:
+        st = oracle.State2D(w.nx, w.ny, *fields)
+    rec, _ = oracle.run2d(st, wp, nu, w.dx, w.dy, w.dt, n, src_kind=w.src_kind, src_params=w.src_params, src_ij=w.src_ij,
+                          probes=w.probes, boundary=w.boundary)
+    return dict(rec=rec, fields=(st.Ez, st.Hx, st.Hy, st.Jz))
+
+
+def _err(a, b):
+    s = np.max(np.abs(b))
+    return float(np.max(np.abs(np.asarray(a, np.float64) - b)) / s) if s > 0 else float(np.max(np.abs(a)))
+
+
+def _check(g, o, tol):
+    assert np.max(np.abs(o["rec"])) > 0
+    assert _err(g["rec"], o["rec"]) <= tol
+    for gf, of in zip(g["fields"], o["fields"]):
+        assert _err(gf, of) <= tol
+
+
+def _edge_workload(nx, ny, nsteps, boundary=wl.BC_MUR, dy_over_dx=1.0, src=None):
+    """tm2d_column with probes on every edge, next to every edge, in the corners, and on the source."""
+    w = wl.tm2d_column(nx, ny, nsteps, boundary=boundary, dy_over_dx=dy_over_dx, nprobes=24)
+    pts = {(0, 0), (nx - 1, 0), (0, ny - 1), (nx - 1, ny - 1), (0, ny // 2), (nx - 1, ny // 2), (nx // 2, 0), (nx // 2, ny - 1),
+           (1, 1), (nx - 2, ny - 2), (1, ny // 2), (nx // 2, 1), (nx // 2, ny // 2), (nx - 2, 1), (min(2, nx - 1), ny - 2)}
+    if src is not None:
+        w.src_ij = src
+    pts.add(tuple(w.src_ij))
+    w.probes = np.array(sorted(pts), np.int64)
+    return w
+
+
+# ----------------------------------------------------------------------------- K1 vs oracle, K2 == K1
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_reduced_column_all_kernels(dtype):
+    m = _mod()
+    w = _edge_workload(530, 310, 150)
+    o = _oracle_run(w)
+    k1 = _gpu_run(w, dtype, m.KERNEL_STEP)
+    assert k1["kernel"] == m.KERNEL_STEP and k1["launches"] == 150
+    _check(k1, o, TOL[dtype])
+    for T in (1, 2, 4, 8, 16):
+        k2 = _gpu_run(w, dtype, m.KERNEL_STREAM, T)
+        assert k2["kernel"] == m.KERNEL_STREAM
+        assert np.array_equal(k2["rec"], k1["rec"]), T
+        for a, b in zip(k2["fields"], k1["fields"]):
+            assert np.array_equal(a, b), T
+    auto = _gpu_run(w, dtype)
+    assert auto["kernel"] == m.KERNEL_STREAM and np.array_equal(auto["rec"], k1["rec"])
+
+
+# sizes: one node inside; strips whose last column falls on lane 0 (57, 249, 265: the shifted last strip); a last strip
+# of one column (241); several strips and segments; rows fewer than the depth
+@pytest.mark.parametrize("nx,ny", [(3, 3), (4, 3), (3, 7), (5, 4), (33, 17), (57, 40), (249, 33), (241, 9), (265, 70),
+                                   (481, 5), (700, 333), (64, 1200)])
+def test_ragged_sizes_mur(nx, ny):
+    m = _mod()
+    nsteps = 37
+    w = _edge_workload(nx, ny, nsteps, src=(nx // 2, ny // 2))
+    o = _oracle_run(w)
+    k1 = _gpu_run(w, "f64", m.KERNEL_STEP)
+    _check(k1, o, 1e-12)
+    for T in (8, 16, 2):
+        k2 = _gpu_run(w, "f64", m.KERNEL_STREAM, T)
+        assert np.array_equal(k2["rec"], k1["rec"]), (T, np.max(np.abs(k2["rec"] - k1["rec"])))
+        for a, b in zip(k2["fields"], k1["fields"]):
+            assert np.array_equal(a, b), T
+
+
+@pytest.mark.parametrize("src", ["edge_x0", "edge_y0", "edge_x1", "edge_y1", "next_to_x0", "next_to_y0", "next_to_y1"])
+@pytest.mark.parametrize("boundary", [wl.BC_MUR, wl.BC_PEC])
+def test_source_on_and_next_to_the_edges(src, boundary):
+    m = _mod()
+    nx, ny = 270, 90
+    pos = {"edge_x0": (0, 40), "edge_y0": (100, 0), "edge_x1": (nx - 1, 33), "edge_y1": (250, ny - 1),
+           "next_to_x0": (1, 50), "next_to_y0": (120, 1), "next_to_y1": (7, ny - 2)}[src]
+    w = _edge_workload(nx, ny, 45, boundary=boundary, dy_over_dx=1.3, src=pos)
+    w.src_kind, w.src_params = wl.SRC_TABLE, tuple(np.sin(0.3 * np.arange(45)) + 0.5)
+    o = _oracle_run(w)
+    k1 = _gpu_run(w, "f64", m.KERNEL_STEP)
+    _check(k1, o, 1e-12)
+    k2 = _gpu_run(w, "f64", m.KERNEL_STREAM, 8)
+    assert np.array_equal(k2["rec"], k1["rec"])
+    for a, b in zip(k2["fields"], k1["fields"]):
+        assert np.array_equal(a, b)
+
+
+def test_initial_fields_restart_and_anisotropic_steps():
+    m = _mod()
+    nx, ny = 300, 260
+    w = _edge_workload(nx, ny, 64, dy_over_dx=0.8)
+    rng = np.random.default_rng(3)
+    wp, _ = w.media()
+    f0 = (1e-3 * rng.uniform(-1, 1, (ny, nx)), 1e-6 * rng.uniform(-1, 1, (ny, nx)), 1e-6 * rng.uniform(-1, 1, (ny, nx)),
+          1e-2 * rng.uniform(-1, 1, (ny, nx)) * (wp > 0))
+    f0[1][-1, :] = 0.0                                       # padding row / column of Hx / Hy
+    f0[2][:, -1] = 0.0
+    o = _oracle_run(w, fields=f0)
+    g = _gpu_run(w, "f64", m.KERNEL_STREAM, 8, fields=f0, splits=[13, 1, 30, 20])
+    _check(g, o, 1e-12)
+    g1 = _gpu_run(w, "f64", m.KERNEL_STEP, fields=f0)
+    assert np.array_equal(g["rec"], g1["rec"])
+    g32 = _gpu_run(w, "f32", m.KERNEL_STREAM, 16, fields=f0)
+    _check(g32, o, 1e-5)
+
+
+def test_cavity_mode_on_the_gpu_follows_the_dispersion_recurrence():
+    """Pin Q3 through the CUDA path: conducting box, one eigenmode, dx != dy."""
+    m = _mod()
+    nx, ny, mm, nn, nsteps = 41, 31, 2, 3, 400
+    dx, dy, dt = DX, 1.3 * DX, 0.9 * DT
+    i = np.arange(nx)[None, :]; j = np.arange(ny)[:, None]
+    mode = np.sin(mm * math.pi * i / (nx - 1)) * np.sin(nn * math.pi * j / (ny - 1))
+    mode[0, :] = mode[-1, :] = 0.0; mode[:, 0] = mode[:, -1] = 0.0
+    L = 4.0 * ((C0 * dt / dx) ** 2 * math.sin(mm * math.pi / (2 * (nx - 1))) ** 2 +
+               (C0 * dt / dy) ** 2 * math.sin(nn * math.pi / (2 * (ny - 1))) ** 2)
+    a = [1.0, 1.0 - L]
+    for _ in range(nsteps - 1):
+        a.append((2.0 - L) * a[-1] - a[-2])
+    a = np.array(a)
+    sim = m.Sim2D(nx, ny, dx, dy, dt)
+    z = np.zeros((ny, nx))
+    sim.set_media(z, z)
+    sim.set_boundary(m.BC_PEC)
+    sim.set_fields(Ez=mode)
+    probes = [(7, 5), (20, 15), (33, 22), (12, 26)]
+    sim.set_probes(probes)
+    sim.run(nsteps)
+    rec = sim.read_probes()
+    for p, (pi, pj) in enumerate(probes):
+        assert np.max(np.abs(rec[p] - a[1:] * mode[pj, pi])) < 5e-12
+    assert np.max(np.abs(sim.get_fields()[0] - a[-1] * mode)) < 5e-12
+    sim.close()
+
+
+def test_kernel_coefficients_against_the_oracle_in_ulps():
+    m = _mod()
+    w = wl.tm2d_column(96, 80, 1, dy_over_dx=1.25)
+    sim = m.Sim2D.from_workload(w)
+    kc = sim.get_kernel_coefficients()
+    wp, nu = w.media()
+    c = oracle.coefficients2d(wp, nu, w.dx, w.dy, w.dt)
+    ref = {"P": c["ca"] - c["cj"] * c["kc"], "ce": c["cex"], "ka": c["ka"], "Q": c["ka"] * c["cj"] * c["kc"] + c["cj"] * c["kb"]}
+    for k, r in ref.items():
+        scale = np.max(np.abs(r))
+        assert np.max(np.abs(kc[k] - r)) <= 8 * np.finfo(np.float64).eps * scale, k
+    assert kc["chx"] == pytest.approx(c["chx"], rel=1e-15) and kc["chy"] == pytest.approx(c["chy"], rel=1e-15)
+    assert kc["mx"] == pytest.approx(c["mx"], rel=1e-15) and kc["my"] == pytest.approx(c["my"], rel=1e-15)
+    assert np.max(np.abs(c["cey"] - c["cex"] * (w.dx / w.dy))) <= 4 * np.finfo(np.float64).eps * np.max(c["cey"])
+    sim.close()
+
+
+def test_error_codes_2d():
+    m = _mod()
+    from paper_1709_00821_b200.rketd import RketdError, EINVAL, ESTATE
+    with pytest.raises(RketdError) as e:
+        m.Sim2D(2, 10, DX, DX, DT)
+    assert e.value.code == EINVAL
+    with pytest.raises(RketdError) as e:
+        m.Sim2D(10, 10, DX, DX, 1.5 * DT)                    # c dt sqrt(2)/dx = 1.06
+    assert e.value.code == EINVAL
+    sim = m.Sim2D(10, 12, DX, DX, DT)
+    with pytest.raises(RketdError) as e:
+        sim.run(1)
+    assert e.value.code == ESTATE
+    for bad in ([(10, 0)], [(0, 12)], [(-1, 3)]):
+        with pytest.raises(RketdError) as e:
+            sim.set_probes(bad)
+        assert e.value.code == EINVAL
+    with pytest.raises(RketdError) as e:
+        sim.set_source(0, SRC, 3, 12)
+    assert e.value.code == EINVAL
+    with pytest.raises(RketdError) as e:
+        sim.set_plan(m.KERNEL_STREAM, 3)
+    assert e.value.code == EINVAL
+    wp = np.zeros((12, 10)); nu = np.zeros((12, 10)); wp[3, 3] = -1.0
+    with pytest.raises(RketdError) as e:
+        sim.set_media(wp, nu)
+    assert e.value.code == EINVAL
+    sim.close()
+
+
+# ----------------------------------------------------------------------------- the size bench.py times
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_full_size_sampled_against_windowed_oracle(dtype):
+    """16384 x 16384 nodes, the launch configuration bench.py times (streaming kernel, default depth); every probe is
+    compared with an oracle run on the window of nodes that can influence it (pin Q7: bit-exact domain of dependence)."""
+    import torch
+    m = _mod()
+    nsteps = 200
+    w = wl.tm2d_column(nsteps=nsteps, nprobes=20)
+    sim = m.Sim2D(w.nx, w.ny, w.dx, w.dy, w.dt, dtype)
+    wp, nu = w.media()
+    sim.set_media(wp, nu)
+    del wp, nu
+    sim.set_fields(Ez=np.ascontiguousarray(w.initial_E(), sim.np_dtype))
+    sim.set_source(w.src_kind, w.src_params, *w.src_ij)
+    sim.set_probes(w.probes)
+    sim.run(nsteps)
+    rec = sim.read_probes().astype(np.float64)
+    assert sim.counter(m.CTR_KERNEL_USED) == m.KERNEL_STREAM
+    assert sim.counter(m.CTR_DEPTH_USED) == (8 if dtype == "f64" else 16)
+    sim.close()
+    torch.cuda.empty_cache()
+    peak = 0.0
+    worst = 0.0
+    r = nsteps + 1
+    refs = []
+    for q, (pi, pj) in enumerate(w.probes):
+        win = (max(0, pi - r), min(w.nx, pi + r + 1), max(0, pj - r), min(w.ny, pj + r + 1))
+        o = oracle.run_workload2d(w, window=win, omp=True)
+        k = [tuple(p) for p in o["probe_ij"]].index((int(pi), int(pj)))
+        refs.append(o["rec"][k])
+        peak = max(peak, np.max(np.abs(o["rec"][k])))
+    for q in range(len(w.probes)):
+        worst = max(worst, np.max(np.abs(rec[q] - refs[q])))
+        # relative to the probe's own peak: the bound K n u of DESIGN.md §5 with the 2-D operation count
+        u = 2.0 ** -53 if dtype == "f64" else 2.0 ** -24
+        assert np.max(np.abs(rec[q] - refs[q])) <= 40 * nsteps * u * max(np.max(np.abs(refs[q])), 1e-3)
+    assert peak > 0.01
+    assert worst / peak <= TOL[dtype]
