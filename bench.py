@@ -29,6 +29,7 @@ from __future__ import annotations
 
 import argparse
 import json
+import math
 import os
 import subprocess
 import sys
@@ -298,6 +299,176 @@ def run_table2(args):
                               "Mur-1 ends here, 5-cell PML there"}), flush=True)
 
 
+
+# ---------------------------------------------------------------------------------------------------------------------
+# 2-D TMz workload: `--workload tm2d` (16384 x 16384 x 1000 steps) or tm2d:<nx>:<ny>:<nsteps>
+# ---------------------------------------------------------------------------------------------------------------------
+FP_INSTR_PER_CELL_STEP_2D = 11   # rketd2d.cu: Hx 2, Hy 2, Ez 5, G 2
+ARRAYS_PER_PASS_2D = 12          # read Ez, Hx, Hy, G, P, ce, ka, Q; write Ez, Hx, Hy, G
+NCU_TRAFFIC_BYTES_2D = {}        # (workload, dtype, depth) -> dram bytes per launch from the committed ncu capture
+
+
+def cpu_baseline_2d(w, target_serial=4e8, target_omp=2.0e9):
+    import oracle
+    oracle.build()
+    cores = os.cpu_count() or 1
+    out = {}
+    steps = min(w.nsteps, 200)
+    for omp, target in ((False, target_serial), (True, target_omp)):
+        side = int(min(min(w.nx, w.ny), max(64, math.isqrt(int(target // steps)))))
+        i0 = min(max(0, w.src_ij[0] - side // 2), w.nx - side)
+        j0 = min(max(0, w.src_ij[1] - side // 2), w.ny - side)
+        t0 = time.perf_counter()
+        oracle.run_workload2d(w, nsteps=steps, window=(i0, i0 + side, j0, j0 + side), omp=omp)
+        dt = time.perf_counter() - t0
+        out[omp] = (side * side * steps / dt / 1e9,
+                    f"nodes {i0}..{i0 + side - 1} x {j0}..{j0 + side - 1} of the {w.nx} x {w.ny} grid x {steps} steps", dt)
+    return {"value": out[True][0], "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": out[True][1] + f" (OpenMP build, {cores} threads, {out[True][2]:.1f} s)",
+            "serial_value": out[False][0],
+            "serial_sample": out[False][1] + f" (serial build, 1 thread, {out[False][2]:.1f} s)"}
+
+
+def make_workload_2d(name: str):
+    from paper_1709_00821_b200 import workloads as wl
+    f = name.split(":")
+    if len(f) == 1:
+        return wl.tm2d_column()
+    return wl.tm2d_column(nx=int(f[1]), ny=int(f[2]), nsteps=int(f[3]))
+
+
+def run_tm2d(args):
+    import torch
+    import torch.distributed as dist
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: librketd has no CPU fallback")
+    from paper_1709_00821_b200 import build as lib_build
+    if int(os.environ.get("LOCAL_RANK", "0")) == 0:
+        lib_build.build_library()
+    else:
+        t_wait = time.time()
+        while lib_build._stale() and time.time() - t_wait < 900:
+            time.sleep(1.0)
+    from paper_1709_00821_b200 import rketd2d
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    w = make_workload_2d(args.workload)
+    esize = 8 if args.dtype == "f64" else 4
+    npdt = np.float64 if args.dtype == "f64" else np.float32
+    stream = torch.cuda.current_stream()
+    wp, nu = w.media()
+    E0 = np.ascontiguousarray(w.initial_E(), npdt)
+    sim = rketd2d.Sim2D(w.nx, w.ny, w.dx, w.dy, w.dt, args.dtype, stream=stream.cuda_stream)
+    wp_d, nu_d = torch.from_numpy(wp).cuda(), torch.from_numpy(nu).cuda()
+    sim.set_media(wp_d, nu_d)
+    del wp_d, nu_d
+    torch.cuda.empty_cache()
+    E0_d = torch.from_numpy(E0).cuda()
+    sim.set_fields(Ez=E0_d)
+    del E0_d
+    sim.set_boundary(w.boundary)
+    sim.set_source(w.src_kind, w.src_params, *w.src_ij)
+    sim.set_probes(w.probes)
+    sim.set_plan(args.kernel, args.depth)
+    units_per_step = w.nx * w.ny * w.nsteps
+    rec_d = torch.empty((len(w.probes), w.nsteps), dtype=torch.float64 if args.dtype == "f64" else torch.float32, device="cuda")
+
+    def one_step():
+        sim.run(w.nsteps)
+        sim.set_probes(w.probes)               # drops the records of this run (the run itself is what is timed)
+
+    for _ in range(args.warmup):
+        one_step()
+    barrier()
+    l0, sl0 = sim.counter(rketd2d.CTR_LAUNCHES), sim.counter(rketd2d.CTR_STEP_LAUNCHES)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as clk:
+        ev0.record(stream)
+        for _ in range(args.steps):
+            sim.run(w.nsteps)
+        ev1.record(stream)
+        barrier()
+    sim.set_probes(w.probes)
+    ms = max_over_ranks(ev0.elapsed_time(ev1), world)
+    launches = sim.counter(rketd2d.CTR_LAUNCHES) - l0
+    step_launches = sim.counter(rketd2d.CTR_STEP_LAUNCHES) - sl0
+    kernel_used, depth = sim.counter(rketd2d.CTR_KERNEL_USED), sim.counter(rketd2d.CTR_DEPTH_USED)
+    strip, halo, seg = (sim.counter(c) for c in (rketd2d.CTR_STRIP_COLS, rketd2d.CTR_HALO_COLS, rketd2d.CTR_SEG_ROWS))
+    value = whole_job_gcells(world, units_per_step, args.steps, ms * 1e-3)
+    hbm_gbs, peak_src, sm_max = measured_peaks()
+    nodes = w.nx * w.ny
+    ms_per_launch = ms / max(1, step_launches)
+    lanes = FP64_LANES_PER_SM if args.dtype == "f64" else FP32_LANES_PER_SM
+    r_alu = 148 * lanes * (sm_max * 1e6) / FP_INSTR_PER_CELL_STEP_2D / 1e9
+    r_hbm1 = hbm_gbs / (ARRAYS_PER_PASS_2D * esize)
+    alg_bytes = ARRAYS_PER_PASS_2D * esize * nodes
+    achieved = alg_bytes / (ms_per_launch * 1e-3) / 1e9
+    redundancy = 1.0
+    if kernel_used == rketd2d.KERNEL_STREAM and strip > 0:
+        redundancy = (strip / max(1, strip - 2 * halo)) * ((seg + 2 * depth) / max(1, seg))
+    roof = {"bound": "hbm", "achieved": achieved, "peak": hbm_gbs, "unit": "GB/s", "frac": achieved / hbm_gbs,
+            "traffic": NCU_TRAFFIC_BYTES_2D.get((w.name, args.dtype, int(depth))), "peak_source": peak_src,
+            "algorithmic_bytes_per_launch": alg_bytes, "ms_per_launch": ms_per_launch, "depth_T": int(depth),
+            "strip_cols": int(strip), "halo_cols": int(halo), "segment_rows": int(seg),
+            "frac_vs_8TBps_nominal": achieved / 8000.0, "gcells_vs_one_step_hbm_roofline": value / world / r_hbm1,
+            "alu_frac": (value / world) * redundancy / r_alu,
+            "note": "achieved = 12 arrays (read Ez,Hx,Hy,G,P,ce,ka,Q; write Ez,Hx,Hy,G) x nodes x esize per pass / mean "
+                    "launch time; every byte serves depth_T steps; alu_frac counts the redundant halo work against "
+                    "148 SMs x lanes x max clock / 11 instr per cell-step"}
+    e2e = None
+    if not args.no_e2e:
+        wp_h, nu_h = torch.from_numpy(wp).pin_memory(), torch.from_numpy(nu).pin_memory()
+        E0_h = torch.from_numpy(E0).pin_memory()
+        out_h = torch.empty((len(w.probes), w.nsteps), dtype=rec_d.dtype).pin_memory()
+        h2d = wp_h.numel() * 8 + nu_h.numel() * 8 + E0_h.numel() * esize
+        d2h = out_h.numel() * esize
+
+        def e2e_step():
+            sim.reset()
+            sim.set_media(wp_h, nu_h)
+            sim.set_fields(Ez=E0_h)
+            sim.run(w.nsteps)
+            sim.read_probes(out_h)
+
+        e2e_step()
+        barrier()
+        t0 = time.perf_counter()
+        nrep = max(1, min(args.steps, 2))
+        for _ in range(nrep):
+            e2e_step()
+        barrier()
+        dt = max_over_ranks(time.perf_counter() - t0, world)
+        e2e = {"value": whole_job_gcells(world, units_per_step, nrep, dt), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(d2h), "steps": nrep,
+               "note": "rketd2d_set_media(wp, nu) + set_fields(Ez0) from pinned host, rketd2d_run, read_probes to pinned host"}
+        del wp_h, nu_h, E0_h, out_h
+    sim.close()
+    cpu = cpu_baseline_2d(w) if (rank == 0 and world == 1 and not args.no_cpu) else None
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": args.dtype, "data": "synthetic",
+                "config": {"workload": w.name, "nx": w.nx, "ny": w.ny, "nsteps_per_run": w.nsteps,
+                           "cell_updates_per_step": units_per_step, "kernel": int(kernel_used), "depth_T": int(depth),
+                           "l2": "inputs larger than L2 (state+coefficients %.1f GB)" % (alg_bytes / 1e9),
+                           "parallelism": "replicas only (the path does not shard)" if world > 1 else "single GPU"},
+                "clocks": clk.summary(), "roofline": roof, "e2e": e2e, "cpu_baseline": cpu,
+                "gpu_launches": int(launches), "stencil_launches": int(step_launches)}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -317,6 +488,8 @@ def main():
         return run_table2(args)
     if args.impl == "reference":
         return run_reference(args)
+    if args.workload.startswith("tm2d"):
+        return run_tm2d(args)
 
     import torch
     import torch.distributed as dist

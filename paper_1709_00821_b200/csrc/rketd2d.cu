@@ -160,6 +160,84 @@ struct K2Shape {
   static constexpr size_t smem = sizeof(R) * ((size_t)kFieldRing * 4 * kNT + (size_t)CR * 4 * kNT + (size_t)2 * T * 3 * (kNT / 32));
 };
 
+// Per-thread constants of a job of the streaming kernel.
+template <typename R>
+struct JobCtx {
+  int i, lane, warp, y_out0, y_out1;
+  bool own_col, xl, xr, xin, src_col, is_mur;
+  R chx_i, chx_im1;
+};
+
+// The T pipeline stages of one iteration (row Y has just entered as (ein, hxin, hyin, gin)).
+//   SPECIAL = false: none of the rows held by the stages is row 0, 1, ny-2, ny-1, the source row or a probe row —
+//                    straight-line code, the stages' independent parts overlap freely;
+//   XEDGE:           this warp holds column 0 or nx-1 (first-order Mur / conductor on the x edges).
+template <typename R, int T, bool SPECIAL, bool XEDGE>
+__device__ __forceinline__ void run_stages(const P2<R> &p, const Arrays<R> &a, const JobCtx<R> &c, const int Y, const uint32_t fq,
+                                           const int cbase, const R *cring, R *xbuf, R (&e)[T], R (&hx)[T], R (&hy)[T],
+                                           R (&g)[T], R (&hxp)[T], R (&xs)[T], R &ein, R &hxin, R &hyin, R &gin) {
+  typedef Ops<R> O;
+  constexpr int NW = kNT / 32;
+  constexpr int CR = K2Shape<R, T>::CR;
+  const int tid = c.warp * 32 + c.lane;
+#pragma unroll
+  for (int s = 0; s < T; ++s) {
+    const int y = Y - 1 - s;
+    int slot = cbase - 1 - s;
+    if (slot < 0) slot += CR;
+    const R *cf = cring + slot * 4 * kNT + tid;
+    const R cP = cf[0], cce = cf[kNT], cka = cf[2 * kNT], cQ = cf[3 * kNT];
+    // rows outside the grid hold zeros, so -chy is right for them too; only row ny-1 (a special row) needs 0
+    const R nchy_y = SPECIAL ? ((y >= 0 && y <= p.ny - 2) ? p.nchy : R(0)) : p.nchy;
+    R e_rt = shfl_down1(e[s]);
+    if (c.lane == 31) e_rt = (c.warp + 1 < NW) ? xbuf[(s * 3 + 0) * NW + c.warp + 1] : R(0);
+    const R hyn = O::hy_new(c.chx_i, e[s], e_rt, hy[s]);
+    R hyn_l = shfl_up1(hyn);
+    if (c.lane == 0)
+      hyn_l = (c.warp > 0) ? O::hy_new(c.chx_im1, xbuf[(s * 3 + 1) * NW + c.warp - 1], e[s], xbuf[(s * 3 + 2) * NW + c.warp - 1]) : R(0);
+    const R hxn = O::hx_new(nchy_y, e[s], ein, hx[s]);
+    R en = O::e_new(cP, cce, p.nr, e[s], g[s], hyn, hyn_l, hxn, hxp[s]);
+    const R gn = O::g_new(cka, cQ, g[s], e[s]);
+    R xs_new = e[s];
+    if (XEDGE) {                         // x edges of the rows 1..ny-2
+      const R en_rt = shfl_down1(en), en_lf = shfl_up1(en), e_lf = shfl_up1(e[s]);
+      if (y >= 1 && y <= p.ny - 2) {
+        if (c.xl) en = c.is_mur ? O::mur(p.mx, e_rt, en_rt, e[s]) : R(0);
+        if (c.xr) en = c.is_mur ? O::mur(p.mx, e_lf, en_lf, e[s]) : R(0);
+      }
+    }
+    if (SPECIAL && ((fq >> (s + 1)) & 1u)) {       // CTA-uniform
+      const bool own = c.own_col && y >= c.y_out0 && y < c.y_out1;
+      if (y == p.ny - 1) en = xs[s];     // computed one iteration ago from rows ny-2 (new) and ny-1 (old)
+      if (y == 0) en = R(0);             // set one iteration later, when E'[1] exists
+      if (y == p.ny - 2) xs_new = (c.xin && c.is_mur) ? O::mur(p.my, e[s], en, ein) : R(0);
+      if (y == 1) {                      // row 0 at level s+1: stage s+1 holds it by now (or it has been stored)
+        R e0 = (c.xin && c.is_mur) ? O::mur(p.my, e[s], en, xs[s]) : R(0);
+        if (p.src_j == 0 && c.src_col) e0 = Arith<R>::add(e0, p.src[s]);
+        if (c.own_col && c.y_out0 == 0 && (p.rowflag[0] & RF_PROBE))
+          for (int q = 0; q < p.nprobes; ++q)
+            if (p.probe_j[q] == 0 && p.probe_i[q] == c.i) p.rec[(int64_t)q * p.rec_stride + p.n0 + s] = e0;
+        if (s + 1 < T) {
+          e[s + 1 < T ? s + 1 : s] = e0;
+          if (c.lane == 0) xbuf[((s + 1) * 3 + 0) * NW + c.warp] = e0;
+          if (c.lane == 31) xbuf[((s + 1) * 3 + 1) * NW + c.warp] = e0;
+          __syncthreads();
+        } else if (c.own_col && c.y_out0 == 0) {
+          a.E2[c.i] = e0;
+        }
+      }
+      if (y == p.src_j && c.src_col && y != 0) en = Arith<R>::add(en, p.src[s]);
+      if (own && y != 0 && (p.rowflag[y] & RF_PROBE))
+        for (int q = 0; q < p.nprobes; ++q)
+          if (p.probe_j[q] == y && p.probe_i[q] == c.i) p.rec[(int64_t)q * p.rec_stride + p.n0 + s] = en;
+    }
+    hxp[s] = hxn;
+    xs[s] = xs_new;
+    e[s] = ein; hx[s] = hxin; hy[s] = hyin; g[s] = gin;
+    ein = en; hxin = hxn; hyin = hyn; gin = gn;
+  }
+}
+
 // Streaming temporal blocking.  Job = (strip of kNT columns, halo HP (+ dlast) on each side) x (segment of Sy rows, T
 // halo rows on each side).  Iteration `it` lets row Y = ya + it enter; stage s (s = 0..T-1) then holds row Y-1-s at
 // level s (E, G at step n0+s, H half a step earlier) in registers, receives row Y-s at level s from stage s-1 (from
@@ -171,7 +249,6 @@ struct K2Shape {
 // shared memory at the end of an iteration (one CTA barrier per row).
 template <typename R, int T>
 __global__ void __launch_bounds__(kNT, 1) k2_2d(const P2<R> p, const Arrays<R> a) {
-  typedef Ops<R> O;
   constexpr int NW = kNT / 32;
   constexpr int CR = K2Shape<R, T>::CR;
   constexpr int FR = kFieldRing;
@@ -179,8 +256,10 @@ __global__ void __launch_bounds__(kNT, 1) k2_2d(const P2<R> p, const Arrays<R> a
   R *fring = reinterpret_cast<R *>(smem_raw);                 // [FR][4][kNT]
   R *cring = fring + FR * 4 * kNT;                            // [CR][4][kNT]
   R *xch = cring + CR * 4 * kNT;                              // [2][T][3][NW]: E of lane 0, E of lane 31, Hy of lane 31
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const bool is_mur = (p.bc == RKETD2D_BC_MUR);
+  const int tid = threadIdx.x;
+  JobCtx<R> c;
+  c.lane = tid & 31; c.warp = tid >> 5;
+  c.is_mur = (p.bc == RKETD2D_BC_MUR);
 
   for (int q = tid; q < 2 * T * 3 * NW; q += kNT) xch[q] = R(0);
   for (int q = 0; q < CR * 4; ++q) cring[q * kNT + tid] = R(0);
@@ -190,16 +269,17 @@ __global__ void __launch_bounds__(kNT, 1) k2_2d(const P2<R> p, const Arrays<R> a
     const int strip = job % p.nstrips, seg = job / p.nstrips;
     const int x0 = strip * p.Wv - p.HP - (strip == p.nstrips - 1 ? p.dlast : 0);
     const int i = x0 + tid;
+    c.i = i;
     const bool incol = (i >= 0 && i < p.nx);
-    const bool own_col = incol && i >= strip * p.Wv && i < (strip + 1) * p.Wv;
-    const int y_out0 = seg * p.Sy, y_out1 = min(p.ny, y_out0 + p.Sy);
-    const int ya = y_out0 - T;
-    const int niter = (y_out1 - y_out0) + 2 * T;
-    const R chx_i = (i >= 0 && i <= p.nx - 2) ? p.chx : R(0);
-    const R chx_im1 = (i >= 1 && i <= p.nx - 1) ? p.chx : R(0);
-    const bool xl = (i == 0), xr = (i == p.nx - 1), xin = (i >= 1 && i <= p.nx - 2);
-    const bool xw = __any_sync(0xffffffffu, xl || xr);
-    const bool src_col = (i == p.src_i);
+    c.own_col = incol && i >= strip * p.Wv && i < (strip + 1) * p.Wv;
+    c.y_out0 = seg * p.Sy; c.y_out1 = min(p.ny, c.y_out0 + p.Sy);
+    const int ya = c.y_out0 - T;
+    const int niter = (c.y_out1 - c.y_out0) + 2 * T;
+    c.chx_i = (i >= 0 && i <= p.nx - 2) ? p.chx : R(0);
+    c.chx_im1 = (i >= 1 && i <= p.nx - 1) ? p.chx : R(0);
+    c.xl = (i == 0); c.xr = (i == p.nx - 1); c.xin = (i >= 1 && i <= p.nx - 2);
+    const bool xw = __any_sync(0xffffffffu, c.xl || c.xr);
+    c.src_col = (i == p.src_i);
 
     R e[T], hx[T], hy[T], g[T], hxp[T], xs[T];
 #pragma unroll
@@ -227,6 +307,7 @@ __global__ void __launch_bounds__(kNT, 1) k2_2d(const P2<R> p, const Arrays<R> a
 #pragma unroll
     for (int r = 0; r < kPF; ++r) issue_row(r);
 
+    constexpr uint32_t kHeldMask = ((1u << T) - 1u) << 1;     // bits of the rows the T stages hold
     int cbase = 0;                         // it % CR
     for (int it = 0; it < niter; ++it) {
       const int Y = ya + it;
@@ -236,79 +317,28 @@ __global__ void __launch_bounds__(kNT, 1) k2_2d(const P2<R> p, const Arrays<R> a
       __syncthreads();                     // the warp-edge values posted at the end of the previous iteration
       const R *fs = fring + (it % FR) * 4 * kNT + tid;
       R ein = fs[0], hxin = fs[kNT], hyin = fs[2 * kNT], gin = fs[3 * kNT];
-      const R *xr_ = xch + ((it + 1) & 1) * (T * 3 * NW);      // read buffer of this iteration
-#pragma unroll
-      for (int s = 0; s < T; ++s) {
-        const int y = Y - 1 - s;
-        int slot = cbase - 1 - s;
-        if (slot < 0) slot += CR;
-        if (slot < 0) slot += CR;
-        const R *c = cring + slot * 4 * kNT + tid;
-        const R cP = c[0], cce = c[kNT], cka = c[2 * kNT], cQ = c[3 * kNT];
-        const R nchy_y = (y >= 0 && y <= p.ny - 2) ? p.nchy : R(0);
-        R e_rt = shfl_down1(e[s]);
-        if (lane == 31) e_rt = (warp + 1 < NW) ? xr_[(s * 3 + 0) * NW + warp + 1] : R(0);
-        const R hyn = O::hy_new(chx_i, e[s], e_rt, hy[s]);
-        R hyn_l = shfl_up1(hyn);
-        if (lane == 0)
-          hyn_l = (warp > 0) ? O::hy_new(chx_im1, xr_[(s * 3 + 1) * NW + warp - 1], e[s], xr_[(s * 3 + 2) * NW + warp - 1]) : R(0);
-        const R hxn = O::hx_new(nchy_y, e[s], ein, hx[s]);
-        R en = O::e_new(cP, cce, p.nr, e[s], g[s], hyn, hyn_l, hxn, hxp[s]);
-        const R gn = O::g_new(cka, cQ, g[s], e[s]);
-        R xs_new = e[s];
-        if (xw) {                          // this warp holds column 0 or nx-1: x edges of the rows 1..ny-2
-          const R en_rt = shfl_down1(en), en_lf = shfl_up1(en), e_lf = shfl_up1(e[s]);
-          if (y >= 1 && y <= p.ny - 2) {
-            if (xl) en = is_mur ? O::mur(p.mx, e_rt, en_rt, e[s]) : R(0);
-            if (xr) en = is_mur ? O::mur(p.mx, e_lf, en_lf, e[s]) : R(0);
-          }
-        }
-        if ((fq >> (s + 1)) & 1u) {        // rows 0, 1, ny-2, ny-1, the source row, rows with probes (CTA-uniform)
-          const bool own = own_col && y >= y_out0 && y < y_out1;
-          if (y == p.ny - 1) en = xs[s];   // computed one iteration ago from rows ny-2 (new) and ny-1 (old)
-          if (y == 0) en = R(0);           // set one iteration later, when E'[1] exists
-          if (y == p.ny - 2) xs_new = (xin && is_mur) ? O::mur(p.my, e[s], en, ein) : R(0);
-          if (y == 1) {                    // row 0 at level s+1: stage s+1 holds it by now (or it has been stored)
-            R e0 = (xin && is_mur) ? O::mur(p.my, e[s], en, xs[s]) : R(0);
-            if (p.src_j == 0 && src_col) e0 = Arith<R>::add(e0, p.src[s]);
-            if (own_col && y_out0 == 0 && (p.rowflag[0] & RF_PROBE))
-              for (int q = 0; q < p.nprobes; ++q)
-                if (p.probe_j[q] == 0 && p.probe_i[q] == i) p.rec[(int64_t)q * p.rec_stride + p.n0 + s] = e0;
-            if (s + 1 < T) {
-              e[s + 1 < T ? s + 1 : s] = e0;
-              R *xw_ = const_cast<R *>(xr_);
-              if (lane == 0) xw_[((s + 1) * 3 + 0) * NW + warp] = e0;
-              if (lane == 31) xw_[((s + 1) * 3 + 1) * NW + warp] = e0;
-              __syncthreads();
-            } else if (own_col && y_out0 == 0) {
-              a.E2[i] = e0;
-            }
-          }
-          if (y == p.src_j && src_col && y != 0) en = Arith<R>::add(en, p.src[s]);
-          if (own && y != 0 && (p.rowflag[y] & RF_PROBE))
-            for (int q = 0; q < p.nprobes; ++q)
-              if (p.probe_j[q] == y && p.probe_i[q] == i) p.rec[(int64_t)q * p.rec_stride + p.n0 + s] = en;
-        }
-        hxp[s] = hxn;
-        xs[s] = xs_new;
-        e[s] = ein; hx[s] = hxin; hy[s] = hyin; g[s] = gin;
-        ein = en; hxin = hxn; hyin = hyn; gin = gn;
-      }
+      R *xbuf = xch + ((it + 1) & 1) * (T * 3 * NW);           // read buffer of this iteration
+      if (fq & kHeldMask)
+        run_stages<R, T, true, true>(p, a, c, Y, fq, cbase, cring, xbuf, e, hx, hy, g, hxp, xs, ein, hxin, hyin, gin);
+      else if (xw)
+        run_stages<R, T, false, true>(p, a, c, Y, fq, cbase, cring, xbuf, e, hx, hy, g, hxp, xs, ein, hxin, hyin, gin);
+      else
+        run_stages<R, T, false, false>(p, a, c, Y, fq, cbase, cring, xbuf, e, hx, hy, g, hxp, xs, ein, hxin, hyin, gin);
       {                                    // (ein, hxin, hyin, gin) is now row Y-T at level T
         const int y = Y - T;
-        if (own_col && y >= y_out0 && y < y_out1) {
+        if (c.own_col && y >= c.y_out0 && y < c.y_out1) {
           const int64_t idx = (int64_t)y * p.pitch + i;
           a.E2[idx] = ein; a.Hx2[idx] = hxin; a.Hy2[idx] = hyin; a.G2[idx] = gin;
         }
       }
       R *xp = xch + (it & 1) * (T * 3 * NW);                   // read in the next iteration
-      if (lane == 0) {
+      if (c.lane == 0) {
 #pragma unroll
-        for (int s = 0; s < T; ++s) xp[(s * 3 + 0) * NW + warp] = e[s];
+        for (int s = 0; s < T; ++s) xp[(s * 3 + 0) * NW + c.warp] = e[s];
       }
-      if (lane == 31) {
+      if (c.lane == 31) {
 #pragma unroll
-        for (int s = 0; s < T; ++s) { xp[(s * 3 + 1) * NW + warp] = e[s]; xp[(s * 3 + 2) * NW + warp] = hy[s]; }
+        for (int s = 0; s < T; ++s) { xp[(s * 3 + 1) * NW + c.warp] = e[s]; xp[(s * 3 + 2) * NW + c.warp] = hy[s]; }
       }
       cbase = (cbase + 1 == CR) ? 0 : cbase + 1;
     }
