@@ -7,12 +7,15 @@
 //
 // The form computed (the 2-D twin of rketd_device.cuh's 7-operation form).  With the six coefficients of SURVEY a0
 // (Ez' = ca Ez - cj Jz + cex dHy - cey dHx,  Jz' = ka Jz + kb Ez + kc Ez') and G := cj Jz - (cj kc) Ez, exactly:
-//   Hx'[j][i] = fma(-chy, Ez[j+1][i] - Ez[j][i], Hx[j][i])                                   eq. (14), y axis
+//   Hx'[j][i] = fma(-chy, Ez[j+1][i], fma(chy, Ez[j][i], Hx[j][i]))                         eq. (14), y axis
 //   Hy'[j][i] = fma(+chx, Ez[j][i+1] - Ez[j][i], Hy[j][i])                                   eq. (14), x axis
-//   Ez'[j][i] = fma(ce, fma(-r, Hx'[j][i] - Hx'[j-1][i], Hy'[j][i] - Hy'[j][i-1]), fma(P, Ez, -G))    eq. (12)+(11)
+//   Ez'[j][i] = fma(A, Ez[j+1][i], B),   A = ce r chy,                                       eq. (12)+(11)
+//               B = fma(ce, fma(-r, fma(chy, Ez[j][i], Hx[j][i]) - Hx'[j-1][i], Hy'[j][i] - Hy'[j][i-1]), fma(P, Ez, -G))
 //   G'[j][i]  = fma(ka, G, Q Ez)                                                            eq. (11)
-// P = ca - cj kc, ce = cex, r = dx/dy (cey = cex r), Q = ka cj kc + cj kb: 11 FP instructions and 4 per-node
-// coefficients per node and step.
+// P = ca - cj kc, ce = cex, r = dx/dy (cey = cex r), Q = ka cj kc + cj kb: 13 FP instructions and 4 per-node
+// coefficients per node and step.  Ez' is written as "gain x the row above + rest" (the same real number as
+// fma(ce, fma(-r, Hx'[j] - Hx'[j-1], dHy), fma(P, Ez, -G))): in the streaming kernel the row above is the only operand
+// that arrives late, so the dependent chain from one pipeline stage to the next is a single fma.
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
@@ -44,7 +47,7 @@ template <typename R>
 struct P2 {
   int nx, ny;
   int64_t pitch;
-  R chx, nchy, nr;             // dt/(mu0 dx), -dt/(mu0 dy), -(dx/dy)
+  R chx, nchy, chy, nr, c2;    // dt/(mu0 dx), -dt/(mu0 dy), +dt/(mu0 dy), -(dx/dy), (dx/dy) dt/(mu0 dy)
   R mx, my;                    // first-order Mur (S-1)/(S+1) per axis
   int bc;
   int src_i, src_j;            // -1: none
@@ -68,12 +71,17 @@ struct Arrays {
 template <typename R>
 struct Ops {
   typedef Arith<R> A;
-  static __device__ __forceinline__ R hx_new(R nchy_j, R e, R e_up, R hx) { return A::fma(nchy_j, A::sub(e_up, e), hx); }
+  // Hx' = (Hx + chy E) - chy E_up: the part without the row above first (chy_j = 0 on the padding row ny-1)
+  static __device__ __forceinline__ R hx_part(R chy_j, R e, R hx) { return A::fma(chy_j, e, hx); }
+  static __device__ __forceinline__ R hx_new(R nchy_j, R e_up, R hxq) { return A::fma(nchy_j, e_up, hxq); }
   static __device__ __forceinline__ R hy_new(R chx_i, R e, R e_rt, R hy) { return A::fma(chx_i, A::sub(e_rt, e), hy); }
-  static __device__ __forceinline__ R e_new(R P, R ce, R nr, R e, R g, R hyn, R hyn_l, R hxn, R hxn_d) {
-    const R t = A::fma(nr, A::sub(hxn, hxn_d), A::sub(hyn, hyn_l));
+  // Ez' = gain * E_up + rest
+  static __device__ __forceinline__ R e_gain(R ce, R c2_j) { return A::mul(ce, c2_j); }
+  static __device__ __forceinline__ R e_rest(R P, R ce, R nr, R e, R g, R hyn, R hyn_l, R hxq, R hxn_d) {
+    const R t = A::fma(nr, A::sub(hxq, hxn_d), A::sub(hyn, hyn_l));
     return A::fma(ce, t, A::fma(P, e, -g));
   }
+  static __device__ __forceinline__ R e_new(R gain, R e_up, R rest) { return A::fma(gain, e_up, rest); }
   static __device__ __forceinline__ R g_new(R ka, R Q, R g, R e) { return A::fma(ka, g, A::mul(Q, e)); }
   // first-order Mur along the inward normal: E'[edge] = Eold[in] + m (E'[in] - Eold[edge])
   static __device__ __forceinline__ R mur(R m, R eold_in, R enew_in, R eold_self) {
@@ -92,13 +100,16 @@ __device__ __forceinline__ R interior_e(const P2<R> &p, const Arrays<R> &a, int 
   const R e_rt = (i + 1 < p.nx) ? a.E[idx + 1] : R(0);
   const R e_up = (j + 1 < p.ny) ? a.E[idx + p.pitch] : R(0);
   const R chx_i = (i <= p.nx - 2) ? p.chx : R(0);
-  const R nchy_j = (j <= p.ny - 2) ? p.nchy : R(0);
-  hxn = O::hx_new(nchy_j, e, e_up, a.Hx[idx]);
+  const bool yin = (j <= p.ny - 2);
+  const R hxq = O::hx_part(yin ? p.chy : R(0), e, a.Hx[idx]);
+  hxn = O::hx_new(yin ? p.nchy : R(0), e_up, hxq);
   hyn = O::hy_new(chx_i, e, e_rt, a.Hy[idx]);
   R hyn_l = R(0), hxn_d = R(0);
   if (i >= 1) hyn_l = O::hy_new(p.chx, a.E[idx - 1], e, a.Hy[idx - 1]);
-  if (j >= 1) hxn_d = O::hx_new(p.nchy, a.E[idx - p.pitch], e, a.Hx[idx - p.pitch]);
-  return O::e_new(a.cP[idx], a.cce[idx], p.nr, e, a.G[idx], hyn, hyn_l, hxn, hxn_d);
+  if (j >= 1) hxn_d = O::hx_new(p.nchy, e, O::hx_part(p.chy, a.E[idx - p.pitch], a.Hx[idx - p.pitch]));
+  const R ce = a.cce[idx];
+  const R rest = O::e_rest(a.cP[idx], ce, p.nr, e, a.G[idx], hyn, hyn_l, hxq, hxn_d);
+  return O::e_new(O::e_gain(ce, yin ? p.c2 : R(0)), e_up, rest);
 }
 
 template <typename R>
@@ -153,11 +164,20 @@ __device__ __forceinline__ R shfl_down1(R v) { return __shfl_down_sync(0xfffffff
 template <typename R>
 __device__ __forceinline__ R shfl_up1(R v) { return __shfl_up_sync(0xffffffffu, v, 1); }
 
+// 2 x R as one shared-memory access (16 B fp64, 8 B fp32)
+__device__ __forceinline__ void ld_pair(const double *q, double &x, double &y) { const double2 v = *reinterpret_cast<const double2 *>(q); x = v.x; y = v.y; }
+__device__ __forceinline__ void ld_pair(const float *q, float &x, float &y) { const float2 v = *reinterpret_cast<const float2 *>(q); x = v.x; y = v.y; }
+__device__ __forceinline__ void st_pair(double *q, double x, double y) { *reinterpret_cast<double2 *>(q) = make_double2(x, y); }
+__device__ __forceinline__ void st_pair(float *q, float x, float y) { *reinterpret_cast<float2 *>(q) = make_float2(x, y); }
+
 constexpr int kFieldRing = kPF + 1;
 template <typename R, int T>
 struct K2Shape {
-  static constexpr int CR = T + kPF + 1;            // coefficient ring: rows Y-T .. Y+kPF are alive at once
-  static constexpr size_t smem = sizeof(R) * ((size_t)kFieldRing * 4 * kNT + (size_t)CR * 4 * kNT + (size_t)2 * T * 3 * (kNT / 32));
+  static constexpr int need = T + kPF + 1;          // coefficient ring: rows Y-T .. Y+kPF are alive at once
+  static constexpr int pow2 = need <= 2 ? 2 : need <= 4 ? 4 : need <= 8 ? 8 : need <= 16 ? 16 : 32;
+  static constexpr size_t bytes(int cr) { return sizeof(R) * ((size_t)kFieldRing * 4 * kNT + (size_t)cr * 4 * kNT + (size_t)2 * T * 4 * (kNT / 32) + (size_t)T * kNT); }
+  static constexpr int CR = bytes(pow2) <= 200 * 1024 ? pow2 : need;   // a power of two when it fits: slot = index & (CR-1)
+  static constexpr size_t smem = bytes(CR);
 };
 
 // Per-thread constants of a job of the streaming kernel.
@@ -168,59 +188,123 @@ struct JobCtx {
   R chx_i, chx_im1;
 };
 
-// The T pipeline stages of one iteration (row Y has just entered as (ein, hxin, hyin, gin)).
-//   SPECIAL = false: none of the rows held by the stages is row 0, 1, ny-2, ny-1, the source row or a probe row —
-//                    straight-line code, the stages' independent parts overlap freely;
+// What a thread keeps per pipeline stage: E, Hx, Hy, G of the row the stage holds.
+template <typename R, int T>
+struct Held {
+  R e[T], hx[T], hy[T], g[T];
+  R hxp_last;          // new Hx of the row before the one the LAST stage holds (for s < T-1 that value is hx[s+1])
+};
+
+// The T pipeline stages of one iteration (row Y has just entered as (ein, hxin, hyin, gin)): reads the held rows `h`,
+// leaves the rows held in the next iteration in `n` (two sets used alternately, so that no register is copied).
+//   SPECIAL = false: none of the rows held by the stages is row 0, 1, ny-2, ny-1, the source row or a probe row.
+//                    Everything that does not need the row above is computed for all stages first (shuffles, new Hy,
+//                    new G, gain and rest of Ez'); what is left is one fma per stage along the pipeline.
+//   SPECIAL = true:  stage by stage, with the y edges, the source and the probes; `xsb` (shared memory, [T][kNT]) keeps
+//                    one spare value per stage across iterations: the old E of the row before (needed on row 1 for the
+//                    Mur value of row 0) or, on row ny-1, the edge value computed one iteration earlier.
 //   XEDGE:           this warp holds column 0 or nx-1 (first-order Mur / conductor on the x edges).
 template <typename R, int T, bool SPECIAL, bool XEDGE>
 __device__ __forceinline__ void run_stages(const P2<R> &p, const Arrays<R> &a, const JobCtx<R> &c, const int Y, const uint32_t fq,
-                                           const int cbase, const R *cring, R *xbuf, R (&e)[T], R (&hx)[T], R (&hy)[T],
-                                           R (&g)[T], R (&hxp)[T], R (&xs)[T], R &ein, R &hxin, R &hyin, R &gin) {
+                                           const int cbase, const R *cring, R *xbuf, R *xsb, Held<R, T> &h, Held<R, T> &n,
+                                           R &ein, R &hxin, R &hyin, R &gin) {
   typedef Ops<R> O;
   constexpr int NW = kNT / 32;
   constexpr int CR = K2Shape<R, T>::CR;
   const int tid = c.warp * 32 + c.lane;
+  R gain[T], rest[T], hxq[T], hyn[T], gn[T];
+  if (!SPECIAL) {
+#pragma unroll
+    for (int s = 0; s < T; ++s) {        // everything that needs old values only
+      int slot = cbase - 1 - s;
+      if ((CR & (CR - 1)) == 0) slot &= CR - 1;
+      else if (slot < 0) slot += CR;
+      const R *cf = cring + slot * 4 * kNT + tid;
+      const R cP = cf[0], cce = cf[kNT], cka = cf[2 * kNT], cQ = cf[3 * kNT];
+      const R es = h.e[s];
+      R e_rt = shfl_down1(es);
+      if (c.lane == 31) e_rt = (c.warp + 1 < NW) ? xbuf[(s * NW + c.warp + 1) * 4 + 2] : R(0);
+      hyn[s] = O::hy_new(c.chx_i, es, e_rt, h.hy[s]);
+      R hyn_l = shfl_up1(hyn[s]);
+      if (c.lane == 0) {
+        R e31 = R(0), hy31 = R(0);
+        if (c.warp > 0) ld_pair(xbuf + (s * NW + c.warp - 1) * 4, e31, hy31);
+        hyn_l = O::hy_new(c.chx_im1, e31, es, hy31);         // 0 for warp 0: its left neighbour holds zeros
+      }
+      // rows outside the grid hold zeros, so chy is right for them too (row ny-1, where it is not, is a special row)
+      hxq[s] = O::hx_part(p.chy, es, h.hx[s]);
+      const R hxp = (s + 1 < T) ? h.hx[s + 1 < T ? s + 1 : s] : h.hxp_last;
+      rest[s] = O::e_rest(cP, cce, p.nr, es, h.g[s], hyn[s], hyn_l, hxq[s], hxp);
+      gain[s] = O::e_gain(cce, p.c2);
+      gn[s] = O::g_new(cka, cQ, h.g[s], es);
+    }
+#pragma unroll
+    for (int s = 0; s < T; ++s) {        // along the pipeline: one fma per stage on the critical path
+      const int y = Y - 1 - s;
+      R en = O::e_new(gain[s], ein, rest[s]);
+      const R hxn = O::hx_new(p.nchy, ein, hxq[s]);
+      if (XEDGE) {                       // x edges of the rows 1..ny-2
+        const R es = h.e[s];
+        const R e_rt = shfl_down1(es), e_lf = shfl_up1(es), en_rt = shfl_down1(en), en_lf = shfl_up1(en);
+        if (y >= 1 && y <= p.ny - 2) {
+          if (c.xl) en = c.is_mur ? O::mur(p.mx, e_rt, en_rt, es) : R(0);
+          if (c.xr) en = c.is_mur ? O::mur(p.mx, e_lf, en_lf, es) : R(0);
+        }
+      }
+      if (s == T - 1) n.hxp_last = hxn;
+      n.e[s] = ein; n.hx[s] = hxin; n.hy[s] = hyin; n.g[s] = gin;
+      ein = en; hxin = hxn; hyin = hyn[s]; gin = gn[s];
+    }
+    return;
+  }
 #pragma unroll
   for (int s = 0; s < T; ++s) {
     const int y = Y - 1 - s;
     int slot = cbase - 1 - s;
-    if (slot < 0) slot += CR;
+    if ((CR & (CR - 1)) == 0) slot &= CR - 1;
+    else if (slot < 0) slot += CR;
     const R *cf = cring + slot * 4 * kNT + tid;
     const R cP = cf[0], cce = cf[kNT], cka = cf[2 * kNT], cQ = cf[3 * kNT];
-    // rows outside the grid hold zeros, so -chy is right for them too; only row ny-1 (a special row) needs 0
-    const R nchy_y = SPECIAL ? ((y >= 0 && y <= p.ny - 2) ? p.nchy : R(0)) : p.nchy;
-    R e_rt = shfl_down1(e[s]);
-    if (c.lane == 31) e_rt = (c.warp + 1 < NW) ? xbuf[(s * 3 + 0) * NW + c.warp + 1] : R(0);
-    const R hyn = O::hy_new(c.chx_i, e[s], e_rt, hy[s]);
-    R hyn_l = shfl_up1(hyn);
-    if (c.lane == 0)
-      hyn_l = (c.warp > 0) ? O::hy_new(c.chx_im1, xbuf[(s * 3 + 1) * NW + c.warp - 1], e[s], xbuf[(s * 3 + 2) * NW + c.warp - 1]) : R(0);
-    const R hxn = O::hx_new(nchy_y, e[s], ein, hx[s]);
-    R en = O::e_new(cP, cce, p.nr, e[s], g[s], hyn, hyn_l, hxn, hxp[s]);
-    const R gn = O::g_new(cka, cQ, g[s], e[s]);
-    R xs_new = e[s];
-    if (XEDGE) {                         // x edges of the rows 1..ny-2
-      const R en_rt = shfl_down1(en), en_lf = shfl_up1(en), e_lf = shfl_up1(e[s]);
+    const bool yin = (y >= 0 && y <= p.ny - 2);
+    const R es = h.e[s];
+    R e_rt = shfl_down1(es);
+    if (c.lane == 31) e_rt = (c.warp + 1 < NW) ? xbuf[(s * NW + c.warp + 1) * 4 + 2] : R(0);
+    const R hyn_s = O::hy_new(c.chx_i, es, e_rt, h.hy[s]);
+    R hyn_l = shfl_up1(hyn_s);
+    if (c.lane == 0) {
+      R e31 = R(0), hy31 = R(0);
+      if (c.warp > 0) ld_pair(xbuf + (s * NW + c.warp - 1) * 4, e31, hy31);
+      hyn_l = O::hy_new(c.chx_im1, e31, es, hy31);
+    }
+    const R hxq_s = O::hx_part(yin ? p.chy : R(0), es, h.hx[s]);
+    const R hxn = O::hx_new(yin ? p.nchy : R(0), ein, hxq_s);
+    const R hxp = (s + 1 < T) ? h.hx[s + 1 < T ? s + 1 : s] : h.hxp_last;
+    R en = O::e_new(O::e_gain(cce, yin ? p.c2 : R(0)), ein, O::e_rest(cP, cce, p.nr, es, h.g[s], hyn_s, hyn_l, hxq_s, hxp));
+    const R gn_s = O::g_new(cka, cQ, h.g[s], es);
+    R xs_new = es;
+    {                                    // x edges of the rows 1..ny-2 (every warp takes the shuffles here)
+      const R en_rt = shfl_down1(en), en_lf = shfl_up1(en), e_lf = shfl_up1(es);
       if (y >= 1 && y <= p.ny - 2) {
-        if (c.xl) en = c.is_mur ? O::mur(p.mx, e_rt, en_rt, e[s]) : R(0);
-        if (c.xr) en = c.is_mur ? O::mur(p.mx, e_lf, en_lf, e[s]) : R(0);
+        if (c.xl) en = c.is_mur ? O::mur(p.mx, e_rt, en_rt, es) : R(0);
+        if (c.xr) en = c.is_mur ? O::mur(p.mx, e_lf, en_lf, es) : R(0);
       }
     }
-    if (SPECIAL && ((fq >> (s + 1)) & 1u)) {       // CTA-uniform
+    if ((fq >> (s + 1)) & 1u) {          // CTA-uniform
       const bool own = c.own_col && y >= c.y_out0 && y < c.y_out1;
-      if (y == p.ny - 1) en = xs[s];     // computed one iteration ago from rows ny-2 (new) and ny-1 (old)
+      const R xs = xsb[s * kNT + tid];
+      if (y == p.ny - 1) en = xs;        // computed one iteration ago from rows ny-2 (new) and ny-1 (old)
       if (y == 0) en = R(0);             // set one iteration later, when E'[1] exists
-      if (y == p.ny - 2) xs_new = (c.xin && c.is_mur) ? O::mur(p.my, e[s], en, ein) : R(0);
+      if (y == p.ny - 2) xs_new = (c.xin && c.is_mur) ? O::mur(p.my, es, en, ein) : R(0);
       if (y == 1) {                      // row 0 at level s+1: stage s+1 holds it by now (or it has been stored)
-        R e0 = (c.xin && c.is_mur) ? O::mur(p.my, e[s], en, xs[s]) : R(0);
+        R e0 = (c.xin && c.is_mur) ? O::mur(p.my, es, en, xs) : R(0);
         if (p.src_j == 0 && c.src_col) e0 = Arith<R>::add(e0, p.src[s]);
         if (c.own_col && c.y_out0 == 0 && (p.rowflag[0] & RF_PROBE))
           for (int q = 0; q < p.nprobes; ++q)
             if (p.probe_j[q] == 0 && p.probe_i[q] == c.i) p.rec[(int64_t)q * p.rec_stride + p.n0 + s] = e0;
         if (s + 1 < T) {
-          e[s + 1 < T ? s + 1 : s] = e0;
-          if (c.lane == 0) xbuf[((s + 1) * 3 + 0) * NW + c.warp] = e0;
-          if (c.lane == 31) xbuf[((s + 1) * 3 + 1) * NW + c.warp] = e0;
+          h.e[s + 1 < T ? s + 1 : s] = e0;
+          if (c.lane == 0) xbuf[((s + 1) * NW + c.warp) * 4 + 2] = e0;
+          if (c.lane == 31) xbuf[((s + 1) * NW + c.warp) * 4 + 0] = e0;
           __syncthreads();
         } else if (c.own_col && c.y_out0 == 0) {
           a.E2[c.i] = e0;
@@ -231,10 +315,10 @@ __device__ __forceinline__ void run_stages(const P2<R> &p, const Arrays<R> &a, c
         for (int q = 0; q < p.nprobes; ++q)
           if (p.probe_j[q] == y && p.probe_i[q] == c.i) p.rec[(int64_t)q * p.rec_stride + p.n0 + s] = en;
     }
-    hxp[s] = hxn;
-    xs[s] = xs_new;
-    e[s] = ein; hx[s] = hxin; hy[s] = hyin; g[s] = gin;
-    ein = en; hxin = hxn; hyin = hyn; gin = gn;
+    xsb[s * kNT + tid] = xs_new;
+    if (s == T - 1) n.hxp_last = hxn;
+    n.e[s] = ein; n.hx[s] = hxin; n.hy[s] = hyin; n.g[s] = gin;
+    ein = en; hxin = hxn; hyin = hyn_s; gin = gn_s;
   }
 }
 
@@ -242,26 +326,28 @@ __device__ __forceinline__ void run_stages(const P2<R> &p, const Arrays<R> &a, c
 // halo rows on each side).  Iteration `it` lets row Y = ya + it enter; stage s (s = 0..T-1) then holds row Y-1-s at
 // level s (E, G at step n0+s, H half a step earlier) in registers, receives row Y-s at level s from stage s-1 (from
 // shared memory for s = 0), and produces level s+1 of its held row, which is what stage s+1 receives.  The last stage
-// writes row Y-T at level T to the other field buffer.  Per stage a thread keeps E, Hx, Hy, G of the held row, the new
-// Hx of the row before, and one spare value for the y edges; the four coefficients of a row wait in a shared-memory
-// ring (written once by cp.async, read by each stage in turn; every thread touches its own column only).  Between
-// lanes new Hy and old E travel by shuffle; between warps old E and old Hy of the warp-edge columns are posted to
-// shared memory at the end of an iteration (one CTA barrier per row).
+// writes row Y-T at level T to the other field buffer.  Per stage a thread keeps E, Hx, Hy, G of the held row and one
+// spare value for the y edges; the four coefficients of a row wait in a shared-memory ring (written once by cp.async,
+// read by each stage in turn; every thread touches its own column only).  Between lanes new Hy and old E travel by
+// shuffle; between warps old E and old Hy of the warp-edge columns are posted to shared memory at the end of an
+// iteration (one CTA barrier per row).
 template <typename R, int T>
 __global__ void __launch_bounds__(kNT, 1) k2_2d(const P2<R> p, const Arrays<R> a) {
   constexpr int NW = kNT / 32;
   constexpr int CR = K2Shape<R, T>::CR;
   constexpr int FR = kFieldRing;
+  constexpr int XB = T * NW * 4;                              // one exchange buffer: [T][NW]{E31, Hy31, E0, -}
   extern __shared__ __align__(16) uint8_t smem_raw[];
   R *fring = reinterpret_cast<R *>(smem_raw);                 // [FR][4][kNT]
   R *cring = fring + FR * 4 * kNT;                            // [CR][4][kNT]
-  R *xch = cring + CR * 4 * kNT;                              // [2][T][3][NW]: E of lane 0, E of lane 31, Hy of lane 31
+  R *xch = cring + CR * 4 * kNT;                              // [2][XB]
+  R *xsb = xch + 2 * XB;                                      // [T][kNT]
   const int tid = threadIdx.x;
   JobCtx<R> c;
   c.lane = tid & 31; c.warp = tid >> 5;
   c.is_mur = (p.bc == RKETD2D_BC_MUR);
 
-  for (int q = tid; q < 2 * T * 3 * NW; q += kNT) xch[q] = R(0);
+  for (int q = tid; q < 2 * XB; q += kNT) xch[q] = R(0);
   for (int q = 0; q < CR * 4; ++q) cring[q * kNT + tid] = R(0);
 
   const int njobs = p.nstrips * p.nsegs;
@@ -274,16 +360,17 @@ __global__ void __launch_bounds__(kNT, 1) k2_2d(const P2<R> p, const Arrays<R> a
     c.own_col = incol && i >= strip * p.Wv && i < (strip + 1) * p.Wv;
     c.y_out0 = seg * p.Sy; c.y_out1 = min(p.ny, c.y_out0 + p.Sy);
     const int ya = c.y_out0 - T;
-    const int niter = (c.y_out1 - c.y_out0) + 2 * T;
+    const int niter = (c.y_out1 - c.y_out0) + 2 * T;          // rows ya .. y_out1-1+T enter
     c.chx_i = (i >= 0 && i <= p.nx - 2) ? p.chx : R(0);
-    c.chx_im1 = (i >= 1 && i <= p.nx - 1) ? p.chx : R(0);
+    c.chx_im1 = (i >= 1 && i <= p.nx - 1 && c.warp > 0) ? p.chx : R(0);
     c.xl = (i == 0); c.xr = (i == p.nx - 1); c.xin = (i >= 1 && i <= p.nx - 2);
     const bool xw = __any_sync(0xffffffffu, c.xl || c.xr);
     c.src_col = (i == p.src_i);
 
-    R e[T], hx[T], hy[T], g[T], hxp[T], xs[T];
+    Held<R, T> hA, hB;
 #pragma unroll
-    for (int s = 0; s < T; ++s) e[s] = hx[s] = hy[s] = g[s] = hxp[s] = xs[s] = R(0);
+    for (int s = 0; s < T; ++s) hA.e[s] = hA.hx[s] = hA.hy[s] = hA.g[s] = R(0);
+    hA.hxp_last = R(0);
     uint32_t fq = 0;
 
     __syncthreads();                       // xch zeroed / the previous job is done with it
@@ -309,21 +396,23 @@ __global__ void __launch_bounds__(kNT, 1) k2_2d(const P2<R> p, const Arrays<R> a
 
     constexpr uint32_t kHeldMask = ((1u << T) - 1u) << 1;     // bits of the rows the T stages hold
     int cbase = 0;                         // it % CR
-    for (int it = 0; it < niter; ++it) {
+
+    auto iteration = [&](const int it, Held<R, T> &h, Held<R, T> &n) {
       const int Y = ya + it;
       issue_row(it + kPF);
       cp_async_wait<kPF>();
+      const bool special = ((fq << 1) & kHeldMask) != 0;       // the flag of row Y is not among the held rows yet
       fq = (fq << 1) | ((Y >= 0 && Y < p.ny) ? (uint32_t)(p.rowflag[Y] & RF_SPECIAL) : 0u);
       __syncthreads();                     // the warp-edge values posted at the end of the previous iteration
       const R *fs = fring + (it % FR) * 4 * kNT + tid;
       R ein = fs[0], hxin = fs[kNT], hyin = fs[2 * kNT], gin = fs[3 * kNT];
-      R *xbuf = xch + ((it + 1) & 1) * (T * 3 * NW);           // read buffer of this iteration
-      if (fq & kHeldMask)
-        run_stages<R, T, true, true>(p, a, c, Y, fq, cbase, cring, xbuf, e, hx, hy, g, hxp, xs, ein, hxin, hyin, gin);
+      R *xbuf = xch + ((it + 1) & 1) * XB;                     // read buffer of this iteration
+      if (special)
+        run_stages<R, T, true, true>(p, a, c, Y, fq, cbase, cring, xbuf, xsb, h, n, ein, hxin, hyin, gin);
       else if (xw)
-        run_stages<R, T, false, true>(p, a, c, Y, fq, cbase, cring, xbuf, e, hx, hy, g, hxp, xs, ein, hxin, hyin, gin);
+        run_stages<R, T, false, true>(p, a, c, Y, fq, cbase, cring, xbuf, xsb, h, n, ein, hxin, hyin, gin);
       else
-        run_stages<R, T, false, false>(p, a, c, Y, fq, cbase, cring, xbuf, e, hx, hy, g, hxp, xs, ein, hxin, hyin, gin);
+        run_stages<R, T, false, false>(p, a, c, Y, fq, cbase, cring, xbuf, xsb, h, n, ein, hxin, hyin, gin);
       {                                    // (ein, hxin, hyin, gin) is now row Y-T at level T
         const int y = Y - T;
         if (c.own_col && y >= c.y_out0 && y < c.y_out1) {
@@ -331,20 +420,26 @@ __global__ void __launch_bounds__(kNT, 1) k2_2d(const P2<R> p, const Arrays<R> a
           a.E2[idx] = ein; a.Hx2[idx] = hxin; a.Hy2[idx] = hyin; a.G2[idx] = gin;
         }
       }
-      R *xp = xch + (it & 1) * (T * 3 * NW);                   // read in the next iteration
-      if (c.lane == 0) {
-#pragma unroll
-        for (int s = 0; s < T; ++s) xp[(s * 3 + 0) * NW + c.warp] = e[s];
-      }
+      R *xp = xch + (it & 1) * XB;                             // read in the next iteration
       if (c.lane == 31) {
 #pragma unroll
-        for (int s = 0; s < T; ++s) { xp[(s * 3 + 1) * NW + c.warp] = e[s]; xp[(s * 3 + 2) * NW + c.warp] = hy[s]; }
+        for (int s = 0; s < T; ++s) st_pair(xp + (s * NW + c.warp) * 4, n.e[s], n.hy[s]);
+      }
+      if (c.lane == 0) {
+#pragma unroll
+        for (int s = 0; s < T; ++s) xp[(s * NW + c.warp) * 4 + 2] = n.e[s];
       }
       cbase = (cbase + 1 == CR) ? 0 : cbase + 1;
+    };
+
+    // two register sets used alternately; an odd count runs one more iteration on a zero row, which stores nothing
+    for (int it = 0; it < niter; it += 2) {
+      iteration(it, hA, hB);
+      iteration(it + 1, hB, hA);
     }
     cp_async_wait<0>();
     __syncthreads();
-    for (int q = tid; q < 2 * T * 3 * NW; q += kNT) xch[q] = R(0);
+    for (int q = tid; q < 2 * XB; q += kNT) xch[q] = R(0);
   }
 }
 
@@ -531,7 +626,9 @@ void fill_params(const rketd2d_sim *s, P2<R> &p, void *rec, int64_t rec_stride, 
   p.nx = s->nx; p.ny = s->ny; p.pitch = s->pitch;
   p.chx = (R)(s->dt / (kMu0 * s->dx));
   p.nchy = (R)(-(s->dt / (kMu0 * s->dy)));
+  p.chy = -p.nchy;
   p.nr = (R)(-(s->dx / s->dy));
+  p.c2 = (R)((s->dx / s->dy) * (s->dt / (kMu0 * s->dy)));
   const double Sx = kC0 * s->dt / s->dx, Sy = kC0 * s->dt / s->dy;
   p.mx = (R)((Sx - 1.0) / (Sx + 1.0));
   p.my = (R)((Sy - 1.0) / (Sy + 1.0));
@@ -581,7 +678,7 @@ cudaError_t launch_k2(rketd2d_sim *s, P2<R> &p, int T) {
     case 2: return launch_k2_T<R, 2>(s, p);
     case 4: return launch_k2_T<R, 4>(s, p);
     case 8: return launch_k2_T<R, 8>(s, p);
-    case 16: return launch_k2_T<R, 16>(s, p);
+    case 16: if (sizeof(R) == 4) return launch_k2_T<float, 16>(s, reinterpret_cast<P2<float> &>(p)); break;
   }
   return cudaErrorInvalidValue;
 }
@@ -807,6 +904,7 @@ int rketd2d_set_plan(rketd2d_sim *s, int kernel, int depth) {
   if (kernel < RKETD2D_KERNEL_AUTO || kernel > RKETD2D_KERNEL_STREAM) return fail2(s, RKETD_EINVAL, "unknown kernel");
   if (depth != 0 && depth != 1 && depth != 2 && depth != 4 && depth != 8 && depth != 16)
     return fail2(s, RKETD_EINVAL, "depth must be 0, 1, 2, 4, 8 or 16");
+  if (depth == 16 && s->dtype == RKETD_F64) return fail2(s, RKETD_EINVAL, "depth 16 is for fp32 (registers and shared memory)");
   s->plan_kernel = kernel;
   s->plan_depth = depth;
   return RKETD_OK;

@@ -84,7 +84,7 @@ def test_reduced_column_all_kernels(dtype):
     k1 = _gpu_run(w, dtype, m.KERNEL_STEP)
     assert k1["kernel"] == m.KERNEL_STEP and k1["launches"] == 150
     _check(k1, o, TOL[dtype])
-    for T in (1, 2, 4, 8, 16):
+    for T in (1, 2, 4, 8) + ((16,) if dtype == "f32" else ()):
         k2 = _gpu_run(w, dtype, m.KERNEL_STREAM, T)
         assert k2["kernel"] == m.KERNEL_STREAM
         assert np.array_equal(k2["rec"], k1["rec"]), T
@@ -105,7 +105,7 @@ def test_ragged_sizes_mur(nx, ny):
     o = _oracle_run(w)
     k1 = _gpu_run(w, "f64", m.KERNEL_STEP)
     _check(k1, o, 1e-12)
-    for T in (8, 16, 2):
+    for T in (8, 4, 2):
         k2 = _gpu_run(w, "f64", m.KERNEL_STREAM, T)
         assert np.array_equal(k2["rec"], k1["rec"]), (T, np.max(np.abs(k2["rec"] - k1["rec"])))
         for a, b in zip(k2["fields"], k1["fields"]):
