@@ -175,7 +175,7 @@ template <typename R, int T>
 struct K2Shape {
   static constexpr int need = T + kPF + 1;          // coefficient ring: rows Y-T .. Y+kPF are alive at once
   static constexpr int pow2 = need <= 2 ? 2 : need <= 4 ? 4 : need <= 8 ? 8 : need <= 16 ? 16 : 32;
-  static constexpr size_t bytes(int cr) { return sizeof(R) * ((size_t)kFieldRing * 4 * kNT + (size_t)cr * 4 * kNT + (size_t)2 * T * 4 * (kNT / 32) + (size_t)T * kNT); }
+  static constexpr size_t bytes(int cr) { return sizeof(R) * ((size_t)kFieldRing * 4 * kNT + (size_t)cr * 4 * kNT + (size_t)2 * T * 4 * (kNT / 32 + 2) + (size_t)T * kNT); }
   static constexpr int CR = bytes(pow2) <= 200 * 1024 ? pow2 : need;   // a power of two when it fits: slot = index & (CR-1)
   static constexpr size_t smem = bytes(CR);
 };
@@ -209,7 +209,7 @@ __device__ __forceinline__ void run_stages(const P2<R> &p, const Arrays<R> &a, c
                                            const int cbase, const R *cring, R *xbuf, R *xsb, Held<R, T> &h, Held<R, T> &n,
                                            R &ein, R &hxin, R &hyin, R &gin) {
   typedef Ops<R> O;
-  constexpr int NW = kNT / 32;
+  constexpr int XS = kNT / 32 + 2;     // exchange slots per stage: one per warp plus a zero slot at each end
   constexpr int CR = K2Shape<R, T>::CR;
   const int tid = c.warp * 32 + c.lane;
   R gain[T], rest[T], hxq[T], hyn[T], gn[T];
@@ -222,15 +222,18 @@ __device__ __forceinline__ void run_stages(const P2<R> &p, const Arrays<R> &a, c
       const R *cf = cring + slot * 4 * kNT + tid;
       const R cP = cf[0], cce = cf[kNT], cka = cf[2 * kNT], cQ = cf[3 * kNT];
       const R es = h.e[s];
+      // neighbours across the warp edge come from the exchange buffer (slots of the strip's outer neighbours hold zeros);
+      // branch-free, so that the whole path stays one block the compiler can interleave
+      const R *xl_ = xbuf + (s * XS + c.warp) * 4;           // slot of warp - 1: {E, Hy of its lane 31}
+      R e31, hy31;
+      ld_pair(xl_, e31, hy31);
+      const R e0r = xl_[2 * 4 + 2];                          // slot of warp + 1: E of its lane 0
       R e_rt = shfl_down1(es);
-      if (c.lane == 31) e_rt = (c.warp + 1 < NW) ? xbuf[(s * NW + c.warp + 1) * 4 + 2] : R(0);
+      e_rt = (c.lane == 31) ? e0r : e_rt;
       hyn[s] = O::hy_new(c.chx_i, es, e_rt, h.hy[s]);
+      const R hyn_edge = O::hy_new(c.chx_im1, e31, es, hy31);
       R hyn_l = shfl_up1(hyn[s]);
-      if (c.lane == 0) {
-        R e31 = R(0), hy31 = R(0);
-        if (c.warp > 0) ld_pair(xbuf + (s * NW + c.warp - 1) * 4, e31, hy31);
-        hyn_l = O::hy_new(c.chx_im1, e31, es, hy31);         // 0 for warp 0: its left neighbour holds zeros
-      }
+      hyn_l = (c.lane == 0) ? hyn_edge : hyn_l;
       // rows outside the grid hold zeros, so chy is right for them too (row ny-1, where it is not, is a special row)
       hxq[s] = O::hx_part(p.chy, es, h.hx[s]);
       const R hxp = (s + 1 < T) ? h.hx[s + 1 < T ? s + 1 : s] : h.hxp_last;
@@ -267,15 +270,16 @@ __device__ __forceinline__ void run_stages(const P2<R> &p, const Arrays<R> &a, c
     const R cP = cf[0], cce = cf[kNT], cka = cf[2 * kNT], cQ = cf[3 * kNT];
     const bool yin = (y >= 0 && y <= p.ny - 2);
     const R es = h.e[s];
+    const R *xl_ = xbuf + (s * XS + c.warp) * 4;
+    R e31, hy31;
+    ld_pair(xl_, e31, hy31);
+    const R e0r = xl_[2 * 4 + 2];
     R e_rt = shfl_down1(es);
-    if (c.lane == 31) e_rt = (c.warp + 1 < NW) ? xbuf[(s * NW + c.warp + 1) * 4 + 2] : R(0);
+    e_rt = (c.lane == 31) ? e0r : e_rt;
     const R hyn_s = O::hy_new(c.chx_i, es, e_rt, h.hy[s]);
+    const R hyn_edge = O::hy_new(c.chx_im1, e31, es, hy31);
     R hyn_l = shfl_up1(hyn_s);
-    if (c.lane == 0) {
-      R e31 = R(0), hy31 = R(0);
-      if (c.warp > 0) ld_pair(xbuf + (s * NW + c.warp - 1) * 4, e31, hy31);
-      hyn_l = O::hy_new(c.chx_im1, e31, es, hy31);
-    }
+    hyn_l = (c.lane == 0) ? hyn_edge : hyn_l;
     const R hxq_s = O::hx_part(yin ? p.chy : R(0), es, h.hx[s]);
     const R hxn = O::hx_new(yin ? p.nchy : R(0), ein, hxq_s);
     const R hxp = (s + 1 < T) ? h.hx[s + 1 < T ? s + 1 : s] : h.hxp_last;
@@ -303,8 +307,8 @@ __device__ __forceinline__ void run_stages(const P2<R> &p, const Arrays<R> &a, c
             if (p.probe_j[q] == 0 && p.probe_i[q] == c.i) p.rec[(int64_t)q * p.rec_stride + p.n0 + s] = e0;
         if (s + 1 < T) {
           h.e[s + 1 < T ? s + 1 : s] = e0;
-          if (c.lane == 0) xbuf[((s + 1) * NW + c.warp) * 4 + 2] = e0;
-          if (c.lane == 31) xbuf[((s + 1) * NW + c.warp) * 4 + 0] = e0;
+          if (c.lane == 0) xbuf[((s + 1) * XS + c.warp + 1) * 4 + 2] = e0;
+          if (c.lane == 31) xbuf[((s + 1) * XS + c.warp + 1) * 4 + 0] = e0;
           __syncthreads();
         } else if (c.own_col && c.y_out0 == 0) {
           a.E2[c.i] = e0;
@@ -336,7 +340,8 @@ __global__ void __launch_bounds__(kNT, 1) k2_2d(const P2<R> p, const Arrays<R> a
   constexpr int NW = kNT / 32;
   constexpr int CR = K2Shape<R, T>::CR;
   constexpr int FR = kFieldRing;
-  constexpr int XB = T * NW * 4;                              // one exchange buffer: [T][NW]{E31, Hy31, E0, -}
+  constexpr int XS = NW + 2;
+  constexpr int XB = T * XS * 4;                              // one exchange buffer: [T][XS]{E31, Hy31, E0, -}, end slots zero
   extern __shared__ __align__(16) uint8_t smem_raw[];
   R *fring = reinterpret_cast<R *>(smem_raw);                 // [FR][4][kNT]
   R *cring = fring + FR * 4 * kNT;                            // [CR][4][kNT]
@@ -423,11 +428,11 @@ __global__ void __launch_bounds__(kNT, 1) k2_2d(const P2<R> p, const Arrays<R> a
       R *xp = xch + (it & 1) * XB;                             // read in the next iteration
       if (c.lane == 31) {
 #pragma unroll
-        for (int s = 0; s < T; ++s) st_pair(xp + (s * NW + c.warp) * 4, n.e[s], n.hy[s]);
+        for (int s = 0; s < T; ++s) st_pair(xp + (s * XS + c.warp + 1) * 4, n.e[s], n.hy[s]);
       }
       if (c.lane == 0) {
 #pragma unroll
-        for (int s = 0; s < T; ++s) xp[(s * NW + c.warp) * 4 + 2] = n.e[s];
+        for (int s = 0; s < T; ++s) xp[(s * XS + c.warp + 1) * 4 + 2] = n.e[s];
       }
       cbase = (cbase + 1 == CR) ? 0 : cbase + 1;
     };
