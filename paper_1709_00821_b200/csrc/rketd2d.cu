@@ -170,14 +170,10 @@ __device__ __forceinline__ void ld_pair(const float *q, float &x, float &y) { co
 __device__ __forceinline__ void st_pair(double *q, double x, double y) { *reinterpret_cast<double2 *>(q) = make_double2(x, y); }
 __device__ __forceinline__ void st_pair(float *q, float x, float y) { *reinterpret_cast<float2 *>(q) = make_float2(x, y); }
 
-constexpr int kFieldRing = kPF + 1;
+constexpr int kRing = kPF + 1;      // entry ring: rows Y .. Y+kPF, 8 arrays each (Ez, Hx, Hy, G, P, ce, ka, Q)
 template <typename R, int T>
 struct K2Shape {
-  static constexpr int need = T + kPF + 1;          // coefficient ring: rows Y-T .. Y+kPF are alive at once
-  static constexpr int pow2 = need <= 2 ? 2 : need <= 4 ? 4 : need <= 8 ? 8 : need <= 16 ? 16 : 32;
-  static constexpr size_t bytes(int cr) { return sizeof(R) * ((size_t)kFieldRing * 4 * kNT + (size_t)cr * 4 * kNT + (size_t)2 * T * 4 * (kNT / 32 + 2) + (size_t)T * kNT); }
-  static constexpr int CR = bytes(pow2) <= 200 * 1024 ? pow2 : need;   // a power of two when it fits: slot = index & (CR-1)
-  static constexpr size_t smem = bytes(CR);
+  static constexpr size_t smem = sizeof(R) * ((size_t)kRing * 8 * kNT + (size_t)2 * T * 4 * (kNT / 32 + 2) + (size_t)T * kNT);
 };
 
 // Per-thread constants of a job of the streaming kernel.
@@ -188,10 +184,11 @@ struct JobCtx {
   R chx_i, chx_im1;
 };
 
-// What a thread keeps per pipeline stage: E, Hx, Hy, G of the row the stage holds.
+// What a thread keeps per pipeline stage: E, Hx, Hy, G and the four coefficients of the row the stage holds (the
+// coefficients travel down the pipeline with their row: registers only change names, nothing is copied or re-read).
 template <typename R, int T>
 struct Held {
-  R e[T], hx[T], hy[T], g[T];
+  R e[T], hx[T], hy[T], g[T], cP[T], cce[T], cka[T], cQ[T];
   R hxp_last;          // new Hx of the row before the one the LAST stage holds (for s < T-1 that value is hx[s+1])
 };
 
@@ -206,21 +203,16 @@ struct Held {
 //   XEDGE:           this warp holds column 0 or nx-1 (first-order Mur / conductor on the x edges).
 template <typename R, int T, bool SPECIAL, bool XEDGE>
 __device__ __forceinline__ void run_stages(const P2<R> &p, const Arrays<R> &a, const JobCtx<R> &c, const int Y, const uint32_t fq,
-                                           const int cbase, const R *cring, R *xbuf, R *xsb, Held<R, T> &h, Held<R, T> &n,
-                                           R &ein, R &hxin, R &hyin, R &gin) {
+                                           R *xbuf, R *xsb, Held<R, T> &h, Held<R, T> &n,
+                                           R &ein, R &hxin, R &hyin, R &gin, R &cPin, R &ccein, R &ckain, R &cQin) {
   typedef Ops<R> O;
   constexpr int XS = kNT / 32 + 2;     // exchange slots per stage: one per warp plus a zero slot at each end
-  constexpr int CR = K2Shape<R, T>::CR;
   const int tid = c.warp * 32 + c.lane;
   R gain[T], rest[T], hxq[T], hyn[T], gn[T];
   if (!SPECIAL) {
 #pragma unroll
     for (int s = 0; s < T; ++s) {        // everything that needs old values only
-      int slot = cbase - 1 - s;
-      if ((CR & (CR - 1)) == 0) slot &= CR - 1;
-      else if (slot < 0) slot += CR;
-      const R *cf = cring + slot * 4 * kNT + tid;
-      const R cP = cf[0], cce = cf[kNT], cka = cf[2 * kNT], cQ = cf[3 * kNT];
+      const R cP = h.cP[s], cce = h.cce[s], cka = h.cka[s], cQ = h.cQ[s];
       const R es = h.e[s];
       // neighbours across the warp edge come from the exchange buffer (slots of the strip's outer neighbours hold zeros);
       // branch-free, so that the whole path stays one block the compiler can interleave
@@ -256,18 +248,16 @@ __device__ __forceinline__ void run_stages(const P2<R> &p, const Arrays<R> &a, c
       }
       if (s == T - 1) n.hxp_last = hxn;
       n.e[s] = ein; n.hx[s] = hxin; n.hy[s] = hyin; n.g[s] = gin;
+      n.cP[s] = cPin; n.cce[s] = ccein; n.cka[s] = ckain; n.cQ[s] = cQin;
       ein = en; hxin = hxn; hyin = hyn[s]; gin = gn[s];
+      cPin = h.cP[s]; ccein = h.cce[s]; ckain = h.cka[s]; cQin = h.cQ[s];
     }
     return;
   }
 #pragma unroll
   for (int s = 0; s < T; ++s) {
     const int y = Y - 1 - s;
-    int slot = cbase - 1 - s;
-    if ((CR & (CR - 1)) == 0) slot &= CR - 1;
-    else if (slot < 0) slot += CR;
-    const R *cf = cring + slot * 4 * kNT + tid;
-    const R cP = cf[0], cce = cf[kNT], cka = cf[2 * kNT], cQ = cf[3 * kNT];
+    const R cP = h.cP[s], cce = h.cce[s], cka = h.cka[s], cQ = h.cQ[s];
     const bool yin = (y >= 0 && y <= p.ny - 2);
     const R es = h.e[s];
     const R *xl_ = xbuf + (s * XS + c.warp) * 4;
@@ -322,7 +312,9 @@ __device__ __forceinline__ void run_stages(const P2<R> &p, const Arrays<R> &a, c
     xsb[s * kNT + tid] = xs_new;
     if (s == T - 1) n.hxp_last = hxn;
     n.e[s] = ein; n.hx[s] = hxin; n.hy[s] = hyin; n.g[s] = gin;
+    n.cP[s] = cPin; n.cce[s] = ccein; n.cka[s] = ckain; n.cQ[s] = cQin;
     ein = en; hxin = hxn; hyin = hyn_s; gin = gn_s;
+    cPin = cP; ccein = cce; ckain = cka; cQin = cQ;
   }
 }
 
@@ -338,14 +330,12 @@ __device__ __forceinline__ void run_stages(const P2<R> &p, const Arrays<R> &a, c
 template <typename R, int T>
 __global__ void __launch_bounds__(kNT, 1) k2_2d(const P2<R> p, const Arrays<R> a) {
   constexpr int NW = kNT / 32;
-  constexpr int CR = K2Shape<R, T>::CR;
-  constexpr int FR = kFieldRing;
+  constexpr int FR = kRing;
   constexpr int XS = NW + 2;
   constexpr int XB = T * XS * 4;                              // one exchange buffer: [T][XS]{E31, Hy31, E0, -}, end slots zero
   extern __shared__ __align__(16) uint8_t smem_raw[];
-  R *fring = reinterpret_cast<R *>(smem_raw);                 // [FR][4][kNT]
-  R *cring = fring + FR * 4 * kNT;                            // [CR][4][kNT]
-  R *xch = cring + CR * 4 * kNT;                              // [2][XB]
+  R *fring = reinterpret_cast<R *>(smem_raw);                 // [FR][8][kNT]
+  R *xch = fring + FR * 8 * kNT;                              // [2][XB]
   R *xsb = xch + 2 * XB;                                      // [T][kNT]
   const int tid = threadIdx.x;
   JobCtx<R> c;
@@ -353,7 +343,6 @@ __global__ void __launch_bounds__(kNT, 1) k2_2d(const P2<R> p, const Arrays<R> a
   c.is_mur = (p.bc == RKETD2D_BC_MUR);
 
   for (int q = tid; q < 2 * XB; q += kNT) xch[q] = R(0);
-  for (int q = 0; q < CR * 4; ++q) cring[q * kNT + tid] = R(0);
 
   const int njobs = p.nstrips * p.nsegs;
   for (int job = blockIdx.x; job < njobs; job += gridDim.x) {
@@ -374,7 +363,7 @@ __global__ void __launch_bounds__(kNT, 1) k2_2d(const P2<R> p, const Arrays<R> a
 
     Held<R, T> hA, hB;
 #pragma unroll
-    for (int s = 0; s < T; ++s) hA.e[s] = hA.hx[s] = hA.hy[s] = hA.g[s] = R(0);
+    for (int s = 0; s < T; ++s) hA.e[s] = hA.hx[s] = hA.hy[s] = hA.g[s] = hA.cP[s] = hA.cce[s] = hA.cka[s] = hA.cQ[s] = R(0);
     hA.hxp_last = R(0);
     uint32_t fq = 0;
 
@@ -384,40 +373,41 @@ __global__ void __launch_bounds__(kNT, 1) k2_2d(const P2<R> p, const Arrays<R> a
       const int Y = ya + ridx;
       const bool valid = incol && Y >= 0 && Y < p.ny && ridx < niter;
       const int64_t idx = valid ? (int64_t)Y * p.pitch + i : 0;
-      R *fd = fring + (ridx % FR) * 4 * kNT + tid;
-      R *cd = cring + (ridx % CR) * 4 * kNT + tid;
+      R *fd = fring + (ridx % FR) * 8 * kNT + tid;
       cp_async_val(fd, a.E + idx, valid);
       cp_async_val(fd + kNT, a.Hx + idx, valid);
       cp_async_val(fd + 2 * kNT, a.Hy + idx, valid);
       cp_async_val(fd + 3 * kNT, a.G + idx, valid);
-      cp_async_val(cd, a.cP + idx, valid);
-      cp_async_val(cd + kNT, a.cce + idx, valid);
-      cp_async_val(cd + 2 * kNT, a.cka + idx, valid);
-      cp_async_val(cd + 3 * kNT, a.cQ + idx, valid);
+      cp_async_val(fd + 4 * kNT, a.cP + idx, valid);
+      cp_async_val(fd + 5 * kNT, a.cce + idx, valid);
+      cp_async_val(fd + 6 * kNT, a.cka + idx, valid);
+      cp_async_val(fd + 7 * kNT, a.cQ + idx, valid);
       cp_async_commit();
     };
 #pragma unroll
     for (int r = 0; r < kPF; ++r) issue_row(r);
 
     constexpr uint32_t kHeldMask = ((1u << T) - 1u) << 1;     // bits of the rows the T stages hold
-    int cbase = 0;                         // it % CR
+    uint32_t flag_next = (ya >= 0 && ya < p.ny) ? (uint32_t)(p.rowflag[ya] & RF_SPECIAL) : 0u;   // flag of the row entering next
 
     auto iteration = [&](const int it, Held<R, T> &h, Held<R, T> &n) {
       const int Y = ya + it;
       issue_row(it + kPF);
       cp_async_wait<kPF>();
       const bool special = ((fq << 1) & kHeldMask) != 0;       // the flag of row Y is not among the held rows yet
-      fq = (fq << 1) | ((Y >= 0 && Y < p.ny) ? (uint32_t)(p.rowflag[Y] & RF_SPECIAL) : 0u);
+      fq = (fq << 1) | flag_next;
+      flag_next = (Y + 1 >= 0 && Y + 1 < p.ny) ? (uint32_t)(p.rowflag[Y + 1] & RF_SPECIAL) : 0u;   // used one iteration later
       __syncthreads();                     // the warp-edge values posted at the end of the previous iteration
-      const R *fs = fring + (it % FR) * 4 * kNT + tid;
+      const R *fs = fring + (it % FR) * 8 * kNT + tid;
       R ein = fs[0], hxin = fs[kNT], hyin = fs[2 * kNT], gin = fs[3 * kNT];
+      R cPin = fs[4 * kNT], ccein = fs[5 * kNT], ckain = fs[6 * kNT], cQin = fs[7 * kNT];
       R *xbuf = xch + ((it + 1) & 1) * XB;                     // read buffer of this iteration
       if (special)
-        run_stages<R, T, true, true>(p, a, c, Y, fq, cbase, cring, xbuf, xsb, h, n, ein, hxin, hyin, gin);
+        run_stages<R, T, true, true>(p, a, c, Y, fq, xbuf, xsb, h, n, ein, hxin, hyin, gin, cPin, ccein, ckain, cQin);
       else if (xw)
-        run_stages<R, T, false, true>(p, a, c, Y, fq, cbase, cring, xbuf, xsb, h, n, ein, hxin, hyin, gin);
+        run_stages<R, T, false, true>(p, a, c, Y, fq, xbuf, xsb, h, n, ein, hxin, hyin, gin, cPin, ccein, ckain, cQin);
       else
-        run_stages<R, T, false, false>(p, a, c, Y, fq, cbase, cring, xbuf, xsb, h, n, ein, hxin, hyin, gin);
+        run_stages<R, T, false, false>(p, a, c, Y, fq, xbuf, xsb, h, n, ein, hxin, hyin, gin, cPin, ccein, ckain, cQin);
       {                                    // (ein, hxin, hyin, gin) is now row Y-T at level T
         const int y = Y - T;
         if (c.own_col && y >= c.y_out0 && y < c.y_out1) {
@@ -434,7 +424,6 @@ __global__ void __launch_bounds__(kNT, 1) k2_2d(const P2<R> p, const Arrays<R> a
 #pragma unroll
         for (int s = 0; s < T; ++s) xp[(s * XS + c.warp + 1) * 4 + 2] = n.e[s];
       }
-      cbase = (cbase + 1 == CR) ? 0 : cbase + 1;
     };
 
     // two register sets used alternately; an odd count runs one more iteration on a zero row, which stores nothing

@@ -97,7 +97,7 @@ def test_reduced_column_all_kernels(dtype):
 # sizes: one node inside; strips whose last column falls on lane 0 (57, 249, 265: the shifted last strip); a last strip
 # of one column (241); several strips and segments; rows fewer than the depth
 @pytest.mark.parametrize("nx,ny", [(3, 3), (4, 3), (3, 7), (5, 4), (33, 17), (57, 40), (249, 33), (241, 9), (265, 70),
-                                   (481, 5), (700, 333), (64, 1200)])
+                                   (481, 5), (700, 333), (64, 1200), (369, 9), (393, 70), (800, 40)])
 def test_ragged_sizes_mur(nx, ny):
     m = _mod()
     nsteps = 37
