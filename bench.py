@@ -303,9 +303,12 @@ def run_table2(args):
 # ---------------------------------------------------------------------------------------------------------------------
 # 2-D TMz workload: `--workload tm2d` (16384 x 16384 x 1000 steps) or tm2d:<nx>:<ny>:<nsteps>
 # ---------------------------------------------------------------------------------------------------------------------
-FP_INSTR_PER_CELL_STEP_2D = 11   # rketd2d.cu: Hx 2, Hy 2, Ez 5, G 2
+FP_INSTR_PER_CELL_STEP_2D = 13   # rketd2d.cu: Hx 2, Hy 2, Ez 7 (gain 1, rest 5, fma 1), G 2
 ARRAYS_PER_PASS_2D = 12          # read Ez, Hx, Hy, G, P, ce, ka, Q; write Ez, Hx, Hy, G
-NCU_TRAFFIC_BYTES_2D = {}        # (workload, dtype, depth) -> dram bytes per launch from the committed ncu capture
+NCU_TRAFFIC_BYTES_2D = {         # (workload, dtype, depth) -> dram bytes per launch from the committed ncu captures
+    ("tm2d_column_16384x16384", "f64", 8): 26.04e9,     # profiles/r01_ncu_full_k2_2d_f64.md (streaming kernel)
+    ("tm2d_column_16384x16384", "f64", 1): 25.79e9,     # same file, one-step kernel k1_2d
+}
 
 
 def cpu_baseline_2d(w, target_serial=4e8, target_omp=2.0e9):
@@ -424,7 +427,7 @@ def run_tm2d(args):
             "alu_frac": (value / world) * redundancy / r_alu,
             "note": "achieved = 12 arrays (read Ez,Hx,Hy,G,P,ce,ka,Q; write Ez,Hx,Hy,G) x nodes x esize per pass / mean "
                     "launch time; every byte serves depth_T steps; alu_frac counts the redundant halo work against "
-                    "148 SMs x lanes x max clock / 11 instr per cell-step"}
+                    "148 SMs x lanes x max clock / 13 instr per cell-step"}
     e2e = None
     if not args.no_e2e:
         wp_h, nu_h = torch.from_numpy(wp).pin_memory(), torch.from_numpy(nu).pin_memory()

@@ -652,7 +652,7 @@ template <typename R, int T>
 cudaError_t launch_k2_T(rketd2d_sim *s, P2<R> &p) {
   const Plan2 pl = make_plan(s, T);
   p.HP = pl.HP; p.Wv = pl.Wv; p.nstrips = pl.nstrips; p.nsegs = pl.nsegs; p.Sy = pl.Sy; p.dlast = pl.dlast;
-  s->ctr_strip = kNT; s->ctr_halo = pl.HP; s->ctr_seg = pl.Sy;
+  if (T == s->ctr_depth_used || s->ctr_strip == 0) { s->ctr_strip = kNT; s->ctr_halo = pl.HP; s->ctr_seg = pl.Sy; }   // the main passes, not a remainder pass
   constexpr size_t smem = K2Shape<R, T>::smem;
   static bool configured = false;
   if (!configured) {
