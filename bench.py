@@ -217,8 +217,20 @@ def run_reference(args):
         return
     import oracle
     oracle.build()
-    w = make_workload(args.workload)
     cores = os.cpu_count() or 1
+    if args.workload.startswith("tm2d"):          # 2-D TMz: a window of the grid around the source
+        w = make_workload_2d(args.workload)
+        steps, side = 100, min(w.nx, w.ny, 2048)
+        i0 = min(max(0, w.src_ij[0] - side // 2), w.nx - side)
+        j0 = min(max(0, w.src_ij[1] - side // 2), w.ny - side)
+        run = lambda: oracle.run_workload2d(w, nsteps=steps, window=(i0, i0 + side, j0, j0 + side), omp=True)
+        sample = (f"nodes {i0}..{i0 + side - 1} x {j0}..{j0 + side - 1} of the {w.nx} x {w.ny} grid x {steps} leapfrog steps "
+                  "per bench step")
+        units = side * side * steps
+        cfg = {"workload": w.name, "nx": w.nx, "ny": w.ny, "nsteps_per_run": w.nsteps,
+               "note": "CPU oracle (OpenMP build) on a bounded sample of the workload"}
+        return _reference_line(args, run, units, sample, cfg, cores)
+    w = make_workload(args.workload)
     if w.nbatch == 1:
         steps = 100
         cells = min(w.ncells, 1 << 22)
@@ -232,18 +244,23 @@ def run_reference(args):
         kw = dict(b0=0, b1=nb)
         sample = f"grids 0..{nb - 1} of {w.nbatch} x {w.ncells} nodes x {steps} leapfrog steps per bench step"
         units = nb * w.ncells * steps
+    cfg = {"workload": w.name, "ncells": w.ncells, "nbatch": w.nbatch, "nsteps_per_run": w.nsteps,
+           "note": "CPU oracle (OpenMP build) on a bounded sample of the workload"}
+    return _reference_line(args, lambda: oracle.run_workload(w, nsteps=steps, omp=True, **kw), units, sample, cfg, cores)
+
+
+def _reference_line(args, run, units, sample, cfg, cores):
     for _ in range(args.warmup):
-        oracle.run_workload(w, nsteps=steps, omp=True, **kw)
+        run()
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        oracle.run_workload(w, nsteps=steps, omp=True, **kw)
+        run()
     dt = time.perf_counter() - t0
     val = units * args.steps / dt / 1e9
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": w.name, "ncells": w.ncells, "nbatch": w.nbatch, "nsteps_per_run": w.nsteps,
-                       "note": "CPU oracle (OpenMP build) on a bounded sample of the workload"},
+            "config": cfg,
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}

@@ -149,6 +149,38 @@ def test_initial_fields_restart_and_anisotropic_steps():
     _check(g32, o, 1e-5)
 
 
+def test_fields_before_media_and_media_change_with_live_fields():
+    """The kernels carry G = cj Jz - cj kc Ez, which depends on the media: Jz given before the media, and a change of
+    media in the middle of a run, must both go through the physical Jz."""
+    m = _mod()
+    nx, ny = 120, 90
+    w = _edge_workload(nx, ny, 40)
+    wp, nu = w.media()
+    rng = np.random.default_rng(9)
+    E0 = 1e-3 * rng.uniform(-1, 1, (ny, nx)); J0 = 1e-2 * rng.uniform(-1, 1, (ny, nx)) * (wp > 0)
+    wp2, nu2 = wp * 0.5 + 1e10, nu * 2.0 + 1e9
+    kw = dict(src_kind=w.src_kind, src_params=w.src_params, src_ij=w.src_ij, probes=w.probes, boundary=w.boundary)
+    st = oracle.State2D(nx, ny, Ez0=E0, Jz0=J0)
+    r1, _ = oracle.run2d(st, wp, nu, w.dx, w.dy, w.dt, 25, **kw)
+    r2, _ = oracle.run2d(st, wp2, nu2, w.dx, w.dy, w.dt, 15, **kw)
+    sim = m.Sim2D(nx, ny, w.dx, w.dy, w.dt)
+    sim.set_fields(Ez=E0, Jz=J0)                       # before any media
+    sim.set_media(wp, nu)
+    sim.set_source(w.src_kind, w.src_params, *w.src_ij)
+    sim.set_probes(w.probes)
+    sim.run(25)
+    sim.set_media(wp2, nu2)                            # live fields
+    sim.run(15)
+    rec = sim.read_probes()
+    ref = np.concatenate([r1, r2], 1)
+    assert _err(rec, ref) <= 1e-12
+    for gf, of in zip(sim.get_fields(), (st.Ez, st.Hx, st.Hy, st.Jz)):
+        assert _err(gf, of) <= 1e-12
+    sim.reset()
+    assert not np.any(sim.get_fields()[0]) and sim.counter(m.CTR_STEPS_DONE) == 0
+    sim.close()
+
+
 def test_cavity_mode_on_the_gpu_follows_the_dispersion_recurrence():
     """Pin Q3 through the CUDA path: conducting box, one eigenmode, dx != dy."""
     m = _mod()
