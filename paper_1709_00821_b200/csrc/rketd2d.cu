@@ -37,7 +37,9 @@ namespace {
 
 constexpr int kMaxProbes2 = 64;
 constexpr int kMaxT = 16;
-constexpr int kNT = 256;       // threads per CTA of the streaming kernel = columns of a strip, one per thread
+// threads per CTA of the streaming kernel = columns of a strip, one per thread; as many as the registers of a depth allow
+template <typename R, int T> struct StripThreads { static constexpr int value = 256; };
+template <> struct StripThreads<float, 8> { static constexpr int value = 384; };   // 136 registers: 12 warps (394 against 338 Gcell/s with 8)
 constexpr int kPF = 3;         // rows in flight (cp.async) ahead of the row entering the pipeline
 constexpr int kK1Rows = 4;     // rows a K1 thread walks
 
@@ -173,7 +175,8 @@ __device__ __forceinline__ void st_pair(float *q, float x, float y) { *reinterpr
 constexpr int kRing = kPF + 1;      // entry ring: rows Y .. Y+kPF, 8 arrays each (Ez, Hx, Hy, G, P, ce, ka, Q)
 template <typename R, int T>
 struct K2Shape {
-  static constexpr size_t smem = sizeof(R) * ((size_t)kRing * 8 * kNT + (size_t)2 * T * 4 * (kNT / 32 + 2) + (size_t)T * kNT);
+  static constexpr int NT = StripThreads<R, T>::value;
+  static constexpr size_t smem = sizeof(R) * ((size_t)kRing * 8 * NT + (size_t)2 * T * 4 * (NT / 32 + 2) + (size_t)T * NT);
 };
 
 // Per-thread constants of a job of the streaming kernel.
@@ -197,7 +200,7 @@ struct Held {
 //   SPECIAL = false: none of the rows held by the stages is row 0, 1, ny-2, ny-1, the source row or a probe row.
 //                    Everything that does not need the row above is computed for all stages first (shuffles, new Hy,
 //                    new G, gain and rest of Ez'); what is left is one fma per stage along the pipeline.
-//   SPECIAL = true:  stage by stage, with the y edges, the source and the probes; `xsb` (shared memory, [T][kNT]) keeps
+//   SPECIAL = true:  stage by stage, with the y edges, the source and the probes; `xsb` (shared memory, [T][NT]) keeps
 //                    one spare value per stage across iterations: the old E of the row before (needed on row 1 for the
 //                    Mur value of row 0) or, on row ny-1, the edge value computed one iteration earlier.
 //   XEDGE:           this warp holds column 0 or nx-1 (first-order Mur / conductor on the x edges).
@@ -206,7 +209,8 @@ __device__ __forceinline__ void run_stages(const P2<R> &p, const Arrays<R> &a, c
                                            R *xbuf, R *xsb, Held<R, T> &h, Held<R, T> &n,
                                            R &ein, R &hxin, R &hyin, R &gin, R &cPin, R &ccein, R &ckain, R &cQin) {
   typedef Ops<R> O;
-  constexpr int XS = kNT / 32 + 2;     // exchange slots per stage: one per warp plus a zero slot at each end
+  constexpr int NT = StripThreads<R, T>::value;
+  constexpr int XS = NT / 32 + 2;     // exchange slots per stage: one per warp plus a zero slot at each end
   const int tid = c.warp * 32 + c.lane;
   R gain[T], rest[T], hxq[T], hyn[T], gn[T];
   if (!SPECIAL) {
@@ -285,7 +289,7 @@ __device__ __forceinline__ void run_stages(const P2<R> &p, const Arrays<R> &a, c
     }
     if ((fq >> (s + 1)) & 1u) {          // CTA-uniform
       const bool own = c.own_col && y >= c.y_out0 && y < c.y_out1;
-      const R xs = xsb[s * kNT + tid];
+      const R xs = xsb[s * NT + tid];
       if (y == p.ny - 1) en = xs;        // computed one iteration ago from rows ny-2 (new) and ny-1 (old)
       if (y == 0) en = R(0);             // set one iteration later, when E'[1] exists
       if (y == p.ny - 2) xs_new = (c.xin && c.is_mur) ? O::mur(p.my, es, en, ein) : R(0);
@@ -309,7 +313,7 @@ __device__ __forceinline__ void run_stages(const P2<R> &p, const Arrays<R> &a, c
         for (int q = 0; q < p.nprobes; ++q)
           if (p.probe_j[q] == y && p.probe_i[q] == c.i) p.rec[(int64_t)q * p.rec_stride + p.n0 + s] = en;
     }
-    xsb[s * kNT + tid] = xs_new;
+    xsb[s * NT + tid] = xs_new;
     if (s == T - 1) n.hxp_last = hxn;
     n.e[s] = ein; n.hx[s] = hxin; n.hy[s] = hyin; n.g[s] = gin;
     n.cP[s] = cPin; n.cce[s] = ccein; n.cka[s] = ckain; n.cQ[s] = cQin;
@@ -318,7 +322,7 @@ __device__ __forceinline__ void run_stages(const P2<R> &p, const Arrays<R> &a, c
   }
 }
 
-// Streaming temporal blocking.  Job = (strip of kNT columns, halo HP (+ dlast) on each side) x (segment of Sy rows, T
+// Streaming temporal blocking.  Job = (strip of NT columns, halo HP (+ dlast) on each side) x (segment of Sy rows, T
 // halo rows on each side).  Iteration `it` lets row Y = ya + it enter; stage s (s = 0..T-1) then holds row Y-1-s at
 // level s (E, G at step n0+s, H half a step earlier) in registers, receives row Y-s at level s from stage s-1 (from
 // shared memory for s = 0), and produces level s+1 of its held row, which is what stage s+1 receives.  The last stage
@@ -328,21 +332,22 @@ __device__ __forceinline__ void run_stages(const P2<R> &p, const Arrays<R> &a, c
 // shuffle; between warps old E and old Hy of the warp-edge columns are posted to shared memory at the end of an
 // iteration (one CTA barrier per row).
 template <typename R, int T>
-__global__ void __launch_bounds__(kNT, 1) k2_2d(const P2<R> p, const Arrays<R> a) {
-  constexpr int NW = kNT / 32;
+__global__ void __launch_bounds__(StripThreads<R, T>::value, 1) k2_2d(const P2<R> p, const Arrays<R> a) {
+  constexpr int NT = StripThreads<R, T>::value;
+  constexpr int NW = NT / 32;
   constexpr int FR = kRing;
   constexpr int XS = NW + 2;
   constexpr int XB = T * XS * 4;                              // one exchange buffer: [T][XS]{E31, Hy31, E0, -}, end slots zero
   extern __shared__ __align__(16) uint8_t smem_raw[];
-  R *fring = reinterpret_cast<R *>(smem_raw);                 // [FR][8][kNT]
-  R *xch = fring + FR * 8 * kNT;                              // [2][XB]
-  R *xsb = xch + 2 * XB;                                      // [T][kNT]
+  R *fring = reinterpret_cast<R *>(smem_raw);                 // [FR][8][NT]
+  R *xch = fring + FR * 8 * NT;                              // [2][XB]
+  R *xsb = xch + 2 * XB;                                      // [T][NT]
   const int tid = threadIdx.x;
   JobCtx<R> c;
   c.lane = tid & 31; c.warp = tid >> 5;
   c.is_mur = (p.bc == RKETD2D_BC_MUR);
 
-  for (int q = tid; q < 2 * XB; q += kNT) xch[q] = R(0);
+  for (int q = tid; q < 2 * XB; q += NT) xch[q] = R(0);
 
   const int njobs = p.nstrips * p.nsegs;
   for (int job = blockIdx.x; job < njobs; job += gridDim.x) {
@@ -373,15 +378,15 @@ __global__ void __launch_bounds__(kNT, 1) k2_2d(const P2<R> p, const Arrays<R> a
       const int Y = ya + ridx;
       const bool valid = incol && Y >= 0 && Y < p.ny && ridx < niter;
       const int64_t idx = valid ? (int64_t)Y * p.pitch + i : 0;
-      R *fd = fring + (ridx % FR) * 8 * kNT + tid;
+      R *fd = fring + (ridx % FR) * 8 * NT + tid;
       cp_async_val(fd, a.E + idx, valid);
-      cp_async_val(fd + kNT, a.Hx + idx, valid);
-      cp_async_val(fd + 2 * kNT, a.Hy + idx, valid);
-      cp_async_val(fd + 3 * kNT, a.G + idx, valid);
-      cp_async_val(fd + 4 * kNT, a.cP + idx, valid);
-      cp_async_val(fd + 5 * kNT, a.cce + idx, valid);
-      cp_async_val(fd + 6 * kNT, a.cka + idx, valid);
-      cp_async_val(fd + 7 * kNT, a.cQ + idx, valid);
+      cp_async_val(fd + NT, a.Hx + idx, valid);
+      cp_async_val(fd + 2 * NT, a.Hy + idx, valid);
+      cp_async_val(fd + 3 * NT, a.G + idx, valid);
+      cp_async_val(fd + 4 * NT, a.cP + idx, valid);
+      cp_async_val(fd + 5 * NT, a.cce + idx, valid);
+      cp_async_val(fd + 6 * NT, a.cka + idx, valid);
+      cp_async_val(fd + 7 * NT, a.cQ + idx, valid);
       cp_async_commit();
     };
 #pragma unroll
@@ -398,9 +403,9 @@ __global__ void __launch_bounds__(kNT, 1) k2_2d(const P2<R> p, const Arrays<R> a
       fq = (fq << 1) | flag_next;
       flag_next = (Y + 1 >= 0 && Y + 1 < p.ny) ? (uint32_t)(p.rowflag[Y + 1] & RF_SPECIAL) : 0u;   // used one iteration later
       __syncthreads();                     // the warp-edge values posted at the end of the previous iteration
-      const R *fs = fring + (it % FR) * 8 * kNT + tid;
-      R ein = fs[0], hxin = fs[kNT], hyin = fs[2 * kNT], gin = fs[3 * kNT];
-      R cPin = fs[4 * kNT], ccein = fs[5 * kNT], ckain = fs[6 * kNT], cQin = fs[7 * kNT];
+      const R *fs = fring + (it % FR) * 8 * NT + tid;
+      R ein = fs[0], hxin = fs[NT], hyin = fs[2 * NT], gin = fs[3 * NT];
+      R cPin = fs[4 * NT], ccein = fs[5 * NT], ckain = fs[6 * NT], cQin = fs[7 * NT];
       R *xbuf = xch + ((it + 1) & 1) * XB;                     // read buffer of this iteration
       if (special)
         run_stages<R, T, true, true>(p, a, c, Y, fq, xbuf, xsb, h, n, ein, hxin, hyin, gin, cPin, ccein, ckain, cQin);
@@ -433,7 +438,7 @@ __global__ void __launch_bounds__(kNT, 1) k2_2d(const P2<R> p, const Arrays<R> a
     }
     cp_async_wait<0>();
     __syncthreads();
-    for (int q = tid; q < 2 * XB; q += kNT) xch[q] = R(0);
+    for (int q = tid; q < 2 * XB; q += NT) xch[q] = R(0);
   }
 }
 
@@ -592,10 +597,10 @@ int build_rowflags(rketd2d_sim *s) {
 }
 
 // strips and segments of the streaming kernel for depth T
-Plan2 make_plan(const rketd2d_sim *s, int T) {
+Plan2 make_plan(const rketd2d_sim *s, int T, int NT) {
   Plan2 pl;
   pl.HP = std::max(8, (T + 7) / 8 * 8);
-  pl.Wv = kNT - 2 * pl.HP;
+  pl.Wv = NT - 2 * pl.HP;
   while ((s->nx % pl.Wv) == 1 && pl.Wv > 16) pl.Wv -= 8;      // the last strip owns at least two columns (x Mur)
   pl.nstrips = (s->nx + pl.Wv - 1) / pl.Wv;
   const int x0_last = (pl.nstrips - 1) * pl.Wv - pl.HP;
@@ -650,9 +655,10 @@ Arrays<R> arrays_of(const rketd2d_sim *s) {
 
 template <typename R, int T>
 cudaError_t launch_k2_T(rketd2d_sim *s, P2<R> &p) {
-  const Plan2 pl = make_plan(s, T);
+  constexpr int NT = StripThreads<R, T>::value;
+  const Plan2 pl = make_plan(s, T, NT);
   p.HP = pl.HP; p.Wv = pl.Wv; p.nstrips = pl.nstrips; p.nsegs = pl.nsegs; p.Sy = pl.Sy; p.dlast = pl.dlast;
-  if (T == s->ctr_depth_used || s->ctr_strip == 0) { s->ctr_strip = kNT; s->ctr_halo = pl.HP; s->ctr_seg = pl.Sy; }   // the main passes, not a remainder pass
+  if (T == s->ctr_depth_used || s->ctr_strip == 0) { s->ctr_strip = NT; s->ctr_halo = pl.HP; s->ctr_seg = pl.Sy; }   // the main passes, not a remainder pass
   constexpr size_t smem = K2Shape<R, T>::smem;
   static bool configured = false;
   if (!configured) {
@@ -661,7 +667,7 @@ cudaError_t launch_k2_T(rketd2d_sim *s, P2<R> &p) {
     configured = true;
   }
   const int grid = pl.nstrips * pl.nsegs;
-  k2_2d<R, T><<<grid, kNT, smem, s->stream>>>(p, arrays_of<R>(s));
+  k2_2d<R, T><<<grid, NT, smem, s->stream>>>(p, arrays_of<R>(s));
   return cudaGetLastError();
 }
 
@@ -671,6 +677,7 @@ cudaError_t launch_k2(rketd2d_sim *s, P2<R> &p, int T) {
     case 1: return launch_k2_T<R, 1>(s, p);
     case 2: return launch_k2_T<R, 2>(s, p);
     case 4: return launch_k2_T<R, 4>(s, p);
+    case 6: return launch_k2_T<R, 6>(s, p);
     case 8: return launch_k2_T<R, 8>(s, p);
     case 16: if (sizeof(R) == 4) return launch_k2_T<float, 16>(s, reinterpret_cast<P2<float> &>(p)); break;
   }
@@ -680,15 +687,18 @@ cudaError_t launch_k2(rketd2d_sim *s, P2<R> &p, int T) {
 template <typename R>
 int run_typed(rketd2d_sim *s, int64_t nsteps, void *rec) {
   const bool stream_kernel = s->plan_kernel != RKETD2D_KERNEL_STEP;
-  const int Tdef = s->plan_depth > 0 ? s->plan_depth : (s->dtype == RKETD_F64 ? 8 : 16);
+  const int Tdef = s->plan_depth > 0 ? s->plan_depth : 8;
   s->ctr_kernel_used = stream_kernel ? RKETD2D_KERNEL_STREAM : RKETD2D_KERNEL_STEP;
   s->ctr_depth_used = stream_kernel ? Tdef : 1;
   int64_t done = 0;
   while (done < nsteps) {
     int T = 1;
     if (stream_kernel) {
-      T = Tdef;
-      while ((int64_t)T > nsteps - done) T >>= 1;
+      const int depths[6] = {16, 8, 6, 4, 2, 1};       // the chosen depth, then what fits the remainder
+      for (int q = 0; q < 6; ++q) {
+        T = depths[q];
+        if (T <= Tdef && (int64_t)T <= nsteps - done && (T != 6 || Tdef == 6)) break;
+      }
     }
     P2<R> p;
     fill_params<R>(s, p, rec, nsteps, done, T);
@@ -896,8 +906,8 @@ int rketd2d_reset(rketd2d_sim *s) {
 int rketd2d_set_plan(rketd2d_sim *s, int kernel, int depth) {
   if (!s) return RKETD_EINVAL;
   if (kernel < RKETD2D_KERNEL_AUTO || kernel > RKETD2D_KERNEL_STREAM) return fail2(s, RKETD_EINVAL, "unknown kernel");
-  if (depth != 0 && depth != 1 && depth != 2 && depth != 4 && depth != 8 && depth != 16)
-    return fail2(s, RKETD_EINVAL, "depth must be 0, 1, 2, 4, 8 or 16");
+  if (depth != 0 && depth != 1 && depth != 2 && depth != 4 && depth != 6 && depth != 8 && depth != 16)
+    return fail2(s, RKETD_EINVAL, "depth must be 0, 1, 2, 4, 6, 8 or 16");
   if (depth == 16 && s->dtype == RKETD_F64) return fail2(s, RKETD_EINVAL, "depth 16 is for fp32 (registers and shared memory)");
   s->plan_kernel = kernel;
   s->plan_depth = depth;
