@@ -84,6 +84,10 @@ int rketd2d_get_fields(rketd2d_sim *s, void *Ez, void *Hx, void *Hy, void *Jz);
 /* Fields zero, step counter 0, records discarded; media, source, probes, boundary kept. */
 int rketd2d_reset(rketd2d_sim *s);
 
+/* Drop the probe records gathered so far (their device buffers are freed); fields, step counter, media, source and
+ * probes are kept.  The next rketd2d_run starts a fresh record.  Synchronises. */
+int rketd2d_discard_records(rketd2d_sim *s);
+
 /* Kernel (RKETD2D_KERNEL_*) and, for the streaming kernel, the temporal depth T in {1, 2, 4, 6, 8} or, fp32 only, 16
  * (0 = default: 8).  All choices compute identical bits.  EINVAL otherwise. */
 int rketd2d_set_plan(rketd2d_sim *s, int kernel, int depth);

@@ -903,6 +903,13 @@ int rketd2d_reset(rketd2d_sim *s) {
   return RKETD_OK;
 }
 
+int rketd2d_discard_records(rketd2d_sim *s) {
+  if (!s) return RKETD_EINVAL;
+  CU_TRY2(s, cudaStreamSynchronize(s->stream));
+  discard_records2(s);
+  return RKETD_OK;
+}
+
 int rketd2d_set_plan(rketd2d_sim *s, int kernel, int depth) {
   if (!s) return RKETD_EINVAL;
   if (kernel < RKETD2D_KERNEL_AUTO || kernel > RKETD2D_KERNEL_STREAM) return fail2(s, RKETD_EINVAL, "unknown kernel");

@@ -19,8 +19,8 @@ CTR_LAUNCHES, CTR_STEP_LAUNCHES, CTR_KERNEL_USED, CTR_DEPTH_USED, CTR_STEPS_DONE
 
 EXPORTS = ["rketd2d_create", "rketd2d_set_media", "rketd2d_set_boundary", "rketd2d_set_source", "rketd2d_set_probes",
            "rketd2d_set_fields", "rketd2d_get_fields", "rketd2d_reset", "rketd2d_set_plan", "rketd2d_run",
-           "rketd2d_read_probes", "rketd2d_get_kernel_coefficients", "rketd2d_get_counter", "rketd2d_destroy",
-           "rketd2d_last_error"]
+           "rketd2d_read_probes", "rketd2d_get_kernel_coefficients", "rketd2d_discard_records", "rketd2d_get_counter",
+           "rketd2d_destroy", "rketd2d_last_error"]
 
 _lib.rketd2d_create.argtypes = [ctypes.POINTER(_vp), _i64, _i64, _dbl, _dbl, _dbl, _i32, _vp]
 _lib.rketd2d_set_media.argtypes = [_vp, _vp, _vp]
@@ -30,6 +30,7 @@ _lib.rketd2d_set_probes.argtypes = [_vp, _vp, _i32]
 _lib.rketd2d_set_fields.argtypes = [_vp, _vp, _vp, _vp, _vp]
 _lib.rketd2d_get_fields.argtypes = [_vp, _vp, _vp, _vp, _vp]
 _lib.rketd2d_reset.argtypes = [_vp]
+_lib.rketd2d_discard_records.argtypes = [_vp]
 _lib.rketd2d_set_plan.argtypes = [_vp, _i32, _i32]
 _lib.rketd2d_run.argtypes = [_vp, _i64]
 _lib.rketd2d_read_probes.argtypes = [_vp, _vp, _i64, ctypes.POINTER(_i64)]
@@ -40,7 +41,7 @@ _lib.rketd2d_destroy.argtypes = [_vp]
 _lib.rketd2d_destroy.restype = None
 _lib.rketd2d_last_error.argtypes = [_vp]
 _lib.rketd2d_last_error.restype = ctypes.c_char_p
-for _n in EXPORTS[:12]:
+for _n in EXPORTS[:13]:
     getattr(_lib, _n).restype = _i32
 
 
@@ -84,6 +85,10 @@ def rketd2d_get_fields(h, Ez=None, Hx=None, Hy=None, Jz=None):
 
 def rketd2d_reset(h):
     _check(h, _lib.rketd2d_reset(h))
+
+
+def rketd2d_discard_records(h):
+    _check(h, _lib.rketd2d_discard_records(h))
 
 
 def rketd2d_set_plan(h, kernel: int = KERNEL_AUTO, depth: int = 0):
@@ -149,6 +154,7 @@ class Sim2D:
 
     def set_fields(self, Ez=None, Hx=None, Hy=None, Jz=None): rketd2d_set_fields(self.h, Ez, Hx, Hy, Jz)
     def reset(self): rketd2d_reset(self.h)
+    def discard_records(self): rketd2d_discard_records(self.h)
     def set_plan(self, kernel=KERNEL_AUTO, depth=0): rketd2d_set_plan(self.h, kernel, depth)
     def run(self, nsteps): rketd2d_run(self.h, nsteps)
     def counter(self, which): return rketd2d_get_counter(self.h, which)

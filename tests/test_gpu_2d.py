@@ -176,6 +176,9 @@ def test_fields_before_media_and_media_change_with_live_fields():
     assert _err(rec, ref) <= 1e-12
     for gf, of in zip(sim.get_fields(), (st.Ez, st.Hx, st.Hy, st.Jz)):
         assert _err(gf, of) <= 1e-12
+    sim.discard_records()
+    sim.run(3)
+    assert sim.read_probes().shape == (len(w.probes), 3) and sim.counter(m.CTR_STEPS_DONE) == 43
     sim.reset()
     assert not np.any(sim.get_fields()[0]) and sim.counter(m.CTR_STEPS_DONE) == 0
     sim.close()
