@@ -261,8 +261,8 @@ def test_error_codes_2d():
 
 
 # ----------------------------------------------------------------------------- the size bench.py times
-@pytest.mark.parametrize("dtype", ["f64", "f32"])
-def test_full_size_sampled_against_windowed_oracle(dtype):
+@pytest.mark.parametrize("dtype,kernel", [("f64", 2), ("f32", 2), ("f64", 1)])
+def test_full_size_sampled_against_windowed_oracle(dtype, kernel):
     """16384 x 16384 nodes, the launch configuration bench.py times (streaming kernel, default depth); every probe is
     compared with an oracle run on the window of nodes that can influence it (pin Q7: bit-exact domain of dependence)."""
     import torch
@@ -276,10 +276,11 @@ def test_full_size_sampled_against_windowed_oracle(dtype):
     sim.set_fields(Ez=np.ascontiguousarray(w.initial_E(), sim.np_dtype))
     sim.set_source(w.src_kind, w.src_params, *w.src_ij)
     sim.set_probes(w.probes)
+    sim.set_plan(kernel, 0)                                  # 2: the streaming kernel at its default depth; 1: one launch per step
     sim.run(nsteps)
     rec = sim.read_probes().astype(np.float64)
-    assert sim.counter(m.CTR_KERNEL_USED) == m.KERNEL_STREAM
-    assert sim.counter(m.CTR_DEPTH_USED) == 8
+    assert sim.counter(m.CTR_KERNEL_USED) == kernel
+    assert sim.counter(m.CTR_DEPTH_USED) == (8 if kernel == m.KERNEL_STREAM else 1)
     sim.close()
     torch.cuda.empty_cache()
     peak = 0.0
