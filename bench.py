@@ -325,6 +325,7 @@ ARRAYS_PER_PASS_2D = 12          # read Ez, Hx, Hy, G, P, ce, ka, Q; write Ez, H
 NCU_TRAFFIC_BYTES_2D = {         # (workload, dtype, depth) -> dram bytes per launch from the committed ncu captures
     ("tm2d_column_16384x16384", "f64", 8): 26.04e9,     # profiles/r01_ncu_full_k2_2d_f64.md (streaming kernel)
     ("tm2d_column_16384x16384", "f64", 1): 25.79e9,     # same file, one-step kernel k1_2d
+    ("tm2d_column_16384x16384", "f32", 8): 12.99e9,     # profiles/r01_ncu_full_k2_2d_f32.md
 }
 
 
