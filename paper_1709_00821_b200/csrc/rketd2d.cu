@@ -393,15 +393,16 @@ __global__ void __launch_bounds__(StripThreads<R, T>::value, 1) k2_2d(const P2<R
     for (int r = 0; r < kPF; ++r) issue_row(r);
 
     constexpr uint32_t kHeldMask = ((1u << T) - 1u) << 1;     // bits of the rows the T stages hold
-    uint32_t flag_next = (ya >= 0 && ya < p.ny) ? (uint32_t)(p.rowflag[ya] & RF_SPECIAL) : 0u;   // flag of the row entering next
+    // flag byte of the row entering next: loaded one iteration ahead and left untouched until then (no instruction waits on the load)
+    uint32_t raw_next = p.rowflag[min(max(ya, 0), p.ny - 1)];
 
     auto iteration = [&](const int it, Held<R, T> &h, Held<R, T> &n) {
       const int Y = ya + it;
       issue_row(it + kPF);
       cp_async_wait<kPF>();
       const bool special = ((fq << 1) & kHeldMask) != 0;       // the flag of row Y is not among the held rows yet
-      fq = (fq << 1) | flag_next;
-      flag_next = (Y + 1 >= 0 && Y + 1 < p.ny) ? (uint32_t)(p.rowflag[Y + 1] & RF_SPECIAL) : 0u;   // used one iteration later
+      fq = (fq << 1) | ((Y >= 0 && Y < p.ny) ? (raw_next & (uint32_t)RF_SPECIAL) : 0u);
+      raw_next = p.rowflag[min(max(Y + 1, 0), p.ny - 1)];
       __syncthreads();                     // the warp-edge values posted at the end of the previous iteration
       const R *fs = fring + (it % FR) * 8 * NT + tid;
       R ein = fs[0], hxin = fs[NT], hyin = fs[2 * NT], gin = fs[3 * NT];
