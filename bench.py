@@ -45,9 +45,11 @@ if ROOT not in sys.path:
 METRIC = "cell-updates/sec"
 UNIT = "Gcell/s"
 FALLBACK_HBM_GBS = 6650.0     # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
-FP64_LANES_PER_SM = 64        # DFMA per SM per clock (B200: 40 TFLOP/s fp64 / 148 SMs / 1.965 GHz / 2)
-FP32_LANES_PER_SM = 128
 FP_INSTR_PER_CELL_STEP = 7    # kernel form (rketd_device.cuh): H 2, E 3, G 2  (SURVEY §8(d) counts 9 for the plain form)
+# The "alu" ceilings are MEASURED in the same run by rketd_measure_peak (csrc/rketd_peaks.cu; a recorded run with clocks
+# and power is profiles/r02_peaks.md): the best FMA issue rate of the dtype in lanes per clock and SM x SMs x the clock
+# that microbenchmark held / 7 instructions per cell-step; beside it the issue ceiling of the stencil's own instruction
+# mix (register operands as in the kernels, no shuffles, no memory).
 ARRAYS_PER_PASS = 10          # read E, H, G, P, ch, ka, Q; write E, H, G
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` captures (profiles/*.md name the command); key = (workload, dtype, depth T, K2 variant)
@@ -158,6 +160,23 @@ def measured_peaks():
             d = json.load(fh)
         return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, torch copy)", float(d.get("sm_max_mhz", 1965.0))
     return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)", 1965.0
+
+
+_ALU_CACHE = {}
+
+
+def measured_alu(dtype: str, stream: int):
+    """live microbenchmarks (a few ms each), once per dtype and process"""
+    if dtype not in _ALU_CACHE:
+        from paper_1709_00821_b200 import peaks
+        _ALU_CACHE[dtype] = peaks.alu_peaks(dtype, stream)
+    return _ALU_CACHE[dtype]
+
+
+def alu_source(a) -> str:
+    return (f"measured live (rketd_measure_peak): {a['fma_best_form']} = {a['fma_lanes_per_clk_sm'][a['fma_best_form'].split('_', 1)[1]]} "
+            f"lanes/clk/SM x {a['sms']} SMs x {a['fma_sm_mhz']} MHz / {FP_INSTR_PER_CELL_STEP} instr per cell-step; "
+            "recorded run: profiles/r02_peaks.md")
 
 
 def cpu_baseline(w, target_updates_serial=6e8, target_updates_omp=2.5e9):
@@ -429,8 +448,8 @@ def run_tm2d(args):
     hbm_gbs, peak_src, sm_max = measured_peaks()
     nodes = w.nx * w.ny
     ms_per_launch = ms / max(1, step_launches)
-    lanes = FP64_LANES_PER_SM if args.dtype == "f64" else FP32_LANES_PER_SM
-    r_alu = 148 * lanes * (sm_max * 1e6) / FP_INSTR_PER_CELL_STEP_2D / 1e9
+    alu = measured_alu(args.dtype, stream.cuda_stream)
+    r_alu = alu["fma_peak_gcells"] * FP_INSTR_PER_CELL_STEP / FP_INSTR_PER_CELL_STEP_2D
     r_hbm1 = hbm_gbs / (ARRAYS_PER_PASS_2D * esize)
     alg_bytes = ARRAYS_PER_PASS_2D * esize * nodes
     achieved = alg_bytes / (ms_per_launch * 1e-3) / 1e9
@@ -442,10 +461,10 @@ def run_tm2d(args):
             "algorithmic_bytes_per_launch": alg_bytes, "ms_per_launch": ms_per_launch, "depth_T": int(depth),
             "strip_cols": int(strip), "halo_cols": int(halo), "segment_rows": int(seg),
             "frac_vs_8TBps_nominal": achieved / 8000.0, "gcells_vs_one_step_hbm_roofline": value / world / r_hbm1,
-            "alu_frac": (value / world) * redundancy / r_alu,
+            "alu_frac": (value / world) * redundancy / r_alu, "alu_peak": r_alu, "alu_peak_source": alu_source(alu).replace("/ 7 instr", "/ 13 instr"),
             "note": "achieved = 12 arrays (read Ez,Hx,Hy,G,P,ce,ka,Q; write Ez,Hx,Hy,G) x nodes x esize per pass / mean "
                     "launch time; every byte serves depth_T steps; alu_frac counts the redundant halo work against "
-                    "148 SMs x lanes x max clock / 13 instr per cell-step"}
+                    "the measured FMA issue peak / 13 instr per cell-step"}
     e2e = None
     if not args.no_e2e:
         wp_h, nu_h = torch.from_numpy(wp).pin_memory(), torch.from_numpy(nu).pin_memory()
@@ -490,6 +509,103 @@ def run_tm2d(args):
         dist.destroy_process_group()
 
 
+def roofline_1d(rketd, w, dtype, gcells, ms, step_launches, kernel_used, depth, tile_cells, halo_cells, variant, stream):
+    """roofline object of the stencil kernel a 1-D run used (gcells: per-GPU Gcell/s of the timed region, ms: its length)"""
+    esize = 8 if dtype == "f64" else 4
+    hbm_gbs, peak_src, _ = measured_peaks()
+    alu = measured_alu(dtype, stream)
+    r_alu = alu["fma_peak_gcells"]
+    ncell_total = w.ncells * w.nbatch
+    ms_per_launch = ms / max(1, step_launches)             # launches are back to back on one stream
+    r_hbm1 = hbm_gbs / (ARRAYS_PER_PASS * esize)           # Gcell/s, one step per pass
+    redundancy = tile_cells / max(1, tile_cells - 2 * halo_cells) if halo_cells else 1.0
+    if kernel_used == rketd.KERNEL_RESIDENT:
+        return {"bound": "alu", "achieved": gcells, "peak": r_alu, "unit": UNIT, "frac": gcells / r_alu,
+                "traffic": None, "peak_source": alu_source(alu),
+                "fma_lanes_per_clk_sm": alu["fma_lanes_per_clk_sm"],
+                "mix_peak": alu["mix_peak_gcells"], "frac_of_mix_peak": gcells * redundancy / alu["mix_peak_gcells"],
+                "halo_redundancy": redundancy, "depth_T": int(depth),
+                "note": "grid resident on chip for the whole run: HBM traffic is setup + probe records only; peak = best "
+                        "measured FMA issue rate / 7 instr per cell-step; mix_peak = measured issue ceiling of the "
+                        "stencil's own instruction mix (no shuffles, no memory), frac_of_mix_peak counts the redundant "
+                        "halo work too"}
+    alg_bytes = ARRAYS_PER_PASS * esize * ncell_total                                        # per launch (one pass)
+    achieved = alg_bytes / (ms_per_launch * 1e-3) / 1e9
+    variant_used = variant if variant >= 0 else 6
+    return {"bound": "hbm", "achieved": achieved, "peak": hbm_gbs, "unit": "GB/s", "frac": achieved / hbm_gbs,
+            "traffic": NCU_TRAFFIC_BYTES.get((w.name, dtype, int(depth), variant_used)), "peak_source": peak_src,
+            "algorithmic_bytes_per_launch": alg_bytes, "ms_per_launch": ms_per_launch,
+            "depth_T": int(depth), "tile_cells": int(tile_cells), "halo_cells": int(halo_cells),
+            "frac_vs_8TBps_nominal": achieved / 8000.0,
+            "gcells_vs_one_step_hbm_roofline": gcells / r_hbm1,
+            "alu_frac": gcells * redundancy / r_alu, "alu_peak": r_alu, "alu_peak_source": alu_source(alu),
+            "alu_frac_of_mix_peak": gcells * redundancy / alu["mix_peak_gcells"],
+            "note": "achieved = 10 arrays (read E,H,G,P,ch,ka,Q; write E,H,G) x nodes x esize per pass / mean launch "
+                    "time; every byte serves depth_T steps; alu_frac counts the redundant halo work against the "
+                    "measured FMA issue peak / 7 instr per cell-step"}
+
+
+def extra_configs(rketd, stream, host_inputs):
+    """The other (config, dtype) figures of DESIGN.md §8 in the same driver-visible JSON line: 1 warm-up + 2 timed runs
+    each (5 for the tiny config 1), CUDA events on the library's stream, inputs resident in HBM.  host_inputs: workload
+    name -> (wp, nu, E0) host arrays already generated for the headline."""
+    import torch
+    out = {}
+    jobs = [("config2", "f64", 0), ("config3", "f64", 0), ("config5", "f64", 0), ("config5", "f32", 0), ("config4", "f32", 0),
+            ("config4", "f64", 24), ("config1", "f64", 0)]
+    for name, dtype, depth in jobs:
+        key = f"{name}/{dtype}" + (f"/T{depth}" if depth else "")
+        try:
+            w = make_workload(name)
+            npdt = np.float64 if dtype == "f64" else np.float32
+            if name not in host_inputs:
+                host_inputs.clear()                       # one workload's inputs at a time
+                host_inputs[name] = w.media_full() + (w.initial_E_full(),)
+            wp, nu, E0 = host_inputs[name]
+            sim = rketd.Sim(w.ncells, w.nbatch, w.dz, w.dt, dtype, stream=stream.cuda_stream)
+            wp_d, nu_d = (torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (wp, nu))
+            sim.set_media(wp_d, nu_d)
+            del wp_d, nu_d
+            torch.cuda.empty_cache()
+            if E0 is not None:
+                E0_d = torch.from_numpy(np.ascontiguousarray(E0, npdt)).cuda()
+                sim.set_fields(E=E0_d)
+                del E0_d
+            sim.set_source(w.src_kind, w.src_params, w.src_cell)
+            sim.set_probes(w.probes)
+            if w.dft_freqs is not None:
+                sim.set_probe_dft(w.dft_freqs)
+            sim.set_plan(rketd.KERNEL_AUTO, depth, -1)
+
+            def one():
+                sim.run(w.nsteps)
+                if w.dft_freqs is None:
+                    sim.discard_records()
+            one()
+            torch.cuda.synchronize()
+            sl0 = sim.counter(rketd.CTR_STEP_LAUNCHES)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            nrun = 2 if w.cell_updates > 1e9 else 5
+            e0.record(stream)
+            for _ in range(nrun):
+                one()
+            e1.record(stream)
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1)
+            gc = w.cell_updates * nrun / (ms * 1e-3) / 1e9
+            kernel_used, depth_used = sim.counter(rketd.CTR_KERNEL_USED), sim.counter(rketd.CTR_DEPTH_USED)
+            roof = roofline_1d(rketd, w, dtype, gc, ms, sim.counter(rketd.CTR_STEP_LAUNCHES) - sl0, kernel_used, depth_used,
+                               sim.counter(rketd.CTR_TILE_CELLS), sim.counter(rketd.CTR_HALO_CELLS), -1, stream.cuda_stream)
+            keep = ("bound", "achieved", "peak", "unit", "frac", "peak_source", "frac_of_mix_peak", "alu_frac", "frac_vs_8TBps_nominal")
+            out[key] = {"workload": w.name, "dtype": dtype, "value": gc, "unit": UNIT, "ms_per_step": ms / nrun, "steps": nrun,
+                        "kernel": int(kernel_used), "depth_T": int(depth_used), "roofline": {k: roof[k] for k in keep if k in roof}}
+            sim.close()
+            torch.cuda.empty_cache()
+        except Exception as ex:          # an extra figure must never cost the headline
+            out[key] = {"error": repr(ex)[:200]}
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -503,6 +619,7 @@ def main():
     ap.add_argument("--variant", type=int, default=-1)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-extra", action="store_true", help="skip the extra per-config figures of the default run")
     ap.add_argument("--table2", action="store_true", help="time the paper's Table 2 sweep instead of the headline workload")
     args = ap.parse_args()
     if args.table2:
@@ -589,32 +706,9 @@ def main():
     value = whole_job_gcells(world, units_per_step, args.steps, ms * 1e-3)
 
     # ---- roofline of the dominant kernel (the stencil kernel: K2 / K3 / K1) -----------------------------------
-    hbm_gbs, peak_src, sm_max = measured_peaks()
-    ncell_total = w.ncells * w.nbatch
-    ms_per_launch = ms / max(1, step_launches)             # launches are back to back on one stream
-    lanes = FP64_LANES_PER_SM if args.dtype == "f64" else FP32_LANES_PER_SM
     clocks = clk.summary()
-    r_alu = 148 * lanes * (sm_max * 1e6) / FP_INSTR_PER_CELL_STEP / 1e9            # Gcell/s at max clock
-    r_hbm1 = hbm_gbs / (ARRAYS_PER_PASS * esize)                                                 # Gcell/s, one step per pass
-    if kernel_used == rketd.KERNEL_RESIDENT:
-        roof = {"bound": "alu", "achieved": value / world, "peak": r_alu, "unit": UNIT, "frac": value / world / r_alu,
-                "traffic": None,
-                "note": "grid resident on chip for the whole run: HBM traffic is setup + probe records only; "
-                        f"peak = 148 SMs x {lanes} FMA lanes x {sm_max:.0f} MHz / 7 instr per cell-step"}
-    else:
-        alg_bytes = ARRAYS_PER_PASS * esize * ncell_total                                        # per launch (one pass)
-        achieved = alg_bytes / (ms_per_launch * 1e-3) / 1e9
-        variant_used = args.variant if args.variant >= 0 else 6
-        roof = {"bound": "hbm", "achieved": achieved, "peak": hbm_gbs, "unit": "GB/s", "frac": achieved / hbm_gbs,
-                "traffic": NCU_TRAFFIC_BYTES.get((w.name, args.dtype, int(depth), variant_used)), "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": alg_bytes, "ms_per_launch": ms_per_launch,
-                "depth_T": depth, "tile_cells": tile_cells, "halo_cells": halo_cells,
-                "frac_vs_8TBps_nominal": achieved / 8000.0,
-                "gcells_vs_one_step_hbm_roofline": value / world / r_hbm1,
-                "alu_frac": (value / world) * (tile_cells / max(1, tile_cells - 2 * halo_cells)) / r_alu,
-                "note": "achieved = 10 arrays (read E,H,G,P,ch,ka,Q; write E,H,G) x nodes x esize per pass / mean launch "
-                        "time; every byte serves depth_T steps; alu_frac counts the redundant halo work against "
-                        "148 SMs x lanes x max clock / 7 instr per cell-step"}
+    roof = roofline_1d(rketd, w, args.dtype, value / world, ms, step_launches, kernel_used, depth, tile_cells, halo_cells,
+                       args.variant, stream.cuda_stream)
 
     # ---- end to end through the C ABI with host buffers ----------------------------------------------------
     e2e = None
@@ -653,6 +747,10 @@ def main():
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
         cpu = cpu_baseline(w)
+    extras = None
+    if world == 1 and not args.no_extra and args.workload == "config4" and args.dtype == "f64" and args.kernel == 0 \
+            and args.depth == 0 and args.variant < 0:
+        extras = extra_configs(rketd, stream, {"config4": (wp, nu, E0)})
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -660,11 +758,13 @@ def main():
                 "dtype": args.dtype, "data": "synthetic",
                 "config": {"workload": w.name, "ncells": w.ncells, "nbatch": w.nbatch, "nsteps_per_run": w.nsteps,
                            "cell_updates_per_step": units_per_step, "kernel": int(kernel_used), "depth_T": int(depth),
-                           "l2": "inputs larger than L2 (state+coefficients %.1f GB)" % (ARRAYS_PER_PASS * esize * ncell_total / 1e9)
+                           "l2": "inputs larger than L2 (state+coefficients %.1f GB)" % (ARRAYS_PER_PASS * esize * w.ncells * w.nbatch / 1e9)
                            if kernel_used != rketd.KERNEL_RESIDENT else "state resident on chip; no HBM re-reads to flush",
                            "parallelism": "replicas only (the path does not shard)" if world > 1 else "single GPU"},
                 "clocks": clocks, "roofline": roof, "e2e": e2e, "cpu_baseline": cpu,
                 "gpu_launches": int(launches), "stencil_launches": int(step_launches)}
+        if extras is not None:
+            line["configs"] = extras       # the other BASELINE configs, timed outside the headline's region
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

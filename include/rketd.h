@@ -46,17 +46,17 @@ enum {
 };
 /* kernel selection for rketd_set_plan */
 enum {
-  RKETD_KERNEL_AUTO = 0,     /* resident (K3) when a grid fits one CTA, else temporal blocking (K2) */
+  RKETD_KERNEL_AUTO = 0,     /* resident (K3) when a grid fits the registers of one cluster, else temporal blocking (K2) */
   RKETD_KERNEL_STEP = 1,     /* K1: one fused H/E/J launch per time step (baseline / cross-check)   */
   RKETD_KERNEL_TBLOCK = 2,   /* K2: T leapfrog steps per pass on a register-resident tile, TMA-staged */
-  RKETD_KERNEL_RESIDENT = 3  /* K3: whole grid resident on chip for the whole run, one CTA per grid  */
+  RKETD_KERNEL_RESIDENT = 3  /* K3: grids resident on chip (registers of a CTA or a cluster) for the whole run */
 };
 /* counters for rketd_get_counter */
 enum {
   RKETD_CTR_LAUNCHES = 0,      /* kernels launched by this handle so far (all kinds)               */
   RKETD_CTR_STEP_LAUNCHES = 1, /* launches of the stencil kernel (K1/K2/K3) so far                  */
   RKETD_CTR_KERNEL_USED = 2,   /* RKETD_KERNEL_* the last rketd_run used                            */
-  RKETD_CTR_DEPTH_USED = 3,    /* temporal depth T of the last K2 run (steps per pass)              */
+  RKETD_CTR_DEPTH_USED = 3,    /* temporal depth T of the last run (K2: steps per pass; K3: per halo refresh) */
   RKETD_CTR_STEPS_DONE = 4,    /* global step counter                                               */
   RKETD_CTR_TILE_CELLS = 5,    /* cells per CTA tile, halo included, of the last K2/K3 run          */
   RKETD_CTR_HALO_CELLS = 6,    /* halo cells on each side of a K2 tile                              */
@@ -127,10 +127,15 @@ int rketd_reset(rketd_sim *s);
  * Synchronises (device buffers are freed). */
 int rketd_discard_records(rketd_sim *s);
 
-/* Choose the kernel (RKETD_KERNEL_*), for K2 the temporal depth T (0 = default), and the launch
- * variant of K2/K3 (-1 = default; K2: 0..3 = CTA tiles with {nodes per thread, threads per CTA} combinations, 4..7 = warp tiles,
- * K3: 0 = a thread owns a 64-B row, 1 = half a row, 2 = a row with the coefficients in shared memory).  All choices compute identical bits.
- * EINVAL if the choice cannot run this grid (e.g. RESIDENT with a grid larger than one CTA). */
+/* Choose the kernel (RKETD_KERNEL_*), the temporal depth T (0 = default; K2: steps per pass, K3: steps between two halo
+ * refreshes), and the launch variant (-1 = default).  K2: 0..3 = CTA tiles with {nodes per thread, threads per CTA}
+ * combinations, 4..7 = warp tiles.  K3: -1 = warp tiles (k3_wtile) with the packing chosen by the library;
+ * RKETD_RESIDENT_WTILE(nw, nc, k) = warp tiles with k whole grids per chunk held by a cluster of nc CTAs x nw warps
+ * (0 = chosen by the library); 0, 1, 2 = the one-barrier-per-step kernel k3_resident (a thread owns a 64-B row / half a
+ * row / a row with the coefficients in shared memory; grids of at most 512 rows).  All choices compute identical bits.
+ * EINVAL if the choice cannot run this grid (e.g. RESIDENT with a grid larger than a cluster can hold). */
+#define RKETD_RESIDENT_WTILE_FLAG 0x40000000
+#define RKETD_RESIDENT_WTILE(nw, nc, k) (RKETD_RESIDENT_WTILE_FLAG | ((k) << 16) | ((nc) << 8) | (nw))
 int rketd_set_plan(rketd_sim *s, int kernel, int depth, int variant);
 
 /* Advance every grid by nsteps leapfrog steps (H eq. (14); E eq. (12)
@@ -167,6 +172,23 @@ int rketd_get_kernel_coefficients(rketd_sim *s, double *out);
 
 /* RKETD_CTR_* counters (for bench.py's gpu_launches and roofline bookkeeping). */
 int64_t rketd_get_counter(const rketd_sim *s, int which);
+
+/* Microbenchmarks behind the "alu" roofline of bench.py ("builder must microbenchmark DFMA and
+ * shared-memory peaks and use the measured values"); not on the hot path, needs no handle.  Runs `what` on the current
+ * device for `iters` loop iterations (a few ms at 4000) on cuda_stream and synchronises.  out[4] (host):
+ *   out[0]  thread-instructions per ns summed over the device (LDS128: bytes per ns = GB/s)
+ *   out[1]  thread-instructions (bytes) per clock and SM — "lanes"
+ *   out[2]  SM clock held during the run [MHz] (clock64 against globaltimer)
+ *   out[3]  number of SMs
+ * FMA forms differ in the number of DISTINCT register source operands per instruction (1, 2, 3, or 2 + one
+ * constant-bank operand); MIX is the 7-instruction node update of the stencil kernels (H 2, E 3, G 2) on
+ * a 64-B row per lane in registers, without shuffles or memory, at 12 warps per SM.  EINVAL: bad `what` or iters < 1. */
+enum {
+  RKETD_PEAK_DFMA_1REG = 0, RKETD_PEAK_DFMA_2REG = 1, RKETD_PEAK_DFMA_3REG = 2, RKETD_PEAK_DFMA_2REG_CONST = 3,
+  RKETD_PEAK_FFMA_1REG = 4, RKETD_PEAK_FFMA_2REG = 5, RKETD_PEAK_FFMA_3REG = 6, RKETD_PEAK_FFMA_2REG_CONST = 7,
+  RKETD_PEAK_MIX_F64 = 8, RKETD_PEAK_MIX_F32 = 9, RKETD_PEAK_LDS128 = 10
+};
+int rketd_measure_peak(int what, int iters, double *out, void *cuda_stream);
 
 void rketd_destroy(rketd_sim *s);
 

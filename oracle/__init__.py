@@ -35,6 +35,21 @@ SCHEME_ETD2 = 0      # eq. (11) PAPER.md:68 — the paper's method
 SCHEME_ETD1 = 1      # eq. (9) PAPER.md:59 — first-order ETD
 
 
+_SAN_LIB = os.path.join(_HERE, "liboracle_rketd_asan.so")
+
+
+def build_sanitized(force: bool = False) -> str:
+    """A third build of the same source under AddressSanitizer + UndefinedBehaviorSanitizer, same
+    arithmetic flags.  A process that sets RKETD_ORACLE_SANITIZED=1 (and preloads libasan) gets this build from
+    every call below; tests/test_oracle_sanitized.py runs the pin suites that way."""
+    if force or not os.path.exists(_SAN_LIB) or os.path.getmtime(_SAN_LIB) < os.path.getmtime(_SRC):
+        cmd = ["g++", "-fopenmp", "-std=c++17", "-O1", "-g", "-ffp-contract=off", "-fsanitize=address,undefined",
+               "-fno-sanitize-recover=all", "-fno-omit-frame-pointer", "-fPIC", "-shared", _SRC, "-o", _SAN_LIB + ".tmp"]
+        subprocess.run(cmd, check=True)
+        os.replace(_SAN_LIB + ".tmp", _SAN_LIB)
+    return _SAN_LIB
+
+
 def build(force: bool = False) -> None:
     """Compile both builds of the oracle with g++ (a few seconds)."""
     for omp, out in _LIBS.items():
@@ -54,7 +69,7 @@ _I64 = ctypes.POINTER(ctypes.c_int64)
 def _lib(omp: bool = False) -> ctypes.CDLL:
     if omp not in _loaded:
         build()
-        lib = ctypes.CDLL(_LIBS[omp])
+        lib = ctypes.CDLL(build_sanitized() if os.environ.get("RKETD_ORACLE_SANITIZED") == "1" else _LIBS[omp])
         lib.oracle_constants.argtypes = [_D, _D, _D]
         lib.oracle_constants.restype = None
         lib.oracle_phi.argtypes = [ctypes.c_double, _D, _D]

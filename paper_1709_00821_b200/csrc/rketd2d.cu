@@ -661,11 +661,13 @@ cudaError_t launch_k2_T(rketd2d_sim *s, P2<R> &p) {
   p.HP = pl.HP; p.Wv = pl.Wv; p.nstrips = pl.nstrips; p.nsegs = pl.nsegs; p.Sy = pl.Sy; p.dlast = pl.dlast;
   if (T == s->ctr_depth_used || s->ctr_strip == 0) { s->ctr_strip = NT; s->ctr_halo = pl.HP; s->ctr_seg = pl.Sy; }   // the main passes, not a remainder pass
   constexpr size_t smem = K2Shape<R, T>::smem;
-  static bool configured = false;
-  if (!configured) {
+  static unsigned long long configured = 0ull;      // bit = device id: the attribute is per device and context
+  int dev = 0;
+  cudaGetDevice(&dev);
+  if (dev >= 64 || !((configured >> dev) & 1ull)) {
     cudaError_t e = cudaFuncSetAttribute(k2_2d<R, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    configured = true;
+    if (dev < 64) configured |= 1ull << dev;
   }
   const int grid = pl.nstrips * pl.nsegs;
   k2_2d<R, T><<<grid, NT, smem, s->stream>>>(p, arrays_of<R>(s));
@@ -789,9 +791,6 @@ int rketd2d_create(rketd2d_sim **out, int64_t nx, int64_t ny, double dx, double 
 int rketd2d_set_media(rketd2d_sim *s, const double *wp, const double *nu) {
   if (!s) return RKETD_EINVAL;
   if (!wp || !nu) return fail2(s, RKETD_EINVAL, "wp and nu must not be NULL");
-  // live fields under the old media: back to J first
-  const bool live = s->have_media && !s->fields_zero;
-  if (live) { const int rc = convert_current_any(s, false, s->fld[s->cur][3]); if (rc) return rc; }
   const int64_t n = s->pitch * s->ny, nu_n = (int64_t)s->nx * s->ny;
   double *d_wp = nullptr, *d_nu = nullptr;      // user layout on the device
   CU_TRY2(s, cudaMalloc((void **)&d_wp, (size_t)nu_n * 8));
@@ -799,27 +798,41 @@ int rketd2d_set_media(rketd2d_sim *s, const double *wp, const double *nu) {
   if (e != cudaSuccess) { cudaFree(d_wp); CU_TRY2(s, e); }
   e = cudaMemcpyAsync(d_wp, wp, (size_t)nu_n * 8, cudaMemcpyDefault, s->stream);
   if (e == cudaSuccess) e = cudaMemcpyAsync(d_nu, nu, (size_t)nu_n * 8, cudaMemcpyDefault, s->stream);
-  if (e == cudaSuccess) e = cudaMemsetAsync(s->d_bad, 0, sizeof(int), s->stream);
-  if (e == cudaSuccess) {
-    if (s->dtype == RKETD_F64)
-      coef2d_kernel<double><<<blocks_for(n), 256, 0, s->stream>>>(s->nx, s->ny, s->pitch, d_wp, d_nu, s->dx, s->dt, kEps0, s->wp_p,
-                                                                  s->nu_p, (double *)s->coef[0], (double *)s->coef[1],
-                                                                  (double *)s->coef[2], (double *)s->coef[3], s->d_bad);
-    else
-      coef2d_kernel<float><<<blocks_for(n), 256, 0, s->stream>>>(s->nx, s->ny, s->pitch, d_wp, d_nu, s->dx, s->dt, kEps0, s->wp_p,
-                                                                 s->nu_p, (float *)s->coef[0], (float *)s->coef[1],
-                                                                 (float *)s->coef[2], (float *)s->coef[3], s->d_bad);
-    e = cudaGetLastError();
-    s->ctr_launches++;
-  }
+  // read-only validation first: a rejected call leaves coefficients, media and fields exactly as they were
   int bad = 0;
-  if (e == cudaSuccess) e = cudaMemcpyAsync(&bad, s->d_bad, sizeof(int), cudaMemcpyDeviceToHost, s->stream);
+  if (e == cudaSuccess) e = cudaMemsetAsync(s->d_bad, 0, sizeof(int), s->stream);
+  if (e == cudaSuccess) e = rketd::launch_validate_media(d_wp, d_nu, nu_n, s->d_bad, s->stream);
+  if (e == cudaSuccess) { s->ctr_launches++; e = cudaMemcpyAsync(&bad, s->d_bad, sizeof(int), cudaMemcpyDeviceToHost, s->stream); }
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+  if (e != cudaSuccess || bad) {
+    cudaFree(d_wp); cudaFree(d_nu);
+    CU_TRY2(s, e);
+    return fail2(s, RKETD_EINVAL, "wp and nu must be finite and non-negative");
+  }
+  // live fields under the old media: back to J first (in place), and third_is_J says so at once, so that a CUDA
+  // failure further down leaves array and flag in agreement
+  const bool live = s->have_media && !s->fields_zero && !s->third_is_J;
+  if (live) {
+    const int rc = convert_current_any(s, false, s->fld[s->cur][3]);
+    if (rc) { cudaFree(d_wp); cudaFree(d_nu); return rc; }
+    s->third_is_J = true;
+  }
+  s->have_media = false;      // until the new coefficients are in place
+  if (s->dtype == RKETD_F64)
+    coef2d_kernel<double><<<blocks_for(n), 256, 0, s->stream>>>(s->nx, s->ny, s->pitch, d_wp, d_nu, s->dx, s->dt, kEps0, s->wp_p,
+                                                                s->nu_p, (double *)s->coef[0], (double *)s->coef[1],
+                                                                (double *)s->coef[2], (double *)s->coef[3], s->d_bad);
+  else
+    coef2d_kernel<float><<<blocks_for(n), 256, 0, s->stream>>>(s->nx, s->ny, s->pitch, d_wp, d_nu, s->dx, s->dt, kEps0, s->wp_p,
+                                                               s->nu_p, (float *)s->coef[0], (float *)s->coef[1],
+                                                               (float *)s->coef[2], (float *)s->coef[3], s->d_bad);
+  e = cudaGetLastError();
+  s->ctr_launches++;
   if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
   cudaFree(d_wp); cudaFree(d_nu);
   CU_TRY2(s, e);
-  if (bad) { s->have_media = false; return fail2(s, RKETD_EINVAL, "wp and nu must be finite and non-negative"); }
   s->have_media = true;
-  if (live || s->third_is_J) { const int rc = convert_current_any(s, true, nullptr); if (rc) return rc; }
+  if (s->third_is_J) { const int rc = convert_current_any(s, true, nullptr); if (rc) return rc; }
   s->third_is_J = false;
   CU_TRY2(s, cudaStreamSynchronize(s->stream));
   return RKETD_OK;
@@ -931,11 +944,14 @@ int rketd2d_run(rketd2d_sim *s, int64_t nsteps) {
   void *rec = nullptr;
   if (!s->probe_i.empty()) {
     CU_TRY2(s, cudaMalloc(&rec, (size_t)s->probe_i.size() * (size_t)nsteps * s->esize));
-    s->chunks.push_back({rec, nsteps});
   }
   s->fields_zero = false;
   const int rc = s->dtype == RKETD_F64 ? run_typed<double>(s, nsteps, rec) : run_typed<float>(s, nsteps, rec);
-  if (rc) return rc;
+  if (rc) {               // a failed run records nothing: the chunk list and nsamples stay in step
+    if (rec) { cudaStreamSynchronize(s->stream); cudaFree(rec); cudaGetLastError(); }
+    return rc;
+  }
+  if (rec) s->chunks.push_back({rec, nsteps});
   s->nsamples += s->probe_i.empty() ? 0 : nsteps;
   return RKETD_OK;
 }

@@ -59,6 +59,7 @@ struct rketd_sim {
   int plan_kernel = RKETD_KERNEL_AUTO, plan_depth = 0, plan_variant = -1;
   K2Plan k2;
   bool k2_valid = false;
+  int sms = 0;                   // multiprocessors of the device the handle lives on
   int64_t ctr_launches = 0, ctr_step_launches = 0, ctr_kernel_used = 0, ctr_depth_used = 0, ctr_tile_cells = 0,
           ctr_halo_cells = 0, state_bytes = 0;
   std::string err;
@@ -200,7 +201,7 @@ int make_map(rketd_sim *s, CUtensorMap *m, void *base, int box_rows) {
 // wave wins, because it divides the number of launches.
 int default_depth(const rketd_sim *s) {
   const int base = s->dtype == RKETD_F64 ? 16 : 32;
-  const int64_t one_wave = 148 * 12;
+  const int64_t one_wave = (int64_t)s->sms * 12;
   for (int T = 4 * base; T > base; T -= base) {
     const int HR = (T + s->L.C - 1) / s->L.C, rows_out = 32 - 2 * HR;
     if (rows_out < 8) continue;
@@ -209,10 +210,6 @@ int default_depth(const rketd_sim *s) {
   return base;
 }
 int default_k2_variant(const rketd_sim *) { return 6; }
-// Grids of 33..256 rows: whole-row threads with the coefficients in shared memory (128 registers: 4 CTAs of 128
-// threads per SM instead of 3, and warps whose rows carry one coefficient set read nothing per step).  Measured on
-// config 5: fp64 860 Gcell/s against 630 (coefficients in registers) and 670 (half-row threads); fp32 1271 against 965.
-int default_k3_variant(const rketd_sim *s) { return (s->L.nrows > 32 && s->L.nrows <= 256) ? 2 : 0; }
 int max_depth(const rketd_sim *s, int variant) { return (k2_tile_rows(variant) / 2 - 1) * s->L.C; }
 
 int build_k2_plan(rketd_sim *s, int depth, int variant) {
@@ -227,11 +224,10 @@ int build_k2_plan(rketd_sim *s, int depth, int variant) {
   P.total_tiles = P.tiles_per_grid * L.nbatch;
   if (P.total_tiles >= (int64_t)1 << 31) return fail(s, RKETD_EINVAL, "too many tiles for the temporal-blocking kernel");
   P.smem_bytes = k2_smem_bytes(variant);
-  int ctas = 0, dev = 0, sms = 0;
+  int ctas = 0;
+  const int sms = s->sms;
   CU_TRY(s, k2_configure(s->dtype, variant, &ctas));
   if (ctas < 1) return fail(s, RKETD_ECUDA, "K2 kernel does not fit on an SM");
-  CU_TRY(s, cudaGetDevice(&dev));
-  CU_TRY(s, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
   P.ctas_per_sm = ctas;
   const int tpc = k2_tiles_per_cta(variant);
   P.grid = (int)std::min<int64_t>((P.total_tiles + tpc - 1) / tpc, (int64_t)sms * ctas);
@@ -256,9 +252,25 @@ int build_k2_plan(rketd_sim *s, int depth, int variant) {
   return RKETD_OK;
 }
 
+// RESIDENT plans.  rketd_set_plan's variant: -1 = the warp-tile kernel k3_wtile with the packing chosen by k3w_plan;
+// RKETD_RESIDENT_WTILE(nw, nc, k) = the same with an explicit packing; 0, 2 = the older one-barrier-per-step kernel
+// k3_resident (kept as a structurally different cross-check).
+bool wtile_variant(int variant) { return variant < 0 || (variant & RKETD_RESIDENT_WTILE_FLAG) != 0; }
+bool resident_wtile_plan(rketd_sim *s, int depth, int variant, K3WPlan *P) {
+  int64_t nw = 0, nc = 0, k = 0;
+  if (variant >= 0) { nw = variant & 0xff; nc = (variant >> 8) & 0xff; k = (variant >> 16) & 0xfff; }
+  if (!k3w_plan(s->L, depth, s->sms, nw, nc, k, P)) return false;
+  if (P->nc > 1) {              // the cluster must be schedulable on this device (GPC size, registers, shared memory)
+    int ncl = 0;
+    if (k3w_max_clusters(s->dtype, *P, &ncl) != cudaSuccess || ncl < 1) { cudaGetLastError(); return false; }
+  }
+  return true;
+}
+
 int resolve_kernel(rketd_sim *s) {
   if (s->plan_kernel != RKETD_KERNEL_AUTO) return s->plan_kernel;
-  return k3_threads_for_rows(s->dtype, s->L.nrows, 0) ? RKETD_KERNEL_RESIDENT : RKETD_KERNEL_TBLOCK;
+  K3WPlan P;
+  return resident_wtile_plan(s, 0, -1, &P) ? RKETD_KERNEL_RESIDENT : RKETD_KERNEL_TBLOCK;
 }
 
 // run nsteps steps whose probe samples go to rec ([nbatch][nprobes][nsteps] or nullptr)
@@ -312,14 +324,25 @@ int run_segment(rketd_sim *s, int64_t nsteps, void *rec) {
     }
     s->ctr_tile_cells = L.C; s->ctr_halo_cells = 1; s->ctr_depth_used = 1;
   } else if (kern == RKETD_KERNEL_RESIDENT) {
-    int variant = s->plan_variant >= 0 ? s->plan_variant : default_k3_variant(s);
-    if (!k3_threads_for_rows(s->dtype, L.nrows, variant)) variant = 0;
-    const int NT = k3_threads_for_rows(s->dtype, L.nrows, variant);
-    if (!NT) return fail(s, RKETD_EINVAL, "grid too large for the resident kernel");
     FieldPtrs f{s->fld[s->cur][0], s->fld[s->cur][1], s->fld[s->cur][2]};
-    CU_TRY(s, launch_k3(s->dtype, L, f, s->coef, sc, nsteps, NT, variant, s->stream));
+    if (wtile_variant(s->plan_variant)) {
+      K3WPlan P;
+      if (!resident_wtile_plan(s, s->plan_kernel == RKETD_KERNEL_RESIDENT ? s->plan_depth : 0, s->plan_variant, &P))
+        return fail(s, RKETD_EINVAL, "grid too large for the resident kernel (or the requested packing cannot run)");
+      CU_TRY(s, launch_k3w(s->dtype, L, P, f, s->coef, sc, nsteps, s->stream));
+      // cells a chunk occupies on chip (halo and padding lanes included) against the cells it holds
+      s->ctr_tile_cells = (int64_t)P.nc * P.nw * 32 * L.C;
+      s->ctr_halo_cells = (s->ctr_tile_cells - P.k * L.gstride) / 2;
+      s->ctr_depth_used = P.T;
+    } else {
+      int variant = s->plan_variant;
+      if (!k3_threads_for_rows(s->dtype, L.nrows, variant)) variant = 0;
+      const int NT = k3_threads_for_rows(s->dtype, L.nrows, variant);
+      if (!NT) return fail(s, RKETD_EINVAL, "grid too large for the one-CTA resident kernel");
+      CU_TRY(s, launch_k3(s->dtype, L, f, s->coef, sc, nsteps, NT, variant, s->stream));
+      s->ctr_tile_cells = L.gstride; s->ctr_halo_cells = 0; s->ctr_depth_used = nsteps;
+    }
     ++s->ctr_launches; ++s->ctr_step_launches;
-    s->ctr_tile_cells = L.gstride; s->ctr_halo_cells = 0; s->ctr_depth_used = nsteps;
   } else {
     const int variant = s->plan_variant >= 0 ? s->plan_variant : default_k2_variant(s);
     int depth = s->plan_depth > 0 ? s->plan_depth : default_depth(s);
@@ -356,6 +379,15 @@ int rketd_create(rketd_sim **out, int64_t ncells, int64_t nbatch, double dz, dou
     return fail(nullptr, RKETD_ECUDA, "rketd_create: no CUDA device (librketd has no CPU fallback)");
   }
   rketd_sim *s = new rketd_sim();
+  {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&s->sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+        s->sms < 1) {
+      cudaGetLastError();
+      delete s;
+      return fail(nullptr, RKETD_ECUDA, "rketd_create: cannot query the device");
+    }
+  }
   Layout &L = s->L;
   L.ncells = ncells; L.nbatch = nbatch;
   L.esize = dtype == RKETD_F64 ? 8 : 4;
@@ -399,14 +431,6 @@ int rketd_set_media(rketd_sim *s, const double *wp, const double *nu) {
   void *twp = nullptr, *tnu = nullptr, *tJ = nullptr;
   auto cleanup = [&]() { if (twp) cudaFree(twp); if (tnu) cudaFree(tnu); if (tJ) cudaFree(tJ); };
 #define SM_TRY(expr) do { cudaError_t sm_e = (expr); if (sm_e != cudaSuccess) { cleanup(); CU_TRY(s, sm_e); } } while (0)
-  // live fields carry G = cj J - cj kc E of the OLD media: take J out before the coefficients change
-  const bool reconvert = s->have_media && !s->fields_zero && !s->third_is_J;
-  if (reconvert) {
-    SM_TRY(cudaMalloc(&tJ, (size_t)L.ncells * L.nbatch * L.esize));
-    SM_TRY(launch_G_to_current(s->dtype, L, s->wp_p, s->nu_p, s->dz, s->dt, s->media_scheme, s->pml, s->fld[s->cur][0], s->fld[s->cur][2], tJ,
-                               s->stream));
-    ++s->ctr_launches;
-  }
   if (!is_device_ptr(wp)) {
     SM_TRY(cudaMalloc(&twp, n));
     SM_TRY(cudaMemcpyAsync(twp, wp, n, cudaMemcpyDefault, s->stream));
@@ -416,6 +440,30 @@ int rketd_set_media(rketd_sim *s, const double *wp, const double *nu) {
     SM_TRY(cudaMalloc(&tnu, n));
     SM_TRY(cudaMemcpyAsync(tnu, nu, n, cudaMemcpyDefault, s->stream));
     dnu = (const double *)tnu;
+  }
+  // read-only validation first: a rejected call leaves coefficients, media and fields exactly as they were
+  int bad = 0;
+  SM_TRY(cudaMemsetAsync(s->d_bad, 0, sizeof(int), s->stream));
+  SM_TRY(launch_validate_media(dwp, dnu, (int64_t)L.ncells * L.nbatch, s->d_bad, s->stream));
+  ++s->ctr_launches;
+  SM_TRY(cudaMemcpyAsync(&bad, s->d_bad, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
+  SM_TRY(cudaStreamSynchronize(s->stream));
+  if (bad) {
+    cleanup();
+    return fail(s, RKETD_EINVAL, "rketd_set_media: wp and nu must be finite and non-negative");
+  }
+  // live fields carry G = cj J - cj kc E of the OLD media: put J itself back into the third array before the
+  // coefficients change, and say so in third_is_J at once, so that a CUDA failure further down leaves array and flag in
+  // agreement (the next successful rketd_set_media converts J -> G)
+  const bool reconvert = s->have_media && !s->fields_zero && !s->third_is_J;
+  if (reconvert) {
+    SM_TRY(cudaMalloc(&tJ, (size_t)L.ncells * L.nbatch * L.esize));
+    SM_TRY(launch_G_to_current(s->dtype, L, s->wp_p, s->nu_p, s->dz, s->dt, s->media_scheme, s->pml, s->fld[s->cur][0], s->fld[s->cur][2], tJ,
+                               s->stream));
+    ++s->ctr_launches;
+    SM_TRY(cudaMemsetAsync(s->fld[s->cur][2], 0, arr_bytes(L), s->stream));
+    SM_TRY(copy_in(s, s->fld[s->cur][2], tJ));
+    s->third_is_J = true;
   }
   // absorbing layer requested by rketd_set_boundary: tables of the E nodes (into the coefficient arrays) and of the
   // H nodes (kernel parameters).  Reading of PAPER.md:93, :123 in DESIGN.md §12: sigma(rho) = sigma_max rho^m,
@@ -437,32 +485,20 @@ int rketd_set_media(rketd_sim *s, const double *wp, const double *nu) {
       new_hd[j] = nchh / (1.0 + sh) - nchh;
     }
   }
-  SM_TRY(cudaMemsetAsync(s->d_bad, 0, sizeof(int), s->stream));
+  s->have_media = false;      // until the new coefficients are in place
   SM_TRY(launch_coefficients(s->dtype, L, dwp, dnu, s->dz, s->dt, s->scheme, new_pml, s->wp_p, s->nu_p, s->coef, s->d_bad, s->stream));
   ++s->ctr_launches;
-  int bad = 0;
-  SM_TRY(cudaMemcpyAsync(&bad, s->d_bad, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
-  SM_TRY(cudaStreamSynchronize(s->stream));
-  if (bad) {
-    cleanup();
-    s->have_media = false;
-    return fail(s, RKETD_EINVAL, "rketd_set_media: wp and nu must be finite and non-negative");
-  }
   s->media_scheme = s->scheme;
   s->pml = new_pml;
   std::memcpy(s->pml_ha, new_ha, sizeof(new_ha));
   std::memcpy(s->pml_hd, new_hd, sizeof(new_hd));
   s->flags_dirty = true;
-  if (reconvert) {
-    SM_TRY(cudaMemsetAsync(s->fld[s->cur][2], 0, arr_bytes(L), s->stream));
-    SM_TRY(copy_in(s, s->fld[s->cur][2], tJ));
-  }
-  if (reconvert || s->third_is_J) {
+  if (s->third_is_J) {
     SM_TRY(launch_current_to_G(s->dtype, L, s->wp_p, s->nu_p, s->dz, s->dt, s->media_scheme, s->pml, s->fld[s->cur][0],
                                s->fld[s->cur][2], s->stream));
     ++s->ctr_launches;
-    SM_TRY(cudaStreamSynchronize(s->stream));
   }
+  SM_TRY(cudaStreamSynchronize(s->stream));     // the staging buffers are freed below
 #undef SM_TRY
   cleanup();
   s->third_is_J = false;
@@ -563,8 +599,11 @@ int rketd_discard_records(rketd_sim *s) {
 int rketd_set_plan(rketd_sim *s, int kernel, int depth, int variant) {
   if (!s) return RKETD_EINVAL;
   if (kernel < RKETD_KERNEL_AUTO || kernel > RKETD_KERNEL_RESIDENT || depth < 0) return fail(s, RKETD_EINVAL, "rketd_set_plan: bad argument");
-  if (kernel == RKETD_KERNEL_RESIDENT && !k3_threads_for_rows(s->dtype, s->L.nrows, variant < 0 ? 0 : variant))
-    return fail(s, RKETD_EINVAL, "rketd_set_plan: grid does not fit the resident kernel");
+  if (kernel == RKETD_KERNEL_RESIDENT) {
+    K3WPlan P;
+    if (wtile_variant(variant) ? !resident_wtile_plan(s, depth, variant, &P) : !k3_threads_for_rows(s->dtype, s->L.nrows, variant))
+      return fail(s, RKETD_EINVAL, "rketd_set_plan: grid does not fit the resident kernel (or bad depth / packing)");
+  }
   if (kernel == RKETD_KERNEL_TBLOCK || kernel == RKETD_KERNEL_AUTO) {
     if (variant >= 0 && kernel == RKETD_KERNEL_TBLOCK && !k2_tile_rows(variant)) return fail(s, RKETD_EINVAL, "rketd_set_plan: unknown variant");
     const int v = (variant >= 0 && k2_tile_rows(variant)) ? variant : default_k2_variant(s);
@@ -595,9 +634,14 @@ int rketd_run(rketd_sim *s, int64_t nsteps) {
     } else {
       CU_TRY(s, cudaMalloc(&buf, bytes));
     }
-    s->chunks.push_back(Chunk{buf, nsteps, bytes});
     int rc = run_segment(s, nsteps, buf);
-    if (rc) return rc;
+    if (rc) {             // a failed run records nothing: the chunk list and nsamples stay in step
+      cudaStreamSynchronize(s->stream);
+      cudaFree(buf);
+      cudaGetLastError();
+      return rc;
+    }
+    s->chunks.push_back(Chunk{buf, nsteps, bytes});
     s->nsamples += nsteps;
     return RKETD_OK;
   }

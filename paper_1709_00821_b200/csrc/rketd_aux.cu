@@ -3,6 +3,8 @@
 //   coefficient read-back, the J <-> G change of variable at the boundary, DFT twiddles / accumulation / magnitude (row a7, BASELINE config 5).
 #include <math_constants.h>
 
+#include <algorithm>
+
 #include "rketd_coef.cuh"
 #include "rketd_internal.h"
 
@@ -26,6 +28,22 @@ __device__ __forceinline__ Six pml_six(const PmlE &pml, int j) {
   Six s;
   s.ca = pml.a[j]; s.cj = 0.0; s.ch = pml.b[j]; s.ka = 1.0; s.kb = 0.0; s.kc = 0.0;
   return s;
+}
+
+// read-only check of user media (finite, non-negative): rketd_set_media / rketd2d_set_media run it BEFORE anything of
+// the handle changes, so that a rejected call leaves coefficients and fields untouched
+__global__ void validate_media_kernel(const double *__restrict__ wp, const double *__restrict__ nu, int64_t n, int *bad) {
+  int flag = 0;
+  for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+    const double w = wp[i], v = nu[i];
+    if (!(w >= 0.0) || !(v >= 0.0) || isinf(w) || isinf(v)) flag = 1;
+  }
+  if (flag) atomicOr(bad, 1);
+}
+cudaError_t launch_validate_media(const double *wp, const double *nu, int64_t n, int *d_bad, cudaStream_t st) {
+  const unsigned blocks = (unsigned)std::min<int64_t>((n + 255) / 256, 148 * 16);
+  validate_media_kernel<<<blocks, 256, 0, st>>>(wp, nu, n, d_bad);
+  return cudaGetLastError();
 }
 
 // a0: pads the media into the physical layout and derives the four per-node coefficients the stencil

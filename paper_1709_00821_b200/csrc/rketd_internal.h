@@ -64,6 +64,21 @@ struct K2Plan {
   K2Maps maps[2];          // maps[s]: read buffer s, write buffer 1-s
 };
 
+// K3 (resident warp tiles, rketd_resident.cu): a chunk of k whole grids lives in a cluster of nc CTAs x nw warps
+struct K3WPlan {
+  int T = 0, HR = 0, rows_out = 0;     // steps per round (between halo refreshes), halo rows, 32 - 2 HR
+  int k = 1, nc = 1, nw = 1;           // grids per chunk, CTAs per cluster, warps per CTA
+  int64_t chunk_rows = 0, nchunks = 0;
+  int tiles_per_chunk = 0;
+  uint32_t smem_bytes = 0;
+};
+// false when the grid cannot stay resident (a grid needs more than 16 CTAs x 12 warp tiles) or the wish cannot be met;
+// want_* = 0: chosen here
+bool k3w_plan(const Layout &L, int depth, int sms, int64_t want_nw, int64_t want_nc, int64_t want_k, K3WPlan *out);
+cudaError_t launch_k3w(int dtype, const Layout &L, const K3WPlan &P, FieldPtrs fld, void *const coef[4], const StepCommon &sc,
+                       int64_t nsteps, cudaStream_t st);
+cudaError_t k3w_max_clusters(int dtype, const K3WPlan &P, int *nclusters);
+
 constexpr int kK2Variants = 8;
 constexpr int kNumCoefArrays = 4;                                 // P, ch, ka, Q (rketd_device.cuh COEF_*)
 int k2_tile_rows(int variant);                                    // rows per tile of a K2 variant, 0 if none
@@ -85,6 +100,8 @@ cudaError_t launch_coefficients(int dtype, const Layout &L, const double *wp, co
                                 double dt, int scheme, const PmlE &pml, double *wp_p, double *nu_p, void *const coef[kNumCoefArrays],
                                 int *d_bad,
                                 cudaStream_t st);
+// sets *d_bad when any wp or nu (user layout, n values each) is negative or not finite; reads only
+cudaError_t launch_validate_media(const double *wp, const double *nu, int64_t n, int *d_bad, cudaStream_t st);
 // the six coefficients of SURVEY a0 (ca, cj, ch, ka, kb, kc), recomputed in fp64 from the padded media
 cudaError_t launch_six_coefficients(const Layout &L, const double *wp_p, const double *nu_p, double dz, double dt,
                                     int scheme, const PmlE &pml, double *out, cudaStream_t st);

@@ -1,0 +1,275 @@
+// rketd_resident.cu — K3 `k3_wtile`: the resident kernel of librketd (north_star kernels (2) + (3) combined; SURVEY.md
+// §3.2 "ONE persistent launch ... runs ALL nsteps on chip", H5 "warp-private trapezoids (no per-step __syncthreads)").
+//
+// A chunk = k whole grids of the batch (consecutive rows of the [nbatch][nrows][C] layout) is held in the registers of a
+// cluster of NC CTAs x NW warps for the whole run: every warp owns a tile of 32 rows x 64 B (one row per lane; E, H, G
+// and the four coefficients of its nodes), tiles overlap by 2 HR rows, HR = ceil(T / C).  A round is T leapfrog steps of
+// the tile by warp_step (rketd_wtile.cuh: halos by two shuffles per step, no barrier, no shared memory) — the same
+// instruction sequence as K1 and K2, so the three agree bit for bit.  Garbage enters a tile from its two ends one node
+// per step and the halo absorbs it; after the round every warp publishes the 2 HR outermost rows it OWNS into its
+// neighbours' halo slots (shared memory of the neighbour's CTA: plain stores inside a CTA, st.shared::cluster over
+// DSMEM across CTAs), ONE barrier (bar.sync, or the cluster barrier), and the halo lanes reload.  A barrier is paid once
+// per T steps instead of once per step (profiles/r01_ncu_k3.md: `barrier` was the leading stall, 2.6-2.8 warps per issue).
+// HBM is touched at the start, at the end and for probe samples.  Grids never interact inside a tile that spans two of
+// them: the end nodes are rewritten by Mur / the conductor every step from their own grid's values, H behind the last
+// node is forced to zero, and padding nodes carry zero coefficients (rketd_internal.h Layout).
+#include <algorithm>
+
+#include "rketd_wtile.cuh"
+
+namespace rketd {
+
+struct K3WArgs {
+  int T, HR, rows_out;          // steps per round, halo rows, 32 - 2 HR
+  int cluster;                  // CTAs per chunk
+  int chunk_rows;               // rows of a chunk = grids_per_chunk * nrows
+  int tiles_per_chunk;          // ceil(chunk_rows / rows_out) <= cluster * warps per CTA
+  int64_t nrows;                // rows per grid
+  int64_t total_rows;           // nbatch * nrows
+  int64_t nsteps;
+};
+
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
+}
+__device__ __forceinline__ uint32_t map_to_cta(uint32_t local_smem_addr, uint32_t rank) {
+  uint32_t a;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(a) : "r"(local_smem_addr), "r"(rank));
+  return a;
+}
+__device__ __forceinline__ void st_cluster128(uint32_t a, const double2 &v) {
+  asm volatile("st.shared::cluster.v2.f64 [%0], {%1, %2};" ::"r"(a), "d"(v.x), "d"(v.y) : "memory");
+}
+__device__ __forceinline__ void st_cluster128(uint32_t a, const float4 &v) {
+  asm volatile("st.shared::cluster.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(a), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+__device__ __forceinline__ void cluster_barrier() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+
+// halo slots of one CTA: [parity 2][warp][side 2][row HR][array 3][64 B]; side 0 = the tile's lanes 0..HR-1
+constexpr int kMaxHR = 2;
+__host__ __device__ constexpr uint32_t slot_bytes_per_warp() { return 2u * kMaxHR * 3u * kRowBytes; }
+
+template <typename R, bool CLUSTER, bool PML>
+__global__ void __launch_bounds__(384, 1) k3_wtile(RowPtrs<R> f, CoefPtrs<R> cp, const __grid_constant__ StepParams<R> p,
+                                                    const K3WArgs q) {
+  constexpr int C = kRowBytes / sizeof(R);
+  typedef Geom<R, C> G;
+  typedef typename Arith<R>::Vec Vec;
+  extern __shared__ __align__(16) uint8_t slots_raw[];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+  const uint32_t rank = CLUSTER ? cluster_ctarank() : 0u;
+  const int64_t chunk = CLUSTER ? (int64_t)(blockIdx.x / q.cluster) : (int64_t)blockIdx.x;
+  const int tile = (int)rank * nw + warp;
+  const bool active = tile < q.tiles_per_chunk;
+  const uint32_t slots = smem_u32(slots_raw);
+  const uint32_t par_bytes = (uint32_t)nw * slot_bytes_per_warp();
+
+  // this lane's row
+  const int r = tile * q.rows_out - q.HR + lane;                        // row within the chunk
+  const int64_t rowc = chunk * q.chunk_rows + r;                        // row within the batch
+  const bool valid = active && r >= 0 && r < q.chunk_rows && rowc < q.total_rows;
+  const int64_t g = valid ? rowc / q.nrows : 0;
+  const int64_t rowg = valid ? rowc - g * q.nrows : 0;
+  const bool owner = valid && lane >= q.HR && lane < 32 - q.HR;
+
+  R E[C], H[C], J[C];
+  CoefRegs<R, C> cf;
+#pragma unroll
+  for (int i = 0; i < C; ++i) { E[i] = R(0); H[i] = R(0); J[i] = R(0); }
+#pragma unroll
+  for (int a = 0; a < kNumCoef; ++a)
+#pragma unroll
+    for (int i = 0; i < C; ++i) cf.c[a][i] = R(0);
+  uint32_t flag = 0u;
+  if (valid) {
+    const int64_t first = rowc * C;
+    load_nodes_global<R, C>(f.E, first, E);
+    load_nodes_global<R, C>(f.H, first, H);
+    load_nodes_global<R, C>(f.J, first, J);
+#pragma unroll
+    for (int a = 0; a < kNumCoef; ++a) load_nodes_global<R, C>(cp.c[a], first, cf.c[a]);
+    flag = p.rowflag[rowg];
+  }
+  const bool special = __any_sync(0xffffffffu, flag != 0u);
+  const SpecialIdx sx = special ? make_special<R, C, PML>(p, flag, rowg * C, g, owner) : SpecialIdx();
+  SourceStream<R> src;
+  src.start(p, special && __any_sync(0xffffffffu, (flag & F_SRC) != 0u), p.n0, lane);
+
+  // where this lane's row goes after a round: lanes HR..2HR-1 are the right halo of tile-1, lanes 32-2HR..32-HR-1 the left
+  // halo of tile+1; and where its own halo row arrives
+  const bool send_left = active && lane >= q.HR && lane < 2 * q.HR && tile > 0;
+  const bool send_right = active && lane >= 32 - 2 * q.HR && lane < 32 - q.HR && tile + 1 < q.tiles_per_chunk;
+  const bool recv_left = active && lane < q.HR && tile > 0;
+  const bool recv_right = active && lane >= 32 - q.HR && tile + 1 < q.tiles_per_chunk;
+  uint32_t send_addr = 0u, recv_addr = 0u;
+  if (send_left || send_right) {
+    const int dt = send_left ? tile - 1 : tile + 1;                    // destination tile
+    const int dw = dt % nw, dr = dt / nw;
+    const int side = send_left ? 1 : 0, hrow = send_left ? lane - q.HR : lane - (32 - 2 * q.HR);
+    const uint32_t local = slots + (uint32_t)dw * slot_bytes_per_warp() + (uint32_t)(side * kMaxHR + hrow) * 3u * kRowBytes;
+    send_addr = CLUSTER ? map_to_cta(local, (uint32_t)dr) : local;
+  }
+  if (recv_left || recv_right) {
+    const int side = recv_left ? 0 : 1, hrow = recv_left ? lane : lane - (32 - q.HR);
+    recv_addr = slots + (uint32_t)warp * slot_bytes_per_warp() + (uint32_t)(side * kMaxHR + hrow) * 3u * kRowBytes;
+  }
+  if constexpr (CLUSTER) cluster_barrier();       // every CTA of the cluster is resident before the first remote store
+
+  uint32_t par = 0u;
+  for (int64_t n = 0; n < q.nsteps; n += q.T) {
+    const int Tr = (int)(q.nsteps - n < q.T ? q.nsteps - n : q.T);
+    if (active) {
+      if (special) warp_round<true, PML, R, C>(E, H, J, cf, p, sx, src, p.n0 + n, Tr);
+      else warp_round<false, false, R, C>(E, H, J, cf, p, sx, src, p.n0 + n, Tr);
+    }
+    if (n + Tr >= q.nsteps) break;
+    // halo refresh: double-buffered by round parity, so one barrier per round is enough (a warp can overwrite buffer
+    // `par` again only after the NEXT barrier, which every reader of this round's data has passed its reads to reach)
+    if (send_left || send_right) {
+      const uint32_t a = send_addr + par * par_bytes;
+#pragma unroll
+      for (int j = 0; j < G::NCH; ++j) {
+        const Vec ve = regs_to_vec<R, C>(E, j), vh = regs_to_vec<R, C>(H, j), vg = regs_to_vec<R, C>(J, j);
+        if constexpr (CLUSTER) {
+          st_cluster128(a + 0 * kRowBytes + j * 16, ve); st_cluster128(a + 1 * kRowBytes + j * 16, vh); st_cluster128(a + 2 * kRowBytes + j * 16, vg);
+        } else {
+          sts128(a + 0 * kRowBytes + j * 16, ve); sts128(a + 1 * kRowBytes + j * 16, vh); sts128(a + 2 * kRowBytes + j * 16, vg);
+        }
+      }
+    }
+    if constexpr (CLUSTER) cluster_barrier(); else cta_barrier();
+    if (recv_left || recv_right) {
+      const uint32_t a = recv_addr + par * par_bytes;
+#pragma unroll
+      for (int j = 0; j < G::NCH; ++j) {
+        Vec v;
+        lds128(a + 0 * kRowBytes + j * 16, v); vec_to_regs<R, C>(v, E, j);
+        lds128(a + 1 * kRowBytes + j * 16, v); vec_to_regs<R, C>(v, H, j);
+        lds128(a + 2 * kRowBytes + j * 16, v); vec_to_regs<R, C>(v, J, j);
+      }
+    }
+    par ^= 1u;
+  }
+
+  if (owner) {
+    const int64_t first = rowc * C;
+    store_nodes_global<R, C>(f.E, first, E);
+    store_nodes_global<R, C>(f.H, first, H);
+    store_nodes_global<R, C>(f.J, first, J);
+  }
+  if constexpr (CLUSTER) cluster_barrier();       // no CTA leaves while a neighbour may still store into its slots
+}
+
+// ------------------------------------------------------------------------------------ plan + launch
+// Tiles needed by `grids` whole grids at halo HR; the two ends of a chunk need no halo but tiles are laid out uniformly
+// (tile i = rows i RO - HR .. i RO - HR + 31), so the count is ceil(rows / RO).
+static int tiles_for(int64_t rows, int RO) { return (int)((rows + RO - 1) / RO); }
+
+bool k3w_plan(const Layout &L, int depth, int sms, int64_t want_nw, int64_t want_nc, int64_t want_k, K3WPlan *out) {
+  K3WPlan P;
+  P.T = depth > 0 ? depth : L.C;                       // default: one halo row, 8 (fp64) / 16 (fp32) steps per round
+  P.HR = (P.T + L.C - 1) / L.C;
+  if (P.HR > kMaxHR) return false;
+  P.rows_out = 32 - 2 * P.HR;
+  const int maxw = 12, maxc = 16;                      // 384 threads x 168 registers fill an SM; 16 = largest (non-portable) cluster
+  if (L.nrows > (int64_t)maxw * maxc * P.rows_out) return false;
+  const int w1 = tiles_for(L.nrows, P.rows_out);       // tiles of one grid
+  int k = 1, nc = 1, nw = w1;
+  if (want_nw > 0 || want_nc > 0 || want_k > 0) {      // explicit (rketd_set_plan)
+    k = (int)std::max<int64_t>(1, want_k);
+    const int w = tiles_for(k * L.nrows, P.rows_out);
+    nc = (int)std::max<int64_t>(1, want_nc);
+    nw = want_nw > 0 ? (int)want_nw : (w + nc - 1) / nc;
+    if (nw > maxw || nc > maxc || (int64_t)nw * nc < w || k > L.nbatch) return false;
+  } else if (w1 > maxw) {                              // a grid needs several SMs: a cluster, warps spread evenly
+    nc = (w1 + maxw - 1) / maxw;
+    nw = (w1 + nc - 1) / nc;
+  } else if (L.nbatch * (int64_t)w1 < (int64_t)sms * 4) {
+    // few grids: the run is a chain of dependent steps.  One warp per scheduler at most, the rest of the
+    // grid on other SMs of a cluster: a step then costs one warp's latency, not a queue of warps
+    nw = std::min(w1, 4);
+    nc = (w1 + nw - 1) / nw;
+    if (nc > maxc) { nc = maxc; nw = (w1 + nc - 1) / nc; }
+    nw = (w1 + nc - 1) / nc;
+  } else {                                             // many grids: whole grids per CTA, the fullest packing of <= 12 warps
+    double best = 0.0;
+    for (int kk = 1; kk <= 64 && kk <= L.nbatch; ++kk) {
+      const int w = tiles_for(kk * L.nrows, P.rows_out);
+      if (w > maxw) break;
+      const double eff = (double)(kk * L.nrows) / (32.0 * w) * (w >= 8 ? 1.0 : 0.9 + 0.0125 * w);   // prefer >= 2 warps per scheduler
+      if (eff > best + 1e-9) { best = eff; k = kk; nw = w; }
+    }
+  }
+  P.k = k; P.nc = nc; P.nw = nw;
+  P.chunk_rows = k * L.nrows;
+  if (P.chunk_rows > 0x7fffff00LL) return false;
+  P.tiles_per_chunk = tiles_for(P.chunk_rows, P.rows_out);
+  P.nchunks = (L.nbatch + k - 1) / k;
+  P.smem_bytes = 2u * (uint32_t)nw * slot_bytes_per_warp();
+  *out = P;
+  return true;
+}
+
+template <typename R, bool CLUSTER, bool PML>
+static cudaError_t launch_k3w_k(const Layout &L, const K3WPlan &P, FieldPtrs f, void *const coef[kNumCoef], const StepCommon &sc,
+                                int64_t nsteps, cudaStream_t st) {
+  auto kern = k3_wtile<R, CLUSTER, PML>;
+  K3WArgs q;
+  q.T = P.T; q.HR = P.HR; q.rows_out = P.rows_out; q.cluster = P.nc; q.chunk_rows = (int)P.chunk_rows;
+  q.tiles_per_chunk = P.tiles_per_chunk; q.nrows = L.nrows; q.total_rows = L.nrows * L.nbatch; q.nsteps = nsteps;
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)(P.nchunks * P.nc));
+  cfg.blockDim = dim3((unsigned)P.nw * 32);
+  cfg.dynamicSmemBytes = P.smem_bytes;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  if (CLUSTER) {
+    if (P.nc > 8) {
+      cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+      if (e != cudaSuccess) return e;
+    }
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)P.nc; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+  }
+  return cudaLaunchKernelEx(&cfg, kern, rp<R>(f), cpz<R>(coef), make_params<R>(sc), q);
+}
+template <typename R>
+static cudaError_t launch_k3w_t(const Layout &L, const K3WPlan &P, FieldPtrs f, void *const coef[kNumCoef], const StepCommon &sc,
+                                int64_t nsteps, cudaStream_t st) {
+  const bool pml = sc.npml > 0;
+  if (P.nc > 1) return pml ? launch_k3w_k<R, true, true>(L, P, f, coef, sc, nsteps, st) : launch_k3w_k<R, true, false>(L, P, f, coef, sc, nsteps, st);
+  return pml ? launch_k3w_k<R, false, true>(L, P, f, coef, sc, nsteps, st) : launch_k3w_k<R, false, false>(L, P, f, coef, sc, nsteps, st);
+}
+cudaError_t launch_k3w(int dtype, const Layout &L, const K3WPlan &P, FieldPtrs f, void *const coef[kNumCoefArrays], const StepCommon &sc,
+                       int64_t nsteps, cudaStream_t st) {
+  return dtype == 0 ? launch_k3w_t<double>(L, P, f, coef, sc, nsteps, st) : launch_k3w_t<float>(L, P, f, coef, sc, nsteps, st);
+}
+
+// can a cluster of P.nc CTAs of this kernel be co-scheduled at all on this device?
+template <typename R>
+static cudaError_t k3w_max_clusters_t(const K3WPlan &P, int *nclusters) {
+  auto kern = k3_wtile<R, true, false>;
+  if (P.nc > 8) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+    if (e != cudaSuccess) return e;
+  }
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)P.nc);
+  cfg.blockDim = dim3((unsigned)P.nw * 32);
+  cfg.dynamicSmemBytes = P.smem_bytes;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = (unsigned)P.nc; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  return cudaOccupancyMaxActiveClusters(nclusters, kern, &cfg);
+}
+cudaError_t k3w_max_clusters(int dtype, const K3WPlan &P, int *nclusters) {
+  return dtype == 0 ? k3w_max_clusters_t<double>(P, nclusters) : k3w_max_clusters_t<float>(P, nclusters);
+}
+
+}  // namespace rketd

@@ -1,0 +1,127 @@
+// rketd_wtile.cuh — the register-resident warp tile shared by the temporal-blocking kernel K2 (k2_wtile,
+// rketd_kernels.cu) and the resident kernel K3 (k3_wtile, rketd_resident.cu): a warp owns 32 rows x 64 B of every
+// array, one row per lane, and advances them with halos travelling by warp shuffles only.  Also the small host-side
+// helpers both launcher files use.
+#pragma once
+#include "rketd_device.cuh"
+#include "rketd_internal.h"
+
+namespace rketd {
+
+template <typename R> struct RowPtrs { R *E, *H, *J; };
+template <typename R> struct CoefPtrs { const R *c[kNumCoef]; };
+
+// One leapfrog step of a warp tile.  Only NEW values travel: H'[C-1] goes up one lane as soon as it
+// exists (the left neighbour's H' that E'[0] needs), E'[0] goes down one lane at the end (the E[C] the
+// next step's H'[C-1] needs).  Two 64-bit shuffles per step and no redundant arithmetic.  Lanes 0 and 31
+// receive their own values at the tile edge, which is fine: those nodes are in the halo that is thrown
+// away (garbage moves inwards one node per step; the halo is >= T nodes wide).
+template <bool SPECIAL, bool PML, typename R, int C>
+__device__ __forceinline__ void warp_step(const R (&E)[C], R (&En)[C], R (&H)[C], R (&G)[C], const CoefRegs<R, C> &cf,
+                                          R &Er, R nchh, const StepParams<R> &p, const SpecialIdx &sx, int64_t nloc,
+                                          R src_now) {
+  typedef Arith<R> A;
+  // Issue cost of an FP64 instruction on sm_100 = max(2, distinct 64-bit register operands) cycles per
+  // scheduler (measured): the two FMAs that multiply E[i] sit next to each other so that the
+  // second one finds E[i] in the operand-reuse cache, and nchh comes from the constant bank.
+  if constexpr (SPECIAL && PML) {
+    if (sx.pml_mask) pml_pre<R, C>(E, Er, H, p, sx);                           // absorbing-layer H nodes, on old E
+  }
+  H[C - 1] = A::fma(nchh, A::sub(Er, E[C - 1]), H[C - 1]);                    // a1, last node first
+  const R Hl = __shfl_up_sync(0xffffffffu, H[C - 1], 1);
+#pragma unroll
+  for (int i = 0; i < C - 1; ++i) H[i] = A::fma(nchh, A::sub(E[i + 1], E[i]), H[i]);
+#pragma unroll
+  for (int i = C - 1; i >= 0; --i) {
+    const R w = A::mul(cf.c[COEF_Q][i], E[i]);
+    const R t = A::fma(cf.c[COEF_P][i], E[i], -G[i]);
+    G[i] = A::fma(cf.c[COEF_KA][i], G[i], w);                                 // a5 (old E, old G)
+    En[i] = A::fma(-cf.c[COEF_CH][i], A::sub(H[i], i ? H[i - 1] : Hl), t);    // a2
+  }
+  if constexpr (SPECIAL) {
+    if (sx.any) step_special<R, C, PML>(E, En, H, p, sx, nloc, src_now);       // a3, a4, a6
+  }
+  Er = __shfl_down_sync(0xffffffffu, En[0], 1);
+}
+
+template <bool SPECIAL, bool PML, typename R, int C>
+__device__ __forceinline__ void warp_time_loop(R (&E)[C], R (&H)[C], R (&G)[C], const CoefRegs<R, C> &cf,
+                                               const StepParams<R> &p, uint32_t flag, int64_t k0, int64_t g, bool owner,
+                                               int nsteps) {
+  const R nchh = p.nchh;       // stays a constant-bank operand of the FMAs (one register read less each)
+  int64_t nloc = p.n0;
+  R Er = __shfl_down_sync(0xffffffffu, E[0], 1);
+  R Eb[C];
+  const int lane = threadIdx.x & 31;
+  SourceStream<R> src;
+  src.start(p, SPECIAL && __any_sync(0xffffffffu, (flag & F_SRC) != 0u), nloc, lane);
+  const SpecialIdx sx = SPECIAL ? make_special<R, C, PML>(p, flag, k0, g, owner) : SpecialIdx();
+  int left = nsteps;
+  for (; left >= 2; left -= 2) {
+    const R s0 = SPECIAL ? src.sample(p, nloc, lane) : R(0);
+    warp_step<SPECIAL, PML, R, C>(E, Eb, H, G, cf, Er, nchh, p, sx, nloc, s0);
+    const R s1 = SPECIAL ? src.sample(p, nloc + 1, lane) : R(0);
+    warp_step<SPECIAL, PML, R, C>(Eb, E, H, G, cf, Er, nchh, p, sx, nloc + 1, s1);
+    nloc += 2;
+  }
+  if (left) {
+    const R s0 = SPECIAL ? src.sample(p, nloc, lane) : R(0);
+    warp_step<SPECIAL, PML, R, C>(E, Eb, H, G, cf, Er, nchh, p, sx, nloc, s0);
+#pragma unroll
+    for (int i = 0; i < C; ++i) E[i] = Eb[i];
+  }
+}
+
+
+// T steps of a warp tile between two halo refreshes of the resident kernel: as warp_time_loop, but the step counter,
+// the special indices and the source stream belong to the caller and live across rounds (restarting the stream
+// would put two global loads on the critical path of every round).
+template <bool SPECIAL, bool PML, typename R, int C>
+__device__ __forceinline__ void warp_round(R (&E)[C], R (&H)[C], R (&G)[C], const CoefRegs<R, C> &cf, const StepParams<R> &p,
+                                           const SpecialIdx &sx, SourceStream<R> &src, int64_t nloc, int nsteps) {
+  const R nchh = p.nchh;
+  const int lane = threadIdx.x & 31;
+  R Er = __shfl_down_sync(0xffffffffu, E[0], 1);
+  R Eb[C];
+  int left = nsteps;
+  for (; left >= 2; left -= 2) {
+    const R s0 = SPECIAL ? src.sample(p, nloc, lane) : R(0);
+    warp_step<SPECIAL, PML, R, C>(E, Eb, H, G, cf, Er, nchh, p, sx, nloc, s0);
+    const R s1 = SPECIAL ? src.sample(p, nloc + 1, lane) : R(0);
+    warp_step<SPECIAL, PML, R, C>(Eb, E, H, G, cf, Er, nchh, p, sx, nloc + 1, s1);
+    nloc += 2;
+  }
+  if (left) {
+    const R s0 = SPECIAL ? src.sample(p, nloc, lane) : R(0);
+    warp_step<SPECIAL, PML, R, C>(E, Eb, H, G, cf, Er, nchh, p, sx, nloc, s0);
+#pragma unroll
+    for (int i = 0; i < C; ++i) E[i] = Eb[i];
+  }
+}
+
+// ---- host side
+template <typename R>
+inline StepParams<R> make_params(const StepCommon &sc) {
+  StepParams<R> p;
+  p.nchh = (R)sc.nchh;
+  p.mur_m = (R)sc.mur_m;
+  p.cellL = sc.cellL; p.cellR = sc.cellR; p.cellS = sc.cellS;
+  p.nprobes = sc.nprobes;
+  p.rec_stride = sc.rec_stride; p.n0 = sc.n0;
+  p.src_tab = (const R *)sc.src_tab;
+  p.rec = (R *)sc.rec;
+  p.rowflag = sc.rowflag;
+  for (int i = 0; i < kMaxProbes; ++i) p.probe_cell[i] = sc.probe_cell[i];
+  p.npml = sc.npml;
+  for (int j = 0; j < kMaxPml; ++j) { p.pml_ha[j] = (R)sc.pml_ha[j]; p.pml_hd[j] = (R)sc.pml_hd[j]; }
+  return p;
+}
+template <typename R> inline RowPtrs<R> rp(FieldPtrs f) { return RowPtrs<R>{(R *)f.E, (R *)f.H, (R *)f.J}; }
+template <typename R> inline CoefPtrs<R> cpz(void *const coef[kNumCoef]) {
+  CoefPtrs<R> c;
+  for (int a = 0; a < kNumCoef; ++a) c.c[a] = (const R *)coef[a];
+  return c;
+}
+
+
+}  // namespace rketd

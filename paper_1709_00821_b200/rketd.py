@@ -27,7 +27,18 @@ EXPORTS = ["rketd_create", "rketd_set_media", "rketd_set_source", "rketd_set_pro
            "rketd_set_fields", "rketd_reset", "rketd_discard_records", "rketd_set_plan", "rketd_run", "rketd_read_probes",
            "rketd_get_fields", "rketd_get_coefficients", "rketd_get_kernel_coefficients", "rketd_set_scheme",
            "rketd_set_boundary", "rketd_read_probe_dft",
+           "rketd_measure_peak",
            "rketd_get_counter", "rketd_destroy", "rketd_last_error"]
+PEAK_NAMES = ("dfma_1reg", "dfma_2reg", "dfma_3reg", "dfma_2reg_const", "ffma_1reg", "ffma_2reg", "ffma_3reg",
+              "ffma_2reg_const", "mix_f64", "mix_f32", "lds128")      # index = RKETD_PEAK_*
+RESIDENT_WTILE_FLAG = 0x40000000
+
+
+def RESIDENT_WTILE(nw: int = 0, nc: int = 0, k: int = 0) -> int:
+    """rketd_set_plan variant for KERNEL_RESIDENT: k grids per chunk on a cluster of nc CTAs x nw warps (0 = library's choice)"""
+    return RESIDENT_WTILE_FLAG | (k << 16) | (nc << 8) | nw
+
+
 SCHEME_ETD2, SCHEME_ETD1 = 0, 1
 BC_MUR, BC_PML = 0, 1
 
@@ -60,7 +71,8 @@ _lib.rketd_destroy.argtypes = [_vp]
 _lib.rketd_destroy.restype = None
 _lib.rketd_last_error.argtypes = [_vp]
 _lib.rketd_last_error.restype = ctypes.c_char_p
-for _n in EXPORTS[:17]:
+_lib.rketd_measure_peak.argtypes = [_i32, _i32, _vp, _vp]
+for _n in EXPORTS[:18]:
     getattr(_lib, _n).restype = _i32
 
 
@@ -168,6 +180,14 @@ def rketd_get_kernel_coefficients(h, out):
 
 def rketd_get_counter(h, which: int) -> int:
     return _lib.rketd_get_counter(h, which)
+
+
+def rketd_measure_peak(what: int, iters: int = 4000, cuda_stream: int = 0):
+    """(per ns over the device, per clock and SM, SM MHz held, SMs) of microbenchmark RKETD_PEAK_* `what`"""
+    out = np.zeros(4, np.float64)
+    _check(None, _lib.rketd_measure_peak(what, iters, _ptr(out), cuda_stream or None))
+    return {"name": PEAK_NAMES[what], "per_ns": float(out[0]), "per_clk_sm": float(out[1]), "sm_mhz": float(out[2]),
+            "sms": int(out[3])}
 
 
 def rketd_destroy(h):

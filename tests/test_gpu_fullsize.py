@@ -4,8 +4,8 @@ The oracle cannot run 2.7e11 cell updates in seconds, so it computes sampled out
   - long lines (configs 2, 4): pin P7 (domain of dependence, tests/test_oracle_pins.py) makes a
     windowed oracle run around a probe bit-identical to the full-line oracle, so every probe record
     and 64 random 4096-node windows of the final state are checked against windowed runs;
-  - batches (configs 3, 5): grids are independent, so a seeded sample of whole grids is checked
-    (including the grids with the extreme drawn parameters).
+  - batches (configs 3, 5): grids are independent; EVERY grid is compared with the OpenMP oracle (in chunks), the grids
+    with the extreme drawn parameters first.
 """
 import numpy as np
 import pytest
@@ -62,6 +62,9 @@ def _line_parity(rk, w, dtype, nwindows=64, wlen=4096):
     # random windows of the final state
     rng = np.random.default_rng(99)
     worst_win = 0.0
+    wp_max = max(float(w.media(lo, hi)[0].max()) for lo, hi in ((0, min(w.ncells, 1 << 21)), (w.ncells // 2, w.ncells // 2 + 1)))
+    floors = {"E": peak, "H": peak / 376.73, "J": 8.854e-12 * wp_max ** 2 * 20e-12 * peak}
+    worst_ns = {"E": 0.0, "H": 0.0, "J": 0.0}
     starts = list(rng.integers(0, w.ncells - wlen, nwindows - 3)) + [0, w.ncells - wlen, w.src_cell - wlen // 2]
     for a in starts:
         a = min(max(int(a), 0), w.ncells - wlen)
@@ -80,9 +83,13 @@ def _line_parity(rk, w, dtype, nwindows=64, wlen=4096):
             err = np.max(np.abs(g - r))
             worst_win = max(worst_win, err / scale)
             assert err <= max(TOL[dtype], DRIFT_K[dtype] * n * UNIT_ROUNDOFF[dtype] if dtype == "f32" else 0.0) * scale, (name, a, err / scale)
-            if name == "E":
-                assert err <= TOL[dtype] * peak, (name, a, err, peak)      # the north_star gate itself
-    print(f"{w.name} {dtype}: worst final-state window error / window peak {worst_win:.3e}")
+            # the north_star gate itself, for all three fields: error against the field peak of the GRID — E: the
+            # record peak; H: that over the vacuum impedance; J: eps0 wp_max^2 tau x peak (tau = 20 ps, the source
+            # width) — the floors of tests/test_gpu_parity.py::check_fields
+            assert err <= TOL[dtype] * floors[name], (name, a, err, floors[name])
+            worst_ns[name] = max(worst_ns[name], err / floors[name])
+    print(f"{w.name} {dtype}: worst final-state window error / window peak {worst_win:.3e}; against the grid peak "
+          f"E {worst_ns['E']:.3e}, H {worst_ns['H']:.3e}, J {worst_ns['J']:.3e}")
 
 
 def test_config2_full(rk):
@@ -96,34 +103,102 @@ def test_config4_full(rk, dtype):
     _line_parity(rk, wl.config4(), dtype)
 
 
+# ---- batches (configs 3, 5): EVERY grid against the OpenMP build of the oracle (pin P9: bit-identical to the serial
+# build), in chunks so that host memory stays bounded.  SURVEY §8(d) "CPU baseline plan" / BASELINE.md §3: all grids when
+# the oracle finishes in time, else >= 512 grids that include the extremes of every drawn parameter.  The grids are
+# therefore visited in the order: extremes first, then all grids in contiguous chunks; the loop stops early only when
+# BATCH_BUDGET_S of oracle time are spent (a slow host), never before 512 grids, and the test prints exactly how many
+# grids were compared.
+BATCH_BUDGET_S = 330.0
+_ORACLE_CACHE = {}
+
+
+def _oracle_batch(w, key, extremes, field, chunk):
+    """oracle results [nbatch, ...] (NaN rows where the budget ran out), cached per workload so that the fp32 and fp64
+    cases share one oracle run.  Order: the extreme grids one by one, then contiguous chunks of `chunk` grids from grid 0
+    (the draws are i.i.d. per grid, so a prefix is as good a seeded sample as any)."""
+    import time
+    if key in _ORACLE_CACHE:
+        return _ORACLE_CACHE[key]
+    out, done = None, np.zeros(w.nbatch, bool)
+    t0 = time.perf_counter()
+    groups = [(int(g), int(g) + 1) for g in dict.fromkeys(extremes)]
+    groups += [(b0, min(w.nbatch, b0 + chunk)) for b0 in range(0, w.nbatch, chunk)]
+    for b0, b1 in groups:
+        if done[b0:b1].all():
+            continue
+        if done.sum() >= 512 and time.perf_counter() - t0 > BATCH_BUDGET_S:
+            break
+        r = oracle.run_workload(w, b0=b0, b1=b1, omp=b1 - b0 > 1)[field]
+        if out is None:
+            out = np.full((w.nbatch,) + r.shape[1:], np.nan)
+        out[b0:b1] = r
+        done[b0:b1] = True
+    _ORACLE_CACHE[key] = (out, done, time.perf_counter() - t0)
+    return _ORACLE_CACHE[key]
+
+
+def _batch_check(name, dtype, gpu, ref, done, extremes, secs):
+    assert done[list(extremes)].all() and done.sum() >= min(512, len(done))
+    idx = np.flatnonzero(done)
+    d = np.abs(gpu[idx].astype(np.float64) - ref[idx]).reshape(len(idx), -1).max(1)
+    pk = np.abs(ref[idx]).reshape(len(idx), -1).max(1)
+    assert np.all(pk > 0), "vacuous: an oracle record is identically zero"
+    err = d / pk
+    worst = int(idx[np.argmax(err)])
+    print(f"{name} {dtype}: {len(idx)} of {len(done)} grids compared with the oracle ({secs:.0f} s of OpenMP oracle time), "
+          f"worst per-grid error {err.max():.3e} at grid {worst}, median {np.median(err):.3e}")
+    assert err.max() <= TOL[dtype], (worst, err.max())
+
+
 def test_config3_full(rk):
-    """4096 grids x 4096 nodes x 20 000 steps, full probe time series; 10 sampled grids vs the oracle."""
+    """4096 grids x 4096 nodes x 20 000 steps, full probe time series (the R/T sweep): every grid."""
     w = wl.config3()
     s = rk.Sim.from_workload(w, "f64")
     s.run(w.nsteps)
     rec = s.read_probes()
     assert s.counter(rk.CTR_KERNEL_USED) == rk.KERNEL_RESIDENT and rec.shape == (4096, 2, 20000)
     s.close()
-    wp, nu = w.media(2000, 2001, 0, 4096)      # the slab's first node carries each grid's drawn (wp, nu)
-    sample = {0, 4095, int(np.argmax(wp)), int(np.argmin(wp)), int(np.argmax(nu)), int(np.argmin(nu))}
-    sample |= {int(g) for g in np.random.default_rng(3).integers(0, 4096, 4)}
-    for g in sorted(sample):
-        ref = oracle.run_workload(w, b0=g, b1=g + 1)["rec"]
-        d = np.max(np.abs(rec[g] - ref[0])) / np.max(np.abs(ref))
-        assert d <= 1e-12, (g, d)
+    wp, nu = w.media(2000, 2401, 0, 4096)      # the slab starts at node 2000 and is 40..400 nodes thick
+    M = (wp > 0).sum(1)
+    assert M.min() >= 40 and M.max() <= 400
+    extremes = [0, 4095] + [int(f(a)) for a in (M, wp[:, 0], nu[:, 0]) for f in (np.argmin, np.argmax)]
+    ref, done, secs = _oracle_batch(w, "config3", extremes, "rec", 128)
+    _batch_check(w.name, "f64", rec, ref, done, extremes, secs)
+
+
+def _config5_extremes(w):
+    """grids holding the smallest / largest of each of the 8 layer widths, layer wp, layer nu, and of the total thickness"""
+    ex = [0, w.nbatch - 1]
+    widths, wps, nus = [], [], []
+    for b0 in range(0, w.nbatch, 8192):
+        wp, nu = w.media(319, 722, b0, min(w.nbatch, b0 + 8192))      # node 319 is vacuum; 8 layers of <= 50 nodes
+        key = wp + 1e-3 * nu
+        edges = np.nonzero(np.diff(key, axis=1) != 0)
+        e = edges[1].reshape(wp.shape[0], 9)                           # 9 interfaces per grid
+        widths.append(np.diff(e, axis=1))
+        rows = np.arange(wp.shape[0])[:, None]
+        wps.append(wp[rows, e[:, :8] + 1])
+        nus.append(nu[rows, e[:, :8] + 1])
+    widths, wps, nus = np.concatenate(widths), np.concatenate(wps), np.concatenate(nus)
+    assert widths.min() >= 5 and widths.max() <= 50
+    for a in (widths, wps, nus):
+        for l in range(8):
+            ex += [int(np.argmin(a[:, l])), int(np.argmax(a[:, l]))]
+    tot = widths.sum(1)
+    ex += [int(np.argmin(tot)), int(np.argmax(tot))]
+    return ex
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_config5_full(rk, dtype):
-    """65 536 grids x 1024 nodes x 5000 steps, |DFT| at 64 frequencies; 16 sampled grids vs the oracle."""
+    """65 536 grids x 1024 nodes x 5000 steps, |DFT| at 64 frequencies: every grid (one oracle run serves both types)."""
     w = wl.config5()
     s = rk.Sim.from_workload(w, dtype)
     s.run(w.nsteps)
     mag = s.read_probes().astype(np.float64)
     assert mag.shape == (65536, 2, 64) and s.counter(rk.CTR_KERNEL_USED) == rk.KERNEL_RESIDENT
     s.close()
-    sample = sorted({0, 65535} | {int(g) for g in np.random.default_rng(5).integers(0, 65536, 14)})
-    for g in sample:
-        ref = oracle.run_workload(w, b0=g, b1=g + 1)["dft_mag"]
-        d = np.max(np.abs(mag[g] - ref[0])) / np.max(np.abs(ref))
-        assert d <= TOL[dtype], (g, d)
+    extremes = _config5_extremes(w)
+    ref, done, secs = _oracle_batch(w, "config5", extremes, "dft_mag", 2048)
+    _batch_check(w.name, dtype, mag, ref, done, extremes, secs)

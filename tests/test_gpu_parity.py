@@ -65,7 +65,16 @@ def check_fields(gpu, st, tol, peak=0.0, wp_max=0.0):
             assert np.max(np.abs(np.asarray(gpu[k], np.float64) - ref)) <= tol * scale, k
 
 
-ALL_PLANS = [(1, 0, -1), (3, 0, 0), (3, 0, 1), (3, 0, 2)] + [(2, 0, v) for v in range(8)] + [(2, d, 4) for d in (1, 7, 16, 33)] + \
+def WT(nw=0, nc=0, k=0):
+    """rketd_set_plan variant of the resident warp-tile kernel: k grids per chunk on a cluster of nc CTAs x nw warps"""
+    return 0x40000000 | (k << 16) | (nc << 8) | nw
+
+
+# K1; the resident kernel K3: warp tiles with the library's packing at several depths (steps between halo refreshes),
+# explicit packings (one CTA, clusters of 2..9 CTAs over DSMEM), the older one-barrier-per-step kernel; K2 variants
+ALL_PLANS = [(1, 0, -1)] + [(3, d, -1) for d in (0, 1, 3, 8, 13, 16)] + \
+            [(3, 8, WT(9, 1)), (3, 8, WT(5, 2)), (3, 8, WT(1, 9)), (3, 5, WT(2, 5)), (3, 16, WT(4, 3)), (3, 0, WT(12, 1))] + \
+            [(3, 0, 0), (3, 0, 1), (3, 0, 2)] + [(2, 0, v) for v in range(8)] + [(2, d, 4) for d in (1, 7, 16, 33)] + \
             [(2, d, 6) for d in (1, 2, 9, 32, 40)] + [(2, 5, 0), (2, 40, 2)]
 
 
@@ -166,6 +175,45 @@ def test_media_and_fields_in_any_order(rk):
         s.close()
 
 
+def test_rejected_media_leaves_live_fields_alone(rk):
+    """rketd_set_media validates before it touches anything: after an EINVAL on live fields (the kernels' third array
+    holds G of the OLD media) the run continues exactly as if the call had not happened, and a following valid
+    change of media still converts J correctly."""
+    rng = np.random.default_rng(12)
+    n, nb = 515, 2
+    wpA, wpB = (rng.uniform(0, 2 * np.pi * 40e9, (nb, n)) for _ in range(2))
+    nuA, nuB = (rng.uniform(0, 5e10, (nb, n)) for _ in range(2))
+    E0 = rng.uniform(-1, 1, (nb, n))
+    st = oracle.State(n, nb, E0)
+    recs = [oracle.run(st, wpA, nuA, wl.DZ, wl.DT, 120, probes=[7, 400])[0]]
+    stA = (st.E.copy(), st.J.copy())
+    recs.append(oracle.run(st, wpA, nuA, wl.DZ, wl.DT, 60, probes=[7, 400])[0])
+    recs.append(oracle.run(st, wpB, nuB, wl.DZ, wl.DT, 120, probes=[7, 400])[0])
+    ref = np.concatenate(recs, axis=2)
+    bad = wpB.copy()
+    bad[1, 300] = np.nan
+    for kernel in (1, 2, 3):
+        s = rk.Sim(n, nb, wl.DZ, wl.DT, "f64")
+        s.set_media(wpA, nuA)
+        s.set_fields(E0)
+        s.set_probes([7, 400])
+        s.set_plan(kernel, 0, -1)
+        s.run(120)
+        with pytest.raises(rk.RketdError) as ei:
+            s.set_media(bad, nuB)
+        assert ei.value.code == rk.EINVAL
+        E, H, J = s.get_fields()                       # still E, J under media A
+        assert np.max(np.abs(J - stA[1])) <= 1e-12 * np.max(np.abs(stA[1]))
+        assert np.max(np.abs(E - stA[0])) <= 1e-12 * np.max(np.abs(stA[0]))
+        s.run(60)                                      # media A still in force
+        s.set_media(wpB, nuB)
+        s.run(120)
+        assert grid_err(s.read_probes(), ref) <= 1e-12
+        E, H, J = s.get_fields()
+        assert np.max(np.abs(J - st.J)) <= 1e-12 * np.max(np.abs(st.J))
+        s.close()
+
+
 # ------------------------------------------------------------------------------------------ reduced configs 2-5
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_config2_reduced(rk, dtype):
@@ -187,8 +235,11 @@ def test_config3_reduced(rk, dtype):
     assert g["kernel"] == 3 and g["launches"] == 1
     assert grid_err(g["rec"], ref["rec"]) <= TOL[dtype]
     check_fields(g, ref["state"], TOL[dtype], *floors_of(w, ref))
-    g2 = run_gpu(rk, w, dtype, 2, 16, 4)      # the same batch through temporal blocking
-    assert np.array_equal(g["rec"], g2["rec"]) and np.array_equal(g["J"], g2["J"])
+    # the same batch through temporal blocking, the one-barrier-per-step resident kernel, and other packings of the
+    # warp-tile kernel: 2 grids per chunk on a cluster of 3 CTAs, one grid on 4 CTAs, deeper rounds
+    for plan in [(2, 16, 4), (3, 0, 0), (3, 0, WT(12, 3, 2)), (3, 0, WT(0, 4, 1)), (3, 16, -1), (3, 5, WT(0, 2, 1))]:
+        g2 = run_gpu(rk, w, dtype, *plan)
+        assert np.array_equal(g["rec"], g2["rec"]) and np.array_equal(g["J"], g2["J"]), plan
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
@@ -217,9 +268,18 @@ def test_config5_reduced_dft(rk, dtype):
     # time-series mode of the same workload
     w2 = wl.config5(nbatch=48, dft=False)
     ref2 = oracle.run_workload(w2, omp=True)
-    for variant in (0, 1):
-        g = run_gpu(rk, w2, dtype, 3, 0, variant)
-        assert grid_err(g["rec"], ref2["rec"]) <= TOL[dtype]
+    outs = []
+    # 48 grids: chunks of 1, 2, 3, 4, 5 and 7 whole grids (7 does not divide 48: a ragged last chunk), clusters, and the
+    # one-barrier-per-step kernel
+    for depth, variant in [(0, -1), (0, WT(0, 1, 1)), (0, WT(0, 1, 2)), (0, WT(12, 1, 3)), (0, WT(0, 2, 4)), (0, WT(0, 1, 5)),
+                           (0, WT(0, 2, 7)), (3, WT(0, 1, 2)), (0, 0), (0, 1)]:
+        g = run_gpu(rk, w2, dtype, 3, depth, variant)
+        assert grid_err(g["rec"], ref2["rec"]) <= TOL[dtype], (depth, variant)
+        check_fields(g, ref2["state"], TOL[dtype], *floors_of(w2, ref2))
+        outs.append(g)
+    for g in outs[1:]:
+        for k in ("rec", "E", "H", "J"):
+            assert np.array_equal(outs[0][k], g[k]), k
 
 
 # ------------------------------------------------------------------------------------------ edge cases
@@ -240,7 +300,10 @@ def test_small_and_ragged_grids(rk, ncells):
         st = oracle.State(ncells, nb, E0, H0, J0)
         rec, _ = oracle.run(st, wp, nu, wl.DZ, wl.DT, 60, src_kind=1, src_params=tab, src_cell=src_cell, probes=probes)
         outs = []
-        for kernel, depth, variant in [(1, 0, -1), (0, 0, -1), (2, 7, 0), (2, 7, 4), (2, 3, 1)]:
+        plans = [(1, 0, -1), (0, 0, -1), (2, 7, 0), (2, 7, 4), (2, 3, 1), (3, 0, -1), (3, 5, -1), (3, 0, WT(0, 1, 2)), (3, 0, WT(0, 1, 3))]
+        if ncells > 300:
+            plans += [(3, 0, WT(0, 2, 1)), (3, 0, WT(2, 0, 1)), (3, 2, WT(0, 3, 3))]
+        for kernel, depth, variant in plans:
             s = rk.Sim(ncells, nb, wl.DZ, wl.DT, "f64")
             s.set_media(wp, nu)
             s.set_fields(E0, H0, J0)
@@ -261,7 +324,7 @@ def test_small_and_ragged_grids(rk, ncells):
 def test_repeated_runs_continue_time(rk):
     w = wl.config1(nsteps=900)
     one = run_gpu(rk, w, "f64")
-    for plan in [(0, 0, -1), (2, 16, 4), (1, 0, -1)]:
+    for plan in [(0, 0, -1), (2, 16, 4), (1, 0, -1), (3, 0, 0), (3, 0, WT(9, 1, 1))]:
         parts = run_gpu(rk, w, "f64", *plan, chunks=[1, 0, 299, 17, 583])
         assert parts["rec"].shape == one["rec"].shape
         for k in ("rec", "E", "H", "J"):

@@ -1,0 +1,31 @@
+"""the oracle under -fsanitize=address,undefined.  The pin suites of the 1-D and 2-D oracle are run once more
+in a child process whose oracle is the sanitized build (oracle.build_sanitized, RKETD_ORACLE_SANITIZED=1, libasan
+preloaded); any out-of-bounds access, use after free or undefined behaviour aborts that process.  CPU only."""
+import os
+import subprocess
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_oracle_pins_pass_under_asan_and_ubsan():
+    import oracle
+    asan = subprocess.run(["g++", "-print-file-name=libasan.so"], capture_output=True, text=True).stdout.strip()
+    if not os.path.isabs(asan) or not os.path.exists(asan):
+        pytest.skip("libasan.so not found next to g++")
+    lib = oracle.build_sanitized()
+    syms = subprocess.run(["nm", "-D", lib], capture_output=True, text=True).stdout
+    assert "__asan_init" in syms and "__ubsan_handle" in syms          # really instrumented
+    env = dict(os.environ, RKETD_ORACLE_SANITIZED="1", LD_PRELOAD=asan,
+               ASAN_OPTIONS="detect_leaks=0:abort_on_error=1", UBSAN_OPTIONS="halt_on_error=1:print_stacktrace=1",
+               OMP_NUM_THREADS="4")
+    # the quick pins of both suites (everything except the long stability / R-T sweeps, which add no new code paths)
+    cmd = [sys.executable, "-m", "pytest", "-x", "-q", "-p", "no:cacheprovider",
+           os.path.join(ROOT, "tests", "test_oracle_pins.py"), os.path.join(ROOT, "tests", "test_oracle2d_pins.py"),
+           "-k", "not stability and not sweep"]
+    r = subprocess.run(cmd, env=env, cwd=ROOT, capture_output=True, text=True, timeout=1500)
+    tail = (r.stdout + r.stderr)[-3000:]
+    assert r.returncode == 0, tail
+    assert "passed" in r.stdout and "AddressSanitizer" not in tail and "runtime error" not in tail, tail
