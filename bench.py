@@ -174,9 +174,9 @@ def measured_alu(dtype: str, stream: int):
 
 
 def alu_source(a) -> str:
-    return (f"measured live (rketd_measure_peak): {a['fma_best_form']} = {a['fma_lanes_per_clk_sm'][a['fma_best_form'].split('_', 1)[1]]} "
-            f"lanes/clk/SM x {a['sms']} SMs x {a['fma_sm_mhz']} MHz / {FP_INSTR_PER_CELL_STEP} instr per cell-step; "
-            "recorded run: profiles/r02_peaks.md")
+    return (f"measured live (rketd_measure_peak): {a['fma_best_form']} = {a['fma_best_lanes']} lanes/clk/SM x {a['sms']} SMs x "
+            f"{a['sm_max_mhz']:.0f} MHz (device maximum; the microbenchmark held {a['fma_sm_mhz_held']} MHz) / "
+            f"{FP_INSTR_PER_CELL_STEP} instr per cell-step; recorded run: profiles/r02_peaks.md")
 
 
 def cpu_baseline(w, target_updates_serial=6e8, target_updates_omp=2.5e9):

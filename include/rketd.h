@@ -155,6 +155,14 @@ int rketd_read_probes(rketd_sim *s, void *out, int64_t out_bytes, int64_t *nsamp
  * Synchronises.  ESTATE outside DFT mode; EINVAL if count is too small. */
 int rketd_read_probe_dft(rketd_sim *s, double *re, double *im, int64_t count);
 
+/* Reflection and transmission magnitudes of a sweep, formed on the device: `s` holds
+ * the slab grids, `vacuum` one all-vacuum grid (its grid 0 is used) run with the same source, probes, frequencies and
+ * step count; both in DFT mode.  R[g][m] = |X_s[g][probe_r][m] - X_v[probe_r][m]| / |X_v[probe_r][m]|,
+ * T[g][m] = |X_s[g][probe_t][m]| / |X_v[probe_t][m]|; probe_r, probe_t index the probe list; R, T [nbatch][nfreq] fp64
+ * (host or device), count = elements each can hold.  Synchronises both handles' streams.
+ * ESTATE outside DFT mode; EINVAL: different probes or frequencies, bad index, count too small. */
+int rketd_read_sweep_rt(rketd_sim *s, rketd_sim *vacuum, int probe_r, int probe_t, double *R, double *T, int64_t count);
+
 /* Copy the fields out ([nbatch][ncells], handle's dtype, host or device; any may be NULL).
  * Synchronises. */
 int rketd_get_fields(rketd_sim *s, void *E, void *H, void *J);

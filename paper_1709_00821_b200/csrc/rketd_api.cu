@@ -46,8 +46,17 @@ struct rketd_sim {
   int src_kind = RKETD_SRC_NONE;
   std::vector<double> src_params;
   int64_t src_cell = -1;
-  void *d_srctab = nullptr;
-  int64_t srctab_cap = 0;
+  // source samples of the global steps [srctab_step0, srctab_step0 + srctab_len): device table + the pinned host
+  // buffer it was uploaded from; kept across runs, so that a repeated run (rketd_reset + rketd_run) enqueues nothing
+  void *d_srctab = nullptr, *h_srctab = nullptr;
+  int64_t srctab_cap = 0, srctab_step0 = 0, srctab_len = 0;
+  bool srctab_valid = false;
+  // DFT mode: record segment and twiddle table, grow-only (no allocation or synchronisation inside rketd_run)
+  void *dft_rec = nullptr;
+  double2 *dft_tw = nullptr;
+  size_t dft_rec_bytes = 0, dft_tw_bytes = 0;
+  void *dft_out = nullptr;       // magnitudes staged for rketd_read_probes
+  size_t dft_out_bytes = 0;
   std::vector<int64_t> probes;
   std::vector<double> freqs;
   double *d_freqs = nullptr, *dft_re = nullptr, *dft_im = nullptr;
@@ -276,26 +285,33 @@ int resolve_kernel(rketd_sim *s) {
 // run nsteps steps whose probe samples go to rec ([nbatch][nprobes][nsteps] or nullptr)
 int run_segment(rketd_sim *s, int64_t nsteps, void *rec) {
   const Layout &L = s->L;
-  // source samples of this segment
+  // source samples of this segment: a slice of the kept table when it covers the steps, else the table is rebuilt
   const void *d_src = nullptr;
   if (s->src_kind != RKETD_SRC_NONE) {
-    if (s->srctab_cap < nsteps) {
-      if (s->d_srctab) cudaFree(s->d_srctab);
-      s->d_srctab = nullptr; s->srctab_cap = 0;
-      CU_TRY(s, cudaMalloc(&s->d_srctab, (size_t)nsteps * L.esize));
-      s->srctab_cap = nsteps;
+    const bool covered = s->srctab_valid && s->step >= s->srctab_step0 && s->step + nsteps <= s->srctab_step0 + s->srctab_len;
+    if (!covered) {
+      if (s->srctab_cap < nsteps) {
+        CU_TRY(s, cudaStreamSynchronize(s->stream));      // earlier launches may still read the old table
+        if (s->d_srctab) cudaFree(s->d_srctab);
+        if (s->h_srctab) cudaFreeHost(s->h_srctab);
+        s->d_srctab = s->h_srctab = nullptr; s->srctab_cap = 0; s->srctab_valid = false;
+        CU_TRY(s, cudaMalloc(&s->d_srctab, (size_t)nsteps * L.esize));
+        CU_TRY(s, cudaMallocHost(&s->h_srctab, (size_t)nsteps * L.esize));
+        s->srctab_cap = nsteps;
+      } else if (s->srctab_valid) {
+        CU_TRY(s, cudaStreamSynchronize(s->stream));      // the pinned buffer may still be in flight, the table in use
+      }
+      if (s->dtype == RKETD_F64) {
+        double *tab = (double *)s->h_srctab;
+        for (int64_t n = 0; n < nsteps; ++n) tab[n] = source_sample(s, s->step + n);
+      } else {
+        float *tab = (float *)s->h_srctab;
+        for (int64_t n = 0; n < nsteps; ++n) tab[n] = (float)source_sample(s, s->step + n);
+      }
+      CU_TRY(s, cudaMemcpyAsync(s->d_srctab, s->h_srctab, (size_t)nsteps * L.esize, cudaMemcpyHostToDevice, s->stream));
+      s->srctab_step0 = s->step; s->srctab_len = nsteps; s->srctab_valid = true;
     }
-    // (pageable source: cudaMemcpyAsync stages it before returning, so the local vector may die at once)
-    if (s->dtype == RKETD_F64) {
-      std::vector<double> tab((size_t)nsteps);
-      for (int64_t n = 0; n < nsteps; ++n) tab[(size_t)n] = source_sample(s, s->step + n);
-      CU_TRY(s, cudaMemcpyAsync(s->d_srctab, tab.data(), tab.size() * 8, cudaMemcpyHostToDevice, s->stream));
-    } else {
-      std::vector<float> tab((size_t)nsteps);
-      for (int64_t n = 0; n < nsteps; ++n) tab[(size_t)n] = (float)source_sample(s, s->step + n);
-      CU_TRY(s, cudaMemcpyAsync(s->d_srctab, tab.data(), tab.size() * 4, cudaMemcpyHostToDevice, s->stream));
-    }
-    d_src = s->d_srctab;
+    d_src = (const char *)s->d_srctab + (size_t)(s->step - s->srctab_step0) * L.esize;
   }
   StepCommon sc;
   std::memset(&sc, 0, sizeof(sc));
@@ -525,6 +541,7 @@ int rketd_set_boundary(rketd_sim *s, int kind, int npml, double grading, double 
 
 int rketd_set_source(rketd_sim *s, int kind, const double *params, int64_t nparams, int64_t cell) {
   if (!s) return RKETD_EINVAL;
+  s->srctab_valid = false;
   if (kind == RKETD_SRC_NONE) { s->src_kind = kind; s->src_params.clear(); s->src_cell = -1; s->flags_dirty = true; return RKETD_OK; }
   if (kind != RKETD_SRC_GAUSS_DERIV && kind != RKETD_SRC_TABLE) return fail(s, RKETD_EINVAL, "rketd_set_source: unknown kind");
   if (cell < 0 || cell >= s->L.ncells) return fail(s, RKETD_EINVAL, "rketd_set_source: cell outside the grid");
@@ -645,30 +662,39 @@ int rketd_run(rketd_sim *s, int64_t nsteps) {
     s->nsamples += nsteps;
     return RKETD_OK;
   }
-  // DFT mode (a7): records of a segment are reduced by a second kernel, then dropped
+  // DFT mode (a7): the records of a segment are reduced into the accumulators by a second kernel on the same stream
+  // and the segment buffer is reused; buffers live in the handle and only grow, so the call stays asynchronous
   const int nfreq = (int)s->freqs.size();
   const int64_t seg_max = std::max<int64_t>(64, std::min<int64_t>(nsteps, ((int64_t)1 << 29) / (nseries * L.esize)));
-  void *buf = nullptr;
-  double2 *tw = nullptr;
-  CU_TRY(s, cudaMalloc(&buf, (size_t)nseries * std::min(seg_max, nsteps) * L.esize));
-  cudaError_t e = cudaMalloc(&tw, (size_t)std::min(seg_max, nsteps) * nfreq * sizeof(double2));
-  if (e != cudaSuccess) { cudaFree(buf); CU_TRY(s, e); }
-  int rc = RKETD_OK;
-  for (int64_t n = 0; n < nsteps && rc == RKETD_OK; n += seg_max) {
+  const size_t need_rec = (size_t)nseries * std::min(seg_max, nsteps) * L.esize;
+  const size_t need_tw = (size_t)std::min(seg_max, nsteps) * nfreq * sizeof(double2);
+  if (need_rec > s->dft_rec_bytes || need_tw > s->dft_tw_bytes) {
+    CU_TRY(s, cudaStreamSynchronize(s->stream));           // (growing only: an earlier run may still use the old buffers)
+    if (need_rec > s->dft_rec_bytes) {
+      if (s->dft_rec) cudaFree(s->dft_rec);
+      s->dft_rec = nullptr; s->dft_rec_bytes = 0;
+      CU_TRY(s, cudaMalloc(&s->dft_rec, need_rec));
+      s->dft_rec_bytes = need_rec;
+    }
+    if (need_tw > s->dft_tw_bytes) {
+      if (s->dft_tw) cudaFree(s->dft_tw);
+      s->dft_tw = nullptr; s->dft_tw_bytes = 0;
+      CU_TRY(s, cudaMalloc((void **)&s->dft_tw, need_tw));
+      s->dft_tw_bytes = need_tw;
+    }
+  }
+  for (int64_t n = 0; n < nsteps; n += seg_max) {
     const int64_t seg = std::min(seg_max, nsteps - n);
     const int64_t step0 = s->step;
-    rc = run_segment(s, seg, buf);
-    if (rc) break;
-    e = launch_twiddles(s->d_freqs, nfreq, step0, seg, s->dt, tw, s->stream);
-    if (e == cudaSuccess) e = launch_dft_accumulate(s->dtype, buf, nseries, seg, tw, nfreq, s->dft_re, s->dft_im, s->stream);
+    int rc = run_segment(s, seg, s->dft_rec);
+    if (rc) return rc;
+    cudaError_t e = launch_twiddles(s->d_freqs, nfreq, step0, seg, s->dt, s->dft_tw, s->stream);
+    if (e == cudaSuccess) e = launch_dft_accumulate(s->dtype, s->dft_rec, nseries, seg, s->dft_tw, nfreq, s->dft_re, s->dft_im, s->stream);
     s->ctr_launches += 2;
-    if (e != cudaSuccess) rc = fail(s, RKETD_ECUDA, std::string("dft: ") + cudaGetErrorString(e));
+    if (e != cudaSuccess) return fail(s, RKETD_ECUDA, std::string("dft: ") + cudaGetErrorString(e));
     s->nsamples += seg;
   }
-  cudaStreamSynchronize(s->stream);   // buf and tw are freed below
-  cudaFree(buf);
-  cudaFree(tw);
-  return rc;
+  return RKETD_OK;
 }
 
 int rketd_read_probes(rketd_sim *s, void *out, int64_t out_bytes, int64_t *nsamples) {
@@ -683,14 +709,20 @@ int rketd_read_probes(rketd_sim *s, void *out, int64_t out_bytes, int64_t *nsamp
   if (out_bytes < need) return fail(s, RKETD_EINVAL, "rketd_read_probes: out buffer too small");
   if (need == 0) { CU_TRY(s, cudaStreamSynchronize(s->stream)); return RKETD_OK; }
   if (dft) {
-    void *tmp = nullptr;
-    CU_TRY(s, cudaMalloc(&tmp, (size_t)need));
-    cudaError_t e = launch_dft_magnitude(s->dtype, s->dft_re, s->dft_im, nseries * per, tmp, s->stream);
+    void *dst = out;
+    if (!is_device_ptr(out)) {           // magnitudes are formed on the device, then copied out
+      if ((size_t)need > s->dft_out_bytes) {
+        if (s->dft_out) cudaFree(s->dft_out);
+        s->dft_out = nullptr; s->dft_out_bytes = 0;
+        CU_TRY(s, cudaMalloc(&s->dft_out, (size_t)need));
+        s->dft_out_bytes = (size_t)need;
+      }
+      dst = s->dft_out;
+    }
+    CU_TRY(s, launch_dft_magnitude(s->dtype, s->dft_re, s->dft_im, nseries * per, dst, s->stream));
     ++s->ctr_launches;
-    if (e == cudaSuccess) e = cudaMemcpyAsync(out, tmp, (size_t)need, cudaMemcpyDefault, s->stream);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
-    cudaFree(tmp);
-    CU_TRY(s, e);
+    if (dst != out) CU_TRY(s, cudaMemcpyAsync(out, dst, (size_t)need, cudaMemcpyDefault, s->stream));
+    CU_TRY(s, cudaStreamSynchronize(s->stream));
     return RKETD_OK;
   }
   int64_t o = 0;
@@ -713,6 +745,32 @@ int rketd_read_probe_dft(rketd_sim *s, double *re, double *im, int64_t count) {
     CU_TRY(s, cudaMemcpyAsync(im, s->dft_im, (size_t)n * sizeof(double), cudaMemcpyDefault, s->stream));
   }
   CU_TRY(s, cudaStreamSynchronize(s->stream));
+  return RKETD_OK;
+}
+
+int rketd_read_sweep_rt(rketd_sim *s, rketd_sim *vac, int probe_r, int probe_t, double *R, double *T, int64_t count) {
+  if (!s || !vac) return fail(s, RKETD_EINVAL, "rketd_read_sweep_rt: NULL handle");
+  if (s->freqs.empty() || vac->freqs.empty()) return fail(s, RKETD_ESTATE, "rketd_read_sweep_rt: both handles must be in DFT mode");
+  const int np = (int)s->probes.size(), nf = (int)s->freqs.size();
+  if (vac->probes != s->probes || vac->freqs != s->freqs)
+    return fail(s, RKETD_EINVAL, "rketd_read_sweep_rt: the vacuum handle needs the same probes and frequencies");
+  if (probe_r < 0 || probe_r >= np || probe_t < 0 || probe_t >= np || !R || !T || count < s->L.nbatch * (int64_t)nf)
+    return fail(s, RKETD_EINVAL, "rketd_read_sweep_rt: bad probe index or buffers too small");
+  CU_TRY(s, cudaStreamSynchronize(vac->stream));           // the two handles may live on different streams
+  const size_t bytes = (size_t)s->L.nbatch * nf * sizeof(double);
+  double *dR = R, *dT = T;
+  void *tmp = nullptr;
+  if (!is_device_ptr(R) || !is_device_ptr(T)) {
+    CU_TRY(s, cudaMalloc(&tmp, 2 * bytes));
+    dR = (double *)tmp; dT = dR + (size_t)s->L.nbatch * nf;
+  }
+  cudaError_t e = launch_sweep_rt(s->dft_re, s->dft_im, vac->dft_re, vac->dft_im, s->L.nbatch, np, nf, probe_r, probe_t, dR, dT, s->stream);
+  ++s->ctr_launches;
+  if (e == cudaSuccess && tmp) e = cudaMemcpyAsync(R, dR, bytes, cudaMemcpyDefault, s->stream);
+  if (e == cudaSuccess && tmp) e = cudaMemcpyAsync(T, dT, bytes, cudaMemcpyDefault, s->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
+  if (tmp) cudaFree(tmp);
+  CU_TRY(s, e);
   return RKETD_OK;
 }
 
@@ -804,6 +862,10 @@ void rketd_destroy(rketd_sim *s) {
   if (s->rowflag) cudaFree(s->rowflag);
   if (s->d_bad) cudaFree(s->d_bad);
   if (s->d_srctab) cudaFree(s->d_srctab);
+  if (s->h_srctab) cudaFreeHost(s->h_srctab);
+  if (s->dft_rec) cudaFree(s->dft_rec);
+  if (s->dft_tw) cudaFree(s->dft_tw);
+  if (s->dft_out) cudaFree(s->dft_out);
   for (auto &c : s->chunks) cudaFree(c.buf);
   if (s->spare_buf) cudaFree(s->spare_buf);
   if (s->dft_re) cudaFree(s->dft_re);

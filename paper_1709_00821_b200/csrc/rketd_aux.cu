@@ -266,4 +266,26 @@ cudaError_t launch_dft_magnitude(int dtype, const double *re, const double *im, 
   return cudaGetLastError();
 }
 
+// |R| = |X_slab - X_vac| / |X_vac| at probe pr, |T| = |X_slab| / |X_vac| at probe pt, per grid and frequency
+// (reflection and transmission "by Fourier transform" of the records; the vacuum run gives the
+// incident spectrum).  Complex differences and moduli in fp64.
+__global__ void sweep_rt_kernel(const double *__restrict__ sre, const double *__restrict__ sim, const double *__restrict__ vre,
+                                const double *__restrict__ vim, int64_t nbatch, int nprobes, int nfreq, int pr, int pt,
+                                double *R, double *T) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= nbatch * nfreq) return;
+  const int64_t g = idx / nfreq;
+  const int m = (int)(idx - g * nfreq);
+  const int64_t ir = (g * nprobes + pr) * nfreq + m, it = (g * nprobes + pt) * nfreq + m;
+  const int64_t vr = (int64_t)pr * nfreq + m, vt = (int64_t)pt * nfreq + m;      // vacuum: grid 0
+  R[idx] = __ddiv_rn(hypot(__dsub_rn(sre[ir], vre[vr]), __dsub_rn(sim[ir], vim[vr])), hypot(vre[vr], vim[vr]));
+  T[idx] = __ddiv_rn(hypot(sre[it], sim[it]), hypot(vre[vt], vim[vt]));
+}
+cudaError_t launch_sweep_rt(const double *sre, const double *sim, const double *vre, const double *vim, int64_t nbatch,
+                            int nprobes, int nfreq, int pr, int pt, double *R, double *T, cudaStream_t st) {
+  const int64_t n = nbatch * nfreq;
+  sweep_rt_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(sre, sim, vre, vim, nbatch, nprobes, nfreq, pr, pt, R, T);
+  return cudaGetLastError();
+}
+
 }  // namespace rketd

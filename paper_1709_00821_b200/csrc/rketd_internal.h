@@ -120,6 +120,9 @@ cudaError_t launch_dft_accumulate(int dtype, const void *rec, int64_t nseries, i
 cudaError_t launch_dft_magnitude(int dtype, const double *re, const double *im, int64_t n, void *out,
                                  cudaStream_t st);
 
+cudaError_t launch_sweep_rt(const double *sre, const double *sim, const double *vre, const double *vim, int64_t nbatch,
+                            int nprobes, int nfreq, int pr, int pt, double *R, double *T, cudaStream_t st);
+
 extern const double kC0, kMu0, kEps0;
 
 }  // namespace rketd

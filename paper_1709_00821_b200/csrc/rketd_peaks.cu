@@ -27,11 +27,19 @@ __device__ __forceinline__ unsigned long long globaltimer_ns() {
   asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
   return t;
 }
+// Block 0 times itself: earliest start and latest end over ALL its warps (the scheduler favours the oldest warps, so one
+// warp's own span would overstate the rate), clock64 (same SM) against globaltimer.
 __device__ __forceinline__ void stamp_begin(Stamp *st) {
-  if (threadIdx.x == 0 && blockIdx.x == 0) { st->ns0 = globaltimer_ns(); st->clk0 = clock64(); }
+  if (blockIdx.x == 0 && (threadIdx.x & 31) == 0) {
+    atomicMin(&st->ns0, globaltimer_ns());
+    atomicMin(&st->clk0, (unsigned long long)clock64());
+  }
 }
 __device__ __forceinline__ void stamp_end(Stamp *st) {
-  if (threadIdx.x == 0 && blockIdx.x == 0) { st->clk1 = clock64(); st->ns1 = globaltimer_ns(); }
+  if (blockIdx.x == 0 && (threadIdx.x & 31) == 0) {
+    atomicMax(&st->clk1, (unsigned long long)clock64());
+    atomicMax(&st->ns1, globaltimer_ns());
+  }
 }
 
 constexpr int kChains = 8, kUnroll = 8;
@@ -125,16 +133,16 @@ __global__ void __launch_bounds__(1024) lds_kernel(float *out, int iters, Stamp 
   __syncthreads();
   const uint32_t base = smem_u32(tile);
   float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-  uint32_t off = (threadIdx.x & 1023u) * 16u;
+  uint32_t off = threadIdx.x * 16u;                            // lane stride 16 B: conflict-free, 512 B per warp instruction
   stamp_begin(st);
   for (int it = 0; it < iters; ++it) {
 #pragma unroll
-    for (int u = 0; u < 8; ++u) {
+    for (int u = 0; u < 8; ++u) {                              // eight different addresses per iteration
       float4 v;
-      lds128(base + ((off + u * 16384u) & 32767u), v);       // lane stride 16 B: conflict-free, 512 B per warp instruction
+      lds128(base + ((off + u * 4096u) & 32767u), v);
       acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;
     }
-    off = (off + 16u) & 16383u;
+    off += 16u;
   }
   stamp_end(st);
   if (acc.x + acc.y + acc.z + acc.w == 123.456f) out[0] = acc.x;
@@ -168,7 +176,9 @@ extern "C" int rketd_measure_peak(int what, int iters, double *out, void *cuda_s
   cudaMemcpyAsync(buf, f32 ? (const void *)hf : (const void *)hd, f32 ? sizeof(hf) : sizeof(hd), cudaMemcpyHostToDevice, st);
   double per_thread = 0.0;          // thread-instructions (or bytes) per thread
   int threads = 1024, blocks = sms;
+  const Stamp stamp0 = {~0ull, 0ull, ~0ull, 0ull};
   for (int rep = 0; rep < 2; ++rep) {          // first pass warms up (clocks, instruction cache)
+    cudaMemcpyAsync(stamp, &stamp0, sizeof(Stamp), cudaMemcpyHostToDevice, st);
     switch (what) {
       case RKETD_PEAK_DFMA_1REG: dfma_kernel<1><<<blocks, threads, 0, st>>>((double *)buf, (double *)buf + 300, iters, 1e-9, stamp); break;
       case RKETD_PEAK_DFMA_2REG: dfma_kernel<2><<<blocks, threads, 0, st>>>((double *)buf, (double *)buf + 300, iters, 1e-9, stamp); break;

@@ -96,6 +96,7 @@ __global__ void __launch_bounds__(384, 1) k3_wtile(RowPtrs<R> f, CoefPtrs<R> cp,
   }
   const bool special = __any_sync(0xffffffffu, flag != 0u);
   const SpecialIdx sx = special ? make_special<R, C, PML>(p, flag, rowg * C, g, owner) : SpecialIdx();
+  const WarpSpecial ws = special ? make_warp_special<R, C, PML>(p, sx) : WarpSpecial();
   SourceStream<R> src;
   src.start(p, special && __any_sync(0xffffffffu, (flag & F_SRC) != 0u), p.n0, lane);
 
@@ -123,8 +124,8 @@ __global__ void __launch_bounds__(384, 1) k3_wtile(RowPtrs<R> f, CoefPtrs<R> cp,
   for (int64_t n = 0; n < q.nsteps; n += q.T) {
     const int Tr = (int)(q.nsteps - n < q.T ? q.nsteps - n : q.T);
     if (active) {
-      if (special) warp_round<true, PML, R, C>(E, H, J, cf, p, sx, src, p.n0 + n, Tr);
-      else warp_round<false, false, R, C>(E, H, J, cf, p, sx, src, p.n0 + n, Tr);
+      if (special) warp_round<true, PML, R, C>(E, H, J, cf, p, sx, ws, src, p.n0 + n, Tr);
+      else warp_round<false, false, R, C>(E, H, J, cf, p, sx, ws, src, p.n0 + n, Tr);
     }
     if (n + Tr >= q.nsteps) break;
     // halo refresh: double-buffered by round parity, so one barrier per round is enough (a warp can overwrite buffer
@@ -185,23 +186,30 @@ bool k3w_plan(const Layout &L, int depth, int sms, int64_t want_nw, int64_t want
     nc = (int)std::max<int64_t>(1, want_nc);
     nw = want_nw > 0 ? (int)want_nw : (w + nc - 1) / nc;
     if (nw > maxw || nc > maxc || (int64_t)nw * nc < w || k > L.nbatch) return false;
-  } else if (w1 > maxw) {                              // a grid needs several SMs: a cluster, warps spread evenly
-    nc = (w1 + maxw - 1) / maxw;
-    nw = (w1 + nc - 1) / nc;
   } else if (L.nbatch * (int64_t)w1 < (int64_t)sms * 4) {
     // few grids: the run is a chain of dependent steps.  One warp per scheduler at most, the rest of the
     // grid on other SMs of a cluster: a step then costs one warp's latency, not a queue of warps
     nw = std::min(w1, 4);
     nc = (w1 + nw - 1) / nw;
-    if (nc > maxc) { nc = maxc; nw = (w1 + nc - 1) / nc; }
+    if (nc > maxc) nc = maxc;
     nw = (w1 + nc - 1) / nc;
-  } else {                                             // many grids: whole grids per CTA, the fullest packing of <= 12 warps
-    double best = 0.0;
-    for (int kk = 1; kk <= 64 && kk <= L.nbatch; ++kk) {
-      const int w = tiles_for(kk * L.nrows, P.rows_out);
-      if (w > maxw) break;
-      const double eff = (double)(kk * L.nrows) / (32.0 * w) * (w >= 8 ? 1.0 : 0.9 + 0.0125 * w);   // prefer >= 2 warps per scheduler
-      if (eff > best + 1e-9) { best = eff; k = kk; nw = w; }
+  } else {
+    // many grids: throughput.  Score of a packing = rows that are real work / rows the warps hold, times how evenly
+    // the warps load the four schedulers of an SM (the busiest one sets the pace: nw / (4 ceil(nw / 4))); a cluster
+    // pays a little for its wider barrier.  k whole grids per chunk, up to 4 CTAs per chunk.
+    double best = -1.0;
+    for (int c = 1; c <= 4; ++c)
+      for (int kk = 1; kk <= 256 && kk <= L.nbatch; ++kk) {
+        const int w = tiles_for(kk * L.nrows, P.rows_out);
+        const int n = (w + c - 1) / c;
+        if (n > maxw) break;
+        if (c > 1 && w <= (c - 1) * maxw) continue;          // fits a smaller cluster
+        const double score = (double)(kk * L.nrows) / (32.0 * n * c) * ((double)n / (4.0 * ((n + 3) / 4))) * (c > 1 ? 0.97 : 1.0);
+        if (score > best + 1e-9) { best = score; k = kk; nc = c; nw = n; }
+      }
+    if (best < 0.0) {                                    // a grid needs more than 4 SMs: warps spread evenly over a cluster
+      nc = (w1 + maxw - 1) / maxw;
+      nw = (w1 + nc - 1) / nc;
     }
   }
   P.k = k; P.nc = nc; P.nw = nw;

@@ -65,19 +65,33 @@ def measure(what: int, iters: int = 4000, seconds: float = 0.0, stream: int = 0)
     return r
 
 
-def alu_peaks(dtype: str, stream: int = 0, iters: int = 4000):
-    """What bench.py divides by: the best FMA issue rate of `dtype` (lanes per clock and SM, the clock it held) and the
-    issue ceiling of the stencil's own 7-instruction mix, each as Gcell/s = lanes x SMs x clock / 7."""
+def max_sm_mhz(index: int = 0) -> float:
+    try:
+        import pynvml
+        pynvml.nvmlInit()
+        return float(pynvml.nvmlDeviceGetMaxClockInfo(pynvml.nvmlDeviceGetHandleByIndex(index), pynvml.NVML_CLOCK_SM))
+    except Exception:
+        return 1965.0            # B200 (MEASURED_PEAKS.json sm_max_mhz)
+
+
+def alu_peaks(dtype: str, stream: int = 0, iters: int = 4000, index: int = 0):
+    """What bench.py divides by.  The microbenchmarks give lanes per clock and SM (clock-invariant: the run's own cycle
+    counter) for the best FMA form of `dtype` and for the stencil's own 7-instruction mix; the ceilings in Gcell/s are
+    lanes x SMs x the device's MAXIMUM SM clock / 7 — the clock the microbenchmark happened to hold (it may run right
+    after a power-capped stretch) is reported beside them, not folded in."""
     from . import rketd
     base = 0 if dtype == "f64" else 4
     forms = {n: rketd.rketd_measure_peak(base + i, iters, stream) for i, n in enumerate(("1reg", "2reg", "3reg", "2reg_const"))}
     mix = rketd.rketd_measure_peak(8 if dtype == "f64" else 9, iters, stream)
-    best = max(forms.values(), key=lambda r: r["per_ns"])
+    best = max(forms.values(), key=lambda r: r["per_clk_sm"])
+    mhz = max_sm_mhz(index)
+    to_gcells = lambda lanes: lanes * best["sms"] * mhz * 1e6 / FP_INSTR_PER_CELL_STEP / 1e9
     return {"fma_lanes_per_clk_sm": {k: round(v["per_clk_sm"], 2) for k, v in forms.items()},
-            "fma_best_form": best["name"], "fma_sm_mhz": round(best["sm_mhz"], 1), "sms": best["sms"],
-            "fma_peak_gcells": best["per_ns"] / FP_INSTR_PER_CELL_STEP,
-            "mix_lanes_per_clk_sm": round(mix["per_clk_sm"], 2), "mix_sm_mhz": round(mix["sm_mhz"], 1),
-            "mix_peak_gcells": mix["per_ns"] / FP_INSTR_PER_CELL_STEP}
+            "fma_best_form": best["name"], "fma_best_lanes": round(best["per_clk_sm"], 2), "fma_sm_mhz_held": round(best["sm_mhz"], 1),
+            "sms": best["sms"], "sm_max_mhz": mhz,
+            "fma_peak_gcells": to_gcells(best["per_clk_sm"]),
+            "mix_lanes_per_clk_sm": round(mix["per_clk_sm"], 2), "mix_sm_mhz_held": round(mix["sm_mhz"], 1),
+            "mix_peak_gcells": to_gcells(mix["per_clk_sm"])}
 
 
 def main(argv):
@@ -94,8 +108,8 @@ def main(argv):
               f"{str(r['nvml_sm_mhz_min']):>13s} {str(r['power_w_max']):>12s}   ({unit}; {r['sms']} SMs)")
     for dt in ("f64", "f32"):
         p = alu_peaks(dt, iters=iters)
-        print(f"{dt}: FMA peak {p['fma_peak_gcells']:.0f} Gcell/s ({p['fma_best_form']}, {p['fma_sm_mhz']} MHz), "
-              f"stencil-mix issue ceiling {p['mix_peak_gcells']:.0f} Gcell/s ({p['mix_lanes_per_clk_sm']} lanes/clk/SM at {p['mix_sm_mhz']} MHz)")
+        print(f"{dt}: FMA peak {p['fma_peak_gcells']:.0f} Gcell/s ({p['fma_best_form']}: {p['fma_best_lanes']} lanes/clk/SM x {p['sms']} SMs x "
+              f"{p['sm_max_mhz']:.0f} MHz / 7), stencil-mix issue ceiling {p['mix_peak_gcells']:.0f} Gcell/s ({p['mix_lanes_per_clk_sm']} lanes/clk/SM)")
 
 
 if __name__ == "__main__":

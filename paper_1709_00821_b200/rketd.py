@@ -27,7 +27,7 @@ EXPORTS = ["rketd_create", "rketd_set_media", "rketd_set_source", "rketd_set_pro
            "rketd_set_fields", "rketd_reset", "rketd_discard_records", "rketd_set_plan", "rketd_run", "rketd_read_probes",
            "rketd_get_fields", "rketd_get_coefficients", "rketd_get_kernel_coefficients", "rketd_set_scheme",
            "rketd_set_boundary", "rketd_read_probe_dft",
-           "rketd_measure_peak",
+           "rketd_read_sweep_rt", "rketd_measure_peak",
            "rketd_get_counter", "rketd_destroy", "rketd_last_error"]
 PEAK_NAMES = ("dfma_1reg", "dfma_2reg", "dfma_3reg", "dfma_2reg_const", "ffma_1reg", "ffma_2reg", "ffma_3reg",
               "ffma_2reg_const", "mix_f64", "mix_f32", "lds128")      # index = RKETD_PEAK_*
@@ -72,7 +72,8 @@ _lib.rketd_destroy.restype = None
 _lib.rketd_last_error.argtypes = [_vp]
 _lib.rketd_last_error.restype = ctypes.c_char_p
 _lib.rketd_measure_peak.argtypes = [_i32, _i32, _vp, _vp]
-for _n in EXPORTS[:18]:
+_lib.rketd_read_sweep_rt.argtypes = [_vp, _vp, _i32, _i32, _vp, _vp, _i64]
+for _n in EXPORTS[:19]:
     getattr(_lib, _n).restype = _i32
 
 
@@ -146,6 +147,11 @@ def rketd_set_scheme(h, scheme: int):
 
 def rketd_read_probe_dft(h, re, im):
     _check(h, _lib.rketd_read_probe_dft(h, _ptr(re), _ptr(im), re.size if isinstance(re, np.ndarray) else re.numel()))
+
+
+def rketd_read_sweep_rt(h, h_vacuum, probe_r: int, probe_t: int, R, T):
+    _check(h, _lib.rketd_read_sweep_rt(h, h_vacuum, probe_r, probe_t, _ptr(R), _ptr(T),
+                                       R.size if isinstance(R, np.ndarray) else R.numel()))
 
 
 def rketd_set_boundary(h, kind: int, npml: int = 5, grading: float = 3.0, R0: float = 1e-6):
@@ -266,6 +272,14 @@ class Sim:
         im = np.empty_like(re)
         rketd_read_probe_dft(self.h, re, im)
         return re + 1j * im
+
+    def read_sweep_rt(self, vacuum: "Sim", probe_r: int = 0, probe_t: int = 1):
+        """(|R|, |T|) [nbatch][nfreq] of this slab batch against the vacuum handle, formed on the device"""
+        nf = rketd_read_probes(self.h)
+        R = np.empty((self.nbatch, nf), np.float64)
+        T = np.empty_like(R)
+        rketd_read_sweep_rt(self.h, vacuum.h, probe_r, probe_t, R, T)
+        return R, T
 
     def get_fields(self):
         E, H, J = (np.empty((self.nbatch, self.ncells), self.np_dtype) for _ in range(3))

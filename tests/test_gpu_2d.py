@@ -321,7 +321,7 @@ def test_full_size_sampled_against_windowed_oracle(dtype, kernel):
     sim.close()
     refs = _oracle_windows_2d(w, half)
     peak = max(np.max(np.abs(o["rec"])) for o in refs)
-    assert peak > 0.5                                         # the source node is a probe: the driven field
+    assert peak > 2e-2                                        # the source node is a probe: the driven field (a line source in 2-D: 0.04)
     u = 2.0 ** -53 if dtype == "f64" else 2.0 ** -24
     floors = (peak, peak / 376.73, peak / 376.73, 8.854e-12 * wp_max ** 2 * 20e-12 * peak)
     worst, worst_rel, worst_f = 0.0, 0.0, [0.0] * 4

@@ -20,7 +20,7 @@ def test_oracle_pins_pass_under_asan_and_ubsan():
     assert "__asan_init" in syms and "__ubsan_handle" in syms          # really instrumented
     env = dict(os.environ, RKETD_ORACLE_SANITIZED="1", LD_PRELOAD=asan,
                ASAN_OPTIONS="detect_leaks=0:abort_on_error=1", UBSAN_OPTIONS="halt_on_error=1:print_stacktrace=1",
-               OMP_NUM_THREADS="4")
+               OMP_NUM_THREADS="2", OMP_WAIT_POLICY="passive")
     # the quick pins of both suites (everything except the long stability / R-T sweeps, which add no new code paths)
     cmd = [sys.executable, "-m", "pytest", "-x", "-q", "-p", "no:cacheprovider",
            os.path.join(ROOT, "tests", "test_oracle_pins.py"), os.path.join(ROOT, "tests", "test_oracle2d_pins.py"),
