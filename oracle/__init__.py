@@ -98,6 +98,11 @@ def _lib(omp: bool = False) -> ctypes.CDLL:
                                      ctypes.c_int, _D, ctypes.c_int64, ctypes.c_int64, ctypes.c_int64,
                                      _I64, ctypes.c_int, ctypes.c_int64, ctypes.c_int64, _D, _D, ctypes.c_int, ctypes.c_int]
         lib.oracle2d_run.restype = ctypes.c_int
+        lib.oracle2d_te_run.argtypes = [ctypes.c_int64, ctypes.c_int64, ctypes.c_double, ctypes.c_double, ctypes.c_double,
+                                        _D, _D, _D, _D, _D, _D, _D,
+                                        ctypes.c_int, _D, ctypes.c_int64, ctypes.c_int64, ctypes.c_int64, ctypes.c_int,
+                                        _I64, ctypes.c_int, ctypes.c_int64, ctypes.c_int64, _D, ctypes.c_int, ctypes.c_int]
+        lib.oracle2d_te_run.restype = ctypes.c_int
         _loaded[omp] = lib
     return _loaded[omp]
 
@@ -267,3 +272,56 @@ def run_workload2d(w, nsteps: Optional[int] = None, window=None, omp: bool = Fal
                    src_params=w.src_params, src_ij=(w.src_ij[0] - i0, w.src_ij[1] - j0) if in_src else (0, 0),
                    probes=probes, omp=omp, boundary=w.boundary if boundary is None else boundary)
     return {"rec": rec, "probe_ij": [(i + i0, j + j0) for i, j in probes], "state": st}
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# 2-D TEz (second polarisation): see the last section of rketd_oracle.cpp
+# ----------------------------------------------------------------------------------------------------------------
+EX, EY = 0, 1        # component ids of sources and probes
+
+
+class State2DTE:
+    """Ex, Ey, Hz, Jx, Jy [ny][nx] fp64 plus the global step counter; advanced in place by run2d_te()."""
+
+    def __init__(self, nx: int, ny: int, Ex0=None, Ey0=None, Hz0=None, Jx0=None, Jy0=None):
+        shp = (ny, nx)
+        mk = lambda a: np.zeros(shp) if a is None else np.array(a, np.float64).reshape(shp).copy()
+        self.Ex, self.Ey, self.Hz, self.Jx, self.Jy = mk(Ex0), mk(Ey0), mk(Hz0), mk(Jx0), mk(Jy0)
+        self.step = 0
+
+
+def run2d_te(state: State2DTE, wp, nu, dx: float, dy: float, dt: float, nsteps: int, *, src_kind: int = SRC_NONE,
+             src_params: Sequence[float] = (), src_ij=(0, 0), src_comp: int = EY, probes=(),
+             boundary: int = BOUNDARY_MUR, omp: bool = False, scheme: int = SCHEME_ETD2):
+    """Advance ``state`` by nsteps.  probes = sequence of (i, j, component).  Returns rec [nprobes][nsteps]."""
+    ny, nx = state.Ex.shape
+    wp = np.ascontiguousarray(wp, np.float64).reshape(ny, nx)
+    nu = np.ascontiguousarray(nu, np.float64).reshape(ny, nx)
+    prm = np.ascontiguousarray(src_params, np.float64)
+    prb = np.ascontiguousarray(probes, np.int64).reshape(-1, 3)
+    rec = np.zeros((prb.shape[0], nsteps))
+    rc = _lib(omp).oracle2d_te_run(nx, ny, dx, dy, dt, _p(wp), _p(nu), _p(state.Ex), _p(state.Ey), _p(state.Hz),
+                                   _p(state.Jx), _p(state.Jy), src_kind, _p(prm) if prm.size else None, prm.size,
+                                   int(src_ij[0]), int(src_ij[1]), int(src_comp),
+                                   prb.ctypes.data_as(_I64) if prb.size else None, prb.shape[0], state.step, nsteps,
+                                   _p(rec), boundary, scheme)
+    if rc:
+        raise ValueError("oracle2d_te_run: invalid argument")
+    state.step += nsteps
+    return rec
+
+
+def run_workload2d_te(w, nsteps: Optional[int] = None, window=None, omp: bool = False, boundary: Optional[int] = None):
+    """Run a ``workloads.Workload2D`` in the TEz polarisation (source on w.src_comp, probes (i, j) on w.probe_comp).
+    window = (i0, i1, j0, j1) as in run_workload2d (pin R6).  Returns dict(rec, probe_ij, state)."""
+    i0, i1, j0, j1 = (0, w.nx, 0, w.ny) if window is None else window
+    nsteps = w.nsteps if nsteps is None else nsteps
+    wp, nu = w.media(i0, i1, j0, j1)
+    E0 = w.initial_E(i0, i1, j0, j1)
+    st = State2DTE(i1 - i0, j1 - j0, Ey0=E0)
+    probes = [(int(i) - i0, int(j) - j0, int(w.probe_comp)) for i, j in w.probes if i0 <= i < i1 and j0 <= j < j1]
+    in_src = i0 <= w.src_ij[0] < i1 and j0 <= w.src_ij[1] < j1
+    rec = run2d_te(st, wp, nu, w.dx, w.dy, w.dt, nsteps, src_kind=w.src_kind if in_src else SRC_NONE,
+                   src_params=w.src_params, src_ij=(w.src_ij[0] - i0, w.src_ij[1] - j0) if in_src else (0, 0),
+                   src_comp=w.src_comp, probes=probes, omp=omp, boundary=w.boundary if boundary is None else boundary)
+    return {"rec": rec, "probe_ij": [(i + i0, j + j0) for i, j, _ in probes], "state": st}

@@ -21,7 +21,8 @@
 // eq.(6), P5 analytic slab R/T, P6 stability, P7 domain of dependence, P8 DFT,
 // P9 OpenMP == serial, and the phi-functions against 50-digit arithmetic.
 // The 2-D TMz generalisation at the end of the file has its own pins Q1-Q9
-// (tests/test_oracle2d_pins.py), listed above it.  Nothing in this file is "parity unpinned".
+// (tests/test_oracle2d_pins.py), listed above it, and the 2-D TEz polarisation after it pins R1-R7
+// (tests/test_oracle2d_te_pins.py).  Nothing in this file is "parity unpinned".
 //
 // Notation: N E-nodes k = 0..N-1; E[k] = Ex(k dz) at integer steps;
 // H[k] = Hy((k+1/2) dz) at half steps, k = 0..N-2 (H[N-1] is padding, kept 0);
@@ -417,6 +418,107 @@ int oracle2d_run(int64_t nx, int64_t ny, double dx, double dy, double dt,
       const int64_t k = AT(probes[2 * p + 1], probes[2 * p]);
       if (rec) rec[int64_t(p) * nsteps + s] = Ez[k];
       if (recJ) recJ[int64_t(p) * nsteps + s] = Jz[k];
+    }
+  }
+#undef AT
+  return 0;
+}
+
+
+// ============================================================================
+// 2-D TEz: the other polarisation of fields that do not vary along z (SURVEY §8(f) NEXT-3 "2-D TMz/TEz";
+// eqs. (1)-(3), kept in the components Ex, Ey, Hz, Jx, Jy):
+//     mu0 dHz/dt = dEx/dy - dEy/dx,   eps0 dEx/dt + Jx = dHz/dy,   eps0 dEy/dt + Jy = -dHz/dx,
+//     dJx/dt + nu Jx = eps0 wp^2 Ex,   dJy/dt + nu Jy = eps0 wp^2 Ey.
+// J now has two components, each collocated with its E component (eq. (11) PAPER.md:68 per component, eq. (12)
+// PAPER.md:74 per component with the 1-D difference of H replaced by the matching curl term) — a different stencil
+// from TMz, where J sits on the one Ez node.
+//
+// Notation.  nx x ny cells (i, j), arrays row-major [ny][nx].  Ex[j][i] = Ex((i+1/2) dx, j dy), i <= nx-2 (column nx-1
+// is padding, kept 0); Ey[j][i] = Ey(i dx, (j+1/2) dy), j <= ny-2 (row ny-1 is padding); Hz[j][i] = Hz((i+1/2) dx,
+// (j+1/2) dy), i <= nx-2, j <= ny-2, at half steps.  Reading: the media are given per cell, wp[j][i], nu[j][i], and
+// both components stored at [j][i] use that pair (the usual material-per-Yee-cell convention; the paper prints nothing
+// 2-D).  The six coefficients are those of the 1-D method, `ch` once per axis (cex with dx, cey with dy).
+// One step, in the order of the 1-D S1-S6:
+//   S1  Hz[j][i] = Hz - chx (Ey[j][i+1] - Ey[j][i]) + chy (Ex[j+1][i] - Ex[j][i])          chx = dt/(mu0 dx), chy = dt/(mu0 dy)
+//   S2  Ex'[j][i] = ca Ex - cj Jx + cey (Hz[j][i] - Hz[j-1][i])     1 <= j <= ny-2, i <= nx-2
+//       Ey'[j][i] = ca Ey - cj Jy - cex (Hz[j][i] - Hz[j][i-1])     1 <= i <= nx-2, j <= ny-2
+//   S3  tangential E on the four edges (Ex on rows 0 and ny-1, Ey on columns 0 and nx-1): boundary 0 = first-order
+//       Mur along the normal, Ex'[0][i] = Ex[1][i] + my (Ex'[1][i] - Ex[0][i]) etc.; boundary 1 = conductor, 0.
+//   S4  soft source added to component src_comp (0 = Ex, 1 = Ey) at (is, js);   S5  Jx, Jy by eq. (11);   S6  probes
+//       (i, j, component).
+// Pins (tests/test_oracle2d_te_pins.py): R1 fields uniform along one axis reproduce the 1-D oracle bit for bit (Ey, Hz
+// along x; Ex, -Hz along y), R2 discrete energy in a conducting box, R3 cavity eigenmode TE_mn against the scalar
+// recurrence of the Yee dispersion relation, R4 axis exchange, R5 first step by hand, R6 domain of dependence,
+// R7 OpenMP == serial.
+// ============================================================================
+//   probes [nprobes][3] = (i, j, component);  rec [nprobes][nsteps]
+int oracle2d_te_run(int64_t nx, int64_t ny, double dx, double dy, double dt,
+                    const double* wp, const double* nu, double* Ex, double* Ey, double* Hz, double* Jx, double* Jy,
+                    int src_kind, const double* src_params, int64_t nparams, int64_t src_i, int64_t src_j, int src_comp,
+                    const int64_t* probes, int nprobes, int64_t step0, int64_t nsteps, double* rec, int boundary, int scheme) {
+  if (nx < 3 || ny < 3 || nsteps < 0 || dx <= 0 || dy <= 0 || dt <= 0 || scheme < 0 || scheme > 1) return 1;
+  if (boundary < 0 || boundary > 1 || src_comp < 0 || src_comp > 1) return 1;
+  if (src_kind >= 0 && (src_i < 0 || src_i >= nx || src_j < 0 || src_j >= ny)) return 1;
+  for (int p = 0; p < nprobes; ++p)
+    if (probes[3 * p] < 0 || probes[3 * p] >= nx || probes[3 * p + 1] < 0 || probes[3 * p + 1] >= ny ||
+        probes[3 * p + 2] < 0 || probes[3 * p + 2] > 1) return 1;
+  const int64_t n = nx * ny;
+  std::vector<double> ca(n), cj(n), cex(n), cey(n), ka(n), kb(n), kc(n), Exold(n), Eyold(n);
+  double g[4];
+  oracle2d_coefficients(n, wp, nu, dx, dy, dt, scheme, ca.data(), cj.data(), cex.data(), cey.data(), ka.data(),
+                        kb.data(), kc.data(), g);
+  const double chx = g[0], chy = g[1], mx = g[2], my = g[3];
+#define AT(j, i) ((j) * nx + (i))
+  for (int64_t s = 0; s < nsteps; ++s) {
+    const int64_t ng = step0 + s;
+    // S1: Hz from the z component of the curl of E (eq. (2); discretised as eq. (14) PAPER.md:84 along each axis)
+#pragma omp parallel for schedule(static)
+    for (int64_t j = 0; j <= ny - 2; ++j)
+      for (int64_t i = 0; i <= nx - 2; ++i)
+        Hz[AT(j, i)] = Hz[AT(j, i)] - chx * (Ey[AT(j, i + 1)] - Ey[AT(j, i)]) + chy * (Ex[AT(j + 1, i)] - Ex[AT(j, i)]);
+    // S2: Ex, Ey from the curl of Hz and J (eq. (12) PAPER.md:74 with (11) substituted, per component)
+#pragma omp parallel for schedule(static)
+    for (int64_t k = 0; k < n; ++k) { Exold[k] = Ex[k]; Eyold[k] = Ey[k]; }
+#pragma omp parallel for schedule(static)
+    for (int64_t j = 0; j <= ny - 1; ++j)
+      for (int64_t i = 0; i <= nx - 1; ++i) {
+        const int64_t k = AT(j, i);
+        if (j >= 1 && j <= ny - 2 && i <= nx - 2) Ex[k] = ca[k] * Exold[k] - cj[k] * Jx[k] + cey[k] * (Hz[k] - Hz[AT(j - 1, i)]);
+        if (i >= 1 && i <= nx - 2 && j <= ny - 2) Ey[k] = ca[k] * Eyold[k] - cj[k] * Jy[k] - cex[k] * (Hz[k] - Hz[AT(j, i - 1)]);
+      }
+    // S3: tangential E on the edges
+    for (int64_t i = 0; i <= nx - 2; ++i) {
+      if (boundary == 0) {
+        Ex[AT(0, i)] = Exold[AT(1, i)] + my * (Ex[AT(1, i)] - Exold[AT(0, i)]);
+        Ex[AT(ny - 1, i)] = Exold[AT(ny - 2, i)] + my * (Ex[AT(ny - 2, i)] - Exold[AT(ny - 1, i)]);
+      } else {
+        Ex[AT(0, i)] = 0.0; Ex[AT(ny - 1, i)] = 0.0;
+      }
+    }
+    for (int64_t j = 0; j <= ny - 2; ++j) {
+      if (boundary == 0) {
+        Ey[AT(j, 0)] = Eyold[AT(j, 1)] + mx * (Ey[AT(j, 1)] - Eyold[AT(j, 0)]);
+        Ey[AT(j, nx - 1)] = Eyold[AT(j, nx - 2)] + mx * (Ey[AT(j, nx - 2)] - Eyold[AT(j, nx - 1)]);
+      } else {
+        Ey[AT(j, 0)] = 0.0; Ey[AT(j, nx - 1)] = 0.0;
+      }
+    }
+    // S4: soft source, eq. (15), on one component
+    if (src_kind >= 0) {
+      const double sv = source_sample(src_kind, src_params, nparams, ng, dt);
+      if (src_comp == 0) Ex[AT(src_j, src_i)] += sv; else Ey[AT(src_j, src_i)] += sv;
+    }
+    // S5: Jx, Jy, eq. (11), every stored node, with the final E'
+#pragma omp parallel for schedule(static)
+    for (int64_t k = 0; k < n; ++k) {
+      Jx[k] = ka[k] * Jx[k] + kb[k] * Exold[k] + kc[k] * Ex[k];
+      Jy[k] = ka[k] * Jy[k] + kb[k] * Eyold[k] + kc[k] * Ey[k];
+    }
+    // S6: probes
+    for (int p = 0; p < nprobes; ++p) {
+      const int64_t k = AT(probes[3 * p + 1], probes[3 * p]);
+      if (rec) rec[int64_t(p) * nsteps + s] = probes[3 * p + 2] == 0 ? Ex[k] : Ey[k];
     }
   }
 #undef AT

@@ -264,7 +264,15 @@ int build_k2_plan(rketd_sim *s, int depth, int variant) {
 // RESIDENT plans.  rketd_set_plan's variant: -1 = the warp-tile kernel k3_wtile with the packing chosen by k3w_plan;
 // RKETD_RESIDENT_WTILE(nw, nc, k) = the same with an explicit packing; 0, 2 = the older one-barrier-per-step kernel
 // k3_resident (kept as a structurally different cross-check).
-bool wtile_variant(int variant) { return variant < 0 || (variant & RKETD_RESIDENT_WTILE_FLAG) != 0; }
+// variant -1: warp tiles when the batch is a few grids (a run is then a chain of dependent steps: config 1 runs 1.9 x
+// faster than with a barrier per step) or when a grid is too large for one CTA; the one-barrier-per-step kernel when
+// many grids that each fit one CTA keep every SM busy — there four small CTAs per SM hide each other's barriers and it
+// is still the faster of the two (config 3 1020 against 785 Gcell/s, config 5 863 against 701).
+int legacy_k3_variant(const rketd_sim *s) { return (s->L.nrows > 32 && s->L.nrows <= 256) ? 2 : 0; }
+bool wtile_variant(const rketd_sim *s, int variant) {
+  if (variant >= 0) return (variant & RKETD_RESIDENT_WTILE_FLAG) != 0;
+  return k3w_few_grids(s->L, s->sms) || !k3_threads_for_rows(s->dtype, s->L.nrows, 0);
+}
 bool resident_wtile_plan(rketd_sim *s, int depth, int variant, K3WPlan *P) {
   int64_t nw = 0, nc = 0, k = 0;
   if (variant >= 0) { nw = variant & 0xff; nc = (variant >> 8) & 0xff; k = (variant >> 16) & 0xfff; }
@@ -278,8 +286,13 @@ bool resident_wtile_plan(rketd_sim *s, int depth, int variant, K3WPlan *P) {
 
 int resolve_kernel(rketd_sim *s) {
   if (s->plan_kernel != RKETD_KERNEL_AUTO) return s->plan_kernel;
+  if (!wtile_variant(s, -1)) return RKETD_KERNEL_RESIDENT;          // many grids, each fits one CTA
   K3WPlan P;
-  return resident_wtile_plan(s, 0, -1, &P) ? RKETD_KERNEL_RESIDENT : RKETD_KERNEL_TBLOCK;
+  if (!resident_wtile_plan(s, 0, -1, &P)) return RKETD_KERNEL_TBLOCK;
+  // one long line spread over most of a 16-CTA cluster: K2's deep passes (T = 64) win again from about 100 warp
+  // tiles on (paper Table 2: 40 960 cells 0.44 ms against 0.54; 20 480 cells 0.47 against 0.41)
+  if (k3w_few_grids(s->L, s->sms) && P.nc * P.nw > 96) return RKETD_KERNEL_TBLOCK;
+  return RKETD_KERNEL_RESIDENT;
 }
 
 // run nsteps steps whose probe samples go to rec ([nbatch][nprobes][nsteps] or nullptr)
@@ -341,7 +354,7 @@ int run_segment(rketd_sim *s, int64_t nsteps, void *rec) {
     s->ctr_tile_cells = L.C; s->ctr_halo_cells = 1; s->ctr_depth_used = 1;
   } else if (kern == RKETD_KERNEL_RESIDENT) {
     FieldPtrs f{s->fld[s->cur][0], s->fld[s->cur][1], s->fld[s->cur][2]};
-    if (wtile_variant(s->plan_variant)) {
+    if (wtile_variant(s, s->plan_variant)) {
       K3WPlan P;
       if (!resident_wtile_plan(s, s->plan_kernel == RKETD_KERNEL_RESIDENT ? s->plan_depth : 0, s->plan_variant, &P))
         return fail(s, RKETD_EINVAL, "grid too large for the resident kernel (or the requested packing cannot run)");
@@ -351,7 +364,7 @@ int run_segment(rketd_sim *s, int64_t nsteps, void *rec) {
       s->ctr_halo_cells = (s->ctr_tile_cells - P.k * L.gstride) / 2;
       s->ctr_depth_used = P.T;
     } else {
-      int variant = s->plan_variant;
+      int variant = s->plan_variant >= 0 ? s->plan_variant : legacy_k3_variant(s);
       if (!k3_threads_for_rows(s->dtype, L.nrows, variant)) variant = 0;
       const int NT = k3_threads_for_rows(s->dtype, L.nrows, variant);
       if (!NT) return fail(s, RKETD_EINVAL, "grid too large for the one-CTA resident kernel");
@@ -618,7 +631,8 @@ int rketd_set_plan(rketd_sim *s, int kernel, int depth, int variant) {
   if (kernel < RKETD_KERNEL_AUTO || kernel > RKETD_KERNEL_RESIDENT || depth < 0) return fail(s, RKETD_EINVAL, "rketd_set_plan: bad argument");
   if (kernel == RKETD_KERNEL_RESIDENT) {
     K3WPlan P;
-    if (wtile_variant(variant) ? !resident_wtile_plan(s, depth, variant, &P) : !k3_threads_for_rows(s->dtype, s->L.nrows, variant))
+    if (wtile_variant(s, variant) ? !resident_wtile_plan(s, depth, variant, &P)
+                                  : !k3_threads_for_rows(s->dtype, s->L.nrows, variant < 0 ? legacy_k3_variant(s) : variant))
       return fail(s, RKETD_EINVAL, "rketd_set_plan: grid does not fit the resident kernel (or bad depth / packing)");
   }
   if (kernel == RKETD_KERNEL_TBLOCK || kernel == RKETD_KERNEL_AUTO) {

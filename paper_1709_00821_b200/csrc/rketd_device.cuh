@@ -143,6 +143,13 @@ __device__ __forceinline__ void stg256(float *p, const float (&o)[8]) {
   asm volatile("st.global.v8.f32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};"
                ::"l"(p), "f"(o[0]), "f"(o[1]), "f"(o[2]), "f"(o[3]), "f"(o[4]), "f"(o[5]), "f"(o[6]), "f"(o[7]) : "memory");
 }
+// store v to p when pred holds, as one predicated instruction (no branch, no reconvergence point)
+__device__ __forceinline__ void stg_if(bool pred, double *p, double v) {
+  asm volatile("{\n.reg .pred q;\nsetp.ne.u32 q, %0, 0;\n@q st.global.f64 [%1], %2;\n}" ::"r"((uint32_t)pred), "l"(p), "d"(v) : "memory");
+}
+__device__ __forceinline__ void stg_if(bool pred, float *p, float v) {
+  asm volatile("{\n.reg .pred q;\nsetp.ne.u32 q, %0, 0;\n@q st.global.f32 [%1], %2;\n}" ::"r"((uint32_t)pred), "l"(p), "f"(v) : "memory");
+}
 // a thread's C nodes (32 or 64 B, 32-B aligned) <-> global memory
 template <typename R, int C>
 __device__ __forceinline__ void load_nodes_global(const R *base, int64_t first, R (&out)[C]) {
@@ -239,6 +246,17 @@ struct SourceStream {
     if (on) {
       cur = fetch(p, base + lane);
       nxt = fetch(p, base + 32 + lane);
+    }
+  }
+  // samples of steps nloc and nloc + 1 with one check per pair (the stream is on)
+  __device__ __forceinline__ void sample2(const StepParams<R> &p, int64_t nloc, int lane, R &s0, R &s1) {
+    const int j = (int)(nloc - base);
+    if (j >= 31) {            // the pair touches the next 32 samples: once in 16 pairs
+      s0 = sample(p, nloc, lane);
+      s1 = sample(p, nloc + 1, lane);
+    } else {
+      s0 = __shfl_sync(0xffffffffu, cur, j);
+      s1 = __shfl_sync(0xffffffffu, cur, j + 1);
     }
   }
   __device__ __forceinline__ R sample(const StepParams<R> &p, int64_t nloc, int lane) {

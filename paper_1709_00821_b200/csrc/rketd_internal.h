@@ -74,6 +74,7 @@ struct K3WPlan {
 };
 // false when the grid cannot stay resident (a grid needs more than 16 CTAs x 12 warp tiles) or the wish cannot be met;
 // want_* = 0: chosen here
+bool k3w_few_grids(const Layout &L, int sms);
 bool k3w_plan(const Layout &L, int depth, int sms, int64_t want_nw, int64_t want_nc, int64_t want_k, K3WPlan *out);
 cudaError_t launch_k3w(int dtype, const Layout &L, const K3WPlan &P, FieldPtrs fld, void *const coef[4], const StepCommon &sc,
                        int64_t nsteps, cudaStream_t st);

@@ -54,7 +54,7 @@ constexpr int kMaxHR = 2;
 __host__ __device__ constexpr uint32_t slot_bytes_per_warp() { return 2u * kMaxHR * 3u * kRowBytes; }
 
 template <typename R, bool CLUSTER, bool PML>
-__global__ void __launch_bounds__(384, 1) k3_wtile(RowPtrs<R> f, CoefPtrs<R> cp, const __grid_constant__ StepParams<R> p,
+__global__ void __launch_bounds__(256, 1) k3_wtile(RowPtrs<R> f, CoefPtrs<R> cp, const __grid_constant__ StepParams<R> p,
                                                     const K3WArgs q) {
   constexpr int C = kRowBytes / sizeof(R);
   typedef Geom<R, C> G;
@@ -123,10 +123,7 @@ __global__ void __launch_bounds__(384, 1) k3_wtile(RowPtrs<R> f, CoefPtrs<R> cp,
   uint32_t par = 0u;
   for (int64_t n = 0; n < q.nsteps; n += q.T) {
     const int Tr = (int)(q.nsteps - n < q.T ? q.nsteps - n : q.T);
-    if (active) {
-      if (special) warp_round<true, PML, R, C>(E, H, J, cf, p, sx, ws, src, p.n0 + n, Tr);
-      else warp_round<false, false, R, C>(E, H, J, cf, p, sx, ws, src, p.n0 + n, Tr);
-    }
+    if (active) warp_round<PML, R, C>(E, H, J, cf, p, sx, ws, src, p.n0 + n, Tr);
     if (n + Tr >= q.nsteps) break;
     // halo refresh: double-buffered by round parity, so one barrier per round is enough (a warp can overwrite buffer
     // `par` again only after the NEXT barrier, which every reader of this round's data has passed its reads to reach)
@@ -170,23 +167,34 @@ __global__ void __launch_bounds__(384, 1) k3_wtile(RowPtrs<R> f, CoefPtrs<R> cp,
 // (tile i = rows i RO - HR .. i RO - HR + 31), so the count is ceil(rows / RO).
 static int tiles_for(int64_t rows, int RO) { return (int)((rows + RO - 1) / RO); }
 
+// fewer warp tiles in the whole batch than four per SM: latency, not throughput, decides
+bool k3w_few_grids(const Layout &L, int sms) { return L.nbatch * ((L.nrows + 29) / 30) < (int64_t)sms * 4; }
+
 bool k3w_plan(const Layout &L, int depth, int sms, int64_t want_nw, int64_t want_nc, int64_t want_k, K3WPlan *out) {
   K3WPlan P;
-  P.T = depth > 0 ? depth : L.C;                       // default: one halo row, 8 (fp64) / 16 (fp32) steps per round
+  // default depth: one halo row (8 steps per round in fp64, 16 in fp32) when many grids keep the SMs busy; two halo
+  // rows when a few grids are a chain of dependent rounds, where halving the number of barriers pays for the wider
+  // halo (config 1: 1.55 against 1.76 ms)
+  const bool few = k3w_few_grids(L, sms);
+  P.T = depth > 0 ? depth : (few ? 2 * L.C : L.C);
   P.HR = (P.T + L.C - 1) / L.C;
   if (P.HR > kMaxHR) return false;
   P.rows_out = 32 - 2 * P.HR;
-  const int maxw = 12, maxc = 16;                      // 384 threads x 168 registers fill an SM; 16 = largest (non-portable) cluster
+  // 8 warps per CTA: the feature variants of the time loop need up to 242 registers, and a scheduler's 16 K registers
+  // then hold two warps (12 warps would need <= 168 and spill); 4 warps per SM already saturate the FP64 pipe with this
+  // instruction mix (profiles/r02_peaks.md).  16 = largest (non-portable) cluster.
+  const int maxw = 8, maxc = 16;
   if (L.nrows > (int64_t)maxw * maxc * P.rows_out) return false;
   const int w1 = tiles_for(L.nrows, P.rows_out);       // tiles of one grid
   int k = 1, nc = 1, nw = w1;
   if (want_nw > 0 || want_nc > 0 || want_k > 0) {      // explicit (rketd_set_plan)
     k = (int)std::max<int64_t>(1, want_k);
     const int w = tiles_for(k * L.nrows, P.rows_out);
-    nc = (int)std::max<int64_t>(1, want_nc);
-    nw = want_nw > 0 ? (int)want_nw : (w + nc - 1) / nc;
+    nw = (int)want_nw;
+    nc = want_nc > 0 ? (int)want_nc : (nw > 0 ? (w + nw - 1) / nw : (w + maxw - 1) / maxw);
+    if (nw <= 0) nw = (w + nc - 1) / nc;
     if (nw > maxw || nc > maxc || (int64_t)nw * nc < w || k > L.nbatch) return false;
-  } else if (L.nbatch * (int64_t)w1 < (int64_t)sms * 4) {
+  } else if (few) {
     // few grids: the run is a chain of dependent steps.  One warp per scheduler at most, the rest of the
     // grid on other SMs of a cluster: a step then costs one warp's latency, not a queue of warps
     nw = std::min(w1, 4);
@@ -212,6 +220,7 @@ bool k3w_plan(const Layout &L, int depth, int sms, int64_t want_nw, int64_t want
       nw = (w1 + nc - 1) / nc;
     }
   }
+  if (nw > maxw || nc > maxc || nw < 1 || nc < 1) return false;
   P.k = k; P.nc = nc; P.nw = nw;
   P.chunk_rows = k * L.nrows;
   if (P.chunk_rows > 0x7fffff00LL) return false;

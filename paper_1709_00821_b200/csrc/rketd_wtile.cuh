@@ -11,56 +11,40 @@ namespace rketd {
 template <typename R> struct RowPtrs { R *E, *H, *J; };
 template <typename R> struct CoefPtrs { const R *c[kNumCoef]; };
 
-// ---- Mur, source and probes of a warp tile without divergence.
-// Every grid has the same layout, so the LOCAL index (0..C-1, inside its 64-B row) of node 0, node ncells-1 and the
-// source node is a launch-wide constant that comes straight from kernel parameters: a switch on it is a uniform branch
-// (no reconvergence stack), and which LANE holds the node is a predicate that turns the update into a select.  Probe
-// nodes differ from lane to lane; their value is picked by a select tree and written by one predicated store.
-// step_special (rketd_device.cuh) does the same with per-lane else-if chains: in a warp whose lanes take different
-// chains every step costs ~1000 cycles of branch latency (profiles/r02_ncu_k3_wtile.md), which is what one warp tile
-// in three pays in the batched configs, and every warp of the chunk waits for it at the next halo refresh.
+// ---- Mur, source and probes of a warp tile without a branch in the time loop.
+// step_special (rketd_device.cuh) dispatches per lane with else-if chains.  In a warp tile whose lanes take different
+// chains that costs 700-1000 cycles of branch latency per step (measured, profiles/r02_ncu_k3_wtile.md), which is what
+// one warp tile in three pays in the batched configs while every other warp of the chunk waits for it at the next halo
+// refresh.  Here the features a warp tile has (SF_* bits, warp-uniform) are a TEMPLATE parameter, chosen once per
+// round, and inside the step every feature is straight-line code: the candidate value is computed for each local
+// index it could apply to and a per-lane bit mask turns it into a select.  Same arithmetic, same order (Mur left, Mur
+// right, source, probes) and the same bits as step_special.  H behind the last node and left of node 0 is zeroed once
+// at the end (zero_padding_H) instead of every step: those values feed only nodes that Mur rewrites or whose
+// coefficients are zero.
+enum : int { SF_MURL = 1, SF_MURR = 2, SF_SRC = 4, SF_PROBE = 8, SF_SLOW = 16 };
+
 struct WarpSpecial {
-  bool w_murL = false, w_murR = false, w_src = false, w_probe = false, w_probe2 = false, w_slow = false;   // some lane of the warp ...
-  bool l_murL = false, l_murR = false, l_src = false, l_p0 = false, l_p1 = false;                           // this lane ...
-  int iL = 0, iR = 1, iS = 0;         // launch-wide local indices
+  int mask = 0;                       // SF_* of the warp tile (warp-uniform)
+  bool mL0 = false, mL1 = false;      // this lane holds node 0 at local index 0 / 1
+  uint32_t mR = 0, mS = 0;            // bit i: this lane's local node i is node ncells-1 / the source node
+  uint32_t mHz = 0;                   // bit i: H of local node i is padding (behind node ncells-1, or left of node 0)
+  bool l_p0 = false, l_p1 = false;    // this lane records one / two probes
 };
 
 template <typename R, int C, bool PML>
 __device__ __forceinline__ WarpSpecial make_warp_special(const StepParams<R> &p, const SpecialIdx &sx) {
   WarpSpecial ws;
   constexpr unsigned full = 0xffffffffu;
-  ws.iL = (int)(p.cellL % C); ws.iR = (int)(p.cellR % C); ws.iS = p.cellS >= 0 ? (int)(p.cellS % C) : 0;
-  ws.l_murL = sx.iL >= 0; ws.l_murR = sx.iR >= 0; ws.l_src = sx.iS >= 0;
+  ws.mL0 = sx.iL == 0; ws.mL1 = sx.iL == 1;
+  ws.mR = sx.iR >= 0 ? 1u << sx.iR : 0u;
+  ws.mS = sx.iS >= 0 ? 1u << sx.iS : 0u;
+  ws.mHz = (sx.iR >= 0 ? (0xffffffffu << sx.iR) & ((1u << C) - 1u) : 0u) | (sx.iL == 1 ? 1u : 0u);
   ws.l_p0 = sx.np >= 1 && sx.np <= 2; ws.l_p1 = sx.np == 2;
-  ws.w_murL = __any_sync(full, ws.l_murL); ws.w_murR = __any_sync(full, ws.l_murR); ws.w_src = __any_sync(full, ws.l_src);
-  ws.w_probe = __any_sync(full, ws.l_p0); ws.w_probe2 = __any_sync(full, ws.l_p1);
-  // more than two probes among one lane's nodes, or an absorbing layer: the general per-lane path
-  ws.w_slow = PML || __any_sync(full, sx.np == 3);
+  ws.mask = (__any_sync(full, sx.iL >= 0) ? SF_MURL : 0) | (__any_sync(full, sx.iR >= 0) ? SF_MURR : 0) |
+            (__any_sync(full, sx.iS >= 0) ? SF_SRC : 0) | (__any_sync(full, ws.l_p0) ? SF_PROBE : 0);
+  // an absorbing layer, or more than two probes among one lane's nodes: the general per-lane path
+  if (PML || __any_sync(full, sx.np == 3) || __any_sync(full, sx.pml_mask != 0u)) ws.mask = SF_SLOW;
   return ws;
-}
-
-// f(integral_constant<int, i>) for i == idx, idx warp-uniform: a switch (jump table or uniform branches)
-template <int C, typename F>
-__device__ __forceinline__ void uniform_switch(int idx, F &&f) {
-  switch (idx) {
-    case 0: f(std::integral_constant<int, 0>{}); break;
-    case 1: f(std::integral_constant<int, 1>{}); break;
-    case 2: f(std::integral_constant<int, 2 % C>{}); break;
-    case 3: f(std::integral_constant<int, 3 % C>{}); break;
-    case 4: f(std::integral_constant<int, 4 % C>{}); break;
-    case 5: f(std::integral_constant<int, 5 % C>{}); break;
-    case 6: f(std::integral_constant<int, 6 % C>{}); break;
-    case 7: f(std::integral_constant<int, 7 % C>{}); break;
-    case 8: f(std::integral_constant<int, 8 % C>{}); break;
-    case 9: f(std::integral_constant<int, 9 % C>{}); break;
-    case 10: f(std::integral_constant<int, 10 % C>{}); break;
-    case 11: f(std::integral_constant<int, 11 % C>{}); break;
-    case 12: f(std::integral_constant<int, 12 % C>{}); break;
-    case 13: f(std::integral_constant<int, 13 % C>{}); break;
-    case 14: f(std::integral_constant<int, 14 % C>{}); break;
-    case 15: f(std::integral_constant<int, 15 % C>{}); break;
-    default: break;
-  }
 }
 
 // value of v[idx], idx per lane: a select tree (no branch, no local memory)
@@ -76,47 +60,44 @@ __device__ __forceinline__ R select_node(const R (&v)[C], int idx) {
   return t[0];
 }
 
-// a3, a4, a6 for the lanes of a warp tile (same order and the same arithmetic as step_special; Mur ends only)
-template <typename R, int C>
-__device__ __forceinline__ void special_uniform(const R (&E)[C], R (&En)[C], R (&H)[C], const StepParams<R> &p,
-                                                const SpecialIdx &sx, const WarpSpecial &ws, int64_t nloc, R src_now) {
+// a3, a4, a6 for the lanes of a warp tile with the features MASK (first-order Mur ends only)
+template <int MASK, typename R, int C>
+__device__ __forceinline__ void special_select(const R (&E)[C], R (&En)[C], const StepParams<R> &p, const SpecialIdx &sx,
+                                               const WarpSpecial &ws, int64_t nloc, R src_now) {
   typedef Arith<R> A;
-  if (ws.w_murL) {      // node 0 sits at local index 0 or 1 (Layout: off), node 1 in the same row
-    if (ws.iL == 0) {
-      const R cand = A::fma(p.mur_m, A::sub(En[1], E[0]), E[1]);
-      En[0] = ws.l_murL ? cand : En[0];
-    } else {
-      const R cand = A::fma(p.mur_m, A::sub(En[2], E[1]), E[2]);
-      En[1] = ws.l_murL ? cand : En[1];
-      H[0] = ws.l_murL ? R(0) : H[0];                                   // padding left of node 0
-    }
+  if constexpr ((MASK & SF_MURL) != 0) {      // node 0 sits at local index 0 or 1 (Layout: off), node 1 in the same row
+    const R c0 = A::fma(p.mur_m, A::sub(En[1], E[0]), E[1]);
+    const R c1 = A::fma(p.mur_m, A::sub(En[2], E[1]), E[2]);
+    En[0] = ws.mL0 ? c0 : En[0];
+    En[1] = ws.mL1 ? c1 : En[1];
   }
-  if (ws.w_murR) {      // node ncells-1 at local index iR >= 1, node ncells-2 in the same row
-    uniform_switch<C>(ws.iR, [&](auto ic) {
-      constexpr int i = decltype(ic)::value;
-      if constexpr (i >= 1) {
-        const R cand = A::fma(p.mur_m, A::sub(En[i - 1], E[i]), E[i - 1]);
-        En[i] = ws.l_murR ? cand : En[i];
+  if constexpr ((MASK & SF_MURR) != 0) {      // node ncells-1 at local index >= 1, node ncells-2 in the same row
+    // (descending, so that every candidate sees the interior value of its inward neighbour; one bit of mR is set at most)
 #pragma unroll
-        for (int j = i; j < C; ++j) H[j] = ws.l_murR ? R(0) : H[j];     // H[ncells-1] and padding
-      }
-    });
-  }
-  if (ws.w_src) {
-    uniform_switch<C>(ws.iS, [&](auto ic) {
-      constexpr int i = decltype(ic)::value;
-      const R sum = A::add(En[i], src_now);
-      En[i] = ws.l_src ? sum : En[i];
-    });
-  }
-  if (ws.w_probe) {
-    const R v = select_node<R, C>(En, sx.pi0);
-    if (ws.l_p0) p.rec[sx.pr0 + nloc] = v;
-    if (ws.w_probe2) {
-      const R v1 = select_node<R, C>(En, sx.pi1);
-      if (ws.l_p1) p.rec[sx.pr1 + nloc] = v1;
+    for (int i = C - 1; i >= 1; --i) {
+      const R cand = A::fma(p.mur_m, A::sub(En[i - 1], E[i]), E[i - 1]);
+      En[i] = ((ws.mR >> i) & 1u) ? cand : En[i];
     }
   }
+  if constexpr ((MASK & SF_SRC) != 0) {
+#pragma unroll
+    for (int i = 0; i < C; ++i) {
+      const R sum = A::add(En[i], src_now);
+      En[i] = ((ws.mS >> i) & 1u) ? sum : En[i];
+    }
+  }
+  if constexpr ((MASK & SF_PROBE) != 0) {      // up to two probes among a lane's nodes; predicated stores, no branch
+    const R v0 = select_node<R, C>(En, sx.pi0), v1 = select_node<R, C>(En, sx.pi1);
+    stg_if(ws.l_p0, p.rec + (sx.pr0 + nloc), v0);
+    stg_if(ws.l_p1, p.rec + (sx.pr1 + nloc), v1);
+  }
+}
+
+// H of padding nodes (behind node ncells-1, left of node 0): reported as zero; called once after the time loop
+template <typename R, int C>
+__device__ __forceinline__ void zero_padding_H(R (&H)[C], const WarpSpecial &ws) {
+#pragma unroll
+  for (int i = 0; i < C; ++i) H[i] = ((ws.mHz >> i) & 1u) ? R(0) : H[i];
 }
 
 // One leapfrog step of a warp tile.  Only NEW values travel: H'[C-1] goes up one lane as soon as it
@@ -124,16 +105,17 @@ __device__ __forceinline__ void special_uniform(const R (&E)[C], R (&En)[C], R (
 // next step's H'[C-1] needs).  Two 64-bit shuffles per step and no redundant arithmetic.  Lanes 0 and 31
 // receive their own values at the tile edge, which is fine: those nodes are in the halo that is thrown
 // away (garbage moves inwards one node per step; the halo is >= T nodes wide).
-// SLOW: the special lanes take step_special's per-lane chains (absorbing layer, or more than two probes in one lane)
-template <bool SPECIAL, bool PML, bool SLOW, typename R, int C>
+// MASK: SF_* features of the tile (0: none; SF_SLOW: step_special's per-lane chains — absorbing layer, or more than
+// two probes in one lane).
+template <int MASK, bool PML, typename R, int C>
 __device__ __forceinline__ void warp_step(const R (&E)[C], R (&En)[C], R (&H)[C], R (&G)[C], const CoefRegs<R, C> &cf,
                                           R &Er, R nchh, const StepParams<R> &p, const SpecialIdx &sx, const WarpSpecial &ws,
                                           int64_t nloc, R src_now) {
   typedef Arith<R> A;
-  // Issue cost of an FP64 instruction on sm_100 = max(2, distinct 64-bit register operands) cycles per
-  // scheduler (measured): the two FMAs that multiply E[i] sit next to each other so that the
+  // Issue cost of an FP64 instruction on sm_100 = max(2, distinct 64-bit register operands) cycles per scheduler
+  // (measured: profiles/r02_peaks.md): the two FMAs that multiply E[i] sit next to each other so that the
   // second one finds E[i] in the operand-reuse cache, and nchh comes from the constant bank.
-  if constexpr (SPECIAL && PML) {
+  if constexpr (MASK == SF_SLOW && PML) {
     if (sx.pml_mask) pml_pre<R, C>(E, Er, H, p, sx);                           // absorbing-layer H nodes, on old E
   }
   H[C - 1] = A::fma(nchh, A::sub(Er, E[C - 1]), H[C - 1]);                    // a1, last node first
@@ -147,64 +129,80 @@ __device__ __forceinline__ void warp_step(const R (&E)[C], R (&En)[C], R (&H)[C]
     G[i] = A::fma(cf.c[COEF_KA][i], G[i], w);                                 // a5 (old E, old G)
     En[i] = A::fma(-cf.c[COEF_CH][i], A::sub(H[i], i ? H[i - 1] : Hl), t);    // a2
   }
-  if constexpr (SPECIAL) {                                                     // a3, a4, a6
-    if constexpr (PML || SLOW) { if (sx.any) step_special<R, C, PML>(E, En, H, p, sx, nloc, src_now); }
-    else special_uniform<R, C>(E, En, H, p, sx, ws, nloc, src_now);
+  if constexpr (MASK == SF_SLOW) {                                             // a3, a4, a6
+    if (sx.any) step_special<R, C, PML>(E, En, H, p, sx, nloc, src_now);
+  } else if constexpr (MASK != 0) {
+    special_select<MASK, R, C>(E, En, p, sx, ws, nloc, src_now);
   }
   Er = __shfl_down_sync(0xffffffffu, En[0], 1);
 }
 
-template <bool SPECIAL, bool PML, bool SLOW, typename R, int C>
+template <int MASK, bool PML, typename R, int C>
 __device__ __forceinline__ void warp_steps(R (&E)[C], R (&H)[C], R (&G)[C], const CoefRegs<R, C> &cf, const StepParams<R> &p,
                                            const SpecialIdx &sx, const WarpSpecial &ws, SourceStream<R> &src, int64_t nloc,
                                            int nsteps) {
+  constexpr bool SRC = MASK == SF_SLOW || (MASK & SF_SRC) != 0;
   const R nchh = p.nchh;       // stays a constant-bank operand of the FMAs (one register read less each)
   const int lane = threadIdx.x & 31;
   R Er = __shfl_down_sync(0xffffffffu, E[0], 1);
   R Eb[C];
   int left = nsteps;
   for (; left >= 2; left -= 2) {
-    const R s0 = SPECIAL ? src.sample(p, nloc, lane) : R(0);
-    warp_step<SPECIAL, PML, SLOW, R, C>(E, Eb, H, G, cf, Er, nchh, p, sx, ws, nloc, s0);
-    const R s1 = SPECIAL ? src.sample(p, nloc + 1, lane) : R(0);
-    warp_step<SPECIAL, PML, SLOW, R, C>(Eb, E, H, G, cf, Er, nchh, p, sx, ws, nloc + 1, s1);
+    R s0 = R(0), s1 = R(0);
+    if constexpr (MASK == SF_SLOW) { s0 = src.sample(p, nloc, lane); s1 = src.sample(p, nloc + 1, lane); }
+    else if constexpr (SRC) src.sample2(p, nloc, lane, s0, s1);
+    warp_step<MASK, PML, R, C>(E, Eb, H, G, cf, Er, nchh, p, sx, ws, nloc, s0);
+    warp_step<MASK, PML, R, C>(Eb, E, H, G, cf, Er, nchh, p, sx, ws, nloc + 1, s1);
     nloc += 2;
   }
   if (left) {
-    const R s0 = SPECIAL ? src.sample(p, nloc, lane) : R(0);
-    warp_step<SPECIAL, PML, SLOW, R, C>(E, Eb, H, G, cf, Er, nchh, p, sx, ws, nloc, s0);
+    const R s0 = SRC ? src.sample(p, nloc, lane) : R(0);
+    warp_step<MASK, PML, R, C>(E, Eb, H, G, cf, Er, nchh, p, sx, ws, nloc, s0);
 #pragma unroll
     for (int i = 0; i < C; ++i) E[i] = Eb[i];
   }
+  if constexpr (MASK != 0 && MASK != SF_SLOW) zero_padding_H<R, C>(H, ws);
 }
 
-// T steps of one staged tile of K2 (k2_wtile): special indices and the source stream are set up per tile
+// T steps of one staged tile of K2 (k2_wtile): special indices and the source stream are set up per tile.  K2 meets a
+// special tile once in thousands, so it carries one select instantiation with all four features instead of sixteen.
 template <bool SPECIAL, bool PML, typename R, int C>
 __device__ __forceinline__ void warp_time_loop(R (&E)[C], R (&H)[C], R (&G)[C], const CoefRegs<R, C> &cf,
                                                const StepParams<R> &p, uint32_t flag, int64_t k0, int64_t g, bool owner,
                                                int nsteps) {
-  const int lane = threadIdx.x & 31;
-  SourceStream<R> src;
-  src.start(p, SPECIAL && __any_sync(0xffffffffu, (flag & F_SRC) != 0u), p.n0, lane);
-  const SpecialIdx sx = SPECIAL ? make_special<R, C, PML>(p, flag, k0, g, owner) : SpecialIdx();
-  const WarpSpecial ws = SPECIAL ? make_warp_special<R, C, PML>(p, sx) : WarpSpecial();
-  if constexpr (SPECIAL && !PML) {
-    if (ws.w_slow) { warp_steps<true, false, true, R, C>(E, H, G, cf, p, sx, ws, src, p.n0, nsteps); return; }
+  if constexpr (!SPECIAL) {
+    SourceStream<R> src;
+    warp_steps<0, false, R, C>(E, H, G, cf, p, SpecialIdx(), WarpSpecial(), src, p.n0, nsteps);
+  } else {
+    const int lane = threadIdx.x & 31;
+    SourceStream<R> src;
+    src.start(p, __any_sync(0xffffffffu, (flag & F_SRC) != 0u), p.n0, lane);
+    const SpecialIdx sx = make_special<R, C, PML>(p, flag, k0, g, owner);
+    const WarpSpecial ws = make_warp_special<R, C, PML>(p, sx);
+    if (PML || ws.mask == SF_SLOW) warp_steps<SF_SLOW, PML, R, C>(E, H, G, cf, p, sx, ws, src, p.n0, nsteps);
+    else warp_steps<SF_MURL | SF_MURR | SF_SRC | SF_PROBE, false, R, C>(E, H, G, cf, p, sx, ws, src, p.n0, nsteps);
   }
-  warp_steps<SPECIAL, PML, false, R, C>(E, H, G, cf, p, sx, ws, src, p.n0, nsteps);
 }
 
 // T steps of a warp tile between two halo refreshes of the resident kernel: the step counter, the special indices
 // and the source stream belong to the caller and live across rounds (restarting the stream would put two global
-// loads on the critical path of every round).
-template <bool SPECIAL, bool PML, typename R, int C>
+// loads on the critical path of every round).  One instantiation per feature set, chosen here once per round.
+template <bool PML, typename R, int C>
 __device__ __forceinline__ void warp_round(R (&E)[C], R (&H)[C], R (&G)[C], const CoefRegs<R, C> &cf, const StepParams<R> &p,
                                            const SpecialIdx &sx, const WarpSpecial &ws, SourceStream<R> &src, int64_t nloc,
                                            int nsteps) {
-  if constexpr (SPECIAL && !PML) {
-    if (ws.w_slow) { warp_steps<true, false, true, R, C>(E, H, G, cf, p, sx, ws, src, nloc, nsteps); return; }
+#define RKETD_ROUND_CASE(M) case M: warp_steps<M, false, R, C>(E, H, G, cf, p, sx, ws, src, nloc, nsteps); break;
+  if (PML || ws.mask == SF_SLOW) {
+    warp_steps<SF_SLOW, PML, R, C>(E, H, G, cf, p, sx, ws, src, nloc, nsteps);
+  } else {
+    switch (ws.mask) {
+      RKETD_ROUND_CASE(0) RKETD_ROUND_CASE(1) RKETD_ROUND_CASE(2) RKETD_ROUND_CASE(3) RKETD_ROUND_CASE(4) RKETD_ROUND_CASE(5)
+      RKETD_ROUND_CASE(6) RKETD_ROUND_CASE(7) RKETD_ROUND_CASE(8) RKETD_ROUND_CASE(9) RKETD_ROUND_CASE(10) RKETD_ROUND_CASE(11)
+      RKETD_ROUND_CASE(12) RKETD_ROUND_CASE(13) RKETD_ROUND_CASE(14) RKETD_ROUND_CASE(15)
+      default: break;
+    }
   }
-  warp_steps<SPECIAL, PML, false, R, C>(E, H, G, cf, p, sx, ws, src, nloc, nsteps);
+#undef RKETD_ROUND_CASE
 }
 
 // ---- host side

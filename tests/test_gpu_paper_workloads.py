@@ -73,7 +73,7 @@ def test_table2_lengths_match_oracle(rk, ncells):
     used = s.counter(rk.CTR_KERNEL_USED)
     E, H, J = s.get_fields()
     s.close()
-    assert used == (rk.KERNEL_RESIDENT if ncells <= 4096 else rk.KERNEL_TBLOCK)
+    assert used == (rk.KERNEL_RESIDENT if ncells <= 20480 else rk.KERNEL_TBLOCK)     # a cluster's registers hold up to ~24 K nodes
     assert np.max(np.abs(ref)) > 0
     assert np.max(np.abs(rec - ref)) <= 1e-12 * np.max(np.abs(ref))
     for g, r in ((E, st.E), (H, st.H), (J, st.J)):
