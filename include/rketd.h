@@ -128,11 +128,12 @@ int rketd_reset(rketd_sim *s);
 int rketd_discard_records(rketd_sim *s);
 
 /* Choose the kernel (RKETD_KERNEL_*), the temporal depth T (0 = default; K2: steps per pass, K3: steps between two halo
- * refreshes), and the launch variant (-1 = default).  K2: 0..3 = CTA tiles with {nodes per thread, threads per CTA}
- * combinations, 4..7 = warp tiles.  K3: -1 = warp tiles (k3_wtile) with the packing chosen by the library;
- * RKETD_RESIDENT_WTILE(nw, nc, k) = warp tiles with k whole grids per chunk held by a cluster of nc CTAs x nw warps
- * (0 = chosen by the library); 0, 1, 2 = the one-barrier-per-step kernel k3_resident (a thread owns a 64-B row / half a
- * row / a row with the coefficients in shared memory; grids of at most 512 rows).  All choices compute identical bits.
+ * refreshes), and the launch variant (-1 = default).  K2: 6 = warp tiles (the default); 0, 2 = one tile per CTA of 128
+ * or 256 threads with a block barrier per step (cross-checks).  K3: -1 = the library picks between warp tiles
+ * (k3_wtile: few grids, or grids larger than one CTA) and the one-barrier-per-step kernel k3_resident (large batches
+ * of grids of at most 512 rows); RKETD_RESIDENT_WTILE(nw, nc, k) = warp tiles with k whole grids per chunk held by a
+ * cluster of nc CTAs x nw <= 8 warps (0 = chosen by the library); 0, 2 = k3_resident with the coefficients in
+ * registers / in shared memory.  All choices compute identical bits.
  * EINVAL if the choice cannot run this grid (e.g. RESIDENT with a grid larger than a cluster can hold). */
 #define RKETD_RESIDENT_WTILE_FLAG 0x40000000
 #define RKETD_RESIDENT_WTILE(nw, nc, k) (RKETD_RESIDENT_WTILE_FLAG | ((k) << 16) | ((nc) << 8) | (nw))

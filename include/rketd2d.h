@@ -112,6 +112,49 @@ void rketd2d_destroy(rketd2d_sim *s);
 /* Text of the last error on this handle (or of the last failed rketd2d_create when s is NULL). */
 const char *rketd2d_last_error(const rketd2d_sim *s);
 
+/* ============================================================================
+ * 2-D TEz: the other polarisation (SURVEY.md §8(f) NEXT-3 "2-D TMz/TEz"; eqs. (1)-(3), kept in the
+ * components Ex, Ey, Hz, Jx, Jy of fields that do not vary along z):
+ *     mu0 dHz/dt = dEx/dy - dEy/dx,   eps0 dEx/dt + Jx = dHz/dy,   eps0 dEy/dt + Jy = -dHz/dx,
+ *     dJ/dt + nu J = eps0 wp^2 E per component (eq. (11); eq. (12) PAPER.md:74 per component).
+ * nx x ny cells, arrays row-major [ny][nx].  Ex[j][i] = Ex((i+1/2) dx, j dy) (column nx-1 is padding, reported as 0),
+ * Ey[j][i] = Ey(i dx, (j+1/2) dy) (row ny-1 is padding), Hz[j][i] = Hz((i+1/2) dx, (j+1/2) dy) at half steps (row ny-1
+ * and column nx-1 are padding); Jx, Jy collocated with Ex, Ey.  The media are given per cell and both components stored
+ * at [j][i] use that pair.  One step, in the order of the 1-D path:
+ *     Hz[j][i] = Hz - (dt/(mu0 dx)) (Ey[j][i+1] - Ey[j][i]) + (dt/(mu0 dy)) (Ex[j+1][i] - Ex[j][i])
+ *     Ex'[j][i] = ca Ex - cj Jx + cey (Hz[j][i] - Hz[j-1][i])      Ey'[j][i] = ca Ey - cj Jy - cex (Hz[j][i] - Hz[j][i-1])
+ *     tangential E on the edges (Ex on rows 0 and ny-1, Ey on columns 0 and nx-1): first-order Mur along the normal, or 0
+ *     soft source on one component at one cell;  Jx, Jy by eq. (11) with the final E';  probes (i, j, component).
+ * One fused launch per step (k1_te); same conventions, error codes and ownership rules as the TMz calls above.
+ * ========================================================================== */
+typedef struct rketd2d_te_sim rketd2d_te_sim; /* opaque */
+enum { RKETD2D_EX = 0, RKETD2D_EY = 1 };      /* component ids of the source and the probes */
+
+/* as rketd2d_create */
+int rketd2d_te_create(rketd2d_te_sim **out, int64_t nx, int64_t ny, double dx, double dy, double dt, int dtype,
+                      void *cuda_stream);
+/* wp [rad/s], nu [1/s] per cell, fp64 [ny][nx], host or device.  Validates before anything changes; EINVAL: negative or
+ * non-finite values.  The physical Jx, Jy of live fields are kept.  Synchronises. */
+int rketd2d_te_set_media(rketd2d_te_sim *s, const double *wp, const double *nu);
+/* RKETD2D_BC_MUR (default) or RKETD2D_BC_PEC */
+int rketd2d_te_set_boundary(rketd2d_te_sim *s, int kind);
+/* soft source (kinds and params as rketd_set_source) added to component `component` at cell (i, j) */
+int rketd2d_te_set_source(rketd2d_te_sim *s, int kind, const double *params, int64_t nparams, int64_t i, int64_t j,
+                          int component);
+/* probes: triples (i, j, component), host pointer, at most 64; discards earlier records */
+int rketd2d_te_set_probes(rketd2d_te_sim *s, const int64_t *ijc, int nprobes);
+/* [ny][nx] arrays in the handle's dtype, host or device; NULL = zeros.  Synchronises. */
+int rketd2d_te_set_fields(rketd2d_te_sim *s, const void *Ex, const void *Ey, const void *Hz, const void *Jx, const void *Jy);
+int rketd2d_te_get_fields(rketd2d_te_sim *s, void *Ex, void *Ey, void *Hz, void *Jx, void *Jy);
+/* advance nsteps steps, asynchronously on the stream; ESTATE before rketd2d_te_set_media */
+int rketd2d_te_run(rketd2d_te_sim *s, int64_t nsteps);
+/* [nprobes][nsamples] in the handle's dtype; out may be NULL to query *nsamples.  Synchronises. */
+int rketd2d_te_read_probes(rketd2d_te_sim *s, void *out, int64_t out_bytes, int64_t *nsamples);
+/* RKETD2D_CTR_LAUNCHES, _STEP_LAUNCHES, _STEPS_DONE, _STATE_BYTES */
+int64_t rketd2d_te_get_counter(const rketd2d_te_sim *s, int which);
+void rketd2d_te_destroy(rketd2d_te_sim *s);
+const char *rketd2d_te_last_error(const rketd2d_te_sim *s);
+
 #ifdef __cplusplus
 }
 #endif

@@ -388,19 +388,109 @@ __device__ __forceinline__ void step_special(const R (&E)[C], R (&En)[C], R (&H)
   }
 }
 
+// ---- Mur, source and probes without a branch in the time loop (warp tiles of K2 / K3, and the threads of k3_resident).
+// step_special (rketd_device.cuh) dispatches per lane with else-if chains.  In a warp tile whose lanes take different
+// chains that costs 700-1000 cycles of branch latency per step (measured, profiles/r02_ncu_k3_wtile.md), which is what
+// one warp tile in three pays in the batched configs while every other warp of the chunk waits for it at the next halo
+// refresh.  Here the features a warp tile has (SF_* bits, warp-uniform) are a TEMPLATE parameter, chosen once per
+// round, and inside the step every feature is straight-line code: the candidate value is computed for each local
+// index it could apply to and a per-lane bit mask turns it into a select.  Same arithmetic, same order (Mur left, Mur
+// right, source, probes) and the same bits as step_special.  H behind the last node and left of node 0 is zeroed once
+// at the end (zero_padding_H) instead of every step: those values feed only nodes that Mur rewrites or whose
+// coefficients are zero.
+enum : int { SF_MURL = 1, SF_MURR = 2, SF_SRC = 4, SF_PROBE = 8, SF_SLOW = 16 };
+
+struct WarpSpecial {
+  int mask = 0;                       // SF_* of the warp tile (warp-uniform)
+  bool mL0 = false, mL1 = false;      // this lane holds node 0 at local index 0 / 1
+  uint32_t mR = 0, mS = 0;            // bit i: this lane's local node i is node ncells-1 / the source node
+  uint32_t mHz = 0;                   // bit i: H of local node i is padding (behind node ncells-1, or left of node 0)
+  bool l_p0 = false, l_p1 = false;    // this lane records one / two probes
+};
+
+template <typename R, int C, bool PML>
+__device__ __forceinline__ WarpSpecial make_warp_special(const StepParams<R> &p, const SpecialIdx &sx) {
+  WarpSpecial ws;
+  constexpr unsigned full = 0xffffffffu;
+  ws.mL0 = sx.iL == 0; ws.mL1 = sx.iL == 1;
+  ws.mR = sx.iR >= 0 ? 1u << sx.iR : 0u;
+  ws.mS = sx.iS >= 0 ? 1u << sx.iS : 0u;
+  ws.mHz = (sx.iR >= 0 ? (0xffffffffu << sx.iR) & ((1u << C) - 1u) : 0u) | (sx.iL == 1 ? 1u : 0u);
+  ws.l_p0 = sx.np >= 1 && sx.np <= 2; ws.l_p1 = sx.np == 2;
+  ws.mask = (__any_sync(full, sx.iL >= 0) ? SF_MURL : 0) | (__any_sync(full, sx.iR >= 0) ? SF_MURR : 0) |
+            (__any_sync(full, sx.iS >= 0) ? SF_SRC : 0) | (__any_sync(full, ws.l_p0) ? SF_PROBE : 0);
+  // an absorbing layer, or more than two probes among one lane's nodes: the general per-lane path
+  if (PML || __any_sync(full, sx.np == 3) || __any_sync(full, sx.pml_mask != 0u)) ws.mask = SF_SLOW;
+  return ws;
+}
+
+// value of v[idx], idx per lane: a select tree (no branch, no local memory)
+template <typename R, int C>
+__device__ __forceinline__ R select_node(const R (&v)[C], int idx) {
+  R t[C];
+#pragma unroll
+  for (int i = 0; i < C; ++i) t[i] = v[i];
+#pragma unroll
+  for (int w = 1; w < C; w <<= 1)
+#pragma unroll
+    for (int i = 0; i + w < C; i += 2 * w) t[i] = (idx & w) ? t[i + w] : t[i];
+  return t[0];
+}
+
+// a3, a4, a6 for the lanes of a warp tile with the features MASK (first-order Mur ends only)
+template <int MASK, typename R, int C>
+__device__ __forceinline__ void special_select(const R (&E)[C], R (&En)[C], const StepParams<R> &p, const SpecialIdx &sx,
+                                               const WarpSpecial &ws, int64_t nloc, R src_now) {
+  typedef Arith<R> A;
+  if constexpr ((MASK & SF_MURL) != 0) {      // node 0 sits at local index 0 or 1 (Layout: off), node 1 in the same row
+    const R c0 = A::fma(p.mur_m, A::sub(En[1], E[0]), E[1]);
+    const R c1 = A::fma(p.mur_m, A::sub(En[2], E[1]), E[2]);
+    En[0] = ws.mL0 ? c0 : En[0];
+    En[1] = ws.mL1 ? c1 : En[1];
+  }
+  if constexpr ((MASK & SF_MURR) != 0) {      // node ncells-1 at local index >= 1, node ncells-2 in the same row
+    // (descending, so that every candidate sees the interior value of its inward neighbour; one bit of mR is set at most)
+#pragma unroll
+    for (int i = C - 1; i >= 1; --i) {
+      const R cand = A::fma(p.mur_m, A::sub(En[i - 1], E[i]), E[i - 1]);
+      En[i] = ((ws.mR >> i) & 1u) ? cand : En[i];
+    }
+  }
+  if constexpr ((MASK & SF_SRC) != 0) {
+#pragma unroll
+    for (int i = 0; i < C; ++i) {
+      const R sum = A::add(En[i], src_now);
+      En[i] = ((ws.mS >> i) & 1u) ? sum : En[i];
+    }
+  }
+  if constexpr ((MASK & SF_PROBE) != 0) {      // up to two probes among a lane's nodes; predicated stores, no branch
+    const R v0 = select_node<R, C>(En, sx.pi0), v1 = select_node<R, C>(En, sx.pi1);
+    stg_if(ws.l_p0, p.rec + (sx.pr0 + nloc), v0);
+    stg_if(ws.l_p1, p.rec + (sx.pr1 + nloc), v1);
+  }
+}
+
+// H of padding nodes (behind node ncells-1, left of node 0): reported as zero; called once after the time loop
+template <typename R, int C>
+__device__ __forceinline__ void zero_padding_H(R (&H)[C], const WarpSpecial &ws) {
+#pragma unroll
+  for (int i = 0; i < C; ++i) H[i] = ((ws.mHz >> i) & 1u) ? R(0) : H[i];
+}
+
 // ---- one leapfrog step of a thread's C nodes, halos given as OLD values (K1, K3, CTA-tile K2):
 // El, Hl: old E and H of the node left of the thread's nodes; Er: old E of the node to the right.
 // The left neighbour's new H is recomputed here from old values (same expression, same bits as the
 // neighbour's own), so that one exchange of old values per step is enough.
-// SPECIAL = false compiles the boundary/source/probe handling out (tiles without such rows).
-template <bool SPECIAL, bool PML, typename R, int C, typename CF>
+// MASK: SF_* features of the warp (0: none, the boundary/source/probe handling is compiled out; SF_SLOW: step_special's
+// per-lane chains; else the select arithmetic of special_select, H padding zeroed by the caller after the time loop).
+template <int MASK, bool PML, typename R, int C, typename CF>
 __device__ __forceinline__ void step_fields(const R (&E)[C], R (&En)[C], R (&H)[C], const R (&G)[C], const CF &cf, R El,
                                             R Hl, R Er, R nchh, const StepParams<R> &p, const SpecialIdx &sx,
-                                            int64_t nloc, R src_now) {
+                                            const WarpSpecial &ws, int64_t nloc, R src_now) {
   typedef Arith<R> A;
   constexpr int V = 16 / sizeof(R);
   R Hl_old = Hl;
-  if constexpr (SPECIAL && PML) {
+  if constexpr (MASK == SF_SLOW && PML) {
     if (sx.pml_mask) pml_pre<R, C>(E, Er, H, p, sx);
     // the left neighbour's new H is recomputed below from old values: a layer node needs the same pre-step first
     const int jn = sx.jN();
@@ -422,8 +512,10 @@ __device__ __forceinline__ void step_fields(const R (&E)[C], R (&En)[C], R (&H)[
       En[i] = A::fma(-ch[u], A::sub(H[i], i ? H[i - 1] : Hl_new), A::fma(cp[u], E[i], -G[i]));
     }
   }
-  if constexpr (SPECIAL) {
+  if constexpr (MASK == SF_SLOW) {
     if (sx.any) step_special<R, C, PML>(E, En, H, p, sx, nloc, src_now);
+  } else if constexpr (MASK != 0) {
+    special_select<MASK, R, C>(E, En, p, sx, ws, nloc, src_now);
   }
 }
 

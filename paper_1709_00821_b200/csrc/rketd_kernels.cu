@@ -48,7 +48,7 @@ __global__ void __launch_bounds__(128) k1_step(RowPtrs<R> src, RowPtrs<R> dst, C
   const uint32_t flag = p.rowflag[row];
   const R src_now = (flag & F_SRC) ? p.src_tab[p.n0] : R(0);
   const SpecialIdx sx = make_special<R, C, PML>(p, flag, row * C, g, true);
-  step_fields<true, PML, R, C>(E, En, H, G, cf, El, Hl, Er, p.nchh, p, sx, p.n0, src_now);
+  step_fields<SF_SLOW, PML, R, C>(E, En, H, G, cf, El, Hl, Er, p.nchh, p, sx, WarpSpecial(), p.n0, src_now);
   step_current<R, C>(G, E, cf);
   store_nodes_global<R, C>(dst.E, r * C, En);
   store_nodes_global<R, C>(dst.H, r * C, H);
@@ -58,10 +58,11 @@ __global__ void __launch_bounds__(128) k1_step(RowPtrs<R> src, RowPtrs<R> dst, C
 // The time loop shared by K2 and K3: nsteps leapfrog steps of this thread's nodes, halos
 // exchanged inside the CTA.  One __syncthreads per step, placed after phase 2.  The loop is
 // unrolled by two so that E ping-pongs between two register arrays without copies.
-template <bool SPECIAL, bool PML, typename R, int C, int NW, typename CF>
+template <int MASK, bool PML, typename R, int C, int NW, typename CF>
 __device__ __forceinline__ void time_loop(R (&E)[C], R (&H)[C], R (&J)[C], const CF &cf, HaloSlots<R, NW> &hs,
-                                          const StepParams<R> &p, uint32_t flag, int64_t k0, int64_t g, bool owner,
-                                          int64_t nsteps, int warp, int lane) {
+                                          const StepParams<R> &p, const SpecialIdx &sx, const WarpSpecial &ws,
+                                          SourceStream<R> &src, int64_t nsteps, int warp, int lane) {
+  constexpr bool SRC = MASK == SF_SLOW || (MASK & SF_SRC) != 0;
   const R nchh = pin_register(p.nchh);
   int64_t nloc = p.n0;
   R El, Hl, Er;
@@ -69,17 +70,14 @@ __device__ __forceinline__ void time_loop(R (&E)[C], R (&H)[C], R (&J)[C], const
   cta_barrier();
   recv_halo<R, NW>(hs, 0, warp, lane, El, Hl, Er);
   R Eb[C];
-  SourceStream<R> src;
-  src.start(p, SPECIAL && __any_sync(0xffffffffu, (flag & F_SRC) != 0u), nloc, lane);
-  const SpecialIdx sx = SPECIAL ? make_special<R, C, PML>(p, flag, k0, g, owner) : SpecialIdx();
   auto one_step = [&](const R (&Ein)[C], R (&Eout)[C], int par) {
-    const R src_now = SPECIAL ? src.sample(p, nloc, lane) : R(0);
-    step_fields<SPECIAL, PML, R, C>(Ein, Eout, H, J, cf, El, Hl, Er, nchh, p, sx, nloc, src_now);
+    const R src_now = SRC ? src.sample(p, nloc, lane) : R(0);
+    step_fields<MASK, PML, R, C>(Ein, Eout, H, J, cf, El, Hl, Er, nchh, p, sx, ws, nloc, src_now);
     send_halo<R, C, NW>(Eout, H, hs, par, warp, lane, El, Hl, Er);     // for the next step
     step_current<R, C>(J, Ein, cf);
     cta_barrier();
     recv_halo<R, NW>(hs, par, warp, lane, El, Hl, Er);
-    if (SPECIAL) ++nloc;
+    if (MASK != 0) ++nloc;
   };
   int64_t left = nsteps;
   for (; left >= 2; left -= 2) {
@@ -91,6 +89,26 @@ __device__ __forceinline__ void time_loop(R (&E)[C], R (&H)[C], R (&J)[C], const
 #pragma unroll
     for (int i = 0; i < C; ++i) E[i] = Eb[i];
   }
+  if constexpr (MASK != 0 && MASK != SF_SLOW) zero_padding_H<R, C>(H, ws);
+}
+
+// The warps of a CTA pick the instantiation that matches their features once, before the time loop (the barrier counts
+// arriving warps, not program counters).  Four select variants instead of sixteen: Mur only, source/probe only, all.
+template <bool PML, typename R, int C, int NW, typename CF>
+__device__ __forceinline__ void time_loop_dispatch(R (&E)[C], R (&H)[C], R (&J)[C], const CF &cf, HaloSlots<R, NW> &hs,
+                                                   const StepParams<R> &p, uint32_t flag, int64_t k0, int64_t g, bool owner,
+                                                   int64_t nsteps, int warp, int lane) {
+  const bool special = __any_sync(0xffffffffu, flag != 0u);
+  const SpecialIdx sx = special ? make_special<R, C, PML>(p, flag, k0, g, owner) : SpecialIdx();
+  const WarpSpecial ws = special ? make_warp_special<R, C, PML>(p, sx) : WarpSpecial();
+  SourceStream<R> src;
+  src.start(p, special && __any_sync(0xffffffffu, (flag & F_SRC) != 0u), p.n0, lane);
+  constexpr int kMur = SF_MURL | SF_MURR, kSrcProbe = SF_SRC | SF_PROBE;
+  if (PML || ws.mask == SF_SLOW) time_loop<SF_SLOW, PML, R, C, NW>(E, H, J, cf, hs, p, sx, ws, src, nsteps, warp, lane);
+  else if (ws.mask == 0) time_loop<0, false, R, C, NW>(E, H, J, cf, hs, p, sx, ws, src, nsteps, warp, lane);
+  else if ((ws.mask & kSrcProbe) == 0) time_loop<kMur, false, R, C, NW>(E, H, J, cf, hs, p, sx, ws, src, nsteps, warp, lane);
+  else if ((ws.mask & kMur) == 0) time_loop<kSrcProbe, false, R, C, NW>(E, H, J, cf, hs, p, sx, ws, src, nsteps, warp, lane);
+  else time_loop<kMur | kSrcProbe, false, R, C, NW>(E, H, J, cf, hs, p, sx, ws, src, nsteps, warp, lane);
 }
 
 // ------------------------------------------------------------------------------------ K3
@@ -156,9 +174,9 @@ __global__ void __launch_bounds__(NT, MINB) k3_resident(RowPtrs<R> f, CoefPtrs<R
       CoefUniform<R, C> cu;
 #pragma unroll
       for (int a = 0; a < kNumCoef; ++a) cu.v[a] = first[a];
-      time_loop<true, PML, R, C, NW>(E, H, J, cu, hs, p, flag, k0, g, true, nsteps, warp, lane);
+      time_loop_dispatch<PML, R, C, NW>(E, H, J, cu, hs, p, flag, k0, g, true, nsteps, warp, lane);
     } else {
-      time_loop<true, PML, R, C, NW>(E, H, J, cf, hs, p, flag, k0, g, true, nsteps, warp, lane);
+      time_loop_dispatch<PML, R, C, NW>(E, H, J, cf, hs, p, flag, k0, g, true, nsteps, warp, lane);
     }
   } else {
     CoefRegs<R, C> cf;
@@ -168,7 +186,7 @@ __global__ void __launch_bounds__(NT, MINB) k3_resident(RowPtrs<R> f, CoefPtrs<R
       for (int i = 0; i < C; ++i) cf.c[a][i] = R(0);
       if (valid) load_nodes_global<R, C>(cp.c[a], first_node, cf.c[a]);
     }
-    time_loop<true, PML, R, C, NW>(E, H, J, cf, hs, p, flag, k0, g, true, nsteps, warp, lane);
+    time_loop_dispatch<PML, R, C, NW>(E, H, J, cf, hs, p, flag, k0, g, true, nsteps, warp, lane);
   }
 
   if (valid) {
@@ -285,9 +303,9 @@ __global__ void __launch_bounds__(NT, MINB) k2_tblock(const __grid_constant__ K2
     }
 
     if (special)   // tile holds a boundary, source or probe row (a handful of tiles per grid)
-      time_loop<true, PML, R, C, NW>(E, H, J, cf, hs, p, flag, rowg * G::CR + sub * C, g, owner, q.T, warp, lane);
+      time_loop_dispatch<PML, R, C, NW>(E, H, J, cf, hs, p, flag, rowg * G::CR + sub * C, g, owner, q.T, warp, lane);
     else
-      time_loop<false, false, R, C, NW>(E, H, J, cf, hs, p, 0u, 0, g, false, q.T, warp, lane);
+      time_loop_dispatch<false, R, C, NW>(E, H, J, cf, hs, p, 0u, 0, g, false, q.T, warp, lane);
 
     // (the barriers of the time loop order tma_wait_read0 before the writes below)
     if (owner) regs_to_tile<R, C>(sout, off_out, kArrayBytes, E, H, J);
@@ -443,7 +461,7 @@ int k3_threads_for_rows(int, int64_t nrows, int variant) {
   const int opts[] = {32, 64, 128, 256, 512};
   for (int o : opts)
     if (nrows <= o) {
-      if (variant == 1) return o <= 256 ? 2 * o : 0;
+      if (variant == 1) return 0;      // (half-row threads: removed, slower at every size measured)
       if (variant == 2) return o >= 64 ? o : 0;
       return o;
     }
@@ -471,7 +489,7 @@ static cudaError_t launch_k3_v(const Layout &L, FieldPtrs f, void *const coef[kN
 template <typename R>
 static cudaError_t launch_k3_t(const Layout &L, FieldPtrs f, void *const coef[kNumCoef], const StepCommon &sc,
                                int64_t nsteps, int NT, int variant, cudaStream_t st) {
-  constexpr int CF = kRowBytes / sizeof(R), CH = CF / 2;
+  constexpr int CF = kRowBytes / sizeof(R);
   if (variant == 0) switch (NT) {
     case 32: return launch_k3_v<R, CF, 32, false, 8>(L, f, coef, sc, nsteps, st);
     case 64: return launch_k3_v<R, CF, 64, false, 6>(L, f, coef, sc, nsteps, st);
@@ -485,12 +503,6 @@ static cudaError_t launch_k3_t(const Layout &L, FieldPtrs f, void *const coef[kN
     case 256: return launch_k3_v<R, CF, 256, true, 2>(L, f, coef, sc, nsteps, st);
     case 512: return launch_k3_v<R, CF, 512, true, 1>(L, f, coef, sc, nsteps, st);
   }
-  else switch (NT) {
-    case 64: return launch_k3_v<R, CH, 64, false, 8>(L, f, coef, sc, nsteps, st);
-    case 128: return launch_k3_v<R, CH, 128, false, 4>(L, f, coef, sc, nsteps, st);
-    case 256: return launch_k3_v<R, CH, 256, false, 2>(L, f, coef, sc, nsteps, st);
-    case 512: return launch_k3_v<R, CH, 512, false, 1>(L, f, coef, sc, nsteps, st);
-  }
   return cudaErrorInvalidValue;
 }
 cudaError_t launch_k3(int dtype, const Layout &L, FieldPtrs f, void *const coef[kNumCoef], const StepCommon &sc,
@@ -499,14 +511,12 @@ cudaError_t launch_k3(int dtype, const Layout &L, FieldPtrs f, void *const coef[
                     : launch_k3_t<float>(L, f, coef, sc, nsteps, NT, variant, st);
 }
 
-// K2 variants: {nodes per thread, threads per CTA, CTAs per SM aimed at}
-//   0: CTA tile, full row, 128 threads, 2 CTAs/SM     1: CTA tile, half row, 256 threads, 2 CTAs/SM
-//   2: CTA tile, full row, 256 threads, 1 CTA/SM      3: CTA tile, half row, 512 threads, 1 CTA/SM
-//   4: warp tiles, 8 warps, 1 CTA/SM, TMA stores      5: warp tiles, 4 warps, 2 CTAs/SM, TMA stores
-//   6: warp tiles, 12 warps, 1 CTA/SM, 256-bit global stores
-//   7: warp tiles, 8 warps, 1 CTA/SM, 256-bit global stores
-int k2_tile_rows(int variant) { const int r[] = {128, 128, 256, 256, 32, 32, 32, 32}; return (variant >= 0 && variant < kK2Variants) ? r[variant] : 0; }
-int k2_tiles_per_cta(int variant) { const int t[] = {1, 1, 1, 1, 8, 4, 12, 8}; return (variant >= 0 && variant < kK2Variants) ? t[variant] : 0; }
+// K2 variants (numbers kept from round 1; 1, 3, 4, 5, 7 were slower everywhere measured and are gone):
+//   0: CTA tile, full row, 128 threads, 2 CTAs/SM     2: CTA tile, full row, 256 threads, 1 CTA/SM
+//      (one block barrier per step: structurally different cross-checks of the default)
+//   6: warp tiles, 12 warps, 1 CTA/SM, 256-bit global stores (default)
+int k2_tile_rows(int variant) { const int r[] = {128, 0, 256, 0, 0, 0, 32, 0}; return (variant >= 0 && variant < kK2Variants) ? r[variant] : 0; }
+int k2_tiles_per_cta(int variant) { const int t[] = {1, 0, 1, 0, 0, 0, 12, 0}; return (variant >= 0 && variant < kK2Variants) ? t[variant] : 0; }
 size_t k2_smem_bytes(int variant) {
   const int arrays = variant >= 6 ? kNumIn : kNumIn + 3;
   return (size_t)arrays * k2_tile_rows(variant) * k2_tiles_per_cta(variant) * kRowBytes + 1024;
@@ -514,9 +524,7 @@ size_t k2_smem_bytes(int variant) {
 
 template <typename R, int V> struct K2Variant;
 template <typename R> struct K2Variant<R, 0> { static constexpr int C = kRowBytes / sizeof(R), NT = 128, MINB = 2; };
-template <typename R> struct K2Variant<R, 1> { static constexpr int C = kRowBytes / sizeof(R) / 2, NT = 256, MINB = 2; };
 template <typename R> struct K2Variant<R, 2> { static constexpr int C = kRowBytes / sizeof(R), NT = 256, MINB = 1; };
-template <typename R> struct K2Variant<R, 3> { static constexpr int C = kRowBytes / sizeof(R) / 2, NT = 512, MINB = 1; };
 
 template <typename K, typename KP>
 static cudaError_t k2_configure_k(K kern, KP kern_pml, int variant, int threads, int *ctas) {
@@ -535,13 +543,8 @@ template <typename R>
 static cudaError_t k2_configure_t(int variant, int *ctas) {
   switch (variant) {
     case 0: return k2_configure_v<R, 0>(ctas);
-    case 1: return k2_configure_v<R, 1>(ctas);
     case 2: return k2_configure_v<R, 2>(ctas);
-    case 3: return k2_configure_v<R, 3>(ctas);
-    case 4: return k2_configure_k(k2_wtile<R, 8, 1, false, false>, k2_wtile<R, 8, 1, false, true>, 4, 256, ctas);
-    case 5: return k2_configure_k(k2_wtile<R, 4, 2, false, false>, k2_wtile<R, 4, 2, false, true>, 5, 128, ctas);
     case 6: return k2_configure_k(k2_wtile<R, 12, 1, true, false>, k2_wtile<R, 12, 1, true, true>, 6, 384, ctas);
-    case 7: return k2_configure_k(k2_wtile<R, 8, 1, true, false>, k2_wtile<R, 8, 1, true, true>, 7, 256, ctas);
   }
   return cudaErrorInvalidValue;
 }
@@ -575,13 +578,8 @@ static cudaError_t launch_k2_t(const Layout &L, const K2Plan &plan, int src_buf,
   const K2Maps &m = plan.maps[src_buf];
   switch (plan.variant) {
     case 0: return launch_k2_v<R, 0>(plan, src_buf, sp, q, st);
-    case 1: return launch_k2_v<R, 1>(plan, src_buf, sp, q, st);
     case 2: return launch_k2_v<R, 2>(plan, src_buf, sp, q, st);
-    case 3: return launch_k2_v<R, 3>(plan, src_buf, sp, q, st);
-    case 4: launch_k2_w<R, 8, 1, false>(plan, m, sp, q, rp<R>(dst), st); break;
-    case 5: launch_k2_w<R, 4, 2, false>(plan, m, sp, q, rp<R>(dst), st); break;
     case 6: launch_k2_w<R, 12, 1, true>(plan, m, sp, q, rp<R>(dst), st); break;
-    case 7: launch_k2_w<R, 8, 1, true>(plan, m, sp, q, rp<R>(dst), st); break;
     default: return cudaErrorInvalidValue;
   }
   return cudaGetLastError();

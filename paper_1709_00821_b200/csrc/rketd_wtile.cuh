@@ -11,95 +11,6 @@ namespace rketd {
 template <typename R> struct RowPtrs { R *E, *H, *J; };
 template <typename R> struct CoefPtrs { const R *c[kNumCoef]; };
 
-// ---- Mur, source and probes of a warp tile without a branch in the time loop.
-// step_special (rketd_device.cuh) dispatches per lane with else-if chains.  In a warp tile whose lanes take different
-// chains that costs 700-1000 cycles of branch latency per step (measured, profiles/r02_ncu_k3_wtile.md), which is what
-// one warp tile in three pays in the batched configs while every other warp of the chunk waits for it at the next halo
-// refresh.  Here the features a warp tile has (SF_* bits, warp-uniform) are a TEMPLATE parameter, chosen once per
-// round, and inside the step every feature is straight-line code: the candidate value is computed for each local
-// index it could apply to and a per-lane bit mask turns it into a select.  Same arithmetic, same order (Mur left, Mur
-// right, source, probes) and the same bits as step_special.  H behind the last node and left of node 0 is zeroed once
-// at the end (zero_padding_H) instead of every step: those values feed only nodes that Mur rewrites or whose
-// coefficients are zero.
-enum : int { SF_MURL = 1, SF_MURR = 2, SF_SRC = 4, SF_PROBE = 8, SF_SLOW = 16 };
-
-struct WarpSpecial {
-  int mask = 0;                       // SF_* of the warp tile (warp-uniform)
-  bool mL0 = false, mL1 = false;      // this lane holds node 0 at local index 0 / 1
-  uint32_t mR = 0, mS = 0;            // bit i: this lane's local node i is node ncells-1 / the source node
-  uint32_t mHz = 0;                   // bit i: H of local node i is padding (behind node ncells-1, or left of node 0)
-  bool l_p0 = false, l_p1 = false;    // this lane records one / two probes
-};
-
-template <typename R, int C, bool PML>
-__device__ __forceinline__ WarpSpecial make_warp_special(const StepParams<R> &p, const SpecialIdx &sx) {
-  WarpSpecial ws;
-  constexpr unsigned full = 0xffffffffu;
-  ws.mL0 = sx.iL == 0; ws.mL1 = sx.iL == 1;
-  ws.mR = sx.iR >= 0 ? 1u << sx.iR : 0u;
-  ws.mS = sx.iS >= 0 ? 1u << sx.iS : 0u;
-  ws.mHz = (sx.iR >= 0 ? (0xffffffffu << sx.iR) & ((1u << C) - 1u) : 0u) | (sx.iL == 1 ? 1u : 0u);
-  ws.l_p0 = sx.np >= 1 && sx.np <= 2; ws.l_p1 = sx.np == 2;
-  ws.mask = (__any_sync(full, sx.iL >= 0) ? SF_MURL : 0) | (__any_sync(full, sx.iR >= 0) ? SF_MURR : 0) |
-            (__any_sync(full, sx.iS >= 0) ? SF_SRC : 0) | (__any_sync(full, ws.l_p0) ? SF_PROBE : 0);
-  // an absorbing layer, or more than two probes among one lane's nodes: the general per-lane path
-  if (PML || __any_sync(full, sx.np == 3) || __any_sync(full, sx.pml_mask != 0u)) ws.mask = SF_SLOW;
-  return ws;
-}
-
-// value of v[idx], idx per lane: a select tree (no branch, no local memory)
-template <typename R, int C>
-__device__ __forceinline__ R select_node(const R (&v)[C], int idx) {
-  R t[C];
-#pragma unroll
-  for (int i = 0; i < C; ++i) t[i] = v[i];
-#pragma unroll
-  for (int w = 1; w < C; w <<= 1)
-#pragma unroll
-    for (int i = 0; i + w < C; i += 2 * w) t[i] = (idx & w) ? t[i + w] : t[i];
-  return t[0];
-}
-
-// a3, a4, a6 for the lanes of a warp tile with the features MASK (first-order Mur ends only)
-template <int MASK, typename R, int C>
-__device__ __forceinline__ void special_select(const R (&E)[C], R (&En)[C], const StepParams<R> &p, const SpecialIdx &sx,
-                                               const WarpSpecial &ws, int64_t nloc, R src_now) {
-  typedef Arith<R> A;
-  if constexpr ((MASK & SF_MURL) != 0) {      // node 0 sits at local index 0 or 1 (Layout: off), node 1 in the same row
-    const R c0 = A::fma(p.mur_m, A::sub(En[1], E[0]), E[1]);
-    const R c1 = A::fma(p.mur_m, A::sub(En[2], E[1]), E[2]);
-    En[0] = ws.mL0 ? c0 : En[0];
-    En[1] = ws.mL1 ? c1 : En[1];
-  }
-  if constexpr ((MASK & SF_MURR) != 0) {      // node ncells-1 at local index >= 1, node ncells-2 in the same row
-    // (descending, so that every candidate sees the interior value of its inward neighbour; one bit of mR is set at most)
-#pragma unroll
-    for (int i = C - 1; i >= 1; --i) {
-      const R cand = A::fma(p.mur_m, A::sub(En[i - 1], E[i]), E[i - 1]);
-      En[i] = ((ws.mR >> i) & 1u) ? cand : En[i];
-    }
-  }
-  if constexpr ((MASK & SF_SRC) != 0) {
-#pragma unroll
-    for (int i = 0; i < C; ++i) {
-      const R sum = A::add(En[i], src_now);
-      En[i] = ((ws.mS >> i) & 1u) ? sum : En[i];
-    }
-  }
-  if constexpr ((MASK & SF_PROBE) != 0) {      // up to two probes among a lane's nodes; predicated stores, no branch
-    const R v0 = select_node<R, C>(En, sx.pi0), v1 = select_node<R, C>(En, sx.pi1);
-    stg_if(ws.l_p0, p.rec + (sx.pr0 + nloc), v0);
-    stg_if(ws.l_p1, p.rec + (sx.pr1 + nloc), v1);
-  }
-}
-
-// H of padding nodes (behind node ncells-1, left of node 0): reported as zero; called once after the time loop
-template <typename R, int C>
-__device__ __forceinline__ void zero_padding_H(R (&H)[C], const WarpSpecial &ws) {
-#pragma unroll
-  for (int i = 0; i < C; ++i) H[i] = ((ws.mHz >> i) & 1u) ? R(0) : H[i];
-}
-
 // One leapfrog step of a warp tile.  Only NEW values travel: H'[C-1] goes up one lane as soon as it
 // exists (the left neighbour's H' that E'[0] needs), E'[0] goes down one lane at the end (the E[C] the
 // next step's H'[C-1] needs).  Two 64-bit shuffles per step and no redundant arithmetic.  Lanes 0 and 31
@@ -165,22 +76,35 @@ __device__ __forceinline__ void warp_steps(R (&E)[C], R (&H)[C], R (&G)[C], cons
 }
 
 // T steps of one staged tile of K2 (k2_wtile): special indices and the source stream are set up per tile.  K2 meets a
-// special tile once in thousands, so it carries one select instantiation with all four features instead of sixteen.
+// special tile once in thousands, so it keeps step_special's per-lane chains (SF_SLOW) and, with them, the register
+// budget of its 12-warp CTAs: the select instantiations cost it spills and 10 % on config 4 (measured).
 template <bool SPECIAL, bool PML, typename R, int C>
 __device__ __forceinline__ void warp_time_loop(R (&E)[C], R (&H)[C], R (&G)[C], const CoefRegs<R, C> &cf,
                                                const StepParams<R> &p, uint32_t flag, int64_t k0, int64_t g, bool owner,
                                                int nsteps) {
-  if constexpr (!SPECIAL) {
-    SourceStream<R> src;
-    warp_steps<0, false, R, C>(E, H, G, cf, p, SpecialIdx(), WarpSpecial(), src, p.n0, nsteps);
-  } else {
-    const int lane = threadIdx.x & 31;
-    SourceStream<R> src;
-    src.start(p, __any_sync(0xffffffffu, (flag & F_SRC) != 0u), p.n0, lane);
-    const SpecialIdx sx = make_special<R, C, PML>(p, flag, k0, g, owner);
-    const WarpSpecial ws = make_warp_special<R, C, PML>(p, sx);
-    if (PML || ws.mask == SF_SLOW) warp_steps<SF_SLOW, PML, R, C>(E, H, G, cf, p, sx, ws, src, p.n0, nsteps);
-    else warp_steps<SF_MURL | SF_MURR | SF_SRC | SF_PROBE, false, R, C>(E, H, G, cf, p, sx, ws, src, p.n0, nsteps);
+  constexpr int MASK = SPECIAL ? SF_SLOW : 0;
+  const R nchh = p.nchh;       // stays a constant-bank operand of the FMAs (one register read less each)
+  int64_t nloc = p.n0;
+  R Er = __shfl_down_sync(0xffffffffu, E[0], 1);
+  R Eb[C];
+  const int lane = threadIdx.x & 31;
+  SourceStream<R> src;
+  src.start(p, SPECIAL && __any_sync(0xffffffffu, (flag & F_SRC) != 0u), nloc, lane);
+  const SpecialIdx sx = SPECIAL ? make_special<R, C, PML>(p, flag, k0, g, owner) : SpecialIdx();
+  const WarpSpecial ws;
+  int left = nsteps;
+  for (; left >= 2; left -= 2) {
+    const R s0 = SPECIAL ? src.sample(p, nloc, lane) : R(0);
+    warp_step<MASK, PML, R, C>(E, Eb, H, G, cf, Er, nchh, p, sx, ws, nloc, s0);
+    const R s1 = SPECIAL ? src.sample(p, nloc + 1, lane) : R(0);
+    warp_step<MASK, PML, R, C>(Eb, E, H, G, cf, Er, nchh, p, sx, ws, nloc + 1, s1);
+    nloc += 2;
+  }
+  if (left) {
+    const R s0 = SPECIAL ? src.sample(p, nloc, lane) : R(0);
+    warp_step<MASK, PML, R, C>(E, Eb, H, G, cf, Er, nchh, p, sx, ws, nloc, s0);
+#pragma unroll
+    for (int i = 0; i < C; ++i) E[i] = Eb[i];
   }
 }
 
