@@ -316,6 +316,8 @@ class Workload2D:
     initial_E: Callable[..., Optional[np.ndarray]]
     dtypes: Tuple[str, ...] = ("f64", "f32")
     notes: str = ""
+    src_comp: int = 1                   # TEz runs: component the soft source drives / the probes read (0 = Ex, 1 = Ey)
+    probe_comp: int = 1
 
     @property
     def cell_updates(self) -> int:
