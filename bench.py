@@ -509,6 +509,101 @@ def run_tm2d(args):
         dist.destroy_process_group()
 
 
+FP_INSTR_PER_CELL_STEP_TE = 15   # rketd2d_te.cu: Hz 4, Ex 4, Ey 3, Gx 2, Gy 2
+ARRAYS_PER_PASS_TE = 14          # read Ex, Ey, Hz, Gx, Gy, P, ce, ka, Q; write Ex, Ey, Hz, Gx, Gy
+
+
+def run_te2d(args):
+    """--workload te2d[:nx:ny:nsteps]: the 2-D TEz polarisation, one fused launch per step (k1_te):
+    HBM-bound, 14 arrays per step.  Same JSON contract as the other workloads."""
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: librketd has no CPU fallback")
+    from paper_1709_00821_b200 import build as lib_build
+    lib_build.build_library()
+    from paper_1709_00821_b200 import rketd2d, workloads as wl
+    f = args.workload.split(":")
+    w = wl.tm2d_column(nsteps=200) if len(f) == 1 else wl.tm2d_column(nx=int(f[1]), ny=int(f[2]), nsteps=int(f[3]))
+    esize = 8 if args.dtype == "f64" else 4
+    npdt = np.float64 if args.dtype == "f64" else np.float32
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    stream = torch.cuda.current_stream()
+    wp, nu = w.media()
+    E0 = np.ascontiguousarray(w.initial_E(), npdt)
+    sim = rketd2d.Sim2DTE(w.nx, w.ny, w.dx, w.dy, w.dt, args.dtype, stream=stream.cuda_stream)
+    wp_d, nu_d = torch.from_numpy(wp).cuda(), torch.from_numpy(nu).cuda()
+    sim.set_media(wp_d, nu_d)
+    del wp_d, nu_d
+    sim.set_fields(Ey=torch.from_numpy(E0).cuda())
+    sim.set_boundary(w.boundary)
+    sim.set_source(w.src_kind, w.src_params, w.src_ij[0], w.src_ij[1], w.src_comp)
+    probes = [(int(i), int(j), int(w.probe_comp)) for i, j in w.probes]
+    sim.set_probes(probes)
+    units = w.nx * w.ny * w.nsteps
+    for _ in range(args.warmup):
+        sim.run(w.nsteps)
+        sim.set_probes(probes)               # drops the records
+    torch.cuda.synchronize()
+    l0 = sim.counter(rketd2d.CTR_STEP_LAUNCHES)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local) as clk:
+        ev0.record(stream)
+        for _ in range(args.steps):
+            sim.run(w.nsteps)
+        ev1.record(stream)
+        torch.cuda.synchronize()
+    ms = ev0.elapsed_time(ev1)
+    launches = sim.counter(rketd2d.CTR_STEP_LAUNCHES) - l0
+    value = units * args.steps / (ms * 1e-3) / 1e9
+    hbm_gbs, peak_src, _ = measured_peaks()
+    alg = ARRAYS_PER_PASS_TE * esize * w.nx * w.ny
+    achieved = alg / (ms / launches * 1e-3) / 1e9
+    roof = {"bound": "hbm", "achieved": achieved, "peak": hbm_gbs, "unit": "GB/s", "frac": achieved / hbm_gbs, "traffic": None,
+            "peak_source": peak_src, "algorithmic_bytes_per_launch": alg, "ms_per_launch": ms / launches, "depth_T": 1,
+            "note": "achieved = 14 arrays (read Ex,Ey,Hz,Gx,Gy,P,ce,ka,Q; write Ex,Ey,Hz,Gx,Gy) x cells x esize per step / mean launch time"}
+    e2e = None
+    if not args.no_e2e:
+        wp_h, nu_h, E0_h = torch.from_numpy(wp).pin_memory(), torch.from_numpy(nu).pin_memory(), torch.from_numpy(E0).pin_memory()
+        out_h = torch.empty((len(probes), w.nsteps), dtype=torch.float64 if args.dtype == "f64" else torch.float32).pin_memory()
+
+        def e2e_step():
+            sim.set_probes(probes)
+            sim.set_media(wp_h, nu_h)
+            sim.set_fields(Ey=E0_h)
+            sim.run(w.nsteps)
+            sim.read_probes(out_h)
+        e2e_step()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        e2e_step()
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        e2e = {"value": units / dt / 1e9, "unit": UNIT, "h2d_bytes_per_step": int(wp_h.numel() * 16 + E0_h.numel() * esize),
+               "d2h_bytes_per_step": int(out_h.numel() * esize), "steps": 1,
+               "note": "rketd2d_te_set_media + set_fields(Ey0) from pinned host, rketd2d_te_run, read_probes to pinned host"}
+    sim.close()
+    cpu = None
+    if not args.no_cpu:
+        import oracle
+        oracle.build()
+        side, steps = min(w.nx, w.ny, 1536), min(w.nsteps, 100)
+        i0 = min(max(0, w.src_ij[0] - side // 2), w.nx - side); j0 = min(max(0, w.src_ij[1] - side // 2), w.ny - side)
+        t0 = time.perf_counter()
+        oracle.run_workload2d_te(w, nsteps=steps, window=(i0, i0 + side, j0, j0 + side), omp=True)
+        dt = time.perf_counter() - t0
+        cpu = {"value": side * side * steps / dt / 1e9, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
+               "sample": f"cells {i0}..{i0 + side - 1} x {j0}..{j0 + side - 1} of the {w.nx} x {w.ny} grid x {steps} steps (OpenMP build, {dt:.1f} s)"}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype,
+            "data": "synthetic",
+            "config": {"workload": w.name + "_TEz", "nx": w.nx, "ny": w.ny, "nsteps_per_run": w.nsteps, "cell_updates_per_step": units,
+                       "kernel": "k1_te", "l2": "inputs larger than L2 (%.1f GB per step)" % (alg / 1e9), "parallelism": "single GPU"},
+            "clocks": clk.summary(), "roofline": roof, "e2e": e2e, "cpu_baseline": cpu, "gpu_launches": int(launches),
+            "stencil_launches": int(launches)}
+    print(json.dumps(line), flush=True)
+
+
 def roofline_1d(rketd, w, dtype, gcells, ms, step_launches, kernel_used, depth, tile_cells, halo_cells, variant, stream):
     """roofline object of the stencil kernel a 1-D run used (gcells: per-GPU Gcell/s of the timed region, ms: its length)"""
     esize = 8 if dtype == "f64" else 4
@@ -628,6 +723,8 @@ def main():
         return run_reference(args)
     if args.workload.startswith("tm2d"):
         return run_tm2d(args)
+    if args.workload.startswith("te2d"):
+        return run_te2d(args)
 
     import torch
     import torch.distributed as dist

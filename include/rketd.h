@@ -195,7 +195,12 @@ int64_t rketd_get_counter(const rketd_sim *s, int which);
 enum {
   RKETD_PEAK_DFMA_1REG = 0, RKETD_PEAK_DFMA_2REG = 1, RKETD_PEAK_DFMA_3REG = 2, RKETD_PEAK_DFMA_2REG_CONST = 3,
   RKETD_PEAK_FFMA_1REG = 4, RKETD_PEAK_FFMA_2REG = 5, RKETD_PEAK_FFMA_3REG = 6, RKETD_PEAK_FFMA_2REG_CONST = 7,
-  RKETD_PEAK_MIX_F64 = 8, RKETD_PEAK_MIX_F32 = 9, RKETD_PEAK_LDS128 = 10
+  RKETD_PEAK_MIX_F64 = 8, RKETD_PEAK_MIX_F32 = 9, RKETD_PEAK_LDS128 = 10,
+  /* latencies: out[0] = ns, out[1] = cycles per operation (16 x iters operations in a dependent chain) */
+  RKETD_LAT_DFMA = 11, RKETD_LAT_SHFL64 = 12,       /* dependent DFMA; 64-bit __shfl_up                                  */
+  RKETD_LAT_STEP_F64 = 13, RKETD_LAT_STEP_F32 = 14, /* one leapfrog step of a warp tile, one warp per scheduler          */
+  RKETD_LAT_BAR_SYNC = 15,                          /* bar.sync of 256 threads                                           */
+  RKETD_LAT_CLUSTER_BARRIER = 16                    /* barrier.cluster arrive.release + wait.acquire, 8 CTAs x 128        */
 };
 int rketd_measure_peak(int what, int iters, double *out, void *cuda_stream);
 

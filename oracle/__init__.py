@@ -103,6 +103,12 @@ def _lib(omp: bool = False) -> ctypes.CDLL:
                                         ctypes.c_int, _D, ctypes.c_int64, ctypes.c_int64, ctypes.c_int64, ctypes.c_int,
                                         _I64, ctypes.c_int, ctypes.c_int64, ctypes.c_int64, _D, ctypes.c_int, ctypes.c_int]
         lib.oracle2d_te_run.restype = ctypes.c_int
+        lib.oracle2d_run_pml.argtypes = [ctypes.c_int64, ctypes.c_int64, ctypes.c_double, ctypes.c_double, ctypes.c_double,
+                                         _D, _D, _D, _D, _D, _D, _D,
+                                         ctypes.c_int, _D, ctypes.c_int64, ctypes.c_int64, ctypes.c_int64,
+                                         _I64, ctypes.c_int, ctypes.c_int64, ctypes.c_int64, _D,
+                                         ctypes.c_int, ctypes.c_double, ctypes.c_double]
+        lib.oracle2d_run_pml.restype = ctypes.c_int
         _loaded[omp] = lib
     return _loaded[omp]
 
@@ -256,6 +262,30 @@ def run2d(state: State2D, wp, nu, dx: float, dy: float, dt: float, nsteps: int, 
         raise ValueError("oracle2d_run: invalid argument")
     state.step += nsteps
     return rec, recJ
+
+
+def run2d_pml(state: State2D, wp, nu, dx: float, dy: float, dt: float, nsteps: int, *, pml=(5, 3.0, 1e-6),
+              src_kind: int = SRC_NONE, src_params: Sequence[float] = (), src_ij=(0, 0), probes=(), omp: bool = False):
+    """2-D TMz with Berenger's split-field layer on the four sides (oracle2d_run_pml).  The split parts Ezx, Ezy are kept
+    on the state (state.Esplit, [2][ny][nx], created as zeros on first use: a field given inside a layer starts as Ezx).
+    Returns rec [nprobes][nsteps]."""
+    ny, nx = state.Ez.shape
+    if not hasattr(state, "Esplit"):
+        state.Esplit = np.zeros((2, ny, nx))
+        state.Esplit[0] = state.Ez
+    wp = np.ascontiguousarray(wp, np.float64).reshape(ny, nx)
+    nu = np.ascontiguousarray(nu, np.float64).reshape(ny, nx)
+    prm = np.ascontiguousarray(src_params, np.float64)
+    prb = np.ascontiguousarray(probes, np.int64).reshape(-1, 2)
+    rec = np.zeros((prb.shape[0], nsteps))
+    rc = _lib(omp).oracle2d_run_pml(nx, ny, dx, dy, dt, _p(wp), _p(nu), _p(state.Ez), _p(state.Hx), _p(state.Hy),
+                                    _p(state.Jz), _p(state.Esplit), src_kind, _p(prm) if prm.size else None, prm.size,
+                                    int(src_ij[0]), int(src_ij[1]), prb.ctypes.data_as(_I64) if prb.size else None,
+                                    prb.shape[0], state.step, nsteps, _p(rec), int(pml[0]), float(pml[1]), float(pml[2]))
+    if rc:
+        raise ValueError("oracle2d_run_pml: invalid argument")
+    state.step += nsteps
+    return rec
 
 
 def run_workload2d(w, nsteps: Optional[int] = None, window=None, omp: bool = False, boundary: Optional[int] = None):

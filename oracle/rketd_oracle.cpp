@@ -525,4 +525,109 @@ int oracle2d_te_run(int64_t nx, int64_t ny, double dx, double dy, double dt,
   return 0;
 }
 
+
+// ============================================================================
+// 2-D TMz with the paper's boundary: Berenger's split-field layer on the four sides ("both the electric and
+// magnetic fields are divided into two directions, both of which execute in their own kernel", :123 "PML ... of 5
+// cells").  Reading: the 1-D reading of §12 applied per axis —
+// sigma_x depends on x only, sigma_y on y only, polynomial grading sigma(rho) = sigma_max rho^m with sigma_max =
+// -(m+1) eps0 c ln(R0) / (2 npml d) for the step d of that axis, matched sigma* = sigma mu0/eps0, a conductor behind
+// the layer (Ez = 0 on the four edges), layer nodes vacuum (media there ignored, Jz = 0).  In the layer Ez = Ezx + Ezy:
+//     Ezx' = ax[i] Ezx + bx[i] (Hy[j][i] - Hy[j][i-1]),   Ezy' = ay[j] Ezy - by[j] (Hx[j][i] - Hx[j-1][i]),
+//     a = (1-s)/(1+s), b = (dt/(eps0 d))/(1+s), s = sigma dt/(2 eps0) at the E node;
+//     Hx' = hay[j] Hx - hby[j] (Ez[j+1][i] - Ez[j][i]),   Hy' = hax[i] Hy + hbx[i] (Ez[j][i+1] - Ez[j][i])   everywhere,
+//     ha = (1-s)/(1+s), hb = (dt/(mu0 d))/(1+s) with s at the H node (half a node deeper); outside the layers ha = 1,
+//     hb = dt/(mu0 d) and the products with 1 are exact, so the interior is the plain update bit for bit.
+// Nodes outside every layer take the unsplit plasma update of oracle2d_run.  Esplit = [2][ny][nx]: Ezx, Ezy (state,
+// meaningful on layer nodes).  Pins (tests/test_oracle2d_pins.py, U1-U4): fields uniform along one axis reproduce the
+// 1-D PML oracle bit for bit (both axes); R0 = 1 equals the conducting box up to rounding; the energy never grows;
+// an obliquely incident pulse comes back smaller than from first-order Mur.
+// ============================================================================
+int oracle2d_run_pml(int64_t nx, int64_t ny, double dx, double dy, double dt,
+                     const double* wp, const double* nu, double* Ez, double* Hx, double* Hy, double* Jz, double* Esplit,
+                     int src_kind, const double* src_params, int64_t nparams, int64_t src_i, int64_t src_j,
+                     const int64_t* probes, int nprobes, int64_t step0, int64_t nsteps,
+                     double* rec, int npml, double pml_m, double pml_R0) {
+  if (nx < 3 || ny < 3 || nsteps < 0 || dx <= 0 || dy <= 0 || dt <= 0 || !Esplit) return 1;
+  if (npml < 1 || 2 * (int64_t)npml + 1 > nx || 2 * (int64_t)npml + 1 > ny || !(pml_R0 > 0.0) || pml_R0 > 1.0 || pml_m < 0.0) return 1;
+  if (src_kind >= 0 && (src_i < 0 || src_i >= nx || src_j < 0 || src_j >= ny)) return 1;
+  for (int p = 0; p < nprobes; ++p)
+    if (probes[2 * p] < 0 || probes[2 * p] >= nx || probes[2 * p + 1] < 0 || probes[2 * p + 1] >= ny) return 1;
+  const int64_t n = nx * ny;
+  std::vector<double> ca(n), cj(n), cex(n), cey(n), ka(n), kb(n), kc(n), Eold(n);
+  double g[4];
+  oracle2d_coefficients(n, wp, nu, dx, dy, dt, 0, ca.data(), cj.data(), cex.data(), cey.data(), ka.data(), kb.data(), kc.data(), g);
+  const double chx = g[0], chy = g[1];
+  // per-axis tables over the whole axis: E nodes 0..N-1, H nodes 0..N-2 (value 1 / plain coefficient outside the layers)
+  auto tables = [&](int64_t N, double d, std::vector<double>& ea, std::vector<double>& eb, std::vector<double>& ha,
+                    std::vector<double>& hb, double ch) {
+    ea.assign(N, 1.0); eb.assign(N, dt / (kEps0 * d)); ha.assign(N, 1.0); hb.assign(N, ch);
+    const double smax = -(pml_m + 1.0) * kEps0 * kC0 * std::log(pml_R0) / (2.0 * double(npml) * d);
+    for (int j = 0; j < npml; ++j) {
+      const double rho_e = double(npml - j) / double(npml);
+      const double rho_h = (double(npml - j) - 0.5) / double(npml);
+      const double se = smax * std::pow(rho_e, pml_m) * dt / (2.0 * kEps0);
+      const double sh = smax * std::pow(rho_h, pml_m) * dt / (2.0 * kEps0);
+      ea[j] = ea[N - 1 - j] = (1.0 - se) / (1.0 + se);
+      eb[j] = eb[N - 1 - j] = (dt / (kEps0 * d)) / (1.0 + se);
+      ha[j] = ha[N - 2 - j] = (1.0 - sh) / (1.0 + sh);
+      hb[j] = hb[N - 2 - j] = ch / (1.0 + sh);
+    }
+  };
+  std::vector<double> eax, ebx, hax, hbx, eay, eby, hay, hby;
+  tables(nx, dx, eax, ebx, hax, hbx, chx);
+  tables(ny, dy, eay, eby, hay, hby, chy);
+  double* Ezx = Esplit;
+  double* Ezy = Esplit + n;
+#define AT(j, i) ((j) * nx + (i))
+  for (int64_t s = 0; s < nsteps; ++s) {
+    const int64_t ng = step0 + s;
+    // S1: H, damped inside the layers
+#pragma omp parallel for schedule(static)
+    for (int64_t j = 0; j < ny; ++j)
+      for (int64_t i = 0; i < nx; ++i) {
+        if (j <= ny - 2) Hx[AT(j, i)] = hay[j] * Hx[AT(j, i)] - hby[j] * (Ez[AT(j + 1, i)] - Ez[AT(j, i)]);
+        if (i <= nx - 2) Hy[AT(j, i)] = hax[i] * Hy[AT(j, i)] + hbx[i] * (Ez[AT(j, i + 1)] - Ez[AT(j, i)]);
+      }
+    // S2: E — split in the layers, the plasma update elsewhere
+#pragma omp parallel for schedule(static)
+    for (int64_t k = 0; k < n; ++k) Eold[k] = Ez[k];
+#pragma omp parallel for schedule(static)
+    for (int64_t j = 1; j <= ny - 2; ++j)
+      for (int64_t i = 1; i <= nx - 2; ++i) {
+        const int64_t k = AT(j, i);
+        const bool layer = i < npml || i > nx - 1 - npml || j < npml || j > ny - 1 - npml;
+        if (layer) {
+          Ezx[k] = eax[i] * Ezx[k] + ebx[i] * (Hy[k] - Hy[AT(j, i - 1)]);
+          Ezy[k] = eay[j] * Ezy[k] - eby[j] * (Hx[k] - Hx[AT(j - 1, i)]);
+          Ez[k] = Ezx[k] + Ezy[k];
+        } else {
+          Ez[k] = ca[k] * Eold[k] - cj[k] * Jz[k] + cex[k] * (Hy[k] - Hy[AT(j, i - 1)]) - cey[k] * (Hx[k] - Hx[AT(j - 1, i)]);
+        }
+      }
+    // S3: the conductor behind the layer
+    for (int64_t j = 0; j < ny; ++j) { Ez[AT(j, 0)] = 0.0; Ez[AT(j, nx - 1)] = 0.0; }
+    for (int64_t i = 0; i < nx; ++i) { Ez[AT(0, i)] = 0.0; Ez[AT(ny - 1, i)] = 0.0; }
+    // S4: soft source (a source inside a layer drives the x part)
+    if (src_kind >= 0) {
+      const double sv = source_sample(src_kind, src_params, nparams, ng, dt);
+      const int64_t k = AT(src_j, src_i);
+      Ez[k] += sv;
+      Ezx[k] += sv;
+    }
+    // S5: J outside the layers (layer nodes are vacuum)
+#pragma omp parallel for schedule(static)
+    for (int64_t j = 0; j < ny; ++j)
+      for (int64_t i = 0; i < nx; ++i) {
+        const int64_t k = AT(j, i);
+        const bool layer = i < npml || i > nx - 1 - npml || j < npml || j > ny - 1 - npml;
+        Jz[k] = layer ? 0.0 : ka[k] * Jz[k] + kb[k] * Eold[k] + kc[k] * Ez[k];
+      }
+    for (int p = 0; p < nprobes; ++p)
+      if (rec) rec[int64_t(p) * nsteps + s] = Ez[AT(probes[2 * p + 1], probes[2 * p])];
+  }
+#undef AT
+  return 0;
+}
+
 }  // extern "C"

@@ -11,11 +11,15 @@
 //     registers, neighbours inside the lane, no shuffles, no memory: the issue ceiling of the real instruction mix at
 //     the occupancy of the warp-tile kernels (12 warps per SM).
 //   LDS.128: every thread reads 16 B per instruction from a conflict-free shared-memory tile.
+//   latencies (cycles per operation in out[1]): a chain of dependent DFMAs, a chain of 64-bit shuffles, one leapfrog
+//     step of a warp tile (warp_step of rketd_wtile.cuh, no special lanes) with one warp per scheduler, bar.sync of
+//     256 threads, the cluster barrier of 8 CTAs x 128 threads.
 #include <cuda_runtime.h>
 #include <stdint.h>
 
 #include "../../include/rketd.h"
 #include "rketd_device.cuh"
+#include "rketd_wtile.cuh"
 
 namespace rketd {
 namespace {
@@ -148,13 +152,71 @@ __global__ void __launch_bounds__(1024) lds_kernel(float *out, int iters, Stamp 
   if (acc.x + acc.y + acc.z + acc.w == 123.456f) out[0] = acc.x;
 }
 
+__global__ void lat_dfma_kernel(double *io, int iters, Stamp *st) {
+  double a = io[0], b = io[1], c = io[2];
+  stamp_begin(st);
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int u = 0; u < 16; ++u) asm volatile("fma.rn.f64 %0, %0, %1, %2;" : "+d"(a) : "d"(b), "d"(c));
+  }
+  stamp_end(st);
+  if (a == 123.456) io[3] = a;
+}
+__global__ void lat_shfl_kernel(double *io, int iters, Stamp *st) {
+  double a = io[threadIdx.x & 3];
+  stamp_begin(st);
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int u = 0; u < 16; ++u) a = __shfl_up_sync(0xffffffffu, a, 1);
+  }
+  stamp_end(st);
+  if (a == 123.456) io[3] = a;
+}
+template <typename R>
+__global__ void __launch_bounds__(128, 1) lat_step_kernel(const R *in, R *out, int nsteps, const __grid_constant__ StepParams<R> p, Stamp *st) {
+  constexpr int C = kRowBytes / sizeof(R);
+  R E[C], H[C], G[C];
+  CoefRegs<R, C> cf;
+#pragma unroll
+  for (int i = 0; i < C; ++i) {
+    E[i] = in[i]; H[i] = in[C + i]; G[i] = in[2 * C + i];
+#pragma unroll
+    for (int a = 0; a < kNumCoef; ++a) cf.c[a][i] = in[(3 + a) * C + i];
+  }
+  SourceStream<R> src;
+  stamp_begin(st);
+  warp_steps<0, false, R, C>(E, H, G, cf, p, SpecialIdx(), WarpSpecial(), src, 0, nsteps);
+  stamp_end(st);
+  R s = 0;
+#pragma unroll
+  for (int i = 0; i < C; ++i) s += E[i] + H[i] + G[i];
+  if (s == R(123.456)) out[0] = s;
+}
+__global__ void lat_bar_kernel(int iters, Stamp *st) {
+  stamp_begin(st);
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int u = 0; u < 16; ++u) asm volatile("bar.sync 0;" ::: "memory");
+  }
+  stamp_end(st);
+}
+__global__ void lat_cluster_kernel(int iters, Stamp *st) {
+  stamp_begin(st);
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int u = 0; u < 16; ++u)
+      asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+  }
+  stamp_end(st);
+}
+
 }  // namespace
 }  // namespace rketd
 
 using namespace rketd;
 
 extern "C" int rketd_measure_peak(int what, int iters, double *out, void *cuda_stream) {
-  if (!out || iters < 1 || what < 0 || what > RKETD_PEAK_LDS128) return RKETD_EINVAL;
+  if (!out || iters < 1 || what < 0 || what > RKETD_LAT_CLUSTER_BARRIER) return RKETD_EINVAL;
   int dev = 0, sms = 0;
   if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
     cudaGetLastError();
@@ -172,7 +234,7 @@ extern "C" int rketd_measure_peak(int what, int iters, double *out, void *cuda_s
   double hd[256];
   float hf[256];
   for (int i = 0; i < 256; ++i) { hd[i] = 1e-3 * (double)((i * 37) % 101 - 50) * 1e-2; hf[i] = (float)hd[i]; }
-  const bool f32 = (what >= RKETD_PEAK_FFMA_1REG && what <= RKETD_PEAK_FFMA_2REG_CONST) || what == RKETD_PEAK_MIX_F32;
+  const bool f32 = (what >= RKETD_PEAK_FFMA_1REG && what <= RKETD_PEAK_FFMA_2REG_CONST) || what == RKETD_PEAK_MIX_F32 || what == RKETD_LAT_STEP_F32;
   cudaMemcpyAsync(buf, f32 ? (const void *)hf : (const void *)hd, f32 ? sizeof(hf) : sizeof(hd), cudaMemcpyHostToDevice, st);
   double per_thread = 0.0;          // thread-instructions (or bytes) per thread
   int threads = 1024, blocks = sms;
@@ -191,6 +253,26 @@ extern "C" int rketd_measure_peak(int what, int iters, double *out, void *cuda_s
       case RKETD_PEAK_MIX_F64: threads = 384; mix_kernel<double><<<blocks, threads, 0, st>>>((double *)buf, (double *)buf + 300, iters, -1e-3, stamp); break;
       case RKETD_PEAK_MIX_F32: threads = 384; mix_kernel<float><<<blocks, threads, 0, st>>>((float *)buf, (float *)buf + 300, iters, -1e-3f, stamp); break;
       case RKETD_PEAK_LDS128: lds_kernel<<<blocks, threads, 32768, st>>>((float *)buf + 300, iters, stamp); break;
+      case RKETD_LAT_DFMA: lat_dfma_kernel<<<1, 32, 0, st>>>((double *)buf, iters, stamp); break;
+      case RKETD_LAT_SHFL64: lat_shfl_kernel<<<1, 32, 0, st>>>((double *)buf, iters, stamp); break;
+      case RKETD_LAT_STEP_F64: {
+        StepParams<double> sp = {}; sp.nchh = -1e-3;
+        lat_step_kernel<double><<<blocks, 128, 0, st>>>((double *)buf, (double *)buf + 300, 16 * iters, sp, stamp);
+      } break;
+      case RKETD_LAT_STEP_F32: {
+        StepParams<float> sp = {}; sp.nchh = -1e-3f;
+        lat_step_kernel<float><<<blocks, 128, 0, st>>>((float *)buf, (float *)buf + 300, 16 * iters, sp, stamp);
+      } break;
+      case RKETD_LAT_BAR_SYNC: lat_bar_kernel<<<1, 256, 0, st>>>(iters, stamp); break;
+      case RKETD_LAT_CLUSTER_BARRIER: {
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(8); cfg.blockDim = dim3(128); cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 8; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr; cfg.numAttrs = 1;
+        cudaLaunchKernelEx(&cfg, lat_cluster_kernel, iters, stamp);
+      } break;
     }
   }
   if (what <= RKETD_PEAK_FFMA_2REG_CONST) per_thread = (double)iters * kUnroll * kChains;
@@ -210,5 +292,10 @@ extern "C" int rketd_measure_peak(int what, int iters, double *out, void *cuda_s
   out[1] = per_thread * threads / cycles;               // thread-instructions (or bytes) per clock and SM
   out[2] = 1e3 * cycles / ns;                           // SM clock held during the run, MHz
   out[3] = (double)sms;
+  if (what >= RKETD_LAT_DFMA) {                          // latencies: per operation instead of per clock
+    const double ops = 16.0 * iters;
+    out[0] = ns / ops;                                   // ns per operation
+    out[1] = cycles / ops;                               // cycles per operation
+  }
   return RKETD_OK;
 }

@@ -103,6 +103,9 @@ def main(argv):
         return
     print(f"{'form':18s} {'per clk and SM':>15s} {'device per ns':>15s} {'SM MHz held':>12s} {'NVML MHz min':>13s} {'power W max':>12s}")
     for r in rows:
+        if r["name"].startswith("lat_"):
+            print(f"{r['name']:28s} {r['per_clk_sm']:10.1f} cycles per operation ({r['per_ns']:.2f} ns at {r['sm_mhz']:.0f} MHz)")
+            continue
         unit = "B" if r["name"] == "lds128" else "thread-instr"
         print(f"{r['name']:18s} {r['per_clk_sm']:15.2f} {r['per_ns']:15.1f} {r['sm_mhz']:12.1f} "
               f"{str(r['nvml_sm_mhz_min']):>13s} {str(r['power_w_max']):>12s}   ({unit}; {r['sms']} SMs)")

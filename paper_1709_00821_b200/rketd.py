@@ -30,7 +30,8 @@ EXPORTS = ["rketd_create", "rketd_set_media", "rketd_set_source", "rketd_set_pro
            "rketd_read_sweep_rt", "rketd_measure_peak",
            "rketd_get_counter", "rketd_destroy", "rketd_last_error"]
 PEAK_NAMES = ("dfma_1reg", "dfma_2reg", "dfma_3reg", "dfma_2reg_const", "ffma_1reg", "ffma_2reg", "ffma_3reg",
-              "ffma_2reg_const", "mix_f64", "mix_f32", "lds128")      # index = RKETD_PEAK_*
+              "ffma_2reg_const", "mix_f64", "mix_f32", "lds128", "lat_dfma", "lat_shfl64", "lat_step_f64", "lat_step_f32",
+              "lat_bar_sync_256", "lat_cluster_barrier_8x128")      # index = RKETD_PEAK_* / RKETD_LAT_*
 RESIDENT_WTILE_FLAG = 0x40000000
 
 

@@ -266,3 +266,109 @@ def test_Q9_run_is_restartable_and_arguments_are_checked():
         oracle.run2d(st, wp, nu, w.dx, w.dy, w.dt, 1, probes=[(w.nx, 0)])
     with pytest.raises(ValueError):
         oracle.run2d(st, wp, nu, w.dx, w.dy, w.dt, 1, src_kind=0, src_params=SRC, src_ij=(0, w.ny))
+
+
+# ============================================================================ the paper's boundary in 2-D: split-field PML
+PML2 = (8, 2.0, 1e-4)
+
+
+@pytest.mark.parametrize("axis", ["x", "y"])
+def test_U1_pml_uniform_along_one_axis_is_the_1d_pml_oracle_bit_for_bit(axis):
+    """Fields uniform along one axis excite only the split part of the other axis: what is left is the 1-D method with
+    the 1-D layer at both ends — same tables, same node depths (E nodes at (npml-k)/npml, H nodes half
+    a node deeper), same conductor behind.  Pins every index of the per-axis tables and which part carries which curl."""
+    n, nother, nsteps = 300, 2 * 120 + 9, 110
+    dvar, doth = DX, 1.7 * DX
+    wp1, nu1 = _slab_media_1d(n, 140, 190)
+    k = np.arange(n, dtype=np.float64)
+    E1 = np.exp(-((k - 60.0) / 9.0) ** 2) * ((k >= PML2[0]) & (k <= n - 1 - PML2[0]))     # nothing inside the layers at t = 0
+    st1 = oracle.State(n, 1, E0=E1)
+    probes1 = [0, 1, 3, 7, 8, 60, 150, n - 9, n - 2, n - 1]
+    rec1, _ = oracle.run(st1, wp1[None], nu1[None], dvar, DT, nsteps, probes=probes1, boundary=oracle.BOUNDARY_PML, pml=PML2)
+    mid = nother // 2
+    if axis == "x":
+        rep = lambda a: np.repeat(a[None, :], nother, 0)
+        st2 = oracle.State2D(n, nother, Ez0=rep(E1))
+        rec2 = oracle.run2d_pml(st2, rep(wp1), rep(nu1), dvar, doth, DT, nsteps, pml=PML2, probes=[(p, mid) for p in probes1])
+        E2, Hvar, J2 = st2.Ez[mid], -st2.Hy[mid], st2.Jz[mid]
+    else:
+        rep = lambda a: np.repeat(a[:, None], nother, 1)
+        st2 = oracle.State2D(nother, n, Ez0=rep(E1))
+        rec2 = oracle.run2d_pml(st2, rep(wp1), rep(nu1), doth, dvar, DT, nsteps, pml=PML2, probes=[(mid, p) for p in probes1])
+        E2, Hvar, J2 = st2.Ez[:, mid], st2.Hx[:, mid], st2.Jz[:, mid]
+    assert np.max(np.abs(rec1)) > 0.1 and np.max(np.abs(rec1[0][3])) > 1e-3          # the pulse has entered the left layer
+    assert np.array_equal(rec2, rec1[0])
+    assert np.array_equal(E2, st1.E[0]) and np.array_equal(Hvar, st1.H[0]) and np.array_equal(J2, st1.J[0])
+
+
+def test_U2_pml_with_R0_one_is_the_conducting_box():
+    """R0 = 1: sigma = 0 everywhere, the split parts add up to the unsplit vacuum update (up to the rounding of the sum
+    Ezx + Ezy) and the four edges are the conductor: the run equals oracle2d_run with BOUNDARY_PEC when the nodes that
+    would be layer are vacuum."""
+    nx, ny, nsteps = 70, 56, 200
+    wp = np.zeros((ny, nx)); nu = np.zeros((ny, nx))
+    wp[25:35, 30:45] = 2 * math.pi * 28.7e9; nu[25:35, 30:45] = 2e10
+    i = np.arange(nx)[None, :]; j = np.arange(ny)[:, None]
+    E0 = np.exp(-((i - 20.0) / 4.0) ** 2 - ((j - 30.0) / 5.0) ** 2)
+    E0[0, :] = E0[-1, :] = 0.0; E0[:, 0] = E0[:, -1] = 0.0
+    a = oracle.State2D(nx, ny, Ez0=E0)
+    ra = oracle.run2d_pml(a, wp, nu, DX, 1.3 * DX, 0.9 * DT, nsteps, pml=(6, 2.0, 1.0), probes=[(35, 28), (3, 3), (60, 50)])
+    b = oracle.State2D(nx, ny, Ez0=E0)
+    rb, _ = oracle.run2d(b, wp, nu, DX, 1.3 * DX, 0.9 * DT, nsteps, probes=[(35, 28), (3, 3), (60, 50)], boundary=oracle.BOUNDARY_PEC)
+    assert np.max(np.abs(rb)) > 0.05
+    assert np.max(np.abs(ra - rb)) <= 1e-13 * np.max(np.abs(rb))
+    assert np.max(np.abs(a.Ez - b.Ez)) <= 1e-13 * np.max(np.abs(b.Ez)) and np.max(np.abs(a.Jz - b.Jz)) <= 1e-13 * np.max(np.abs(b.Jz))
+
+
+def test_U3_pml_absorbs_an_oblique_pulse_better_than_first_order_mur_and_never_feeds_energy():
+    """A point-like pulse next to a corner: its circular wavefront meets the sides at every angle.  Peak of what comes back
+    to a probe in the middle, relative to the direct pulse: the layer (10 nodes) beats first-order Mur, which is exact at
+    normal incidence only; and the field energy of the lossless vacuum run only goes down once the front is in the layer."""
+    nx, ny, nsteps = 161, 161, 700
+    z = np.zeros((ny, nx))
+    i = np.arange(nx)[None, :]; j = np.arange(ny)[:, None]
+    E0 = np.exp(-((i - 40.0) / 3.0) ** 2 - ((j - 40.0) / 3.0) ** 2)
+    probe = [(80, 80)]
+    a = oracle.State2D(nx, ny, Ez0=E0)
+    ra = oracle.run2d_pml(a, z, z, DX, DX, DT, nsteps, pml=(10, 3.0, 1e-6), probes=probe)[0]
+    b = oracle.State2D(nx, ny, Ez0=E0)
+    rb = oracle.run2d(b, z, z, DX, DX, DT, nsteps, probes=probe, boundary=oracle.BOUNDARY_MUR)[0][0]
+    big = oracle.State2D(3 * nx, 3 * ny, Ez0=np.pad(E0, ((ny, ny), (nx, nx))))           # no boundary within reach: the reference
+    rr = oracle.run2d(big, np.zeros((3 * ny, 3 * nx)), np.zeros((3 * ny, 3 * nx)), DX, DX, DT, nsteps,
+                      probes=[(80 + nx, 80 + ny)], boundary=oracle.BOUNDARY_PEC)[0][0]
+    direct = np.max(np.abs(rr))
+    err_pml, err_mur = np.max(np.abs(ra - rr)) / direct, np.max(np.abs(rb - rr)) / direct
+    print(f"reflection seen at the probe: PML(10) {err_pml:.2e}, Mur-1 {err_mur:.2e}")
+    assert direct > 1e-2 and err_pml < 0.25 * err_mur and err_pml < 5e-3
+    c = oracle.State2D(nx, ny, Ez0=E0)
+    W = []
+    Hx0, Hy0 = c.Hx.copy(), c.Hy.copy()
+    for n in range(300):
+        E_n = c.Ez.copy()
+        oracle.run2d_pml(c, z, z, DX, DX, DT, 1, pml=(10, 3.0, 1e-6))
+        W.append(EPS0 * np.sum(E_n ** 2) + MU0 * (np.sum(c.Hx * Hx0) + np.sum(c.Hy * Hy0)))
+        Hx0, Hy0 = c.Hx.copy(), c.Hy.copy()
+    W = np.array(W)
+    assert np.all(np.diff(W) <= 1e-12 * W[0]) and W[-1] < 0.5 * W[0]
+
+
+def test_U4_pml_restart_and_argument_checks():
+    nx, ny = 60, 50
+    rng = np.random.default_rng(6)
+    wp = rng.uniform(0, 2 * math.pi * 40e9, (ny, nx)); nu = rng.uniform(0, 5e10, (ny, nx))
+    E0 = rng.uniform(-1, 1, (ny, nx))
+    a = oracle.State2D(nx, ny, Ez0=E0)
+    ra = oracle.run2d_pml(a, wp, nu, DX, DX, DT, 60, pml=PML2, src_kind=0, src_params=SRC, src_ij=(3, 20), probes=[(3, 20), (30, 25)])
+    out = []
+    for omp in (False, True):
+        b = oracle.State2D(nx, ny, Ez0=E0)
+        r1 = oracle.run2d_pml(b, wp, nu, DX, DX, DT, 25, pml=PML2, src_kind=0, src_params=SRC, src_ij=(3, 20), probes=[(3, 20), (30, 25)], omp=omp)
+        r2 = oracle.run2d_pml(b, wp, nu, DX, DX, DT, 35, pml=PML2, src_kind=0, src_params=SRC, src_ij=(3, 20), probes=[(3, 20), (30, 25)], omp=omp)
+        out.append(np.concatenate([r1, r2], 1))
+        assert np.array_equal(a.Ez, b.Ez) and np.array_equal(a.Esplit, b.Esplit) and np.array_equal(a.Jz, b.Jz)
+    assert np.array_equal(out[0], ra) and np.array_equal(out[1], ra)
+    assert not np.any(a.Jz[:PML2[0]]) and not np.any(a.Jz[:, -PML2[0]:])              # layer nodes carry no current
+    c = oracle.State2D(nx, ny)
+    for bad in ((0, 2.0, 1e-4), (30, 2.0, 1e-4), (5, 2.0, 0.0), (5, -1.0, 1e-4)):
+        with pytest.raises(ValueError):
+            oracle.run2d_pml(c, wp, nu, DX, DX, DT, 1, pml=bad)
