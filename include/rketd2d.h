@@ -33,7 +33,8 @@ typedef struct rketd2d_sim rketd2d_sim; /* opaque */
 /* grid edges for rketd2d_set_boundary */
 enum {
   RKETD2D_BC_MUR = 0,        /* first-order Mur along the normal of each edge (the 1-D rule a3 per edge); the default */
-  RKETD2D_BC_PEC = 1         /* perfect conductor: Ez = 0 on the four edges                                            */
+  RKETD2D_BC_PEC = 1,        /* perfect conductor: Ez = 0 on the four edges                                            */
+  RKETD2D_BC_PML = 2         /* the paper's split-field layer + conductor: set by rketd2d_set_boundary_pml only         */
 };
 /* kernel selection for rketd2d_set_plan */
 enum {
@@ -94,6 +95,16 @@ int rketd2d_set_plan(rketd2d_sim *s, int kernel, int depth);
 
 /* Advance by nsteps leapfrog steps, asynchronously on the stream.  Repeatable.  ESTATE before rketd2d_set_media. */
 int rketd2d_run(rketd2d_sim *s, int64_t nsteps);
+
+/* The paper's boundary (PAPER.md:93 "both the electric and magnetic fields are divided into two directions", :123 "PML
+ * ... of 5 cells"): Berenger's split-field layer of npml nodes on the four sides, a conductor behind it.  The paper gives
+ * no conductivity profile; the reading built is the 1-D one (rketd_set_boundary) per axis: sigma_x(x),
+ * sigma_y(y) = sigma_max rho^grading, sigma_max = -(grading+1) eps0 c ln(R0) / (2 npml d) for the step d of the axis,
+ * matched magnetic conductivity; Ez = Ezx + Ezy on layer nodes, which are vacuum (media given there are ignored, Jz = 0).
+ * Takes effect at the next rketd2d_set_media (which derives the coefficients): call it before; rketd2d_set_boundary
+ * with MUR / PEC switches back (again at the next rketd2d_set_media).  Runs in the one-step kernel (the streaming
+ * kernel has no layer).  EINVAL: npml outside 1..64, 2 npml + 1 > nx or ny, R0 outside (0, 1], grading < 0. */
+int rketd2d_set_boundary_pml(rketd2d_sim *s, int npml, double grading, double R0);
 
 /* Synchronise and copy out the probe records: [nprobes][nsamples] in the handle's dtype (host or device), sample n
  * is Ez at time (n+1) dt.  out may be NULL to query *nsamples.  EINVAL if out_bytes is too small. */

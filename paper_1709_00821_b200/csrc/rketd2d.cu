@@ -150,6 +150,66 @@ __global__ void __launch_bounds__(128) k1_2d(const P2<R> p, const Arrays<R> a) {
   }
 }
 
+// ------------------------------------------------------------------------------------------------ K1 with the paper's layer
+// Berenger's split-field layer on the four sides, a conductor behind it (rketd2d_set_boundary_pml; PAPER.md:93, :123;
+// reading in DESIGN.md §15 = the 1-D reading of §12 per axis).  Per-axis tables over the whole axis (1 / the plain
+// coefficient outside the layers): H is damped everywhere by its table, Ez = Ezx + Ezy on layer nodes, the plasma update
+// in the (P, G) form elsewhere.  One launch per step, like k1_2d.
+template <typename R>
+struct PmlTabs {
+  const R *hax, *hbx, *eax, *ebx;      // [nx]: Hy' = hax Hy + hbx dEz/di;  Ezx' = eax Ezx + ebx dHy/di
+  const R *hay, *hby, *eay, *eby;      // [ny]: Hx' = hay Hx - hby dEz/dj;  Ezy' = eay Ezy - eby dHx/dj
+  const R *Ezx, *Ezy;
+  R *Ezx2, *Ezy2;
+  int npml;
+};
+template <typename R>
+__device__ __forceinline__ R pml_hx(const P2<R> &p, const Arrays<R> &a, const PmlTabs<R> &t, int i, int j) {
+  typedef Arith<R> A;
+  if (j < 0 || j > p.ny - 2) return R(0);
+  const int64_t k = (int64_t)j * p.pitch + i;
+  return A::fma(-t.hby[j], A::sub(a.E[k + p.pitch], a.E[k]), A::mul(t.hay[j], a.Hx[k]));
+}
+template <typename R>
+__device__ __forceinline__ R pml_hy(const P2<R> &p, const Arrays<R> &a, const PmlTabs<R> &t, int i, int j) {
+  typedef Arith<R> A;
+  if (i < 0 || i > p.nx - 2) return R(0);
+  const int64_t k = (int64_t)j * p.pitch + i;
+  return A::fma(t.hbx[i], A::sub(a.E[k + 1], a.E[k]), A::mul(t.hax[i], a.Hy[k]));
+}
+template <typename R>
+__global__ void __launch_bounds__(128) k1_2d_pml(const P2<R> p, const Arrays<R> a, const PmlTabs<R> t) {
+  typedef Arith<R> A;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= p.nx) return;
+  const int j0 = blockIdx.y * kK1Rows, j1 = min(p.ny, j0 + kK1Rows);
+  for (int j = j0; j < j1; ++j) {
+    const int64_t k = (int64_t)j * p.pitch + i;
+    const R e = a.E[k];
+    const R hxn = pml_hx(p, a, t, i, j), hyn = pml_hy(p, a, t, i, j);
+    const bool edge = i == 0 || i == p.nx - 1 || j == 0 || j == p.ny - 1;
+    const bool layer = i < t.npml || i > p.nx - 1 - t.npml || j < t.npml || j > p.ny - 1 - t.npml;
+    R en = R(0), exn = R(0), eyn = R(0), gn = R(0);
+    if (!edge) {
+      const R dhy = A::sub(hyn, pml_hy(p, a, t, i - 1, j)), dhx = A::sub(hxn, pml_hx(p, a, t, i, j - 1));
+      if (layer) {
+        exn = A::fma(t.ebx[i], dhy, A::mul(t.eax[i], t.Ezx[k]));
+        eyn = A::fma(-t.eby[j], dhx, A::mul(t.eay[j], t.Ezy[k]));
+        en = A::add(exn, eyn);
+      } else {
+        en = A::fma(a.cce[k], A::fma(p.nr, dhx, dhy), A::fma(a.cP[k], e, -a.G[k]));
+        gn = A::fma(a.cka[k], a.G[k], A::mul(a.cQ[k], e));
+      }
+    }
+    if (i == p.src_i && j == p.src_j) { en = A::add(en, p.src[0]); exn = A::add(exn, p.src[0]); }
+    a.Hx2[k] = hxn; a.Hy2[k] = hyn; a.G2[k] = gn; a.E2[k] = en;
+    t.Ezx2[k] = exn; t.Ezy2[k] = eyn;
+    if (p.rowflag[j] & RF_PROBE)
+      for (int q = 0; q < p.nprobes; ++q)
+        if (p.probe_i[q] == i && p.probe_j[q] == j) p.rec[(int64_t)q * p.rec_stride + p.n0] = en;
+  }
+}
+
 // ------------------------------------------------------------------------------------------------ K2
 template <typename R>
 __device__ __forceinline__ void cp_async_val(R *smem_dst, const R *gsrc, bool valid) {
@@ -448,7 +508,7 @@ __global__ void __launch_bounds__(StripThreads<R, T>::value, 1) k2_2d(const P2<R
 template <typename R>
 __global__ void coef2d_kernel(int nx, int ny, int64_t pitch, const double *__restrict__ wp, const double *__restrict__ nu,
                               double dx, double dt, double eps0, double *wp_p, double *nu_p, R *cP, R *cce, R *cka, R *cQ,
-                              int *bad) {
+                              int *bad, int npml) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= pitch * ny) return;
   const int64_t j = idx / pitch, i = idx - j * pitch;
@@ -457,6 +517,7 @@ __global__ void coef2d_kernel(int nx, int ny, int64_t pitch, const double *__res
     w = wp[j * nx + i];
     v = nu[j * nx + i];
     if (!(w >= 0.0) || !(v >= 0.0) || isinf(w) || isinf(v)) atomicOr(bad, 1);
+    if (npml > 0 && (i < npml || i > nx - 1 - npml || j < npml || j > ny - 1 - npml)) { w = 0.0; v = 0.0; }   // layer nodes are vacuum
     const rketd::Six s = rketd::six_coefficients(w, v, dx, dt, eps0, 0);
     const double kcp = __dmul_rn(s.cj, s.kc), kbp = __dmul_rn(s.cj, s.kb);
     vP = __dsub_rn(s.ca, kcp);
@@ -525,7 +586,13 @@ struct rketd2d_sim {
   uint8_t *rowflag = nullptr;
   int *d_bad = nullptr;
   bool flags_dirty = true, have_media = false, fields_zero = true, third_is_J = false;
-  int bc = RKETD2D_BC_MUR;
+  int bc = RKETD2D_BC_MUR, bc_next = RKETD2D_BC_MUR;
+  // the paper's layer (rketd2d_set_boundary_pml): requested parameters; `pml_live` = the live coefficients were derived
+  // with it (layer nodes vacuum); split parts Ezx, Ezy (ping-pong) and the eight per-axis tables, allocated on first use
+  int pml_npml = 0, pml_live = 0;
+  double pml_m = 3.0, pml_R0 = 1e-6;
+  void *split[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};
+  void *tabs = nullptr;
   int src_kind = RKETD_SRC_NONE;
   std::vector<double> src_params;
   int src_i = -1, src_j = -1;
@@ -689,7 +756,8 @@ cudaError_t launch_k2(rketd2d_sim *s, P2<R> &p, int T) {
 
 template <typename R>
 int run_typed(rketd2d_sim *s, int64_t nsteps, void *rec) {
-  const bool stream_kernel = s->plan_kernel != RKETD2D_KERNEL_STEP;
+  const bool pml = s->bc == RKETD2D_BC_PML;
+  const bool stream_kernel = s->plan_kernel != RKETD2D_KERNEL_STEP && !pml;      // the layer runs in the one-step kernel
   const int Tdef = s->plan_depth > 0 ? s->plan_depth : 8;
   s->ctr_kernel_used = stream_kernel ? RKETD2D_KERNEL_STREAM : RKETD2D_KERNEL_STEP;
   s->ctr_depth_used = stream_kernel ? Tdef : 1;
@@ -709,7 +777,19 @@ int run_typed(rketd2d_sim *s, int64_t nsteps, void *rec) {
       CU_TRY2(s, launch_k2<R>(s, p, T));
     } else {
       dim3 grid((unsigned)((s->nx + 127) / 128), (unsigned)((s->ny + kK1Rows - 1) / kK1Rows));
-      k1_2d<R><<<grid, 128, 0, s->stream>>>(p, arrays_of<R>(s));
+      if (pml) {
+        PmlTabs<R> t;
+        const R *tb = (const R *)s->tabs;
+        t.hax = tb; t.hbx = tb + s->nx; t.eax = tb + 2 * s->nx; t.ebx = tb + 3 * s->nx;
+        const R *ty = tb + 4 * (int64_t)s->nx;
+        t.hay = ty; t.hby = ty + s->ny; t.eay = ty + 2 * s->ny; t.eby = ty + 3 * s->ny;
+        t.Ezx = (const R *)s->split[s->cur][0]; t.Ezy = (const R *)s->split[s->cur][1];
+        t.Ezx2 = (R *)s->split[1 - s->cur][0]; t.Ezy2 = (R *)s->split[1 - s->cur][1];
+        t.npml = s->pml_live;
+        k1_2d_pml<R><<<grid, 128, 0, s->stream>>>(p, arrays_of<R>(s), t);
+      } else {
+        k1_2d<R><<<grid, 128, 0, s->stream>>>(p, arrays_of<R>(s));
+      }
       CU_TRY2(s, cudaGetLastError());
     }
     s->cur = 1 - s->cur;
@@ -736,6 +816,44 @@ int convert_current(rketd2d_sim *s, bool to_G, void *dstJ) {
 }
 int convert_current_any(rketd2d_sim *s, bool to_G, void *dstJ) {
   return s->dtype == RKETD_F64 ? convert_current<double>(s, to_G, dstJ) : convert_current<float>(s, to_G, dstJ);
+}
+
+// split parts (allocated once) and the eight per-axis tables of the layer, in the handle's dtype:
+// tabs = [hax, hbx, eax, ebx](nx each) then [hay, hby, eay, eby](ny each); 1 / the plain coefficient outside the layers
+int prepare_pml(rketd2d_sim *s, int npml) {
+  for (int b = 0; b < 2; ++b)
+    for (int c = 0; c < 2; ++c)
+      if (!s->split[b][c]) {
+        CU_TRY2(s, cudaMalloc(&s->split[b][c], arr_bytes2(s)));
+        CU_TRY2(s, cudaMemsetAsync(s->split[b][c], 0, arr_bytes2(s), s->stream));
+        s->state_bytes += (int64_t)arr_bytes2(s);
+      }
+  const size_t nt = (size_t)4 * s->nx + (size_t)4 * s->ny;
+  if (!s->tabs) CU_TRY2(s, cudaMalloc(&s->tabs, nt * s->esize));
+  std::vector<double> t(nt);
+  auto fill = [&](double *base, int N, double d) {
+    double *ha = base, *hb = base + N, *ea = base + 2 * N, *eb = base + 3 * N;
+    for (int k = 0; k < N; ++k) { ha[k] = 1.0; hb[k] = s->dt / (kMu0 * d); ea[k] = 1.0; eb[k] = s->dt / (kEps0 * d); }
+    const double smax = -(s->pml_m + 1.0) * kEps0 * kC0 * std::log(s->pml_R0) / (2.0 * (double)npml * d);
+    for (int j = 0; j < npml; ++j) {
+      const double se = smax * std::pow((double)(npml - j) / npml, s->pml_m) * s->dt / (2.0 * kEps0);
+      const double sh = smax * std::pow(((double)(npml - j) - 0.5) / npml, s->pml_m) * s->dt / (2.0 * kEps0);
+      ea[j] = ea[N - 1 - j] = (1.0 - se) / (1.0 + se);
+      eb[j] = eb[N - 1 - j] = (s->dt / (kEps0 * d)) / (1.0 + se);
+      ha[j] = ha[N - 2 - j] = (1.0 - sh) / (1.0 + sh);
+      hb[j] = hb[N - 2 - j] = (s->dt / (kMu0 * d)) / (1.0 + sh);
+    }
+  };
+  fill(t.data(), s->nx, s->dx);
+  fill(t.data() + 4 * (size_t)s->nx, s->ny, s->dy);
+  if (s->dtype == RKETD_F64) {
+    CU_TRY2(s, cudaMemcpyAsync(s->tabs, t.data(), nt * 8, cudaMemcpyHostToDevice, s->stream));
+  } else {
+    std::vector<float> tf(t.begin(), t.end());
+    CU_TRY2(s, cudaMemcpyAsync(s->tabs, tf.data(), nt * 4, cudaMemcpyHostToDevice, s->stream));
+  }
+  CU_TRY2(s, cudaStreamSynchronize(s->stream));      // t is a local
+  return RKETD_OK;
 }
 
 }  // namespace
@@ -817,21 +935,32 @@ int rketd2d_set_media(rketd2d_sim *s, const double *wp, const double *nu) {
     if (rc) { cudaFree(d_wp); cudaFree(d_nu); return rc; }
     s->third_is_J = true;
   }
+  const int npml_new = s->pml_npml;
+  if (npml_new > 0) {                              // the paper's layer: split parts and per-axis tables
+    const int rc = prepare_pml(s, npml_new);
+    if (rc) { cudaFree(d_wp); cudaFree(d_nu); return rc; }
+  }
   s->have_media = false;      // until the new coefficients are in place
   if (s->dtype == RKETD_F64)
     coef2d_kernel<double><<<blocks_for(n), 256, 0, s->stream>>>(s->nx, s->ny, s->pitch, d_wp, d_nu, s->dx, s->dt, kEps0, s->wp_p,
                                                                 s->nu_p, (double *)s->coef[0], (double *)s->coef[1],
-                                                                (double *)s->coef[2], (double *)s->coef[3], s->d_bad);
+                                                                (double *)s->coef[2], (double *)s->coef[3], s->d_bad, npml_new);
   else
     coef2d_kernel<float><<<blocks_for(n), 256, 0, s->stream>>>(s->nx, s->ny, s->pitch, d_wp, d_nu, s->dx, s->dt, kEps0, s->wp_p,
                                                                s->nu_p, (float *)s->coef[0], (float *)s->coef[1],
-                                                               (float *)s->coef[2], (float *)s->coef[3], s->d_bad);
+                                                               (float *)s->coef[2], (float *)s->coef[3], s->d_bad, npml_new);
   e = cudaGetLastError();
   s->ctr_launches++;
   if (e == cudaSuccess) e = cudaStreamSynchronize(s->stream);
   cudaFree(d_wp); cudaFree(d_nu);
   CU_TRY2(s, e);
   s->have_media = true;
+  if (npml_new > 0 && s->pml_live == 0) {          // entering the layer with live fields: Ez starts as its x part
+    CU_TRY2(s, cudaMemcpyAsync(s->split[s->cur][0], s->fld[s->cur][0], arr_bytes2(s), cudaMemcpyDeviceToDevice, s->stream));
+    CU_TRY2(s, cudaMemsetAsync(s->split[s->cur][1], 0, arr_bytes2(s), s->stream));
+  }
+  s->pml_live = npml_new;
+  s->bc = npml_new > 0 ? RKETD2D_BC_PML : s->bc_next;
   if (s->third_is_J) { const int rc = convert_current_any(s, true, nullptr); if (rc) return rc; }
   s->third_is_J = false;
   CU_TRY2(s, cudaStreamSynchronize(s->stream));
@@ -840,8 +969,18 @@ int rketd2d_set_media(rketd2d_sim *s, const double *wp, const double *nu) {
 
 int rketd2d_set_boundary(rketd2d_sim *s, int kind) {
   if (!s) return RKETD_EINVAL;
-  if (kind != RKETD2D_BC_MUR && kind != RKETD2D_BC_PEC) return fail2(s, RKETD_EINVAL, "unknown boundary kind");
-  s->bc = kind;
+  if (kind != RKETD2D_BC_MUR && kind != RKETD2D_BC_PEC) return fail2(s, RKETD_EINVAL, "unknown boundary kind (the layer: rketd2d_set_boundary_pml)");
+  if (s->pml_live > 0) { s->pml_npml = 0; s->bc_next = kind; return RKETD_OK; }      // leaves the layer at the next rketd2d_set_media
+  s->pml_npml = 0;
+  s->bc = s->bc_next = kind;
+  return RKETD_OK;
+}
+
+int rketd2d_set_boundary_pml(rketd2d_sim *s, int npml, double grading, double R0) {
+  if (!s) return RKETD_EINVAL;
+  if (npml < 1 || npml > 64 || 2 * (int64_t)npml + 1 > s->nx || 2 * (int64_t)npml + 1 > s->ny || !(R0 > 0.0) || R0 > 1.0 || !(grading >= 0.0))
+    return fail2(s, RKETD_EINVAL, "need 1 <= npml <= 64, 2 npml + 1 <= nx, ny, 0 < R0 <= 1, grading >= 0");
+  s->pml_npml = npml; s->pml_m = grading; s->pml_R0 = R0;
   return RKETD_OK;
 }
 
@@ -882,6 +1021,10 @@ int rketd2d_set_fields(rketd2d_sim *s, const void *Ez, const void *Hx, const voi
     else CU_TRY2(s, cudaMemsetAsync(s->fld[s->cur][f], 0, arr_bytes2(s), s->stream));
   }
   s->fields_zero = !Ez && !Hx && !Hy && !Jz;
+  if (s->split[0][0]) {                            // the layer's split parts restart from Ezx = Ez, Ezy = 0
+    CU_TRY2(s, cudaMemcpyAsync(s->split[s->cur][0], s->fld[s->cur][0], arr_bytes2(s), cudaMemcpyDeviceToDevice, s->stream));
+    CU_TRY2(s, cudaMemsetAsync(s->split[s->cur][1], 0, arr_bytes2(s), s->stream));
+  }
   if (s->have_media) { const int rc = convert_current_any(s, true, nullptr); if (rc) return rc; s->third_is_J = false; }
   else s->third_is_J = true;
   CU_TRY2(s, cudaStreamSynchronize(s->stream));
@@ -910,6 +1053,8 @@ int rketd2d_reset(rketd2d_sim *s) {
   if (!s) return RKETD_EINVAL;
   CU_TRY2(s, cudaStreamSynchronize(s->stream));
   for (int f = 0; f < 4; ++f) CU_TRY2(s, cudaMemsetAsync(s->fld[s->cur][f], 0, arr_bytes2(s), s->stream));
+  for (int c = 0; c < 2; ++c)
+    if (s->split[s->cur][c]) CU_TRY2(s, cudaMemsetAsync(s->split[s->cur][c], 0, arr_bytes2(s), s->stream));
   discard_records2(s);
   s->step = 0;
   s->fields_zero = true;
@@ -1023,6 +1168,9 @@ void rketd2d_destroy(rketd2d_sim *s) {
     for (int f = 0; f < 4; ++f) cudaFree(s->fld[b][f]);
   for (int c = 0; c < 4; ++c) cudaFree(s->coef[c]);
   cudaFree(s->wp_p); cudaFree(s->nu_p); cudaFree(s->rowflag); cudaFree(s->d_bad);
+  for (int b = 0; b < 2; ++b)
+    for (int c = 0; c < 2; ++c) cudaFree(s->split[b][c]);
+  cudaFree(s->tabs);
   for (auto &c : s->chunks) cudaFree(c.buf);
   cudaGetLastError();
   delete s;

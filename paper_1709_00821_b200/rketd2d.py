@@ -12,12 +12,12 @@ import numpy as np
 
 from .rketd import (F32, F64, OK, RketdError, _dbl, _i32, _i64, _lib, _ptr, _vp)
 
-BC_MUR, BC_PEC = 0, 1
+BC_MUR, BC_PEC, BC_PML = 0, 1, 2
 KERNEL_AUTO, KERNEL_STEP, KERNEL_STREAM = 0, 1, 2
 CTR_LAUNCHES, CTR_STEP_LAUNCHES, CTR_KERNEL_USED, CTR_DEPTH_USED, CTR_STEPS_DONE, CTR_STRIP_COLS, CTR_HALO_COLS, \
     CTR_SEG_ROWS, CTR_STATE_BYTES = range(9)
 
-EXPORTS = ["rketd2d_create", "rketd2d_set_media", "rketd2d_set_boundary", "rketd2d_set_source", "rketd2d_set_probes",
+EXPORTS = ["rketd2d_create", "rketd2d_set_media", "rketd2d_set_boundary_pml", "rketd2d_set_boundary", "rketd2d_set_source", "rketd2d_set_probes",
            "rketd2d_set_fields", "rketd2d_get_fields", "rketd2d_reset", "rketd2d_set_plan", "rketd2d_run",
            "rketd2d_read_probes", "rketd2d_get_kernel_coefficients", "rketd2d_discard_records", "rketd2d_get_counter",
            "rketd2d_destroy", "rketd2d_last_error"]
@@ -30,6 +30,7 @@ EX, EY = 0, 1                # component ids of TEz sources and probes
 _lib.rketd2d_create.argtypes = [ctypes.POINTER(_vp), _i64, _i64, _dbl, _dbl, _dbl, _i32, _vp]
 _lib.rketd2d_set_media.argtypes = [_vp, _vp, _vp]
 _lib.rketd2d_set_boundary.argtypes = [_vp, _i32]
+_lib.rketd2d_set_boundary_pml.argtypes = [_vp, _i32, _dbl, _dbl]
 _lib.rketd2d_set_source.argtypes = [_vp, _i32, _vp, _i64, _i64, _i64]
 _lib.rketd2d_set_probes.argtypes = [_vp, _vp, _i32]
 _lib.rketd2d_set_fields.argtypes = [_vp, _vp, _vp, _vp, _vp]
@@ -46,7 +47,7 @@ _lib.rketd2d_destroy.argtypes = [_vp]
 _lib.rketd2d_destroy.restype = None
 _lib.rketd2d_last_error.argtypes = [_vp]
 _lib.rketd2d_last_error.restype = ctypes.c_char_p
-for _n in EXPORTS[:13]:
+for _n in EXPORTS[:14]:
     getattr(_lib, _n).restype = _i32
 _lib.rketd2d_te_create.argtypes = [ctypes.POINTER(_vp), _i64, _i64, _dbl, _dbl, _dbl, _i32, _vp]
 _lib.rketd2d_te_set_media.argtypes = [_vp, _vp, _vp]
@@ -85,6 +86,10 @@ def rketd2d_set_media(h, wp, nu):
 
 def rketd2d_set_boundary(h, kind: int):
     _check(h, _lib.rketd2d_set_boundary(h, kind))
+
+
+def rketd2d_set_boundary_pml(h, npml: int = 5, grading: float = 3.0, R0: float = 1e-6):
+    _check(h, _lib.rketd2d_set_boundary_pml(h, npml, grading, R0))
 
 
 def rketd2d_set_source(h, kind: int, params: Sequence[float], i: int, j: int):
@@ -168,6 +173,7 @@ class Sim2D:
 
     def set_media(self, wp, nu): rketd2d_set_media(self.h, wp, nu)
     def set_boundary(self, kind): rketd2d_set_boundary(self.h, kind)
+    def set_boundary_pml(self, npml=5, grading=3.0, R0=1e-6): rketd2d_set_boundary_pml(self.h, npml, grading, R0)
     def set_source(self, kind, params, i, j): rketd2d_set_source(self.h, kind, params, i, j)
 
     def set_probes(self, ij):

@@ -349,3 +349,78 @@ def test_full_size_sampled_against_windowed_oracle(dtype, kernel):
           f"per probe {worst_rel:.3e}; final fields on {len(refs)} boxes of {2 * half + 1}^2 nodes against the grid peak: "
           + ", ".join(f"{n} {v:.3e}" for n, v in zip("Ez Hx Hy Jz".split(), worst_f)))
     assert worst / peak <= TOL[dtype]
+
+
+# ----------------------------------------------------------------------------- the paper's boundary: split-field PML
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_pml_layer_against_the_oracle(dtype):
+    """rketd2d_set_boundary_pml: random media, a source next to a corner inside the layer region's
+    reach, probes inside the layers, on the conductor and in the interior; records and final Ez, Hx, Hy, Jz against
+    oracle2d_run_pml; then back to Mur."""
+    m = _mod()
+    nx, ny, nsteps = 150, 110, 160
+    pml = (8, 2.0, 1e-4)
+    rng = np.random.default_rng(21)
+    wp = rng.uniform(0, 2 * np.pi * 40e9, (ny, nx)) * (rng.uniform(size=(ny, nx)) > 0.5)
+    nu = rng.uniform(0, 5e10, (ny, nx))
+    src = (20, 15)
+    probes = [src, (3, 50), (nx - 4, 60), (70, 2), (75, ny - 3), (0, 30), (nx // 2, ny // 2), (9, 9), (nx - 9, ny - 9)]
+    st = oracle.State2D(nx, ny)
+    ref = oracle.run2d_pml(st, wp, nu, DX, 1.2 * DX, 0.9 * DT, nsteps, pml=pml, src_kind=0, src_params=(20e-12, 30e-12, 1.0),
+                           src_ij=src, probes=probes)
+    sim = m.Sim2D(nx, ny, DX, 1.2 * DX, 0.9 * DT, dtype)
+    sim.set_boundary_pml(*pml)
+    sim.set_media(wp, nu)
+    sim.set_source(0, (20e-12, 30e-12, 1.0), *src)
+    sim.set_probes(probes)
+    for part in (1, 59, 100):
+        sim.run(part)
+    rec = sim.read_probes().astype(np.float64)
+    assert sim.counter(m.CTR_KERNEL_USED) == m.KERNEL_STEP            # the layer runs in the one-step kernel
+    Ez, Hx, Hy, Jz = (f.astype(np.float64) for f in sim.get_fields())
+    tol = TOL[dtype]
+    assert np.max(np.abs(ref)) > 0.1 and _err(rec, ref) <= tol
+    pk = np.max(np.abs(st.Ez))
+    assert np.max(np.abs(Ez - st.Ez)) <= tol * pk and np.max(np.abs(Hx - st.Hx)) <= tol * pk / 376.73
+    assert np.max(np.abs(Hy - st.Hy)) <= tol * pk / 376.73 and np.max(np.abs(Jz - st.Jz)) <= tol * np.max(np.abs(st.Jz))
+    assert not np.any(Jz[:pml[0]]) and not np.any(Jz[:, -pml[0]:])       # layer nodes carry no current
+    # back to first-order Mur (takes effect with the next media), fields reset
+    sim.set_boundary(m.BC_MUR)
+    sim.set_media(wp, nu)
+    sim.reset()
+    sim.run(40)
+    st2 = oracle.State2D(nx, ny)
+    ref2, _ = oracle.run2d(st2, wp, nu, DX, 1.2 * DX, 0.9 * DT, 40, src_kind=0, src_params=(20e-12, 30e-12, 1.0), src_ij=src, probes=probes)
+    assert _err(sim.read_probes(), ref2) <= tol
+    from paper_1709_00821_b200.rketd import RketdError
+    for bad in ((0, 2.0, 1e-4), (60, 2.0, 1e-4), (5, 2.0, 0.0), (5, -1.0, 1e-4)):
+        with pytest.raises(RketdError):
+            sim.set_boundary_pml(*bad)
+    sim.close()
+
+
+def test_pml_reflection_floor_on_the_gpu():
+    """the oblique-pulse experiment of oracle pin U3 through the CUDA path: what comes back to the probe with the layer
+    is a small fraction of what first-order Mur returns"""
+    m = _mod()
+    nx = ny = 161
+    z = np.zeros((ny, nx))
+    i = np.arange(nx)[None, :]; j = np.arange(ny)[:, None]
+    E0 = np.exp(-((i - 40.0) / 3.0) ** 2 - ((j - 40.0) / 3.0) ** 2)
+    big = oracle.State2D(3 * nx, 3 * ny, Ez0=np.pad(E0, ((ny, ny), (nx, nx))))
+    rr = oracle.run2d(big, np.zeros((3 * ny, 3 * nx)), np.zeros((3 * ny, 3 * nx)), DX, DX, DT, 700, probes=[(80 + nx, 80 + ny)],
+                      boundary=oracle.BOUNDARY_PEC)[0][0]
+    back = {}
+    for kind in ("pml", "mur"):
+        sim = m.Sim2D(nx, ny, DX, DX, DT)
+        if kind == "pml":
+            sim.set_boundary_pml(10, 3.0, 1e-6)
+        sim.set_media(z, z)
+        sim.set_fields(Ez=E0)
+        sim.set_probes([(80, 80)])
+        sim.set_plan(m.KERNEL_STEP, 0)
+        sim.run(700)
+        back[kind] = np.max(np.abs(sim.read_probes()[0] - rr)) / np.max(np.abs(rr))
+        sim.close()
+    print(f"reflection seen at the probe (GPU): PML(10) {back['pml']:.2e}, Mur-1 {back['mur']:.2e}")
+    assert back["pml"] < 0.25 * back["mur"] and back["pml"] < 5e-3
