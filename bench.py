@@ -691,7 +691,8 @@ def extra_configs(rketd, stream, host_inputs):
             kernel_used, depth_used = sim.counter(rketd.CTR_KERNEL_USED), sim.counter(rketd.CTR_DEPTH_USED)
             roof = roofline_1d(rketd, w, dtype, gc, ms, sim.counter(rketd.CTR_STEP_LAUNCHES) - sl0, kernel_used, depth_used,
                                sim.counter(rketd.CTR_TILE_CELLS), sim.counter(rketd.CTR_HALO_CELLS), -1, stream.cuda_stream)
-            keep = ("bound", "achieved", "peak", "unit", "frac", "peak_source", "frac_of_mix_peak", "alu_frac", "frac_vs_8TBps_nominal")
+            keep = ("bound", "achieved", "peak", "unit", "frac", "peak_source", "frac_of_mix_peak", "alu_frac", "alu_frac_of_mix_peak",
+                    "frac_vs_8TBps_nominal")
             out[key] = {"workload": w.name, "dtype": dtype, "value": gc, "unit": UNIT, "ms_per_step": ms / nrun, "steps": nrun,
                         "kernel": int(kernel_used), "depth_T": int(depth_used), "roofline": {k: roof[k] for k in keep if k in roof}}
             sim.close()

@@ -136,6 +136,7 @@ int rketd_discard_records(rketd_sim *s);
  * registers / in shared memory.  All choices compute identical bits.
  * EINVAL if the choice cannot run this grid (e.g. RESIDENT with a grid larger than a cluster can hold). */
 #define RKETD_RESIDENT_WTILE_FLAG 0x40000000
+#define RKETD_RESIDENT_WTILE_NOLEAN 0x20000000 /* or-ed in: the 232-register instantiation (coefficients in registers) */
 #define RKETD_RESIDENT_WTILE(nw, nc, k) (RKETD_RESIDENT_WTILE_FLAG | ((k) << 16) | ((nc) << 8) | (nw))
 int rketd_set_plan(rketd_sim *s, int kernel, int depth, int variant);
 

@@ -276,7 +276,15 @@ bool wtile_variant(const rketd_sim *s, int variant) {
 bool resident_wtile_plan(rketd_sim *s, int depth, int variant, K3WPlan *P) {
   int64_t nw = 0, nc = 0, k = 0;
   if (variant >= 0) { nw = variant & 0xff; nc = (variant >> 8) & 0xff; k = (variant >> 16) & 0xfff; }
-  if (!k3w_plan(s->L, depth, s->sms, nw, nc, k, P)) return false;
+  // the lean instantiation (<= 128 registers) serves Mur ends with at most two probes among the nodes of one lane
+  bool lean = s->bc_npml == 0 && s->pml.npml == 0 && !(variant >= 0 && (variant & RKETD_RESIDENT_WTILE_NOLEAN));
+  if (lean) {
+    std::vector<int64_t> rows;
+    for (int64_t c : s->probes) rows.push_back((s->L.off + c) / s->L.C);
+    std::sort(rows.begin(), rows.end());
+    for (size_t i = 2; i < rows.size(); ++i) lean = lean && rows[i] != rows[i - 2];
+  }
+  if (!k3w_plan(s->L, depth, s->sms, nw, nc, k, lean, P)) return false;
   if (P->nc > 1) {              // the cluster must be schedulable on this device (GPC size, registers, shared memory)
     int ncl = 0;
     if (k3w_max_clusters(s->dtype, *P, &ncl) != cudaSuccess || ncl < 1) { cudaGetLastError(); return false; }

@@ -53,9 +53,11 @@ __device__ __forceinline__ void cluster_barrier() {
 constexpr int kMaxHR = 2;
 __host__ __device__ constexpr uint32_t slot_bytes_per_warp() { return 2u * kMaxHR * 3u * kRowBytes; }
 
-template <typename R, bool CLUSTER, bool PML>
-__global__ void __launch_bounds__(256, 1) k3_wtile(RowPtrs<R> f, CoefPtrs<R> cp, const __grid_constant__ StepParams<R> p,
-                                                    const K3WArgs q) {
+// LEAN: E in place and coefficients from four registers or the warp's shared-memory rows (warp_step_lean): 168
+// registers, twelve warps per SM instead of eight.  The host picks it unless a layer is live or one lane records more than two probes.
+template <typename R, bool CLUSTER, bool PML, bool LEAN>
+__global__ void __launch_bounds__(LEAN ? 384 : 256, 1) k3_wtile(RowPtrs<R> f, CoefPtrs<R> cp, const __grid_constant__ StepParams<R> p,
+                                                               const K3WArgs q) {
   constexpr int C = kRowBytes / sizeof(R);
   typedef Geom<R, C> G;
   typedef typename Arith<R>::Vec Vec;
@@ -77,22 +79,48 @@ __global__ void __launch_bounds__(256, 1) k3_wtile(RowPtrs<R> f, CoefPtrs<R> cp,
   const bool owner = valid && lane >= q.HR && lane < 32 - q.HR;
 
   R E[C], H[C], J[C];
-  CoefRegs<R, C> cf;
+  typename std::conditional<LEAN, int, CoefRegs<R, C>>::type cf_regs;      // (LEAN keeps no per-node coefficient registers)
+  CoefUniform<R, C> cu;
+  CoefWarpSmem<R, C> cs;
+  bool warp_uniform = false;
 #pragma unroll
   for (int i = 0; i < C; ++i) { E[i] = R(0); H[i] = R(0); J[i] = R(0); }
-#pragma unroll
-  for (int a = 0; a < kNumCoef; ++a)
-#pragma unroll
-    for (int i = 0; i < C; ++i) cf.c[a][i] = R(0);
   uint32_t flag = 0u;
   if (valid) {
     const int64_t first = rowc * C;
     load_nodes_global<R, C>(f.E, first, E);
     load_nodes_global<R, C>(f.H, first, H);
     load_nodes_global<R, C>(f.J, first, J);
-#pragma unroll
-    for (int a = 0; a < kNumCoef; ++a) load_nodes_global<R, C>(cp.c[a], first, cf.c[a]);
     flag = p.rowflag[rowg];
+  }
+  if constexpr (LEAN) {
+    // coefficients: each lane stages its row of the four arrays in the warp's shared-memory area (only this warp reads
+    // it back) and notes whether its nodes all carry one set; a warp of such lanes then runs from four registers
+    const uint32_t cbase = slots + 2u * par_bytes;
+    cs.base = ((cbase + 1023u) & ~1023u) + (uint32_t)warp * (kNumCoef * 32u * kRowBytes);
+    cs.lane = lane;
+    bool uni = true;
+#pragma unroll
+    for (int a = 0; a < kNumCoef; ++a) {
+      R c[C];
+#pragma unroll
+      for (int i = 0; i < C; ++i) c[i] = R(0);
+      if (valid) load_nodes_global<R, C>(cp.c[a], rowc * C, c);
+      cu.v[a] = c[0];
+#pragma unroll
+      for (int i = 1; i < C; ++i) uni = uni && (c[i] == c[0]);
+#pragma unroll
+      for (int j = 0; j < G::NCH; ++j) sts128(cs.base + a * (32 * kRowBytes) + swz_off(lane, j), regs_to_vec<R, C>(c, j));
+    }
+    warp_uniform = __all_sync(0xffffffffu, uni);
+    __syncwarp();
+  } else {
+#pragma unroll
+    for (int a = 0; a < kNumCoef; ++a) {
+#pragma unroll
+      for (int i = 0; i < C; ++i) cf_regs.c[a][i] = R(0);
+      if (valid) load_nodes_global<R, C>(cp.c[a], rowc * C, cf_regs.c[a]);
+    }
   }
   const bool special = __any_sync(0xffffffffu, flag != 0u);
   const SpecialIdx sx = special ? make_special<R, C, PML>(p, flag, rowg * C, g, owner) : SpecialIdx();
@@ -123,7 +151,14 @@ __global__ void __launch_bounds__(256, 1) k3_wtile(RowPtrs<R> f, CoefPtrs<R> cp,
   uint32_t par = 0u;
   for (int64_t n = 0; n < q.nsteps; n += q.T) {
     const int Tr = (int)(q.nsteps - n < q.T ? q.nsteps - n : q.T);
-    if (active) warp_round<PML, R, C>(E, H, J, cf, p, sx, ws, src, p.n0 + n, Tr);
+    if (active) {
+      if constexpr (LEAN) {
+        if (warp_uniform) warp_round_lean<R, C>(E, H, J, cu, p, sx, ws, src, p.n0 + n, Tr);
+        else warp_round_lean<R, C>(E, H, J, cs, p, sx, ws, src, p.n0 + n, Tr);
+      } else {
+        warp_round<PML, R, C>(E, H, J, cf_regs, p, sx, ws, src, p.n0 + n, Tr);
+      }
+    }
     if (n + Tr >= q.nsteps) break;
     // halo refresh: double-buffered by round parity, so one barrier per round is enough (a warp can overwrite buffer
     // `par` again only after the NEXT barrier, which every reader of this round's data has passed its reads to reach)
@@ -170,8 +205,9 @@ static int tiles_for(int64_t rows, int RO) { return (int)((rows + RO - 1) / RO);
 // fewer warp tiles in the whole batch than four per SM: latency, not throughput, decides
 bool k3w_few_grids(const Layout &L, int sms) { return L.nbatch * ((L.nrows + 29) / 30) < (int64_t)sms * 4; }
 
-bool k3w_plan(const Layout &L, int depth, int sms, int64_t want_nw, int64_t want_nc, int64_t want_k, K3WPlan *out) {
+bool k3w_plan(const Layout &L, int depth, int sms, int64_t want_nw, int64_t want_nc, int64_t want_k, bool lean, K3WPlan *out) {
   K3WPlan P;
+  P.lean = lean;
   // default depth: one halo row (8 steps per round in fp64, 16 in fp32) when many grids keep the SMs busy; two halo
   // rows when a few grids are a chain of dependent rounds, where halving the number of barriers pays for the wider
   // halo (config 1: 1.55 against 1.76 ms)
@@ -183,7 +219,7 @@ bool k3w_plan(const Layout &L, int depth, int sms, int64_t want_nw, int64_t want
   // 8 warps per CTA: the feature variants of the time loop need up to 242 registers, and a scheduler's 16 K registers
   // then hold two warps (12 warps would need <= 168 and spill); 4 warps per SM already saturate the FP64 pipe with this
   // instruction mix (profiles/r02_peaks.md).  16 = largest (non-portable) cluster.
-  const int maxw = 8, maxc = 16;
+  const int maxw = lean ? 12 : 8, maxc = 16;       // (the lean instantiation: 168 registers, three warps per scheduler)
   if (L.nrows > (int64_t)maxw * maxc * P.rows_out) return false;
   const int w1 = tiles_for(L.nrows, P.rows_out);       // tiles of one grid
   int k = 1, nc = 1, nw = w1;
@@ -212,7 +248,8 @@ bool k3w_plan(const Layout &L, int depth, int sms, int64_t want_nw, int64_t want
         const int n = (w + c - 1) / c;
         if (n > maxw) break;
         if (c > 1 && w <= (c - 1) * maxw) continue;          // fits a smaller cluster
-        const double score = (double)(kk * L.nrows) / (32.0 * n * c) * ((double)n / (4.0 * ((n + 3) / 4))) * (c > 1 ? 0.97 : 1.0);
+        const int cap = lean ? 12 : 8;                        // warps an SM holds at this kernel's register count
+        const double score = (double)(kk * L.nrows) / (32.0 * n * c) * ((double)((cap / n) * n) / cap) * (c > 1 ? 0.97 : 1.0);
         if (score > best + 1e-9) { best = score; k = kk; nc = c; nw = n; }
       }
     if (best < 0.0) {                                    // a grid needs more than 4 SMs: warps spread evenly over a cluster
@@ -226,15 +263,19 @@ bool k3w_plan(const Layout &L, int depth, int sms, int64_t want_nw, int64_t want
   if (P.chunk_rows > 0x7fffff00LL) return false;
   P.tiles_per_chunk = tiles_for(P.chunk_rows, P.rows_out);
   P.nchunks = (L.nbatch + k - 1) / k;
-  P.smem_bytes = 2u * (uint32_t)nw * slot_bytes_per_warp();
+  P.smem_bytes = 2u * (uint32_t)nw * slot_bytes_per_warp() + (lean ? 1024u + (uint32_t)nw * kNumCoef * 32u * kRowBytes : 0u);
   *out = P;
   return true;
 }
 
-template <typename R, bool CLUSTER, bool PML>
+template <typename R, bool CLUSTER, bool PML, bool LEAN>
 static cudaError_t launch_k3w_k(const Layout &L, const K3WPlan &P, FieldPtrs f, void *const coef[kNumCoef], const StepCommon &sc,
                                 int64_t nsteps, cudaStream_t st) {
-  auto kern = k3_wtile<R, CLUSTER, PML>;
+  auto kern = k3_wtile<R, CLUSTER, PML, LEAN>;
+  if (P.smem_bytes > 48 * 1024) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P.smem_bytes);
+    if (e != cudaSuccess) return e;
+  }
   K3WArgs q;
   q.T = P.T; q.HR = P.HR; q.rows_out = P.rows_out; q.cluster = P.nc; q.chunk_rows = (int)P.chunk_rows;
   q.tiles_per_chunk = P.tiles_per_chunk; q.nrows = L.nrows; q.total_rows = L.nrows * L.nbatch; q.nsteps = nsteps;
@@ -259,8 +300,10 @@ template <typename R>
 static cudaError_t launch_k3w_t(const Layout &L, const K3WPlan &P, FieldPtrs f, void *const coef[kNumCoef], const StepCommon &sc,
                                 int64_t nsteps, cudaStream_t st) {
   const bool pml = sc.npml > 0;
-  if (P.nc > 1) return pml ? launch_k3w_k<R, true, true>(L, P, f, coef, sc, nsteps, st) : launch_k3w_k<R, true, false>(L, P, f, coef, sc, nsteps, st);
-  return pml ? launch_k3w_k<R, false, true>(L, P, f, coef, sc, nsteps, st) : launch_k3w_k<R, false, false>(L, P, f, coef, sc, nsteps, st);
+  if (P.lean && !pml)
+    return P.nc > 1 ? launch_k3w_k<R, true, false, true>(L, P, f, coef, sc, nsteps, st) : launch_k3w_k<R, false, false, true>(L, P, f, coef, sc, nsteps, st);
+  if (P.nc > 1) return pml ? launch_k3w_k<R, true, true, false>(L, P, f, coef, sc, nsteps, st) : launch_k3w_k<R, true, false, false>(L, P, f, coef, sc, nsteps, st);
+  return pml ? launch_k3w_k<R, false, true, false>(L, P, f, coef, sc, nsteps, st) : launch_k3w_k<R, false, false, false>(L, P, f, coef, sc, nsteps, st);
 }
 cudaError_t launch_k3w(int dtype, const Layout &L, const K3WPlan &P, FieldPtrs f, void *const coef[kNumCoefArrays], const StepCommon &sc,
                        int64_t nsteps, cudaStream_t st) {
@@ -270,7 +313,7 @@ cudaError_t launch_k3w(int dtype, const Layout &L, const K3WPlan &P, FieldPtrs f
 // can a cluster of P.nc CTAs of this kernel be co-scheduled at all on this device?
 template <typename R>
 static cudaError_t k3w_max_clusters_t(const K3WPlan &P, int *nclusters) {
-  auto kern = k3_wtile<R, true, false>;
+  auto kern = P.lean ? k3_wtile<R, true, false, true> : k3_wtile<R, true, false, false>;
   if (P.nc > 8) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
     if (e != cudaSuccess) return e;

@@ -129,6 +129,118 @@ __device__ __forceinline__ void warp_round(R (&E)[C], R (&H)[C], R (&G)[C], cons
 #undef RKETD_ROUND_CASE
 }
 
+// ---- the lean warp tile of the resident kernel: E advanced IN PLACE (no second E buffer) and the coefficients taken
+// from a source CF instead of 4 C registers per lane — four registers when the lane's nodes all carry one coefficient
+// set (piecewise-constant media: every lane that does not straddle an interface; CoefUniform), the warp's own swizzled
+// shared-memory rows otherwise (CoefWarpSmem).  About 100 registers instead of 232: three to four chunks share an SM
+// and fill each other's barrier waits.  Same operations per node, same order of the special nodes, same bits.
+template <typename R, int C>
+struct CoefWarpSmem {
+  static constexpr int V = 16 / sizeof(R);
+  uint32_t base;              // shared address of this lane's row in array 0: warp area + swizzle applied per chunk
+  int lane;
+  template <int a>
+  __device__ __forceinline__ void chunk(int j, R (&out)[V]) const {
+    typename Arith<R>::Vec v;
+    lds128(base + a * (32 * kRowBytes) + swz_off(lane, j), v);
+    vec_unpack(v, out);
+  }
+};
+
+// One step, in place.  Ascending node order: E'[i] needs the old E[i] only (through t and the current update), the Mur
+// candidate of node i needs the NEW E[i-1] and the OLD E[i-1], E[i] — one rolling temporary.
+template <int MASK, typename R, int C, typename CF>
+__device__ __forceinline__ void warp_step_lean(R (&E)[C], R (&H)[C], R (&G)[C], const CF &cf, R &Er, R nchh,
+                                               const StepParams<R> &p, const SpecialIdx &sx, const WarpSpecial &ws,
+                                               int64_t nloc, R src_now) {
+  typedef Arith<R> A;
+  constexpr int V = 16 / sizeof(R);
+  H[C - 1] = A::fma(nchh, A::sub(Er, E[C - 1]), H[C - 1]);                    // a1, last node first
+  const R Hl = __shfl_up_sync(0xffffffffu, H[C - 1], 1);
+#pragma unroll
+  for (int i = 0; i < C - 1; ++i) H[i] = A::fma(nchh, A::sub(E[i + 1], E[i]), H[i]);
+  const R e0 = E[0], e1 = E[1], e2 = E[2];                                    // old values Mur at node 0 needs
+  R prev_old = R(0);
+#pragma unroll
+  for (int j = 0; j < C / V; ++j) {
+    R cP[V], cch[V], cka[V], cQ[V];
+    cf.template chunk<COEF_P>(j, cP); cf.template chunk<COEF_CH>(j, cch);
+    cf.template chunk<COEF_KA>(j, cka); cf.template chunk<COEF_Q>(j, cQ);
+#pragma unroll
+    for (int u = 0; u < V; ++u) {
+      const int i = j * V + u;
+      const R eo = E[i];
+      const R w = A::mul(cQ[u], eo);
+      const R t = A::fma(cP[u], eo, -G[i]);
+      G[i] = A::fma(cka[u], G[i], w);                                         // a5 (old E, old G)
+      R en = A::fma(-cch[u], A::sub(H[i], i ? H[i - 1] : Hl), t);             // a2
+      if constexpr ((MASK & SF_MURR) != 0) {
+        if (i >= 1) {
+          const R cand = A::fma(p.mur_m, A::sub(E[i - 1], eo), prev_old);     // E[i-1] is already the new interior value
+          en = ((ws.mR >> i) & 1u) ? cand : en;
+        }
+        prev_old = eo;
+      }
+      E[i] = en;
+    }
+  }
+  if constexpr ((MASK & SF_MURL) != 0) {
+    const R c0 = A::fma(p.mur_m, A::sub(E[1], e0), e1);
+    const R c1 = A::fma(p.mur_m, A::sub(E[2], e1), e2);
+    E[0] = ws.mL0 ? c0 : E[0];
+    E[1] = ws.mL1 ? c1 : E[1];
+  }
+  if constexpr ((MASK & SF_SRC) != 0) {
+#pragma unroll
+    for (int i = 0; i < C; ++i) {
+      const R sum = A::add(E[i], src_now);
+      E[i] = ((ws.mS >> i) & 1u) ? sum : E[i];
+    }
+  }
+  if constexpr ((MASK & SF_PROBE) != 0) {
+    const R v0 = select_node<R, C>(E, sx.pi0), v1 = select_node<R, C>(E, sx.pi1);
+    stg_if(ws.l_p0, p.rec + (sx.pr0 + nloc), v0);
+    stg_if(ws.l_p1, p.rec + (sx.pr1 + nloc), v1);
+  }
+  Er = __shfl_down_sync(0xffffffffu, E[0], 1);
+}
+
+template <int MASK, typename R, int C, typename CF>
+__device__ __forceinline__ void warp_steps_lean(R (&E)[C], R (&H)[C], R (&G)[C], const CF &cf, const StepParams<R> &p,
+                                                const SpecialIdx &sx, const WarpSpecial &ws, SourceStream<R> &src,
+                                                int64_t nloc, int nsteps) {
+  const R nchh = p.nchh;
+  const int lane = threadIdx.x & 31;
+  R Er = __shfl_down_sync(0xffffffffu, E[0], 1);
+  int left = nsteps;
+  for (; left >= 2; left -= 2) {
+    R s0 = R(0), s1 = R(0);
+    if constexpr ((MASK & SF_SRC) != 0) src.sample2(p, nloc, lane, s0, s1);
+    warp_step_lean<MASK, R, C>(E, H, G, cf, Er, nchh, p, sx, ws, nloc, s0);
+    warp_step_lean<MASK, R, C>(E, H, G, cf, Er, nchh, p, sx, ws, nloc + 1, s1);
+    nloc += 2;
+  }
+  if (left) {
+    const R s0 = (MASK & SF_SRC) != 0 ? src.sample(p, nloc, lane) : R(0);
+    warp_step_lean<MASK, R, C>(E, H, G, cf, Er, nchh, p, sx, ws, nloc, s0);
+  }
+  if constexpr (MASK != 0) zero_padding_H<R, C>(H, ws);
+}
+
+template <typename R, int C, typename CF>
+__device__ __forceinline__ void warp_round_lean(R (&E)[C], R (&H)[C], R (&G)[C], const CF &cf, const StepParams<R> &p,
+                                                const SpecialIdx &sx, const WarpSpecial &ws, SourceStream<R> &src,
+                                                int64_t nloc, int nsteps) {
+#define RKETD_LEAN_CASE(M) case M: warp_steps_lean<M, R, C>(E, H, G, cf, p, sx, ws, src, nloc, nsteps); break;
+  switch (ws.mask) {
+    RKETD_LEAN_CASE(0) RKETD_LEAN_CASE(1) RKETD_LEAN_CASE(2) RKETD_LEAN_CASE(3) RKETD_LEAN_CASE(4) RKETD_LEAN_CASE(5)
+    RKETD_LEAN_CASE(6) RKETD_LEAN_CASE(7) RKETD_LEAN_CASE(8) RKETD_LEAN_CASE(9) RKETD_LEAN_CASE(10) RKETD_LEAN_CASE(11)
+    RKETD_LEAN_CASE(12) RKETD_LEAN_CASE(13) RKETD_LEAN_CASE(14) RKETD_LEAN_CASE(15)
+    default: break;
+  }
+#undef RKETD_LEAN_CASE
+}
+
 // ---- host side
 template <typename R>
 inline StepParams<R> make_params(const StepCommon &sc) {
