@@ -137,6 +137,8 @@ int rketd_discard_records(rketd_sim *s);
  * EINVAL if the choice cannot run this grid (e.g. RESIDENT with a grid larger than a cluster can hold). */
 #define RKETD_RESIDENT_WTILE_FLAG 0x40000000
 #define RKETD_RESIDENT_WTILE_NOLEAN 0x20000000 /* or-ed in: the 232-register instantiation (coefficients in registers) */
+#define RKETD_RESIDENT_WTILE_LEAN 0x10000000   /* or-ed in: the 168-register instantiation (E in place, coefficients from four
+                                                  registers or shared memory); default for many grids */
 #define RKETD_RESIDENT_WTILE(nw, nc, k) (RKETD_RESIDENT_WTILE_FLAG | ((k) << 16) | ((nc) << 8) | (nw))
 int rketd_set_plan(rketd_sim *s, int kernel, int depth, int variant);
 

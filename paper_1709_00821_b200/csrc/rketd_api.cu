@@ -277,7 +277,10 @@ bool resident_wtile_plan(rketd_sim *s, int depth, int variant, K3WPlan *P) {
   int64_t nw = 0, nc = 0, k = 0;
   if (variant >= 0) { nw = variant & 0xff; nc = (variant >> 8) & 0xff; k = (variant >> 16) & 0xfff; }
   // the lean instantiation (<= 128 registers) serves Mur ends with at most two probes among the nodes of one lane
-  bool lean = s->bc_npml == 0 && s->pml.npml == 0 && !(variant >= 0 && (variant & RKETD_RESIDENT_WTILE_NOLEAN));
+  // (measured: +26 % on config 3, +55 % on config 5 when many chunks share the SMs; 12 % slower on config 1, where one chunk is
+  // a chain of dependent steps and the in-place update lengthens it — so: many grids only, unless the variant says otherwise)
+  const bool ask_lean = variant >= 0 && (variant & RKETD_RESIDENT_WTILE_LEAN), ask_fat = variant >= 0 && (variant & RKETD_RESIDENT_WTILE_NOLEAN);
+  bool lean = s->bc_npml == 0 && s->pml.npml == 0 && !ask_fat && (ask_lean || !k3w_few_grids(s->L, s->sms));
   if (lean) {
     std::vector<int64_t> rows;
     for (int64_t c : s->probes) rows.push_back((s->L.off + c) / s->L.C);

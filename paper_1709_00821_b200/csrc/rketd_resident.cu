@@ -314,6 +314,10 @@ cudaError_t launch_k3w(int dtype, const Layout &L, const K3WPlan &P, FieldPtrs f
 template <typename R>
 static cudaError_t k3w_max_clusters_t(const K3WPlan &P, int *nclusters) {
   auto kern = P.lean ? k3_wtile<R, true, false, true> : k3_wtile<R, true, false, false>;
+  if (P.smem_bytes > 48 * 1024) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P.smem_bytes);
+    if (e != cudaSuccess) return e;
+  }
   if (P.nc > 8) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
     if (e != cudaSuccess) return e;

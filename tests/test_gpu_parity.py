@@ -70,10 +70,14 @@ def WT(nw=0, nc=0, k=0):
     return 0x40000000 | (k << 16) | (nc << 8) | nw
 
 
+LEAN, NOLEAN = 0x10000000, 0x20000000      # the 168- / 232-register instantiation of k3_wtile (default: by batch size)
+
+
 # K1; the resident kernel K3: warp tiles with the library's packing at several depths (steps between halo refreshes),
 # explicit packings (one CTA, clusters of 2..9 CTAs over DSMEM), the older one-barrier-per-step kernel; K2 variants
 ALL_PLANS = [(1, 0, -1)] + [(3, d, -1) for d in (0, 1, 3, 8, 13, 16)] + \
             [(3, 8, WT(8, 2)), (3, 8, WT(5, 2)), (3, 8, WT(1, 9)), (3, 5, WT(2, 5)), (3, 16, WT(4, 3)), (3, 0, WT(3, 3))] + \
+            [(3, 8, WT(8, 2) | LEAN), (3, 7, WT(9, 1) | LEAN), (3, 16, WT(2, 5) | LEAN), (3, 0, WT(3, 3) | LEAN), (3, 0, WT(5, 2) | NOLEAN)] + \
             [(3, 0, 0), (3, 0, 2)] + [(2, 0, v) for v in (0, 2, 6)] + [(2, d, 0) for d in (1, 7, 16, 33)] + \
             [(2, d, 6) for d in (1, 2, 9, 32, 40)] + [(2, 5, 0), (2, 40, 2)]
 
@@ -237,7 +241,8 @@ def test_config3_reduced(rk, dtype):
     check_fields(g, ref["state"], TOL[dtype], *floors_of(w, ref))
     # the same batch through temporal blocking, the one-barrier-per-step resident kernel, and other packings of the
     # warp-tile kernel: 2 grids per chunk on a cluster of 3 CTAs, one grid on 4 CTAs, deeper rounds
-    for plan in [(2, 16, 0), (3, 0, 0), (3, 0, WT(8, 5, 2)), (3, 0, WT(0, 4, 1)), (3, 16, -1), (3, 5, WT(0, 3, 1))]:
+    for plan in [(2, 16, 0), (3, 0, 0), (3, 0, WT(8, 5, 2)), (3, 0, WT(0, 4, 1)), (3, 16, -1), (3, 5, WT(0, 3, 1)),
+                 (3, 8, WT(12, 3, 2) | LEAN), (3, 0, WT(0, 2, 1) | LEAN), (3, 9, WT(0, 4, 1) | LEAN)]:
         g2 = run_gpu(rk, w, dtype, *plan)
         assert np.array_equal(g["rec"], g2["rec"]) and np.array_equal(g["J"], g2["J"]), plan
 
@@ -272,7 +277,8 @@ def test_config5_reduced_dft(rk, dtype):
     # 48 grids: chunks of 1, 2, 3, 4, 5 and 7 whole grids (7 does not divide 48: a ragged last chunk), clusters, and the
     # one-barrier-per-step kernel
     for depth, variant in [(0, -1), (0, WT(0, 1, 1)), (0, WT(0, 2, 2)), (0, WT(0, 2, 3)), (0, WT(0, 3, 4)), (0, WT(0, 3, 5)),
-                           (0, WT(0, 4, 7)), (3, WT(0, 2, 2)), (0, 0), (0, 2)]:
+                           (0, WT(0, 4, 7)), (3, WT(0, 2, 2)), (0, 0), (0, 2),
+                           (0, WT(0, 1, 1) | LEAN), (0, WT(0, 1, 2) | LEAN), (5, WT(0, 2, 5) | LEAN), (0, WT(0, 1, 1) | NOLEAN)]:
         g = run_gpu(rk, w2, dtype, 3, depth, variant)
         assert grid_err(g["rec"], ref2["rec"]) <= TOL[dtype], (depth, variant)
         check_fields(g, ref2["state"], TOL[dtype], *floors_of(w2, ref2))
@@ -302,7 +308,8 @@ def test_small_and_ragged_grids(rk, ncells):
         outs = []
         plans = [(1, 0, -1), (0, 0, -1), (2, 7, 0), (2, 7, 6), (2, 3, 2), (3, 0, -1), (3, 5, -1), (3, 0, WT(0, 0, 2)), (3, 0, WT(0, 0, 3))]
         if ncells > 300:
-            plans += [(3, 0, WT(0, 3, 1)), (3, 0, WT(2, 0, 1)), (3, 2, WT(0, 0, 3))]
+            plans += [(3, 0, WT(0, 3, 1)), (3, 0, WT(2, 0, 1)), (3, 2, WT(0, 0, 3)), (3, 0, WT(0, 0, 3) | LEAN)]
+        plans += [(3, 0, WT(0, 0, 1) | LEAN), (3, 3, WT(0, 0, 2) | LEAN)]
         for kernel, depth, variant in plans:
             s = rk.Sim(ncells, nb, wl.DZ, wl.DT, "f64")
             s.set_media(wp, nu)
