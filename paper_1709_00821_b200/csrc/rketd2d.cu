@@ -232,7 +232,18 @@ __device__ __forceinline__ void ld_pair(const float *q, float &x, float &y) { co
 __device__ __forceinline__ void st_pair(double *q, double x, double y) { *reinterpret_cast<double2 *>(q) = make_double2(x, y); }
 __device__ __forceinline__ void st_pair(float *q, float x, float y) { *reinterpret_cast<float2 *>(q) = make_float2(x, y); }
 
-constexpr int kRing = kPF + 1;      // entry ring: rows Y .. Y+kPF, 8 arrays each (Ez, Hx, Hy, G, P, ce, ka, Q)
+// Rows of the eight input arrays arrive as 2-D tiled TMA boxes {strip columns, 1 row} (cp.async.bulk.tensor.2d, SASS UTMALDG):
+// one elected thread issues them, completion on the ring slot's mbarrier; columns and rows outside the grid are zero-filled
+// by the hardware (the tensor map's extent is nx x ny), which is what the strip halo at the grid's edges needs.
+struct Maps2D { CUtensorMap m[8]; };      // Ez, Hx, Hy, G of the source buffer, then P, ce, ka, Q
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const void *tmap, uint64_t *bar, int c0, int c1) {
+  asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+               ::"r"(dst), "l"(tmap), "r"(rketd::smem_u32(bar)), "r"(c0), "r"(c1) : "memory");
+}
+template <int NT> struct TmaBox { static constexpr int W = NT <= 256 ? NT : NT / 2, N = NT / W; };   // box width <= 256 elements
+
+constexpr int kRing = kPF + 1;      // entry ring, 8 arrays per row (Ez, Hx, Hy, G, P, ce, ka, Q): one slot more than the rows in
+                                    // flight, so that a slot is refilled two iterations after it was read (a barrier lies between)
 template <typename R, int T>
 struct K2Shape {
   static constexpr int NT = StripThreads<R, T>::value;
@@ -392,13 +403,14 @@ __device__ __forceinline__ void run_stages(const P2<R> &p, const Arrays<R> &a, c
 // shuffle; between warps old E and old Hy of the warp-edge columns are posted to shared memory at the end of an
 // iteration (one CTA barrier per row).
 template <typename R, int T>
-__global__ void __launch_bounds__(StripThreads<R, T>::value, 1) k2_2d(const P2<R> p, const Arrays<R> a) {
+__global__ void __launch_bounds__(StripThreads<R, T>::value, 1) k2_2d(const P2<R> p, const Arrays<R> a, const __grid_constant__ Maps2D maps) {
   constexpr int NT = StripThreads<R, T>::value;
   constexpr int NW = NT / 32;
   constexpr int FR = kRing;
   constexpr int XS = NW + 2;
   constexpr int XB = T * XS * 4;                              // one exchange buffer: [T][XS]{E31, Hy31, E0, -}, end slots zero
-  extern __shared__ __align__(16) uint8_t smem_raw[];
+  extern __shared__ __align__(128) uint8_t smem_raw[];
+  __shared__ __align__(8) uint64_t ring_bar[kRing];           // one mbarrier per ring slot
   R *fring = reinterpret_cast<R *>(smem_raw);                 // [FR][8][NT]
   R *xch = fring + FR * 8 * NT;                              // [2][XB]
   R *xsb = xch + 2 * XB;                                      // [T][NT]
@@ -408,7 +420,13 @@ __global__ void __launch_bounds__(StripThreads<R, T>::value, 1) k2_2d(const P2<R
   c.is_mur = (p.bc == RKETD2D_BC_MUR);
 
   for (int q = tid; q < 2 * XB; q += NT) xch[q] = R(0);
-
+  if (tid == 0) {
+#pragma unroll
+    for (int r = 0; r < FR; ++r) rketd::mbar_init(&ring_bar[r], 8);      // eight issuing lanes, one per array
+    rketd::fence_barrier_init();
+  }
+  uint32_t rows_issued = 0, rows_taken = 0;                   // running counts over all jobs of this CTA: slot = count % FR,
+                                                              // mbarrier phase parity = (count / FR) & 1
   const int njobs = p.nstrips * p.nsegs;
   for (int job = blockIdx.x; job < njobs; job += gridDim.x) {
     const int strip = job % p.nstrips, seg = job / p.nstrips;
@@ -434,23 +452,23 @@ __global__ void __launch_bounds__(StripThreads<R, T>::value, 1) k2_2d(const P2<R
 
     __syncthreads();                       // xch zeroed / the previous job is done with it
 
-    auto issue_row = [&](int ridx) {       // ridx = row index relative to ya
-      const int Y = ya + ridx;
-      const bool valid = incol && Y >= 0 && Y < p.ny && ridx < niter;
-      const int64_t idx = valid ? (int64_t)Y * p.pitch + i : 0;
-      R *fd = fring + (ridx % FR) * 8 * NT + tid;
-      cp_async_val(fd, a.E + idx, valid);
-      cp_async_val(fd + NT, a.Hx + idx, valid);
-      cp_async_val(fd + 2 * NT, a.Hy + idx, valid);
-      cp_async_val(fd + 3 * NT, a.G + idx, valid);
-      cp_async_val(fd + 4 * NT, a.cP + idx, valid);
-      cp_async_val(fd + 5 * NT, a.cce + idx, valid);
-      cp_async_val(fd + 6 * NT, a.cka + idx, valid);
-      cp_async_val(fd + 7 * NT, a.cQ + idx, valid);
-      cp_async_commit();
-    };
+    const int nrows_job = (niter + 1) & ~1;                   // rows that enter (the iteration count is rounded up to even)
+    // lane 0 of warp `arr` (arr = 0..7) brings in array `arr` of a row: eight lanes share the issue work
+    const bool issuer = c.lane == 0 && c.warp < 8;
+    auto issue_row = [&](int ridx) {       // ridx = row index relative to ya; issuing lanes only
+      if (ridx >= nrows_job) return;
+      const uint32_t slot = rows_issued % FR;
+      ++rows_issued;
+      rketd::mbar_expect_tx(&ring_bar[slot], (uint32_t)(NT * sizeof(R)));
+      const uint32_t dst = rketd::smem_u32(fring + slot * 8 * NT + c.warp * NT);
 #pragma unroll
-    for (int r = 0; r < kPF; ++r) issue_row(r);
+      for (int h = 0; h < TmaBox<NT>::N; ++h)
+        tma_load_2d(dst + (uint32_t)(h * TmaBox<NT>::W * sizeof(R)), &maps.m[c.warp], &ring_bar[slot], x0 + h * TmaBox<NT>::W, ya + ridx);
+    };
+    if (issuer) {
+#pragma unroll
+      for (int r = 0; r < kPF; ++r) issue_row(r);
+    }
 
     constexpr uint32_t kHeldMask = ((1u << T) - 1u) << 1;     // bits of the rows the T stages hold
     // flag byte of the row entering next: loaded one iteration ahead and left untouched until then (no instruction waits on the load)
@@ -458,13 +476,16 @@ __global__ void __launch_bounds__(StripThreads<R, T>::value, 1) k2_2d(const P2<R
 
     auto iteration = [&](const int it, Held<R, T> &h, Held<R, T> &n) {
       const int Y = ya + it;
-      issue_row(it + kPF);
-      cp_async_wait<kPF>();
       const bool special = ((fq << 1) & kHeldMask) != 0;       // the flag of row Y is not among the held rows yet
       fq = (fq << 1) | ((Y >= 0 && Y < p.ny) ? (raw_next & (uint32_t)RF_SPECIAL) : 0u);
       raw_next = p.rowflag[min(max(Y + 1, 0), p.ny - 1)];
-      __syncthreads();                     // the warp-edge values posted at the end of the previous iteration
-      const R *fs = fring + (it % FR) * 8 * NT + tid;
+      __syncthreads();                     // the warp-edge values posted at the end of the previous iteration; and every
+                                           // thread has read the ring slot of the previous iteration, which is refilled now
+      if (issuer) issue_row(it + kPF);
+      const uint32_t slot = rows_taken % FR;
+      rketd::mbar_wait(&ring_bar[slot], (rows_taken / FR) & 1u);
+      ++rows_taken;
+      const R *fs = fring + slot * 8 * NT + tid;
       R ein = fs[0], hxin = fs[NT], hyin = fs[2 * NT], gin = fs[3 * NT];
       R cPin = fs[4 * NT], ccein = fs[5 * NT], ckain = fs[6 * NT], cQin = fs[7 * NT];
       R *xbuf = xch + ((it + 1) & 1) * XB;                     // read buffer of this iteration
@@ -497,8 +518,7 @@ __global__ void __launch_bounds__(StripThreads<R, T>::value, 1) k2_2d(const P2<R
       iteration(it, hA, hB);
       iteration(it + 1, hB, hA);
     }
-    cp_async_wait<0>();
-    __syncthreads();
+    __syncthreads();                       // every issued row of the job has been taken (nrows_job of each)
     for (int q = tid; q < 2 * XB; q += NT) xch[q] = R(0);
   }
 }
@@ -664,6 +684,33 @@ int build_rowflags(rketd2d_sim *s) {
   return RKETD_OK;
 }
 
+typedef CUresult (*EncodeTiled2)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
+                                 const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+// 2-D views {nx, ny} (row pitch = s->pitch elements) of the eight arrays the streaming kernel reads from the current
+// buffer, box {boxw, 1}, no swizzle; out-of-range elements read as zero
+int build_maps2d(rketd2d_sim *s, int boxw, Maps2D *out) {
+  static EncodeTiled2 enc = nullptr;
+  if (!enc) {
+    void *fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess)
+      return fail2(s, RKETD_ECUDA, "cuTensorMapEncodeTiled not available from the driver");
+    enc = (EncodeTiled2)fn;
+  }
+  void *base[8] = {s->fld[s->cur][0], s->fld[s->cur][1], s->fld[s->cur][2], s->fld[s->cur][3], s->coef[0], s->coef[1], s->coef[2], s->coef[3]};
+  for (int a = 0; a < 8; ++a) {
+    cuuint64_t dims[2] = {(cuuint64_t)s->nx, (cuuint64_t)s->ny};
+    cuuint64_t strides[1] = {(cuuint64_t)s->pitch * (cuuint64_t)s->esize};
+    cuuint32_t box[2] = {(cuuint32_t)boxw, 1u}, estr[2] = {1u, 1u};
+    const CUresult r = enc(&out->m[a], s->esize == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, base[a], dims,
+                           strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) return fail2(s, RKETD_ECUDA, "cuTensorMapEncodeTiled failed: " + std::to_string((int)r));
+  }
+  return RKETD_OK;
+}
+
 // strips and segments of the streaming kernel for depth T
 Plan2 make_plan(const rketd2d_sim *s, int T, int NT) {
   Plan2 pl;
@@ -737,7 +784,9 @@ cudaError_t launch_k2_T(rketd2d_sim *s, P2<R> &p) {
     if (dev < 64) configured |= 1ull << dev;
   }
   const int grid = pl.nstrips * pl.nsegs;
-  k2_2d<R, T><<<grid, NT, smem, s->stream>>>(p, arrays_of<R>(s));
+  Maps2D maps;
+  { const int rc = build_maps2d(s, TmaBox<NT>::W, &maps); if (rc) return cudaErrorInvalidValue; }
+  k2_2d<R, T><<<grid, NT, smem, s->stream>>>(p, arrays_of<R>(s), maps);
   return cudaGetLastError();
 }
 

@@ -98,6 +98,16 @@ def test_no_cpu_fallback_without_a_device(lib_path):
 HEADER2D = os.path.join(ROOT, "include", "rketd2d.h")
 
 
+def test_2d_streaming_kernel_loads_rows_by_tma(lib_path):
+    """k2_2d takes its rows as 2-D TMA boxes: every instantiation of it has UTMALDG in its SASS (and no LDGSTS row copies)."""
+    sass = subprocess.run(["cuobjdump", "-sass", lib_path], capture_output=True, text=True, check=True).stdout
+    funcs = re.split(r"\n\s*Function : ", sass)
+    k2 = [f for f in funcs if "k2_2d" in f.split("\n", 1)[0]]
+    assert len(k2) >= 10
+    for f in k2:
+        assert "UTMALDG" in f and "LDGSTS" not in f, f.split("\n", 1)[0]
+
+
 def declared_functions_2d():
     src = re.sub(r"/\*.*?\*/", "", open(HEADER2D).read(), flags=re.S)
     return sorted(set(re.findall(r"\b(rketd2d_[a-z_]+)\s*\(", src)))
