@@ -179,6 +179,25 @@ def alu_source(a) -> str:
             f"{FP_INSTR_PER_CELL_STEP} instr per cell-step; recorded run: profiles/r02_peaks.md")
 
 
+def _time_oracle(oracle, w, nsteps, omp, b0=0, b1=None, cells=None):
+    """seconds of oracle.run alone (its coefficient setup S0 included — it is part of the call) on a window / subset of
+    the workload: the inputs are generated and the library is loaded BEFORE the clock starts"""
+    b1 = w.nbatch if b1 is None else b1
+    lo, hi = (0, w.ncells) if cells is None else cells
+    wp, nu = w.media(lo, hi, b0, b1)
+    st = oracle.State(hi - lo, b1 - b0, w.initial_E(lo, hi, b0, b1))
+    probes = [int(p) - lo for p in w.probes if lo <= p < hi]
+    in_src = lo <= w.src_cell < hi
+    dft = None
+    if w.dft_freqs is not None:
+        dft = (np.zeros((b1 - b0, len(probes), len(w.dft_freqs))), np.zeros((b1 - b0, len(probes), len(w.dft_freqs))))
+    oracle.run(oracle.State(8, 1), np.zeros((1, 8)), np.zeros((1, 8)), w.dz, w.dt, 1, omp=omp)      # loads the library
+    t0 = time.perf_counter()
+    oracle.run(st, wp, nu, w.dz, w.dt, nsteps, src_kind=w.src_kind if in_src else oracle.SRC_NONE, src_params=w.src_params,
+               src_cell=w.src_cell - lo if in_src else 0, probes=probes, freqs=w.dft_freqs, dft=dft, omp=omp)
+    return time.perf_counter() - t0
+
+
 def cpu_baseline(w, target_updates_serial=6e8, target_updates_omp=2.5e9):
     """The oracle as it stands (S0 coefficient setup included — it is part of oracle_run), serial and
     OpenMP builds, on a prefix / subset of the same workload."""
@@ -201,9 +220,7 @@ def cpu_baseline(w, target_updates_serial=6e8, target_updates_omp=2.5e9):
             kw = dict(b0=0, b1=nb)
             sample = f"grids 0..{nb - 1} of {w.nbatch} x {w.ncells} nodes x {steps} steps"
             units = nb * w.ncells * steps
-        t0 = time.perf_counter()
-        oracle.run_workload(w, nsteps=steps, omp=omp, **kw)
-        dt = time.perf_counter() - t0
+        dt = _time_oracle(oracle, w, steps, omp, **kw)
         out["omp" if omp else "serial"] = (units / dt / 1e9, sample, dt)
     return {"value": out["omp"][0], "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": out["omp"][1] + f" (OpenMP build, {cores} threads, {out['omp'][2]:.1f} s)",
@@ -699,6 +716,57 @@ def extra_configs(rketd, stream, host_inputs):
             torch.cuda.empty_cache()
         except Exception as ex:          # an extra figure must never cost the headline
             out[key] = {"error": repr(ex)[:200]}
+    host_inputs.clear()
+    out.update(extra_2d(stream))
+    return out
+
+
+def extra_2d(stream):
+    """the 2-D workloads in the same line: 16384 x 16384 cells x 200 steps, fp64, TMz through the
+    streaming kernel k2_2d and TEz through k1_te; 1 warm-up + 2 timed runs, CUDA events, inputs resident in HBM"""
+    import torch
+    from paper_1709_00821_b200 import rketd2d, workloads as wl
+    out = {}
+    try:
+        w = wl.tm2d_column(nsteps=200)
+        wp, nu = w.media()
+        E0 = np.ascontiguousarray(w.initial_E())
+        hbm_gbs, peak_src, _ = measured_peaks()
+        for key in ("tm2d/f64", "te2d/f64"):
+            te = key.startswith("te")
+            sim = (rketd2d.Sim2DTE if te else rketd2d.Sim2D)(w.nx, w.ny, w.dx, w.dy, w.dt, "f64", stream=stream.cuda_stream)
+            wp_d, nu_d = torch.from_numpy(wp).cuda(), torch.from_numpy(nu).cuda()
+            sim.set_media(wp_d, nu_d)
+            del wp_d, nu_d
+            E0_d = torch.from_numpy(E0).cuda()
+            if te:
+                sim.set_fields(Ey=E0_d)
+                sim.set_source(w.src_kind, w.src_params, w.src_ij[0], w.src_ij[1], w.src_comp)
+            else:
+                sim.set_fields(Ez=E0_d)
+                sim.set_source(w.src_kind, w.src_params, *w.src_ij)
+            del E0_d
+            torch.cuda.empty_cache()
+            sim.run(w.nsteps)
+            torch.cuda.synchronize()
+            l0 = sim.counter(rketd2d.CTR_STEP_LAUNCHES)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            for _ in range(2):
+                sim.run(w.nsteps)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1)
+            launches = sim.counter(rketd2d.CTR_STEP_LAUNCHES) - l0
+            arrays = ARRAYS_PER_PASS_TE if te else ARRAYS_PER_PASS_2D
+            achieved = arrays * 8 * w.nx * w.ny / (ms / launches * 1e-3) / 1e9
+            out[key] = {"workload": w.name + ("_TEz" if te else ""), "dtype": "f64", "value": 2 * w.cell_updates / (ms * 1e-3) / 1e9, "unit": UNIT,
+                        "ms_per_step": ms / 2, "steps": 2, "kernel": "k1_te" if te else "k2_2d", "depth_T": 1 if te else int(sim.counter(rketd2d.CTR_DEPTH_USED)),
+                        "roofline": {"bound": "hbm", "achieved": achieved, "peak": hbm_gbs, "unit": "GB/s", "frac": achieved / hbm_gbs, "peak_source": peak_src}}
+            sim.close()
+            torch.cuda.empty_cache()
+    except Exception as ex:
+        out["2d"] = {"error": repr(ex)[:200]}
     return out
 
 
