@@ -359,9 +359,9 @@ def run_table2(args):
 FP_INSTR_PER_CELL_STEP_2D = 13   # rketd2d.cu: Hx 2, Hy 2, Ez 7 (gain 1, rest 5, fma 1), G 2
 ARRAYS_PER_PASS_2D = 12          # read Ez, Hx, Hy, G, P, ce, ka, Q; write Ez, Hx, Hy, G
 NCU_TRAFFIC_BYTES_2D = {         # (workload, dtype, depth) -> dram bytes per launch from the committed ncu captures
-    ("tm2d_column_16384x16384", "f64", 8): 26.04e9,     # profiles/r01_ncu_full_k2_2d_f64.md (streaming kernel)
+    ("tm2d_column_16384x16384", "f64", 8): 26.12e9,     # profiles/r02_ncu_2d.md (streaming kernel, rows by TMA)
     ("tm2d_column_16384x16384", "f64", 1): 25.79e9,     # same file, one-step kernel k1_2d
-    ("tm2d_column_16384x16384", "f32", 8): 12.99e9,     # profiles/r01_ncu_full_k2_2d_f32.md
+    ("tm2d_column_16384x16384", "f32", 8): 13.05e9,     # profiles/r02_ncu_2d.md
 }
 
 
@@ -576,7 +576,8 @@ def run_te2d(args):
     hbm_gbs, peak_src, _ = measured_peaks()
     alg = ARRAYS_PER_PASS_TE * esize * w.nx * w.ny
     achieved = alg / (ms / launches * 1e-3) / 1e9
-    roof = {"bound": "hbm", "achieved": achieved, "peak": hbm_gbs, "unit": "GB/s", "frac": achieved / hbm_gbs, "traffic": None,
+    traffic = 31.13e9 if (w.nx, w.ny, args.dtype) == (16384, 16384, "f64") else None      # profiles/r02_ncu_2d.md (k1_te)
+    roof = {"bound": "hbm", "achieved": achieved, "peak": hbm_gbs, "unit": "GB/s", "frac": achieved / hbm_gbs, "traffic": traffic,
             "peak_source": peak_src, "algorithmic_bytes_per_launch": alg, "ms_per_launch": ms / launches, "depth_T": 1,
             "note": "achieved = 14 arrays (read Ex,Ey,Hz,Gx,Gy,P,ce,ka,Q; write Ex,Ey,Hz,Gx,Gy) x cells x esize per step / mean launch time"}
     e2e = None
