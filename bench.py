@@ -14,8 +14,10 @@ so every launch streams from HBM ("inputs larger than L2").
 
   value     whole-job Gcell/s with inputs resident in HBM; CUDA events on the library's stream,
             barrier + synchronize on both sides, max over ranks.
-  e2e       the same job through the C ABI with HOST buffers: set_media (wp, nu), set_fields (E0)
-            from pinned host memory, rketd_run, read_probes to pinned host memory — all timed.
+  e2e       the same job through the C ABI with HOST buffers: media (wp, nu) and E0 from pinned host
+            memory, the run, read_probes to pinned host memory — all timed.  value = the one-call job
+            rketd_run_from_host (copies of later pieces of the line overlap the steps of earlier ones);
+            sequence_of_calls = rketd_set_media + rketd_set_fields + rketd_run, the same bits.
   roofline  dominant kernel (K2 temporal blocking): algorithmic bytes per launch (10 arrays x N nodes:
             read E,H,G + four coefficients P,ch,ka,Q, write E,H,G — 80 B per node and pass in fp64; the
             plain six-coefficient form of SURVEY §8(d) would be 96 B) / average launch duration, against
@@ -889,25 +891,39 @@ def main():
         h2d = wp_h.numel() * 8 + nu_h.numel() * 8 + (0 if E0_h is None else E0_h.numel() * esize)
         d2h = out_h.numel() * esize
 
-        def e2e_step():
+        def e2e_sequence():
             sim.reset()
             sim.set_media(wp_h, nu_h)
             sim.set_fields(E=E0_h)
             sim.run(w.nsteps)
             sim.read_probes(out_h)
 
-        e2e_step()
-        barrier()
-        t0 = time.perf_counter()
+        def e2e_one_call():                  # the same job; for one long line the copies overlap the steps
+            sim.run_from_host(wp_h, nu_h, E0_h, w.nsteps)
+            sim.read_probes(out_h)
+
         nrep = max(1, min(args.steps, 3))
-        for _ in range(nrep):
-            e2e_step()
-        barrier()
-        dt = time.perf_counter() - t0
-        dt = max_over_ranks(dt, world)
+
+        def wall(fn):
+            fn()
+            barrier()
+            t0 = time.perf_counter()
+            for _ in range(nrep):
+                fn()
+            barrier()
+            return max_over_ranks(time.perf_counter() - t0, world)
+
+        dt_seq = wall(e2e_sequence)
+        rec_seq = out_h.clone()
+        dt = wall(e2e_one_call) if w.nbatch == 1 else dt_seq
+        if w.nbatch == 1 and not torch.equal(out_h, rec_seq):
+            raise SystemExit("bench.py: rketd_run_from_host and the sequence of calls disagree")
         e2e = {"value": whole_job_gcells(world, units_per_step, nrep, dt), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
-               "d2h_bytes_per_step": int(d2h), "steps": nrep,
-               "note": "set_media(wp, nu) + set_fields(E0) from pinned host, rketd_run, read_probes to pinned host"}
+               "d2h_bytes_per_step": int(d2h), "steps": nrep, "pieces": int(sim.counter(rketd.CTR_PIECES)) if w.nbatch == 1 else 0,
+               "sequence_of_calls": whole_job_gcells(world, units_per_step, nrep, dt_seq),
+               "note": "inputs in pinned host memory, probe records read back to pinned host memory; value: rketd_run_from_host "
+                       "(one call; a single long line is staged in pieces whose copies overlap the steps), sequence_of_calls: "
+                       "rketd_reset + rketd_set_media + rketd_set_fields + rketd_run"}
         del wp_h, nu_h, E0_h, out_h
     sim.close()
 

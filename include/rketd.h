@@ -60,7 +60,8 @@ enum {
   RKETD_CTR_STEPS_DONE = 4,    /* global step counter                                               */
   RKETD_CTR_TILE_CELLS = 5,    /* cells per CTA tile, halo included, of the last K2/K3 run          */
   RKETD_CTR_HALO_CELLS = 6,    /* halo cells on each side of a K2 tile                              */
-  RKETD_CTR_STATE_BYTES = 7    /* device bytes held by this handle (fields + coefficients)          */
+  RKETD_CTR_STATE_BYTES = 7,   /* device bytes held by this handle (fields + coefficients)          */
+  RKETD_CTR_PIECES = 8         /* pieces the last rketd_run_from_host cut the line into (0: it ran as the plain sequence of calls) */
 };
 
 /* Create a simulation of nbatch grids of ncells nodes ("grid" of the north_star =
@@ -146,6 +147,22 @@ int rketd_set_plan(rketd_sim *s, int kernel, int depth, int variant);
  * with (11); Mur-1 at both ends; soft source; J eq. (11); probe record), asynchronously on the
  * stream.  Repeatable: time continues.  ESTATE before rketd_set_media. */
 int rketd_run(rketd_sim *s, int64_t nsteps);
+
+/* A whole job whose inputs live in HOST memory, in one call: the same result, bit for bit, as
+ *     rketd_reset(s); rketd_set_media(s, wp, nu); rketd_set_fields(s, E0, NULL, NULL); rketd_run(s, nsteps);
+ * (same steps: eq. (14), :76-:78 eqs. (11), (12)), but for one long line (nbatch = 1, temporal-blocking
+ * kernel K2, no probe DFT) the line is cut into pieces of whole tiles, the host->device copies of later pieces run on a
+ * second stream while earlier pieces step, and the K2 passes run in a time-skewed order: pass p of piece c covers the
+ * tiles [b_c - p k, b_(c+1) - p k), k = ceil(halo rows / rows a tile writes), so that every tile finds the previous
+ * level of its halo.  Other shapes run as the plain sequence above.
+ * wp, nu: [ncells] doubles, E0: [ncells] elements of the handle's dtype or NULL (E = 0); host pointers (pinned memory
+ * for the overlap; pageable and device pointers work, without overlap).  The buffers may be reused after the return:
+ * the call synchronises the handle's stream.  npieces: 0 = chosen by the library (12, of at least 8 waves of tiles
+ * each; measured flat between 8 and 16 on a 2^28-node line), > 0 = that many (tests).  Media are validated while the
+ * pieces are staged: on EINVAL (negative or non-finite wp, nu) the handle is left reset and WITHOUT media — unlike
+ * rketd_set_media the old media are gone.
+ * Step counter restarts at 0, earlier records are discarded, source, probes, boundary and plan are kept. */
+int rketd_run_from_host(rketd_sim *s, const double *wp, const double *nu, const void *E0, int64_t nsteps, int npieces);
 
 /* Synchronise and copy out the probe records (host or device `out`, handle's dtype).
  * Time-series mode: [nbatch][nprobes][nsamples], nsamples = steps run since the records were last

@@ -69,6 +69,11 @@ struct rketd_sim {
   K2Plan k2;
   bool k2_valid = false;
   int sms = 0;                   // multiprocessors of the device the handle lives on
+  // rketd_run_from_host: the copies of later pieces run on a stream of their own, one event per piece
+  cudaStream_t copy_stream = nullptr;
+  cudaEvent_t ev_ready = nullptr;
+  std::vector<cudaEvent_t> ev_piece;
+  int64_t ctr_pieces = 0;
   int64_t ctr_launches = 0, ctr_step_launches = 0, ctr_kernel_used = 0, ctr_depth_used = 0, ctr_tile_cells = 0,
           ctr_halo_cells = 0, state_bytes = 0;
   std::string err;
@@ -306,8 +311,8 @@ int resolve_kernel(rketd_sim *s) {
   return RKETD_KERNEL_RESIDENT;
 }
 
-// run nsteps steps whose probe samples go to rec ([nbatch][nprobes][nsteps] or nullptr)
-int run_segment(rketd_sim *s, int64_t nsteps, void *rec) {
+// source table and launch-wide parameters of a segment of nsteps steps that starts at s->step
+int prepare_common(rketd_sim *s, int64_t nsteps, void *rec, StepCommon &sc) {
   const Layout &L = s->L;
   // source samples of this segment: a slice of the kept table when it covers the steps, else the table is rebuilt
   const void *d_src = nullptr;
@@ -337,7 +342,6 @@ int run_segment(rketd_sim *s, int64_t nsteps, void *rec) {
     }
     d_src = (const char *)s->d_srctab + (size_t)(s->step - s->srctab_step0) * L.esize;
   }
-  StepCommon sc;
   std::memset(&sc, 0, sizeof(sc));
   sc.nchh = -(s->dt / (kMu0 * s->dz));
   const double S = kC0 * s->dt / s->dz;
@@ -350,6 +354,34 @@ int run_segment(rketd_sim *s, int64_t nsteps, void *rec) {
   sc.npml = s->pml.npml;
   std::memcpy(sc.pml_ha, s->pml_ha, sizeof(sc.pml_ha));
   std::memcpy(sc.pml_hd, s->pml_hd, sizeof(sc.pml_hd));
+  return RKETD_OK;
+}
+
+// absorbing layer requested by rketd_set_boundary: tables of the E nodes (into the coefficient arrays) and of the H nodes
+// (kernel parameters)
+void make_pml_tables(const rketd_sim *s, PmlE &new_pml, double (&new_ha)[kMaxPml], double (&new_hd)[kMaxPml]) {
+  new_pml.npml = s->bc_npml;
+  if (s->bc_npml > 0) {
+    const int np = s->bc_npml;
+    const double smax = -(s->bc_m + 1.0) * kEps0 * kC0 * std::log(s->bc_R0) / (2.0 * (double)np * s->dz);
+    const double nchh = -(s->dt / (kMu0 * s->dz));
+    for (int j = 0; j < np; ++j) {
+      const double rho_e = (double)(np - j) / (double)np, rho_h = ((double)(np - j) - 0.5) / (double)np;
+      const double se = smax * std::pow(rho_e, s->bc_m) * s->dt / (2.0 * kEps0);
+      const double sh = smax * std::pow(rho_h, s->bc_m) * s->dt / (2.0 * kEps0);
+      new_pml.a[j] = (1.0 - se) / (1.0 + se);
+      new_pml.b[j] = (s->dt / (kEps0 * s->dz)) / (1.0 + se);
+      new_ha[j] = (1.0 - sh) / (1.0 + sh);
+      new_hd[j] = nchh / (1.0 + sh) - nchh;
+    }
+  }
+}
+
+// run nsteps steps whose probe samples go to rec ([nbatch][nprobes][nsteps] or nullptr)
+int run_segment(rketd_sim *s, int64_t nsteps, void *rec) {
+  const Layout &L = s->L;
+  StepCommon sc;
+  { int rc = prepare_common(s, nsteps, rec, sc); if (rc) return rc; }
 
   const int kern = resolve_kernel(s);
   s->ctr_kernel_used = kern;
@@ -510,21 +542,7 @@ int rketd_set_media(rketd_sim *s, const double *wp, const double *nu) {
   // sigma_max = -(m+1) eps0 c ln(R0) / (2 npml dz), rho = depth / thickness, matched sigma* = sigma mu0/eps0.
   PmlE new_pml{};
   double new_ha[kMaxPml] = {}, new_hd[kMaxPml] = {};
-  new_pml.npml = s->bc_npml;
-  if (s->bc_npml > 0) {
-    const int np = s->bc_npml;
-    const double smax = -(s->bc_m + 1.0) * kEps0 * kC0 * std::log(s->bc_R0) / (2.0 * (double)np * s->dz);
-    const double nchh = -(s->dt / (kMu0 * s->dz));
-    for (int j = 0; j < np; ++j) {
-      const double rho_e = (double)(np - j) / (double)np, rho_h = ((double)(np - j) - 0.5) / (double)np;
-      const double se = smax * std::pow(rho_e, s->bc_m) * s->dt / (2.0 * kEps0);
-      const double sh = smax * std::pow(rho_h, s->bc_m) * s->dt / (2.0 * kEps0);
-      new_pml.a[j] = (1.0 - se) / (1.0 + se);
-      new_pml.b[j] = (s->dt / (kEps0 * s->dz)) / (1.0 + se);
-      new_ha[j] = (1.0 - sh) / (1.0 + sh);
-      new_hd[j] = nchh / (1.0 + sh) - nchh;
-    }
-  }
+  make_pml_tables(s, new_pml, new_ha, new_hd);
   s->have_media = false;      // until the new coefficients are in place
   SM_TRY(launch_coefficients(s->dtype, L, dwp, dnu, s->dz, s->dt, s->scheme, new_pml, s->wp_p, s->nu_p, s->coef, s->d_bad, s->stream));
   ++s->ctr_launches;
@@ -722,6 +740,141 @@ int rketd_run(rketd_sim *s, int64_t nsteps) {
   return RKETD_OK;
 }
 
+int rketd_run_from_host(rketd_sim *s, const double *wp, const double *nu, const void *E0, int64_t nsteps, int npieces) {
+  if (!s || !wp || !nu) return fail(s, RKETD_EINVAL, "rketd_run_from_host: NULL argument");
+  if (nsteps < 0 || npieces < 0) return fail(s, RKETD_EINVAL, "rketd_run_from_host: nsteps < 0 or npieces < 0");
+  const Layout &L = s->L;
+  s->ctr_pieces = 0;
+  // the time-skewed order needs one line and the temporal-blocking kernel; everything else is the plain sequence
+  if (L.nbatch != 1 || !s->freqs.empty() || nsteps == 0 || resolve_kernel(s) != RKETD_KERNEL_TBLOCK) {
+    int rc = rketd_reset(s);
+    if (!rc) rc = rketd_set_media(s, wp, nu);
+    if (!rc) rc = rketd_set_fields(s, E0, nullptr, nullptr);
+    if (!rc) rc = rketd_run(s, nsteps);
+    return rc;
+  }
+  if (!s->copy_stream) {
+    CU_TRY(s, cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking));
+    CU_TRY(s, cudaEventCreateWithFlags(&s->ev_ready, cudaEventDisableTiming));
+  }
+  int rc = rketd_reset(s);                       // E = H = G = 0 in the current buffers, records dropped, step 0
+  if (rc) return rc;
+  PmlE new_pml{};
+  double new_ha[kMaxPml] = {}, new_hd[kMaxPml] = {};
+  make_pml_tables(s, new_pml, new_ha, new_hd);
+  if (std::memcmp(&new_pml, &s->pml, sizeof(PmlE)) != 0) s->flags_dirty = true;
+  s->have_media = false;                         // until every piece has been staged and found valid
+  s->media_scheme = s->scheme;
+  s->pml = new_pml;
+  std::memcpy(s->pml_ha, new_ha, sizeof(new_ha));
+  std::memcpy(s->pml_hd, new_hd, sizeof(new_hd));
+  if (s->flags_dirty) { rc = rebuild_rowflags(s); if (rc) return rc; }
+
+  const int variant = s->plan_variant >= 0 ? s->plan_variant : default_k2_variant(s);
+  int depth = s->plan_depth > 0 ? s->plan_depth : default_depth(s);
+  depth = std::min<int>(depth, max_depth(s, variant));
+  rc = build_k2_plan(s, depth, variant);
+  if (rc) return rc;
+  const K2Plan &P = s->k2;
+
+  void *buf = nullptr;
+  size_t bytes = 0;
+  if (!s->probes.empty()) {
+    bytes = s->probes.size() * (size_t)nsteps * L.esize;
+    if (s->spare_buf && s->spare_bytes >= bytes) {
+      buf = s->spare_buf; bytes = s->spare_bytes;
+      s->spare_buf = nullptr; s->spare_bytes = 0;
+    } else {
+      CU_TRY(s, cudaMalloc(&buf, bytes));
+    }
+  }
+  auto give_back = [&]() {                       // a failed job records nothing
+    if (!buf) return;
+    cudaStreamSynchronize(s->stream);
+    if (!s->spare_buf) { s->spare_buf = buf; s->spare_bytes = bytes; } else cudaFree(buf);
+    buf = nullptr;
+  };
+#define RH_TRY(expr) do { cudaError_t rh_e = (expr); if (rh_e != cudaSuccess) { cudaStreamSynchronize(s->copy_stream); give_back(); CU_TRY(s, rh_e); } } while (0)
+  StepCommon sc;
+  rc = prepare_common(s, nsteps, buf, sc);
+  if (rc) { give_back(); return rc; }
+
+  // pieces of whole tiles; a pass moves every piece boundary k tiles to the left (the tiles right of it lack their halo)
+  const int64_t Tt = P.tiles_per_grid, k = (P.HR + P.rows_out - 1) / P.rows_out;
+  const int64_t piece_tiles = npieces > 0 ? (Tt + npieces - 1) / npieces
+                                          : std::max<int64_t>((Tt + 11) / 12, (int64_t)8 * s->sms * k2_tiles_per_cta(variant));
+  const int64_t npc = (Tt + piece_tiles - 1) / piece_tiles;
+  while ((int64_t)s->ev_piece.size() < npc) {
+    cudaEvent_t e;
+    RH_TRY(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    s->ev_piece.push_back(e);
+  }
+  const int cur0 = s->cur;
+  RH_TRY(cudaMemsetAsync(s->d_bad, 0, sizeof(int), s->stream));
+  RH_TRY(cudaEventRecord(s->ev_ready, s->stream));                     // the cleared arrays, and everything before
+  RH_TRY(cudaStreamWaitEvent(s->copy_stream, s->ev_ready, 0));
+  const int64_t node_per_tile = (int64_t)P.rows_out * L.C;
+  auto piece_nodes = [&](int64_t c, int64_t &i0, int64_t &i1) {       // physical nodes of piece c
+    i0 = c * piece_tiles * node_per_tile;
+    i1 = c == npc - 1 ? L.gstride : std::min<int64_t>(L.gstride, (c + 1) * piece_tiles * node_per_tile);
+  };
+  for (int64_t c = 0; c < npc; ++c) {
+    int64_t i0, i1;
+    piece_nodes(c, i0, i1);
+    const int64_t k0 = std::max<int64_t>(i0 - L.off, 0), k1 = std::min<int64_t>(i1 - L.off, L.ncells);
+    if (k1 > k0) {
+      const size_t n = (size_t)(k1 - k0);
+      RH_TRY(cudaMemcpyAsync(s->wp_p + L.off + k0, wp + k0, n * sizeof(double), cudaMemcpyDefault, s->copy_stream));
+      RH_TRY(cudaMemcpyAsync(s->nu_p + L.off + k0, nu + k0, n * sizeof(double), cudaMemcpyDefault, s->copy_stream));
+      if (E0)
+        RH_TRY(cudaMemcpyAsync((char *)s->fld[cur0][0] + (size_t)(L.off + k0) * L.esize, (const char *)E0 + (size_t)k0 * L.esize,
+                               n * L.esize, cudaMemcpyDefault, s->copy_stream));
+    }
+    RH_TRY(cudaEventRecord(s->ev_piece[(size_t)c], s->copy_stream));
+  }
+  const int64_t npass = (nsteps + depth - 1) / depth;
+  for (int64_t c = 0; c < npc; ++c) {
+    int64_t i0, i1;
+    piece_nodes(c, i0, i1);
+    RH_TRY(cudaStreamWaitEvent(s->stream, s->ev_piece[(size_t)c], 0));
+    RH_TRY(launch_stage_piece(s->dtype, L, i0, i1, s->dz, s->dt, s->media_scheme, s->pml, s->wp_p, s->nu_p, s->coef,
+                              s->fld[cur0][0], s->fld[cur0][2], s->d_bad, s->stream));
+    ++s->ctr_launches;
+    const int64_t b0 = c * piece_tiles, b1 = std::min<int64_t>(Tt, b0 + piece_tiles);
+    for (int64_t p = 1; p <= npass; ++p) {
+      const int64_t tb = std::max<int64_t>(0, b0 - p * k), te = c == npc - 1 ? Tt : b1 - p * k;
+      if (te <= tb) continue;
+      const int src_buf = (cur0 + (int)((p - 1) & 1)) & 1;
+      sc.n0 = (p - 1) * depth;
+      FieldPtrs dst{s->fld[1 - src_buf][0], s->fld[1 - src_buf][1], s->fld[1 - src_buf][2]};
+      RH_TRY(launch_k2(s->dtype, L, P, src_buf, dst, sc, (int)std::min<int64_t>(depth, nsteps - sc.n0), s->stream, tb, te));
+      ++s->ctr_launches; ++s->ctr_step_launches;
+    }
+  }
+  int bad = 0;
+  RH_TRY(cudaMemcpyAsync(&bad, s->d_bad, sizeof(int), cudaMemcpyDeviceToHost, s->stream));
+  RH_TRY(cudaStreamSynchronize(s->stream));
+#undef RH_TRY
+  s->ctr_kernel_used = RKETD_KERNEL_TBLOCK;
+  s->ctr_tile_cells = (int64_t)P.rows * L.C; s->ctr_halo_cells = (int64_t)P.HR * L.C; s->ctr_depth_used = depth;
+  s->ctr_pieces = npc;
+  if (bad) {                                     // the steps ran on garbage: nothing of this job is kept
+    give_back();
+    rketd_reset(s);
+    return fail(s, RKETD_EINVAL, "rketd_run_from_host: wp and nu must be finite and non-negative (the handle now has no media)");
+  }
+  s->cur = (cur0 + (int)(npass & 1)) & 1;
+  s->step = nsteps;
+  s->have_media = true;
+  s->fields_zero = false;
+  s->third_is_J = false;
+  if (buf) {
+    s->chunks.push_back(Chunk{buf, nsteps, bytes});
+    s->nsamples += nsteps;
+  }
+  return RKETD_OK;
+}
+
 int rketd_read_probes(rketd_sim *s, void *out, int64_t out_bytes, int64_t *nsamples) {
   if (!s) return RKETD_EINVAL;
   const Layout &L = s->L;
@@ -870,6 +1023,7 @@ int64_t rketd_get_counter(const rketd_sim *s, int which) {
     case RKETD_CTR_TILE_CELLS: return s->ctr_tile_cells;
     case RKETD_CTR_HALO_CELLS: return s->ctr_halo_cells;
     case RKETD_CTR_STATE_BYTES: return s->state_bytes;
+    case RKETD_CTR_PIECES: return s->ctr_pieces;
   }
   return -1;
 }
@@ -877,6 +1031,9 @@ int64_t rketd_get_counter(const rketd_sim *s, int which) {
 void rketd_destroy(rketd_sim *s) {
   if (!s) return;
   cudaStreamSynchronize(s->stream);
+  if (s->copy_stream) { cudaStreamSynchronize(s->copy_stream); cudaStreamDestroy(s->copy_stream); }
+  if (s->ev_ready) cudaEventDestroy(s->ev_ready);
+  for (cudaEvent_t e : s->ev_piece) cudaEventDestroy(e);
   for (int b = 0; b < 2; ++b)
     for (int a = 0; a < 3; ++a)
       if (s->fld[b][a]) cudaFree(s->fld[b][a]);

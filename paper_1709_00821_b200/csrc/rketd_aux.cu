@@ -86,6 +86,48 @@ cudaError_t launch_coefficients(int dtype, const Layout &L, const double *wp, co
   return cudaGetLastError();
 }
 
+// rketd_run_from_host, one piece of a single line (nbatch = 1): the physical nodes [i0, i1).  The media of the piece
+// were copied straight into wp_p / nu_p (for one grid the padded layout is the user's shifted by L.off) and E0 into E.
+// Same arithmetic as coefficients_kernel and current_to_G_kernel with J = 0, so the job is bit-identical to
+// rketd_set_media + rketd_set_fields(E0, NULL, NULL).
+template <typename R>
+__global__ void stage_piece_kernel(Layout L, int64_t i0, int64_t i1, double dz, double dt, double eps0, int scheme, PmlE pml,
+                                   double *wp_p, double *nu_p, R *cP, R *cch, R *cka, R *cQ, const R *E, R *G, int *bad) {
+  const int64_t idx = i0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= i1) return;
+  const int64_t k = idx - L.off;
+  double vP = 0, vch = 0, vka = 0, vQ = 0, vG = 0;
+  if (k >= 0 && k < L.ncells) {
+    const double w = wp_p[idx], v = nu_p[idx];
+    if (!(w >= 0.0) || !(v >= 0.0) || isinf(w) || isinf(v)) atomicOr(bad, 1);
+    const int jp = pml_index(pml, k, L.ncells);
+    const Six s = jp >= 0 ? pml_six(pml, jp) : six_coefficients(w, v, dz, dt, eps0, scheme);
+    const double kcp = __dmul_rn(s.cj, s.kc), kbp = __dmul_rn(s.cj, s.kb);
+    vP = __dsub_rn(s.ca, kcp);
+    vch = s.ch;
+    vka = s.ka;
+    vQ = __dadd_rn(__dmul_rn(s.ka, kcp), kbp);
+    if (jp < 0) vG = __fma_rn(-kcp, (double)E[idx], __dmul_rn(s.cj, 0.0));
+  } else {
+    wp_p[idx] = 0.0; nu_p[idx] = 0.0;
+  }
+  cP[idx] = (R)vP; cch[idx] = (R)vch; cka[idx] = (R)vka; cQ[idx] = (R)vQ;
+  G[idx] = (R)vG;
+}
+cudaError_t launch_stage_piece(int dtype, const Layout &L, int64_t i0, int64_t i1, double dz, double dt, int scheme, const PmlE &pml,
+                               double *wp_p, double *nu_p, void *const coef[kNumCoefArrays], const void *E, void *G, int *d_bad,
+                               cudaStream_t st) {
+  if (i1 <= i0) return cudaSuccess;
+  const unsigned blocks = (unsigned)((i1 - i0 + 255) / 256);
+  if (dtype == 0)
+    stage_piece_kernel<double><<<blocks, 256, 0, st>>>(L, i0, i1, dz, dt, kEps0, scheme, pml, wp_p, nu_p, (double *)coef[0], (double *)coef[1],
+                                                       (double *)coef[2], (double *)coef[3], (const double *)E, (double *)G, d_bad);
+  else
+    stage_piece_kernel<float><<<blocks, 256, 0, st>>>(L, i0, i1, dz, dt, kEps0, scheme, pml, wp_p, nu_p, (float *)coef[0], (float *)coef[1],
+                                                      (float *)coef[2], (float *)coef[3], (const float *)E, (float *)G, d_bad);
+  return cudaGetLastError();
+}
+
 __global__ void six_coefficients_kernel(Layout L, const double *__restrict__ wp_p, const double *__restrict__ nu_p,
                                         double dz, double dt, double eps0, int scheme, PmlE pml, double *out) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;

@@ -90,8 +90,9 @@ int k3_threads_for_rows(int dtype, int64_t nrows, int variant);   // threads per
 
 cudaError_t launch_k1(int dtype, const Layout &L, FieldPtrs src, FieldPtrs dst, void *const coef[kNumCoefArrays],
                       const StepCommon &sc, cudaStream_t st);
+// tile_end >= 0: only the tiles [tile_begin, tile_end) of the plan (rketd_run_from_host)
 cudaError_t launch_k2(int dtype, const Layout &L, const K2Plan &plan, int src_buf, FieldPtrs dst, const StepCommon &sc,
-                      int steps, cudaStream_t st);
+                      int steps, cudaStream_t st, int64_t tile_begin = 0, int64_t tile_end = -1);
 cudaError_t launch_k3(int dtype, const Layout &L, FieldPtrs fld, void *const coef[kNumCoefArrays], const StepCommon &sc,
                       int64_t nsteps, int NT, int variant, cudaStream_t st);
 cudaError_t k2_configure(int dtype, int variant, int *ctas_per_sm);   // sets smem attribute, returns occupancy
@@ -111,6 +112,9 @@ cudaError_t launch_six_coefficients(const Layout &L, const double *wp_p, const d
 cudaError_t launch_unpack_coefficients(int dtype, const Layout &L, void *const coef[kNumCoefArrays], double *out,
                                        cudaStream_t st);
 // J <-> G = cj J - cj kc E on the padded arrays (in place on the third field array)
+cudaError_t launch_stage_piece(int dtype, const Layout &L, int64_t i0, int64_t i1, double dz, double dt, int scheme, const PmlE &pml,
+                               double *wp_p, double *nu_p, void *const coef[kNumCoefArrays], const void *E, void *G, int *d_bad,
+                               cudaStream_t st);
 cudaError_t launch_current_to_G(int dtype, const Layout &L, const double *wp_p, const double *nu_p, double dz,
                                 double dt, int scheme, const PmlE &pml, const void *E, void *JG, cudaStream_t st);
 cudaError_t launch_G_to_current(int dtype, const Layout &L, const double *wp_p, const double *nu_p, double dz,

@@ -202,6 +202,7 @@ struct K2Args {
   int HR;                 // halo rows
   int rows_out;           // ROWS - 2 HR
   uint32_t tiles_per_grid, total_tiles;   // 32-bit on purpose: tile index arithmetic sits between two tiles
+  uint32_t tile_first;    // this launch covers the tiles [tile_first, total_tiles) (rketd_run_from_host: pieces of a line)
   int64_t nrows;
   int spread;             // warp tiles: 1 = fewer tiles than one wave of warps: deal them out across the SMs first
 };
@@ -271,7 +272,7 @@ __global__ void __launch_bounds__(NT, MINB) k2_tblock(const __grid_constant__ K2
     fence_barrier_init();
   }
   __syncthreads();
-  uint32_t tile = blockIdx.x;
+  uint32_t tile = q.tile_first + blockIdx.x;
   if (tid == 0 && tile < q.total_tiles) issue_loads(tile);
   uint32_t phase = 0;
 
@@ -367,7 +368,7 @@ __global__ void __launch_bounds__(NW * 32, MINB) k2_wtile(const __grid_constant_
   // the warps of a CTA work on consecutive tiles, so that the tiles in flight at any time are neighbours
   // in memory and the halo rows two tiles share are served by L2
   // (a problem smaller than one wave is latency bound: there one warp per SM beats twelve warps sharing an SM)
-  uint32_t tile = q.spread ? warp * gridDim.x + blockIdx.x : blockIdx.x * NW + warp;
+  uint32_t tile = q.tile_first + (q.spread ? warp * gridDim.x + blockIdx.x : blockIdx.x * NW + warp);
   uint32_t g = 0, ti = 0, flag = 0;
   int row0 = 0;
   if (tile < q.total_tiles) {
@@ -568,12 +569,22 @@ static void launch_k2_w(const K2Plan &plan, const K2Maps &m, const StepParams<R>
   else k2_wtile<R, NW, MINB, DIRECT, false><<<plan.grid, NW * 32, plan.smem_bytes, st>>>(m, sp, q, dst);
 }
 template <typename R>
-static cudaError_t launch_k2_t(const Layout &L, const K2Plan &plan, int src_buf, FieldPtrs dst, const StepCommon &sc,
-                               int steps, cudaStream_t st) {
+static cudaError_t launch_k2_t(const Layout &L, const K2Plan &plan_all, int src_buf, FieldPtrs dst, const StepCommon &sc,
+                               int steps, int64_t tile_begin, int64_t tile_end, cudaStream_t st) {
   K2Args q;
+  K2Plan plan = plan_all;
   q.T = steps; q.HR = plan.HR; q.rows_out = plan.rows_out;
   q.tiles_per_grid = (uint32_t)plan.tiles_per_grid; q.total_tiles = (uint32_t)plan.total_tiles; q.nrows = L.nrows;
   q.spread = plan.spread;
+  q.tile_first = 0;
+  if (tile_end >= 0) {     // a range of tiles: the grid shrinks with it
+    if (tile_begin < 0 || tile_end > plan.total_tiles || tile_begin >= tile_end) return cudaErrorInvalidValue;
+    q.tile_first = (uint32_t)tile_begin; q.total_tiles = (uint32_t)tile_end;
+    const int tpc = k2_tiles_per_cta(plan.variant);
+    const int64_t n = tile_end - tile_begin;
+    if (plan.spread) plan.grid = (int)std::min<int64_t>(n, plan.grid);
+    else plan.grid = (int)std::min<int64_t>((n + tpc - 1) / tpc, plan.grid);
+  }
   const StepParams<R> sp = make_params<R>(sc);
   const K2Maps &m = plan.maps[src_buf];
   switch (plan.variant) {
@@ -585,9 +596,9 @@ static cudaError_t launch_k2_t(const Layout &L, const K2Plan &plan, int src_buf,
   return cudaGetLastError();
 }
 cudaError_t launch_k2(int dtype, const Layout &L, const K2Plan &plan, int src_buf, FieldPtrs dst, const StepCommon &sc,
-                      int steps, cudaStream_t st) {
-  return dtype == 0 ? launch_k2_t<double>(L, plan, src_buf, dst, sc, steps, st)
-                    : launch_k2_t<float>(L, plan, src_buf, dst, sc, steps, st);
+                      int steps, cudaStream_t st, int64_t tile_begin, int64_t tile_end) {
+  return dtype == 0 ? launch_k2_t<double>(L, plan, src_buf, dst, sc, steps, tile_begin, tile_end, st)
+                    : launch_k2_t<float>(L, plan, src_buf, dst, sc, steps, tile_begin, tile_end, st);
 }
 
 }  // namespace rketd

@@ -21,10 +21,11 @@ OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, 1, 2, 3, 4
 SRC_NONE, SRC_GAUSS_DERIV, SRC_TABLE = -1, 0, 1
 KERNEL_AUTO, KERNEL_STEP, KERNEL_TBLOCK, KERNEL_RESIDENT = 0, 1, 2, 3
 CTR_LAUNCHES, CTR_STEP_LAUNCHES, CTR_KERNEL_USED, CTR_DEPTH_USED, CTR_STEPS_DONE, CTR_TILE_CELLS, \
-    CTR_HALO_CELLS, CTR_STATE_BYTES = range(8)
+    CTR_HALO_CELLS, CTR_STATE_BYTES, CTR_PIECES = range(9)
 
 EXPORTS = ["rketd_create", "rketd_set_media", "rketd_set_source", "rketd_set_probes", "rketd_set_probe_dft",
-           "rketd_set_fields", "rketd_reset", "rketd_discard_records", "rketd_set_plan", "rketd_run", "rketd_read_probes",
+           "rketd_set_fields", "rketd_reset", "rketd_discard_records", "rketd_set_plan", "rketd_run", "rketd_run_from_host",
+           "rketd_read_probes",
            "rketd_get_fields", "rketd_get_coefficients", "rketd_get_kernel_coefficients", "rketd_set_scheme",
            "rketd_set_boundary", "rketd_read_probe_dft",
            "rketd_read_sweep_rt", "rketd_measure_peak",
@@ -59,6 +60,7 @@ _lib.rketd_reset.argtypes = [_vp]
 _lib.rketd_discard_records.argtypes = [_vp]
 _lib.rketd_set_plan.argtypes = [_vp, _i32, _i32, _i32]
 _lib.rketd_run.argtypes = [_vp, _i64]
+_lib.rketd_run_from_host.argtypes = [_vp, _vp, _vp, _vp, _i64, _i32]
 _lib.rketd_read_probes.argtypes = [_vp, _vp, _i64, ctypes.POINTER(_i64)]
 _lib.rketd_get_fields.argtypes = [_vp, _vp, _vp, _vp]
 _lib.rketd_get_coefficients.argtypes = [_vp, _vp, _vp]
@@ -167,6 +169,10 @@ def rketd_run(h, nsteps: int):
     _check(h, _lib.rketd_run(h, nsteps))
 
 
+def rketd_run_from_host(h, wp, nu, E0, nsteps: int, npieces: int = 0):
+    _check(h, _lib.rketd_run_from_host(h, _ptr(wp), _ptr(nu), _ptr(E0), nsteps, npieces))
+
+
 def rketd_read_probes(h, out=None, out_bytes: int = 0) -> int:
     n = _i64()
     _check(h, _lib.rketd_read_probes(h, _ptr(out), out_bytes, ctypes.byref(n)))
@@ -256,6 +262,11 @@ class Sim:
 
     def set_boundary(self, kind, npml=5, grading=3.0, R0=1e-6): rketd_set_boundary(self.h, kind, npml, grading, R0)
     def run(self, nsteps): rketd_run(self.h, nsteps)
+
+    def run_from_host(self, wp, nu, E=None, nsteps=0, npieces=0):
+        """reset + set_media + set_fields(E) + run in one call, copies overlapped with the steps (one long line)"""
+        rketd_run_from_host(self.h, wp, nu, E, nsteps, npieces)
+
     def counter(self, which): return rketd_get_counter(self.h, which)
 
     def read_probes(self, out=None):
