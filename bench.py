@@ -83,8 +83,9 @@ def make_workload(name: str):
 class ClockSampler:
     """Samples SM clock and throttle reasons of one GPU every 100 ms while the timed region runs."""
 
-    def __init__(self, index: int):
+    def __init__(self, index: int, period: float = 0.1):
         self.index = index
+        self.period = period
         self.samples = []
         self.power = []
         self.reasons = set()
@@ -118,7 +119,7 @@ class ClockSampler:
                         self.reasons.add(k)
             except Exception:
                 pass
-            self._stop.wait(0.1)
+            self._stop.wait(self.period)
 
     def _poll_smi(self):
         q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
@@ -701,11 +702,12 @@ def extra_configs(rketd, stream, host_inputs):
             sl0 = sim.counter(rketd.CTR_STEP_LAUNCHES)
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             nrun = 2 if w.cell_updates > 1e9 else 5
-            e0.record(stream)
-            for _ in range(nrun):
-                one()
-            e1.record(stream)
-            torch.cuda.synchronize()
+            with ClockSampler(torch.cuda.current_device(), period=0.02) as clk:
+                e0.record(stream)
+                for _ in range(nrun):
+                    one()
+                e1.record(stream)
+                torch.cuda.synchronize()
             ms = e0.elapsed_time(e1)
             gc = w.cell_updates * nrun / (ms * 1e-3) / 1e9
             kernel_used, depth_used = sim.counter(rketd.CTR_KERNEL_USED), sim.counter(rketd.CTR_DEPTH_USED)
@@ -715,6 +717,14 @@ def extra_configs(rketd, stream, host_inputs):
                     "frac_vs_8TBps_nominal")
             out[key] = {"workload": w.name, "dtype": dtype, "value": gc, "unit": UNIT, "ms_per_step": ms / nrun, "steps": nrun,
                         "kernel": int(kernel_used), "depth_T": int(depth_used), "roofline": {k: roof[k] for k in keep if k in roof}}
+            c = clk.summary()
+            if c["samples"] >= 3 and c["sm_mhz"] and c["sm_max_mhz"]:
+                # the board holds its 1 kW cap by lowering the SM clock under FP64 load: the same fraction against the issue
+                # ceiling at the clock the run actually held (the figures above are against the device's maximum clock)
+                out[key]["clocks"] = c
+                for k in ("frac_of_mix_peak", "alu_frac_of_mix_peak"):
+                    if k in roof:
+                        out[key]["roofline"][k + "_at_held_clock"] = roof[k] * c["sm_max_mhz"] / c["sm_mhz"]
             sim.close()
             torch.cuda.empty_cache()
         except Exception as ex:          # an extra figure must never cost the headline

@@ -18,6 +18,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "librketd.so")
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
+              "-Xfatbin", "-compress-all",      # the sm_100a images shrink 4 x (21 -> 5 MB); cuobjdump reads them as before
               "-Xcompiler", "-fPIC"]
 
 

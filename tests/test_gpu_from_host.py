@@ -94,7 +94,7 @@ def test_pinned_and_device_inputs_and_no_initial_field(rk):
 def test_against_the_oracle(rk):
     n, nsteps = 20_000, 260
     wp, nu, E0 = _inputs(n, "f64", 21)
-    probes, src_cell = [3, 9_000, 12_345, n - 1], 10_000
+    probes, src_cell = [3, 9_950, 10_060, n - 1], 10_000
     st = oracle.State(n, 1, E0=E0[None])
     ref, _ = oracle.run(st, wp[None], nu[None], DZ, DT, nsteps, src_kind=0, src_params=SRC, src_cell=src_cell, probes=probes)
     s = _setup(rk, n, "f64", 16, probes, src_cell, 0)
