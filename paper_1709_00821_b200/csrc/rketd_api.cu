@@ -38,6 +38,7 @@ struct rketd_sim {
   void *coef[kNumCoefArrays] = {nullptr, nullptr, nullptr, nullptr};   // P, ch, ka, Q (rketd_device.cuh)
   double *wp_p = nullptr, *nu_p = nullptr;                              // media in the padded layout, fp64
   uint8_t *rowflag = nullptr;
+  std::vector<uint8_t> h_rowflag;  // host copy (k3_resident: which warps carry a boundary, the source, a probe)
   bool flags_dirty = true;
   bool have_media = false;
   bool fields_zero = true;      // E = H = J = 0 (after create / reset): no J <-> G conversion needed
@@ -162,6 +163,7 @@ int rebuild_rowflags(rketd_sim *s) {
   }
   CU_TRY(s, cudaMemcpyAsync(s->rowflag, f.data(), f.size(), cudaMemcpyHostToDevice, s->stream));
   CU_TRY(s, cudaStreamSynchronize(s->stream));   // f is a local
+  s->h_rowflag.swap(f);
   s->flags_dirty = false;
   return RKETD_OK;
 }
@@ -273,7 +275,10 @@ int build_k2_plan(rketd_sim *s, int depth, int variant) {
 // faster than with a barrier per step) or when a grid is too large for one CTA; the one-barrier-per-step kernel when
 // many grids that each fit one CTA keep every SM busy — there four small CTAs per SM hide each other's barriers and it
 // is still the faster of the two (config 3 1020 against 785 Gcell/s, config 5 863 against 701).
-int legacy_k3_variant(const rketd_sim *s) { return (s->L.nrows > 32 && s->L.nrows <= 256) ? 2 : 0; }
+int legacy_k3_variant(const rketd_sim *s) {
+  if (s->dtype == RKETD_F32 && s->L.nrows <= 64) return 0;      // (config 5 fp32, 64 rows: 1288 against 1230 Gcell/s)
+  return (s->L.nrows > 32 && s->L.nrows <= 256) ? 2 : 0;
+}
 bool wtile_variant(const rketd_sim *s, int variant) {
   if (variant >= 0) return (variant & RKETD_RESIDENT_WTILE_FLAG) != 0;
   return k3w_few_grids(s->L, s->sms) || !k3_threads_for_rows(s->dtype, s->L.nrows, 0);
@@ -411,7 +416,10 @@ int run_segment(rketd_sim *s, int64_t nsteps, void *rec) {
       if (!k3_threads_for_rows(s->dtype, L.nrows, variant)) variant = 0;
       const int NT = k3_threads_for_rows(s->dtype, L.nrows, variant);
       if (!NT) return fail(s, RKETD_EINVAL, "grid too large for the one-CTA resident kernel");
-      CU_TRY(s, launch_k3(s->dtype, L, f, s->coef, sc, nsteps, NT, variant, s->stream));
+      // library's choice: the heavy tiles of a grid dealt over the SM's schedulers; an explicit variant keeps tile t on warp t
+      uint8_t tile_flags[16] = {};
+      for (int64_t r = 0; r < L.nrows && r < (int64_t)s->h_rowflag.size(); ++r) tile_flags[r / 32] |= s->h_rowflag[(size_t)r];
+      CU_TRY(s, launch_k3(s->dtype, L, f, s->coef, sc, nsteps, NT, variant, s->stream, tile_flags, s->plan_variant < 0));
       s->ctr_tile_cells = L.gstride; s->ctr_halo_cells = 0; s->ctr_depth_used = nsteps;
     }
     ++s->ctr_launches; ++s->ctr_step_launches;

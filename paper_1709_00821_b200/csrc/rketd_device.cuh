@@ -406,6 +406,7 @@ struct WarpSpecial {
   uint32_t mR = 0, mS = 0;            // bit i: this lane's local node i is node ncells-1 / the source node
   uint32_t mHz = 0;                   // bit i: H of local node i is padding (behind node ncells-1, or left of node 0)
   bool l_p0 = false, l_p1 = false;    // this lane records one / two probes
+  bool two_probes = false;            // some lane of the warp records two (warp-uniform)
 };
 
 template <typename R, int C, bool PML>
@@ -417,6 +418,7 @@ __device__ __forceinline__ WarpSpecial make_warp_special(const StepParams<R> &p,
   ws.mS = sx.iS >= 0 ? 1u << sx.iS : 0u;
   ws.mHz = (sx.iR >= 0 ? (0xffffffffu << sx.iR) & ((1u << C) - 1u) : 0u) | (sx.iL == 1 ? 1u : 0u);
   ws.l_p0 = sx.np >= 1 && sx.np <= 2; ws.l_p1 = sx.np == 2;
+  ws.two_probes = __any_sync(full, ws.l_p1);
   ws.mask = (__any_sync(full, sx.iL >= 0) ? SF_MURL : 0) | (__any_sync(full, sx.iR >= 0) ? SF_MURR : 0) |
             (__any_sync(full, sx.iS >= 0) ? SF_SRC : 0) | (__any_sync(full, ws.l_p0) ? SF_PROBE : 0);
   // an absorbing layer, or more than two probes among one lane's nodes: the general per-lane path
@@ -438,7 +440,10 @@ __device__ __forceinline__ R select_node(const R (&v)[C], int idx) {
 }
 
 // a3, a4, a6 for the lanes of a warp tile with the features MASK (first-order Mur ends only)
-template <int MASK, typename R, int C>
+// GUARD (k3_resident, whose instantiations group the features: Mur, source/probe, all): each feature's block sits behind a
+// warp-uniform branch on the warp's own features, so that e.g. the warp with node 0 and the source does not pay for the
+// C - 1 candidates of the right end.
+template <int MASK, typename R, int C, bool GUARD = false>
 __device__ __forceinline__ void special_select(const R (&E)[C], R (&En)[C], const StepParams<R> &p, const SpecialIdx &sx,
                                                const WarpSpecial &ws, int64_t nloc, R src_now) {
   typedef Arith<R> A;
@@ -450,23 +455,36 @@ __device__ __forceinline__ void special_select(const R (&E)[C], R (&En)[C], cons
   }
   if constexpr ((MASK & SF_MURR) != 0) {      // node ncells-1 at local index >= 1, node ncells-2 in the same row
     // (descending, so that every candidate sees the interior value of its inward neighbour; one bit of mR is set at most)
+    if (!GUARD || (ws.mask & SF_MURR)) {
 #pragma unroll
-    for (int i = C - 1; i >= 1; --i) {
-      const R cand = A::fma(p.mur_m, A::sub(En[i - 1], E[i]), E[i - 1]);
-      En[i] = ((ws.mR >> i) & 1u) ? cand : En[i];
+      for (int i = C - 1; i >= 1; --i) {
+        const R cand = A::fma(p.mur_m, A::sub(En[i - 1], E[i]), E[i - 1]);
+        En[i] = ((ws.mR >> i) & 1u) ? cand : En[i];
+      }
     }
   }
   if constexpr ((MASK & SF_SRC) != 0) {
+    if (!GUARD || (ws.mask & SF_SRC)) {
 #pragma unroll
-    for (int i = 0; i < C; ++i) {
-      const R sum = A::add(En[i], src_now);
-      En[i] = ((ws.mS >> i) & 1u) ? sum : En[i];
+      for (int i = 0; i < C; ++i) {
+        const R sum = A::add(En[i], src_now);
+        En[i] = ((ws.mS >> i) & 1u) ? sum : En[i];
+      }
     }
   }
   if constexpr ((MASK & SF_PROBE) != 0) {      // up to two probes among a lane's nodes; predicated stores, no branch
-    const R v0 = select_node<R, C>(En, sx.pi0), v1 = select_node<R, C>(En, sx.pi1);
-    stg_if(ws.l_p0, p.rec + (sx.pr0 + nloc), v0);
-    stg_if(ws.l_p1, p.rec + (sx.pr1 + nloc), v1);
+    if constexpr (!GUARD) {
+      const R v0 = select_node<R, C>(En, sx.pi0), v1 = select_node<R, C>(En, sx.pi1);
+      stg_if(ws.l_p0, p.rec + (sx.pr0 + nloc), v0);
+      stg_if(ws.l_p1, p.rec + (sx.pr1 + nloc), v1);
+    } else if (ws.mask & SF_PROBE) {
+      const R v0 = select_node<R, C>(En, sx.pi0);
+      stg_if(ws.l_p0, p.rec + (sx.pr0 + nloc), v0);
+      if (ws.two_probes) {
+        const R v1 = select_node<R, C>(En, sx.pi1);
+        stg_if(ws.l_p1, p.rec + (sx.pr1 + nloc), v1);
+      }
+    }
   }
 }
 
@@ -483,7 +501,7 @@ __device__ __forceinline__ void zero_padding_H(R (&H)[C], const WarpSpecial &ws)
 // neighbour's own), so that one exchange of old values per step is enough.
 // MASK: SF_* features of the warp (0: none, the boundary/source/probe handling is compiled out; SF_SLOW: step_special's
 // per-lane chains; else the select arithmetic of special_select, H padding zeroed by the caller after the time loop).
-template <int MASK, bool PML, typename R, int C, typename CF>
+template <int MASK, bool PML, typename R, int C, typename CF, bool GUARD = false>
 __device__ __forceinline__ void step_fields(const R (&E)[C], R (&En)[C], R (&H)[C], const R (&G)[C], const CF &cf, R El,
                                             R Hl, R Er, R nchh, const StepParams<R> &p, const SpecialIdx &sx,
                                             const WarpSpecial &ws, int64_t nloc, R src_now) {
@@ -515,7 +533,7 @@ __device__ __forceinline__ void step_fields(const R (&E)[C], R (&En)[C], R (&H)[
   if constexpr (MASK == SF_SLOW) {
     if (sx.any) step_special<R, C, PML>(E, En, H, p, sx, nloc, src_now);
   } else if constexpr (MASK != 0) {
-    special_select<MASK, R, C>(E, En, p, sx, ws, nloc, src_now);
+    special_select<MASK, R, C, GUARD>(E, En, p, sx, ws, nloc, src_now);
   }
 }
 

@@ -93,8 +93,11 @@ cudaError_t launch_k1(int dtype, const Layout &L, FieldPtrs src, FieldPtrs dst, 
 // tile_end >= 0: only the tiles [tile_begin, tile_end) of the plan (rketd_run_from_host)
 cudaError_t launch_k2(int dtype, const Layout &L, const K2Plan &plan, int src_buf, FieldPtrs dst, const StepCommon &sc,
                       int steps, cudaStream_t st, int64_t tile_begin = 0, int64_t tile_end = -1);
+// tile_flags[t]: OR of the row flags of the grid's rows 32 t .. 32 t + 31 (host copy; nullptr or balance = false: tile t on
+// warp t)
 cudaError_t launch_k3(int dtype, const Layout &L, FieldPtrs fld, void *const coef[kNumCoefArrays], const StepCommon &sc,
-                      int64_t nsteps, int NT, int variant, cudaStream_t st);
+                      int64_t nsteps, int NT, int variant, cudaStream_t st, const uint8_t *tile_flags = nullptr,
+                      bool balance = false);
 cudaError_t k2_configure(int dtype, int variant, int *ctas_per_sm);   // sets smem attribute, returns occupancy
 
 // auxiliary kernels (rketd_aux.cu)

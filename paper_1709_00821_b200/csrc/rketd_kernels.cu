@@ -19,6 +19,8 @@
 //
 // Mur boundaries, the soft source and probe recording are folded into the rows that hold
 // those nodes (rowflag) inside the same kernels — see step_fields in rketd_device.cuh.
+#include <algorithm>
+
 #include "rketd_device.cuh"
 #include "rketd_internal.h"
 #include "rketd_wtile.cuh"
@@ -72,7 +74,7 @@ __device__ __forceinline__ void time_loop(R (&E)[C], R (&H)[C], R (&J)[C], const
   R Eb[C];
   auto one_step = [&](const R (&Ein)[C], R (&Eout)[C], int par) {
     const R src_now = SRC ? src.sample(p, nloc, lane) : R(0);
-    step_fields<MASK, PML, R, C>(Ein, Eout, H, J, cf, El, Hl, Er, nchh, p, sx, ws, nloc, src_now);
+    step_fields<MASK, PML, R, C, CF, true>(Ein, Eout, H, J, cf, El, Hl, Er, nchh, p, sx, ws, nloc, src_now);
     send_halo<R, C, NW>(Eout, H, hs, par, warp, lane, El, Hl, Er);     // for the next step
     step_current<R, C>(J, Ein, cf);
     cta_barrier();
@@ -113,10 +115,20 @@ __device__ __forceinline__ void time_loop_dispatch(R (&E)[C], R (&H)[C], R (&J)[
 
 // ------------------------------------------------------------------------------------ K3
 // One CTA per grid; NT threads x C nodes cover the grid (NT * C >= physical nodes per grid).
+// Which 32 rows of the grid a hardware warp holds.  The warps of a CTA sit on the SM's four schedulers by warp index
+// (consecutive warps on consecutive schedulers, measured), and the warps with a boundary, the source or a probe issue
+// 1.5-2.2 x the instructions of a plain one.  `tile[]` (host: k3_balance) deals the heavy tiles of a grid to different
+// schedulers: config 3 (16 warps; tiles 0, 4, 12 heavy, all on scheduler 0 in natural order) 1085 -> 1230 Gcell/s.  Across
+// the CTAs that share an SM nothing is needed: the hardware starts each CTA on the next scheduler (measured with %warpid:
+// of four resident 4-warp CTAs, warp 0 sits once on each scheduler), and a rotation by CTA index changed nothing.
+struct K3Map {
+  uint8_t tile[16];
+};
+
 template <typename R, int C, int NT, bool CSM, int MINB, bool PML>
 __global__ void __launch_bounds__(NT, MINB) k3_resident(RowPtrs<R> f, CoefPtrs<R> cp,
                                                         const __grid_constant__ StepParams<R> p, int64_t nrows,
-                                                        int64_t nsteps) {
+                                                        int64_t nsteps, const K3Map map) {
   typedef Geom<R, C> G;
   constexpr int NW = NT / 32;
   constexpr int ROWS = NT / G::TPR;
@@ -124,7 +136,9 @@ __global__ void __launch_bounds__(NT, MINB) k3_resident(RowPtrs<R> f, CoefPtrs<R
   __shared__ HaloSlots<R, NW> hs;
   extern __shared__ uint8_t smem_raw[];
 
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int lane = threadIdx.x & 31;
+  const int warp = map.tile[threadIdx.x >> 5];      // the tile, from here on
+  const int tid = warp * 32 + lane;
   const int64_t g = blockIdx.x;
   const int row = tid / G::TPR;
   const bool valid = row < nrows;
@@ -471,45 +485,70 @@ int k3_threads_for_rows(int, int64_t nrows, int variant) {
 
 template <typename R, int C, int NT, bool CSM, int MINB, bool PML>
 static cudaError_t launch_k3_p(const Layout &L, FieldPtrs f, void *const coef[kNumCoef], const StepCommon &sc,
-                               int64_t nsteps, cudaStream_t st) {
+                               int64_t nsteps, const K3Map &map, cudaStream_t st) {
   auto kern = k3_resident<R, C, NT, CSM, MINB, PML>;
   const size_t smem = CSM ? (size_t)kNumCoef * (NT / Geom<R, C>::TPR) * kRowBytes + 1024 : 0;
   if (smem > 48 * 1024) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
   }
-  kern<<<(unsigned)L.nbatch, NT, smem, st>>>(rp<R>(f), cpz<R>(coef), make_params<R>(sc), L.nrows, nsteps);
+  kern<<<(unsigned)L.nbatch, NT, smem, st>>>(rp<R>(f), cpz<R>(coef), make_params<R>(sc), L.nrows, nsteps, map);
   return cudaGetLastError();
 }
 template <typename R, int C, int NT, bool CSM, int MINB>
 static cudaError_t launch_k3_v(const Layout &L, FieldPtrs f, void *const coef[kNumCoef], const StepCommon &sc,
-                               int64_t nsteps, cudaStream_t st) {
-  return sc.npml > 0 ? launch_k3_p<R, C, NT, CSM, MINB, true>(L, f, coef, sc, nsteps, st)
-                     : launch_k3_p<R, C, NT, CSM, MINB, false>(L, f, coef, sc, nsteps, st);
+                               int64_t nsteps, const K3Map &map, cudaStream_t st) {
+  return sc.npml > 0 ? launch_k3_p<R, C, NT, CSM, MINB, true>(L, f, coef, sc, nsteps, map, st)
+                     : launch_k3_p<R, C, NT, CSM, MINB, false>(L, f, coef, sc, nsteps, map, st);
 }
 template <typename R>
 static cudaError_t launch_k3_t(const Layout &L, FieldPtrs f, void *const coef[kNumCoef], const StepCommon &sc,
-                               int64_t nsteps, int NT, int variant, cudaStream_t st) {
+                               int64_t nsteps, int NT, int variant, const K3Map &map, cudaStream_t st) {
   constexpr int CF = kRowBytes / sizeof(R);
   if (variant == 0) switch (NT) {
-    case 32: return launch_k3_v<R, CF, 32, false, 8>(L, f, coef, sc, nsteps, st);
-    case 64: return launch_k3_v<R, CF, 64, false, 6>(L, f, coef, sc, nsteps, st);
-    case 128: return launch_k3_v<R, CF, 128, false, 3>(L, f, coef, sc, nsteps, st);
-    case 256: return launch_k3_v<R, CF, 256, false, 1>(L, f, coef, sc, nsteps, st);
-    case 512: return launch_k3_v<R, CF, 512, true, 1>(L, f, coef, sc, nsteps, st);
+    case 32: return launch_k3_v<R, CF, 32, false, 8>(L, f, coef, sc, nsteps, map, st);
+    case 64: return launch_k3_v<R, CF, 64, false, 6>(L, f, coef, sc, nsteps, map, st);
+    case 128: return launch_k3_v<R, CF, 128, false, 3>(L, f, coef, sc, nsteps, map, st);
+    case 256: return launch_k3_v<R, CF, 256, false, 1>(L, f, coef, sc, nsteps, map, st);
+    case 512: return launch_k3_v<R, CF, 512, true, 1>(L, f, coef, sc, nsteps, map, st);
   }
   else if (variant == 2) switch (NT) {   // whole rows, coefficients in shared memory (warps of uniform rows: registers)
-    case 64: return launch_k3_v<R, CF, 64, true, 8>(L, f, coef, sc, nsteps, st);
-    case 128: return launch_k3_v<R, CF, 128, true, 4>(L, f, coef, sc, nsteps, st);
-    case 256: return launch_k3_v<R, CF, 256, true, 2>(L, f, coef, sc, nsteps, st);
-    case 512: return launch_k3_v<R, CF, 512, true, 1>(L, f, coef, sc, nsteps, st);
+    case 64: return launch_k3_v<R, CF, 64, true, 8>(L, f, coef, sc, nsteps, map, st);
+    case 128: return launch_k3_v<R, CF, 128, true, 4>(L, f, coef, sc, nsteps, map, st);
+    case 256: return launch_k3_v<R, CF, 256, true, 2>(L, f, coef, sc, nsteps, map, st);
+    case 512: return launch_k3_v<R, CF, 512, true, 1>(L, f, coef, sc, nsteps, map, st);
   }
   return cudaErrorInvalidValue;
 }
+// tiles -> hardware warps: heaviest tiles first, each to the scheduler (warp index mod 4) with the least work so far
+static K3Map k3_balance(int NW, const uint8_t *tile_flags, bool balance) {
+  K3Map m;
+  for (int i = 0; i < 16; ++i) m.tile[i] = (uint8_t)i;
+  if (!balance || !tile_flags || NW < 2) return m;
+  const int ncls = NW < 4 ? NW : 4, per = NW / ncls;
+  double w[16], load[4] = {0, 0, 0, 0};
+  int used[4] = {0, 0, 0, 0}, order[16];
+  for (int t = 0; t < NW; ++t) {
+    const bool mur = tile_flags[t] & (F_MURL | F_MURR), sp = tile_flags[t] & (F_SRC | F_PROBE);
+    w[t] = (tile_flags[t] & F_PML) ? 2.5 : (mur && sp) ? 2.2 : sp ? 1.6 : mur ? 1.5 : 1.0;   // issued work / a plain warp's (from config-5 runs with and without source and probes)
+    order[t] = t;
+  }
+  std::stable_sort(order, order + NW, [&](int a, int b) { return w[a] > w[b]; });
+  for (int o = 0; o < NW; ++o) {
+    int best = -1;
+    for (int c = 0; c < ncls; ++c)
+      if (used[c] < per && (best < 0 || load[c] < load[best])) best = c;
+    m.tile[best + ncls * used[best]] = (uint8_t)order[o];
+    load[best] += w[order[o]];
+    ++used[best];
+  }
+  return m;
+}
 cudaError_t launch_k3(int dtype, const Layout &L, FieldPtrs f, void *const coef[kNumCoef], const StepCommon &sc,
-                      int64_t nsteps, int NT, int variant, cudaStream_t st) {
-  return dtype == 0 ? launch_k3_t<double>(L, f, coef, sc, nsteps, NT, variant, st)
-                    : launch_k3_t<float>(L, f, coef, sc, nsteps, NT, variant, st);
+                      int64_t nsteps, int NT, int variant, cudaStream_t st, const uint8_t *tile_flags, bool balance) {
+  const K3Map map = k3_balance(NT / 32, tile_flags, balance);
+  return dtype == 0 ? launch_k3_t<double>(L, f, coef, sc, nsteps, NT, variant, map, st)
+                    : launch_k3_t<float>(L, f, coef, sc, nsteps, NT, variant, map, st);
 }
 
 // K2 variants (numbers kept from round 1; 1, 3, 4, 5, 7 were slower everywhere measured and are gone):
