@@ -140,7 +140,10 @@ int rketd_discard_records(rketd_sim *s);
 #define RKETD_RESIDENT_WTILE_NOLEAN 0x20000000 /* or-ed in: the 232-register instantiation (coefficients in registers) */
 #define RKETD_RESIDENT_WTILE_LEAN 0x10000000   /* or-ed in: the 168-register instantiation (E in place, coefficients from four
                                                   registers or shared memory); default for many grids */
-#define RKETD_RESIDENT_WTILE(nw, nc, k) (RKETD_RESIDENT_WTILE_FLAG | ((k) << 16) | ((nc) << 8) | (nw))
+#define RKETD_RESIDENT_WTILE_HALF 0x08000000   /* or-ed in: a lane holds half a 64-B row (twice the warps per grid, half the dependent
+                                                  work per step); default for a few grids with Mur ends */
+#define RKETD_RESIDENT_WTILE_NOHALF 0x04000000 /* or-ed in: whole rows per lane */
+#define RKETD_RESIDENT_WTILE(nw, nc, k) (RKETD_RESIDENT_WTILE_FLAG | ((k) << 16) | ((nc) << 8) | (nw))   /* k < 1024 */
 int rketd_set_plan(rketd_sim *s, int kernel, int depth, int variant);
 
 /* Advance every grid by nsteps leapfrog steps (H eq. (14); E eq. (12)

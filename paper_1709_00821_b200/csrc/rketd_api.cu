@@ -285,24 +285,34 @@ bool wtile_variant(const rketd_sim *s, int variant) {
 }
 bool resident_wtile_plan(rketd_sim *s, int depth, int variant, K3WPlan *P) {
   int64_t nw = 0, nc = 0, k = 0;
-  if (variant >= 0) { nw = variant & 0xff; nc = (variant >> 8) & 0xff; k = (variant >> 16) & 0xfff; }
+  if (variant >= 0) { nw = variant & 0xff; nc = (variant >> 8) & 0xff; k = (variant >> 16) & 0x3ff; }
+  const bool few = k3w_few_grids(s->L, s->sms), no_layer = s->bc_npml == 0 && s->pml.npml == 0;
   // the lean instantiation (<= 128 registers) serves Mur ends with at most two probes among the nodes of one lane
   // (measured: +26 % on config 3, +55 % on config 5 when many chunks share the SMs; 12 % slower on config 1, where one chunk is
   // a chain of dependent steps and the in-place update lengthens it — so: many grids only, unless the variant says otherwise)
   const bool ask_lean = variant >= 0 && (variant & RKETD_RESIDENT_WTILE_LEAN), ask_fat = variant >= 0 && (variant & RKETD_RESIDENT_WTILE_NOLEAN);
-  bool lean = s->bc_npml == 0 && s->pml.npml == 0 && !ask_fat && (ask_lean || !k3w_few_grids(s->L, s->sms));
+  const bool ask_half = variant >= 0 && (variant & RKETD_RESIDENT_WTILE_HALF), ask_full = variant >= 0 && (variant & RKETD_RESIDENT_WTILE_NOHALF);
+  bool lean = no_layer && !ask_fat && !ask_half && (ask_lean || !few);
   if (lean) {
     std::vector<int64_t> rows;
     for (int64_t c : s->probes) rows.push_back((s->L.off + c) / s->L.C);
     std::sort(rows.begin(), rows.end());
     for (size_t i = 2; i < rows.size(); ++i) lean = lean && rows[i] != rows[i - 2];
   }
-  if (!k3w_plan(s->L, depth, s->sms, nw, nc, k, lean, P)) return false;
-  if (P->nc > 1) {              // the cluster must be schedulable on this device (GPC size, registers, shared memory)
+  // half rows per lane (a few grids = a chain of dependent steps: a step of 4 fp64 nodes per lane takes 75 cycles against 141,
+  // profiles/r02_peaks.md); Mur ends only, at most two probes in one lane's nodes (else the general path, which is slower)
+  bool half = no_layer && !lean && !ask_full && (ask_half || (few && variant < 0));
+  auto schedulable = [&](K3WPlan *Q) {
+    if (Q->nc <= 1 && !Q->half) return true;   // the cluster must be schedulable on this device (GPC size, registers, shared memory)
     int ncl = 0;
-    if (k3w_max_clusters(s->dtype, *P, &ncl) != cudaSuccess || ncl < 1) { cudaGetLastError(); return false; }
+    if (k3w_max_clusters(s->dtype, *Q, &ncl) != cudaSuccess || ncl < 1) { cudaGetLastError(); return false; }
+    return true;
+  };
+  if (half) {
+    if (k3w_plan(s->L, depth, s->sms, nw, nc, k, false, true, P) && schedulable(P)) return true;
+    if (ask_half) return false;
   }
-  return true;
+  return k3w_plan(s->L, depth, s->sms, nw, nc, k, lean, false, P) && schedulable(P);
 }
 
 int resolve_kernel(rketd_sim *s) {
@@ -312,7 +322,7 @@ int resolve_kernel(rketd_sim *s) {
   if (!resident_wtile_plan(s, 0, -1, &P)) return RKETD_KERNEL_TBLOCK;
   // one long line spread over most of a 16-CTA cluster: K2's deep passes (T = 64) win again from about 100 warp
   // tiles on (paper Table 2: 40 960 cells 0.44 ms against 0.54; 20 480 cells 0.47 against 0.41)
-  if (k3w_few_grids(s->L, s->sms) && P.nc * P.nw > 96) return RKETD_KERNEL_TBLOCK;
+  if (k3w_few_grids(s->L, s->sms) && P.nc * P.nw > (P.half ? 128 : 96)) return RKETD_KERNEL_TBLOCK;
   return RKETD_KERNEL_RESIDENT;
 }
 
@@ -408,7 +418,7 @@ int run_segment(rketd_sim *s, int64_t nsteps, void *rec) {
         return fail(s, RKETD_EINVAL, "grid too large for the resident kernel (or the requested packing cannot run)");
       CU_TRY(s, launch_k3w(s->dtype, L, P, f, s->coef, sc, nsteps, s->stream));
       // cells a chunk occupies on chip (halo and padding lanes included) against the cells it holds
-      s->ctr_tile_cells = (int64_t)P.nc * P.nw * 32 * L.C;
+      s->ctr_tile_cells = (int64_t)P.nc * P.nw * 32 * (P.half ? L.C / 2 : L.C);
       s->ctr_halo_cells = (s->ctr_tile_cells - P.k * L.gstride) / 2;
       s->ctr_depth_used = P.T;
     } else {

@@ -270,6 +270,61 @@ struct SourceStream {
   }
 };
 
+// The same samples for the resident warp tiles (k3_wtile), one round of T <= 64 steps at a time: the samples of the round
+// sit in the warp's own shared-memory strip (one LDS per step, no shuffle with a computed lane, no branch); the next
+// round's are fetched into a register pair while this round steps, so no global load is ever waited for.
+__device__ __forceinline__ void lds_scalar(uint32_t a, double &v) { asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a)); }
+__device__ __forceinline__ void lds_scalar(uint32_t a, float &v) { asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a)); }
+__device__ __forceinline__ void sts_scalar(uint32_t a, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
+__device__ __forceinline__ void sts_scalar(uint32_t a, float v) { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory"); }
+template <typename R>
+struct SourceRound {
+  static constexpr uint32_t kBytesPerWarp = 64u * sizeof(double);
+  uint32_t strip = 0;           // shared address of the warp's strip (64 samples)
+  int64_t round0 = 0;           // step index of the strip's first sample
+  R nxt0 = R(0), nxt1 = R(0);   // samples lane, lane + 32 of the next round
+  bool on = false;
+  int T = 0;
+  __device__ __forceinline__ R fetch(const StepParams<R> &p, int64_t idx) const {
+    return (p.src_tab != nullptr && idx < p.rec_stride) ? p.src_tab[idx] : R(0);
+  }
+  __device__ __forceinline__ void publish(int lane) {
+    sts_scalar(strip + (uint32_t)lane * (uint32_t)sizeof(R), nxt0);
+    sts_scalar(strip + (uint32_t)(lane + 32) * (uint32_t)sizeof(R), nxt1);
+    __syncwarp();
+  }
+  // on: some lane of this warp holds the source node (warp-uniform); steps_per_round <= 64
+  __device__ __forceinline__ void start(const StepParams<R> &p, bool warp_has_source, int64_t n0, int lane, int steps_per_round, uint32_t strip_addr) {
+    on = warp_has_source; T = steps_per_round; strip = strip_addr; round0 = n0;
+    if (on) {
+      nxt0 = fetch(p, n0 + lane); nxt1 = fetch(p, n0 + 32 + lane);
+      publish(lane);
+      nxt0 = fetch(p, n0 + T + lane); nxt1 = fetch(p, n0 + T + 32 + lane);
+    }
+  }
+  // before the round that starts at step n (not the first one)
+  __device__ __forceinline__ void next_round(const StepParams<R> &p, int64_t n, int lane) {
+    if (on) {
+      __syncwarp();
+      round0 = n;
+      publish(lane);
+      nxt0 = fetch(p, n + T + lane); nxt1 = fetch(p, n + T + 32 + lane);
+    }
+  }
+  __device__ __forceinline__ R sample(const StepParams<R> &, int64_t nloc, int) const {
+    R v = R(0);
+    if (on) lds_scalar(strip + (uint32_t)(nloc - round0) * (uint32_t)sizeof(R), v);
+    return v;
+  }
+  __device__ __forceinline__ void sample2(const StepParams<R> &, int64_t nloc, int, R &s0, R &s1) const {
+    s0 = R(0); s1 = R(0);
+    if (on) {
+      const uint32_t a = strip + (uint32_t)(nloc - round0) * (uint32_t)sizeof(R);
+      lds_scalar(a, s0); lds_scalar(a + (uint32_t)sizeof(R), s1);
+    }
+  }
+};
+
 // ---- Mur (a3), soft source (a4), probe record (a6) and padding hygiene for the threads whose nodes include a
 // boundary, the source or a probe.  These threads run alone in their warp (divergent), so what counts is the
 // number of instructions on that path: everything that does not change from step to step is worked out once

@@ -72,11 +72,12 @@ struct K3WPlan {
   int tiles_per_chunk = 0;
   uint32_t smem_bytes = 0;
   bool lean = false;                   // the <= 128-register instantiation (E in place, coefficients from 4 registers / shared memory)
+  bool half = false;                   // a lane holds half a 64-B row: rows above count half rows (few grids: shorter dependent steps)
 };
 // false when the grid cannot stay resident (a grid needs more than 16 CTAs x 12 warp tiles) or the wish cannot be met;
 // want_* = 0: chosen here
 bool k3w_few_grids(const Layout &L, int sms);
-bool k3w_plan(const Layout &L, int depth, int sms, int64_t want_nw, int64_t want_nc, int64_t want_k, bool lean, K3WPlan *out);
+bool k3w_plan(const Layout &L, int depth, int sms, int64_t want_nw, int64_t want_nc, int64_t want_k, bool lean, bool half, K3WPlan *out);
 cudaError_t launch_k3w(int dtype, const Layout &L, const K3WPlan &P, FieldPtrs fld, void *const coef[4], const StepCommon &sc,
                        int64_t nsteps, cudaStream_t st);
 cudaError_t k3w_max_clusters(int dtype, const K3WPlan &P, int *nclusters);

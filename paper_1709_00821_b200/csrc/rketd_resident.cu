@@ -19,6 +19,8 @@
 
 namespace rketd {
 
+// "row" below = the C nodes one lane holds: a 64-B row of the layout, or half of one (HALF: twice the warps on a grid,
+// half the dependent work per step — what a few grids, i.e. a chain of dependent steps, want)
 struct K3WArgs {
   int T, HR, rows_out;          // steps per round, halo rows, 32 - 2 HR
   int cluster;                  // CTAs per chunk
@@ -49,16 +51,24 @@ __device__ __forceinline__ void cluster_barrier() {
   asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
 
+#ifdef RKETD_K3W_TRACE
+__device__ long long g_k3w_trace[16 * 12 * 8 * 6];
+#define K3W_STAMP(k) do { if (lane == 0 && rnd >= 100 && rnd < 108) g_k3w_trace[((blockIdx.x * 12 + warp) * 8 + (rnd - 100)) * 6 + (k)] = clock64(); } while (0)
+#else
+#define K3W_STAMP(k) do { } while (0)
+#endif
+
 // halo slots of one CTA: [parity 2][warp][side 2][row HR][array 3][64 B]; side 0 = the tile's lanes 0..HR-1
-constexpr int kMaxHR = 2;
+constexpr int kMaxHR = 4;
 __host__ __device__ constexpr uint32_t slot_bytes_per_warp() { return 2u * kMaxHR * 3u * kRowBytes; }
 
 // LEAN: E in place and coefficients from four registers or the warp's shared-memory rows (warp_step_lean): 168
 // registers, twelve warps per SM instead of eight.  The host picks it unless a layer is live or one lane records more than two probes.
-template <typename R, bool CLUSTER, bool PML, bool LEAN>
+template <typename R, bool CLUSTER, bool PML, bool LEAN, bool HALF = false>
 __global__ void __launch_bounds__(LEAN ? 384 : 256, 1) k3_wtile(RowPtrs<R> f, CoefPtrs<R> cp, const __grid_constant__ StepParams<R> p,
                                                                const K3WArgs q) {
-  constexpr int C = kRowBytes / sizeof(R);
+  static_assert(!HALF || (!LEAN && !PML), "half rows: plain instantiation only");
+  constexpr int C = (int)(kRowBytes / sizeof(R)) / (HALF ? 2 : 1);
   typedef Geom<R, C> G;
   typedef typename Arith<R>::Vec Vec;
   extern __shared__ __align__(16) uint8_t slots_raw[];
@@ -91,12 +101,12 @@ __global__ void __launch_bounds__(LEAN ? 384 : 256, 1) k3_wtile(RowPtrs<R> f, Co
     load_nodes_global<R, C>(f.E, first, E);
     load_nodes_global<R, C>(f.H, first, H);
     load_nodes_global<R, C>(f.J, first, J);
-    flag = p.rowflag[rowg];
+    flag = p.rowflag[HALF ? rowg >> 1 : rowg];
   }
   if constexpr (LEAN) {
     // coefficients: each lane stages its row of the four arrays in the warp's shared-memory area (only this warp reads
     // it back) and notes whether its nodes all carry one set; a warp of such lanes then runs from four registers
-    const uint32_t cbase = slots + 2u * par_bytes;
+    const uint32_t cbase = slots + 2u * par_bytes + (uint32_t)nw * SourceRound<R>::kBytesPerWarp;
     cs.base = ((cbase + 1023u) & ~1023u) + (uint32_t)warp * (kNumCoef * 32u * kRowBytes);
     cs.lane = lane;
     bool uni = true;
@@ -125,8 +135,9 @@ __global__ void __launch_bounds__(LEAN ? 384 : 256, 1) k3_wtile(RowPtrs<R> f, Co
   const bool special = __any_sync(0xffffffffu, flag != 0u);
   const SpecialIdx sx = special ? make_special<R, C, PML>(p, flag, rowg * C, g, owner) : SpecialIdx();
   const WarpSpecial ws = special ? make_warp_special<R, C, PML>(p, sx) : WarpSpecial();
-  SourceStream<R> src;
-  src.start(p, special && __any_sync(0xffffffffu, (flag & F_SRC) != 0u), p.n0, lane);
+  SourceRound<R> src;           // the round's source samples in the warp's strip behind the halo slots
+  src.start(p, special && __any_sync(0xffffffffu, (flag & F_SRC) != 0u), p.n0, lane, q.T,
+            slots + 2u * par_bytes + (uint32_t)warp * SourceRound<R>::kBytesPerWarp);
 
   // where this lane's row goes after a round: lanes HR..2HR-1 are the right halo of tile-1, lanes 32-2HR..32-HR-1 the left
   // halo of tile+1; and where its own halo row arrives
@@ -149,8 +160,12 @@ __global__ void __launch_bounds__(LEAN ? 384 : 256, 1) k3_wtile(RowPtrs<R> f, Co
   if constexpr (CLUSTER) cluster_barrier();       // every CTA of the cluster is resident before the first remote store
 
   uint32_t par = 0u;
+  [[maybe_unused]] int rnd = -1;
   for (int64_t n = 0; n < q.nsteps; n += q.T) {
     const int Tr = (int)(q.nsteps - n < q.T ? q.nsteps - n : q.T);
+    ++rnd;
+    K3W_STAMP(0);
+    if (n > 0) src.next_round(p, p.n0 + n, lane);
     if (active) {
       if constexpr (LEAN) {
         if (warp_uniform) warp_round_lean<R, C>(E, H, J, cu, p, sx, ws, src, p.n0 + n, Tr);
@@ -159,6 +174,7 @@ __global__ void __launch_bounds__(LEAN ? 384 : 256, 1) k3_wtile(RowPtrs<R> f, Co
         warp_round<PML, R, C>(E, H, J, cf_regs, p, sx, ws, src, p.n0 + n, Tr);
       }
     }
+    K3W_STAMP(1);
     if (n + Tr >= q.nsteps) break;
     // halo refresh: double-buffered by round parity, so one barrier per round is enough (a warp can overwrite buffer
     // `par` again only after the NEXT barrier, which every reader of this round's data has passed its reads to reach)
@@ -174,7 +190,9 @@ __global__ void __launch_bounds__(LEAN ? 384 : 256, 1) k3_wtile(RowPtrs<R> f, Co
         }
       }
     }
+    K3W_STAMP(2);
     if constexpr (CLUSTER) cluster_barrier(); else cta_barrier();
+    K3W_STAMP(3);
     if (recv_left || recv_right) {
       const uint32_t a = recv_addr + par * par_bytes;
 #pragma unroll
@@ -186,6 +204,7 @@ __global__ void __launch_bounds__(LEAN ? 384 : 256, 1) k3_wtile(RowPtrs<R> f, Co
       }
     }
     par ^= 1u;
+    K3W_STAMP(4);
   }
 
   if (owner) {
@@ -205,27 +224,31 @@ static int tiles_for(int64_t rows, int RO) { return (int)((rows + RO - 1) / RO);
 // fewer warp tiles in the whole batch than four per SM: latency, not throughput, decides
 bool k3w_few_grids(const Layout &L, int sms) { return L.nbatch * ((L.nrows + 29) / 30) < (int64_t)sms * 4; }
 
-bool k3w_plan(const Layout &L, int depth, int sms, int64_t want_nw, int64_t want_nc, int64_t want_k, bool lean, K3WPlan *out) {
+bool k3w_plan(const Layout &L, int depth, int sms, int64_t want_nw, int64_t want_nc, int64_t want_k, bool lean, bool half, K3WPlan *out) {
   K3WPlan P;
+  if (half && lean) return false;
   P.lean = lean;
+  P.half = half;
+  const int Cl = half ? L.C / 2 : L.C;                 // nodes per lane
+  const int64_t nrows = half ? 2 * L.nrows : L.nrows;   // lane rows per grid
   // default depth: one halo row (8 steps per round in fp64, 16 in fp32) when many grids keep the SMs busy; two halo
   // rows when a few grids are a chain of dependent rounds, where halving the number of barriers pays for the wider
   // halo (config 1: 1.55 against 1.76 ms)
   const bool few = k3w_few_grids(L, sms);
   P.T = depth > 0 ? depth : (few ? 2 * L.C : L.C);
-  P.HR = (P.T + L.C - 1) / L.C;
+  P.HR = (P.T + Cl - 1) / Cl;
   if (P.HR > kMaxHR) return false;
   P.rows_out = 32 - 2 * P.HR;
   // 8 warps per CTA: the feature variants of the time loop need up to 242 registers, and a scheduler's 16 K registers
   // then hold two warps (12 warps would need <= 168 and spill); 4 warps per SM already saturate the FP64 pipe with this
   // instruction mix (profiles/r02_peaks.md).  16 = largest (non-portable) cluster.
   const int maxw = lean ? 12 : 8, maxc = 16;       // (the lean instantiation: 168 registers, three warps per scheduler)
-  if (L.nrows > (int64_t)maxw * maxc * P.rows_out) return false;
-  const int w1 = tiles_for(L.nrows, P.rows_out);       // tiles of one grid
+  if (nrows > (int64_t)maxw * maxc * P.rows_out) return false;
+  const int w1 = tiles_for(nrows, P.rows_out);       // tiles of one grid
   int k = 1, nc = 1, nw = w1;
   if (want_nw > 0 || want_nc > 0 || want_k > 0) {      // explicit (rketd_set_plan)
     k = (int)std::max<int64_t>(1, want_k);
-    const int w = tiles_for(k * L.nrows, P.rows_out);
+    const int w = tiles_for(k * nrows, P.rows_out);
     nw = (int)want_nw;
     nc = want_nc > 0 ? (int)want_nc : (nw > 0 ? (w + nw - 1) / nw : (w + maxw - 1) / maxw);
     if (nw <= 0) nw = (w + nc - 1) / nc;
@@ -244,12 +267,12 @@ bool k3w_plan(const Layout &L, int depth, int sms, int64_t want_nw, int64_t want
     double best = -1.0;
     for (int c = 1; c <= 4; ++c)
       for (int kk = 1; kk <= 256 && kk <= L.nbatch; ++kk) {
-        const int w = tiles_for(kk * L.nrows, P.rows_out);
+        const int w = tiles_for(kk * nrows, P.rows_out);
         const int n = (w + c - 1) / c;
         if (n > maxw) break;
         if (c > 1 && w <= (c - 1) * maxw) continue;          // fits a smaller cluster
         const int cap = lean ? 12 : 8;                        // warps an SM holds at this kernel's register count
-        const double score = (double)(kk * L.nrows) / (32.0 * n * c) * ((double)((cap / n) * n) / cap) * (c > 1 ? 0.97 : 1.0);
+        const double score = (double)(kk * nrows) / (32.0 * n * c) * ((double)((cap / n) * n) / cap) * (c > 1 ? 0.97 : 1.0);
         if (score > best + 1e-9) { best = score; k = kk; nc = c; nw = n; }
       }
     if (best < 0.0) {                                    // a grid needs more than 4 SMs: warps spread evenly over a cluster
@@ -259,26 +282,27 @@ bool k3w_plan(const Layout &L, int depth, int sms, int64_t want_nw, int64_t want
   }
   if (nw > maxw || nc > maxc || nw < 1 || nc < 1) return false;
   P.k = k; P.nc = nc; P.nw = nw;
-  P.chunk_rows = k * L.nrows;
+  P.chunk_rows = k * nrows;
   if (P.chunk_rows > 0x7fffff00LL) return false;
   P.tiles_per_chunk = tiles_for(P.chunk_rows, P.rows_out);
   P.nchunks = (L.nbatch + k - 1) / k;
-  P.smem_bytes = 2u * (uint32_t)nw * slot_bytes_per_warp() + (lean ? 1024u + (uint32_t)nw * kNumCoef * 32u * kRowBytes : 0u);
+  P.smem_bytes = 2u * (uint32_t)nw * slot_bytes_per_warp() + (uint32_t)nw * 64u * (uint32_t)sizeof(double) +      // halo slots, source strips
+                 (lean ? 1024u + (uint32_t)nw * kNumCoef * 32u * kRowBytes : 0u);
   *out = P;
   return true;
 }
 
-template <typename R, bool CLUSTER, bool PML, bool LEAN>
+template <typename R, bool CLUSTER, bool PML, bool LEAN, bool HALF = false>
 static cudaError_t launch_k3w_k(const Layout &L, const K3WPlan &P, FieldPtrs f, void *const coef[kNumCoef], const StepCommon &sc,
                                 int64_t nsteps, cudaStream_t st) {
-  auto kern = k3_wtile<R, CLUSTER, PML, LEAN>;
+  auto kern = k3_wtile<R, CLUSTER, PML, LEAN, HALF>;
   if (P.smem_bytes > 48 * 1024) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P.smem_bytes);
     if (e != cudaSuccess) return e;
   }
   K3WArgs q;
   q.T = P.T; q.HR = P.HR; q.rows_out = P.rows_out; q.cluster = P.nc; q.chunk_rows = (int)P.chunk_rows;
-  q.tiles_per_chunk = P.tiles_per_chunk; q.nrows = L.nrows; q.total_rows = L.nrows * L.nbatch; q.nsteps = nsteps;
+  q.tiles_per_chunk = P.tiles_per_chunk; q.nrows = (HALF ? 2 : 1) * L.nrows; q.total_rows = q.nrows * L.nbatch; q.nsteps = nsteps;
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)(P.nchunks * P.nc));
   cfg.blockDim = dim3((unsigned)P.nw * 32);
@@ -300,6 +324,10 @@ template <typename R>
 static cudaError_t launch_k3w_t(const Layout &L, const K3WPlan &P, FieldPtrs f, void *const coef[kNumCoef], const StepCommon &sc,
                                 int64_t nsteps, cudaStream_t st) {
   const bool pml = sc.npml > 0;
+  if (P.half) {                                  // (clusters only: one instantiation per type; a cluster of one CTA is fine)
+    if (pml || P.lean) return cudaErrorInvalidValue;
+    return launch_k3w_k<R, true, false, false, true>(L, P, f, coef, sc, nsteps, st);
+  }
   if (P.lean && !pml)
     return P.nc > 1 ? launch_k3w_k<R, true, false, true>(L, P, f, coef, sc, nsteps, st) : launch_k3w_k<R, false, false, true>(L, P, f, coef, sc, nsteps, st);
   if (P.nc > 1) return pml ? launch_k3w_k<R, true, true, false>(L, P, f, coef, sc, nsteps, st) : launch_k3w_k<R, true, false, false>(L, P, f, coef, sc, nsteps, st);
@@ -313,7 +341,7 @@ cudaError_t launch_k3w(int dtype, const Layout &L, const K3WPlan &P, FieldPtrs f
 // can a cluster of P.nc CTAs of this kernel be co-scheduled at all on this device?
 template <typename R>
 static cudaError_t k3w_max_clusters_t(const K3WPlan &P, int *nclusters) {
-  auto kern = P.lean ? k3_wtile<R, true, false, true> : k3_wtile<R, true, false, false>;
+  auto kern = P.half ? k3_wtile<R, true, false, false, true> : P.lean ? k3_wtile<R, true, false, true> : k3_wtile<R, true, false, false>;
   if (P.smem_bytes > 48 * 1024) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P.smem_bytes);
     if (e != cudaSuccess) return e;
@@ -337,3 +365,9 @@ cudaError_t k3w_max_clusters(int dtype, const K3WPlan &P, int *nclusters) {
 }
 
 }  // namespace rketd
+
+#ifdef RKETD_K3W_TRACE
+extern "C" int rketd_debug_k3w_trace(long long *out, int n) {
+  return (int)cudaMemcpyFromSymbol(out, rketd::g_k3w_trace, sizeof(long long) * n);
+}
+#endif

@@ -48,9 +48,9 @@ __device__ __forceinline__ void warp_step(const R (&E)[C], R (&En)[C], R (&H)[C]
   Er = __shfl_down_sync(0xffffffffu, En[0], 1);
 }
 
-template <int MASK, bool PML, typename R, int C>
+template <int MASK, bool PML, typename R, int C, typename SRCT>
 __device__ __forceinline__ void warp_steps(R (&E)[C], R (&H)[C], R (&G)[C], const CoefRegs<R, C> &cf, const StepParams<R> &p,
-                                           const SpecialIdx &sx, const WarpSpecial &ws, SourceStream<R> &src, int64_t nloc,
+                                           const SpecialIdx &sx, const WarpSpecial &ws, SRCT &src, int64_t nloc,
                                            int nsteps) {
   constexpr bool SRC = MASK == SF_SLOW || (MASK & SF_SRC) != 0;
   const R nchh = p.nchh;       // stays a constant-bank operand of the FMAs (one register read less each)
@@ -111,9 +111,9 @@ __device__ __forceinline__ void warp_time_loop(R (&E)[C], R (&H)[C], R (&G)[C], 
 // T steps of a warp tile between two halo refreshes of the resident kernel: the step counter, the special indices
 // and the source stream belong to the caller and live across rounds (restarting the stream would put two global
 // loads on the critical path of every round).  One instantiation per feature set, chosen here once per round.
-template <bool PML, typename R, int C>
+template <bool PML, typename R, int C, typename SRCT>
 __device__ __forceinline__ void warp_round(R (&E)[C], R (&H)[C], R (&G)[C], const CoefRegs<R, C> &cf, const StepParams<R> &p,
-                                           const SpecialIdx &sx, const WarpSpecial &ws, SourceStream<R> &src, int64_t nloc,
+                                           const SpecialIdx &sx, const WarpSpecial &ws, SRCT &src, int64_t nloc,
                                            int nsteps) {
 #define RKETD_ROUND_CASE(M) case M: warp_steps<M, false, R, C>(E, H, G, cf, p, sx, ws, src, nloc, nsteps); break;
   if (PML || ws.mask == SF_SLOW) {
@@ -205,9 +205,9 @@ __device__ __forceinline__ void warp_step_lean(R (&E)[C], R (&H)[C], R (&G)[C], 
   Er = __shfl_down_sync(0xffffffffu, E[0], 1);
 }
 
-template <int MASK, typename R, int C, typename CF>
+template <int MASK, typename R, int C, typename CF, typename SRCT>
 __device__ __forceinline__ void warp_steps_lean(R (&E)[C], R (&H)[C], R (&G)[C], const CF &cf, const StepParams<R> &p,
-                                                const SpecialIdx &sx, const WarpSpecial &ws, SourceStream<R> &src,
+                                                const SpecialIdx &sx, const WarpSpecial &ws, SRCT &src,
                                                 int64_t nloc, int nsteps) {
   const R nchh = p.nchh;
   const int lane = threadIdx.x & 31;
@@ -227,9 +227,9 @@ __device__ __forceinline__ void warp_steps_lean(R (&E)[C], R (&H)[C], R (&G)[C],
   if constexpr (MASK != 0) zero_padding_H<R, C>(H, ws);
 }
 
-template <typename R, int C, typename CF>
+template <typename R, int C, typename CF, typename SRCT>
 __device__ __forceinline__ void warp_round_lean(R (&E)[C], R (&H)[C], R (&G)[C], const CF &cf, const StepParams<R> &p,
-                                                const SpecialIdx &sx, const WarpSpecial &ws, SourceStream<R> &src,
+                                                const SpecialIdx &sx, const WarpSpecial &ws, SRCT &src,
                                                 int64_t nloc, int nsteps) {
 #define RKETD_LEAN_CASE(M) case M: warp_steps_lean<M, R, C>(E, H, G, cf, p, sx, ws, src, nloc, nsteps); break;
   switch (ws.mask) {

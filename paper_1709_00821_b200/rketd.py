@@ -34,6 +34,7 @@ PEAK_NAMES = ("dfma_1reg", "dfma_2reg", "dfma_3reg", "dfma_2reg_const", "ffma_1r
               "ffma_2reg_const", "mix_f64", "mix_f32", "lds128", "lat_dfma", "lat_shfl64", "lat_step_f64", "lat_step_f32",
               "lat_bar_sync_256", "lat_cluster_barrier_8x128")      # index = RKETD_PEAK_* / RKETD_LAT_*
 RESIDENT_WTILE_FLAG = 0x40000000
+RESIDENT_WTILE_NOLEAN, RESIDENT_WTILE_LEAN, RESIDENT_WTILE_HALF, RESIDENT_WTILE_NOHALF = 0x20000000, 0x10000000, 0x08000000, 0x04000000
 
 
 def RESIDENT_WTILE(nw: int = 0, nc: int = 0, k: int = 0) -> int:

@@ -71,6 +71,7 @@ def WT(nw=0, nc=0, k=0):
 
 
 LEAN, NOLEAN = 0x10000000, 0x20000000      # the 168- / 232-register instantiation of k3_wtile (default: by batch size)
+HALF, NOHALF = 0x08000000, 0x04000000      # a lane holds half a 64-B row / a whole one (default: half rows for a few grids)
 
 
 # K1; the resident kernel K3: warp tiles with the library's packing at several depths (steps between halo refreshes),
@@ -78,6 +79,7 @@ LEAN, NOLEAN = 0x10000000, 0x20000000      # the 168- / 232-register instantiati
 ALL_PLANS = [(1, 0, -1)] + [(3, d, -1) for d in (0, 1, 3, 8, 13, 16)] + \
             [(3, 8, WT(8, 2)), (3, 8, WT(5, 2)), (3, 8, WT(1, 9)), (3, 5, WT(2, 5)), (3, 16, WT(4, 3)), (3, 0, WT(3, 3))] + \
             [(3, 8, WT(8, 2) | LEAN), (3, 7, WT(9, 1) | LEAN), (3, 16, WT(2, 5) | LEAN), (3, 0, WT(3, 3) | LEAN), (3, 0, WT(5, 2) | NOLEAN)] + \
+            [(3, 16, WT() | HALF), (3, 8, WT(3, 0) | HALF), (3, 4, WT(8, 0) | HALF), (3, 13, WT(2, 11) | HALF), (3, 0, WT() | NOHALF), (3, 5, WT() | NOHALF)] + \
             [(3, 0, 0), (3, 0, 2)] + [(2, 0, v) for v in (0, 2, 6)] + [(2, d, 0) for d in (1, 7, 16, 33)] + \
             [(2, d, 6) for d in (1, 2, 9, 32, 40)] + [(2, 5, 0), (2, 40, 2)]
 
@@ -278,7 +280,8 @@ def test_config5_reduced_dft(rk, dtype):
     # one-barrier-per-step kernel
     for depth, variant in [(0, -1), (0, WT(0, 1, 1)), (0, WT(0, 2, 2)), (0, WT(0, 2, 3)), (0, WT(0, 3, 4)), (0, WT(0, 3, 5)),
                            (0, WT(0, 4, 7)), (3, WT(0, 2, 2)), (0, 0), (0, 2),
-                           (0, WT(0, 1, 1) | LEAN), (0, WT(0, 1, 2) | LEAN), (5, WT(0, 2, 5) | LEAN), (0, WT(0, 1, 1) | NOLEAN)]:
+                           (0, WT(0, 1, 1) | LEAN), (0, WT(0, 1, 2) | LEAN), (5, WT(0, 2, 5) | LEAN), (0, WT(0, 1, 1) | NOLEAN),
+                           (0, WT(0, 0, 1) | HALF), (5, WT(0, 6, 5) | HALF), (0, WT(8, 0, 2) | HALF)]:
         g = run_gpu(rk, w2, dtype, 3, depth, variant)
         assert grid_err(g["rec"], ref2["rec"]) <= TOL[dtype], (depth, variant)
         check_fields(g, ref2["state"], TOL[dtype], *floors_of(w2, ref2))
@@ -310,6 +313,7 @@ def test_small_and_ragged_grids(rk, ncells):
         if ncells > 300:
             plans += [(3, 0, WT(0, 3, 1)), (3, 0, WT(2, 0, 1)), (3, 2, WT(0, 0, 3)), (3, 0, WT(0, 0, 3) | LEAN)]
         plans += [(3, 0, WT(0, 0, 1) | LEAN), (3, 3, WT(0, 0, 2) | LEAN)]
+        plans += [(3, 0, WT(0, 0, 2) | HALF), (3, 3, WT(0, 0, 3) | HALF), (3, 0, WT() | NOHALF)]
         for kernel, depth, variant in plans:
             s = rk.Sim(ncells, nb, wl.DZ, wl.DT, "f64")
             s.set_media(wp, nu)
