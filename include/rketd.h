@@ -227,6 +227,26 @@ enum {
 };
 int rketd_measure_peak(int what, int iters, double *out, void *cuda_stream);
 
+/* Row a7 for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): probe records -> DFT magnitudes in ONE call that allocates nothing and does not synchronise
+ * (the records' "Fourier transform"; the definition of rketd_set_probe_dft):
+ *   out[s][m] = | sum_{n < nsamples} rec[s][n] exp(-j 2 pi f_m (step0 + n + 1) dt) |,  sums in fp64.
+ * rec [nseries][nsamples] and out [nseries][nfreq] in `dtype` (the layout rketd_read_probes gives with nseries =
+ * nbatch x nprobes; step0 = step index of sample 0, 0 for a record from the start), freqs_hz [nfreq] fp64 — all three in
+ * DEVICE memory of the current device, owned by the caller; cuda_stream as in rketd_create.  The twiddle table lives in a
+ * static device array of RKETD_NOALLOC_MAX_TWIDDLES entries (8 MiB on every GPU that loads the library, until exit),
+ * shared by all calls: a call rewrites what it reads, so nothing needs clearing, but calls that OVERLAP on the GPU
+ * (different streams without ordering) race on it.  EINVAL (text: rketd_noalloc_last_error): bad dtype, negative size,
+ * dt <= 0, NULL or host pointers, nsamples x nfreq > RKETD_NOALLOC_MAX_TWIDDLES, nseries > RKETD_NOALLOC_MAX_SERIES;
+ * ECUDA: no device / launch failure.  nseries = 0 or nfreq = 0: nothing to do, OK. */
+#define RKETD_NOALLOC_MAX_TWIDDLES (1 << 19)
+#define RKETD_NOALLOC_MAX_SERIES (1 << 24)
+int rketd_probe_dft_noalloc(int dtype, const void *rec, int64_t nseries, int64_t nsamples, int64_t step0, double dt,
+                            const double *freqs_hz, int nfreq, void *out, void *cuda_stream);
+
+/* Text of the calling thread's last failed rketd_probe_dft_noalloc ("" if none). */
+const char *rketd_noalloc_last_error(void);
+
 void rketd_destroy(rketd_sim *s);
 
 /* Text of the last error on this handle (or of the last failed rketd_create when s is NULL). */

@@ -28,7 +28,7 @@ EXPORTS = ["rketd_create", "rketd_set_media", "rketd_set_source", "rketd_set_pro
            "rketd_read_probes",
            "rketd_get_fields", "rketd_get_coefficients", "rketd_get_kernel_coefficients", "rketd_set_scheme",
            "rketd_set_boundary", "rketd_read_probe_dft",
-           "rketd_read_sweep_rt", "rketd_measure_peak",
+           "rketd_read_sweep_rt", "rketd_measure_peak", "rketd_probe_dft_noalloc", "rketd_noalloc_last_error",
            "rketd_get_counter", "rketd_destroy", "rketd_last_error"]
 PEAK_NAMES = ("dfma_1reg", "dfma_2reg", "dfma_3reg", "dfma_2reg_const", "ffma_1reg", "ffma_2reg", "ffma_3reg",
               "ffma_2reg_const", "mix_f64", "mix_f32", "lds128", "lat_dfma", "lat_shfl64", "lat_step_f64", "lat_step_f32",
@@ -77,6 +77,10 @@ _lib.rketd_last_error.argtypes = [_vp]
 _lib.rketd_last_error.restype = ctypes.c_char_p
 _lib.rketd_measure_peak.argtypes = [_i32, _i32, _vp, _vp]
 _lib.rketd_read_sweep_rt.argtypes = [_vp, _vp, _i32, _i32, _vp, _vp, _i64]
+_lib.rketd_probe_dft_noalloc.argtypes = [_i32, _vp, _i64, _i64, _i64, _dbl, _vp, _i32, _vp, _vp]
+_lib.rketd_probe_dft_noalloc.restype = _i32
+_lib.rketd_noalloc_last_error.argtypes = []
+_lib.rketd_noalloc_last_error.restype = ctypes.c_char_p
 for _n in EXPORTS[:19]:
     getattr(_lib, _n).restype = _i32
 
@@ -202,6 +206,22 @@ def rketd_measure_peak(what: int, iters: int = 4000, cuda_stream: int = 0):
     _check(None, _lib.rketd_measure_peak(what, iters, _ptr(out), cuda_stream or None))
     return {"name": PEAK_NAMES[what], "per_ns": float(out[0]), "per_clk_sm": float(out[1]), "sm_mhz": float(out[2]),
             "sms": int(out[3])}
+
+
+NOALLOC_MAX_TWIDDLES, NOALLOC_MAX_SERIES = 1 << 19, 1 << 24
+
+
+def rketd_probe_dft_noalloc(dtype: int, rec, nseries: int, nsamples: int, step0: int, dt: float, freqs_hz, nfreq: int, out,
+                            cuda_stream: int = 0):
+    """records -> |DFT| without any allocation (include/rketd.h); rec, freqs_hz, out: DEVICE tensors or raw addresses"""
+    rc = _lib.rketd_probe_dft_noalloc(dtype, _ptr(rec), nseries, nsamples, step0, dt, _ptr(freqs_hz), nfreq, _ptr(out),
+                                      cuda_stream or None)
+    if rc != OK:
+        raise RketdError(rc, rketd_noalloc_last_error())
+
+
+def rketd_noalloc_last_error() -> str:
+    return (_lib.rketd_noalloc_last_error() or b"").decode()
 
 
 def rketd_destroy(h):
