@@ -453,7 +453,8 @@ __device__ __forceinline__ void step_special(const R (&E)[C], R (&En)[C], R (&H)
 // right, source, probes) and the same bits as step_special.  H behind the last node and left of node 0 is zeroed once
 // at the end (zero_padding_H) instead of every step: those values feed only nodes that Mur rewrites or whose
 // coefficients are zero.
-enum : int { SF_MURL = 1, SF_MURR = 2, SF_SRC = 4, SF_PROBE = 8, SF_SLOW = 16 };
+enum : int { SF_MURL = 1, SF_MURR = 2, SF_SRC = 4, SF_PROBE = 8, SF_SLOW = 16,
+              SF_FAST = 32 };   // with feature bits: every feature of the warp sits at a fixed local index (WarpSpecial::fast)
 
 struct WarpSpecial {
   int mask = 0;                       // SF_* of the warp tile (warp-uniform)
@@ -462,6 +463,8 @@ struct WarpSpecial {
   uint32_t mHz = 0;                   // bit i: H of local node i is padding (behind node ncells-1, or left of node 0)
   bool l_p0 = false, l_p1 = false;    // this lane records one / two probes
   bool two_probes = false;            // some lane of the warp records two (warp-uniform)
+  int fast = 0;                       // SF_* bits (warp-uniform): the feature sits at the one local index a lane can name
+                                      // without a search — node ncells-1 last in its lane, the source / every probe first
 };
 
 template <typename R, int C, bool PML>
@@ -474,6 +477,8 @@ __device__ __forceinline__ WarpSpecial make_warp_special(const StepParams<R> &p,
   ws.mHz = (sx.iR >= 0 ? (0xffffffffu << sx.iR) & ((1u << C) - 1u) : 0u) | (sx.iL == 1 ? 1u : 0u);
   ws.l_p0 = sx.np >= 1 && sx.np <= 2; ws.l_p1 = sx.np == 2;
   ws.two_probes = __any_sync(full, ws.l_p1);
+  ws.fast = (__any_sync(full, sx.iR >= 0 && sx.iR != C - 1) ? 0 : SF_MURR) | (__any_sync(full, sx.iS > 0) ? 0 : SF_SRC) |
+            ((ws.two_probes || __any_sync(full, ws.l_p0 && sx.pi0 != 0)) ? 0 : SF_PROBE);
   ws.mask = (__any_sync(full, sx.iL >= 0) ? SF_MURL : 0) | (__any_sync(full, sx.iR >= 0) ? SF_MURR : 0) |
             (__any_sync(full, sx.iS >= 0) ? SF_SRC : 0) | (__any_sync(full, ws.l_p0) ? SF_PROBE : 0);
   // an absorbing layer, or more than two probes among one lane's nodes: the general per-lane path
@@ -502,6 +507,28 @@ template <int MASK, typename R, int C, bool GUARD = false>
 __device__ __forceinline__ void special_select(const R (&E)[C], R (&En)[C], const StepParams<R> &p, const SpecialIdx &sx,
                                                const WarpSpecial &ws, int64_t nloc, R src_now) {
   typedef Arith<R> A;
+  if constexpr ((MASK & SF_FAST) != 0) {
+    // Every feature at a fixed local index (node ncells-1 last in its lane, the source and every probe first, at most one
+    // probe per lane): one candidate each, turned into a select by the lane's own bits; no branch and no search.  This is
+    // every BASELINE config (grid lengths, source and probe cells are multiples of the row).  Same expressions on the same
+    // operands as below, in the same order.
+    if constexpr ((MASK & SF_MURL) != 0) {
+      const R c0 = A::fma(p.mur_m, A::sub(En[1], E[0]), E[1]);
+      const R c1 = A::fma(p.mur_m, A::sub(En[2], E[1]), E[2]);
+      En[0] = ws.mL0 ? c0 : En[0];
+      En[1] = ws.mL1 ? c1 : En[1];
+    }
+    if constexpr ((MASK & SF_MURR) != 0) {
+      const R cand = A::fma(p.mur_m, A::sub(En[C - 2], E[C - 1]), E[C - 2]);
+      En[C - 1] = ((ws.mR >> (C - 1)) & 1u) ? cand : En[C - 1];
+    }
+    if constexpr ((MASK & SF_SRC) != 0) {
+      const R sum = A::add(En[0], src_now);
+      En[0] = (ws.mS & 1u) ? sum : En[0];
+    }
+    if constexpr ((MASK & SF_PROBE) != 0) stg_if(ws.l_p0, p.rec + (sx.pr0 + nloc), En[0]);
+    return;
+  }
   if constexpr ((MASK & SF_MURL) != 0) {      // node 0 sits at local index 0 or 1 (Layout: off), node 1 in the same row
     const R c0 = A::fma(p.mur_m, A::sub(En[1], E[0]), E[1]);
     const R c1 = A::fma(p.mur_m, A::sub(En[2], E[1]), E[2]);
@@ -510,7 +537,12 @@ __device__ __forceinline__ void special_select(const R (&E)[C], R (&En)[C], cons
   }
   if constexpr ((MASK & SF_MURR) != 0) {      // node ncells-1 at local index >= 1, node ncells-2 in the same row
     // (descending, so that every candidate sees the interior value of its inward neighbour; one bit of mR is set at most)
-    if (!GUARD || (ws.mask & SF_MURR)) {
+    // GUARD: grids whose length is a multiple of the row (every BASELINE config) hold node ncells-1 last in its lane: one
+    // candidate instead of C - 1 (the same expression on the same operands: the same bits)
+    if (GUARD && (ws.mask & SF_MURR) && (ws.fast & SF_MURR)) {
+      const R cand = A::fma(p.mur_m, A::sub(En[C - 2], E[C - 1]), E[C - 2]);
+      En[C - 1] = ((ws.mR >> (C - 1)) & 1u) ? cand : En[C - 1];
+    } else if (!GUARD || (ws.mask & SF_MURR)) {
 #pragma unroll
       for (int i = C - 1; i >= 1; --i) {
         const R cand = A::fma(p.mur_m, A::sub(En[i - 1], E[i]), E[i - 1]);
@@ -519,7 +551,10 @@ __device__ __forceinline__ void special_select(const R (&E)[C], R (&En)[C], cons
     }
   }
   if constexpr ((MASK & SF_SRC) != 0) {
-    if (!GUARD || (ws.mask & SF_SRC)) {
+    if (GUARD && (ws.mask & SF_SRC) && (ws.fast & SF_SRC)) {      // the source node is the first of its lane
+      const R sum = A::add(En[0], src_now);
+      En[0] = (ws.mS & 1u) ? sum : En[0];
+    } else if (!GUARD || (ws.mask & SF_SRC)) {
 #pragma unroll
       for (int i = 0; i < C; ++i) {
         const R sum = A::add(En[i], src_now);
@@ -532,6 +567,8 @@ __device__ __forceinline__ void special_select(const R (&E)[C], R (&En)[C], cons
       const R v0 = select_node<R, C>(En, sx.pi0), v1 = select_node<R, C>(En, sx.pi1);
       stg_if(ws.l_p0, p.rec + (sx.pr0 + nloc), v0);
       stg_if(ws.l_p1, p.rec + (sx.pr1 + nloc), v1);
+    } else if ((ws.mask & SF_PROBE) && (ws.fast & SF_PROBE)) {      // every probe of the warp is the first node of its lane
+      stg_if(ws.l_p0, p.rec + (sx.pr0 + nloc), En[0]);
     } else if (ws.mask & SF_PROBE) {
       const R v0 = select_node<R, C>(En, sx.pi0);
       stg_if(ws.l_p0, p.rec + (sx.pr0 + nloc), v0);
@@ -637,6 +674,37 @@ template <typename R, int NW>
 __device__ __forceinline__ void recv_halo(const HaloSlots<R, NW> &hs, int par, int warp, int lane, R &El, R &Hl,
                                           R &Er) {
   const R a = hs.e_last[par][warp], b = hs.h_last[par][warp], c = hs.e_first[par][warp + 2];
+  El = lane == 0 ? a : El;
+  Hl = lane == 0 ? b : Hl;
+  Er = lane == 31 ? c : Er;
+}
+
+// The same exchange through a 32-bit shared-space address held in a register (wa = address of HaloSlots + warp * sizeof(R),
+// taken once before the time loop).  Through the struct reference the compiler rebuilds the generic address of the slots at
+// every access (S2UR SR_CgaCtaId + ULEA, 25 cycles of latency three times per step: 8 % of all stall samples of config 5
+// fp32, profiles/r02_ncu_k3.md).
+template <typename R, int NW>
+__device__ __forceinline__ constexpr uint32_t halo_off(int array, int par, int w) {
+  return (uint32_t)(((array * 2 + par) * (NW + 2) + w) * (int)sizeof(R));
+}
+template <typename R, int C, int NW>
+__device__ __forceinline__ void send_halo_a(const R (&E)[C], const R (&H)[C], uint32_t wa, int par, int lane, R &El, R &Hl,
+                                            R &Er) {
+  El = __shfl_up_sync(0xffffffffu, E[C - 1], 1);
+  Hl = __shfl_up_sync(0xffffffffu, H[C - 1], 1);
+  Er = __shfl_down_sync(0xffffffffu, E[0], 1);
+  if (lane == 0) sts_scalar(wa + halo_off<R, NW>(0, par, 1), E[0]);
+  if (lane == 31) {
+    sts_scalar(wa + halo_off<R, NW>(1, par, 1), E[C - 1]);
+    sts_scalar(wa + halo_off<R, NW>(2, par, 1), H[C - 1]);
+  }
+}
+template <typename R, int NW>
+__device__ __forceinline__ void recv_halo_a(uint32_t wa, int par, int lane, R &El, R &Hl, R &Er) {
+  R a, b, c;
+  lds_scalar(wa + halo_off<R, NW>(1, par, 0), a);
+  lds_scalar(wa + halo_off<R, NW>(2, par, 0), b);
+  lds_scalar(wa + halo_off<R, NW>(0, par, 2), c);
   El = lane == 0 ? a : El;
   Hl = lane == 0 ? b : Hl;
   Er = lane == 31 ? c : Er;

@@ -20,6 +20,7 @@
 // Mur boundaries, the soft source and probe recording are folded into the rows that hold
 // those nodes (rowflag) inside the same kernels — see step_fields in rketd_device.cuh.
 #include <algorithm>
+#include <cstddef>
 
 #include "rketd_device.cuh"
 #include "rketd_internal.h"
@@ -68,17 +69,21 @@ __device__ __forceinline__ void time_loop(R (&E)[C], R (&H)[C], R (&J)[C], const
   const R nchh = pin_register(p.nchh);
   int64_t nloc = p.n0;
   R El, Hl, Er;
-  send_halo<R, C, NW>(E, H, hs, 0, warp, lane, El, Hl, Er);
+  typedef HaloSlots<R, NW> HS;
+  static_assert(offsetof(HS, e_first) == 0 && offsetof(HS, e_last) == 2 * (NW + 2) * sizeof(R) &&
+                    offsetof(HS, h_last) == 4 * (NW + 2) * sizeof(R), "halo_off assumes this layout");
+  const uint32_t wa = pin_register(smem_u32(&hs) + (uint32_t)warp * (uint32_t)sizeof(R));
+  send_halo_a<R, C, NW>(E, H, wa, 0, lane, El, Hl, Er);
   cta_barrier();
-  recv_halo<R, NW>(hs, 0, warp, lane, El, Hl, Er);
+  recv_halo_a<R, NW>(wa, 0, lane, El, Hl, Er);
   R Eb[C];
   auto one_step = [&](const R (&Ein)[C], R (&Eout)[C], int par) {
     const R src_now = SRC ? src.sample(p, nloc, lane) : R(0);
     step_fields<MASK, PML, R, C, CF, true>(Ein, Eout, H, J, cf, El, Hl, Er, nchh, p, sx, ws, nloc, src_now);
-    send_halo<R, C, NW>(Eout, H, hs, par, warp, lane, El, Hl, Er);     // for the next step
+    send_halo_a<R, C, NW>(Eout, H, wa, par, lane, El, Hl, Er);     // for the next step
     step_current<R, C>(J, Ein, cf);
     cta_barrier();
-    recv_halo<R, NW>(hs, par, warp, lane, El, Hl, Er);
+    recv_halo_a<R, NW>(wa, par, lane, El, Hl, Er);
     if (MASK != 0) ++nloc;
   };
   int64_t left = nsteps;
@@ -106,8 +111,12 @@ __device__ __forceinline__ void time_loop_dispatch(R (&E)[C], R (&H)[C], R (&J)[
   SourceStream<R> src;
   src.start(p, special && __any_sync(0xffffffffu, (flag & F_SRC) != 0u), p.n0, lane);
   constexpr int kMur = SF_MURL | SF_MURR, kSrcProbe = SF_SRC | SF_PROBE;
+  constexpr int kFastAll = SF_MURR | SF_SRC | SF_PROBE;
   if (PML || ws.mask == SF_SLOW) time_loop<SF_SLOW, PML, R, C, NW>(E, H, J, cf, hs, p, sx, ws, src, nsteps, warp, lane);
   else if (ws.mask == 0) time_loop<0, false, R, C, NW>(E, H, J, cf, hs, p, sx, ws, src, nsteps, warp, lane);
+  // every feature at a fixed local index (all BASELINE configs): straight-line selects, no branch in the step
+  else if (ws.fast == kFastAll && (ws.mask & SF_SRC)) time_loop<SF_FAST | kMur | kSrcProbe, false, R, C, NW>(E, H, J, cf, hs, p, sx, ws, src, nsteps, warp, lane);
+  else if (ws.fast == kFastAll) time_loop<SF_FAST | kMur | SF_PROBE, false, R, C, NW>(E, H, J, cf, hs, p, sx, ws, src, nsteps, warp, lane);
   else if ((ws.mask & kSrcProbe) == 0) time_loop<kMur, false, R, C, NW>(E, H, J, cf, hs, p, sx, ws, src, nsteps, warp, lane);
   else if ((ws.mask & kMur) == 0) time_loop<kSrcProbe, false, R, C, NW>(E, H, J, cf, hs, p, sx, ws, src, nsteps, warp, lane);
   else time_loop<kMur | kSrcProbe, false, R, C, NW>(E, H, J, cf, hs, p, sx, ws, src, nsteps, warp, lane);
