@@ -679,6 +679,12 @@ __device__ __forceinline__ void recv_halo(const HaloSlots<R, NW> &hs, int par, i
   Er = lane == 31 ? c : Er;
 }
 
+__device__ __forceinline__ void sts_if(bool pred, uint32_t a, double v) {
+  asm volatile("{\n.reg .pred p;\nsetp.ne.u32 p, %0, 0;\n@p st.shared.f64 [%1], %2;\n}\n" ::"r"((uint32_t)pred), "r"(a), "d"(v) : "memory");
+}
+__device__ __forceinline__ void sts_if(bool pred, uint32_t a, float v) {
+  asm volatile("{\n.reg .pred p;\nsetp.ne.u32 p, %0, 0;\n@p st.shared.f32 [%1], %2;\n}\n" ::"r"((uint32_t)pred), "r"(a), "f"(v) : "memory");
+}
 // The same exchange through a 32-bit shared-space address held in a register (wa = address of HaloSlots + warp * sizeof(R),
 // taken once before the time loop).  Through the struct reference the compiler rebuilds the generic address of the slots at
 // every access (S2UR SR_CgaCtaId + ULEA, 25 cycles of latency three times per step: 8 % of all stall samples of config 5
@@ -693,11 +699,9 @@ __device__ __forceinline__ void send_halo_a(const R (&E)[C], const R (&H)[C], ui
   El = __shfl_up_sync(0xffffffffu, E[C - 1], 1);
   Hl = __shfl_up_sync(0xffffffffu, H[C - 1], 1);
   Er = __shfl_down_sync(0xffffffffu, E[0], 1);
-  if (lane == 0) sts_scalar(wa + halo_off<R, NW>(0, par, 1), E[0]);
-  if (lane == 31) {
-    sts_scalar(wa + halo_off<R, NW>(1, par, 1), E[C - 1]);
-    sts_scalar(wa + halo_off<R, NW>(2, par, 1), H[C - 1]);
-  }
+  sts_if(lane == 0, wa + halo_off<R, NW>(0, par, 1), E[0]);            // predicated stores: no branch in the step
+  sts_if(lane == 31, wa + halo_off<R, NW>(1, par, 1), E[C - 1]);
+  sts_if(lane == 31, wa + halo_off<R, NW>(2, par, 1), H[C - 1]);
 }
 template <typename R, int NW>
 __device__ __forceinline__ void recv_halo_a(uint32_t wa, int par, int lane, R &El, R &Hl, R &Er) {
