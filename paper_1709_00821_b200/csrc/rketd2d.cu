@@ -232,6 +232,14 @@ __device__ __forceinline__ void ld_pair(const float *q, float &x, float &y) { co
 __device__ __forceinline__ void st_pair(double *q, double x, double y) { *reinterpret_cast<double2 *>(q) = make_double2(x, y); }
 __device__ __forceinline__ void st_pair(float *q, float x, float y) { *reinterpret_cast<float2 *>(q) = make_float2(x, y); }
 
+// predicated shared stores (no branch, no reconvergence point around the warp-edge posts of every iteration)
+__device__ __forceinline__ void st_pair_if(bool pred, uint32_t a, double x, double y) {
+  asm volatile("{\n.reg .pred q;\nsetp.ne.u32 q, %0, 0;\n@q st.shared.v2.f64 [%1], {%2, %3};\n}" ::"r"((uint32_t)pred), "r"(a), "d"(x), "d"(y) : "memory");
+}
+__device__ __forceinline__ void st_pair_if(bool pred, uint32_t a, float x, float y) {
+  asm volatile("{\n.reg .pred q;\nsetp.ne.u32 q, %0, 0;\n@q st.shared.v2.f32 [%1], {%2, %3};\n}" ::"r"((uint32_t)pred), "r"(a), "f"(x), "f"(y) : "memory");
+}
+
 // Rows of the eight input arrays arrive as 2-D tiled TMA boxes {strip columns, 1 row} (cp.async.bulk.tensor.2d, SASS UTMALDG):
 // one elected thread issues them, completion on the ring slot's mbarrier; columns and rows outside the grid are zero-filled
 // by the hardware (the tensor map's extent is nx x ny), which is what the strip halo at the grid's edges needs.
@@ -414,6 +422,7 @@ __global__ void __launch_bounds__(StripThreads<R, T>::value, 1) k2_2d(const P2<R
   R *fring = reinterpret_cast<R *>(smem_raw);                 // [FR][8][NT]
   R *xch = fring + FR * 8 * NT;                              // [2][XB]
   R *xsb = xch + 2 * XB;                                      // [T][NT]
+  const uint32_t xch_addr = rketd::smem_u32(xch);
   const int tid = threadIdx.x;
   JobCtx<R> c;
   c.lane = tid & 31; c.warp = tid >> 5;
@@ -502,14 +511,13 @@ __global__ void __launch_bounds__(StripThreads<R, T>::value, 1) k2_2d(const P2<R
           a.E2[idx] = ein; a.Hx2[idx] = hxin; a.Hy2[idx] = hyin; a.G2[idx] = gin;
         }
       }
-      R *xp = xch + (it & 1) * XB;                             // read in the next iteration
-      if (c.lane == 31) {
+      // warp-edge values for the next iteration: lane 31 posts {E, Hy}, lane 0 posts E, as predicated stores
+      const uint32_t xpa = xch_addr + (uint32_t)(((it & 1) * XB + (c.warp + 1) * 4) * (int)sizeof(R));
+      const bool l31 = c.lane == 31, l0 = c.lane == 0;
 #pragma unroll
-        for (int s = 0; s < T; ++s) st_pair(xp + (s * XS + c.warp + 1) * 4, n.e[s], n.hy[s]);
-      }
-      if (c.lane == 0) {
-#pragma unroll
-        for (int s = 0; s < T; ++s) xp[(s * XS + c.warp + 1) * 4 + 2] = n.e[s];
+      for (int s = 0; s < T; ++s) {
+        st_pair_if(l31, xpa + (uint32_t)(s * XS * 4 * (int)sizeof(R)), n.e[s], n.hy[s]);
+        rketd::sts_if(l0, xpa + (uint32_t)((s * XS * 4 + 2) * (int)sizeof(R)), n.e[s]);
       }
     };
 
