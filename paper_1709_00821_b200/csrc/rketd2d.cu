@@ -240,6 +240,13 @@ __device__ __forceinline__ void st_pair_if(bool pred, uint32_t a, float x, float
   asm volatile("{\n.reg .pred q;\nsetp.ne.u32 q, %0, 0;\n@q st.shared.v2.f32 [%1], {%2, %3};\n}" ::"r"((uint32_t)pred), "r"(a), "f"(x), "f"(y) : "memory");
 }
 
+__device__ __forceinline__ void lds_if_lane31(int lane, uint32_t a, double &v) {
+  asm volatile("{\n.reg .pred q;\nsetp.eq.u32 q, %1, 31;\n@q ld.shared.f64 %0, [%2];\n}" : "+d"(v) : "r"(lane), "r"(a) : "memory");
+}
+__device__ __forceinline__ void lds_if_lane31(int lane, uint32_t a, float &v) {
+  asm volatile("{\n.reg .pred q;\nsetp.eq.u32 q, %1, 31;\n@q ld.shared.f32 %0, [%2];\n}" : "+f"(v) : "r"(lane), "r"(a) : "memory");
+}
+
 // Rows of the eight input arrays arrive as 2-D tiled TMA boxes {strip columns, 1 row} (cp.async.bulk.tensor.2d, SASS UTMALDG):
 // one elected thread issues them, completion on the ring slot's mbarrier; columns and rows outside the grid are zero-filled
 // by the hardware (the tensor map's extent is nx x ny), which is what the strip halo at the grid's edges needs.
@@ -302,9 +309,8 @@ __device__ __forceinline__ void run_stages(const P2<R> &p, const Arrays<R> &a, c
       const R *xl_ = xbuf + (s * XS + c.warp) * 4;           // slot of warp - 1: {E, Hy of its lane 31}
       R e31, hy31;
       ld_pair(xl_, e31, hy31);
-      const R e0r = xl_[2 * 4 + 2];                          // slot of warp + 1: E of its lane 0
       R e_rt = shfl_down1(es);
-      e_rt = (c.lane == 31) ? e0r : e_rt;
+      lds_if_lane31(c.lane, rketd::smem_u32(xl_ + 2 * 4 + 2), e_rt);      // slot of warp + 1: E of its lane 0 (lane 31 only)
       hyn[s] = O::hy_new(c.chx_i, es, e_rt, h.hy[s]);
       const R hyn_edge = O::hy_new(c.chx_im1, e31, es, hy31);
       R hyn_l = shfl_up1(hyn[s]);
